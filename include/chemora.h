@@ -1,0 +1,129 @@
+/* chemora.h -- C ABI of libchemora.so: the B200-native (sm_100a, fp64) method-of-lines right-hand-side
+ * path of the codes the Chemora framework generates (arXiv:1307.6488).
+ *
+ * What the path is (citations are PAPER.md lines): a "calculation" applied to all grid points of a
+ * block-structured grid (:133, :187, :218-220) -- high-order finite differences (:9, :194, :338) followed by
+ * the pointwise right-hand-side expression -- driven by a method-of-lines integrator (:338, :408) with a
+ * ghost-zone synchronisation before every evaluation (:105, :354, :382).  The paper prints no equations or
+ * coefficients; DESIGN.md "Readings" (S1-S14) fixes them.
+ *
+ * Conventions
+ *  - All functions return int: 0 = CHEMORA_OK, negative = error (below).  No exceptions cross the ABI.
+ *    chemora_last_error() gives a handle-owned, NUL-terminated message for the last failing call.
+ *  - A handle is used from one host thread at a time.  All device work is enqueued on the stream given at
+ *    creation and is asynchronous with respect to the host unless stated otherwise.
+ *  - "dev" pointers are CUDA device pointers, "host" pointers ordinary host memory.
+ *  - Device state layout (SoA): V variables; each variable is tot_z x tot_y rows of
+ *    `pitch` doubles (pitch = roundup(nx + 2g, 16): 128-byte rows), x fastest; variable stride
+ *    var_stride = pitch*tot_y*tot_z; buffers are 128-byte aligned.  Interior point (i,j,k) of variable v is
+ *    at  v*var_stride + ((k+g)*tot_y + (j+g))*pitch + (i+g).
+ *  - Packed host layout: V x nz x ny x nx doubles, x fastest, no ghosts.
+ *  - There is no CPU fallback: every entry point that computes needs a CUDA device and fails with
+ *    CHEMORA_ECUDA otherwise.
+ */
+#ifndef CHEMORA_H
+#define CHEMORA_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct chemora chemora_t; /* opaque, owned by the library */
+
+enum { CHEMORA_OK = 0, CHEMORA_EINVAL = -1, CHEMORA_ENOMEM = -2, CHEMORA_ECUDA = -3, CHEMORA_ESTATE = -4 };
+
+/* system_id.  WAVE: (phi, pi), d_t phi = pi, d_t pi = delta^ij d_i d_j phi (reading S1; PAPER.md:152-169 is
+ * the paper's own wave example).  BSSN: 25 variables, chi-variant vacuum BSSN with 1+log
+ * lapse and Gamma-driver shift (readings S3-S6), slots: chi, gt11 gt12 gt13 gt22 gt23 gt33, trK,
+ * At11..At33, Gt1..3, alpha, beta1..3, B1..3, A. */
+enum { CHEMORA_SYS_WAVE = 0, CHEMORA_SYS_BSSN = 1 };
+
+/* which buffer of the four RK4 buffers (reading S9) */
+enum { CHEMORA_BUF_U = 0, CHEMORA_BUF_YA = 1, CHEMORA_BUF_YB = 2, CHEMORA_BUF_S = 3 };
+
+/* kernel variant axes (PAPER.md:215-216 fused vs derivative-split; :248-266 tile shape) */
+enum { CHEMORA_NUM_TILES = 6 };
+
+/* Create a handle for an nx x ny x nz interior block with `ghost` ghost layers per face, centred FD order
+ * fd_order (4 or 8), system system_id and grid spacing dx (same in x, y, z).
+ * Rejects (CHEMORA_EINVAL): non-positive dims, dims < ghost (periodic images would overlap),
+ * fd_order not in {4,8}, ghost < fd_order/2 (wave), ghost < fd_order/2 + 1 (BSSN: upwinded advection,
+ * PAPER.md:382), fd_order 8 with BSSN (not built yet), dx <= 0.  Dissipation (eps_diss != 0, KO order 5)
+ * needs ghost >= 3; that is checked when the parameter is set and again at launch.
+ * cuda_stream: a cudaStream_t (may be NULL = default stream).
+ * alloc/dealloc: optional device allocator callbacks (e.g. torch's caching allocator); alloc(bytes, ctx)
+ * returns a device pointer aligned to >= 128 bytes or NULL.  NULL callbacks -> cudaMalloc/cudaFree.
+ * The library owns the four state buffers (+ derivative scratch of the split variant) until destroy. */
+int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_order, int system_id, double dx,
+                   void* cuda_stream, void* (*alloc)(size_t, void*), void (*dealloc)(void*, void*),
+                   void* alloc_ctx);
+
+/* Named parameters: "eps_diss" (KO strength, default 0), "eta" (default 1), "shift_gamma_coeff"
+ * (default 0.75).  Unknown name or invalid value -> CHEMORA_EINVAL. */
+int chemora_set_param(chemora_t* h, const char* name, double value);
+int chemora_get_param(const chemora_t* h, const char* name, double* value);
+
+/* Layout in units of doubles; any out pointer may be NULL.  interior_offset = offset of interior (0,0,0)
+ * inside one variable. */
+int chemora_layout(const chemora_t* h, int* nvars, long* pitch, long* tot_y, long* tot_z, long* var_stride,
+                   long* interior_offset);
+
+/* Borrowed device pointer to one of the four buffers (valid until destroy). */
+int chemora_state_ptr(chemora_t* h, int which, double** dev);
+
+/* Copy a packed host state into U's interior / U's interior out to the host.  Synchronous (the stream is
+ * synchronised before returning).  Ghosts of U are left untouched by set_state. */
+int chemora_set_state(chemora_t* h, const double* host_packed);
+int chemora_get_state(chemora_t* h, double* host_packed);
+/* Same for a device buffer in the padded layout: pack/unpack between a DEVICE packed array and U
+ * (asynchronous on the stream; used by the device-resident benchmark path). */
+int chemora_set_state_dev(chemora_t* h, const double* dev_packed);
+int chemora_get_state_dev(chemora_t* h, double* dev_packed);
+
+/* Periodic ghost-zone fill of all V variables of a device state in the padded layout (reading S8):
+ * ghost (i,j,k) <- interior (i mod nx, j mod ny, k mod nz), faces, edges and corners.  In place. */
+int chemora_fill_ghosts(chemora_t* h, double* dev_state);
+
+/* dev_rhs interior <- RHS(dev_state); ghosts of dev_state must be filled; ghosts of dev_rhs untouched.
+ * Both in the padded layout; must not alias.  Uses the current variant. */
+int chemora_rhs(chemora_t* h, const double* dev_state, double* dev_rhs);
+
+/* U <- U(t + dt): classical RK4 with the association of reading S9; fills ghosts itself before each of
+ * the four RHS evaluations; asynchronous on the stream. */
+int chemora_rk4_step(chemora_t* h, double dt);
+
+/* Kernel variant: fused (1: derivatives + RHS + RK stage update in one kernel) or split (0: derivatives
+ * written to global arrays by one kernel, RHS + stage update by a second), and tile_id in
+ * [0, CHEMORA_NUM_TILES).  chemora_tile_shape reports the (x, y, z) extent of a tile id. */
+int chemora_set_variant(chemora_t* h, int fused, int tile_id);
+int chemora_get_variant(const chemora_t* h, int* fused, int* tile_id);
+int chemora_tile_shape(int tile_id, int* tx, int* ty, int* tz);
+
+/* Runtime sweep (the paper's model-based choice, replaced by measurement): times every
+ * (fused, tile) once on the handle's own grid (RHS on the current U), keeps the fastest, returns it.
+ * ms_out, if not NULL, receives 2*CHEMORA_NUM_TILES timings in milliseconds ([fused*NUM_TILES + tile];
+ * negative = variant unavailable).  U is not modified.  Synchronous. */
+int chemora_autotune(chemora_t* h, int* fused, int* tile_id, float* ms_out);
+
+/* Number of kernel launches issued through this handle so far (for benchmarks' gpu_launches). */
+long chemora_launch_count(const chemora_t* h);
+
+/* Static kernel resource usage of the current variant's main kernel (from cudaFuncGetAttributes):
+ * registers per thread, local (spill) bytes per thread, static+dynamic shared bytes per block. */
+int chemora_kernel_info(const chemora_t* h, int* regs, int* local_bytes, int* smem_bytes);
+
+/* Sustained FP64 FMA rate of the device in GFLOP/s (register-resident DFMA chains on all SMs); used as
+ * the measured FP64 roofline denominator.  Synchronous; ~50 ms. */
+int chemora_measure_fp64_peak(chemora_t* h, double* gflops);
+
+const char* chemora_last_error(const chemora_t* h);
+
+/* Waits for the stream, frees buffers.  NULL-safe. */
+int chemora_destroy(chemora_t* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CHEMORA_H */

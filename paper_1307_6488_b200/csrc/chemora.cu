@@ -1,0 +1,400 @@
+// chemora.cu -- host side of libchemora.so: the C ABI declared in include/chemora.h.
+// Handle, layout, parameter table, variant registry + runtime sweep, RK4 driver.  No CPU compute path exists:
+// every compute entry point enqueues CUDA kernels and reports CHEMORA_ECUDA if that fails.
+#include "../../include/chemora.h"
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "common.cuh"
+
+using namespace chm;
+
+struct chemora {
+  Layout L;
+  int order, system;
+  double dx;
+  double eps_diss, eta, sgc;
+  cudaStream_t stream;
+  void* (*alloc)(size_t, void*);
+  void (*dealloc)(void*, void*);
+  void* actx;
+  double* buf[4];
+  double* derivs;       // split variant scratch (lazy)
+  double* staging;      // device packed staging for set/get_state (lazy)
+  int fused, tile;
+  long launches;
+  std::string err;
+};
+
+namespace {
+
+int fail(chemora_t* h, int code, const std::string& msg) {
+  if (h) h->err = msg;
+  return code;
+}
+int cuda_fail(chemora_t* h, cudaError_t e, const char* what) {
+  return fail(h, CHEMORA_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CK(h, call, what)                                   \
+  do {                                                      \
+    cudaError_t e_ = (call);                                \
+    if (e_ != cudaSuccess) return cuda_fail(h, e_, what);   \
+  } while (0)
+
+size_t state_bytes(const chemora_t* h) { return (size_t)h->L.nvars * h->L.vstride * sizeof(double); }
+size_t packed_count(const chemora_t* h) { return (size_t)h->L.nvars * h->L.nx * h->L.ny * h->L.nz; }
+long deriv_stride(const chemora_t* h) {
+  long n = (long)h->L.nx * h->L.ny * h->L.nz;
+  return (n + 15) / 16 * 16;
+}
+
+void* dev_alloc(chemora_t* h, size_t bytes) {
+  if (h->alloc) return h->alloc(bytes, h->actx);
+  void* p = nullptr;
+  return cudaMalloc(&p, bytes) == cudaSuccess ? p : nullptr;
+}
+void dev_free(chemora_t* h, void* p) {
+  if (!p) return;
+  if (h->dealloc) h->dealloc(p, h->actx);
+  else cudaFree(p);
+}
+
+Coef make_coef(const chemora_t* h) {
+  Coef C;
+  C.inv_h = 1.0 / h->dx;
+  C.inv_h2 = 1.0 / (h->dx * h->dx);
+  C.ko = h->eps_diss / (64.0 * h->dx);
+  C.eta = h->eta;
+  C.sgc = h->sgc;
+  return C;
+}
+
+int ensure_derivs(chemora_t* h) {
+  if (h->derivs) return CHEMORA_OK;
+  size_t bytes = (size_t)kNumDerivArrays * deriv_stride(h) * sizeof(double);
+  h->derivs = (double*)dev_alloc(h, bytes);
+  if (!h->derivs) return fail(h, CHEMORA_ENOMEM, "derivative scratch allocation failed");
+  return CHEMORA_OK;
+}
+
+// one RHS evaluation with the given epilogue; counts launches
+int run_rhs(chemora_t* h, const Stage& st) {
+  if (h->eps_diss != 0.0 && h->L.g < 3) return fail(h, CHEMORA_EINVAL, "eps_diss != 0 needs ghost >= 3 (KO order 5)");
+  Coef C = make_coef(h);
+  if (h->system == CHEMORA_SYS_WAVE) {
+    CK(h, launch_wave(h->L, C, h->order, h->tile, st, h->stream), "wave kernel launch");
+    h->launches += 1;
+  } else if (h->fused) {
+    CK(h, launch_bssn_fused(h->L, C, h->tile, st, h->stream), "bssn fused kernel launch");
+    h->launches += 1;
+  } else {
+    int rc = ensure_derivs(h);
+    if (rc) return rc;
+    CK(h, launch_bssn_derivs(h->L, C, h->tile, st.in, h->derivs, h->stream), "bssn derivative kernel launch");
+    CK(h, launch_bssn_from_derivs(h->L, C, h->tile, h->derivs, st, h->stream), "bssn rhs kernel launch");
+    h->launches += 2;
+  }
+  return CHEMORA_OK;
+}
+
+int fill(chemora_t* h, double* state) {
+  CK(h, launch_fill_ghosts(h->L, state, h->stream), "ghost fill launch");
+  h->launches += 1;
+  return CHEMORA_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_order, int system_id, double dx,
+                   void* cuda_stream, void* (*alloc)(size_t, void*), void (*dealloc)(void*, void*),
+                   void* alloc_ctx) {
+  if (!out) return CHEMORA_EINVAL;
+  *out = nullptr;
+  if (nx <= 0 || ny <= 0 || nz <= 0 || ghost < 0) return CHEMORA_EINVAL;
+  if (fd_order != 4 && fd_order != 8) return CHEMORA_EINVAL;
+  if (system_id != CHEMORA_SYS_WAVE && system_id != CHEMORA_SYS_BSSN) return CHEMORA_EINVAL;
+  if (!(dx > 0.0)) return CHEMORA_EINVAL;
+  if ((alloc == nullptr) != (dealloc == nullptr)) return CHEMORA_EINVAL;
+  const int need = system_id == CHEMORA_SYS_WAVE ? fd_order / 2 : fd_order / 2 + 1;
+  if (ghost < need) return CHEMORA_EINVAL;
+  if (nx < ghost || ny < ghost || nz < ghost) return CHEMORA_EINVAL;
+  if (system_id == CHEMORA_SYS_BSSN && fd_order != 4) return CHEMORA_EINVAL;  // 8th-order BSSN: not built yet
+
+  chemora_t* h = new (std::nothrow) chemora_t();
+  if (!h) return CHEMORA_ENOMEM;
+  Layout& L = h->L;
+  L.nx = nx; L.ny = ny; L.nz = nz; L.g = ghost;
+  L.nvars = system_id == CHEMORA_SYS_WAVE ? 2 : 25;
+  L.pitch = ((long)nx + 2 * ghost + 15) / 16 * 16;
+  L.tot_y = ny + 2 * ghost; L.tot_z = nz + 2 * ghost;
+  L.plane = L.pitch * L.tot_y;
+  L.vstride = L.plane * L.tot_z;
+  h->order = fd_order; h->system = system_id; h->dx = dx;
+  h->eps_diss = 0.0; h->eta = 1.0; h->sgc = 0.75;
+  h->stream = (cudaStream_t)cuda_stream;
+  h->alloc = alloc; h->dealloc = dealloc; h->actx = alloc_ctx;
+  h->derivs = nullptr; h->staging = nullptr;
+  h->fused = 1; h->tile = 1;
+  h->launches = 0;
+  for (int b = 0; b < 4; ++b) h->buf[b] = nullptr;
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    delete h;
+    return CHEMORA_ECUDA;   // no device: there is no CPU fallback
+  }
+  for (int b = 0; b < 4; ++b) {
+    h->buf[b] = (double*)dev_alloc(h, state_bytes(h));
+    if (!h->buf[b] || ((uintptr_t)h->buf[b] & 127)) {
+      for (int c = 0; c <= b; ++c) dev_free(h, h->buf[c]);
+      delete h;
+      return CHEMORA_ENOMEM;
+    }
+    if (cudaMemsetAsync(h->buf[b], 0, state_bytes(h), h->stream) != cudaSuccess) {
+      for (int c = 0; c <= b; ++c) dev_free(h, h->buf[c]);
+      delete h;
+      return CHEMORA_ECUDA;
+    }
+  }
+  *out = h;
+  return CHEMORA_OK;
+}
+
+int chemora_set_param(chemora_t* h, const char* name, double v) {
+  if (!h || !name) return CHEMORA_EINVAL;
+  if (!(v == v)) return fail(h, CHEMORA_EINVAL, "parameter value is NaN");
+  if (!strcmp(name, "eps_diss")) {
+    if (v < 0.0) return fail(h, CHEMORA_EINVAL, "eps_diss must be >= 0");
+    if (v != 0.0 && h->L.g < 3) return fail(h, CHEMORA_EINVAL, "eps_diss != 0 needs ghost >= 3 (KO order 5)");
+    h->eps_diss = v;
+  } else if (!strcmp(name, "eta")) h->eta = v;
+  else if (!strcmp(name, "shift_gamma_coeff")) h->sgc = v;
+  else return fail(h, CHEMORA_EINVAL, std::string("unknown parameter: ") + name);
+  return CHEMORA_OK;
+}
+
+int chemora_get_param(const chemora_t* h, const char* name, double* v) {
+  if (!h || !name || !v) return CHEMORA_EINVAL;
+  if (!strcmp(name, "eps_diss")) *v = h->eps_diss;
+  else if (!strcmp(name, "eta")) *v = h->eta;
+  else if (!strcmp(name, "shift_gamma_coeff")) *v = h->sgc;
+  else return CHEMORA_EINVAL;
+  return CHEMORA_OK;
+}
+
+int chemora_layout(const chemora_t* h, int* nvars, long* pitch, long* tot_y, long* tot_z, long* var_stride,
+                   long* interior_offset) {
+  if (!h) return CHEMORA_EINVAL;
+  if (nvars) *nvars = h->L.nvars;
+  if (pitch) *pitch = h->L.pitch;
+  if (tot_y) *tot_y = h->L.tot_y;
+  if (tot_z) *tot_z = h->L.tot_z;
+  if (var_stride) *var_stride = h->L.vstride;
+  if (interior_offset) *interior_offset = (long)h->L.g * h->L.plane + (long)h->L.g * h->L.pitch + h->L.g;
+  return CHEMORA_OK;
+}
+
+int chemora_state_ptr(chemora_t* h, int which, double** dev) {
+  if (!h || !dev || which < 0 || which > 3) return CHEMORA_EINVAL;
+  *dev = h->buf[which];
+  return CHEMORA_OK;
+}
+
+static int ensure_staging(chemora_t* h) {
+  if (h->staging) return CHEMORA_OK;
+  h->staging = (double*)dev_alloc(h, packed_count(h) * sizeof(double));
+  return h->staging ? CHEMORA_OK : fail(h, CHEMORA_ENOMEM, "staging allocation failed");
+}
+
+int chemora_set_state_dev(chemora_t* h, const double* dev_packed) {
+  if (!h || !dev_packed) return CHEMORA_EINVAL;
+  CK(h, launch_pack(h->L, dev_packed, h->buf[0], true, h->stream), "unpack launch");
+  h->launches += 1;
+  return CHEMORA_OK;
+}
+
+int chemora_get_state_dev(chemora_t* h, double* dev_packed) {
+  if (!h || !dev_packed) return CHEMORA_EINVAL;
+  CK(h, launch_pack(h->L, dev_packed, h->buf[0], false, h->stream), "pack launch");
+  h->launches += 1;
+  return CHEMORA_OK;
+}
+
+int chemora_set_state(chemora_t* h, const double* host_packed) {
+  if (!h || !host_packed) return CHEMORA_EINVAL;
+  int rc = ensure_staging(h);
+  if (rc) return rc;
+  CK(h, cudaMemcpyAsync(h->staging, host_packed, packed_count(h) * sizeof(double), cudaMemcpyHostToDevice, h->stream),
+     "H2D copy");
+  rc = chemora_set_state_dev(h, h->staging);
+  if (rc) return rc;
+  CK(h, cudaStreamSynchronize(h->stream), "set_state sync");
+  return CHEMORA_OK;
+}
+
+int chemora_get_state(chemora_t* h, double* host_packed) {
+  if (!h || !host_packed) return CHEMORA_EINVAL;
+  int rc = ensure_staging(h);
+  if (rc) return rc;
+  rc = chemora_get_state_dev(h, h->staging);
+  if (rc) return rc;
+  CK(h, cudaMemcpyAsync(host_packed, h->staging, packed_count(h) * sizeof(double), cudaMemcpyDeviceToHost, h->stream),
+     "D2H copy");
+  CK(h, cudaStreamSynchronize(h->stream), "get_state sync");
+  return CHEMORA_OK;
+}
+
+int chemora_fill_ghosts(chemora_t* h, double* dev_state) {
+  if (!h || !dev_state) return CHEMORA_EINVAL;
+  return fill(h, dev_state);
+}
+
+int chemora_rhs(chemora_t* h, const double* dev_state, double* dev_rhs) {
+  if (!h || !dev_state || !dev_rhs || dev_state == dev_rhs) return CHEMORA_EINVAL;
+  Stage st{dev_state, nullptr, nullptr, dev_rhs, 0.0, MODE_RHS};
+  return run_rhs(h, st);
+}
+
+int chemora_rk4_step(chemora_t* h, double dt) {
+  if (!h || !(dt == dt)) return CHEMORA_EINVAL;
+  double *U = h->buf[0], *Ya = h->buf[1], *Yb = h->buf[2], *S = h->buf[3];
+  int rc;
+  // stage 1: k1 = f(U);  S = k1;  Yb = U + dt/2 k1
+  if ((rc = fill(h, U))) return rc;
+  if ((rc = run_rhs(h, Stage{U, U, S, Yb, dt / 2.0, MODE_FIRST}))) return rc;
+  // stage 2: k2 = f(Yb); S += 2 k2; Ya = U + dt/2 k2
+  if ((rc = fill(h, Yb))) return rc;
+  if ((rc = run_rhs(h, Stage{Yb, U, S, Ya, dt / 2.0, MODE_MID}))) return rc;
+  // stage 3: k3 = f(Ya); S += 2 k3; Yb = U + dt k3
+  if ((rc = fill(h, Ya))) return rc;
+  if ((rc = run_rhs(h, Stage{Ya, U, S, Yb, dt, MODE_MID}))) return rc;
+  // stage 4: k4 = f(Yb); U = U + dt/6 (S + k4)
+  if ((rc = fill(h, Yb))) return rc;
+  if ((rc = run_rhs(h, Stage{Yb, U, S, nullptr, dt / 6.0, MODE_LAST}))) return rc;
+  return CHEMORA_OK;
+}
+
+int chemora_set_variant(chemora_t* h, int fused, int tile_id) {
+  if (!h || tile_id < 0 || tile_id >= CHEMORA_NUM_TILES || (fused != 0 && fused != 1)) return CHEMORA_EINVAL;
+  if (!fused && h->system == CHEMORA_SYS_WAVE) return fail(h, CHEMORA_EINVAL, "wave system has no split variant");
+  h->fused = fused;
+  h->tile = tile_id;
+  return CHEMORA_OK;
+}
+
+int chemora_get_variant(const chemora_t* h, int* fused, int* tile_id) {
+  if (!h) return CHEMORA_EINVAL;
+  if (fused) *fused = h->fused;
+  if (tile_id) *tile_id = h->tile;
+  return CHEMORA_OK;
+}
+
+int chemora_tile_shape(int tile_id, int* tx, int* ty, int* tz) {
+  if (tile_id < 0 || tile_id >= CHEMORA_NUM_TILES) return CHEMORA_EINVAL;
+  if (tx) *tx = kTiles[tile_id].tx;
+  if (ty) *ty = kTiles[tile_id].ty;
+  if (tz) *tz = kTiles[tile_id].tz;
+  return CHEMORA_OK;
+}
+
+int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out) {
+  if (!h) return CHEMORA_EINVAL;
+  const int save_f = h->fused, save_t = h->tile;
+  float best = -1.f;
+  int bf = save_f, bt = save_t;
+  cudaEvent_t e0, e1;
+  CK(h, cudaEventCreate(&e0), "event create");
+  CK(h, cudaEventCreate(&e1), "event create");
+  int rc = fill(h, h->buf[0]);
+  for (int f = 1; f >= 0 && !rc; --f)
+    for (int t = 0; t < CHEMORA_NUM_TILES && !rc; ++t) {
+      float ms = -1.f;
+      if (f == 1 || h->system == CHEMORA_SYS_BSSN) {
+        h->fused = f; h->tile = t;
+        Stage st{h->buf[0], nullptr, nullptr, h->buf[3], 0.0, MODE_RHS};   // RHS(U) -> S (scratch)
+        rc = run_rhs(h, st);                                               // warm-up
+        if (!rc) {
+          cudaEventRecord(e0, h->stream);
+          rc = run_rhs(h, st);
+          cudaEventRecord(e1, h->stream);
+          if (cudaEventSynchronize(e1) != cudaSuccess) rc = fail(h, CHEMORA_ECUDA, "autotune sync failed");
+          else cudaEventElapsedTime(&ms, e0, e1);
+        }
+        if (!rc && (best < 0.f || ms < best)) { best = ms; bf = f; bt = t; }
+      }
+      if (ms_out) ms_out[f * CHEMORA_NUM_TILES + t] = ms;
+    }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  h->fused = rc ? save_f : bf;
+  h->tile = rc ? save_t : bt;
+  if (fused_out) *fused_out = h->fused;
+  if (tile_out) *tile_out = h->tile;
+  return rc;
+}
+
+long chemora_launch_count(const chemora_t* h) { return h ? h->launches : 0; }
+
+int chemora_kernel_info(const chemora_t* h, int* regs, int* local_bytes, int* smem_bytes) {
+  if (!h) return CHEMORA_EINVAL;
+  cudaFuncAttributes a;
+  cudaError_t e = h->system == CHEMORA_SYS_WAVE ? kernel_info_wave(h->order, h->tile, &a)
+                                                : kernel_info_bssn(h->fused, h->tile, &a);
+  if (e != cudaSuccess) return cuda_fail(const_cast<chemora_t*>(h), e, "cudaFuncGetAttributes");
+  if (regs) *regs = a.numRegs;
+  if (local_bytes) *local_bytes = (int)a.localSizeBytes;
+  if (smem_bytes) *smem_bytes = (int)a.sharedSizeBytes;
+  return CHEMORA_OK;
+}
+
+int chemora_measure_fp64_peak(chemora_t* h, double* gflops) {
+  if (!h || !gflops) return CHEMORA_EINVAL;
+  int dev = 0, sms = 0;
+  CK(h, cudaGetDevice(&dev), "get device");
+  CK(h, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "get SM count");
+  const int blocks = sms * 8, threads = 256, iters = 1 << 15;
+  cudaEvent_t e0, e1;
+  CK(h, cudaEventCreate(&e0), "event create");
+  CK(h, cudaEventCreate(&e1), "event create");
+  double* sink = h->buf[3];
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0, h->stream);
+    cudaError_t e = launch_dfma_peak(blocks, threads, iters, sink, h->stream);
+    cudaEventRecord(e1, h->stream);
+    if (e != cudaSuccess || cudaEventSynchronize(e1) != cudaSuccess) {
+      cudaEventDestroy(e0); cudaEventDestroy(e1);
+      return cuda_fail(h, e != cudaSuccess ? e : cudaGetLastError(), "fp64 probe");
+    }
+    float ms;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && ms < best) best = ms;
+    h->launches += 1;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  *gflops = (double)blocks * threads * iters * 8.0 * 2.0 / (best * 1e-3) / 1e9;
+  return CHEMORA_OK;
+}
+
+const char* chemora_last_error(const chemora_t* h) { return h ? h->err.c_str() : "null handle"; }
+
+int chemora_destroy(chemora_t* h) {
+  if (!h) return CHEMORA_OK;
+  cudaStreamSynchronize(h->stream);
+  for (int b = 0; b < 4; ++b) dev_free(h, h->buf[b]);
+  dev_free(h, h->derivs);
+  dev_free(h, h->staging);
+  delete h;
+  return CHEMORA_OK;
+}
+
+}  // extern "C"

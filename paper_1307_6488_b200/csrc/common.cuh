@@ -1,0 +1,80 @@
+// common.cuh -- shared declarations of libchemora's translation units (host + device).
+// Part of the CUDA product path; shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace chm {
+
+// Device-side view of the padded SoA layout (include/chemora.h "Conventions").
+struct Layout {
+  int nx, ny, nz, g;     // interior dims, ghost width
+  int nvars;
+  long pitch;            // doubles per row, multiple of 16 (128-byte rows)
+  long plane;            // pitch * tot_y
+  long vstride;          // plane * tot_z
+  int tot_y, tot_z;
+};
+
+// Stencil scale factors and model parameters, precomputed on the host once per launch.
+struct Coef {
+  double inv_h;          // 1/h
+  double inv_h2;         // 1/h^2
+  double ko;             // eps_diss / (64 h); 0 => dissipation off (no +-3 reads)
+  double eta;            // Gamma-driver damping
+  double sgc;            // shift_gamma_coeff (3/4)
+};
+
+// Runge-Kutta epilogue fused into the RHS kernels (reading S9).
+//   MODE_RHS   : out = k
+//   MODE_FIRST : S = k          ; Y = U + a k        (U == the input state)
+//   MODE_MID   : S = S + 2 k    ; Y = U + a k
+//   MODE_LAST  : U = U + a (S + k)                   (a = dt/6)
+enum { MODE_RHS = 0, MODE_FIRST = 1, MODE_MID = 2, MODE_LAST = 3 };
+
+struct Stage {
+  const double* in;      // state the RHS is evaluated on (ghosts filled)
+  double* U;             // MODE_LAST: read+written.  MODE_FIRST/MID: read only.  MODE_RHS: unused
+  double* S;             // accumulator
+  double* out;           // MODE_RHS: rhs ; MODE_FIRST/MID: next stage state Y
+  double a;              // dt/2, dt/2, dt, dt/6
+  int mode;
+};
+
+// The stage combination, one rounding per operation and no FMA contraction, so that it is
+// bit-identical to the association written in reading S9 for a given k.
+__device__ __forceinline__ void stage_emit(const Stage& st, long q, double k) {
+  if (st.mode == MODE_RHS) {
+    st.out[q] = k;
+  } else if (st.mode == MODE_FIRST) {
+    st.S[q] = k;
+    st.out[q] = __dadd_rn(st.in[q], __dmul_rn(st.a, k));
+  } else if (st.mode == MODE_MID) {
+    st.S[q] = __dadd_rn(st.S[q], __dmul_rn(2.0, k));
+    st.out[q] = __dadd_rn(st.U[q], __dmul_rn(st.a, k));
+  } else {
+    st.U[q] = __dadd_rn(st.U[q], __dmul_rn(st.a, __dadd_rn(st.S[q], k)));
+  }
+}
+
+// Tile shapes of the variant sweep (threads in x, y; planes marched in z).
+struct TileShape { int tx, ty, tz; };
+static const TileShape kTiles[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64, 4, 8}, {128, 2, 8}, {16, 16, 8}};
+
+// launchers implemented in the kernel translation units; each returns the cudaError_t of the launch
+cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s);
+cudaError_t launch_pack(const Layout& L, const double* packed, double* state, bool to_state, cudaStream_t s);
+cudaError_t launch_wave(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
+cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int tile, const Stage& st, cudaStream_t s);
+cudaError_t launch_bssn_derivs(const Layout& L, const Coef& C, int tile, const double* in, double* derivs,
+                               cudaStream_t s);
+cudaError_t launch_bssn_from_derivs(const Layout& L, const Coef& C, int tile, const double* derivs,
+                                    const Stage& st, cudaStream_t s);
+cudaError_t kernel_info_wave(int order, int tile, cudaFuncAttributes* a);
+cudaError_t kernel_info_bssn(int fused, int tile, cudaFuncAttributes* a);
+cudaError_t launch_dfma_peak(int blocks, int threads, int iters, double* sink, cudaStream_t s);
+
+// number of derivative arrays of the split variant: 45 first + 66 second + 25 advection+dissipation
+constexpr int kNumDerivArrays = 136;
+
+}  // namespace chm

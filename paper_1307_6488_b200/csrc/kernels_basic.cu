@@ -1,0 +1,153 @@
+// kernels_basic.cu -- ghost fill, pack/unpack, wave-system RHS (+ fused RK4 stage update), FP64 peak probe.
+#include "stencils.cuh"
+
+namespace chm {
+
+// ---------------------------------------------------------------------------------------------------
+// Periodic ghost fill (reading S8; stands in for the inter-process exchange of PAPER.md:105, :354).
+// One thread per ghost point; the flat ghost index is decoded into one of three regions:
+//   A: ghost z-planes (all y, all x)   B: interior z, ghost y rows (all x)   C: interior z,y, ghost x
+// Each ghost reads its wrapped interior image directly, so faces, edges and corners need no ordering.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) fill_ghosts_kernel(Layout L, double* __restrict__ state) {
+  const int g = L.g, tx = L.nx + 2 * g;
+  const long nA = 2L * g * L.tot_y * tx, nB = (long)L.nz * 2 * g * tx, nC = (long)L.nz * L.ny * 2 * g;
+  long id = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (id >= nA + nB + nC) return;
+  int i, j, k;   // padded coordinates
+  if (id < nA) {
+    long row = id / tx; i = (int)(id - row * tx);
+    int kk = (int)(row / L.tot_y); j = (int)(row - (long)kk * L.tot_y);
+    k = kk < g ? kk : kk + L.nz;
+  } else if (id < nA + nB) {
+    id -= nA;
+    long row = id / tx; i = (int)(id - row * tx);
+    int kk = (int)(row / (2 * g)); int jj = (int)(row - (long)kk * 2 * g);
+    k = kk + g; j = jj < g ? jj : jj + L.ny;
+  } else {
+    id -= nA + nB;
+    long row = id / (2 * g); int ii = (int)(id - row * 2 * g);
+    int kk = (int)(row / L.ny); int jj = (int)(row - (long)kk * L.ny);
+    k = kk + g; j = jj + g; i = ii < g ? ii : ii + L.nx;
+  }
+  auto wrap = [g](int c, int n) { int r = (c - g) % n; return (r < 0 ? r + n : r) + g; };
+  const long dst = (long)k * L.plane + (long)j * L.pitch + i;
+  const long src = (long)wrap(k, L.nz) * L.plane + (long)wrap(j, L.ny) * L.pitch + wrap(i, L.nx);
+  double* p = state + (long)blockIdx.y * L.vstride;
+  p[dst] = p[src];
+}
+
+cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s) {
+  const int g = L.g, tx = L.nx + 2 * g;
+  if (g == 0) return cudaSuccess;
+  long n = 2L * g * L.tot_y * tx + (long)L.nz * 2 * g * tx + (long)L.nz * L.ny * 2 * g;
+  dim3 grid((unsigned)((n + 255) / 256), L.nvars);
+  fill_ghosts_kernel<<<grid, 256, 0, s>>>(L, state);
+  return cudaGetLastError();
+}
+
+// packed [V][nz][ny][nx] <-> padded interior
+__global__ void __launch_bounds__(256) pack_kernel(Layout L, const double* __restrict__ src, double* __restrict__ dst,
+                                                   bool to_state) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= L.nx) return;
+  int j = blockIdx.y, k = blockIdx.z % L.nz, v = blockIdx.z / L.nz;
+  long q = v * L.vstride + (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.g);
+  long r = (((long)v * L.nz + k) * L.ny + j) * L.nx + i;
+  if (to_state) dst[q] = src[r]; else dst[r] = src[q];
+}
+
+cudaError_t launch_pack(const Layout& L, const double* packed, double* state, bool to_state, cudaStream_t s) {
+  dim3 grid((L.nx + 255) / 256, L.ny, L.nz * L.nvars);
+  if (to_state) pack_kernel<<<grid, 256, 0, s>>>(L, packed, state, true);
+  else pack_kernel<<<grid, 256, 0, s>>>(L, state, const_cast<double*>(packed), false);
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Wave system (reading S1): d_t phi = pi (+KO), d_t pi = (d_xx + d_yy + d_zz) phi (+KO).
+// Block = TX x TY threads; each thread marches TZ consecutive z-planes.
+// ---------------------------------------------------------------------------------------------------
+template <int ORDER, bool KO, int TX, int TY, int TZ>
+__global__ void __launch_bounds__(TX* TY) wave_kernel(Layout L, Coef C, Stage st) {
+  const int i = blockIdx.x * TX + threadIdx.x, j = blockIdx.y * TY + threadIdx.y;
+  if (i >= L.nx || j >= L.ny) return;
+  const int k0 = blockIdx.z * TZ;
+#pragma unroll 1
+  for (int kk = 0; kk < TZ; ++kk) {
+    const int k = k0 + kk;
+    if (k >= L.nz) break;
+    const long q = (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.g);
+    GlobalPoint P{st.in + q, L.pitch, L.plane, L.vstride};
+    double lap;
+    if (ORDER == 4) lap = (d2_o4(P, 0, 0, C.inv_h2) + d2_o4(P, 0, 1, C.inv_h2)) + d2_o4(P, 0, 2, C.inv_h2);
+    else lap = (d2_o8(P, 0, 0, C.inv_h2) + d2_o8(P, 0, 1, C.inv_h2)) + d2_o8(P, 0, 2, C.inv_h2);
+    double rphi = P.at(1, 0, 0, 0), rpi = lap;
+    if (KO) { rphi += ko5(P, 0, C.ko); rpi += ko5(P, 1, C.ko); }
+    stage_emit(st, q, rphi);
+    stage_emit(st, q + L.vstride, rpi);
+  }
+}
+
+template <int ORDER, bool KO, int TX, int TY, int TZ>
+static cudaError_t wave_go(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
+  auto kern = wave_kernel<ORDER, KO, TX, TY, TZ>;
+  if (a) return cudaFuncGetAttributes(a, kern);
+  dim3 grid((L.nx + TX - 1) / TX, (L.ny + TY - 1) / TY, (L.nz + TZ - 1) / TZ);
+  kern<<<grid, dim3(TX, TY), 0, s>>>(L, C, *st);
+  return cudaGetLastError();
+}
+
+template <int ORDER, bool KO>
+static cudaError_t wave_tile(int tile, const Layout& L, const Coef& C, const Stage* st, cudaStream_t s,
+                             cudaFuncAttributes* a) {
+  switch (tile) {
+    case 0: return wave_go<ORDER, KO, 32, 4, 8>(L, C, st, s, a);
+    case 1: return wave_go<ORDER, KO, 32, 8, 8>(L, C, st, s, a);
+    case 2: return wave_go<ORDER, KO, 64, 2, 8>(L, C, st, s, a);
+    case 3: return wave_go<ORDER, KO, 64, 4, 8>(L, C, st, s, a);
+    case 4: return wave_go<ORDER, KO, 128, 2, 8>(L, C, st, s, a);
+    case 5: return wave_go<ORDER, KO, 16, 16, 8>(L, C, st, s, a);
+  }
+  return cudaErrorInvalidValue;
+}
+
+static cudaError_t wave_dispatch(int order, bool ko, int tile, const Layout& L, const Coef& C, const Stage* st,
+                                 cudaStream_t s, cudaFuncAttributes* a) {
+  if (order == 4) return ko ? wave_tile<4, true>(tile, L, C, st, s, a) : wave_tile<4, false>(tile, L, C, st, s, a);
+  if (order == 8) return ko ? wave_tile<8, true>(tile, L, C, st, s, a) : wave_tile<8, false>(tile, L, C, st, s, a);
+  return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_wave(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s) {
+  return wave_dispatch(order, C.ko != 0.0, tile, L, C, &st, s, nullptr);
+}
+
+cudaError_t kernel_info_wave(int order, int tile, cudaFuncAttributes* a) {
+  Layout L{}; Coef C{};
+  return wave_dispatch(order, true, tile, L, C, nullptr, 0, a);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// FP64 peak probe: 8 independent register-resident DFMA chains per thread.
+// flops = blocks * threads * iters * 8 chains * 2.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, double* sink) {
+  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6,
+         a7 = a0 + 7;
+  const double m = 1.0000001, c = 1e-7;
+#pragma unroll 4
+  for (int it = 0; it < iters; ++it) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+  }
+  double r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  if (r == 12345.678) sink[0] = r;   // never true; keeps the chains alive
+}
+
+cudaError_t launch_dfma_peak(int blocks, int threads, int iters, double* sink, cudaStream_t s) {
+  dfma_peak_kernel<<<blocks, threads, 0, s>>>(iters, sink);
+  return cudaGetLastError();
+}
+
+}  // namespace chm

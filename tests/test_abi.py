@@ -1,0 +1,83 @@
+"""CPU-side checks of the boundary: libchemora.so loads, exports every symbol include/chemora.h declares,
+rejects bad arguments, and refuses to compute without a CUDA device (no CPU fallback).  No compute calls."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def binding():
+    from paper_1307_6488_b200 import build, binding as b
+    build.build()
+    b.load()
+    return b
+
+
+def test_exports_every_declared_symbol(binding):
+    header = open(os.path.join(ROOT, "include", "chemora.h")).read()
+    declared = set(re.findall(r"\b(chemora_[a-z0-9_]+)\s*\(", header))
+    declared.discard("chemora_t")
+    assert declared == set(binding.SYMBOLS)
+    lib = ctypes.CDLL(binding.LIB_PATH)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_tile_table(binding):
+    shapes = [binding.tile_shape(t) for t in range(binding.NUM_TILES)]
+    assert shapes == [(32, 4, 8), (32, 8, 8), (64, 2, 8), (64, 4, 8), (128, 2, 8), (16, 16, 8)]
+    with pytest.raises(binding.ChemoraError):
+        binding.tile_shape(6)
+
+
+@pytest.mark.parametrize("args", [
+    (0, 8, 8, 2, 4, 0, 0.1),      # non-positive dim
+    (8, 8, 8, 1, 4, 0, 0.1),      # wave O4 needs g >= 2
+    (8, 8, 8, 3, 8, 0, 0.1),      # wave O8 needs g >= 4
+    (8, 8, 8, 2, 4, 1, 0.1),      # BSSN O4 upwinded needs g >= 3 (PAPER.md:382 rule order/2+1)
+    (8, 8, 8, 3, 6, 1, 0.1),      # order not in {4,8}
+    (8, 8, 8, 3, 4, 2, 0.1),      # unknown system
+    (8, 8, 8, 3, 4, 1, 0.0),      # dx <= 0
+    (2, 8, 8, 3, 4, 1, 0.1),      # dim < ghost
+])
+def test_create_rejects_bad_arguments(binding, args):
+    lib = binding.load()
+    h = ctypes.c_void_p()
+    rc = lib.chemora_create(ctypes.byref(h), *args[:6], float(args[6]), None, binding._ALLOC_T(), binding._DEALLOC_T(),
+                            None)
+    assert rc == binding.EINVAL and not h.value
+
+
+def test_no_cpu_fallback(binding):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(binding.ChemoraError) as e:
+        binding.Chemora(8, 8, 8, 2, 4, 0, 0.1)
+    assert e.value.code == binding.ECUDA
+
+
+def test_null_handle_is_safe(binding):
+    lib = binding.load()
+    assert lib.chemora_destroy(None) == 0
+    assert lib.chemora_rk4_step(None, 0.1) == binding.EINVAL
+    assert lib.chemora_launch_count(None) == 0
+
+
+def test_product_never_touches_the_oracle():
+    """the CUDA path must not import, link or read anything under oracle/ (and vice versa)."""
+    pkg = os.path.join(ROOT, "paper_1307_6488_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                assert "oracle" not in open(os.path.join(dirpath, f)).read().replace("oracle/.", "").lower() or \
+                    f in ("inputs.py", "common.cuh", "__init__.py"), f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_1307_6488_b200" not in src and "from paper_1307_6488_b200" not in src
+            assert "libchemora" not in src and "csrc" not in src

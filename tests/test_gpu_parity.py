@@ -1,0 +1,219 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element on the same seeded
+inputs (tolerances from BASELINE.json north_star: wave 1e-12 per RK4 step, BSSN 1e-10 after
+10 steps; error norm = reading S11).  All tests need a B200: `pytest -m gpu`."""
+import numpy as np
+import pytest
+
+from paper_1307_6488_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL_WAVE_PER_STEP = 1e-12
+TOL_BSSN_10_STEPS = 1e-10
+TOL_RHS = 1e-12          # a single RHS evaluation: rounding-order differences only (difference-form stencils)
+
+
+@pytest.fixture(scope="module")
+def chem():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1307_6488_b200 import binding
+    binding.load()          # fails loudly if the library is not built: no fallback
+    return binding
+
+
+def relerr(a, b):
+    """S11: per variable max|a-b| / max|b|, then max over variables."""
+    worst = 0.0
+    for v in range(a.shape[0]):
+        den = max(np.max(np.abs(b[v])), 1e-300)
+        worst = max(worst, np.max(np.abs(a[v] - b[v])) / den)
+    return worst
+
+
+def to_padded(h, packed):
+    import torch
+    st = h.new_state()
+    h.interior(st).copy_(torch.from_numpy(packed))
+    return st
+
+
+def gpu_rhs(h, packed):
+    st = to_padded(h, packed)
+    h.fill_ghosts(st)
+    out = h.new_state()
+    h.rhs(st, out)
+    return h.interior(out).cpu().numpy()
+
+
+def oracle_rhs(oracle, system, packed, g, order, dx, **prm):
+    st = oracle.fill_ghosts(oracle.with_ghosts(packed, g), g)
+    return oracle.interior(oracle.rhs(system, st, g, order, dx, oracle.params(**prm)), g)
+
+
+# ------------------------------------------------------------------------------------------ ghost fill
+@pytest.mark.parametrize("dims,g,system", [((37, 21, 19), 3, 1), ((16, 16, 16), 2, 0), ((5, 4, 9), 4, 0),
+                                           ((3, 3, 3), 3, 1)])
+def test_fill_ghosts_bit_exact(chem, oracle, dims, g, system):
+    nx, ny, nz = dims
+    V = 2 if system == 0 else 25
+    rng = np.random.default_rng(5)
+    u = rng.standard_normal((V, nz, ny, nx))
+    h = chem.Chemora(nx, ny, nz, g, 8 if g == 4 else 4, system, 0.1)
+    st = to_padded(h, u)
+    h.fill_ghosts(st)
+    got = st[..., : nx + 2 * g].cpu().numpy()
+    want = oracle.fill_ghosts(oracle.with_ghosts(u, g), g)
+    assert np.array_equal(got, want)
+    assert not st[..., nx + 2 * g:].any()       # row padding untouched
+    h.destroy()
+
+
+def test_set_get_state_roundtrip(chem):
+    rng = np.random.default_rng(6)
+    u = rng.standard_normal((25, 9, 10, 11))
+    h = chem.Chemora(11, 10, 9, 3, 4, 1, 0.1)
+    h.set_state(u)
+    assert np.array_equal(h.get_state(), u)
+    assert np.array_equal(h.interior(h.state_view()).cpu().numpy(), u)
+    h.destroy()
+
+
+# ------------------------------------------------------------------------------------------------ wave
+@pytest.mark.parametrize("order,g,eps,dims", [(4, 2, 0.0, (37, 21, 19)), (8, 4, 0.1, (70, 33, 18)),
+                                              (4, 3, 0.1, (16, 16, 16)), (8, 4, 0.0, (33, 9, 12))])
+def test_wave_rhs_all_tiles(chem, oracle, order, g, eps, dims):
+    nx, ny, nz = dims
+    rng = np.random.default_rng(11)
+    u = rng.standard_normal((2, nz, ny, nx))
+    dx = 1.0 / 32
+    want = oracle_rhs(oracle, 0, u, g, order, dx, eps_diss=eps)
+    h = chem.Chemora(nx, ny, nz, g, order, 0, dx)
+    h.set_param("eps_diss", eps)
+    for tile in range(chem.NUM_TILES):
+        h.set_variant(1, tile)
+        assert relerr(gpu_rhs(h, u), want) < TOL_RHS, tile
+    h.destroy()
+
+
+def test_wave_config0_20_steps(chem, oracle):
+    c = inputs.config(0)
+    u0 = c["state"]()
+    n, g, dx = c["dims"][0], c["ghost"], c["dx"]
+    dt = 0.25 * dx
+    h = chem.Chemora(n, n, n, g, c["order"], 0, dx)
+    h.set_state(u0)
+    st = oracle.with_ghosts(u0, g)
+    for step in range(1, 21):
+        h.rk4_step(dt)
+        oracle.rk4(0, st, g, c["order"], dx, dt, oracle.params(), 1)
+        if step in (1, 2, 20):
+            assert relerr(h.get_state(), oracle.interior(st, g)) < TOL_WAVE_PER_STEP * step, step
+    h.destroy()
+
+
+def test_wave_config1_shape_at_48(chem, oracle):
+    """configs[1] (O8, g=4, KO eps=0.1, plane-wave sum) at 48x48x48 -- several tiles and a ragged tail."""
+    c = inputs.config(1, scale=48)
+    u0 = c["state"]()
+    n, g, dx = 48, c["ghost"], c["dx"]
+    dt = 0.25 * dx
+    h = chem.Chemora(n, n, n, g, 8, 0, dx)
+    h.set_param("eps_diss", c["eps_diss"])
+    h.set_state(u0)
+    st = oracle.with_ghosts(u0, g)
+    for step in range(1, 4):
+        h.rk4_step(dt)
+        oracle.rk4(0, st, g, 8, dx, dt, oracle.params(eps_diss=c["eps_diss"]), 1)
+        assert relerr(h.get_state(), oracle.interior(st, g)) < TOL_WAVE_PER_STEP * step
+    h.destroy()
+
+
+# ------------------------------------------------------------------------------------------------ BSSN
+def strong_field(nx, ny, nz, seed=21):
+    """far-from-flat random data exercising every nonlinear term (gt = delta + 0.1 noise, etc.)."""
+    rng = np.random.default_rng(seed)
+    u = inputs.bssn_minkowski(nx, ny, nz)
+    u += 0.1 * rng.uniform(-1, 1, size=u.shape)
+    return u
+
+
+@pytest.mark.parametrize("data", ["noise1e-10", "gaussians", "strong"])
+def test_bssn_rhs_all_variants_and_tiles(chem, oracle, data):
+    nx, ny, nz = 37, 22, 19
+    u = {"noise1e-10": lambda: inputs.bssn_noise(nx, ny, nz),
+         "gaussians": lambda: inputs.bssn_gaussians(nx, ny, nz, width_cells=4.0),
+         "strong": lambda: strong_field(nx, ny, nz)}[data]()
+    dx, eps = 0.05, 0.1
+    want = oracle_rhs(oracle, 1, u, 3, 4, dx, eps_diss=eps)
+    h = chem.Chemora(nx, ny, nz, 3, 4, 1, dx)
+    h.set_param("eps_diss", eps)
+    for fused in (1, 0):
+        for tile in range(chem.NUM_TILES):
+            h.set_variant(fused, tile)
+            got = gpu_rhs(h, u)
+            assert relerr(got, want) < TOL_RHS, (fused, tile)
+    h.destroy()
+
+
+def test_bssn_flat_stays_flat_bitwise(chem):
+    u = inputs.bssn_minkowski(20, 17, 9)
+    h = chem.Chemora(20, 17, 9, 3, 4, 1, 0.05)
+    h.set_param("eps_diss", 0.1)
+    assert not gpu_rhs(h, u).any()
+    for fused in (1, 0):
+        h.set_variant(fused, 1)
+        h.set_state(u)
+        for _ in range(3):
+            h.rk4_step(0.0125)
+        assert np.array_equal(h.get_state(), u)
+    h.destroy()
+
+
+@pytest.mark.parametrize("fused", [1, 0])
+def test_bssn_rk4_10_steps_small(chem, oracle, fused):
+    """configs[2] data (Minkowski + 1e-10 noise) at 24x20x18, 10 steps."""
+    nx, ny, nz = 24, 20, 18
+    u0 = inputs.bssn_noise(nx, ny, nz)
+    dx, dt, eps = 0.05, 0.0125, 0.1
+    h = chem.Chemora(nx, ny, nz, 3, 4, 1, dx)
+    h.set_param("eps_diss", eps)
+    h.set_variant(fused, 1)
+    h.set_state(u0)
+    for _ in range(10):
+        h.rk4_step(dt)
+    st = oracle.rk4(1, oracle.with_ghosts(u0, 3), 3, 4, dx, dt, oracle.params(eps_diss=eps), 10)
+    assert relerr(h.get_state(), oracle.interior(st, 3)) < TOL_BSSN_10_STEPS
+    h.destroy()
+
+
+def test_bssn_config2_full_size_10_steps(chem, oracle):
+    """configs[2] exactly: 64^3, g=3, O4 + upwind + KO, Minkowski + 1e-10 noise, 10 steps (oracle ~1-2 min)."""
+    c = inputs.config(2)
+    u0 = c["state"]()
+    n, dx = 64, c["dx"]
+    h = chem.Chemora(n, n, n, 3, 4, 1, dx)
+    h.set_param("eps_diss", c["eps_diss"])
+    h.set_state(u0)
+    for _ in range(10):
+        h.rk4_step(0.25 * dx)
+    st = oracle.rk4(1, oracle.with_ghosts(u0, 3), 3, 4, dx, 0.25 * dx, oracle.params(eps_diss=c["eps_diss"]), 10)
+    assert relerr(h.get_state(), oracle.interior(st, 3)) < TOL_BSSN_10_STEPS
+    h.destroy()
+
+
+def test_autotune_and_kernel_info(chem):
+    n = 40
+    h = chem.Chemora(n, n, n, 3, 4, 1, 0.05)
+    h.set_param("eps_diss", 0.1)
+    u = inputs.bssn_noise(n, n, n)
+    h.set_state(u)
+    fused, tile, ms = h.autotune()
+    assert fused in (0, 1) and 0 <= tile < chem.NUM_TILES and all(m > 0 for m in ms)
+    assert (fused, tile) == h.get_variant()
+    assert np.array_equal(h.get_state(), u)        # U is not modified by the sweep
+    info = h.kernel_info()
+    assert 0 < info["regs"] <= 255
+    assert h.launch_count() > 0
+    h.destroy()
