@@ -1,0 +1,269 @@
+#!/usr/bin/env python
+"""bench.py -- BSSN RHS+RK4 grid-point updates/sec, fp64 4th-order 256^3 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--size 256]
+
+A "step" is one pass of the whole hot path over the grid: 4 x (ghost fill + fused derivative/RHS/RK4-stage
+kernel) = one chemora_rk4_step.  Workload: BASELINE.json configs[3] (BSSN, 256^3, g=3, O4 + upwind + KO,
+Minkowski + 1e-4 Gaussians), synthetic, seeded.  One process per GPU; the path does not shard without a
+halo exchange (north_star: one GPU), so N>1 runs N independent replicas ("replicas only", weak scaling).
+--impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload.
+Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "BSSN RHS+RK4 grid-point updates/sec, fp64 4th-order 256^3"
+UNIT = "grid-point updates/s"
+# algorithmic HBM traffic of the fused 4-buffer RK4 scheme (reading S9), V = 25:
+# stage 1 reads U, writes S,Yb (75 doubles); stages 2-3 read Y,U,S write S,Y' (125 each); stage 4 reads
+# Y,S,U writes U (100): 425 doubles = 3400 B per grid-point update, i.e. 850 B per RHS-kernel launch and point.
+BYTES_PER_UPDATE = 3400.0
+BYTES_PER_POINT_PER_LAUNCH = BYTES_PER_UPDATE / 4.0
+# counted with the paper's convention -- see DESIGN.md
+FLOPS_PER_RHS_POINT = 4460.0
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)), "measured (MEASURED_PEAKS.json)"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.lines, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def time_oracle(sample_n, steps, warmup):
+    """The oracle as it stands, on the host cores, on a bounded sample: configs[3] recipe at sample_n^3."""
+    from oracle import oracle
+    from paper_1307_6488_b200 import inputs
+    c = inputs.config(3, scale=sample_n)
+    cores = len(os.sched_getaffinity(0))
+    oracle.set_threads(cores)
+    st = oracle.with_ghosts(c["state"](), c["ghost"])
+    prm = oracle.params(eps_diss=c["eps_diss"])
+    dt = 0.25 * c["dx"]
+    if warmup:
+        oracle.rk4(oracle.SYS_BSSN, st, c["ghost"], c["order"], c["dx"], dt, prm, warmup)
+    t0 = time.perf_counter()
+    oracle.rk4(oracle.SYS_BSSN, st, c["ghost"], c["order"], c["dx"], dt, prm, steps)
+    el = time.perf_counter() - t0
+    return sample_n ** 3 * steps / el, el, cores
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n = args.ref_sample
+    steps, warmup = max(1, args.steps), args.warmup
+    # keep the whole run within a few minutes whatever K is: cap the oracle work at ~6e6 point updates
+    while n > 16 and n ** 3 * (steps + warmup) > 6e6:
+        n -= 8
+    val, el, cores = time_oracle(n, steps, warmup)
+    sample = "%d RK4 steps (+%d warm-up) of the configs[3] recipe on a %d^3 periodic block, %d OpenMP threads" % (
+        steps, warmup, n, cores)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": warmup, "ms_per_step": el / steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "BSSN O4 fp64, configs[3] recipe, bounded sample %d^3 (CPU oracle)" % n},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    from paper_1307_6488_b200 import binding, inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device and no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    n = args.size
+    c = inputs.config(3, scale=n)
+    g, dx = c["ghost"], c["dx"]
+    dt = 0.25 * dx
+    u0 = inputs.bssn_gaussians(n, n, n, seed=inputs.SEED_BASE + 3 + rank)   # one replica per rank
+    h = binding.Chemora(n, n, n, g, c["order"], binding.SYS_BSSN, dx, device="cuda:%d" % local)
+    h.set_param("eps_diss", c["eps_diss"])
+    host = torch.from_numpy(u0).pin_memory()
+    h.set_state(host.numpy())
+    if args.variant == "auto":
+        fused, tile, sweep_ms = h.autotune()
+    else:
+        fused, tile = [int(x) for x in args.variant.split(",")]
+        h.set_variant(fused, tile)
+        sweep_ms = None
+    info = h.kernel_info()
+
+    # ---- device-resident timing: W warm-up, then exactly K steps ------------------------------------------
+    for _ in range(args.warmup):
+        h.rk4_step(dt)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    h.timing(1)
+    l0 = h.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        h.rk4_step(dt)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = h.launch_count() - l0
+    kt = h.timing_read()
+    h.timing(0)
+    clocks = sampler.stop() if rank == 0 else None
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = world * n ** 3 * args.steps / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers: H2D + K' steps... per step: set_state, rk4_step, get_state
+    e2e_steps = max(1, min(args.e2e_steps, args.steps))
+    out = torch.empty_like(host).pin_memory()
+    h.set_state(host.numpy()); h.rk4_step(dt); h.get_state(out.numpy())   # warm-up (staging allocation)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        h.set_state(host.numpy())
+        h.rk4_step(dt)
+        h.get_state(out.numpy())
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_val = world * n ** 3 * e2e_steps / float(t.item())
+    nbytes = host.numel() * 8
+
+    fp64_gf = h.measure_fp64_peak() if rank == 0 else None
+    h.destroy()
+    if dist is not None:
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+
+    pk, pk_src = peaks()
+    rhs_launch_ms = kt["rhs_ms"] / max(kt["rhs_launches"], 1) * (1 if fused else 2)   # per RHS evaluation
+    achieved = BYTES_PER_POINT_PER_LAUNCH * n ** 3 / (rhs_launch_ms * 1e-3) / 1e9
+    hbm_peak = pk["hbm_gbs"]
+    gf = FLOPS_PER_RHS_POINT * n ** 3 / (rhs_launch_ms * 1e-3) / 1e9
+    cpu_val, cpu_el, cores = time_oracle(args.cpu_sample, 2, 0)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BSSN (25 vars) O4 centred FD + upwind advection + KO5, fp64, %d^3 interior, g=3, "
+                               "RK4 4-buffer, configs[3] recipe (Minkowski + 1e-4 Gaussians)" % n,
+                   "variant": {"fused": fused, "tile": list(binding.tile_shape(tile, binding.SYS_BSSN, fused)), "sweep_ms": sweep_ms},
+                   "kernel": info, "multi_gpu": "replicas only",
+                   "l2": "inputs larger than L2 (%.2f GB per state buffer vs 126 MB)" % (h.nvars * h.var_stride * 8 / 1e9)},
+        "roofline": {"bound": "hbm", "kernel": "bssn_tma_kernel" if fused else "bssn_derivs+from_derivs",
+                     "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
+                     "traffic": None, "peak_source": pk_src, "ms_per_launch": rhs_launch_ms,
+                     "share_of_step": kt["rhs_ms"] / ms, "fill_share_of_step": kt["fill_ms"] / ms},
+        "roofline_fp64": {"bound": "alu", "achieved": gf, "peak": fp64_gf, "unit": "GFLOP/s",
+                          "frac": gf / fp64_gf if fp64_gf else None, "flops_per_rhs_point": FLOPS_PER_RHS_POINT,
+                          "peak_source": "measured in this run: DFMA chains on all SMs (chemora_measure_fp64_peak)"},
+        "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": "2 RK4 steps of the configs[3] recipe on a %d^3 periodic block (%.1f s)" % (
+                             args.cpu_sample, cpu_el)},
+        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                "steps": e2e_steps},
+        "gpu_launches": launches, "clocks": clocks,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--size", type=int, default=256)
+    ap.add_argument("--variant", default="auto", help="'auto' (runtime sweep) or 'fused,tile' e.g. 1,3")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-sample", type=int, default=64)
+    ap.add_argument("--ref-sample", type=int, default=64)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -96,19 +96,29 @@ int chemora_rk4_step(chemora_t* h, double dt);
 
 /* Kernel variant: fused (1: derivatives + RHS + RK stage update in one kernel) or split (0: derivatives
  * written to global arrays by one kernel, RHS + stage update by a second), and tile_id in
- * [0, CHEMORA_NUM_TILES).  chemora_tile_shape reports the (x, y, z) extent of a tile id. */
+ * [0, CHEMORA_NUM_TILES).  chemora_tile_shape reports the (x, y, z) extent of a tile id: for the fused BSSN
+ * kernel a 3-D tile with one grid point per thread (staged with a 3-cell halo by TMA); for the split BSSN
+ * kernels and the wave kernel an x*y thread block marching z planes. */
 int chemora_set_variant(chemora_t* h, int fused, int tile_id);
 int chemora_get_variant(const chemora_t* h, int* fused, int* tile_id);
-int chemora_tile_shape(int tile_id, int* tx, int* ty, int* tz);
+int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, int* tz);
 
 /* Runtime sweep (the paper's model-based choice, replaced by measurement): times every
- * (fused, tile) once on the handle's own grid (RHS on the current U), keeps the fastest, returns it.
+ * (fused, tile) once on the handle's own grid (one middle RK4 stage evaluated on the current U, results
+ * into the scratch buffers S and Ya), keeps the fastest, returns it.
  * ms_out, if not NULL, receives 2*CHEMORA_NUM_TILES timings in milliseconds ([fused*NUM_TILES + tile];
  * negative = variant unavailable).  U is not modified.  Synchronous. */
 int chemora_autotune(chemora_t* h, int* fused, int* tile_id, float* ms_out);
 
 /* Number of kernel launches issued through this handle so far (for benchmarks' gpu_launches). */
 long chemora_launch_count(const chemora_t* h);
+
+/* Per-kernel device timing for benchmarks: chemora_timing(h, 1) starts recording a CUDA-event pair on the
+ * handle's stream around every RHS evaluation (all kernels of the current variant) and around every ghost
+ * fill, and resets the totals; chemora_timing(h, 0) stops.  chemora_timing_read synchronises the stream
+ * and returns the summed durations in milliseconds and the number of kernels launched inside them. */
+int chemora_timing(chemora_t* h, int enable);
+int chemora_timing_read(chemora_t* h, double* rhs_ms, long* rhs_launches, double* fill_ms, long* fill_launches);
 
 /* Static kernel resource usage of the current variant's main kernel (from cudaFuncGetAttributes):
  * registers per thread, local (spill) bytes per thread, static+dynamic shared bytes per block. */

@@ -23,7 +23,7 @@ SYMBOLS = ["chemora_create", "chemora_set_param", "chemora_get_param", "chemora_
            "chemora_set_state", "chemora_get_state", "chemora_set_state_dev", "chemora_get_state_dev",
            "chemora_fill_ghosts", "chemora_rhs", "chemora_rk4_step", "chemora_set_variant",
            "chemora_get_variant", "chemora_tile_shape", "chemora_autotune", "chemora_launch_count",
-           "chemora_kernel_info", "chemora_measure_fp64_peak", "chemora_last_error", "chemora_destroy"]
+           "chemora_kernel_info", "chemora_timing", "chemora_timing_read", "chemora_measure_fp64_peak", "chemora_last_error", "chemora_destroy"]
 
 _ALLOC_T = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
 _DEALLOC_T = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p)
@@ -59,11 +59,12 @@ def load():
         "chemora_fill_ghosts": [vp, vp], "chemora_rhs": [vp, vp, vp],
         "chemora_rk4_step": [vp, d],
         "chemora_set_variant": [vp, i, i], "chemora_get_variant": [vp, ip, ip],
-        "chemora_tile_shape": [i, ip, ip, ip],
+        "chemora_tile_shape": [i, i, i, ip, ip, ip],
         "chemora_autotune": [vp, ip, ip, ctypes.POINTER(ctypes.c_float)],
         "chemora_launch_count": [vp],
         "chemora_kernel_info": [vp, ip, ip, ip],
         "chemora_measure_fp64_peak": [vp, dp],
+        "chemora_timing": [vp, i], "chemora_timing_read": [vp, dp, lp, dp, lp],
         "chemora_last_error": [vp], "chemora_destroy": [vp],
     }
     for name, args in sig.items():
@@ -76,9 +77,9 @@ def load():
     return lib
 
 
-def tile_shape(tile_id):
+def tile_shape(tile_id, system_id=SYS_BSSN, fused=1):
     a, b, c = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
-    rc = load().chemora_tile_shape(tile_id, a, b, c)
+    rc = load().chemora_tile_shape(system_id, fused, tile_id, a, b, c)
     if rc:
         raise ChemoraError(rc)
     return a.value, b.value, c.value
@@ -216,6 +217,14 @@ class Chemora:
         r, l, s = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
         self._ck(self.lib.chemora_kernel_info(self._h, r, l, s))
         return dict(regs=r.value, local_bytes=l.value, smem_bytes=s.value)
+
+    def timing(self, enable):
+        self._ck(self.lib.chemora_timing(self._h, int(enable)))
+
+    def timing_read(self):
+        a, b, c, d = ctypes.c_double(), ctypes.c_long(), ctypes.c_double(), ctypes.c_long()
+        self._ck(self.lib.chemora_timing_read(self._h, a, b, c, d))
+        return dict(rhs_ms=a.value, rhs_launches=b.value, fill_ms=c.value, fill_launches=d.value)
 
     def measure_fp64_peak(self):
         v = ctypes.c_double()

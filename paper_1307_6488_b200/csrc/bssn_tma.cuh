@@ -1,0 +1,158 @@
+// bssn_tma.cuh -- device side of the fused BSSN kernel: persistent CTAs, one grid point per thread, the
+// (tile + 3-cell halo) box of ONE variable at a time staged into shared memory by TMA (cp.async.bulk.tensor)
+// through a 5-slot mbarrier ring, so that every stencil read is an LDS with a compile-time offset.
+// The variables are consumed in an order chosen to keep the live register set small (H2 in SURVEY.md):
+//   beta^i -> gt_ij -> [Christoffels, quadratic part of R~_ij] -> Gt^i -> chi -> alpha -> K -> At_ij -> B^i -> A
+// Each variable's derivatives are contracted / folded into the few values the pointwise expression needs as
+// soon as they are produced, and each right-hand side leaves through the fused RK4 stage update the moment
+// it is complete.  Mathematics: readings S2-S6, S10 of DESIGN.md (same system as bssn_point.cuh; that file
+// serves the split variant).
+#pragma once
+#include <cuda.h>
+
+#include "bssn_point.cuh"
+
+namespace chm {
+
+// ---- TMA / mbarrier PTX wrappers ----------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, uint64_t* bar, int x, int y, int z,
+                                            int v) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+      ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z), "r"(v) : "memory");
+}
+
+// ---- stencil reads from the staged box -------------------------------------------------------------------------
+// `c` points at this thread's own grid point inside the current slot; BX, BY are the box row / plane extents.
+template <int BX, int BY>
+struct BoxPoint {
+  const double* c;
+  __device__ __forceinline__ double at(int di, int dj, int dk) const { return c[(dk * BY + dj) * BX + di]; }
+  __device__ __forceinline__ double ax(int a, int m) const {
+    return a == 0 ? at(m, 0, 0) : (a == 1 ? at(0, m, 0) : at(0, 0, m));
+  }
+  __device__ __forceinline__ double ax2(int a, int m, int b, int n) const {
+    int d[3] = {0, 0, 0};
+    d[a] = m; d[b] = n;
+    return at(d[0], d[1], d[2]);
+  }
+};
+
+// Per-point upwind/dissipation weights: beta^a d^up_a u + KO(u) = sum_a  wq[a] * q_a(u) + ws[a] * sp_a(u)
+//   q_a  = s3 - 6 s2 + 15 s1   (s_k = (u[+k]-u0) + (u[-k]-u0))      symmetric 7-point (the KO stencil)
+//   sp_a = 21 e1 - 6 e2 + e3   (e_k = u[+k] - u[-k])                 antisymmetric 7-point
+// because the one-point-off-centre upwind stencils of reading S2 satisfy  up(+-) = (sp +- q) / 24h, so
+//   wq[a] = |beta^a| / 24h + eps/64h ,   ws[a] = beta^a / 24h .
+struct AdvW { double wq[3], ws[3]; };
+
+// one axis of one variable: centred d1, d2 and the advection+dissipation contribution, all from 6 reads
+template <class P>
+__device__ __forceinline__ void axis_full(const P& p, double f0, int a, const Coef& C, const AdvW& w, double& d1,
+                                          double& d2, double& ad) {
+  const double p1 = p.ax(a, 1), m1 = p.ax(a, -1), p2 = p.ax(a, 2), m2 = p.ax(a, -2), p3 = p.ax(a, 3), m3 = p.ax(a, -3);
+  const double e1 = p1 - m1, e2 = p2 - m2, e3 = p3 - m3;
+  const double s1 = (p1 - f0) + (m1 - f0), s2 = (p2 - f0) + (m2 - f0), s3 = (p3 - f0) + (m3 - f0);
+  d1 = (8.0 * e1 - e2) * (C.inv_h * (1.0 / 12.0));
+  d2 = (16.0 * s1 - s2) * (C.inv_h2 * (1.0 / 12.0));
+  const double q = (s3 - 6.0 * s2) + 15.0 * s1;
+  const double sp = (21.0 * e1 - 6.0 * e2) + e3;
+  ad += w.wq[a] * q + w.ws[a] * sp;
+}
+template <class P>
+__device__ __forceinline__ void axis_d1_ad(const P& p, double f0, int a, const Coef& C, const AdvW& w, double& d1,
+                                           double& ad) {
+  const double p1 = p.ax(a, 1), m1 = p.ax(a, -1), p2 = p.ax(a, 2), m2 = p.ax(a, -2), p3 = p.ax(a, 3), m3 = p.ax(a, -3);
+  const double e1 = p1 - m1, e2 = p2 - m2, e3 = p3 - m3;
+  const double s1 = (p1 - f0) + (m1 - f0), s2 = (p2 - f0) + (m2 - f0), s3 = (p3 - f0) + (m3 - f0);
+  d1 = (8.0 * e1 - e2) * (C.inv_h * (1.0 / 12.0));
+  const double q = (s3 - 6.0 * s2) + 15.0 * s1;
+  const double sp = (21.0 * e1 - 6.0 * e2) + e3;
+  ad += w.wq[a] * q + w.ws[a] * sp;
+}
+template <class P>
+__device__ __forceinline__ void axis_ad(const P& p, double f0, int a, const AdvW& w, double& ad) {
+  const double p1 = p.ax(a, 1), m1 = p.ax(a, -1), p2 = p.ax(a, 2), m2 = p.ax(a, -2), p3 = p.ax(a, 3), m3 = p.ax(a, -3);
+  const double e1 = p1 - m1, e2 = p2 - m2, e3 = p3 - m3;
+  const double s1 = (p1 - f0) + (m1 - f0), s2 = (p2 - f0) + (m2 - f0), s3 = (p3 - f0) + (m3 - f0);
+  const double q = (s3 - 6.0 * s2) + 15.0 * s1;
+  const double sp = (21.0 * e1 - 6.0 * e2) + e3;
+  ad += w.wq[a] * q + w.ws[a] * sp;
+}
+// dissipation only (slot A): ko * q
+template <class P>
+__device__ __forceinline__ double axis_q(const P& p, double f0, int a) {
+  const double s1 = (p.ax(a, 1) - f0) + (p.ax(a, -1) - f0), s2 = (p.ax(a, 2) - f0) + (p.ax(a, -2) - f0),
+               s3 = (p.ax(a, 3) - f0) + (p.ax(a, -3) - f0);
+  return (s3 - 6.0 * s2) + 15.0 * s1;
+}
+// mixed derivative d_a d_b (a != b), 16 reads
+template <class P>
+__device__ __forceinline__ double mixed(const P& p, int a, int b, const Coef& C) {
+  double r[4];
+  const int off[4] = {1, -1, 2, -2};
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    const int m = off[t];
+    const double e1 = p.ax2(a, m, b, 1) - p.ax2(a, m, b, -1);
+    const double e2 = p.ax2(a, m, b, 2) - p.ax2(a, m, b, -2);
+    r[t] = 8.0 * e1 - e2;
+  }
+  return (8.0 * (r[0] - r[1]) - (r[2] - r[3])) * (C.inv_h2 * (1.0 / 144.0));
+}
+
+// all of one "full" variable (beta^i, gt_ij, chi, alpha): d1[3], packed d2[6], ad
+template <class P>
+__device__ __forceinline__ void var_full(const P& p, const Coef& C, const AdvW& w, double* d1, double* d2, double& ad) {
+  const double f0 = p.at(0, 0, 0);
+  ad = 0.0;
+  axis_full(p, f0, 0, C, w, d1[0], d2[0], ad);
+  axis_full(p, f0, 1, C, w, d1[1], d2[3], ad);
+  axis_full(p, f0, 2, C, w, d1[2], d2[5], ad);
+  d2[1] = mixed(p, 0, 1, C);
+  d2[2] = mixed(p, 0, 2, C);
+  d2[4] = mixed(p, 1, 2, C);
+}
+template <class P>
+__device__ __forceinline__ void var_d1_ad(const P& p, const Coef& C, const AdvW& w, double* d1, double& ad) {
+  const double f0 = p.at(0, 0, 0);
+  ad = 0.0;
+  axis_d1_ad(p, f0, 0, C, w, d1[0], ad);
+  axis_d1_ad(p, f0, 1, C, w, d1[1], ad);
+  axis_d1_ad(p, f0, 2, C, w, d1[2], ad);
+}
+template <class P>
+__device__ __forceinline__ double var_ad(const P& p, const AdvW& w) {
+  const double f0 = p.at(0, 0, 0);
+  double ad = 0.0;
+  axis_ad(p, f0, 0, w, ad);
+  axis_ad(p, f0, 1, w, ad);
+  axis_ad(p, f0, 2, w, ad);
+  return ad;
+}
+
+// consumption order of the 25 variables (slot of order index o is o % 5)
+__device__ __forceinline__ constexpr int order_var(int o) {
+  return o < 3 ? V_BETA + o : o < 9 ? V_GT + (o - 3) : o < 12 ? V_GAM + (o - 9) : o == 12 ? V_CHI : o == 13 ? V_ALPHA
+         : o == 14 ? V_K : o < 21 ? V_AT + (o - 15) : o < 24 ? V_B + (o - 21) : V_A;
+}
+
+}  // namespace chm

@@ -28,6 +28,10 @@ struct chemora {
   double* staging;      // device packed staging for set/get_state (lazy)
   int fused, tile;
   long launches;
+  // optional per-kernel timing (chemora_timing): event pairs around every RHS evaluation / ghost fill
+  bool timing;
+  std::vector<cudaEvent_t> ev[2];   // [0] rhs, [1] fill; consecutive (start, stop) pairs
+  long ev_launches[2];
   std::string err;
 };
 
@@ -82,8 +86,27 @@ int ensure_derivs(chemora_t* h) {
   return CHEMORA_OK;
 }
 
+void tick(chemora_t* h, int cat) {
+  if (!h->timing) return;
+  cudaEvent_t e;
+  if (cudaEventCreate(&e) != cudaSuccess) return;
+  cudaEventRecord(e, h->stream);
+  h->ev[cat].push_back(e);
+}
+
+int run_rhs_inner(chemora_t* h, const Stage& st);
+
 // one RHS evaluation with the given epilogue; counts launches
 int run_rhs(chemora_t* h, const Stage& st) {
+  tick(h, 0);
+  long before = h->launches;
+  int rc = run_rhs_inner(h, st);
+  tick(h, 0);
+  if (h->timing) h->ev_launches[0] += h->launches - before;
+  return rc;
+}
+
+int run_rhs_inner(chemora_t* h, const Stage& st) {
   if (h->eps_diss != 0.0 && h->L.g < 3) return fail(h, CHEMORA_EINVAL, "eps_diss != 0 needs ghost >= 3 (KO order 5)");
   Coef C = make_coef(h);
   if (h->system == CHEMORA_SYS_WAVE) {
@@ -103,8 +126,11 @@ int run_rhs(chemora_t* h, const Stage& st) {
 }
 
 int fill(chemora_t* h, double* state) {
+  tick(h, 1);
   CK(h, launch_fill_ghosts(h->L, state, h->stream), "ghost fill launch");
+  tick(h, 1);
   h->launches += 1;
+  if (h->timing) h->ev_launches[1] += 1;
   return CHEMORA_OK;
 }
 
@@ -143,6 +169,8 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
   h->derivs = nullptr; h->staging = nullptr;
   h->fused = 1; h->tile = 1;
   h->launches = 0;
+  h->timing = false;
+  h->ev_launches[0] = h->ev_launches[1] = 0;
   for (int b = 0; b < 4; ++b) h->buf[b] = nullptr;
 
   int ndev = 0;
@@ -297,11 +325,12 @@ int chemora_get_variant(const chemora_t* h, int* fused, int* tile_id) {
   return CHEMORA_OK;
 }
 
-int chemora_tile_shape(int tile_id, int* tx, int* ty, int* tz) {
+int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, int* tz) {
   if (tile_id < 0 || tile_id >= CHEMORA_NUM_TILES) return CHEMORA_EINVAL;
-  if (tx) *tx = kTiles[tile_id].tx;
-  if (ty) *ty = kTiles[tile_id].ty;
-  if (tz) *tz = kTiles[tile_id].tz;
+  const TileShape* T = (system_id == CHEMORA_SYS_BSSN && fused) ? kTilesFused : kTilesMarch;
+  if (tx) *tx = T[tile_id].tx;
+  if (ty) *ty = T[tile_id].ty;
+  if (tz) *tz = T[tile_id].tz;
   return CHEMORA_OK;
 }
 
@@ -319,7 +348,9 @@ int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out)
       float ms = -1.f;
       if (f == 1 || h->system == CHEMORA_SYS_BSSN) {
         h->fused = f; h->tile = t;
-        Stage st{h->buf[0], nullptr, nullptr, h->buf[3], 0.0, MODE_RHS};   // RHS(U) -> S (scratch)
+        // a middle RK4 stage (the common case) on scratch operands: k = f(U); S += 2k; Ya = U + a k.
+        // S and Ya are scratch between steps (stage 1 overwrites them); U is only read.
+        Stage st{h->buf[0], h->buf[0], h->buf[3], h->buf[1], 1e-3, MODE_MID};
         rc = run_rhs(h, st);                                               // warm-up
         if (!rc) {
           cudaEventRecord(e0, h->stream);
@@ -343,11 +374,44 @@ int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out)
 
 long chemora_launch_count(const chemora_t* h) { return h ? h->launches : 0; }
 
+static void drop_events(chemora_t* h) {
+  for (int c = 0; c < 2; ++c) {
+    for (cudaEvent_t e : h->ev[c]) cudaEventDestroy(e);
+    h->ev[c].clear();
+    h->ev_launches[c] = 0;
+  }
+}
+
+int chemora_timing(chemora_t* h, int enable) {
+  if (!h) return CHEMORA_EINVAL;
+  drop_events(h);
+  h->timing = enable != 0;
+  return CHEMORA_OK;
+}
+
+int chemora_timing_read(chemora_t* h, double* rhs_ms, long* rhs_launches, double* fill_ms, long* fill_launches) {
+  if (!h) return CHEMORA_EINVAL;
+  CK(h, cudaStreamSynchronize(h->stream), "timing sync");
+  double tot[2] = {0.0, 0.0};
+  for (int c = 0; c < 2; ++c)
+    for (size_t i = 0; i + 1 < h->ev[c].size(); i += 2) {
+      float ms = 0.f;
+      CK(h, cudaEventElapsedTime(&ms, h->ev[c][i], h->ev[c][i + 1]), "event elapsed");
+      tot[c] += ms;
+    }
+  if (rhs_ms) *rhs_ms = tot[0];
+  if (fill_ms) *fill_ms = tot[1];
+  if (rhs_launches) *rhs_launches = h->ev_launches[0];
+  if (fill_launches) *fill_launches = h->ev_launches[1];
+  return CHEMORA_OK;
+}
+
 int chemora_kernel_info(const chemora_t* h, int* regs, int* local_bytes, int* smem_bytes) {
   if (!h) return CHEMORA_EINVAL;
   cudaFuncAttributes a;
   cudaError_t e = h->system == CHEMORA_SYS_WAVE ? kernel_info_wave(h->order, h->tile, &a)
-                                                : kernel_info_bssn(h->fused, h->tile, &a);
+                  : h->fused               ? kernel_info_bssn_fused(h->tile, &a)
+                                           : kernel_info_bssn_split(1, h->tile, &a);
   if (e != cudaSuccess) return cuda_fail(const_cast<chemora_t*>(h), e, "cudaFuncGetAttributes");
   if (regs) *regs = a.numRegs;
   if (local_bytes) *local_bytes = (int)a.localSizeBytes;
@@ -390,6 +454,7 @@ const char* chemora_last_error(const chemora_t* h) { return h ? h->err.c_str() :
 int chemora_destroy(chemora_t* h) {
   if (!h) return CHEMORA_OK;
   cudaStreamSynchronize(h->stream);
+  drop_events(h);
   for (int b = 0; b < 4; ++b) dev_free(h, h->buf[b]);
   dev_free(h, h->derivs);
   dev_free(h, h->staging);

@@ -57,9 +57,31 @@ __device__ __forceinline__ void stage_emit(const Stage& st, long q, double k) {
   }
 }
 
-// Tile shapes of the variant sweep (threads in x, y; planes marched in z).
+// Split form of stage_emit: fetch the operands early (stage_prefetch), combine and store later.
+struct StagePre { double u, s; };
+__device__ __forceinline__ void stage_prefetch(const Stage& st, long q, StagePre& r) {
+  if (st.mode == MODE_FIRST) r.u = st.in[q];
+  else if (st.mode != MODE_RHS) { r.u = st.U[q]; r.s = st.S[q]; }
+}
+__device__ __forceinline__ void stage_emit(const Stage& st, long q, double k, const StagePre& pr) {
+  if (st.mode == MODE_RHS) {
+    st.out[q] = k;
+  } else if (st.mode == MODE_FIRST) {
+    st.S[q] = k;
+    st.out[q] = __dadd_rn(pr.u, __dmul_rn(st.a, k));
+  } else if (st.mode == MODE_MID) {
+    st.S[q] = __dadd_rn(pr.s, __dmul_rn(2.0, k));
+    st.out[q] = __dadd_rn(pr.u, __dmul_rn(st.a, k));
+  } else {
+    st.U[q] = __dadd_rn(pr.u, __dmul_rn(st.a, __dadd_rn(pr.s, k)));
+  }
+}
+
+// Tile shapes of the variant sweep.  Fused kernel: 3-D tile, one point per thread.  Split kernels and the wave
+// kernel: x,y = thread block, z = planes marched per block.
 struct TileShape { int tx, ty, tz; };
-static const TileShape kTiles[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64, 4, 8}, {128, 2, 8}, {16, 16, 8}};
+static const TileShape kTilesFused[6] = {{16, 4, 4}, {16, 8, 2}, {32, 4, 2}, {32, 2, 4}, {8, 8, 4}, {16, 4, 2}};
+static const TileShape kTilesMarch[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64, 4, 8}, {128, 2, 8}, {16, 16, 8}};
 
 // launchers implemented in the kernel translation units; each returns the cudaError_t of the launch
 cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s);
@@ -71,7 +93,8 @@ cudaError_t launch_bssn_derivs(const Layout& L, const Coef& C, int tile, const d
 cudaError_t launch_bssn_from_derivs(const Layout& L, const Coef& C, int tile, const double* derivs,
                                     const Stage& st, cudaStream_t s);
 cudaError_t kernel_info_wave(int order, int tile, cudaFuncAttributes* a);
-cudaError_t kernel_info_bssn(int fused, int tile, cudaFuncAttributes* a);
+cudaError_t kernel_info_bssn_fused(int tile, cudaFuncAttributes* a);
+cudaError_t kernel_info_bssn_split(int which, int tile, cudaFuncAttributes* a);
 cudaError_t launch_dfma_peak(int blocks, int threads, int iters, double* sink, cudaStream_t s);
 
 // number of derivative arrays of the split variant: 45 first + 66 second + 25 advection+dissipation

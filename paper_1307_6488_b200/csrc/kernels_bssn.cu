@@ -1,5 +1,6 @@
-// kernels_bssn.cu -- BSSN right-hand side kernels: fused (derivatives + RHS + RK4 stage update in one kernel)
-// and split (derivatives to global arrays, then RHS + stage update).
+// kernels_bssn.cu -- BSSN right-hand side, split variant: one kernel writes the derivative
+// arrays to global memory, a second evaluates the RHS from them (+ RK4 stage update).  The fused kernel is in
+// kernels_bssn_tma.cu.
 #include "bssn_point.cuh"
 #include "stencils.cuh"
 
@@ -55,22 +56,6 @@ __host__ __device__ inline long packed_stride(const Layout& L) {
 }
 
 template <int TX, int TY, int TZ>
-__global__ void __launch_bounds__(TX* TY) bssn_fused_kernel(Layout L, Coef C, Stage st) {
-  const int i = blockIdx.x * TX + threadIdx.x, j = blockIdx.y * TY + threadIdx.y;
-  if (i >= L.nx || j >= L.ny) return;
-  const int k0 = blockIdx.z * TZ;
-#pragma unroll 1
-  for (int kk = 0; kk < TZ; ++kk) {
-    const int k = k0 + kk;
-    if (k >= L.nz) break;
-    const long q = (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.g);
-    OnTheFly<GlobalPoint> D{{st.in + q, L.pitch, L.plane, L.vstride}, C, {0, 0, 0}};
-    D.beta[0] = D.f(V_BETA); D.beta[1] = D.f(V_BETA + 1); D.beta[2] = D.f(V_BETA + 2);
-    bssn_point(D, C, [&](int v, double r) { stage_emit(st, q + v * L.vstride, r); });
-  }
-}
-
-template <int TX, int TY, int TZ>
 __global__ void __launch_bounds__(TX* TY) bssn_derivs_kernel(Layout L, Coef C, const double* __restrict__ in,
                                                             double* __restrict__ derivs) {
   const int i = blockIdx.x * TX + threadIdx.x, j = blockIdx.y * TY + threadIdx.y;
@@ -121,16 +106,12 @@ __global__ void __launch_bounds__(TX* TY) bssn_from_derivs_kernel(Layout L, Coef
   }
 }
 
-// which: 0 fused, 1 derivs, 2 from_derivs
+// which: 1 derivs, 2 from_derivs
 template <int TX, int TY, int TZ>
 static cudaError_t bssn_go(int which, const Layout& L, const Coef& C, const Stage* st, const double* in,
                            double* derivs, cudaStream_t s, cudaFuncAttributes* a) {
   dim3 grid((L.nx + TX - 1) / TX, (L.ny + TY - 1) / TY, (L.nz + TZ - 1) / TZ), block(TX, TY);
-  if (which == 0) {
-    auto kern = bssn_fused_kernel<TX, TY, TZ>;
-    if (a) return cudaFuncGetAttributes(a, kern);
-    kern<<<grid, block, 0, s>>>(L, C, *st);
-  } else if (which == 1) {
+  if (which == 1) {
     auto kern = bssn_derivs_kernel<TX, TY, TZ>;
     if (a) return cudaFuncGetAttributes(a, kern);
     kern<<<grid, block, 0, s>>>(L, C, in, derivs);
@@ -155,9 +136,6 @@ static cudaError_t bssn_dispatch(int which, int tile, const Layout& L, const Coe
   return cudaErrorInvalidValue;
 }
 
-cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int tile, const Stage& st, cudaStream_t s) {
-  return bssn_dispatch(0, tile, L, C, &st, nullptr, nullptr, s, nullptr);
-}
 cudaError_t launch_bssn_derivs(const Layout& L, const Coef& C, int tile, const double* in, double* derivs,
                                cudaStream_t s) {
   return bssn_dispatch(1, tile, L, C, nullptr, in, derivs, s, nullptr);
@@ -166,9 +144,9 @@ cudaError_t launch_bssn_from_derivs(const Layout& L, const Coef& C, int tile, co
                                     cudaStream_t s) {
   return bssn_dispatch(2, tile, L, C, &st, nullptr, const_cast<double*>(derivs), s, nullptr);
 }
-cudaError_t kernel_info_bssn(int fused, int tile, cudaFuncAttributes* a) {
+cudaError_t kernel_info_bssn_split(int which, int tile, cudaFuncAttributes* a) {
   Layout L{}; Coef C{};
-  return bssn_dispatch(fused ? 0 : 1, tile, L, C, nullptr, nullptr, nullptr, 0, a);
+  return bssn_dispatch(which, tile, L, C, nullptr, nullptr, nullptr, 0, a);
 }
 
 }  // namespace chm

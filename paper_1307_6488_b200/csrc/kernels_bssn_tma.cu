@@ -1,0 +1,414 @@
+// kernels_bssn_tma.cu -- the fused BSSN kernel (derivatives + RHS + RK4 stage update), sm_100a:
+// persistent CTAs, TMA-staged per-variable boxes in a 5-slot mbarrier ring, compile-time stencil offsets.
+// See bssn_tma.cuh for the design; DESIGN.md "Kernels" for the roofline that bounds it.
+#include "bssn_tma.cuh"
+
+namespace chm {
+
+constexpr int kSlots = 5;   // 25 variables % 5 == 0: the slot of a variable is the same in every tile
+
+template <int TX, int TY, int TZ>
+struct TmaCfg {
+  static constexpr int BX = TX + 6, BY = TY + 6, BZ = TZ + 6;
+  static constexpr int SLOT = (BX * BY * BZ + 15) / 16 * 16;          // doubles, 128-byte multiple
+  static constexpr uint32_t BOX_BYTES = (uint32_t)BX * BY * BZ * 8u;
+  static constexpr size_t SMEM = (size_t)kSlots * SLOT * 8 + kSlots * 8 + 128;
+  static constexpr int THREADS = TX * TY * TZ;
+};
+
+template <int TX, int TY, int TZ>
+__global__ void __launch_bounds__(TX* TY* TZ, 1)
+bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage st, int ntx, int nty, int ntiles) {
+  using Cfg = TmaCfg<TX, TY, TZ>;
+  constexpr int BX = Cfg::BX, BY = Cfg::BY, SLOT = Cfg::SLOT;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double* sm = reinterpret_cast<double*>(smem_raw);   // dynamic smem base: 128-byte aligned (no static smem)
+  uint64_t* full = reinterpret_cast<uint64_t*>(sm + kSlots * SLOT);
+
+  const int tid = threadIdx.x;
+  const int lx = tid % TX, ly = (tid / TX) % TY, lz = tid / (TX * TY);
+  const int coff = ((lz + 3) * BY + (ly + 3)) * BX + lx + 3;
+  const int goff = L.g - 3;   // box origin relative to the tile origin, padded coordinates
+
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < kSlots; ++s) mbar_init(&full[s], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+
+  // producer (thread 0): box of variable order o of the tile whose origin (padded, minus halo) is (x0,y0,z0)
+  auto issue = [&](int o, int x0, int y0, int z0) {
+    const int slot = o % kSlots;
+    mbar_expect_tx(&full[slot], Cfg::BOX_BYTES);
+    tma_load_4d(sm + slot * SLOT, &tm, &full[slot], x0, y0, z0, order_var(o));
+  };
+  auto origin = [&](int tile, int& x0, int& y0, int& z0) {
+    const int bz = tile / (ntx * nty), rem = tile - bz * ntx * nty, by = rem / ntx, bx = rem - by * ntx;
+    x0 = bx * TX + goff; y0 = by * TY + goff; z0 = bz * TZ + goff;
+  };
+  if (tid == 0 && (int)blockIdx.x < ntiles) {
+    int x0, y0, z0;
+    origin(blockIdx.x, x0, y0, z0);
+#pragma unroll
+    for (int o = 0; o < kSlots; ++o) issue(o, x0, y0, z0);
+  }
+
+  int t = 0;
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++t) {
+    const int bz = tile / (ntx * nty), rem = tile - bz * ntx * nty, by = rem / ntx, bx = rem - by * ntx;
+    const int i = bx * TX + lx, j = by * TY + ly, k = bz * TZ + lz;
+    const bool valid = i < L.nx && j < L.ny && k < L.nz;
+    const long q = (long)((valid ? k : 0) + L.g) * L.plane + (long)((valid ? j : 0) + L.g) * L.pitch +
+                   ((valid ? i : 0) + L.g);
+    const double* __restrict__ in = st.in + q;
+    auto cen = [&](int v) { return __ldg(in + v * L.vstride); };
+    // RK4 stage operands of variable v, fetched at the START of the section that will emit v so that their
+    // DRAM latency hides behind the section's stencil work
+    auto pre = [&](int v) {
+      StagePre r{0.0, 0.0};
+      if (valid) stage_prefetch(st, q + v * L.vstride, r);
+      return r;
+    };
+    auto emit = [&](int v, double k, const StagePre& pr) { if (valid) stage_emit(st, q + v * L.vstride, k, pr); };
+
+    // section o: wait for its box, hand out the accessor; done(o): release the slot, prefetch 5 loads ahead
+    auto box = [&](int o) {
+      mbar_wait(&full[o % kSlots], (uint32_t)((t + o / kSlots) & 1));
+      return BoxPoint<BX, BY>{sm + (o % kSlots) * SLOT + coff};
+    };
+    int nx0 = 0, ny0 = 0, nz0 = 0;           // next tile of this CTA (thread 0 prefetches its first 5 boxes)
+    const bool has_next = tile + (int)gridDim.x < ntiles;
+    if (tid == 0 && has_next) origin(tile + gridDim.x, nx0, ny0, nz0);
+    auto done = [&](int o) {
+      __syncthreads();
+      if (tid == 0) {
+        if (o + kSlots < 25) issue(o + kSlots, bx * TX + goff, by * TY + goff, bz * TZ + goff);
+        else if (has_next) issue(o + kSlots - 25, nx0, ny0, nz0);
+      }
+    };
+
+    const double third = 1.0 / 3.0, two_thirds = 2.0 / 3.0;
+    // ---- point values needed before their own boxes arrive: metric, shift ----------------------------------
+    double g[6], gu[6];
+#pragma unroll
+    for (int s = 0; s < 6; ++s) g[s] = cen(V_GT + s);
+    {
+      const double c00 = g[3] * g[5] - g[4] * g[4], c01 = g[2] * g[4] - g[1] * g[5], c02 = g[1] * g[4] - g[2] * g[3];
+      const double idet = 1.0 / (g[0] * c00 + g[1] * c01 + g[2] * c02);
+      gu[0] = c00 * idet; gu[1] = c01 * idet; gu[2] = c02 * idet;
+      gu[3] = (g[0] * g[5] - g[2] * g[2]) * idet;
+      gu[4] = (g[1] * g[2] - g[0] * g[4]) * idet;
+      gu[5] = (g[0] * g[3] - g[1] * g[1]) * idet;
+    }
+    AdvW w;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      const double b = cen(V_BETA + a);
+      w.ws[a] = b * (C.inv_h * (1.0 / 24.0));
+      w.wq[a] = fabs(b) * (C.inv_h * (1.0 / 24.0)) + C.ko;
+    }
+    const double alpha = cen(V_ALPHA), trK = cen(V_K), chi = cen(V_CHI);
+
+    // ---- o = 0..2: beta^i : d_j beta^i, gtu^{jk} d_j d_k beta^i, d_j (d_k beta^k) ----------------------------
+    double db[3][3], lapb[3], gdiv[3] = {0.0, 0.0, 0.0};   // db[j][i] = d_j beta^i ; gdiv[j] = d_j d_k beta^k
+#pragma unroll
+    for (int i2 = 0; i2 < 3; ++i2) {
+      const StagePre pr = pre(V_BETA + i2);
+      const double Bc = cen(V_B + i2);
+      auto p = box(i2);
+      double d1[3], d2[6], ad;
+      var_full(p, C, w, d1, d2, ad);
+      done(i2);
+#pragma unroll
+      for (int a = 0; a < 3; ++a) { db[a][i2] = d1[a]; gdiv[a] += d2[sym(a, i2)]; }
+      lapb[i2] = sdot(gu, d2);
+      emit(V_BETA + i2, C.sgc * Bc + ad, pr);
+    }
+    const double divb = (db[0][0] + db[1][1]) + db[2][2];
+
+    // ---- o = 3..8: gt_ij : d_k gt_ij kept for the Christoffels, gtu^{lm} d_l d_m gt_ij folded into R~_ij ---
+    double At[6], Rt[6], dg[3][6];
+#pragma unroll
+    for (int s = 0; s < 6; ++s) At[s] = cen(V_AT + s);
+#pragma unroll
+    for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+      for (int j2 = i2; j2 < 3; ++j2) {
+        const int s = sym(i2, j2);
+        const StagePre pr = pre(V_GT + s);
+        auto p = box(3 + s);
+        double d1[3], d2[6], ad;
+        var_full(p, C, w, d1, d2, ad);
+        done(3 + s);
+        dg[0][s] = d1[0]; dg[1][s] = d1[1]; dg[2][s] = d1[2];
+        Rt[s] = -0.5 * sdot(gu, d2);
+        double lie = 0.0;
+#pragma unroll
+        for (int k2 = 0; k2 < 3; ++k2) lie += g[sym(i2, k2)] * db[j2][k2] + g[sym(j2, k2)] * db[i2][k2];
+        emit(V_GT + s, (lie - two_thirds * g[s] * divb) - 2.0 * alpha * At[s] + ad, pr);
+      }
+
+    // ---- Christoffels: Cl[k][s(i,j)] = Gamma~_kij, Cu[k][s] = Gamma~^k_ij, Gn[k] = gtu^{ij} Gamma~^k_ij ----
+    double Cu[3][6], Gn[3];
+    {
+      double Cl[3][6];
+#pragma unroll
+      for (int k2 = 0; k2 < 3; ++k2)
+#pragma unroll
+        for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+          for (int j2 = i2; j2 < 3; ++j2)
+            Cl[k2][sym(i2, j2)] = 0.5 * ((dg[i2][sym(k2, j2)] + dg[j2][sym(k2, i2)]) - dg[k2][sym(i2, j2)]);
+#pragma unroll
+      for (int k2 = 0; k2 < 3; ++k2) {
+#pragma unroll
+        for (int s = 0; s < 6; ++s)
+          Cu[k2][s] = gu[sym(k2, 0)] * Cl[0][s] + gu[sym(k2, 1)] * Cl[1][s] + gu[sym(k2, 2)] * Cl[2][s];
+        Gn[k2] = sdot(gu, Cu[k2]);
+      }
+      // R~_ij += 1/2 Gamma~^k_n (Gamma~_ijk + Gamma~_jik)
+      //        + gtu^{lm} (Gamma~^k_li Gamma~_jkm + Gamma~^k_lj Gamma~_ikm + Gamma~^k_im Gamma~_klj)
+#pragma unroll
+      for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+        for (int j2 = i2; j2 < 3; ++j2) {
+          double acc = 0.0;
+#pragma unroll
+          for (int k2 = 0; k2 < 3; ++k2) acc += Gn[k2] * (Cl[i2][sym(j2, k2)] + Cl[j2][sym(i2, k2)]);
+          acc *= 0.5;
+#pragma unroll
+          for (int l = 0; l < 3; ++l)
+#pragma unroll
+            for (int m = 0; m < 3; ++m) {
+              double qq = 0.0;
+#pragma unroll
+              for (int k2 = 0; k2 < 3; ++k2)
+                qq += Cu[k2][sym(l, i2)] * Cl[j2][sym(k2, m)] + Cu[k2][sym(l, j2)] * Cl[i2][sym(k2, m)] +
+                      Cu[k2][sym(i2, m)] * Cl[k2][sym(l, j2)];
+              acc += gu[sym(l, m)] * qq;
+            }
+          Rt[sym(i2, j2)] += acc;
+        }
+    }
+
+    // ---- o = 9..11: Gt^k : R~_ij += 1/2 (gt_ki d_j Gt^k + gt_kj d_i Gt^k); advection kept for the end ------
+    double adG[3];
+#pragma unroll
+    for (int k2 = 0; k2 < 3; ++k2) {
+      auto p = box(9 + k2);
+      double d1[3];
+      var_d1_ad(p, C, w, d1, adG[k2]);
+      done(9 + k2);
+#pragma unroll
+      for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+        for (int j2 = i2; j2 < 3; ++j2)
+          Rt[sym(i2, j2)] += 0.5 * (g[sym(k2, i2)] * d1[j2] + g[sym(k2, j2)] * d1[i2]);
+    }
+
+    // ---- o = 12: chi : R_ij = R~_ij + R^chi_ij --------------------------------------------------------------
+    const double ichi = 1.0 / chi;
+    double dchi[3];
+    {
+      const StagePre pr = pre(V_CHI);
+      auto p = box(12);
+      double d2[6], ad;
+      var_full(p, C, w, dchi, d2, ad);
+      done(12);
+      emit(V_CHI, two_thirds * chi * (alpha * trK - divb) + ad, pr);
+      double cd[6], cc[6];   // D~_i D~_j chi ; d_i chi d_j chi
+#pragma unroll
+      for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = a; b < 3; ++b) {
+          const int s = sym(a, b);
+          cd[s] = d2[s] - (Cu[0][s] * dchi[0] + Cu[1][s] * dchi[1] + Cu[2][s] * dchi[2]);
+          cc[s] = dchi[a] * dchi[b];
+        }
+      const double trcd = sdot(gu, cd), trcc = sdot(gu, cc);
+      const double h2 = 0.5 * ichi, h4 = 0.25 * ichi * ichi;
+#pragma unroll
+      for (int s = 0; s < 6; ++s) Rt[s] += h2 * (cd[s] + g[s] * trcd) - h4 * (cc[s] + 3.0 * g[s] * trcc);
+    }
+
+    // ---- o = 13: alpha : X_ij = alpha R_ij - D_i D_j alpha ; D^2 alpha -----------------------------------------
+    double dal[3], lap_alpha;
+    {
+      const StagePre pr = pre(V_ALPHA);
+      auto p = box(13);
+      double d2[6], ad;
+      var_full(p, C, w, dal, d2, ad);
+      done(13);
+      emit(V_ALPHA, -2.0 * alpha * trK + ad, pr);
+      double cd[6], ca[6];   // d_i d_j alpha - Gamma~^k_ij d_k alpha ; d_i chi d_j alpha + d_j chi d_i alpha
+#pragma unroll
+      for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = a; b < 3; ++b) {
+          const int s = sym(a, b);
+          cd[s] = d2[s] - (Cu[0][s] * dal[0] + Cu[1][s] * dal[1] + Cu[2][s] * dal[2]);
+          ca[s] = dchi[a] * dal[b] + dchi[b] * dal[a];
+        }
+      const double trcd = sdot(gu, cd), trca = 0.5 * sdot(gu, ca);   // trca = gtu^{kl} d_k chi d_l alpha
+      lap_alpha = chi * trcd - 0.5 * trca;
+      const double h2 = 0.5 * ichi;
+#pragma unroll
+      for (int s = 0; s < 6; ++s) Rt[s] = alpha * Rt[s] - (cd[s] + h2 * (ca[s] - g[s] * trca));   // Rt now holds X_ij
+    }
+
+    // ---- extrinsic curvature with raised indices -------------------------------------------------------------
+    double Am[3][3], Au[6];   // At^i_j ; At^{ij}
+#pragma unroll
+    for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+      for (int j2 = 0; j2 < 3; ++j2)
+        Am[i2][j2] = gu[sym(i2, 0)] * At[sym(0, j2)] + gu[sym(i2, 1)] * At[sym(1, j2)] + gu[sym(i2, 2)] * At[sym(2, j2)];
+#pragma unroll
+    for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+      for (int j2 = i2; j2 < 3; ++j2)
+        Au[sym(i2, j2)] = Am[i2][0] * gu[sym(0, j2)] + Am[i2][1] * gu[sym(1, j2)] + Am[i2][2] * gu[sym(2, j2)];
+
+    // ---- o = 14: K -------------------------------------------------------------------------------------------
+    double dK[3];
+    {
+      const StagePre pr = pre(V_K);
+      auto p = box(14);
+      double ad;
+      var_d1_ad(p, C, w, dK, ad);
+      done(14);
+      emit(V_K, (alpha * (sdot(Au, At) + third * trK * trK) - lap_alpha) + ad, pr);
+    }
+
+    // ---- o = 15..20: At_ij -------------------------------------------------------------------------------------
+    {
+      const double trX = sdot(gu, Rt);
+#pragma unroll
+      for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+        for (int j2 = i2; j2 < 3; ++j2) {
+          const int s = sym(i2, j2);
+          const StagePre pr = pre(V_AT + s);
+          auto p = box(15 + s);
+          const double ad = var_ad(p, w);
+          done(15 + s);
+          double AA = 0.0, lie = 0.0;
+#pragma unroll
+          for (int k2 = 0; k2 < 3; ++k2) {
+            AA += At[sym(i2, k2)] * Am[k2][j2];
+            lie += At[sym(i2, k2)] * db[j2][k2] + At[sym(j2, k2)] * db[i2][k2];
+          }
+          emit(V_AT + s, chi * (Rt[s] - third * g[s] * trX) + alpha * (trK * At[s] - 2.0 * AA) +
+                             (lie - two_thirds * At[s] * divb) + ad, pr);
+        }
+    }
+
+    // ---- o = 21..23: B^i, together with Gt^i ---------------------------------------------------------------------
+#pragma unroll
+    for (int i2 = 0; i2 < 3; ++i2) {
+      const StagePre prG = pre(V_GAM + i2), prB = pre(V_B + i2);
+      auto p = box(21 + i2);
+      const double Bi = p.at(0, 0, 0);
+      const double adB = var_ad(p, w);
+      done(21 + i2);
+      double r = lapb[i2];
+      double t2 = sdot(Cu[i2], Au);   // Gamma~^i_jk At^{jk}
+#pragma unroll
+      for (int j2 = 0; j2 < 3; ++j2) {
+        r += third * gu[sym(i2, j2)] * gdiv[j2];
+        t2 -= two_thirds * gu[sym(i2, j2)] * dK[j2] + 1.5 * ichi * Au[sym(i2, j2)] * dchi[j2];
+        r -= 2.0 * Au[sym(i2, j2)] * dal[j2] + Gn[j2] * db[j2][i2];
+      }
+      r += 2.0 * alpha * t2 + two_thirds * Gn[i2] * divb;
+      emit(V_GAM + i2, r + adG[i2], prG);
+      emit(V_B + i2, (r - C.eta * Bi) + adB, prB);
+    }
+
+    // ---- o = 24: A (inert slot, dissipation only) -----------------------------------------------------------------
+    {
+      const StagePre pr = pre(V_A);
+      auto p = box(24);
+      const double f0 = p.at(0, 0, 0);
+      const double qsum = (axis_q(p, f0, 0) + axis_q(p, f0, 1)) + axis_q(p, f0, 2);
+      done(24);
+      emit(V_A, C.ko * qsum, pr);
+    }
+  }
+}
+
+// ---- host side: tensor map + launch -----------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  }
+  return fn;
+}
+
+template <int TX, int TY, int TZ>
+static cudaError_t tma_go(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
+  using Cfg = TmaCfg<TX, TY, TZ>;
+  auto kern = bssn_tma_kernel<TX, TY, TZ>;
+  if (a) return cudaFuncGetAttributes(a, kern);
+  EncodeTiledFn enc = encode_fn();
+  if (!enc) return cudaErrorNotSupported;
+  CUtensorMap tm;
+  cuuint64_t dims[4] = {(cuuint64_t)L.pitch, (cuuint64_t)L.tot_y, (cuuint64_t)L.tot_z, (cuuint64_t)L.nvars};
+  cuuint64_t strides[3] = {(cuuint64_t)L.pitch * 8, (cuuint64_t)L.plane * 8, (cuuint64_t)L.vstride * 8};
+  cuuint32_t box[4] = {(cuuint32_t)Cfg::BX, (cuuint32_t)Cfg::BY, (cuuint32_t)Cfg::BZ, 1};
+  cuuint32_t estr[4] = {1, 1, 1, 1};
+  CUresult r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(st->in), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  int dev = 0, sms = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int ntx = (L.nx + TX - 1) / TX, nty = (L.ny + TY - 1) / TY, ntz = (L.nz + TZ - 1) / TZ;
+  const int ntiles = ntx * nty * ntz;
+  int blocks_per_sm = 1;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, Cfg::THREADS, Cfg::SMEM);
+  if (blocks_per_sm < 1) blocks_per_sm = 1;
+  const int grid = ntiles < sms * blocks_per_sm ? ntiles : sms * blocks_per_sm;
+  kern<<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, L, C, *st, ntx, nty, ntiles);
+  return cudaGetLastError();
+}
+
+static cudaError_t tma_dispatch(int tile, const Layout& L, const Coef& C, const Stage* st, cudaStream_t s,
+                                cudaFuncAttributes* a) {
+  switch (tile) {
+    case 0: return tma_go<16, 4, 4>(L, C, st, s, a);
+    case 1: return tma_go<16, 8, 2>(L, C, st, s, a);
+    case 2: return tma_go<32, 4, 2>(L, C, st, s, a);
+    case 3: return tma_go<32, 2, 4>(L, C, st, s, a);
+    case 4: return tma_go<8, 8, 4>(L, C, st, s, a);
+    case 5: return tma_go<16, 4, 2>(L, C, st, s, a);
+  }
+  return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int tile, const Stage& st, cudaStream_t s) {
+  return tma_dispatch(tile, L, C, &st, s, nullptr);
+}
+cudaError_t kernel_info_bssn_fused(int tile, cudaFuncAttributes* a) {
+  Layout L{}; Coef C{};
+  return tma_dispatch(tile, L, C, nullptr, 0, a);
+}
+
+}  // namespace chm

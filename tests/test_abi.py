@@ -28,8 +28,10 @@ def test_exports_every_declared_symbol(binding):
 
 
 def test_tile_table(binding):
-    shapes = [binding.tile_shape(t) for t in range(binding.NUM_TILES)]
+    shapes = [binding.tile_shape(t, binding.SYS_BSSN, 0) for t in range(binding.NUM_TILES)]
     assert shapes == [(32, 4, 8), (32, 8, 8), (64, 2, 8), (64, 4, 8), (128, 2, 8), (16, 16, 8)]
+    fused = [binding.tile_shape(t, binding.SYS_BSSN, 1) for t in range(binding.NUM_TILES)]
+    assert all(x * y * z in (128, 256) for x, y, z in fused)      # one grid point per thread
     with pytest.raises(binding.ChemoraError):
         binding.tile_shape(6)
 
