@@ -14,9 +14,11 @@
  *    creation and is asynchronous with respect to the host unless stated otherwise.
  *  - "dev" pointers are CUDA device pointers, "host" pointers ordinary host memory.
  *  - Device state layout (SoA): V variables; each variable is tot_z x tot_y rows of
- *    `pitch` doubles (pitch = roundup(nx + 2g, 16): 128-byte rows), x fastest; variable stride
+ *    `pitch` doubles (pitch = roundup(xo + nx + g, 16): 128-byte rows), x fastest; variable stride
  *    var_stride = pitch*tot_y*tot_z; buffers are 128-byte aligned.  Interior point (i,j,k) of variable v is
- *    at  v*var_stride + ((k+g)*tot_y + (j+g))*pitch + (i+g).
+ *    at  v*var_stride + ((k+g)*tot_y + (j+g))*pitch + (i+xo), where xo = g except for BSSN with even g,
+ *    where xo = g+1 (keeps the fused kernel's TMA halo boxes 16-byte aligned).  Always take the offsets
+ *    from chemora_layout (interior_offset = (g*tot_y + g)*pitch + xo).
  *  - Packed host layout: V x nz x ny x nx doubles, x fastest, no ghosts.
  *  - There is no CPU fallback: every entry point that computes needs a CUDA device and fails with
  *    CHEMORA_ECUDA otherwise.

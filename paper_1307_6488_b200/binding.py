@@ -127,6 +127,7 @@ class Chemora:
         self._ck(self.lib.chemora_layout(self._h, nv, pitch, ty, tz, vs, io))
         self.nvars, self.pitch, self.tot_y, self.tot_z = nv.value, pitch.value, ty.value, tz.value
         self.var_stride, self.interior_offset = vs.value, io.value
+        self.xoff = self.interior_offset % self.pitch      # x index of interior point 0 inside a row
 
     # -- helpers -------------------------------------------------------------------------------------
     def _ck(self, rc):
@@ -157,8 +158,13 @@ class Chemora:
         return p.value
 
     def interior(self, padded):
-        g, (nx, ny, nz) = self.ghost, self.dims
-        return padded[:, g:g + nz, g:g + ny, g:g + nx]
+        g, xo, (nx, ny, nz) = self.ghost, self.xoff, self.dims
+        return padded[:, g:g + nz, g:g + ny, xo:xo + nx]
+
+    def ghosted(self, padded):
+        """the [V, nz+2g, ny+2g, nx+2g] part of a padded state (interior + ghosts, no row padding)"""
+        g, xo, nx = self.ghost, self.xoff, self.dims[0]
+        return padded[..., xo - g:xo + nx + g]
 
     # -- the C entry points ---------------------------------------------------------------------------
     def set_param(self, name, value):

@@ -158,7 +158,8 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
   Layout& L = h->L;
   L.nx = nx; L.ny = ny; L.nz = nz; L.g = ghost;
   L.nvars = system_id == CHEMORA_SYS_WAVE ? 2 : 25;
-  L.pitch = ((long)nx + 2 * ghost + 15) / 16 * 16;
+  L.xo = (system_id == CHEMORA_SYS_BSSN && ((ghost - 3) & 1)) ? ghost + 1 : ghost;
+  L.pitch = ((long)L.xo + nx + ghost + 15) / 16 * 16;
   L.tot_y = ny + 2 * ghost; L.tot_z = nz + 2 * ghost;
   L.plane = L.pitch * L.tot_y;
   L.vstride = L.plane * L.tot_z;
@@ -226,7 +227,7 @@ int chemora_layout(const chemora_t* h, int* nvars, long* pitch, long* tot_y, lon
   if (tot_y) *tot_y = h->L.tot_y;
   if (tot_z) *tot_z = h->L.tot_z;
   if (var_stride) *var_stride = h->L.vstride;
-  if (interior_offset) *interior_offset = (long)h->L.g * h->L.plane + (long)h->L.g * h->L.pitch + h->L.g;
+  if (interior_offset) *interior_offset = (long)h->L.g * h->L.plane + (long)h->L.g * h->L.pitch + h->L.xo;
   return CHEMORA_OK;
 }
 

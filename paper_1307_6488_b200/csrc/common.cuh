@@ -9,6 +9,8 @@ namespace chm {
 // Device-side view of the padded SoA layout (include/chemora.h "Conventions").
 struct Layout {
   int nx, ny, nz, g;     // interior dims, ghost width
+  int xo;                // x index of interior point 0 inside a row: g, or g+1 when that makes (xo - 3) even,
+                         // so that the fused BSSN kernel's TMA halo boxes start on a 16-byte boundary
   int nvars;
   long pitch;            // doubles per row, multiple of 16 (128-byte rows)
   long plane;            // pitch * tot_y
@@ -80,7 +82,7 @@ __device__ __forceinline__ void stage_emit(const Stage& st, long q, double k, co
 // Tile shapes of the variant sweep.  Fused kernel: 3-D tile, one point per thread.  Split kernels and the wave
 // kernel: x,y = thread block, z = planes marched per block.
 struct TileShape { int tx, ty, tz; };
-static const TileShape kTilesFused[6] = {{16, 4, 4}, {16, 8, 2}, {32, 4, 2}, {32, 2, 4}, {8, 8, 4}, {16, 4, 2}};
+static const TileShape kTilesFused[6] = {{16, 4, 4}, {16, 8, 2}, {8, 8, 4}, {8, 4, 8}, {16, 2, 8}, {16, 4, 2}};
 static const TileShape kTilesMarch[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64, 4, 8}, {128, 2, 8}, {16, 16, 8}};
 
 // launchers implemented in the kernel translation units; each returns the cudaError_t of the launch

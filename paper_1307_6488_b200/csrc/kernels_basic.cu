@@ -31,8 +31,9 @@ __global__ void __launch_bounds__(256) fill_ghosts_kernel(Layout L, double* __re
     k = kk + g; j = jj + g; i = ii < g ? ii : ii + L.nx;
   }
   auto wrap = [g](int c, int n) { int r = (c - g) % n; return (r < 0 ? r + n : r) + g; };
-  const long dst = (long)k * L.plane + (long)j * L.pitch + i;
-  const long src = (long)wrap(k, L.nz) * L.plane + (long)wrap(j, L.ny) * L.pitch + wrap(i, L.nx);
+  const int xs = L.xo - g;   // first ghost column of a row
+  const long dst = (long)k * L.plane + (long)j * L.pitch + i + xs;
+  const long src = (long)wrap(k, L.nz) * L.plane + (long)wrap(j, L.ny) * L.pitch + wrap(i, L.nx) + xs;
   double* p = state + (long)blockIdx.y * L.vstride;
   p[dst] = p[src];
 }
@@ -52,7 +53,7 @@ __global__ void __launch_bounds__(256) pack_kernel(Layout L, const double* __res
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= L.nx) return;
   int j = blockIdx.y, k = blockIdx.z % L.nz, v = blockIdx.z / L.nz;
-  long q = v * L.vstride + (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.g);
+  long q = v * L.vstride + (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.xo);
   long r = (((long)v * L.nz + k) * L.ny + j) * L.nx + i;
   if (to_state) dst[q] = src[r]; else dst[r] = src[q];
 }
@@ -77,7 +78,7 @@ __global__ void __launch_bounds__(TX* TY) wave_kernel(Layout L, Coef C, Stage st
   for (int kk = 0; kk < TZ; ++kk) {
     const int k = k0 + kk;
     if (k >= L.nz) break;
-    const long q = (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.g);
+    const long q = (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.xo);
     GlobalPoint P{st.in + q, L.pitch, L.plane, L.vstride};
     double lap;
     if (ORDER == 4) lap = (d2_o4(P, 0, 0, C.inv_h2) + d2_o4(P, 0, 1, C.inv_h2)) + d2_o4(P, 0, 2, C.inv_h2);

@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(TX* TY) bssn_derivs_kernel(Layout L, Coef C, c
   for (int kk = 0; kk < TZ; ++kk) {
     const int k = k0 + kk;
     if (k >= L.nz) break;
-    const long q = (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.g);
+    const long q = (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.xo);
     double* o = derivs + ((long)k * L.ny + j) * L.nx + i;
     OnTheFly<GlobalPoint> D{{in + q, L.pitch, L.plane, L.vstride}, C, {0, 0, 0}};
     D.beta[0] = D.f(V_BETA); D.beta[1] = D.f(V_BETA + 1); D.beta[2] = D.f(V_BETA + 2);
@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(TX* TY) bssn_from_derivs_kernel(Layout L, Coef
   for (int kk = 0; kk < TZ; ++kk) {
     const int k = k0 + kk;
     if (k >= L.nz) break;
-    const long q = (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.g);
+    const long q = (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.xo);
     FromArrays D{st.in + q, L.vstride, derivs + ((long)k * L.ny + j) * L.nx + i, n};
     bssn_point(D, C, [&](int v, double r) { stage_emit(st, q + v * L.vstride, r); });
   }

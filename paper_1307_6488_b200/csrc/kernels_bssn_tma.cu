@@ -6,33 +6,54 @@
 namespace chm {
 
 constexpr int kSlots = 5;   // 25 variables % 5 == 0: the slot of a variable is the same in every tile
+// point ("centre") values staged per tile: variables 0..13 (chi, gt, K, At) and 17..23 (alpha, beta, B)
+constexpr int kCenVars = 21;
+__device__ __forceinline__ constexpr int cen_index(int v) { return v < 14 ? v : v - 3; }
+// variables whose right-hand side leaves in section o (first, second; -1 = none)
+__device__ __forceinline__ constexpr int emit_var(int o, int n) {
+  return o < 9 ? (n == 0 ? order_var(o) : -1) : o < 12 ? -1 : o < 21 ? (n == 0 ? order_var(o) : -1)
+         : o < 24 ? (n == 0 ? V_GAM + (o - 21) : V_B + (o - 21)) : (n == 0 ? V_A : -1);
+}
 
 template <int TX, int TY, int TZ>
 struct TmaCfg {
+  static_assert(TX % 2 == 0 && ((TX + 2) * TY * TZ) % 16 == 0, "tile boxes must stay 128-byte aligned in smem");
   static constexpr int BX = TX + 6, BY = TY + 6, BZ = TZ + 6;
   static constexpr int SLOT = (BX * BY * BZ + 15) / 16 * 16;          // doubles, 128-byte multiple
   static constexpr uint32_t BOX_BYTES = (uint32_t)BX * BY * BZ * 8u;
-  static constexpr size_t SMEM = (size_t)kSlots * SLOT * 8 + kSlots * 8 + 128;
   static constexpr int THREADS = TX * TY * TZ;
+  static constexpr int TILE = (TX + 2) * TY * TZ;                      // doubles in one (TX+2,TY,TZ) tile box
+  static constexpr uint32_t TILE_BYTES = (uint32_t)TILE * 8u;
+  static constexpr int SLOTX = SLOT + 4 * TILE;   // box + RK4 operands (U,S) of up to two emitted variables
+  static constexpr int CEN = kCenVars * TILE;     // point values needed ahead of their own boxes
+  static constexpr size_t SMEM = (size_t)(kSlots * SLOTX + CEN) * 8 + (kSlots + 1) * 8 + 128;
 };
 
 template <int TX, int TY, int TZ>
 __global__ void __launch_bounds__(TX* TY* TZ, 1)
-bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage st, int ntx, int nty, int ntiles) {
+bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ CUtensorMap tmCen,
+                const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS, Layout L, Coef C,
+                Stage st, int ntx, int nty, int ntiles) {
   using Cfg = TmaCfg<TX, TY, TZ>;
-  constexpr int BX = Cfg::BX, BY = Cfg::BY, SLOT = Cfg::SLOT;
+  constexpr int BX = Cfg::BX, BY = Cfg::BY, SLOT = Cfg::SLOT, SLOTX = Cfg::SLOTX, TILE = Cfg::TILE, CEN = Cfg::CEN;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double* sm = reinterpret_cast<double*>(smem_raw);   // dynamic smem base: 128-byte aligned (no static smem)
-  uint64_t* full = reinterpret_cast<uint64_t*>(sm + kSlots * SLOT);
+  double* cbuf = sm + kSlots * SLOTX;                                  // [kCenVars][TILE]
+  uint64_t* full = reinterpret_cast<uint64_t*>(cbuf + CEN);            // [kSlots] boxes, then [1] point values
+  uint64_t* cfull = full + kSlots;
+  const int nops = st.mode == MODE_RHS ? 0 : (st.mode == MODE_FIRST ? 1 : 2);   // RK4 operands per emitted var
 
   const int tid = threadIdx.x;
   const int lx = tid % TX, ly = (tid / TX) % TY, lz = tid / (TX * TY);
   const int coff = ((lz + 3) * BY + (ly + 3)) * BX + lx + 3;
-  const int goff = L.g - 3;   // box origin relative to the tile origin, padded coordinates
+  // halo-box origin relative to the tile origin in padded coordinates.  TMA needs every row of a box to start
+  // on a 16-byte boundary: the layout makes L.xo - 3 even, and the (TX,TY,TZ) tile boxes (point values, RK4
+  // operands) are loaded two columns wider, from x0 + 2, and read at column + 1.
+  const int goffx = L.xo - 3, goff = L.g - 3;
 
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < kSlots; ++s) mbar_init(&full[s], 1);
+    for (int s = 0; s < kSlots + 1; ++s) mbar_init(&full[s], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
@@ -41,16 +62,31 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
   // producer (thread 0): box of variable order o of the tile whose origin (padded, minus halo) is (x0,y0,z0)
   auto issue = [&](int o, int x0, int y0, int z0) {
     const int slot = o % kSlots;
-    mbar_expect_tx(&full[slot], Cfg::BOX_BYTES);
-    tma_load_4d(sm + slot * SLOT, &tm, &full[slot], x0, y0, z0, order_var(o));
+    double* dst = sm + slot * SLOTX;
+    const int v0 = emit_var(o, 0), v1 = emit_var(o, 1);
+    const int nem = (v0 >= 0) + (v1 >= 0);
+    mbar_expect_tx(&full[slot], Cfg::BOX_BYTES + (uint32_t)(nops * nem) * Cfg::TILE_BYTES);
+    tma_load_4d(dst, &tm, &full[slot], x0, y0, z0, order_var(o));
+    if (v0 >= 0 && nops >= 1) tma_load_4d(dst + SLOT, &tmU, &full[slot], x0 + 2, y0 + 3, z0 + 3, v0);
+    if (v0 >= 0 && nops == 2) tma_load_4d(dst + SLOT + TILE, &tmS, &full[slot], x0 + 2, y0 + 3, z0 + 3, v0);
+    if (v1 >= 0 && nops >= 1) tma_load_4d(dst + SLOT + 2 * TILE, &tmU, &full[slot], x0 + 2, y0 + 3, z0 + 3, v1);
+    if (v1 >= 0 && nops == 2) tma_load_4d(dst + SLOT + 3 * TILE, &tmS, &full[slot], x0 + 2, y0 + 3, z0 + 3, v1);
+  };
+  // point values of tile number tt of this CTA (three 7-variable boxes: vars 0..6, 7..13, 17..23)
+  auto issue_cen = [&](int x0, int y0, int z0) {
+    mbar_expect_tx(cfull, (uint32_t)kCenVars * Cfg::TILE_BYTES);
+    tma_load_4d(cbuf, &tmCen, cfull, x0 + 2, y0 + 3, z0 + 3, 0);
+    tma_load_4d(cbuf + 7 * TILE, &tmCen, cfull, x0 + 2, y0 + 3, z0 + 3, 7);
+    tma_load_4d(cbuf + 14 * TILE, &tmCen, cfull, x0 + 2, y0 + 3, z0 + 3, 17);
   };
   auto origin = [&](int tile, int& x0, int& y0, int& z0) {
     const int bz = tile / (ntx * nty), rem = tile - bz * ntx * nty, by = rem / ntx, bx = rem - by * ntx;
-    x0 = bx * TX + goff; y0 = by * TY + goff; z0 = bz * TZ + goff;
+    x0 = bx * TX + goffx; y0 = by * TY + goff; z0 = bz * TZ + goff;
   };
   if (tid == 0 && (int)blockIdx.x < ntiles) {
     int x0, y0, z0;
     origin(blockIdx.x, x0, y0, z0);
+    issue_cen(x0, y0, z0);
 #pragma unroll
     for (int o = 0; o < kSlots; ++o) issue(o, x0, y0, z0);
   }
@@ -61,22 +97,22 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
     const int i = bx * TX + lx, j = by * TY + ly, k = bz * TZ + lz;
     const bool valid = i < L.nx && j < L.ny && k < L.nz;
     const long q = (long)((valid ? k : 0) + L.g) * L.plane + (long)((valid ? j : 0) + L.g) * L.pitch +
-                   ((valid ? i : 0) + L.g);
-    const double* __restrict__ in = st.in + q;
-    auto cen = [&](int v) { return __ldg(in + v * L.vstride); };
-    // RK4 stage operands of variable v, fetched at the START of the section that will emit v so that their
-    // DRAM latency hides behind the section's stencil work
-    auto pre = [&](int v) {
-      StagePre r{0.0, 0.0};
-      if (valid) stage_prefetch(st, q + v * L.vstride, r);
-      return r;
+                   ((valid ? i : 0) + L.xo);
+    const int toff = (lz * TY + ly) * (TX + 2) + lx + 1;   // this thread's point inside a tile box
+    const double* cb = cbuf + toff;
+    auto cen = [&](int v) { return cb[cen_index(v) * TILE]; };
+    // RK4 stage operands (U, S) of the n-th variable emitted by section o: staged by TMA next to the box;
+    // read after box(o) and before done(o)
+    auto pre = [&](int o, int n) {
+      const double* op = sm + (o % kSlots) * SLOTX + SLOT + 2 * n * TILE + toff;
+      return StagePre{op[0], op[TILE]};
     };
     auto emit = [&](int v, double k, const StagePre& pr) { if (valid) stage_emit(st, q + v * L.vstride, k, pr); };
 
     // section o: wait for its box, hand out the accessor; done(o): release the slot, prefetch 5 loads ahead
     auto box = [&](int o) {
       mbar_wait(&full[o % kSlots], (uint32_t)((t + o / kSlots) & 1));
-      return BoxPoint<BX, BY>{sm + (o % kSlots) * SLOT + coff};
+      return BoxPoint<BX, BY>{sm + (o % kSlots) * SLOTX + coff};
     };
     int nx0 = 0, ny0 = 0, nz0 = 0;           // next tile of this CTA (thread 0 prefetches its first 5 boxes)
     const bool has_next = tile + (int)gridDim.x < ntiles;
@@ -84,12 +120,15 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
     auto done = [&](int o) {
       __syncthreads();
       if (tid == 0) {
-        if (o + kSlots < 25) issue(o + kSlots, bx * TX + goff, by * TY + goff, bz * TZ + goff);
+        // the point values are last read at the top of section 3 (At): after section 5 the buffer is free
+        if (o == 5 && has_next) issue_cen(nx0, ny0, nz0);
+        if (o + kSlots < 25) issue(o + kSlots, bx * TX + goffx, by * TY + goff, bz * TZ + goff);
         else if (has_next) issue(o + kSlots - 25, nx0, ny0, nz0);
       }
     };
 
     const double third = 1.0 / 3.0, two_thirds = 2.0 / 3.0;
+    mbar_wait(cfull, (uint32_t)(t & 1));
     // ---- point values needed before their own boxes arrive: metric, shift ----------------------------------
     double g[6], gu[6];
 #pragma unroll
@@ -115,9 +154,9 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
     double db[3][3], lapb[3], gdiv[3] = {0.0, 0.0, 0.0};   // db[j][i] = d_j beta^i ; gdiv[j] = d_j d_k beta^k
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2) {
-      const StagePre pr = pre(V_BETA + i2);
       const double Bc = cen(V_B + i2);
       auto p = box(i2);
+      const StagePre pr = pre(i2, 0);
       double d1[3], d2[6], ad;
       var_full(p, C, w, d1, d2, ad);
       done(i2);
@@ -137,8 +176,8 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
 #pragma unroll
       for (int j2 = i2; j2 < 3; ++j2) {
         const int s = sym(i2, j2);
-        const StagePre pr = pre(V_GT + s);
         auto p = box(3 + s);
+        const StagePre pr = pre(3 + s, 0);
         double d1[3], d2[6], ad;
         var_full(p, C, w, d1, d2, ad);
         done(3 + s);
@@ -212,8 +251,8 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
     const double ichi = 1.0 / chi;
     double dchi[3];
     {
-      const StagePre pr = pre(V_CHI);
       auto p = box(12);
+      const StagePre pr = pre(12, 0);
       double d2[6], ad;
       var_full(p, C, w, dchi, d2, ad);
       done(12);
@@ -236,8 +275,8 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
     // ---- o = 13: alpha : X_ij = alpha R_ij - D_i D_j alpha ; D^2 alpha -----------------------------------------
     double dal[3], lap_alpha;
     {
-      const StagePre pr = pre(V_ALPHA);
       auto p = box(13);
+      const StagePre pr = pre(13, 0);
       double d2[6], ad;
       var_full(p, C, w, dal, d2, ad);
       done(13);
@@ -274,8 +313,8 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
     // ---- o = 14: K -------------------------------------------------------------------------------------------
     double dK[3];
     {
-      const StagePre pr = pre(V_K);
       auto p = box(14);
+      const StagePre pr = pre(14, 0);
       double ad;
       var_d1_ad(p, C, w, dK, ad);
       done(14);
@@ -290,8 +329,8 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
 #pragma unroll
         for (int j2 = i2; j2 < 3; ++j2) {
           const int s = sym(i2, j2);
-          const StagePre pr = pre(V_AT + s);
           auto p = box(15 + s);
+          const StagePre pr = pre(15 + s, 0);
           const double ad = var_ad(p, w);
           done(15 + s);
           double AA = 0.0, lie = 0.0;
@@ -308,8 +347,8 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
     // ---- o = 21..23: B^i, together with Gt^i ---------------------------------------------------------------------
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2) {
-      const StagePre prG = pre(V_GAM + i2), prB = pre(V_B + i2);
       auto p = box(21 + i2);
+      const StagePre prG = pre(21 + i2, 0), prB = pre(21 + i2, 1);
       const double Bi = p.at(0, 0, 0);
       const double adB = var_ad(p, w);
       done(21 + i2);
@@ -328,8 +367,8 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
 
     // ---- o = 24: A (inert slot, dissipation only) -----------------------------------------------------------------
     {
-      const StagePre pr = pre(V_A);
       auto p = box(24);
+      const StagePre pr = pre(24, 0);
       const double f0 = p.at(0, 0, 0);
       const double qsum = (axis_q(p, f0, 0) + axis_q(p, f0, 1)) + axis_q(p, f0, 2);
       done(24);
@@ -362,7 +401,7 @@ static cudaError_t tma_go(const Layout& L, const Coef& C, const Stage* st, cudaS
   if (a) return cudaFuncGetAttributes(a, kern);
   EncodeTiledFn enc = encode_fn();
   if (!enc) return cudaErrorNotSupported;
-  CUtensorMap tm;
+  CUtensorMap tm, tmCen, tmU, tmS;
   cuuint64_t dims[4] = {(cuuint64_t)L.pitch, (cuuint64_t)L.tot_y, (cuuint64_t)L.tot_z, (cuuint64_t)L.nvars};
   cuuint64_t strides[3] = {(cuuint64_t)L.pitch * 8, (cuuint64_t)L.plane * 8, (cuuint64_t)L.vstride * 8};
   cuuint32_t box[4] = {(cuuint32_t)Cfg::BX, (cuuint32_t)Cfg::BY, (cuuint32_t)Cfg::BZ, 1};
@@ -371,6 +410,18 @@ static cudaError_t tma_go(const Layout& L, const Coef& C, const Stage* st, cudaS
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  auto tile_map = [&](CUtensorMap* m, const double* base, int nv) {
+    cuuint32_t b[4] = {(cuuint32_t)(TX + 2), (cuuint32_t)TY, (cuuint32_t)TZ, (cuuint32_t)nv};
+    return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(base), dims, strides, b, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  };
+  // RK4 operands: MODE_FIRST reads U == in; MODE_MID / MODE_LAST read U and S; MODE_RHS none (maps unused)
+  const double* ubase = st->mode == MODE_FIRST || st->mode == MODE_RHS ? st->in : st->U;
+  const double* sbase = st->mode == MODE_MID || st->mode == MODE_LAST ? st->S : st->in;
+  if (tile_map(&tmCen, st->in, 7) != CUDA_SUCCESS || tile_map(&tmU, ubase, 1) != CUDA_SUCCESS ||
+      tile_map(&tmS, sbase, 1) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
@@ -386,7 +437,7 @@ static cudaError_t tma_go(const Layout& L, const Coef& C, const Stage* st, cudaS
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, Cfg::THREADS, Cfg::SMEM);
   if (blocks_per_sm < 1) blocks_per_sm = 1;
   const int grid = ntiles < sms * blocks_per_sm ? ntiles : sms * blocks_per_sm;
-  kern<<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, L, C, *st, ntx, nty, ntiles);
+  kern<<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, L, C, *st, ntx, nty, ntiles);
   return cudaGetLastError();
 }
 
@@ -395,9 +446,9 @@ static cudaError_t tma_dispatch(int tile, const Layout& L, const Coef& C, const 
   switch (tile) {
     case 0: return tma_go<16, 4, 4>(L, C, st, s, a);
     case 1: return tma_go<16, 8, 2>(L, C, st, s, a);
-    case 2: return tma_go<32, 4, 2>(L, C, st, s, a);
-    case 3: return tma_go<32, 2, 4>(L, C, st, s, a);
-    case 4: return tma_go<8, 8, 4>(L, C, st, s, a);
+    case 2: return tma_go<8, 8, 4>(L, C, st, s, a);
+    case 3: return tma_go<8, 4, 8>(L, C, st, s, a);
+    case 4: return tma_go<16, 2, 8>(L, C, st, s, a);
     case 5: return tma_go<16, 4, 2>(L, C, st, s, a);
   }
   return cudaErrorInvalidValue;

@@ -54,19 +54,19 @@ def oracle_rhs(oracle, system, packed, g, order, dx, **prm):
 
 # ------------------------------------------------------------------------------------------ ghost fill
 @pytest.mark.parametrize("dims,g,system", [((37, 21, 19), 3, 1), ((16, 16, 16), 2, 0), ((5, 4, 9), 4, 0),
-                                           ((3, 3, 3), 3, 1)])
+                                           ((3, 3, 3), 3, 1), ((9, 6, 7), 4, 1)])
 def test_fill_ghosts_bit_exact(chem, oracle, dims, g, system):
     nx, ny, nz = dims
     V = 2 if system == 0 else 25
     rng = np.random.default_rng(5)
     u = rng.standard_normal((V, nz, ny, nx))
-    h = chem.Chemora(nx, ny, nz, g, 8 if g == 4 else 4, system, 0.1)
+    h = chem.Chemora(nx, ny, nz, g, 8 if (g == 4 and system == 0) else 4, system, 0.1)
     st = to_padded(h, u)
     h.fill_ghosts(st)
-    got = st[..., : nx + 2 * g].cpu().numpy()
+    got = h.ghosted(st).cpu().numpy()
     want = oracle.fill_ghosts(oracle.with_ghosts(u, g), g)
     assert np.array_equal(got, want)
-    assert not st[..., nx + 2 * g:].any()       # row padding untouched
+    assert not st[..., h.xoff + nx + g:].any() and not st[..., : h.xoff - g].any()      # row padding untouched
     h.destroy()
 
 
@@ -154,6 +154,20 @@ def test_bssn_rhs_all_variants_and_tiles(chem, oracle, data):
             h.set_variant(fused, tile)
             got = gpu_rhs(h, u)
             assert relerr(got, want) < TOL_RHS, (fused, tile)
+    h.destroy()
+
+
+def test_bssn_even_ghost_width(chem, oracle):
+    """g = 4 with BSSN: the layout shifts the interior by one column (xo = g+1) to keep TMA rows aligned."""
+    nx, ny, nz, g = 21, 9, 10, 4
+    u = strong_field(nx, ny, nz, seed=22)
+    want = oracle_rhs(oracle, 1, u, g, 4, 0.05, eps_diss=0.1)
+    h = chem.Chemora(nx, ny, nz, g, 4, 1, 0.05)
+    assert h.xoff == g + 1
+    h.set_param("eps_diss", 0.1)
+    for fused in (1, 0):
+        h.set_variant(fused, 0)
+        assert relerr(gpu_rhs(h, u), want) < TOL_RHS, fused
     h.destroy()
 
 
