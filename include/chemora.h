@@ -63,7 +63,9 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
                    void* alloc_ctx);
 
 /* Named parameters: "eps_diss" (KO strength, default 0), "eta" (default 1), "shift_gamma_coeff"
- * (default 0.75).  Unknown name or invalid value -> CHEMORA_EINVAL. */
+ * (default 0.75); tuning: "col_rows" (default 32: y-extent in grid rows of the columns in which the fused BSSN
+ * kernel visits its tiles, chosen so the halo planes shared by z-neighbour tiles stay in L2).
+ * Unknown name or invalid value -> CHEMORA_EINVAL. */
 int chemora_set_param(chemora_t* h, const char* name, double value);
 int chemora_get_param(const chemora_t* h, const char* name, double* value);
 

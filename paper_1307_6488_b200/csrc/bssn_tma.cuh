@@ -41,6 +41,34 @@ __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, ui
       ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z), "r"(v) : "memory");
 }
 
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_normal() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ void tma_load_4d_hint(void* dst, const CUtensorMap* tm, uint64_t* bar, int x, int y, int z,
+                                                 int v, uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+      " [%0], [%1, {%3, %4, %5, %6}], [%2], %7;"
+      ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z), "r"(v), "l"(policy) : "memory");
+}
+// shared-memory counter increment, relaxed: no MEMBAR (an acq_rel atomic compiles to MEMBAR.ALL.CTA, which also
+// waits for the warp's outstanding global stores).  The ordering needed -- this warp's LDS reads of a buffer
+// before the increment -- comes from the SM executing one warp's shared-memory instructions in program order
+// (the property the usual "LDS ... then mbarrier.arrive" consumer release relies on); the refill is an async
+// TMA write issued after the last increment was observed.
+__device__ __forceinline__ unsigned smem_add_relaxed(unsigned* p, unsigned v) {
+  unsigned old;
+  asm volatile("atom.relaxed.cta.shared::cta.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(smem_u32(p)), "r"(v) : "memory");
+  return old;
+}
+
 // ---- stencil reads from the staged box -------------------------------------------------------------------------
 // `c` points at this thread's own grid point inside the current slot; BX, BY are the box row / plane extents.
 template <int BX, int BY>
@@ -75,7 +103,8 @@ __device__ __forceinline__ void axis_full(const P& p, double f0, int a, const Co
   d2 = (16.0 * s1 - s2) * (C.inv_h2 * (1.0 / 12.0));
   const double q = (s3 - 6.0 * s2) + 15.0 * s1;
   const double sp = (21.0 * e1 - 6.0 * e2) + e3;
-  ad += w.wq[a] * q + w.ws[a] * sp;
+  const double c = w.wq[a] * q + w.ws[a] * sp;
+  ad = a == 0 ? c : ad + c;   // axis 0 starts the sum (no 0.0 + c instruction)
 }
 template <class P>
 __device__ __forceinline__ void axis_d1_ad(const P& p, double f0, int a, const Coef& C, const AdvW& w, double& d1,
@@ -86,7 +115,8 @@ __device__ __forceinline__ void axis_d1_ad(const P& p, double f0, int a, const C
   d1 = (8.0 * e1 - e2) * (C.inv_h * (1.0 / 12.0));
   const double q = (s3 - 6.0 * s2) + 15.0 * s1;
   const double sp = (21.0 * e1 - 6.0 * e2) + e3;
-  ad += w.wq[a] * q + w.ws[a] * sp;
+  const double c = w.wq[a] * q + w.ws[a] * sp;
+  ad = a == 0 ? c : ad + c;   // axis 0 starts the sum (no 0.0 + c instruction)
 }
 template <class P>
 __device__ __forceinline__ void axis_ad(const P& p, double f0, int a, const AdvW& w, double& ad) {
@@ -95,7 +125,8 @@ __device__ __forceinline__ void axis_ad(const P& p, double f0, int a, const AdvW
   const double s1 = (p1 - f0) + (m1 - f0), s2 = (p2 - f0) + (m2 - f0), s3 = (p3 - f0) + (m3 - f0);
   const double q = (s3 - 6.0 * s2) + 15.0 * s1;
   const double sp = (21.0 * e1 - 6.0 * e2) + e3;
-  ad += w.wq[a] * q + w.ws[a] * sp;
+  const double c = w.wq[a] * q + w.ws[a] * sp;
+  ad = a == 0 ? c : ad + c;   // axis 0 starts the sum (no 0.0 + c instruction)
 }
 // dissipation only (slot A): ko * q
 template <class P>
@@ -123,7 +154,6 @@ __device__ __forceinline__ double mixed(const P& p, int a, int b, const Coef& C)
 template <class P>
 __device__ __forceinline__ void var_full(const P& p, const Coef& C, const AdvW& w, double* d1, double* d2, double& ad) {
   const double f0 = p.at(0, 0, 0);
-  ad = 0.0;
   axis_full(p, f0, 0, C, w, d1[0], d2[0], ad);
   axis_full(p, f0, 1, C, w, d1[1], d2[3], ad);
   axis_full(p, f0, 2, C, w, d1[2], d2[5], ad);
@@ -134,7 +164,6 @@ __device__ __forceinline__ void var_full(const P& p, const Coef& C, const AdvW& 
 template <class P>
 __device__ __forceinline__ void var_d1_ad(const P& p, const Coef& C, const AdvW& w, double* d1, double& ad) {
   const double f0 = p.at(0, 0, 0);
-  ad = 0.0;
   axis_d1_ad(p, f0, 0, C, w, d1[0], ad);
   axis_d1_ad(p, f0, 1, C, w, d1[1], ad);
   axis_d1_ad(p, f0, 2, C, w, d1[2], ad);
@@ -142,7 +171,7 @@ __device__ __forceinline__ void var_d1_ad(const P& p, const Coef& C, const AdvW&
 template <class P>
 __device__ __forceinline__ double var_ad(const P& p, const AdvW& w) {
   const double f0 = p.at(0, 0, 0);
-  double ad = 0.0;
+  double ad;
   axis_ad(p, f0, 0, w, ad);
   axis_ad(p, f0, 1, w, ad);
   axis_ad(p, f0, 2, w, ad);

@@ -163,6 +163,7 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
   L.tot_y = ny + 2 * ghost; L.tot_z = nz + 2 * ghost;
   L.plane = L.pitch * L.tot_y;
   L.vstride = L.plane * L.tot_z;
+  L.col_rows = 32;
   h->order = fd_order; h->system = system_id; h->dx = dx;
   h->eps_diss = 0.0; h->eta = 1.0; h->sgc = 0.75;
   h->stream = (cudaStream_t)cuda_stream;
@@ -206,7 +207,10 @@ int chemora_set_param(chemora_t* h, const char* name, double v) {
     h->eps_diss = v;
   } else if (!strcmp(name, "eta")) h->eta = v;
   else if (!strcmp(name, "shift_gamma_coeff")) h->sgc = v;
-  else return fail(h, CHEMORA_EINVAL, std::string("unknown parameter: ") + name);
+  else if (!strcmp(name, "col_rows")) {
+    if (v < 1.0 || v > 1e6) return fail(h, CHEMORA_EINVAL, "col_rows must be >= 1");
+    h->L.col_rows = (int)v;
+  } else return fail(h, CHEMORA_EINVAL, std::string("unknown parameter: ") + name);
   return CHEMORA_OK;
 }
 
@@ -215,6 +219,7 @@ int chemora_get_param(const chemora_t* h, const char* name, double* v) {
   if (!strcmp(name, "eps_diss")) *v = h->eps_diss;
   else if (!strcmp(name, "eta")) *v = h->eta;
   else if (!strcmp(name, "shift_gamma_coeff")) *v = h->sgc;
+  else if (!strcmp(name, "col_rows")) *v = h->L.col_rows;
   else return CHEMORA_EINVAL;
   return CHEMORA_OK;
 }

@@ -2,9 +2,18 @@
 // Part of the CUDA product path; shares nothing with oracle/.
 #pragma once
 #include <cuda_runtime.h>
+#ifndef CHM_STCS
+#define CHM_STCS 1
+#endif
 #include <stdint.h>
 
 namespace chm {
+
+#if CHM_STCS
+#define CHM_ST(p, v) __stcs(p, v)   // streaming store: written once, re-read only by a later launch
+#else
+#define CHM_ST(p, v) (*(p) = (v))
+#endif
 
 // Device-side view of the padded SoA layout (include/chemora.h "Conventions").
 struct Layout {
@@ -16,6 +25,7 @@ struct Layout {
   long plane;            // pitch * tot_y
   long vstride;          // plane * tot_z
   int tot_y, tot_z;
+  int col_rows;          // fused BSSN kernel: y-extent (grid rows) of a tile-traversal column (L2 reuse of halos)
 };
 
 // Stencil scale factors and model parameters, precomputed on the host once per launch.
@@ -67,15 +77,15 @@ __device__ __forceinline__ void stage_prefetch(const Stage& st, long q, StagePre
 }
 __device__ __forceinline__ void stage_emit(const Stage& st, long q, double k, const StagePre& pr) {
   if (st.mode == MODE_RHS) {
-    st.out[q] = k;
+    CHM_ST(&st.out[q], k);
   } else if (st.mode == MODE_FIRST) {
-    st.S[q] = k;
-    st.out[q] = __dadd_rn(pr.u, __dmul_rn(st.a, k));
+    CHM_ST(&st.S[q], k);
+    CHM_ST(&st.out[q], __dadd_rn(pr.u, __dmul_rn(st.a, k)));
   } else if (st.mode == MODE_MID) {
-    st.S[q] = __dadd_rn(pr.s, __dmul_rn(2.0, k));
-    st.out[q] = __dadd_rn(pr.u, __dmul_rn(st.a, k));
+    CHM_ST(&st.S[q], __dadd_rn(pr.s, __dmul_rn(2.0, k)));
+    CHM_ST(&st.out[q], __dadd_rn(pr.u, __dmul_rn(st.a, k)));
   } else {
-    st.U[q] = __dadd_rn(pr.u, __dmul_rn(st.a, __dadd_rn(pr.s, k)));
+    CHM_ST(&st.U[q], __dadd_rn(pr.u, __dmul_rn(st.a, __dadd_rn(pr.s, k))));
   }
 }
 

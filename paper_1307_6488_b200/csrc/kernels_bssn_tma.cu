@@ -1,7 +1,19 @@
 // kernels_bssn_tma.cu -- the fused BSSN kernel (derivatives + RHS + RK4 stage update), sm_100a:
 // persistent CTAs, TMA-staged per-variable boxes in a 5-slot mbarrier ring, compile-time stencil offsets.
+// No block-wide barrier in the tile loop: a slot is released warp by warp through a shared-memory counter and
+// the last warp to leave it issues the slot's next TMA load, so warps drift apart (up to 5 variables) and the
+// shared-memory-read phase of one warp overlaps the FP64 phase of another.  Tiles are visited column by column
+// (full x extent, Layout::col_rows rows of y, all z) so that the z-halo of a box is still in L2 when the tile
+// above it is processed; the read-once RK4 operands carry an L2 evict-first policy and stores are streaming.
 // See bssn_tma.cuh for the design; DESIGN.md "Kernels" for the roofline that bounds it.
 #include "bssn_tma.cuh"
+
+#ifndef CHM_BLOCKSYNC
+#define CHM_BLOCKSYNC 0
+#endif
+#ifndef CHM_L2HINT
+#define CHM_L2HINT 1
+#endif
 
 namespace chm {
 
@@ -26,40 +38,56 @@ struct TmaCfg {
   static constexpr uint32_t TILE_BYTES = (uint32_t)TILE * 8u;
   static constexpr int SLOTX = SLOT + 4 * TILE;   // box + RK4 operands (U,S) of up to two emitted variables
   static constexpr int CEN = kCenVars * TILE;     // point values needed ahead of their own boxes
-  static constexpr size_t SMEM = (size_t)(kSlots * SLOTX + CEN) * 8 + (kSlots + 1) * 8 + 128;
+  static constexpr size_t SMEM = (size_t)(kSlots * SLOTX + CEN) * 8 + (kSlots + 1) * 8 + (kSlots + 1) * 4 + 128;
+  static constexpr int NWARPS = THREADS / 32;
+  static_assert((NWARPS & (NWARPS - 1)) == 0, "release counters wrap modulo 2^32");
 };
 
 template <int TX, int TY, int TZ>
 __global__ void __launch_bounds__(TX* TY* TZ, 1)
 bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ CUtensorMap tmCen,
                 const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS, Layout L, Coef C,
-                Stage st, int ntx, int nty, int ntiles) {
+                Stage st, int ntx, int nty, int ntz, int cy) {
   using Cfg = TmaCfg<TX, TY, TZ>;
   constexpr int BX = Cfg::BX, BY = Cfg::BY, SLOT = Cfg::SLOT, SLOTX = Cfg::SLOTX, TILE = Cfg::TILE, CEN = Cfg::CEN;
+  constexpr unsigned NW = Cfg::NWARPS;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double* sm = reinterpret_cast<double*>(smem_raw);   // dynamic smem base: 128-byte aligned (no static smem)
   double* cbuf = sm + kSlots * SLOTX;                                  // [kCenVars][TILE]
   uint64_t* full = reinterpret_cast<uint64_t*>(cbuf + CEN);            // [kSlots] boxes, then [1] point values
   uint64_t* cfull = full + kSlots;
+  unsigned* cnt = reinterpret_cast<unsigned*>(cfull + 1);              // [kSlots] + [1]: warps that left a buffer
   const int nops = st.mode == MODE_RHS ? 0 : (st.mode == MODE_FIRST ? 1 : 2);   // RK4 operands per emitted var
+  const int ntiles = ntx * nty * ntz;
 
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31;
   const int lx = tid % TX, ly = (tid / TX) % TY, lz = tid / (TX * TY);
   const int coff = ((lz + 3) * BY + (ly + 3)) * BX + lx + 3;
   // halo-box origin relative to the tile origin in padded coordinates.  TMA needs every row of a box to start
   // on a 16-byte boundary: the layout makes L.xo - 3 even, and the (TX,TY,TZ) tile boxes (point values, RK4
   // operands) are loaded two columns wider, from x0 + 2, and read at column + 1.
   const int goffx = L.xo - 3, goff = L.g - 3;
+  const uint64_t pol_stream = CHM_L2HINT ? l2_policy_evict_first() : l2_policy_normal();   // U, S: read once per launch
 
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < kSlots + 1; ++s) mbar_init(&full[s], 1);
+    for (int s = 0; s < kSlots + 1; ++s) { mbar_init(&full[s], 1); cnt[s] = 0u; }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncthreads();
 
-  // producer (thread 0): box of variable order o of the tile whose origin (padded, minus halo) is (x0,y0,z0)
+  // tile order (see the file header): idx -> (bx, by, bz)
+  auto decode = [&](int idx, int& bx, int& by, int& bz) {
+    const int per_col = ntx * cy * ntz;
+    const int c = idx / per_col;
+    int r = idx - c * per_col;
+    const int cyt = min(cy, nty - c * cy), layer = ntx * cyt;
+    bz = r / layer; r -= bz * layer;
+    const int ry = r / ntx;
+    by = c * cy + ry; bx = r - ry * ntx;
+  };
+  // box of variable order o of the tile whose origin (padded, minus halo) is (x0,y0,z0); issued by one thread
   auto issue = [&](int o, int x0, int y0, int z0) {
     const int slot = o % kSlots;
     double* dst = sm + slot * SLOTX;
@@ -67,25 +95,35 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     const int nem = (v0 >= 0) + (v1 >= 0);
     mbar_expect_tx(&full[slot], Cfg::BOX_BYTES + (uint32_t)(nops * nem) * Cfg::TILE_BYTES);
     tma_load_4d(dst, &tm, &full[slot], x0, y0, z0, order_var(o));
-    if (v0 >= 0 && nops >= 1) tma_load_4d(dst + SLOT, &tmU, &full[slot], x0 + 2, y0 + 3, z0 + 3, v0);
-    if (v0 >= 0 && nops == 2) tma_load_4d(dst + SLOT + TILE, &tmS, &full[slot], x0 + 2, y0 + 3, z0 + 3, v0);
-    if (v1 >= 0 && nops >= 1) tma_load_4d(dst + SLOT + 2 * TILE, &tmU, &full[slot], x0 + 2, y0 + 3, z0 + 3, v1);
-    if (v1 >= 0 && nops == 2) tma_load_4d(dst + SLOT + 3 * TILE, &tmS, &full[slot], x0 + 2, y0 + 3, z0 + 3, v1);
+    if (v0 >= 0 && nops >= 1) tma_load_4d_hint(dst + SLOT, &tmU, &full[slot], x0 + 2, y0 + 3, z0 + 3, v0, pol_stream);
+    if (v0 >= 0 && nops == 2) tma_load_4d_hint(dst + SLOT + TILE, &tmS, &full[slot], x0 + 2, y0 + 3, z0 + 3, v0, pol_stream);
+    if (v1 >= 0 && nops >= 1) tma_load_4d_hint(dst + SLOT + 2 * TILE, &tmU, &full[slot], x0 + 2, y0 + 3, z0 + 3, v1, pol_stream);
+    if (v1 >= 0 && nops == 2) tma_load_4d_hint(dst + SLOT + 3 * TILE, &tmS, &full[slot], x0 + 2, y0 + 3, z0 + 3, v1, pol_stream);
   };
-  // point values of tile number tt of this CTA (three 7-variable boxes: vars 0..6, 7..13, 17..23)
+  // point values of a tile (three 7-variable boxes: vars 0..6, 7..13, 17..23)
   auto issue_cen = [&](int x0, int y0, int z0) {
     mbar_expect_tx(cfull, (uint32_t)kCenVars * Cfg::TILE_BYTES);
     tma_load_4d(cbuf, &tmCen, cfull, x0 + 2, y0 + 3, z0 + 3, 0);
     tma_load_4d(cbuf + 7 * TILE, &tmCen, cfull, x0 + 2, y0 + 3, z0 + 3, 7);
     tma_load_4d(cbuf + 14 * TILE, &tmCen, cfull, x0 + 2, y0 + 3, z0 + 3, 17);
   };
-  auto origin = [&](int tile, int& x0, int& y0, int& z0) {
-    const int bz = tile / (ntx * nty), rem = tile - bz * ntx * nty, by = rem / ntx, bx = rem - by * ntx;
-    x0 = bx * TX + goffx; y0 = by * TY + goff; z0 = bz * TZ + goff;
+  // one warp leaves buffer b (all its reads of it are done); true for lane 0 of the last of the NW warps
+  auto leave = [&](int b) {
+#if CHM_BLOCKSYNC
+    __syncthreads();
+    return tid == 0;
+#endif
+    __syncwarp();
+    bool last = false;
+    if (lane == 0) {
+      last = (smem_add_relaxed(&cnt[b], 1u) & (NW - 1)) == NW - 1;
+    }
+    return last;
   };
   if (tid == 0 && (int)blockIdx.x < ntiles) {
-    int x0, y0, z0;
-    origin(blockIdx.x, x0, y0, z0);
+    int bx, by, bz;
+    decode(blockIdx.x, bx, by, bz);
+    const int x0 = bx * TX + goffx, y0 = by * TY + goff, z0 = bz * TZ + goff;
     issue_cen(x0, y0, z0);
 #pragma unroll
     for (int o = 0; o < kSlots; ++o) issue(o, x0, y0, z0);
@@ -93,7 +131,8 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 
   int t = 0;
   for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++t) {
-    const int bz = tile / (ntx * nty), rem = tile - bz * ntx * nty, by = rem / ntx, bx = rem - by * ntx;
+    int bx, by, bz;
+    decode(tile, bx, by, bz);
     const int i = bx * TX + lx, j = by * TY + ly, k = bz * TZ + lz;
     const bool valid = i < L.nx && j < L.ny && k < L.nz;
     const long q = (long)((valid ? k : 0) + L.g) * L.plane + (long)((valid ? j : 0) + L.g) * L.pitch +
@@ -109,22 +148,28 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     };
     auto emit = [&](int v, double k, const StagePre& pr) { if (valid) stage_emit(st, q + v * L.vstride, k, pr); };
 
-    // section o: wait for its box, hand out the accessor; done(o): release the slot, prefetch 5 loads ahead
+    // section o: wait for its box, hand out the accessor; done(o): this warp leaves the slot; the last warp to
+    // leave refills it with the box 5 loads ahead (of this tile, or of this CTA's next tile)
     auto box = [&](int o) {
       mbar_wait(&full[o % kSlots], (uint32_t)((t + o / kSlots) & 1));
       return BoxPoint<BX, BY>{sm + (o % kSlots) * SLOTX + coff};
     };
-    int nx0 = 0, ny0 = 0, nz0 = 0;           // next tile of this CTA (thread 0 prefetches its first 5 boxes)
     const bool has_next = tile + (int)gridDim.x < ntiles;
-    if (tid == 0 && has_next) origin(tile + gridDim.x, nx0, ny0, nz0);
+    int nx0 = 0, ny0 = 0, nz0 = 0;           // origin of this CTA's next tile
+    if (has_next) {
+      int b0, b1, b2;
+      decode(tile + gridDim.x, b0, b1, b2);
+      nx0 = b0 * TX + goffx; ny0 = b1 * TY + goff; nz0 = b2 * TZ + goff;
+    }
     auto done = [&](int o) {
-      __syncthreads();
-      if (tid == 0) {
-        // the point values are last read at the top of section 3 (At): after section 5 the buffer is free
-        if (o == 5 && has_next) issue_cen(nx0, ny0, nz0);
+      if (leave(o % kSlots)) {
         if (o + kSlots < 25) issue(o + kSlots, bx * TX + goffx, by * TY + goff, bz * TZ + goff);
         else if (has_next) issue(o + kSlots - 25, nx0, ny0, nz0);
       }
+    };
+    // the point values are last read just before section 3 (At)
+    auto done_cen = [&]() {
+      if (leave(kSlots) && has_next) issue_cen(nx0, ny0, nz0);
     };
 
     const double third = 1.0 / 3.0, two_thirds = 2.0 / 3.0;
@@ -151,7 +196,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     const double alpha = cen(V_ALPHA), trK = cen(V_K), chi = cen(V_CHI);
 
     // ---- o = 0..2: beta^i : d_j beta^i, gtu^{jk} d_j d_k beta^i, d_j (d_k beta^k) ----------------------------
-    double db[3][3], lapb[3], gdiv[3] = {0.0, 0.0, 0.0};   // db[j][i] = d_j beta^i ; gdiv[j] = d_j d_k beta^k
+    double db[3][3], lapb[3], gdiv[3];   // db[j][i] = d_j beta^i ; gdiv[j] = d_j d_k beta^k
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2) {
       const double Bc = cen(V_B + i2);
@@ -161,7 +206,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       var_full(p, C, w, d1, d2, ad);
       done(i2);
 #pragma unroll
-      for (int a = 0; a < 3; ++a) { db[a][i2] = d1[a]; gdiv[a] += d2[sym(a, i2)]; }
+      for (int a = 0; a < 3; ++a) { db[a][i2] = d1[a]; gdiv[a] = i2 == 0 ? d2[sym(a, i2)] : gdiv[a] + d2[sym(a, i2)]; }
       lapb[i2] = sdot(gu, d2);
       emit(V_BETA + i2, C.sgc * Bc + ad, pr);
     }
@@ -171,6 +216,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     double At[6], Rt[6], dg[3][6];
 #pragma unroll
     for (int s = 0; s < 6; ++s) At[s] = cen(V_AT + s);
+    done_cen();
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2)
 #pragma unroll
@@ -183,9 +229,12 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
         done(3 + s);
         dg[0][s] = d1[0]; dg[1][s] = d1[1]; dg[2][s] = d1[2];
         Rt[s] = -0.5 * sdot(gu, d2);
-        double lie = 0.0;
+        double lie;
 #pragma unroll
-        for (int k2 = 0; k2 < 3; ++k2) lie += g[sym(i2, k2)] * db[j2][k2] + g[sym(j2, k2)] * db[i2][k2];
+        for (int k2 = 0; k2 < 3; ++k2) {
+          const double c = g[sym(i2, k2)] * db[j2][k2] + g[sym(j2, k2)] * db[i2][k2];
+          lie = k2 == 0 ? c : lie + c;
+        }
         emit(V_GT + s, (lie - two_thirds * g[s] * divb) - 2.0 * alpha * At[s] + ad, pr);
       }
 
@@ -209,27 +258,37 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       }
       // R~_ij += 1/2 Gamma~^k_n (Gamma~_ijk + Gamma~_jik)
       //        + gtu^{lm} (Gamma~^k_li Gamma~_jkm + Gamma~^k_lj Gamma~_ikm + Gamma~^k_im Gamma~_klj)
+      // with the inverse metric contracted once: W[i][m] = gtu^{lm} Gamma~^k_li (per k), so the three products are
+      //   sum_m W[i][m] Gamma~_jkm + W[j][m] Gamma~_ikm   and   sum_l W[i][l] Gamma~_klj
 #pragma unroll
       for (int i2 = 0; i2 < 3; ++i2)
 #pragma unroll
         for (int j2 = i2; j2 < 3; ++j2) {
-          double acc = 0.0;
-#pragma unroll
-          for (int k2 = 0; k2 < 3; ++k2) acc += Gn[k2] * (Cl[i2][sym(j2, k2)] + Cl[j2][sym(i2, k2)]);
-          acc *= 0.5;
-#pragma unroll
-          for (int l = 0; l < 3; ++l)
-#pragma unroll
-            for (int m = 0; m < 3; ++m) {
-              double qq = 0.0;
-#pragma unroll
-              for (int k2 = 0; k2 < 3; ++k2)
-                qq += Cu[k2][sym(l, i2)] * Cl[j2][sym(k2, m)] + Cu[k2][sym(l, j2)] * Cl[i2][sym(k2, m)] +
-                      Cu[k2][sym(i2, m)] * Cl[k2][sym(l, j2)];
-              acc += gu[sym(l, m)] * qq;
-            }
-          Rt[sym(i2, j2)] += acc;
+          const double c = (Gn[0] * (Cl[i2][sym(j2, 0)] + Cl[j2][sym(i2, 0)]) +
+                            Gn[1] * (Cl[i2][sym(j2, 1)] + Cl[j2][sym(i2, 1)])) +
+                           Gn[2] * (Cl[i2][sym(j2, 2)] + Cl[j2][sym(i2, 2)]);
+          Rt[sym(i2, j2)] += 0.5 * c;
         }
+#pragma unroll
+      for (int k2 = 0; k2 < 3; ++k2) {
+        double W[3][3];
+#pragma unroll
+        for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+          for (int m = 0; m < 3; ++m)
+            W[i2][m] = gu[sym(0, m)] * Cu[k2][sym(0, i2)] + gu[sym(1, m)] * Cu[k2][sym(1, i2)] +
+                       gu[sym(2, m)] * Cu[k2][sym(2, i2)];
+#pragma unroll
+        for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+          for (int j2 = i2; j2 < 3; ++j2) {
+            double acc = W[i2][0] * Cl[k2][sym(0, j2)] + W[i2][1] * Cl[k2][sym(1, j2)] + W[i2][2] * Cl[k2][sym(2, j2)];
+            const double t1 = W[i2][0] * Cl[j2][sym(k2, 0)] + W[i2][1] * Cl[j2][sym(k2, 1)] + W[i2][2] * Cl[j2][sym(k2, 2)];
+            if (i2 == j2) acc += 2.0 * t1;
+            else acc += t1 + (W[j2][0] * Cl[i2][sym(k2, 0)] + W[j2][1] * Cl[i2][sym(k2, 1)] + W[j2][2] * Cl[i2][sym(k2, 2)]);
+            Rt[sym(i2, j2)] += acc;
+          }
+      }
     }
 
     // ---- o = 9..11: Gt^k : R~_ij += 1/2 (gt_ki d_j Gt^k + gt_kj d_i Gt^k); advection kept for the end ------
@@ -333,11 +392,12 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
           const StagePre pr = pre(15 + s, 0);
           const double ad = var_ad(p, w);
           done(15 + s);
-          double AA = 0.0, lie = 0.0;
+          double AA, lie;
 #pragma unroll
           for (int k2 = 0; k2 < 3; ++k2) {
-            AA += At[sym(i2, k2)] * Am[k2][j2];
-            lie += At[sym(i2, k2)] * db[j2][k2] + At[sym(j2, k2)] * db[i2][k2];
+            const double c = At[sym(i2, k2)] * db[j2][k2] + At[sym(j2, k2)] * db[i2][k2];
+            AA = k2 == 0 ? At[sym(i2, k2)] * Am[k2][j2] : AA + At[sym(i2, k2)] * Am[k2][j2];
+            lie = k2 == 0 ? c : lie + c;
           }
           emit(V_AT + s, chi * (Rt[s] - third * g[s] * trX) + alpha * (trK * At[s] - 2.0 * AA) +
                              (lie - two_thirds * At[s] * divb) + ad, pr);
@@ -437,7 +497,8 @@ static cudaError_t tma_go(const Layout& L, const Coef& C, const Stage* st, cudaS
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, Cfg::THREADS, Cfg::SMEM);
   if (blocks_per_sm < 1) blocks_per_sm = 1;
   const int grid = ntiles < sms * blocks_per_sm ? ntiles : sms * blocks_per_sm;
-  kern<<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, L, C, *st, ntx, nty, ntiles);
+  const int cy = L.col_rows / TY > 0 ? L.col_rows / TY : 1;   // tile rows per traversal column
+  kern<<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, L, C, *st, ntx, nty, ntz, cy);
   return cudaGetLastError();
 }
 
