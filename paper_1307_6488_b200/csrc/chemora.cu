@@ -110,16 +110,17 @@ int run_rhs_inner(chemora_t* h, const Stage& st) {
   if (h->eps_diss != 0.0 && h->L.g < 3) return fail(h, CHEMORA_EINVAL, "eps_diss != 0 needs ghost >= 3 (KO order 5)");
   Coef C = make_coef(h);
   if (h->system == CHEMORA_SYS_WAVE) {
-    CK(h, launch_wave(h->L, C, h->order, h->tile, st, h->stream), "wave kernel launch");
+    CK(h, launch_wave(h->L, C, h->order, h->tile % 6, st, h->stream), "wave kernel launch");
     h->launches += 1;
   } else if (h->fused) {
-    CK(h, launch_bssn_fused(h->L, C, h->tile, st, h->stream), "bssn fused kernel launch");
+    if (h->tile >= 6) CK(h, launch_bssn_ws(h->L, C, h->tile - 6, st, h->stream), "bssn warp-specialised kernel launch");
+    else CK(h, launch_bssn_fused(h->L, C, h->tile, st, h->stream), "bssn fused kernel launch");
     h->launches += 1;
   } else {
     int rc = ensure_derivs(h);
     if (rc) return rc;
-    CK(h, launch_bssn_derivs(h->L, C, h->tile, st.in, h->derivs, h->stream), "bssn derivative kernel launch");
-    CK(h, launch_bssn_from_derivs(h->L, C, h->tile, h->derivs, st, h->stream), "bssn rhs kernel launch");
+    CK(h, launch_bssn_derivs(h->L, C, h->tile % 6, st.in, h->derivs, h->stream), "bssn derivative kernel launch");
+    CK(h, launch_bssn_from_derivs(h->L, C, h->tile % 6, h->derivs, st, h->stream), "bssn rhs kernel launch");
     h->launches += 2;
   }
   return CHEMORA_OK;
@@ -333,10 +334,11 @@ int chemora_get_variant(const chemora_t* h, int* fused, int* tile_id) {
 
 int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, int* tz) {
   if (tile_id < 0 || tile_id >= CHEMORA_NUM_TILES) return CHEMORA_EINVAL;
-  const TileShape* T = (system_id == CHEMORA_SYS_BSSN && fused) ? kTilesFused : kTilesMarch;
-  if (tx) *tx = T[tile_id].tx;
-  if (ty) *ty = T[tile_id].ty;
-  if (tz) *tz = T[tile_id].tz;
+  const bool f = system_id == CHEMORA_SYS_BSSN && fused;
+  const TileShape T = f ? kTilesFused[tile_id] : kTilesMarch[tile_id % 6];
+  if (tx) *tx = T.tx;
+  if (ty) *ty = T.ty;
+  if (tz) *tz = T.tz;
   return CHEMORA_OK;
 }
 
@@ -415,9 +417,10 @@ int chemora_timing_read(chemora_t* h, double* rhs_ms, long* rhs_launches, double
 int chemora_kernel_info(const chemora_t* h, int* regs, int* local_bytes, int* smem_bytes) {
   if (!h) return CHEMORA_EINVAL;
   cudaFuncAttributes a;
-  cudaError_t e = h->system == CHEMORA_SYS_WAVE ? kernel_info_wave(h->order, h->tile, &a)
-                  : h->fused               ? kernel_info_bssn_fused(h->tile, &a)
-                                           : kernel_info_bssn_split(1, h->tile, &a);
+  cudaError_t e = h->system == CHEMORA_SYS_WAVE ? kernel_info_wave(h->order, h->tile % 6, &a)
+                  : !h->fused              ? kernel_info_bssn_split(1, h->tile % 6, &a)
+                  : h->tile >= 6           ? kernel_info_bssn_ws(h->tile - 6, &a)
+                                           : kernel_info_bssn_fused(h->tile, &a);
   if (e != cudaSuccess) return cuda_fail(const_cast<chemora_t*>(h), e, "cudaFuncGetAttributes");
   if (regs) *regs = a.numRegs;
   if (local_bytes) *local_bytes = (int)a.localSizeBytes;

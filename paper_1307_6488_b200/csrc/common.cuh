@@ -92,7 +92,9 @@ __device__ __forceinline__ void stage_emit(const Stage& st, long q, double k, co
 // Tile shapes of the variant sweep.  Fused kernel: 3-D tile, one point per thread.  Split kernels and the wave
 // kernel: x,y = thread block, z = planes marched per block.
 struct TileShape { int tx, ty, tz; };
-static const TileShape kTilesFused[6] = {{16, 4, 4}, {16, 8, 2}, {8, 8, 4}, {8, 4, 8}, {16, 2, 8}, {16, 4, 2}};
+// ids 6..8: the warp-specialised fused kernel (kernels_bssn_ws.cu) on the three 256-point shapes
+static const TileShape kTilesFused[9] = {{16, 4, 4}, {16, 8, 2}, {8, 8, 4}, {8, 4, 8}, {16, 2, 8}, {16, 4, 2},
+                                         {16, 4, 4}, {16, 8, 2}, {16, 2, 8}};
 static const TileShape kTilesMarch[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64, 4, 8}, {128, 2, 8}, {16, 16, 8}};
 
 // launchers implemented in the kernel translation units; each returns the cudaError_t of the launch
@@ -100,6 +102,8 @@ cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s);
 cudaError_t launch_pack(const Layout& L, const double* packed, double* state, bool to_state, cudaStream_t s);
 cudaError_t launch_wave(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
 cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int tile, const Stage& st, cudaStream_t s);
+cudaError_t launch_bssn_ws(const Layout& L, const Coef& C, int which, const Stage& st, cudaStream_t s);
+cudaError_t kernel_info_bssn_ws(int which, cudaFuncAttributes* a);
 cudaError_t launch_bssn_derivs(const Layout& L, const Coef& C, int tile, const double* in, double* derivs,
                                cudaStream_t s);
 cudaError_t launch_bssn_from_derivs(const Layout& L, const Coef& C, int tile, const double* derivs,
