@@ -89,6 +89,22 @@ __device__ __forceinline__ void stage_emit(const Stage& st, long q, double k, co
   }
 }
 
+// Same with the mode as a compile-time constant (no branches in the epilogue of the fused BSSN kernel).
+template <int MODE>
+__device__ __forceinline__ void stage_emit_t(const Stage& st, long q, double k, const StagePre& pr) {
+  if (MODE == MODE_RHS) {
+    CHM_ST(&st.out[q], k);
+  } else if (MODE == MODE_FIRST) {
+    CHM_ST(&st.S[q], k);
+    CHM_ST(&st.out[q], __dadd_rn(pr.u, __dmul_rn(st.a, k)));
+  } else if (MODE == MODE_MID) {
+    CHM_ST(&st.S[q], __dadd_rn(pr.s, __dmul_rn(2.0, k)));
+    CHM_ST(&st.out[q], __dadd_rn(pr.u, __dmul_rn(st.a, k)));
+  } else {
+    CHM_ST(&st.U[q], __dadd_rn(pr.u, __dmul_rn(st.a, __dadd_rn(pr.s, k))));
+  }
+}
+
 // Tile shapes of the variant sweep.  Fused kernel: 3-D tile, one point per thread.  Split kernels and the wave
 // kernel: x,y = thread block, z = planes marched per block.
 struct TileShape { int tx, ty, tz; };

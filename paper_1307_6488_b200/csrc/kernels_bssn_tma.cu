@@ -11,6 +11,9 @@
 #ifndef CHM_BLOCKSYNC
 #define CHM_BLOCKSYNC 0
 #endif
+#ifndef CHM_TWOPASS
+#define CHM_TWOPASS 0   // mixed second derivatives as D_x(D_y f), D_x(D_z f), D_y(D_z f) through shared memory
+#endif
 #ifndef CHM_L2HINT
 #define CHM_L2HINT 1
 #endif
@@ -38,12 +41,17 @@ struct TmaCfg {
   static constexpr uint32_t TILE_BYTES = (uint32_t)TILE * 8u;
   static constexpr int SLOTX = SLOT + 4 * TILE;   // box + RK4 operands (U,S) of up to two emitted variables
   static constexpr int CEN = kCenVars * TILE;     // point values needed ahead of their own boxes
-  static constexpr size_t SMEM = (size_t)(kSlots * SLOTX + CEN) * 8 + (kSlots + 1) * 8 + (kSlots + 1) * 4 + 128;
+  // first derivatives shared between threads for the mixed second derivatives (two buffers, alternating):
+  // D_y f on the tile + 2 columns of x-halo, D_z f on the tile + 2 columns of x-halo + 2 rows of y-halo
+  static constexpr int DYX = TX + 4;
+  static constexpr int DY_N = DYX * TY * TZ, DZ_N = DYX * (TY + 4) * TZ;
+  static constexpr int DB = CHM_TWOPASS ? (DY_N + DZ_N + 15) / 16 * 16 : 0;
+  static constexpr size_t SMEM = (size_t)(kSlots * SLOTX + CEN + 2 * DB) * 8 + (kSlots + 1) * 8 + (kSlots + 1) * 4 + 128;
   static constexpr int NWARPS = THREADS / 32;
   static_assert((NWARPS & (NWARPS - 1)) == 0, "release counters wrap modulo 2^32");
 };
 
-template <int TX, int TY, int TZ>
+template <int TX, int TY, int TZ, int MODE>
 __global__ void __launch_bounds__(TX* TY* TZ, 1)
 bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ CUtensorMap tmCen,
                 const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS, Layout L, Coef C,
@@ -54,10 +62,11 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double* sm = reinterpret_cast<double*>(smem_raw);   // dynamic smem base: 128-byte aligned (no static smem)
   double* cbuf = sm + kSlots * SLOTX;                                  // [kCenVars][TILE]
-  uint64_t* full = reinterpret_cast<uint64_t*>(cbuf + CEN);            // [kSlots] boxes, then [1] point values
+  double* dbuf = cbuf + CEN;                                           // [2][DB] shared first derivatives
+  uint64_t* full = reinterpret_cast<uint64_t*>(dbuf + 2 * Cfg::DB);    // [kSlots] boxes, then [1] point values
   uint64_t* cfull = full + kSlots;
   unsigned* cnt = reinterpret_cast<unsigned*>(cfull + 1);              // [kSlots] + [1]: warps that left a buffer
-  const int nops = st.mode == MODE_RHS ? 0 : (st.mode == MODE_FIRST ? 1 : 2);   // RK4 operands per emitted var
+  constexpr int nops = MODE == MODE_RHS ? 0 : (MODE == MODE_FIRST ? 1 : 2);   // RK4 operands per emitted var
   const int ntiles = ntx * nty * ntz;
 
   const int tid = threadIdx.x, lane = tid & 31;
@@ -146,7 +155,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       const double* op = sm + (o % kSlots) * SLOTX + SLOT + 2 * n * TILE + toff;
       return StagePre{op[0], op[TILE]};
     };
-    auto emit = [&](int v, double k, const StagePre& pr) { if (valid) stage_emit(st, q + v * L.vstride, k, pr); };
+    auto emit = [&](int v, double k, const StagePre& pr) { if (valid) stage_emit_t<MODE>(st, q + v * L.vstride, k, pr); };
 
     // section o: wait for its box, hand out the accessor; done(o): this warp leaves the slot; the last warp to
     // leave refills it with the box 5 loads ahead (of this tile, or of this CTA's next tile)
@@ -170,6 +179,49 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     // the point values are last read just before section 3 (At)
     auto done_cen = [&]() {
       if (leave(kSlots) && has_next) issue_cen(nx0, ny0, nz0);
+    };
+
+    // all derivatives of a "full" variable (section o, n-th full variable of the tile), then done(o).
+    // Two-pass mixed derivatives: every thread publishes D_y f and D_z f of its own point (it has them already),
+    // the block adds them on the 2-cell x-halo (and D_z f on the 2-cell y-halo), and after one block barrier
+    // d_xy = D_x(D_y f), d_xz = D_x(D_z f), d_yz = D_y(D_z f) cost 4 reads each instead of 16.
+    auto full_var = [&](const BoxPoint<BX, BY>& p, const AdvW& w, int o, int n, double* d1, double* d2, double& ad) {
+#if CHM_TWOPASS
+      constexpr int DYX = Cfg::DYX, ZS = BX * BY;
+      const double f0 = p.at(0, 0, 0);
+      axis_full(p, f0, 0, C, w, d1[0], d2[0], ad);
+      axis_full(p, f0, 1, C, w, d1[1], d2[3], ad);
+      axis_full(p, f0, 2, C, w, d1[2], d2[5], ad);
+      double* Dy = dbuf + ((t + n) & 1) * Cfg::DB;
+      double* Dz = Dy + Cfg::DY_N;
+      const double c12 = C.inv_h * (1.0 / 12.0);
+      Dy[(lz * TY + ly) * DYX + lx + 2] = d1[1];
+      Dz[(lz * (TY + 4) + ly + 2) * DYX + lx + 2] = d1[2];
+      const double* sb = p.c - coff;   // slot base
+      for (int h = tid; h < TX * 4 * TZ; h += Cfg::THREADS) {          // D_z f on the y-halo rows -2,-1,TY,TY+1
+        const int hx = h % TX, hyi = (h / TX) % 4, hz = h / (TX * 4);
+        const int yy = hyi < 2 ? hyi - 2 : TY + hyi - 2;
+        const double* c = sb + ((hz + 3) * BY + (yy + 3)) * BX + hx + 3;
+        Dz[(hz * (TY + 4) + yy + 2) * DYX + hx + 2] = (8.0 * (c[ZS] - c[-ZS]) - (c[2 * ZS] - c[-2 * ZS])) * c12;
+      }
+      for (int h = tid; h < 4 * TY * TZ; h += Cfg::THREADS) {          // D_y f, D_z f on the x-halo columns
+        const int hxi = h % 4, hy = (h / 4) % TY, hz = h / (4 * TY);
+        const int xx = hxi < 2 ? hxi - 2 : TX + hxi - 2;
+        const double* c = sb + ((hz + 3) * BY + (hy + 3)) * BX + xx + 3;
+        Dy[(hz * TY + hy) * DYX + xx + 2] = (8.0 * (c[BX] - c[-BX]) - (c[2 * BX] - c[-2 * BX])) * c12;
+        Dz[(hz * (TY + 4) + hy + 2) * DYX + xx + 2] = (8.0 * (c[ZS] - c[-ZS]) - (c[2 * ZS] - c[-2 * ZS])) * c12;
+      }
+      done(o);
+      __syncthreads();
+      const double* y = Dy + (lz * TY + ly) * DYX + lx + 2;
+      const double* z = Dz + (lz * (TY + 4) + ly + 2) * DYX + lx + 2;
+      d2[1] = (8.0 * (y[1] - y[-1]) - (y[2] - y[-2])) * c12;
+      d2[2] = (8.0 * (z[1] - z[-1]) - (z[2] - z[-2])) * c12;
+      d2[4] = (8.0 * (z[DYX] - z[-DYX]) - (z[2 * DYX] - z[-2 * DYX])) * c12;
+#else
+      var_full(p, C, w, d1, d2, ad);
+      done(o);
+#endif
     };
 
     const double third = 1.0 / 3.0, two_thirds = 2.0 / 3.0;
@@ -203,8 +255,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       auto p = box(i2);
       const StagePre pr = pre(i2, 0);
       double d1[3], d2[6], ad;
-      var_full(p, C, w, d1, d2, ad);
-      done(i2);
+      full_var(p, w, i2, i2, d1, d2, ad);
 #pragma unroll
       for (int a = 0; a < 3; ++a) { db[a][i2] = d1[a]; gdiv[a] = i2 == 0 ? d2[sym(a, i2)] : gdiv[a] + d2[sym(a, i2)]; }
       lapb[i2] = sdot(gu, d2);
@@ -225,8 +276,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
         auto p = box(3 + s);
         const StagePre pr = pre(3 + s, 0);
         double d1[3], d2[6], ad;
-        var_full(p, C, w, d1, d2, ad);
-        done(3 + s);
+        full_var(p, w, 3 + s, 3 + s, d1, d2, ad);
         dg[0][s] = d1[0]; dg[1][s] = d1[1]; dg[2][s] = d1[2];
         Rt[s] = -0.5 * sdot(gu, d2);
         double lie;
@@ -313,8 +363,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       auto p = box(12);
       const StagePre pr = pre(12, 0);
       double d2[6], ad;
-      var_full(p, C, w, dchi, d2, ad);
-      done(12);
+      full_var(p, w, 12, 9, dchi, d2, ad);
       emit(V_CHI, two_thirds * chi * (alpha * trK - divb) + ad, pr);
       double cd[6], cc[6];   // D~_i D~_j chi ; d_i chi d_j chi
 #pragma unroll
@@ -337,8 +386,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       auto p = box(13);
       const StagePre pr = pre(13, 0);
       double d2[6], ad;
-      var_full(p, C, w, dal, d2, ad);
-      done(13);
+      full_var(p, w, 13, 10, dal, d2, ad);
       emit(V_ALPHA, -2.0 * alpha * trK + ad, pr);
       double cd[6], ca[6];   // d_i d_j alpha - Gamma~^k_ij d_k alpha ; d_i chi d_j alpha + d_j chi d_i alpha
 #pragma unroll
@@ -454,10 +502,10 @@ static EncodeTiledFn encode_fn() {
   return fn;
 }
 
-template <int TX, int TY, int TZ>
-static cudaError_t tma_go(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
+template <int TX, int TY, int TZ, int MODE>
+static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
   using Cfg = TmaCfg<TX, TY, TZ>;
-  auto kern = bssn_tma_kernel<TX, TY, TZ>;
+  auto kern = bssn_tma_kernel<TX, TY, TZ, MODE>;
   if (a) return cudaFuncGetAttributes(a, kern);
   EncodeTiledFn enc = encode_fn();
   if (!enc) return cudaErrorNotSupported;
@@ -500,6 +548,17 @@ static cudaError_t tma_go(const Layout& L, const Coef& C, const Stage* st, cudaS
   const int cy = L.col_rows / TY > 0 ? L.col_rows / TY : 1;   // tile rows per traversal column
   kern<<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, L, C, *st, ntx, nty, ntz, cy);
   return cudaGetLastError();
+}
+
+template <int TX, int TY, int TZ>
+static cudaError_t tma_go(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
+  switch (st ? st->mode : MODE_MID) {   // kernel_info reports the common (middle-stage) instance
+    case MODE_RHS: return tma_go_mode<TX, TY, TZ, MODE_RHS>(L, C, st, s, a);
+    case MODE_FIRST: return tma_go_mode<TX, TY, TZ, MODE_FIRST>(L, C, st, s, a);
+    case MODE_MID: return tma_go_mode<TX, TY, TZ, MODE_MID>(L, C, st, s, a);
+    case MODE_LAST: return tma_go_mode<TX, TY, TZ, MODE_LAST>(L, C, st, s, a);
+  }
+  return cudaErrorInvalidValue;
 }
 
 static cudaError_t tma_dispatch(int tile, const Layout& L, const Coef& C, const Stage* st, cudaStream_t s,
