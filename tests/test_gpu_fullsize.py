@@ -1,0 +1,94 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (variant picked by the runtime
+sweep), on sampled outputs the oracle can compute one by one (`pytest -m gpu`).
+
+A grid point after n RK4 steps depends on the initial data within 12 n cells (4 stages x 3-cell stencils; 16 n for
+the 8th-order wave system), so the oracle evolves a small periodic block cut around each sample (the cut's own
+wrap-around is wrong, but cannot reach the block's centre) and the centre is compared with the GPU state.
+Error norm: S11 with the per-variable maximum taken over the whole GPU state."""
+import numpy as np
+import pytest
+
+from paper_1307_6488_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+def cut(u, centre, half):
+    """periodic cube of side 2*half around `centre` (x, y, z) from a packed [V, nz, ny, nx] array"""
+    _, nz, ny, nx = u.shape
+    ix = np.arange(centre[0] - half, centre[0] + half) % nx
+    iy = np.arange(centre[1] - half, centre[1] + half) % ny
+    iz = np.arange(centre[2] - half, centre[2] + half) % nz
+    return np.ascontiguousarray(u[:, iz][:, :, iy][:, :, :, ix])
+
+
+def check_samples(oracle, system, u0, got, centres, reach, core, g, order, dx, dt, prm, steps, tol):
+    V = u0.shape[0]
+    scale = [float(np.max(np.abs(got[v]))) for v in range(V)]
+    half = core + reach
+    worst = 0.0
+    for c in centres:
+        blk = cut(u0, c, half)
+        st = oracle.rk4(system, oracle.with_ghosts(blk, g), g, order, dx, dt, prm, steps)
+        want = oracle.interior(st, g)[:, reach:reach + 2 * core, reach:reach + 2 * core, reach:reach + 2 * core]
+        have = cut(got, c, core)
+        for v in range(V):
+            err = float(np.max(np.abs(have[v] - want[v])))
+            if scale[v] == 0.0:
+                assert err == 0.0, (c, v)
+            else:
+                worst = max(worst, err / scale[v])
+    assert worst < tol, worst
+    return worst
+
+
+def test_bssn_config3_256_sampled(oracle):
+    """configs[3]: BSSN 256^3, Minkowski + 1e-4 Gaussians, 2 RK4 steps; tolerance = 2/10 of 1e-10 per 10 steps."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1307_6488_b200 import binding
+    c = inputs.config(3)
+    n, g, dx = 256, c["ghost"], c["dx"]
+    dt, steps = 0.25 * dx, 2
+    u0 = c["state"]()
+    h = binding.Chemora(n, n, n, g, c["order"], binding.SYS_BSSN, dx)
+    h.set_param("eps_diss", c["eps_diss"])
+    h.set_state(u0)
+    h.autotune()                       # what bench.py does
+    for _ in range(steps):
+        h.rk4_step(dt)
+    got = h.get_state()
+    h.destroy()
+    rng = np.random.default_rng(7)
+    centres = [(0, 0, 0), (255, 128, 3)] + [tuple(int(x) for x in rng.integers(0, n, 3)) for _ in range(3)]
+    # one sample on the steepest part of the data: where |grad alpha| is largest
+    ga = np.abs(np.gradient(u0[17, :, :, :], axis=2))
+    k, j, i = np.unravel_index(int(np.argmax(ga)), ga.shape)
+    centres.append((int(i), int(j), int(k)))
+    check_samples(oracle, oracle.SYS_BSSN, u0, got, centres, reach=12 * steps, core=4, g=g, order=4, dx=dx, dt=dt,
+                  prm=oracle.params(eps_diss=c["eps_diss"]), steps=steps, tol=2e-11)
+
+
+def test_wave_config1_256_sampled(oracle):
+    """configs[1]: wave 256^3, O8 + KO, 8 plane waves, 2 RK4 steps; 1e-12 per step."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1307_6488_b200 import binding
+    c = inputs.config(1)
+    n, g, dx = 256, c["ghost"], c["dx"]
+    dt, steps = 0.25 * dx, 2
+    u0 = c["state"]()
+    h = binding.Chemora(n, n, n, g, 8, binding.SYS_WAVE, dx)
+    h.set_param("eps_diss", c["eps_diss"])
+    h.set_state(u0)
+    h.autotune()
+    for _ in range(steps):
+        h.rk4_step(dt)
+    got = h.get_state()
+    h.destroy()
+    rng = np.random.default_rng(8)
+    centres = [(0, 0, 0), (255, 0, 128)] + [tuple(int(x) for x in rng.integers(0, n, 3)) for _ in range(3)]
+    check_samples(oracle, oracle.SYS_WAVE, u0, got, centres, reach=16 * steps, core=4, g=g, order=8, dx=dx, dt=dt,
+                  prm=oracle.params(eps_diss=c["eps_diss"]), steps=steps, tol=1e-12 * steps)
