@@ -30,8 +30,12 @@ UNIT = "grid-point updates/s"
 # Y,S,U writes U (100): 425 doubles = 3400 B per grid-point update, i.e. 850 B per RHS-kernel launch and point.
 BYTES_PER_UPDATE = 3400.0
 BYTES_PER_POINT_PER_LAUNCH = BYTES_PER_UPDATE / 4.0
-# counted with the paper's convention -- see DESIGN.md
-FLOPS_PER_RHS_POINT = 4460.0
+# FP64 work the fused kernel executes per point and RHS evaluation: 1591 DADD + 656 DMUL + 2 x 1130 DFMA (SASS of the
+# middle-stage instance).  An upper bound on the paper's convention.
+FLOPS_PER_RHS_POINT = 4507.0
+# dram__bytes_read.sum + dram__bytes_write.sum of the fused kernel at 256^3, mean over the 4 launches of an RK4 step
+# (ncu --set full, profiles/r01_c_fused_ncu_full.md); None for other variants / sizes
+NCU_TRAFFIC_BYTES_256 = 18.17e9
 
 
 def peaks():
@@ -230,9 +234,10 @@ def run_ours(args):
                    "variant": {"fused": fused, "tile": list(binding.tile_shape(tile, binding.SYS_BSSN, fused)), "sweep_ms": sweep_ms},
                    "kernel": info, "multi_gpu": "replicas only",
                    "l2": "inputs larger than L2 (%.2f GB per state buffer vs 126 MB)" % (h.nvars * h.var_stride * 8 / 1e9)},
-        "roofline": {"bound": "hbm", "kernel": "bssn_tma_kernel" if fused else "bssn_derivs+from_derivs",
+        "roofline": {"bound": "hbm", "kernel": ("bssn_ws_kernel" if tile >= 6 else "bssn_tma_kernel") if fused else "bssn_derivs+from_derivs",
                      "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
-                     "traffic": None, "peak_source": pk_src, "ms_per_launch": rhs_launch_ms,
+                     "traffic": NCU_TRAFFIC_BYTES_256 if (fused and tile < 6 and n == 256) else None, "traffic_unit": "bytes per launch (ncu)",
+                     "algorithmic_bytes_per_launch": BYTES_PER_POINT_PER_LAUNCH * n ** 3, "peak_source": pk_src, "ms_per_launch": rhs_launch_ms,
                      "share_of_step": kt["rhs_ms"] / ms, "fill_share_of_step": kt["fill_ms"] / ms},
         "roofline_fp64": {"bound": "alu", "achieved": gf, "peak": fp64_gf, "unit": "GFLOP/s",
                           "frac": gf / fp64_gf if fp64_gf else None, "flops_per_rhs_point": FLOPS_PER_RHS_POINT,
@@ -247,6 +252,37 @@ def run_ours(args):
     print(json.dumps(line))
 
 
+def run_sweep(args):
+    """configs[4]: fused vs split x tile ids on 96^3, 160^3, 200x200x400 (Minkowski + 1e-10 noise): ms per RHS
+    evaluation (one middle RK4 stage, timed by chemora_autotune), updates/s, registers, algorithmic HBM GB/s."""
+    import torch
+    from paper_1307_6488_b200 import binding, inputs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device and no CPU fallback")
+    table = []
+    for (nx, ny, nz) in inputs.SWEEP_GRIDS:
+        h = binding.Chemora(nx, ny, nz, 3, 4, binding.SYS_BSSN, 0.05)
+        h.set_param("eps_diss", 0.1)
+        h.set_state(inputs.bssn_noise(nx, ny, nz))
+        fused, tile, ms = h.autotune()
+        for f in (1, 0):
+            for t in range(binding.NUM_TILES):
+                m = ms[f * binding.NUM_TILES + t]
+                if m <= 0 or (f == 0 and t >= 6):
+                    continue
+                h.set_variant(f, t)
+                info = h.kernel_info()
+                npts = nx * ny * nz
+                bytes_pt = BYTES_PER_POINT_PER_LAUNCH + (0 if f else 2176.0)   # split: 136 arrays written + read
+                table.append({"grid": [nx, ny, nz], "fused": f, "tile_id": t,
+                              "tile": list(binding.tile_shape(t, binding.SYS_BSSN, f)), "ms_per_rhs": round(m, 4),
+                              "updates_per_s": npts / (4 * m * 1e-3), "regs": info["regs"],
+                              "spill_bytes": info["local_bytes"], "hbm_gbs_algorithmic": bytes_pt * npts / (m * 1e-3) / 1e9,
+                              "best": (f, t) == (fused, tile)})
+        h.destroy()
+    print(json.dumps({"metric": "BSSN RHS variant sweep (configs[4])", "unit": "ms per RHS evaluation", "rows": table}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -258,8 +294,11 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-sample", type=int, default=64)
     ap.add_argument("--ref-sample", type=int, default=64)
+    ap.add_argument("--sweep", action="store_true", help="configs[4] variant/tile sweep instead of the headline run")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
