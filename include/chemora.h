@@ -46,7 +46,7 @@ enum { CHEMORA_SYS_WAVE = 0, CHEMORA_SYS_BSSN = 1 };
 enum { CHEMORA_BUF_U = 0, CHEMORA_BUF_YA = 1, CHEMORA_BUF_YB = 2, CHEMORA_BUF_S = 3 };
 
 /* kernel variant axes (PAPER.md:215-216 fused vs derivative-split; :248-266 tile shape) */
-enum { CHEMORA_NUM_TILES = 9 };
+enum { CHEMORA_NUM_TILES = 11 };
 
 /* Create a handle for an nx x ny x nz interior block with `ghost` ghost layers per face, centred FD order
  * fd_order (4 or 8), system system_id and grid spacing dx (same in x, y, z).
@@ -103,8 +103,10 @@ int chemora_rk4_step(chemora_t* h, double dt);
  * [0, CHEMORA_NUM_TILES).  chemora_tile_shape reports the (x, y, z) extent of a tile id: for the fused BSSN
  * kernel a 3-D tile with one grid point per thread (staged with a 3-cell halo by TMA); ids 0..5 are six
  * shapes of the uniform kernel (every warp does the same work), ids 6..8 the warp-specialised kernel
- * (8 point warps + 4 stencil warps per CTA) on the shapes of ids 0, 1 and 4.  For the split BSSN kernels and
- * the wave kernel a tile is an x*y thread block marching z planes; there ids 6..8 repeat ids 0..2. */
+ * (8 point warps + 4 stencil warps per CTA) on the shapes of ids 0, 1 and 4, ids 9..10 the uniform kernel on
+ * 384-point tiles (12 warps per CTA at 168 registers, long-lived per-point values parked in tensor memory).
+ * For the split BSSN kernels and the wave kernel a tile is an x*y thread block marching z planes; there an id
+ * >= 6 repeats id - 6. */
 int chemora_set_variant(chemora_t* h, int fused, int tile_id);
 int chemora_get_variant(const chemora_t* h, int* fused, int* tile_id);
 int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, int* tz);

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libchemora.so")
 
 SYS_WAVE, SYS_BSSN = 0, 1
 BUF_U, BUF_YA, BUF_YB, BUF_S = 0, 1, 2, 3
-NUM_TILES = 9
+NUM_TILES = 11
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 
 # every symbol include/chemora.h declares (tests check that the library exports all of them)

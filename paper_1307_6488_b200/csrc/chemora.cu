@@ -113,7 +113,7 @@ int run_rhs_inner(chemora_t* h, const Stage& st) {
     CK(h, launch_wave(h->L, C, h->order, h->tile % 6, st, h->stream), "wave kernel launch");
     h->launches += 1;
   } else if (h->fused) {
-    if (h->tile >= 6) CK(h, launch_bssn_ws(h->L, C, h->tile - 6, st, h->stream), "bssn warp-specialised kernel launch");
+    if (h->tile >= 6 && h->tile < 9) CK(h, launch_bssn_ws(h->L, C, h->tile - 6, st, h->stream), "bssn warp-specialised kernel launch");
     else CK(h, launch_bssn_fused(h->L, C, h->tile, st, h->stream), "bssn fused kernel launch");
     h->launches += 1;
   } else {
@@ -419,7 +419,7 @@ int chemora_kernel_info(const chemora_t* h, int* regs, int* local_bytes, int* sm
   cudaFuncAttributes a;
   cudaError_t e = h->system == CHEMORA_SYS_WAVE ? kernel_info_wave(h->order, h->tile % 6, &a)
                   : !h->fused              ? kernel_info_bssn_split(1, h->tile % 6, &a)
-                  : h->tile >= 6           ? kernel_info_bssn_ws(h->tile - 6, &a)
+                  : h->tile >= 6 && h->tile < 9 ? kernel_info_bssn_ws(h->tile - 6, &a)
                                            : kernel_info_bssn_fused(h->tile, &a);
   if (e != cudaSuccess) return cuda_fail(const_cast<chemora_t*>(h), e, "cudaFuncGetAttributes");
   if (regs) *regs = a.numRegs;

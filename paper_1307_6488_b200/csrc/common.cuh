@@ -108,9 +108,10 @@ __device__ __forceinline__ void stage_emit_t(const Stage& st, long q, double k, 
 // Tile shapes of the variant sweep.  Fused kernel: 3-D tile, one point per thread.  Split kernels and the wave
 // kernel: x,y = thread block, z = planes marched per block.
 struct TileShape { int tx, ty, tz; };
-// ids 6..8: the warp-specialised fused kernel (kernels_bssn_ws.cu) on the three 256-point shapes
-static const TileShape kTilesFused[9] = {{16, 4, 4}, {16, 8, 2}, {8, 8, 4}, {8, 4, 8}, {16, 2, 8}, {16, 4, 2},
-                                         {16, 4, 4}, {16, 8, 2}, {16, 2, 8}};
+// ids 6..8: the warp-specialised fused kernel (kernels_bssn_ws.cu) on the three 256-point shapes;
+// ids 9..10: the uniform kernel on 384-point tiles (12 warps, live values parked in tensor memory)
+static const TileShape kTilesFused[11] = {{16, 4, 4}, {16, 8, 2}, {8, 8, 4}, {8, 4, 8}, {16, 2, 8}, {16, 4, 2},
+                                          {16, 4, 4}, {16, 8, 2}, {16, 2, 8}, {16, 4, 6}, {16, 6, 4}};
 static const TileShape kTilesMarch[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64, 4, 8}, {128, 2, 8}, {16, 16, 8}};
 
 // launchers implemented in the kernel translation units; each returns the cudaError_t of the launch

@@ -14,13 +14,20 @@
 #ifndef CHM_TWOPASS
 #define CHM_TWOPASS 0   // mixed second derivatives as D_x(D_y f), D_x(D_z f), D_y(D_z f) through shared memory
 #endif
+#ifndef CHM_PAIR
+#define CHM_PAIR 0      // evaluate the stencils of 3 (beta^i) / 2 (gt_ij) staged boxes in one block: more independent
+#endif                  // LDS and FP64 chains in flight per warp while few values are live (early sections)
+#ifndef CHM_TMEM
+#define CHM_TMEM 0      // park long-lived per-point values (the 18 Christoffel symbols) in tensor memory
+#endif
 #ifndef CHM_L2HINT
 #define CHM_L2HINT 1
 #endif
 
 namespace chm {
 
-constexpr int kSlots = 5;   // 25 variables % 5 == 0: the slot of a variable is the same in every tile
+// box ring: 5 slots for the 256-point tiles (25 variables % 5 == 0: the slot of a variable is the same in every
+// tile), 4 for the 384-point tiles (shared memory), where slot and parity follow from the load number 25 t + o
 // point ("centre") values staged per tile: variables 0..13 (chi, gt, K, At) and 17..23 (alpha, beta, B)
 constexpr int kCenVars = 21;
 __device__ __forceinline__ constexpr int cen_index(int v) { return v < 14 ? v : v - 3; }
@@ -37,6 +44,9 @@ struct TmaCfg {
   static constexpr int SLOT = (BX * BY * BZ + 15) / 16 * 16;          // doubles, 128-byte multiple
   static constexpr uint32_t BOX_BYTES = (uint32_t)BX * BY * BZ * 8u;
   static constexpr int THREADS = TX * TY * TZ;
+  static constexpr bool HEAVY = THREADS > 256;    // 12 warps at 168 registers: live values parked in tensor memory
+  static constexpr int NS = HEAVY ? 4 : 5;        // ring slots
+  static constexpr bool PARK = HEAVY || CHM_TMEM;
   static constexpr int TILE = (TX + 2) * TY * TZ;                      // doubles in one (TX+2,TY,TZ) tile box
   static constexpr uint32_t TILE_BYTES = (uint32_t)TILE * 8u;
   static constexpr int SLOTX = SLOT + 4 * TILE;   // box + RK4 operands (U,S) of up to two emitted variables
@@ -46,9 +56,8 @@ struct TmaCfg {
   static constexpr int DYX = TX + 4;
   static constexpr int DY_N = DYX * TY * TZ, DZ_N = DYX * (TY + 4) * TZ;
   static constexpr int DB = CHM_TWOPASS ? (DY_N + DZ_N + 15) / 16 * 16 : 0;
-  static constexpr size_t SMEM = (size_t)(kSlots * SLOTX + CEN + 2 * DB) * 8 + (kSlots + 1) * 8 + (kSlots + 1) * 4 + 128;
+  static constexpr size_t SMEM = (size_t)(NS * SLOTX + CEN + 2 * DB) * 8 + (NS + 1) * 8 + (NS + 1) * 4 + 64 + 16 + 64 + 128;
   static constexpr int NWARPS = THREADS / 32;
-  static_assert((NWARPS & (NWARPS - 1)) == 0, "release counters wrap modulo 2^32");
 };
 
 template <int TX, int TY, int TZ, int MODE>
@@ -59,6 +68,10 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
   using Cfg = TmaCfg<TX, TY, TZ>;
   constexpr int BX = Cfg::BX, BY = Cfg::BY, SLOT = Cfg::SLOT, SLOTX = Cfg::SLOTX, TILE = Cfg::TILE, CEN = Cfg::CEN;
   constexpr unsigned NW = Cfg::NWARPS;
+  constexpr int kSlots = Cfg::NS;
+  constexpr bool PARK = Cfg::PARK;
+  // parking map (offsets in doubles inside the thread's 84-double area)
+  constexpr int P_CU = 0, P_DG = 18, P_DB = 42, P_LG = 52, P_AT = 58, P_ADG = 64, P_GN = 68, P_DCA = 72, P_AU = 78;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double* sm = reinterpret_cast<double*>(smem_raw);   // dynamic smem base: 128-byte aligned (no static smem)
   double* cbuf = sm + kSlots * SLOTX;                                  // [kCenVars][TILE]
@@ -84,7 +97,21 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
-  __syncthreads();
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(cnt + kSlots + 1);
+  int* org = reinterpret_cast<int*>((reinterpret_cast<uintptr_t>(tmem_slot + 1) + 15) & ~uintptr_t(15));   // [4][4]
+  uint32_t park = 0;   // this thread's parking area in tensor memory: its lane, 168 columns (84 doubles)
+  if constexpr (PARK) {
+    if (tid < 32) {   // warp 0 allocates all 512 columns (one CTA per SM)
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    park = *tmem_slot + ((uint32_t)(32 * ((tid >> 5) & 3)) << 16) + (uint32_t)((tid >> 7) * 168);
+  } else {
+    __syncthreads();
+  }
 
   // tile order (see the file header): idx -> (bx, by, bz)
   auto decode = [&](int idx, int& bx, int& by, int& bz) {
@@ -96,9 +123,20 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     const int ry = r / ntx;
     by = c * cy + ry; bx = r - ry * ntx;
   };
+  // Origins (padded coordinates minus halo) of this CTA's tiles t and t+1 live in a 4-entry shared-memory ring
+  // (entry t & 3: x0, y0, z0, valid), written one tile ahead by lane 0 of every warp (identical values), so the
+  // refill path needs no registers for them.  Warps drift less than one tile apart, so entries t, t+1 are stable.
+  auto put_origin = [&](int e, int tl) {
+    int b0 = 0, b1 = 0, b2 = 0;
+    const bool ok = tl < ntiles;
+    if (ok) decode(tl, b0, b1, b2);
+    if (lane == 0) {
+      int4 v = make_int4(b0 * TX + goffx, b1 * TY + goff, b2 * TZ + goff, ok ? 1 : 0);
+      *reinterpret_cast<int4*>(org + 4 * (e & 3)) = v;
+    }
+  };
   // box of variable order o of the tile whose origin (padded, minus halo) is (x0,y0,z0); issued by one thread
-  auto issue = [&](int o, int x0, int y0, int z0) {
-    const int slot = o % kSlots;
+  auto issue = [&](int o, int slot, int x0, int y0, int z0) {
     double* dst = sm + slot * SLOTX;
     const int v0 = emit_var(o, 0), v1 = emit_var(o, 1);
     const int nem = (v0 >= 0) + (v1 >= 0);
@@ -125,24 +163,37 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     __syncwarp();
     bool last = false;
     if (lane == 0) {
-      last = (smem_add_relaxed(&cnt[b], 1u) & (NW - 1)) == NW - 1;
+      last = (smem_add_relaxed(&cnt[b], 1u) + 1u) % NW == 0u;
     }
     return last;
   };
+  put_origin(0, blockIdx.x);
+  __syncthreads();
   if (tid == 0 && (int)blockIdx.x < ntiles) {
-    int bx, by, bz;
-    decode(blockIdx.x, bx, by, bz);
-    const int x0 = bx * TX + goffx, y0 = by * TY + goff, z0 = bz * TZ + goff;
+    const int x0 = org[0], y0 = org[1], z0 = org[2];
     issue_cen(x0, y0, z0);
 #pragma unroll
-    for (int o = 0; o < kSlots; ++o) issue(o, x0, y0, z0);
+    for (int o = 0; o < kSlots; ++o) issue(o, o, x0, y0, z0);
   }
 
   int t = 0;
   for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++t) {
-    int bx, by, bz;
-    decode(tile, bx, by, bz);
-    const int i = bx * TX + lx, j = by * TY + ly, k = bz * TZ + lz;
+    // 256-point tiles have the registers to keep this tile's and the next tile's origin (measured faster);
+    // 384-point tiles read them from the shared-memory ring where a refill is issued
+    int4 own, nxt = make_int4(0, 0, 0, 0);
+    if constexpr (Cfg::HEAVY) {
+      own = *reinterpret_cast<const int4*>(org + 4 * (t & 3));
+      put_origin(t + 1, tile + gridDim.x);
+    } else {
+      int b0, b1, b2;
+      decode(tile, b0, b1, b2);
+      own = make_int4(b0 * TX + goffx, b1 * TY + goff, b2 * TZ + goff, 1);
+      if (tile + (int)gridDim.x < ntiles) {
+        decode(tile + gridDim.x, b0, b1, b2);
+        nxt = make_int4(b0 * TX + goffx, b1 * TY + goff, b2 * TZ + goff, 1);
+      }
+    }
+    const int i = own.x - goffx + lx, j = own.y - goff + ly, k = own.z - goff + lz;
     const bool valid = i < L.nx && j < L.ny && k < L.nz;
     const long q = (long)((valid ? k : 0) + L.g) * L.plane + (long)((valid ? j : 0) + L.g) * L.pitch +
                    ((valid ? i : 0) + L.xo);
@@ -151,8 +202,11 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     auto cen = [&](int v) { return cb[cen_index(v) * TILE]; };
     // RK4 stage operands (U, S) of the n-th variable emitted by section o: staged by TMA next to the box;
     // read after box(o) and before done(o)
+    // ring slot and mbarrier parity of section o of this CTA's t-th tile (load number 25 t + o)
+    auto slot_of = [&](int o) { return kSlots == 5 ? o % 5 : (t + o) & 3; };
+    auto parity_of = [&](int o) { return (uint32_t)(kSlots == 5 ? (t + o / 5) & 1 : ((25 * t + o) >> 2) & 1); };
     auto pre = [&](int o, int n) {
-      const double* op = sm + (o % kSlots) * SLOTX + SLOT + 2 * n * TILE + toff;
+      const double* op = sm + slot_of(o) * SLOTX + SLOT + 2 * n * TILE + toff;
       return StagePre{op[0], op[TILE]};
     };
     auto emit = [&](int v, double k, const StagePre& pr) { if (valid) stage_emit_t<MODE>(st, q + v * L.vstride, k, pr); };
@@ -160,25 +214,23 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     // section o: wait for its box, hand out the accessor; done(o): this warp leaves the slot; the last warp to
     // leave refills it with the box 5 loads ahead (of this tile, or of this CTA's next tile)
     auto box = [&](int o) {
-      mbar_wait(&full[o % kSlots], (uint32_t)((t + o / kSlots) & 1));
-      return BoxPoint<BX, BY>{sm + (o % kSlots) * SLOTX + coff};
+      mbar_wait(&full[slot_of(o)], parity_of(o));
+      return BoxPoint<BX, BY>{sm + slot_of(o) * SLOTX + coff};
     };
-    const bool has_next = tile + (int)gridDim.x < ntiles;
-    int nx0 = 0, ny0 = 0, nz0 = 0;           // origin of this CTA's next tile
-    if (has_next) {
-      int b0, b1, b2;
-      decode(tile + gridDim.x, b0, b1, b2);
-      nx0 = b0 * TX + goffx; ny0 = b1 * TY + goff; nz0 = b2 * TZ + goff;
-    }
     auto done = [&](int o) {
-      if (leave(o % kSlots)) {
-        if (o + kSlots < 25) issue(o + kSlots, bx * TX + goffx, by * TY + goff, bz * TZ + goff);
-        else if (has_next) issue(o + kSlots - 25, nx0, ny0, nz0);
+      if (leave(slot_of(o))) {   // the refill is load number 25 t + o + kSlots: same slot
+        const int4 a = !Cfg::HEAVY ? (o + kSlots < 25 ? own : nxt)
+                                   : *reinterpret_cast<const int4*>(org + 4 * ((o + kSlots < 25 ? t : t + 1) & 3));
+        if (o + kSlots < 25) issue(o + kSlots, slot_of(o), a.x, a.y, a.z);
+        else if (a.w) issue(o + kSlots - 25, slot_of(o), a.x, a.y, a.z);
       }
     };
     // the point values are last read just before section 3 (At)
     auto done_cen = [&]() {
-      if (leave(kSlots) && has_next) issue_cen(nx0, ny0, nz0);
+      if (leave(kSlots)) {
+        const int4 a = !Cfg::HEAVY ? nxt : *reinterpret_cast<const int4*>(org + 4 * ((t + 1) & 3));
+        if (a.w) issue_cen(a.x, a.y, a.z);
+      }
     };
 
     // all derivatives of a "full" variable (section o, n-th full variable of the tile), then done(o).
@@ -249,6 +301,31 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 
     // ---- o = 0..2: beta^i : d_j beta^i, gtu^{jk} d_j d_k beta^i, d_j (d_k beta^k) ----------------------------
     double db[3][3], lapb[3], gdiv[3];   // db[j][i] = d_j beta^i ; gdiv[j] = d_j d_k beta^k
+#if CHM_PAIR && !CHM_TWOPASS
+    {
+      double d1[3][3], d2[3][6], ad[3], Bc[3];
+      StagePre pr[3];
+#pragma unroll
+      for (int i2 = 0; i2 < 3; ++i2) Bc[i2] = cen(V_B + i2);
+      const BoxPoint<BX, BY> p0 = box(0), p1 = box(1), p2 = box(2);
+#pragma unroll
+      for (int i2 = 0; i2 < 3; ++i2) pr[i2] = pre(i2, 0);
+      var_full(p0, C, w, d1[0], d2[0], ad[0]);
+      var_full(p1, C, w, d1[1], d2[1], ad[1]);
+      var_full(p2, C, w, d1[2], d2[2], ad[2]);
+      done(0); done(1); done(2);
+#pragma unroll
+      for (int i2 = 0; i2 < 3; ++i2) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+          db[a][i2] = d1[i2][a];
+          gdiv[a] = i2 == 0 ? d2[i2][sym(a, i2)] : gdiv[a] + d2[i2][sym(a, i2)];
+        }
+        lapb[i2] = sdot(gu, d2[i2]);
+        emit(V_BETA + i2, C.sgc * Bc[i2] + ad[i2], pr[i2]);
+      }
+    }
+#else
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2) {
       const double Bc = cen(V_B + i2);
@@ -261,13 +338,44 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       lapb[i2] = sdot(gu, d2);
       emit(V_BETA + i2, C.sgc * Bc + ad, pr);
     }
-    const double divb = (db[0][0] + db[1][1]) + db[2][2];
+#endif
+    double divb = (db[0][0] + db[1][1]) + db[2][2];
+    if constexpr (PARK) {   // needed again only by the Gt^i right-hand side (sections 21..23)
+      const double lg[6] = {lapb[0], lapb[1], lapb[2], gdiv[0], gdiv[1], gdiv[2]};
+      tmem_park<6>(park, P_LG, lg);
+    }
 
     // ---- o = 3..8: gt_ij : d_k gt_ij kept for the Christoffels, gtu^{lm} d_l d_m gt_ij folded into R~_ij ---
     double At[6], Rt[6], dg[3][6];
 #pragma unroll
     for (int s = 0; s < 6; ++s) At[s] = cen(V_AT + s);
     done_cen();
+#if CHM_PAIR && !CHM_TWOPASS
+#pragma unroll
+    for (int pp = 0; pp < 3; ++pp) {
+      constexpr int I2[6] = {0, 0, 0, 1, 1, 2}, J2[6] = {0, 1, 2, 1, 2, 2};   // packed index -> (i, j)
+      const int sa = 2 * pp, sb = 2 * pp + 1;
+      const BoxPoint<BX, BY> pa = box(3 + sa), pb = box(3 + sb);
+      const StagePre pra = pre(3 + sa, 0), prb = pre(3 + sb, 0);
+      double d1[2][3], d2[2][6], ad[2];
+      var_full(pa, C, w, d1[0], d2[0], ad[0]);
+      var_full(pb, C, w, d1[1], d2[1], ad[1]);
+      done(3 + sa); done(3 + sb);
+#pragma unroll
+      for (int h2 = 0; h2 < 2; ++h2) {
+        const int s = 2 * pp + h2, i2 = I2[s], j2 = J2[s];
+        dg[0][s] = d1[h2][0]; dg[1][s] = d1[h2][1]; dg[2][s] = d1[h2][2];
+        Rt[s] = -0.5 * sdot(gu, d2[h2]);
+        double lie;
+#pragma unroll
+        for (int k2 = 0; k2 < 3; ++k2) {
+          const double c = g[sym(i2, k2)] * db[j2][k2] + g[sym(j2, k2)] * db[i2][k2];
+          lie = k2 == 0 ? c : lie + c;
+        }
+        emit(V_GT + s, (lie - two_thirds * g[s] * divb) - 2.0 * alpha * At[s] + ad[h2], h2 == 0 ? pra : prb);
+      }
+    }
+#else
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2)
 #pragma unroll
@@ -277,7 +385,12 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
         const StagePre pr = pre(3 + s, 0);
         double d1[3], d2[6], ad;
         full_var(p, w, 3 + s, 3 + s, d1, d2, ad);
-        dg[0][s] = d1[0]; dg[1][s] = d1[1]; dg[2][s] = d1[2];
+        if constexpr (PARK) {
+          const double d4[4] = {d1[0], d1[1], d1[2], 0.0};
+          tmem_park<4>(park, P_DG + 4 * s, d4);
+        } else {
+          dg[0][s] = d1[0]; dg[1][s] = d1[1]; dg[2][s] = d1[2];
+        }
         Rt[s] = -0.5 * sdot(gu, d2);
         double lie;
 #pragma unroll
@@ -288,9 +401,22 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
         emit(V_GT + s, (lie - two_thirds * g[s] * divb) - 2.0 * alpha * At[s] + ad, pr);
       }
 
+#endif
+
     // ---- Christoffels: Cl[k][s(i,j)] = Gamma~_kij, Cu[k][s] = Gamma~^k_ij, Gn[k] = gtu^{ij} Gamma~^k_ij ----
     double Cu[3][6], Gn[3];
     {
+      if constexpr (PARK) {   // make room: d_j beta^i and At_ij rest in tensor memory until the At_ij sections
+        const double t10[10] = {db[0][0], db[0][1], db[0][2], db[1][0], db[1][1], db[1][2], db[2][0], db[2][1], db[2][2], divb};
+        tmem_park<10>(park, P_DB, t10);
+        tmem_park<6>(park, P_AT, At);
+#pragma unroll
+        for (int s = 0; s < 6; ++s) {
+          double d4[4];
+          tmem_unpark<4>(park, P_DG + 4 * s, d4);
+          dg[0][s] = d4[0]; dg[1][s] = d4[1]; dg[2][s] = d4[2];
+        }
+      }
       double Cl[3][6];
 #pragma unroll
       for (int k2 = 0; k2 < 3; ++k2)
@@ -299,35 +425,24 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 #pragma unroll
           for (int j2 = i2; j2 < 3; ++j2)
             Cl[k2][sym(i2, j2)] = 0.5 * ((dg[i2][sym(k2, j2)] + dg[j2][sym(k2, i2)]) - dg[k2][sym(i2, j2)]);
-#pragma unroll
-      for (int k2 = 0; k2 < 3; ++k2) {
-#pragma unroll
-        for (int s = 0; s < 6; ++s)
-          Cu[k2][s] = gu[sym(k2, 0)] * Cl[0][s] + gu[sym(k2, 1)] * Cl[1][s] + gu[sym(k2, 2)] * Cl[2][s];
-        Gn[k2] = sdot(gu, Cu[k2]);
-      }
       // R~_ij += 1/2 Gamma~^k_n (Gamma~_ijk + Gamma~_jik)
       //        + gtu^{lm} (Gamma~^k_li Gamma~_jkm + Gamma~^k_lj Gamma~_ikm + Gamma~^k_im Gamma~_klj)
       // with the inverse metric contracted once: W[i][m] = gtu^{lm} Gamma~^k_li (per k), so the three products are
-      //   sum_m W[i][m] Gamma~_jkm + W[j][m] Gamma~_ikm   and   sum_l W[i][l] Gamma~_klj
-#pragma unroll
-      for (int i2 = 0; i2 < 3; ++i2)
-#pragma unroll
-        for (int j2 = i2; j2 < 3; ++j2) {
-          const double c = (Gn[0] * (Cl[i2][sym(j2, 0)] + Cl[j2][sym(i2, 0)]) +
-                            Gn[1] * (Cl[i2][sym(j2, 1)] + Cl[j2][sym(i2, 1)])) +
-                           Gn[2] * (Cl[i2][sym(j2, 2)] + Cl[j2][sym(i2, 2)]);
-          Rt[sym(i2, j2)] += 0.5 * c;
-        }
+      //   sum_m W[i][m] Gamma~_jkm + W[j][m] Gamma~_ikm   and   sum_l W[i][l] Gamma~_klj.
+      // One k at a time, so that only Gamma~^k_ij of that k is live next to Gamma~_kij.
 #pragma unroll
       for (int k2 = 0; k2 < 3; ++k2) {
+        double Ck[6];
+#pragma unroll
+        for (int s = 0; s < 6; ++s)
+          Ck[s] = gu[sym(k2, 0)] * Cl[0][s] + gu[sym(k2, 1)] * Cl[1][s] + gu[sym(k2, 2)] * Cl[2][s];
+        Gn[k2] = sdot(gu, Ck);
         double W[3][3];
 #pragma unroll
         for (int i2 = 0; i2 < 3; ++i2)
 #pragma unroll
           for (int m = 0; m < 3; ++m)
-            W[i2][m] = gu[sym(0, m)] * Cu[k2][sym(0, i2)] + gu[sym(1, m)] * Cu[k2][sym(1, i2)] +
-                       gu[sym(2, m)] * Cu[k2][sym(2, i2)];
+            W[i2][m] = gu[sym(0, m)] * Ck[sym(0, i2)] + gu[sym(1, m)] * Ck[sym(1, i2)] + gu[sym(2, m)] * Ck[sym(2, i2)];
 #pragma unroll
         for (int i2 = 0; i2 < 3; ++i2)
 #pragma unroll
@@ -338,9 +453,27 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
             else acc += t1 + (W[j2][0] * Cl[i2][sym(k2, 0)] + W[j2][1] * Cl[i2][sym(k2, 1)] + W[j2][2] * Cl[i2][sym(k2, 2)]);
             Rt[sym(i2, j2)] += acc;
           }
+        if constexpr (PARK) tmem_park<6>(park, P_CU + 6 * k2, Ck);
+        else {
+#pragma unroll
+          for (int s = 0; s < 6; ++s) Cu[k2][s] = Ck[s];
+        }
       }
+#pragma unroll
+      for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+        for (int j2 = i2; j2 < 3; ++j2) {
+          const double c = (Gn[0] * (Cl[i2][sym(j2, 0)] + Cl[j2][sym(i2, 0)]) +
+                            Gn[1] * (Cl[i2][sym(j2, 1)] + Cl[j2][sym(i2, 1)])) +
+                           Gn[2] * (Cl[i2][sym(j2, 2)] + Cl[j2][sym(i2, 2)]);
+          Rt[sym(i2, j2)] += 0.5 * c;
+        }
     }
 
+    if constexpr (PARK) {
+      const double g4[4] = {Gn[0], Gn[1], Gn[2], 0.0};
+      tmem_park<4>(park, P_GN, g4);
+    }
     // ---- o = 9..11: Gt^k : R~_ij += 1/2 (gt_ki d_j Gt^k + gt_kj d_i Gt^k); advection kept for the end ------
     double adG[3];
 #pragma unroll
@@ -355,6 +488,10 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
         for (int j2 = i2; j2 < 3; ++j2)
           Rt[sym(i2, j2)] += 0.5 * (g[sym(k2, i2)] * d1[j2] + g[sym(k2, j2)] * d1[i2]);
     }
+    if constexpr (PARK) {
+      const double a4[4] = {adG[0], adG[1], adG[2], 0.0};
+      tmem_park<4>(park, P_ADG, a4);
+    }
 
     // ---- o = 12: chi : R_ij = R~_ij + R^chi_ij --------------------------------------------------------------
     const double ichi = 1.0 / chi;
@@ -366,12 +503,23 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       full_var(p, w, 12, 9, dchi, d2, ad);
       emit(V_CHI, two_thirds * chi * (alpha * trK - divb) + ad, pr);
       double cd[6], cc[6];   // D~_i D~_j chi ; d_i chi d_j chi
+      if constexpr (PARK) {   // Gamma~^k_ij one k at a time from tensor memory
+#pragma unroll
+        for (int s = 0; s < 6; ++s) cd[s] = d2[s];
+#pragma unroll
+        for (int k2 = 0; k2 < 3; ++k2) {
+          double Ck[6];
+          tmem_unpark<6>(park, P_CU + 6 * k2, Ck);
+#pragma unroll
+          for (int s = 0; s < 6; ++s) cd[s] -= Ck[s] * dchi[k2];
+        }
+      }
 #pragma unroll
       for (int a = 0; a < 3; ++a)
 #pragma unroll
         for (int b = a; b < 3; ++b) {
           const int s = sym(a, b);
-          cd[s] = d2[s] - (Cu[0][s] * dchi[0] + Cu[1][s] * dchi[1] + Cu[2][s] * dchi[2]);
+          if constexpr (!PARK) cd[s] = d2[s] - (Cu[0][s] * dchi[0] + Cu[1][s] * dchi[1] + Cu[2][s] * dchi[2]);
           cc[s] = dchi[a] * dchi[b];
         }
       const double trcd = sdot(gu, cd), trcc = sdot(gu, cc);
@@ -389,12 +537,23 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       full_var(p, w, 13, 10, dal, d2, ad);
       emit(V_ALPHA, -2.0 * alpha * trK + ad, pr);
       double cd[6], ca[6];   // d_i d_j alpha - Gamma~^k_ij d_k alpha ; d_i chi d_j alpha + d_j chi d_i alpha
+      if constexpr (PARK) {
+#pragma unroll
+        for (int s = 0; s < 6; ++s) cd[s] = d2[s];
+#pragma unroll
+        for (int k2 = 0; k2 < 3; ++k2) {
+          double Ck[6];
+          tmem_unpark<6>(park, P_CU + 6 * k2, Ck);
+#pragma unroll
+          for (int s = 0; s < 6; ++s) cd[s] -= Ck[s] * dal[k2];
+        }
+      }
 #pragma unroll
       for (int a = 0; a < 3; ++a)
 #pragma unroll
         for (int b = a; b < 3; ++b) {
           const int s = sym(a, b);
-          cd[s] = d2[s] - (Cu[0][s] * dal[0] + Cu[1][s] * dal[1] + Cu[2][s] * dal[2]);
+          if constexpr (!PARK) cd[s] = d2[s] - (Cu[0][s] * dal[0] + Cu[1][s] * dal[1] + Cu[2][s] * dal[2]);
           ca[s] = dchi[a] * dal[b] + dchi[b] * dal[a];
         }
       const double trcd = sdot(gu, cd), trca = 0.5 * sdot(gu, ca);   // trca = gtu^{kl} d_k chi d_l alpha
@@ -403,9 +562,14 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 #pragma unroll
       for (int s = 0; s < 6; ++s) Rt[s] = alpha * Rt[s] - (cd[s] + h2 * (ca[s] - g[s] * trca));   // Rt now holds X_ij
     }
+    if constexpr (PARK) {   // d_i chi, d_i alpha: next used by the Gt^i right-hand side
+      const double dc[6] = {dchi[0], dchi[1], dchi[2], dal[0], dal[1], dal[2]};
+      tmem_park<6>(park, P_DCA, dc);
+    }
 
     // ---- extrinsic curvature with raised indices -------------------------------------------------------------
     double Am[3][3], Au[6];   // At^i_j ; At^{ij}
+    if constexpr (PARK) tmem_unpark<6>(park, P_AT, At);
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2)
 #pragma unroll
@@ -427,8 +591,18 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       done(14);
       emit(V_K, (alpha * (sdot(Au, At) + third * trK * trK) - lap_alpha) + ad, pr);
     }
+    if constexpr (PARK) tmem_park<6>(park, P_AU, Au);
 
     // ---- o = 15..20: At_ij -------------------------------------------------------------------------------------
+    if constexpr (PARK) {
+      double t10[10];
+      tmem_unpark<10>(park, P_DB, t10);
+#pragma unroll
+      for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) db[a][b] = t10[3 * a + b];
+      divb = t10[9];
+    }
     {
       const double trX = sdot(gu, Rt);
 #pragma unroll
@@ -453,6 +627,19 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     }
 
     // ---- o = 21..23: B^i, together with Gt^i ---------------------------------------------------------------------
+    if constexpr (PARK) {
+      double lg[6], a4[4];
+      tmem_unpark<6>(park, P_LG, lg);
+      tmem_unpark<4>(park, P_ADG, a4);
+#pragma unroll
+      for (int a = 0; a < 3; ++a) { lapb[a] = lg[a]; gdiv[a] = lg[3 + a]; adG[a] = a4[a]; }
+      double g4[4], dc[6];
+      tmem_unpark<4>(park, P_GN, g4);
+      tmem_unpark<6>(park, P_DCA, dc);
+      tmem_unpark<6>(park, P_AU, Au);
+#pragma unroll
+      for (int a = 0; a < 3; ++a) { Gn[a] = g4[a]; dchi[a] = dc[a]; dal[a] = dc[3 + a]; }
+    }
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2) {
       auto p = box(21 + i2);
@@ -461,6 +648,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       const double adB = var_ad(p, w);
       done(21 + i2);
       double r = lapb[i2];
+      if constexpr (PARK) tmem_unpark<6>(park, P_CU + 6 * i2, &Cu[i2][0]);
       double t2 = sdot(Cu[i2], Au);   // Gamma~^i_jk At^{jk}
 #pragma unroll
       for (int j2 = 0; j2 < 3; ++j2) {
@@ -482,6 +670,11 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       done(24);
       emit(V_A, C.ko * qsum, pr);
     }
+  }
+  if constexpr (PARK) {
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(*tmem_slot) : "memory");
   }
 }
 
@@ -570,6 +763,8 @@ static cudaError_t tma_dispatch(int tile, const Layout& L, const Coef& C, const 
     case 3: return tma_go<8, 4, 8>(L, C, st, s, a);
     case 4: return tma_go<16, 2, 8>(L, C, st, s, a);
     case 5: return tma_go<16, 4, 2>(L, C, st, s, a);
+    case 9: return tma_go<16, 4, 6>(L, C, st, s, a);     // 12 warps, 168 registers, tensor-memory parking
+    case 10: return tma_go<16, 6, 4>(L, C, st, s, a);
   }
   return cudaErrorInvalidValue;
 }

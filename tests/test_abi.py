@@ -30,9 +30,9 @@ def test_exports_every_declared_symbol(binding):
 def test_tile_table(binding):
     shapes = [binding.tile_shape(t, binding.SYS_BSSN, 0) for t in range(binding.NUM_TILES)]
     assert shapes[:6] == [(32, 4, 8), (32, 8, 8), (64, 2, 8), (64, 4, 8), (128, 2, 8), (16, 16, 8)]
-    assert shapes[6:] == shapes[:3]                                   # ids 6..8 repeat 0..2 for marching kernels
+    assert shapes[6:] == [shapes[t % 6] for t in range(6, binding.NUM_TILES)]                                   # ids >= 6 repeat id - 6 for marching kernels
     fused = [binding.tile_shape(t, binding.SYS_BSSN, 1) for t in range(binding.NUM_TILES)]
-    assert all(x * y * z in (128, 256) for x, y, z in fused)      # one grid point per thread
+    assert all(x * y * z in (128, 256, 384) for x, y, z in fused)      # one grid point per thread
     with pytest.raises(binding.ChemoraError):
         binding.tile_shape(binding.NUM_TILES)
 
