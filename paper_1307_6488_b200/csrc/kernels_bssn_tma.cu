@@ -12,8 +12,8 @@
 #define CHM_BLOCKSYNC 0
 #endif
 #ifndef CHM_TWOPASS
-#define CHM_TWOPASS 0   // mixed second derivatives as D_x(D_y f), D_x(D_z f), D_y(D_z f) through shared memory
-#endif
+#define CHM_TWOPASS 1   // mixed second derivatives as D_x(D_y f), D_x(D_z f), D_y(D_z f) through shared memory, on the
+#endif                  // tiles whose z-planes are one or two warps (plane-local barrier); 2 = on every 256-point tile
 #ifndef CHM_PAIR
 #define CHM_PAIR 0      // evaluate the stencils of 3 (beta^i) / 2 (gt_ij) staged boxes in one block: more independent
 #endif                  // LDS and FP64 chains in flight per warp while few values are live (early sections)
@@ -55,7 +55,8 @@ struct TmaCfg {
   // D_y f on the tile + 2 columns of x-halo, D_z f on the tile + 2 columns of x-halo + 2 rows of y-halo
   static constexpr int DYX = TX + 4;
   static constexpr int DY_N = DYX * TY * TZ, DZ_N = DYX * (TY + 4) * TZ;
-  static constexpr int DB = CHM_TWOPASS ? (DY_N + DZ_N + 15) / 16 * 16 : 0;
+  static constexpr bool TWOPASS = !HEAVY && (CHM_TWOPASS == 2 || (CHM_TWOPASS == 1 && (TX * TY == 64 || TX * TY == 32)));
+  static constexpr int DB = TWOPASS ? (DY_N + DZ_N + 15) / 16 * 16 : 0;
   static constexpr size_t SMEM = (size_t)(NS * SLOTX + CEN + 2 * DB) * 8 + (NS + 1) * 8 + (NS + 1) * 4 + 64 + 16 + 64 + 128;
   static constexpr int NWARPS = THREADS / 32;
 };
@@ -238,7 +239,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     // the block adds them on the 2-cell x-halo (and D_z f on the 2-cell y-halo), and after one block barrier
     // d_xy = D_x(D_y f), d_xz = D_x(D_z f), d_yz = D_y(D_z f) cost 4 reads each instead of 16.
     auto full_var = [&](const BoxPoint<BX, BY>& p, const AdvW& w, int o, int n, double* d1, double* d2, double& ad) {
-#if CHM_TWOPASS
+      if constexpr (Cfg::TWOPASS) {
       constexpr int DYX = Cfg::DYX, ZS = BX * BY;
       const double f0 = p.at(0, 0, 0);
       axis_full(p, f0, 0, C, w, d1[0], d2[0], ad);
@@ -250,30 +251,84 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       Dy[(lz * TY + ly) * DYX + lx + 2] = d1[1];
       Dz[(lz * (TY + 4) + ly + 2) * DYX + lx + 2] = d1[2];
       const double* sb = p.c - coff;   // slot base
+      if constexpr (TX * TY == 64) {
+        // One z-plane of the tile = 64 threads = two warps, and every first derivative a thread reads below comes
+        // from its own plane: the plane's two warps fill the plane's halo entries and meet at a 64-thread named
+        // barrier instead of a block barrier.
+        for (int u = tid & 63; u < TX * 4; u += 64) {                    // D_z f on the y-halo rows -2,-1,TY,TY+1
+          const int hx = u % TX, hyi = u / TX;
+          const int yy = hyi < 2 ? hyi - 2 : TY + hyi - 2;
+          const double* c = sb + ((lz + 3) * BY + (yy + 3)) * BX + hx + 3;
+          Dz[(lz * (TY + 4) + yy + 2) * DYX + hx + 2] = (8.0 * (c[ZS] - c[-ZS]) - (c[2 * ZS] - c[-2 * ZS])) * c12;
+        }
+        // D_y f, D_z f on the 4 x-halo columns: 8 * TY evaluations per plane, done by one of the plane's two
+        // warps, chosen so that every scheduler (warp w runs on scheduler w % 4) gets the same share
+        if ((tid >> 5) == 2 * lz + (((lz + 1) >> 1) & 1)) {
+          for (int l = lane; l < 8 * TY; l += 32) {
+            const int kind = l / (4 * TY), hh = l % (4 * TY);
+            const int hxi = hh % 4, hy = hh / 4;
+            const int xx = hxi < 2 ? hxi - 2 : TX + hxi - 2;
+            const double* c = sb + ((lz + 3) * BY + (hy + 3)) * BX + xx + 3;
+            const int st1 = kind == 0 ? BX : ZS;
+            const double v = (8.0 * (c[st1] - c[-st1]) - (c[2 * st1] - c[-2 * st1])) * c12;
+            if (kind == 0) Dy[(lz * TY + hy) * DYX + xx + 2] = v;
+            else Dz[(lz * (TY + 4) + hy + 2) * DYX + xx + 2] = v;
+          }
+        }
+        done(o);
+        asm volatile("bar.sync %0, 64;" ::"r"(1 + lz) : "memory");
+      } else if constexpr (TX * TY == 32) {
+        // One z-plane of the tile = one warp: the warp fills its own plane's halo entries; no barrier at all.
+#pragma unroll
+        for (int e = 0; e < (TX * 4) / 32; ++e) {                         // D_z f on the y-halo rows
+          const int u = lane + 32 * e, hx = u % TX, hyi = u / TX;
+          const int yy = hyi < 2 ? hyi - 2 : TY + hyi - 2;
+          const double* c = sb + ((lz + 3) * BY + (yy + 3)) * BX + hx + 3;
+          Dz[(lz * (TY + 4) + yy + 2) * DYX + hx + 2] = (8.0 * (c[ZS] - c[-ZS]) - (c[2 * ZS] - c[-2 * ZS])) * c12;
+        }
+        if (lane < 8 * TY) {                                              // D_y f, D_z f on the 4 x-halo columns
+          const int kind = lane / (4 * TY), hh = lane % (4 * TY);
+          const int hxi = hh % 4, hy = hh / 4;
+          const int xx = hxi < 2 ? hxi - 2 : TX + hxi - 2;
+          const double* c = sb + ((lz + 3) * BY + (hy + 3)) * BX + xx + 3;
+          const int st1 = kind == 0 ? BX : ZS;
+          const double v = (8.0 * (c[st1] - c[-st1]) - (c[2 * st1] - c[-2 * st1])) * c12;
+          if (kind == 0) Dy[(lz * TY + hy) * DYX + xx + 2] = v;
+          else Dz[(lz * (TY + 4) + hy + 2) * DYX + xx + 2] = v;
+        }
+        done(o);
+        __syncwarp();
+      } else {
       for (int h = tid; h < TX * 4 * TZ; h += Cfg::THREADS) {          // D_z f on the y-halo rows -2,-1,TY,TY+1
         const int hx = h % TX, hyi = (h / TX) % 4, hz = h / (TX * 4);
         const int yy = hyi < 2 ? hyi - 2 : TY + hyi - 2;
         const double* c = sb + ((hz + 3) * BY + (yy + 3)) * BX + hx + 3;
         Dz[(hz * (TY + 4) + yy + 2) * DYX + hx + 2] = (8.0 * (c[ZS] - c[-ZS]) - (c[2 * ZS] - c[-2 * ZS])) * c12;
       }
-      for (int h = tid; h < 4 * TY * TZ; h += Cfg::THREADS) {          // D_y f, D_z f on the x-halo columns
-        const int hxi = h % 4, hy = (h / 4) % TY, hz = h / (4 * TY);
+      // D_y f and D_z f on the 4 x-halo columns: 2 * 4 * TY * TZ single evaluations, spread over the first
+      // warps so that every scheduler (warp w runs on scheduler w % 4) gets the same share
+      for (int h = tid; h < 8 * TY * TZ; h += Cfg::THREADS) {
+        const int kind = h / (4 * TY * TZ), hh = h - kind * (4 * TY * TZ);
+        const int hxi = hh % 4, hy = (hh / 4) % TY, hz = hh / (4 * TY);
         const int xx = hxi < 2 ? hxi - 2 : TX + hxi - 2;
         const double* c = sb + ((hz + 3) * BY + (hy + 3)) * BX + xx + 3;
-        Dy[(hz * TY + hy) * DYX + xx + 2] = (8.0 * (c[BX] - c[-BX]) - (c[2 * BX] - c[-2 * BX])) * c12;
-        Dz[(hz * (TY + 4) + hy + 2) * DYX + xx + 2] = (8.0 * (c[ZS] - c[-ZS]) - (c[2 * ZS] - c[-2 * ZS])) * c12;
+        const int st1 = kind == 0 ? BX : ZS;
+        const double v = (8.0 * (c[st1] - c[-st1]) - (c[2 * st1] - c[-2 * st1])) * c12;
+        if (kind == 0) Dy[(hz * TY + hy) * DYX + xx + 2] = v;
+        else Dz[(hz * (TY + 4) + hy + 2) * DYX + xx + 2] = v;
       }
       done(o);
       __syncthreads();
+      }
       const double* y = Dy + (lz * TY + ly) * DYX + lx + 2;
       const double* z = Dz + (lz * (TY + 4) + ly + 2) * DYX + lx + 2;
       d2[1] = (8.0 * (y[1] - y[-1]) - (y[2] - y[-2])) * c12;
       d2[2] = (8.0 * (z[1] - z[-1]) - (z[2] - z[-2])) * c12;
       d2[4] = (8.0 * (z[DYX] - z[-DYX]) - (z[2 * DYX] - z[-2 * DYX])) * c12;
-#else
-      var_full(p, C, w, d1, d2, ad);
-      done(o);
-#endif
+      } else {
+        var_full(p, C, w, d1, d2, ad);
+        done(o);
+      }
     };
 
     const double third = 1.0 / 3.0, two_thirds = 2.0 / 3.0;
@@ -301,7 +356,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 
     // ---- o = 0..2: beta^i : d_j beta^i, gtu^{jk} d_j d_k beta^i, d_j (d_k beta^k) ----------------------------
     double db[3][3], lapb[3], gdiv[3];   // db[j][i] = d_j beta^i ; gdiv[j] = d_j d_k beta^k
-#if CHM_PAIR && !CHM_TWOPASS
+#if CHM_PAIR && CHM_TWOPASS == 0
     {
       double d1[3][3], d2[3][6], ad[3], Bc[3];
       StagePre pr[3];
@@ -350,7 +405,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 #pragma unroll
     for (int s = 0; s < 6; ++s) At[s] = cen(V_AT + s);
     done_cen();
-#if CHM_PAIR && !CHM_TWOPASS
+#if CHM_PAIR && CHM_TWOPASS == 0
 #pragma unroll
     for (int pp = 0; pp < 3; ++pp) {
       constexpr int I2[6] = {0, 0, 0, 1, 1, 2}, J2[6] = {0, 1, 2, 1, 2, 2};   // packed index -> (i, j)
