@@ -30,12 +30,12 @@ UNIT = "grid-point updates/s"
 # Y,S,U writes U (100): 425 doubles = 3400 B per grid-point update, i.e. 850 B per RHS-kernel launch and point.
 BYTES_PER_UPDATE = 3400.0
 BYTES_PER_POINT_PER_LAUNCH = BYTES_PER_UPDATE / 4.0
-# FP64 work the fused kernel executes per point and RHS evaluation: 1591 DADD + 656 DMUL + 2 x 1130 DFMA (SASS of the
-# middle-stage instance).  An upper bound on the paper's convention.
-FLOPS_PER_RHS_POINT = 4507.0
+# FP64 work the fused kernel executes per point and RHS evaluation: 1365 DADD + 671 DMUL + 2 x 1026 DFMA (SASS of the
+# middle-stage instance of the default tile).  An upper bound on the paper's convention.
+FLOPS_PER_RHS_POINT = 4088.0
 # dram__bytes_read.sum + dram__bytes_write.sum of the fused kernel at 256^3, mean over the 4 launches of an RK4 step
-# (ncu --set full, profiles/r01_c_fused_ncu_full.md); None for other variants / sizes
-NCU_TRAFFIC_BYTES_256 = 18.17e9
+# (ncu --set full, profiles/r01_d_fused_ncu_full.md); None for other variants / sizes
+NCU_TRAFFIC_BYTES_256 = 18.25e9
 
 
 def peaks():
@@ -132,7 +132,7 @@ def run_reference(args):
 def run_ours(args):
     import numpy as np
     import torch
-    from paper_1307_6488_b200 import binding, inputs
+    from paper_1307_6488_b200 import binding, inputs, replicas
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -154,7 +154,7 @@ def run_ours(args):
     c = inputs.config(3, scale=n)
     g, dx = c["ghost"], c["dx"]
     dt = 0.25 * dx
-    u0 = inputs.bssn_gaussians(n, n, n, seed=inputs.SEED_BASE + 3 + rank)   # one replica per rank
+    u0 = inputs.bssn_gaussians(n, n, n, seed=replicas.replica_seed(inputs.SEED_BASE + 3, rank))   # one replica per rank
     h = binding.Chemora(n, n, n, g, c["order"], binding.SYS_BSSN, dx, device="cuda:%d" % local)
     h.set_param("eps_diss", c["eps_diss"])
     host = torch.from_numpy(u0).pin_memory()
@@ -188,11 +188,8 @@ def run_ours(args):
     kt = h.timing_read()
     h.timing(0)
     clocks = sampler.stop() if rank == 0 else None
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
-    value = world * n ** 3 * args.steps / (ms * 1e-3)
+    value, worst = replicas.aggregate_throughput(ms * 1e-3, n ** 3 * args.steps, dist, "cuda")   # max over ranks
+    ms = worst * 1e3
 
     # ---- end to end through the C ABI with HOST buffers: H2D + K' steps... per step: set_state, rk4_step, get_state
     e2e_steps = max(1, min(args.e2e_steps, args.steps))
@@ -206,10 +203,7 @@ def run_ours(args):
         h.get_state(out.numpy())
     barrier()
     e2e_s = time.perf_counter() - t0
-    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_val = world * n ** 3 * e2e_steps / float(t.item())
+    e2e_val, _ = replicas.aggregate_throughput(e2e_s, n ** 3 * e2e_steps, dist, "cuda")
     nbytes = host.numel() * 8
 
     fp64_gf = h.measure_fp64_peak() if rank == 0 else None
