@@ -58,6 +58,16 @@ __device__ __forceinline__ void tma_load_4d_hint(void* dst, const CUtensorMap* t
       " [%0], [%1, {%3, %4, %5, %6}], [%2], %7;"
       ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z), "r"(v), "l"(policy) : "memory");
 }
+// One arrival on a "buffer released" mbarrier (expected count = number of warps); true if it was the last one of the
+// phase (the state returned by arrive is the one before this arrival: one arrival pending = ours).  Release semantics
+// order the warp's earlier reads of the buffer before the arrival; no MEMBAR is generated (SYNCS.ARRIVE).
+__device__ __forceinline__ bool mbar_arrive_is_last(uint64_t* bar) {
+  uint64_t state;
+  uint32_t pending;
+  asm volatile("mbarrier.arrive.shared::cta.b64 %0, [%1];" : "=l"(state) : "r"(smem_u32(bar)) : "memory");
+  asm volatile("mbarrier.pending_count.b64 %0, %1;" : "=r"(pending) : "l"(state));
+  return pending == 1;
+}
 // shared-memory counter increment, relaxed: no MEMBAR (an acq_rel atomic compiles to MEMBAR.ALL.CTA, which also
 // waits for the warp's outstanding global stores).  The ordering needed -- this warp's LDS reads of a buffer
 // before the increment -- comes from the SM executing one warp's shared-memory instructions in program order

@@ -91,17 +91,19 @@ __device__ __forceinline__ void stage_emit(const Stage& st, long q, double k, co
 
 // Same with the mode as a compile-time constant (no branches in the epilogue of the fused BSSN kernel).
 template <int MODE>
-__device__ __forceinline__ void stage_emit_t(const Stage& st, long q, double k, const StagePre& pr) {
+__device__ __forceinline__ void stage_emit_t(const Stage& st, long q, double k, const StagePre& pr, bool valid) {
+  // values first, stores under one predicate (no divergent region around the arithmetic)
   if (MODE == MODE_RHS) {
-    CHM_ST(&st.out[q], k);
+    if (valid) CHM_ST(&st.out[q], k);
   } else if (MODE == MODE_FIRST) {
-    CHM_ST(&st.S[q], k);
-    CHM_ST(&st.out[q], __dadd_rn(pr.u, __dmul_rn(st.a, k)));
+    const double y = __dadd_rn(pr.u, __dmul_rn(st.a, k));
+    if (valid) { CHM_ST(&st.S[q], k); CHM_ST(&st.out[q], y); }
   } else if (MODE == MODE_MID) {
-    CHM_ST(&st.S[q], __dadd_rn(pr.s, __dmul_rn(2.0, k)));
-    CHM_ST(&st.out[q], __dadd_rn(pr.u, __dmul_rn(st.a, k)));
+    const double s2 = __dadd_rn(pr.s, __dmul_rn(2.0, k)), y = __dadd_rn(pr.u, __dmul_rn(st.a, k));
+    if (valid) { CHM_ST(&st.S[q], s2); CHM_ST(&st.out[q], y); }
   } else {
-    CHM_ST(&st.U[q], __dadd_rn(pr.u, __dmul_rn(st.a, __dadd_rn(pr.s, k))));
+    const double u = __dadd_rn(pr.u, __dmul_rn(st.a, __dadd_rn(pr.s, k)));
+    if (valid) CHM_ST(&st.U[q], u);
   }
 }
 

@@ -57,7 +57,7 @@ struct TmaCfg {
   static constexpr int DY_N = DYX * TY * TZ, DZ_N = DYX * (TY + 4) * TZ;
   static constexpr bool TWOPASS = !HEAVY && (CHM_TWOPASS == 2 || (CHM_TWOPASS == 1 && (TX * TY == 64 || TX * TY == 32)));
   static constexpr int DB = TWOPASS ? (DY_N + DZ_N + 15) / 16 * 16 : 0;
-  static constexpr size_t SMEM = (size_t)(NS * SLOTX + CEN + 2 * DB) * 8 + (NS + 1) * 8 + (NS + 1) * 4 + 64 + 16 + 64 + 128;
+  static constexpr size_t SMEM = (size_t)(NS * SLOTX + CEN + 2 * DB) * 8 + (NS + 1) * 8 + (NS + 1) * 8 + 64 + 16 + 64 + 128;
   static constexpr int NWARPS = THREADS / 32;
 };
 
@@ -79,7 +79,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
   double* dbuf = cbuf + CEN;                                           // [2][DB] shared first derivatives
   uint64_t* full = reinterpret_cast<uint64_t*>(dbuf + 2 * Cfg::DB);    // [kSlots] boxes, then [1] point values
   uint64_t* cfull = full + kSlots;
-  unsigned* cnt = reinterpret_cast<unsigned*>(cfull + 1);              // [kSlots] + [1]: warps that left a buffer
+  uint64_t* empty = cfull + 1;                                         // [kSlots] + [1]: warps that left a buffer
   constexpr int nops = MODE == MODE_RHS ? 0 : (MODE == MODE_FIRST ? 1 : 2);   // RK4 operands per emitted var
   const int ntiles = ntx * nty * ntz;
 
@@ -94,11 +94,11 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < kSlots + 1; ++s) { mbar_init(&full[s], 1); cnt[s] = 0u; }
+    for (int s = 0; s < kSlots + 1; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NW); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(cnt + kSlots + 1);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(empty + kSlots + 1);
   int* org = reinterpret_cast<int*>((reinterpret_cast<uintptr_t>(tmem_slot + 1) + 15) & ~uintptr_t(15));   // [4][4]
   uint32_t park = 0;   // this thread's parking area in tensor memory: its lane, 168 columns (84 doubles)
   if constexpr (PARK) {
@@ -164,7 +164,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     __syncwarp();
     bool last = false;
     if (lane == 0) {
-      last = (smem_add_relaxed(&cnt[b], 1u) + 1u) % NW == 0u;
+      last = mbar_arrive_is_last(&empty[b]);
     }
     return last;
   };
@@ -210,7 +210,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       const double* op = sm + slot_of(o) * SLOTX + SLOT + 2 * n * TILE + toff;
       return StagePre{op[0], op[TILE]};
     };
-    auto emit = [&](int v, double k, const StagePre& pr) { if (valid) stage_emit_t<MODE>(st, q + v * L.vstride, k, pr); };
+    auto emit = [&](int v, double k, const StagePre& pr) { stage_emit_t<MODE>(st, q + v * L.vstride, k, pr, valid); };
 
     // section o: wait for its box, hand out the accessor; done(o): this warp leaves the slot; the last warp to
     // leave refills it with the box 5 loads ahead (of this tile, or of this CTA's next tile)
