@@ -8,7 +8,7 @@
 // See bssn_tma.cuh for the design; DESIGN.md "Kernels" for the roofline that bounds it.
 #include "bssn_tma.cuh"
 
-#ifndef CHM_BLOCKSYNC
+#ifndef CHM_BLOCKSYNC   // experiment switch: block barrier per variable instead of warp-wise slot release
 #define CHM_BLOCKSYNC 0
 #endif
 #ifndef CHM_TWOPASS
@@ -55,7 +55,7 @@ struct TmaCfg {
   // D_y f on the tile + 2 columns of x-halo, D_z f on the tile + 2 columns of x-halo + 2 rows of y-halo
   static constexpr int DYX = TX + 4;
   static constexpr int DY_N = DYX * TY * TZ, DZ_N = DYX * (TY + 4) * TZ;
-  static constexpr bool TWOPASS = !HEAVY && (CHM_TWOPASS == 2 || (CHM_TWOPASS == 1 && (TX * TY == 64 || TX * TY == 32)));
+  static constexpr bool TWOPASS = !HEAVY && (CHM_TWOPASS == 2 || (CHM_TWOPASS == 1 && (TX * TY == 64 || TX * TY == 32))   // 128-thread planes: measured no gain);
   static constexpr int DB = TWOPASS ? (DY_N + DZ_N + 15) / 16 * 16 : 0;
   static constexpr size_t SMEM = (size_t)(NS * SLOTX + CEN + 2 * DB) * 8 + (NS + 1) * 8 + (NS + 1) * 8 + 64 + 16 + 64 + 128;
   static constexpr int NWARPS = THREADS / 32;
@@ -251,32 +251,33 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       Dy[(lz * TY + ly) * DYX + lx + 2] = d1[1];
       Dz[(lz * (TY + 4) + ly + 2) * DYX + lx + 2] = d1[2];
       const double* sb = p.c - coff;   // slot base
-      if constexpr (TX * TY == 64) {
-        // One z-plane of the tile = 64 threads = two warps, and every first derivative a thread reads below comes
-        // from its own plane: the plane's two warps fill the plane's halo entries and meet at a 64-thread named
-        // barrier instead of a block barrier.
-        for (int u = tid & 63; u < TX * 4; u += 64) {                    // D_z f on the y-halo rows -2,-1,TY,TY+1
+      if constexpr (TX * TY == 64 || TX * TY == 128) {
+        // One z-plane of the tile = PLANE threads = two or four warps, and every first derivative a thread reads
+        // below comes from its own plane: the plane's warps fill the plane's halo entries and meet at a
+        // PLANE-thread named barrier instead of a block barrier.
+        constexpr int PLANE = TX * TY, WPP = PLANE / 32;
+        const int u0 = tid % PLANE;
+        for (int u = u0; u < TX * 4; u += PLANE) {                       // D_z f on the y-halo rows -2,-1,TY,TY+1
           const int hx = u % TX, hyi = u / TX;
           const int yy = hyi < 2 ? hyi - 2 : TY + hyi - 2;
           const double* c = sb + ((lz + 3) * BY + (yy + 3)) * BX + hx + 3;
           Dz[(lz * (TY + 4) + yy + 2) * DYX + hx + 2] = (8.0 * (c[ZS] - c[-ZS]) - (c[2 * ZS] - c[-2 * ZS])) * c12;
         }
-        // D_y f, D_z f on the 4 x-halo columns: 8 * TY evaluations per plane, done by one of the plane's two
-        // warps, chosen so that every scheduler (warp w runs on scheduler w % 4) gets the same share
-        if ((tid >> 5) == 2 * lz + (((lz + 1) >> 1) & 1)) {
-          for (int l = lane; l < 8 * TY; l += 32) {
-            const int kind = l / (4 * TY), hh = l % (4 * TY);
-            const int hxi = hh % 4, hy = hh / 4;
-            const int xx = hxi < 2 ? hxi - 2 : TX + hxi - 2;
-            const double* c = sb + ((lz + 3) * BY + (hy + 3)) * BX + xx + 3;
-            const int st1 = kind == 0 ? BX : ZS;
-            const double v = (8.0 * (c[st1] - c[-st1]) - (c[2 * st1] - c[-2 * st1])) * c12;
-            if (kind == 0) Dy[(lz * TY + hy) * DYX + xx + 2] = v;
-            else Dz[(lz * (TY + 4) + hy + 2) * DYX + xx + 2] = v;
-          }
+        // D_y f, D_z f on the 4 x-halo columns: 8 * TY evaluations per plane, started at a warp of the plane
+        // chosen so that every scheduler (warp w runs on scheduler w % 4) gets the same share
+        const int start = WPP == 2 ? (((lz + 1) >> 1) & 1) : (2 * lz) % WPP;
+        for (int l = (u0 - 32 * start + PLANE) % PLANE; l < 8 * TY; l += PLANE) {
+          const int kind = l / (4 * TY), hh = l % (4 * TY);
+          const int hxi = hh % 4, hy = hh / 4;
+          const int xx = hxi < 2 ? hxi - 2 : TX + hxi - 2;
+          const double* c = sb + ((lz + 3) * BY + (hy + 3)) * BX + xx + 3;
+          const int st1 = kind == 0 ? BX : ZS;
+          const double v = (8.0 * (c[st1] - c[-st1]) - (c[2 * st1] - c[-2 * st1])) * c12;
+          if (kind == 0) Dy[(lz * TY + hy) * DYX + xx + 2] = v;
+          else Dz[(lz * (TY + 4) + hy + 2) * DYX + xx + 2] = v;
         }
         done(o);
-        asm volatile("bar.sync %0, 64;" ::"r"(1 + lz) : "memory");
+        asm volatile("bar.sync %0, %1;" ::"r"(1 + lz), "n"(PLANE) : "memory");
       } else if constexpr (TX * TY == 32) {
         // One z-plane of the tile = one warp: the warp fills its own plane's halo entries; no barrier at all.
 #pragma unroll

@@ -11,12 +11,6 @@
 // stencil warps add a third warp to every scheduler without costing the point warps their registers, and take
 // 20 % of the instruction stream off them.  PAPER.md:268-270 ("fat kernels") is the problem this addresses.
 #include "bssn_tma.cuh"
-#ifndef CHM_WS_DBG
-#define CHM_WS_DBG 0
-#endif
-#ifndef CHM_WS_NOSETMAX
-#define CHM_WS_NOSETMAX 0
-#endif
 
 namespace chm {
 
@@ -149,12 +143,7 @@ bssn_ws_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ C
 
   if (!point_role) {
     // =============================== stencil warps: two grid points per thread ===============================
-#if !CHM_WS_NOSETMAX
     asm volatile("setmaxnreg.dec.sync.aligned.u32 72;");
-#endif
-#if CHM_WS_DBG == 4
-    return;
-#endif
     const int ptid = tid - NPT;
     int coffS[2], toffS[2];
 #pragma unroll
@@ -186,9 +175,6 @@ bssn_ws_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ C
           w[n].wq[a] = fabs(b) * (C.inv_h * (1.0 / 24.0)) + C.ko;
         }
       if (leave(cntC, 12u) && has_next) issue_cen(nx0, ny0, nz0);
-#if CHM_WS_DBG == 5
-      return;
-#endif
 
 #pragma unroll
       for (int ps = 0; ps < kNumS; ++ps) {
@@ -200,9 +186,6 @@ bssn_ws_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ C
         for (int n = 0; n < 2; ++n) {
           const BoxPoint<BX, BY> p{sm + (kRing + slot) * SLOT + coffS[n]};
           double* r = res + line0(o) * NPT + ptid + n * K::NPROD;
-#if CHM_WS_DBG == 1
-          r[0] = 0.0; continue;
-#endif
           if (o <= 14) {                       // Gt^k, K: centred first derivatives + advection/dissipation
             double d1[3], ad;
             var_d1_ad(p, C, w[n], d1, ad);
@@ -228,9 +211,7 @@ bssn_ws_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ C
   }
 
   // ================================= point warps: one grid point per thread =================================
-#if !CHM_WS_NOSETMAX
   asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
-#endif
   const int lx = tid % TX, ly = (tid / TX) % TY, lz = tid / (TX * TY);
   const int coff = ((lz + 3) * BY + (ly + 3)) * BX + lx + 3;
   const int toff = (lz * TY + ly) * (TX + 2) + lx + 1;   // this thread's point inside a tile box
@@ -250,18 +231,11 @@ bssn_ws_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ C
     auto pre = [&](int v) {
       StagePre pr{0.0, 0.0};
       const long qq = q + v * L.vstride;
-#if CHM_WS_DBG == 2
-      return pr;
-#endif
       if (st.mode == MODE_FIRST) pr.u = __ldg(st.in + qq);
       else if (st.mode != MODE_RHS) { pr.u = __ldcs(st.U + qq); pr.s = __ldcs(st.S + qq); }
       return pr;
     };
-#if CHM_WS_DBG == 3
-    auto emit = [&](int v, double kk, const StagePre& pr) { if (valid && kk == 1.2345e300) stage_emit(st, q + v * L.vstride, kk, pr); };
-#else
     auto emit = [&](int v, double kk, const StagePre& pr) { if (valid) stage_emit(st, q + v * L.vstride, kk, pr); };
-#endif
     auto box = [&](int o) {
       const int c = point_c(o), slot = c % kRing;
       mbar_wait(&fullP[slot], (uint32_t)((t * ring_uses(kNumP, slot) + c / kRing) & 1));
@@ -283,11 +257,7 @@ bssn_ws_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ C
       }
     };
     // results of a section evaluated by the stencil warps: wait for them / hand the lines back
-#if CHM_WS_DBG == 4
-    auto results = [&](int o) { return rs + line0(o) * NPT; };
-#else
     auto results = [&](int o) { mbar_wait(&rfull[ridx(o)], (uint32_t)(t & 1)); return rs + line0(o) * NPT; };
-#endif
     auto results_done = [&](int o) {
       __syncwarp();
       if (lane == 0) mbar_arrive(&rempty[ridx(o)]);
