@@ -45,7 +45,9 @@ struct TmaCfg {
   static constexpr uint32_t BOX_BYTES = (uint32_t)BX * BY * BZ * 8u;
   static constexpr int THREADS = TX * TY * TZ;
   static constexpr bool HEAVY = THREADS > 256;    // 12 warps at 168 registers: live values parked in tensor memory
-  static constexpr int NS = HEAVY ? 4 : 5;        // ring slots
+  // ring slots (a 6-slot ring fits the 16x4x4 tile but its run-time slot index costs more than the depth gains:
+  // 8.2 ms vs 6.3 ms)
+  static constexpr int NS = HEAVY ? 4 : 5;
   static constexpr bool PARK = HEAVY || CHM_TMEM;
   static constexpr int TILE = (TX + 2) * TY * TZ;                      // doubles in one (TX+2,TY,TZ) tile box
   static constexpr uint32_t TILE_BYTES = (uint32_t)TILE * 8u;
@@ -55,7 +57,8 @@ struct TmaCfg {
   // D_y f on the tile + 2 columns of x-halo, D_z f on the tile + 2 columns of x-halo + 2 rows of y-halo
   static constexpr int DYX = TX + 4;
   static constexpr int DY_N = DYX * TY * TZ, DZ_N = DYX * (TY + 4) * TZ;
-  static constexpr bool TWOPASS = !HEAVY && (CHM_TWOPASS == 2 || (CHM_TWOPASS == 1 && (TX * TY == 64 || TX * TY == 32))   // 128-thread planes: measured no gain);
+  // (planes of 128 threads: measured no gain over the one-pass form)
+  static constexpr bool TWOPASS = !HEAVY && (CHM_TWOPASS == 2 || (CHM_TWOPASS == 1 && (TX * TY == 64 || TX * TY == 32)));
   static constexpr int DB = TWOPASS ? (DY_N + DZ_N + 15) / 16 * 16 : 0;
   static constexpr size_t SMEM = (size_t)(NS * SLOTX + CEN + 2 * DB) * 8 + (NS + 1) * 8 + (NS + 1) * 8 + 64 + 16 + 64 + 128;
   static constexpr int NWARPS = THREADS / 32;
@@ -204,8 +207,8 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     // RK4 stage operands (U, S) of the n-th variable emitted by section o: staged by TMA next to the box;
     // read after box(o) and before done(o)
     // ring slot and mbarrier parity of section o of this CTA's t-th tile (load number 25 t + o)
-    auto slot_of = [&](int o) { return kSlots == 5 ? o % 5 : (t + o) & 3; };
-    auto parity_of = [&](int o) { return (uint32_t)(kSlots == 5 ? (t + o / 5) & 1 : ((25 * t + o) >> 2) & 1); };
+    auto slot_of = [&](int o) { return kSlots == 5 ? o % 5 : (25 * t + o) % kSlots; };
+    auto parity_of = [&](int o) { return (uint32_t)(kSlots == 5 ? (t + o / 5) & 1 : ((25 * t + o) / kSlots) & 1); };
     auto pre = [&](int o, int n) {
       const double* op = sm + slot_of(o) * SLOTX + SLOT + 2 * n * TILE + toff;
       return StagePre{op[0], op[TILE]};
