@@ -197,8 +197,8 @@ void fill_ghosts(double* f, const Grid& G) {
 // System 0 (reading S1): scalar wave equation, first order in time, V = 2: (phi, pi)
 //   d_t phi = pi (+ KO),   d_t pi = delta^{ij} d_i d_j phi (+ KO)
 // ---------------------------------------------------------------------------------------
-enum { SYS_WAVE = 0, SYS_BSSN = 1 };
-int nvars_of(int system) { return system == SYS_WAVE ? 2 : 25; }
+enum { SYS_WAVE = 0, SYS_BSSN = 1, SYS_WAVE1 = 2 };
+int nvars_of(int system) { return system == SYS_WAVE ? 2 : system == SYS_BSSN ? 25 : 5; }
 
 struct Params {
   double eps_diss;  // KO strength; 0 switches the KO term off (and its +-3 reads)
@@ -223,6 +223,35 @@ void wave_rhs(const double* state, double* rhs, const Grid& G, const Params& P) 
         }
         rhs[p] = rphi;
         rhs[n + p] = rpi;
+      }
+}
+
+// ---------------------------------------------------------------------------------------
+// System 2 ("Sample 1"): the scalar wave equation in fully first-order form,
+// V = 5: (u, rho, v_1, v_2, v_3), propagation speed 1:
+//   D_t u = rho ;  D_t rho = delta^{ij} D_i v_j ;  D_t v_i = D_i rho      (+ KO on every variable)
+// D_i = centred first derivative of the chosen order (reading S2).
+// ---------------------------------------------------------------------------------------
+void wave1_rhs(const double* state, double* rhs, const Grid& G, const Params& P) {
+  const long n = G.npts();
+  const double* u = state;
+  const double* rho = state + n;
+  const double* v[3] = {state + 2 * n, state + 3 * n, state + 4 * n};
+#pragma omp parallel for schedule(static)
+  for (int k = 0; k < G.nz; ++k)
+    for (int j = 0; j < G.ny; ++j)
+      for (int i = 0; i < G.nx; ++i) {
+        long p = idx(G, i, j, k);
+        double r[5];
+        r[0] = rho[p];
+        r[1] = (d1(v[0], G, i, j, k, 0) + d1(v[1], G, i, j, k, 1)) + d1(v[2], G, i, j, k, 2);
+        for (int a = 0; a < 3; ++a) r[2 + a] = d1(rho, G, i, j, k, a);
+        if (P.eps_diss != 0.0) {
+          r[0] += ko5(u, G, i, j, k, P.eps_diss);
+          r[1] += ko5(rho, G, i, j, k, P.eps_diss);
+          for (int a = 0; a < 3; ++a) r[2 + a] += ko5(v[a], G, i, j, k, P.eps_diss);
+        }
+        for (int c = 0; c < 5; ++c) rhs[c * n + p] = r[c];
       }
 }
 
@@ -477,6 +506,7 @@ void bssn_rhs(const double* state, double* rhs, const Grid& G, const Params& P) 
 
 void rhs_any(int system, const double* state, double* rhs, const Grid& G, const Params& P) {
   if (system == SYS_WAVE) wave_rhs(state, rhs, G, P);
+  else if (system == SYS_WAVE1) wave1_rhs(state, rhs, G, P);
   else bssn_rhs(state, rhs, G, P);
 }
 

@@ -14,8 +14,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "oracle.cpp")
 _LIB = os.path.join(_HERE, "liboracle.so")
 
-SYS_WAVE, SYS_BSSN = 0, 1
-NVARS = {SYS_WAVE: 2, SYS_BSSN: 25}
+SYS_WAVE, SYS_BSSN, SYS_WAVE1 = 0, 1, 2
+NVARS = {SYS_WAVE: 2, SYS_BSSN: 25, SYS_WAVE1: 5}
 OP_D1, OP_DD, OP_UPW, OP_KO = 0, 1, 2, 3
 
 _lib = None

@@ -13,7 +13,7 @@ import numpy as np
 
 SEED_BASE = 13076488
 
-SYS_WAVE, SYS_BSSN = 0, 1
+SYS_WAVE, SYS_BSSN, SYS_WAVE1 = 0, 1, 2
 
 # BSSN slot order (reading S3)
 BSSN_NAMES = ["chi", "gt11", "gt12", "gt13", "gt22", "gt23", "gt33", "trK",
@@ -64,6 +64,22 @@ def wave_plane_sum(nx, ny, nz, nwaves=8, seed=SEED_BASE + 1):
         pi -= w * np.cos(arg)
     out = np.empty((2, nz, ny, nx), dtype=np.float64)
     out[0], out[1] = phi, pi
+    return out
+
+
+WAVE1_NAMES = ["u", "rho", "v1", "v2", "v3"]
+
+
+def wave1_gaussian(nx, ny, nz, amp=1.0, width_cells=4.0):
+    """The paper's Sample-1 initial data: u = 0, rho = A exp(-1/2 (r/W)^2), v_i = 0, centred in the
+    unit periodic cube (minimum-image distance), W = width_cells grid spacings."""
+    out = np.zeros((5, nz, ny, nx), dtype=np.float64)
+    d = []
+    for n in (nz, ny, nx):
+        x = np.abs(np.arange(n, dtype=np.float64) - n / 2.0)
+        d.append(np.minimum(x, n - x))
+    r2 = d[0][:, None, None] ** 2 + d[1][None, :, None] ** 2 + d[2][None, None, :] ** 2
+    out[1] = amp * np.exp(-0.5 * r2 / width_cells ** 2)
     return out
 
 
