@@ -39,8 +39,10 @@ enum { CHEMORA_OK = 0, CHEMORA_EINVAL = -1, CHEMORA_ENOMEM = -2, CHEMORA_ECUDA =
 /* system_id.  WAVE: (phi, pi), d_t phi = pi, d_t pi = delta^ij d_i d_j phi (reading S1; PAPER.md:152-169 is
  * the paper's own wave example).  BSSN: 25 variables, chi-variant vacuum BSSN with 1+log
  * lapse and Gamma-driver shift (readings S3-S6), slots: chi, gt11 gt12 gt13 gt22 gt23 gt33, trK,
- * At11..At33, Gt1..3, alpha, beta1..3, B1..3, A. */
-enum { CHEMORA_SYS_WAVE = 0, CHEMORA_SYS_BSSN = 1 };
+ * At11..At33, Gt1..3, alpha, beta1..3, B1..3, A.  WAVE1: the paper's Sample 1 itself, the wave
+ * equation in fully first-order form, 5 variables (u, rho, v_1, v_2, v_3): D_t u = rho, D_t rho = delta^ij D_i v_j,
+ * D_t v_i = D_i rho, with centred first derivatives of order fd_order (needs ghost >= fd_order/2). */
+enum { CHEMORA_SYS_WAVE = 0, CHEMORA_SYS_BSSN = 1, CHEMORA_SYS_WAVE1 = 2 };
 
 /* which buffer of the four RK4 buffers (reading S9) */
 enum { CHEMORA_BUF_U = 0, CHEMORA_BUF_YA = 1, CHEMORA_BUF_YB = 2, CHEMORA_BUF_S = 3 };

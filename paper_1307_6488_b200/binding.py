@@ -13,7 +13,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libchemora.so")
 
-SYS_WAVE, SYS_BSSN = 0, 1
+SYS_WAVE, SYS_BSSN, SYS_WAVE1 = 0, 1, 2
 BUF_U, BUF_YA, BUF_YB, BUF_S = 0, 1, 2, 3
 NUM_TILES = 11
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4

@@ -112,6 +112,9 @@ int run_rhs_inner(chemora_t* h, const Stage& st) {
   if (h->system == CHEMORA_SYS_WAVE) {
     CK(h, launch_wave(h->L, C, h->order, h->tile % 6, st, h->stream), "wave kernel launch");
     h->launches += 1;
+  } else if (h->system == CHEMORA_SYS_WAVE1) {
+    CK(h, launch_wave1(h->L, C, h->order, h->tile % 6, st, h->stream), "first-order wave kernel launch");
+    h->launches += 1;
   } else if (h->fused) {
     if (h->tile >= 6 && h->tile < 9) CK(h, launch_bssn_ws(h->L, C, h->tile - 6, st, h->stream), "bssn warp-specialised kernel launch");
     else CK(h, launch_bssn_fused(h->L, C, h->tile, st, h->stream), "bssn fused kernel launch");
@@ -146,10 +149,10 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
   *out = nullptr;
   if (nx <= 0 || ny <= 0 || nz <= 0 || ghost < 0) return CHEMORA_EINVAL;
   if (fd_order != 4 && fd_order != 8) return CHEMORA_EINVAL;
-  if (system_id != CHEMORA_SYS_WAVE && system_id != CHEMORA_SYS_BSSN) return CHEMORA_EINVAL;
+  if (system_id != CHEMORA_SYS_WAVE && system_id != CHEMORA_SYS_BSSN && system_id != CHEMORA_SYS_WAVE1) return CHEMORA_EINVAL;
   if (!(dx > 0.0)) return CHEMORA_EINVAL;
   if ((alloc == nullptr) != (dealloc == nullptr)) return CHEMORA_EINVAL;
-  const int need = system_id == CHEMORA_SYS_WAVE ? fd_order / 2 : fd_order / 2 + 1;
+  const int need = system_id == CHEMORA_SYS_BSSN ? fd_order / 2 + 1 : fd_order / 2;
   if (ghost < need) return CHEMORA_EINVAL;
   if (nx < ghost || ny < ghost || nz < ghost) return CHEMORA_EINVAL;
   if (system_id == CHEMORA_SYS_BSSN && fd_order != 4) return CHEMORA_EINVAL;  // 8th-order BSSN: not built yet
@@ -158,7 +161,7 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
   if (!h) return CHEMORA_ENOMEM;
   Layout& L = h->L;
   L.nx = nx; L.ny = ny; L.nz = nz; L.g = ghost;
-  L.nvars = system_id == CHEMORA_SYS_WAVE ? 2 : 25;
+  L.nvars = system_id == CHEMORA_SYS_WAVE ? 2 : system_id == CHEMORA_SYS_WAVE1 ? 5 : 25;
   L.xo = (system_id == CHEMORA_SYS_BSSN && ((ghost - 3) & 1)) ? ghost + 1 : ghost;
   L.pitch = ((long)L.xo + nx + ghost + 15) / 16 * 16;
   L.tot_y = ny + 2 * ghost; L.tot_z = nz + 2 * ghost;
@@ -319,7 +322,7 @@ int chemora_rk4_step(chemora_t* h, double dt) {
 
 int chemora_set_variant(chemora_t* h, int fused, int tile_id) {
   if (!h || tile_id < 0 || tile_id >= CHEMORA_NUM_TILES || (fused != 0 && fused != 1)) return CHEMORA_EINVAL;
-  if (!fused && h->system == CHEMORA_SYS_WAVE) return fail(h, CHEMORA_EINVAL, "wave system has no split variant");
+  if (!fused && h->system != CHEMORA_SYS_BSSN) return fail(h, CHEMORA_EINVAL, "wave systems have no split variant");
   h->fused = fused;
   h->tile = tile_id;
   return CHEMORA_OK;
@@ -354,7 +357,7 @@ int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out)
   for (int f = 1; f >= 0 && !rc; --f)
     for (int t = 0; t < CHEMORA_NUM_TILES && !rc; ++t) {
       float ms = -1.f;
-      if (f == 1 || h->system == CHEMORA_SYS_BSSN) {
+      if ((f == 1 && (h->system == CHEMORA_SYS_BSSN || t < 6)) || (f == 0 && h->system == CHEMORA_SYS_BSSN && t < 6)) {
         h->fused = f; h->tile = t;
         // a middle RK4 stage (the common case) on scratch operands: k = f(U); S += 2k; Ya = U + a k.
         // S and Ya are scratch between steps (stage 1 overwrites them); U is only read.
@@ -418,6 +421,7 @@ int chemora_kernel_info(const chemora_t* h, int* regs, int* local_bytes, int* sm
   if (!h) return CHEMORA_EINVAL;
   cudaFuncAttributes a;
   cudaError_t e = h->system == CHEMORA_SYS_WAVE ? kernel_info_wave(h->order, h->tile % 6, &a)
+                  : h->system == CHEMORA_SYS_WAVE1 ? kernel_info_wave1(h->order, h->tile % 6, &a)
                   : !h->fused              ? kernel_info_bssn_split(1, h->tile % 6, &a)
                   : h->tile >= 6 && h->tile < 9 ? kernel_info_bssn_ws(h->tile - 6, &a)
                                            : kernel_info_bssn_fused(h->tile, &a);

@@ -120,6 +120,8 @@ static const TileShape kTilesMarch[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64
 cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s);
 cudaError_t launch_pack(const Layout& L, const double* packed, double* state, bool to_state, cudaStream_t s);
 cudaError_t launch_wave(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
+cudaError_t launch_wave1(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
+cudaError_t kernel_info_wave1(int order, int tile, cudaFuncAttributes* a);
 cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int tile, const Stage& st, cudaStream_t s);
 cudaError_t launch_bssn_ws(const Layout& L, const Coef& C, int which, const Stage& st, cudaStream_t s);
 cudaError_t kernel_info_bssn_ws(int which, cudaFuncAttributes* a);

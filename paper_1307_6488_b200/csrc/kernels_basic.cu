@@ -130,6 +130,76 @@ cudaError_t kernel_info_wave(int order, int tile, cudaFuncAttributes* a) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// First-order wave system of the paper's Sample 1, V = 5: (u, rho, v_1, v_2, v_3):
+//   D_t u = rho ;  D_t rho = delta^{ij} D_i v_j ;  D_t v_i = D_i rho   (+ KO on every variable)
+// Same launch shape as the (phi, pi) kernel: block = TX x TY threads marching TZ planes, loads through L1.
+// ---------------------------------------------------------------------------------------------------
+template <int ORDER, bool KO, int TX, int TY, int TZ>
+__global__ void __launch_bounds__(TX* TY) wave1_kernel(Layout L, Coef C, Stage st) {
+  const int i = blockIdx.x * TX + threadIdx.x, j = blockIdx.y * TY + threadIdx.y;
+  if (i >= L.nx || j >= L.ny) return;
+  const int k0 = blockIdx.z * TZ;
+#pragma unroll 1
+  for (int kk = 0; kk < TZ; ++kk) {
+    const int k = k0 + kk;
+    if (k >= L.nz) break;
+    const long q = (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.xo);
+    GlobalPoint P{st.in + q, L.pitch, L.plane, L.vstride};
+    auto d1 = [&](int v, int a) { return ORDER == 4 ? d1_o4(P, v, a, C.inv_h) : d1_o8(P, v, a, C.inv_h); };
+    double r[5];
+    r[0] = P.at(1, 0, 0, 0);
+    r[1] = (d1(2, 0) + d1(3, 1)) + d1(4, 2);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) r[2 + a] = d1(1, a);
+    if (KO) {
+#pragma unroll
+      for (int v = 0; v < 5; ++v) r[v] += ko5(P, v, C.ko);
+    }
+#pragma unroll
+    for (int v = 0; v < 5; ++v) stage_emit(st, q + v * L.vstride, r[v]);
+  }
+}
+
+template <int ORDER, bool KO, int TX, int TY, int TZ>
+static cudaError_t wave1_go(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
+  auto kern = wave1_kernel<ORDER, KO, TX, TY, TZ>;
+  if (a) return cudaFuncGetAttributes(a, kern);
+  dim3 grid((L.nx + TX - 1) / TX, (L.ny + TY - 1) / TY, (L.nz + TZ - 1) / TZ);
+  kern<<<grid, dim3(TX, TY), 0, s>>>(L, C, *st);
+  return cudaGetLastError();
+}
+
+template <int ORDER, bool KO>
+static cudaError_t wave1_tile(int tile, const Layout& L, const Coef& C, const Stage* st, cudaStream_t s,
+                              cudaFuncAttributes* a) {
+  switch (tile) {
+    case 0: return wave1_go<ORDER, KO, 32, 4, 8>(L, C, st, s, a);
+    case 1: return wave1_go<ORDER, KO, 32, 8, 8>(L, C, st, s, a);
+    case 2: return wave1_go<ORDER, KO, 64, 2, 8>(L, C, st, s, a);
+    case 3: return wave1_go<ORDER, KO, 64, 4, 8>(L, C, st, s, a);
+    case 4: return wave1_go<ORDER, KO, 128, 2, 8>(L, C, st, s, a);
+    case 5: return wave1_go<ORDER, KO, 16, 16, 8>(L, C, st, s, a);
+  }
+  return cudaErrorInvalidValue;
+}
+
+static cudaError_t wave1_dispatch(int order, bool ko, int tile, const Layout& L, const Coef& C, const Stage* st,
+                                  cudaStream_t s, cudaFuncAttributes* a) {
+  if (order == 4) return ko ? wave1_tile<4, true>(tile, L, C, st, s, a) : wave1_tile<4, false>(tile, L, C, st, s, a);
+  if (order == 8) return ko ? wave1_tile<8, true>(tile, L, C, st, s, a) : wave1_tile<8, false>(tile, L, C, st, s, a);
+  return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_wave1(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s) {
+  return wave1_dispatch(order, C.ko != 0.0, tile, L, C, &st, s, nullptr);
+}
+
+cudaError_t kernel_info_wave1(int order, int tile, cudaFuncAttributes* a) {
+  Layout L{}; Coef C{};
+  return wave1_dispatch(order, true, tile, L, C, nullptr, 0, a);
+}
+
+// ---------------------------------------------------------------------------------------------------
 // FP64 peak probe: 8 independent register-resident DFMA chains per thread.
 // flops = blocks * threads * iters * 8 chains * 2.
 // ---------------------------------------------------------------------------------------------------

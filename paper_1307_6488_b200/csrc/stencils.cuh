@@ -88,7 +88,17 @@ __device__ __forceinline__ double ko5(const P& f, int v, double ko) {
   return ko * ((ko5_axis(f, v, 0) + ko5_axis(f, v, 1)) + ko5_axis(f, v, 2));
 }
 
-// ---- 8th order (wave system) -------------------------------------------------------------------------
+// ---- 8th order (wave systems) ------------------------------------------------------------------------
+// 1st derivative (3,-32,168,-672,0,672,-168,32,-3)/840h
+template <class P>
+__device__ __forceinline__ double d1_o8(const P& f, int v, int a, double inv_h) {
+  double e1 = f.ax(v, a, 1) - f.ax(v, a, -1);
+  double e2 = f.ax(v, a, 2) - f.ax(v, a, -2);
+  double e3 = f.ax(v, a, 3) - f.ax(v, a, -3);
+  double e4 = f.ax(v, a, 4) - f.ax(v, a, -4);
+  return ((672.0 * e1 - 168.0 * e2) + (32.0 * e3 - 3.0 * e4)) * (inv_h * (1.0 / 840.0));
+}
+
 // 2nd derivative (-9,128,-1008,8064,-14350,8064,-1008,128,-9)/5040h^2
 template <class P>
 __device__ __forceinline__ double d2_o8(const P& f, int v, int a, double inv_h2) {

@@ -43,7 +43,8 @@ def test_tile_table(binding):
     (8, 8, 8, 3, 8, 0, 0.1),      # wave O8 needs g >= 4
     (8, 8, 8, 2, 4, 1, 0.1),      # BSSN O4 upwinded needs g >= 3 (PAPER.md:382 rule order/2+1)
     (8, 8, 8, 3, 6, 1, 0.1),      # order not in {4,8}
-    (8, 8, 8, 3, 4, 2, 0.1),      # unknown system
+    (8, 8, 8, 3, 4, 3, 0.1),      # unknown system
+    (8, 8, 8, 3, 8, 2, 0.1),      # first-order wave system O8 needs g >= 4
     (8, 8, 8, 3, 4, 1, 0.0),      # dx <= 0
     (2, 8, 8, 3, 4, 1, 0.1),      # dim < ghost
 ])

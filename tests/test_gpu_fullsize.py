@@ -92,3 +92,25 @@ def test_wave_config1_256_sampled(oracle):
     centres = [(0, 0, 0), (255, 0, 128)] + [tuple(int(x) for x in rng.integers(0, n, 3)) for _ in range(3)]
     check_samples(oracle, oracle.SYS_WAVE, u0, got, centres, reach=16 * steps, core=4, g=g, order=8, dx=dx, dt=dt,
                   prm=oracle.params(eps_diss=c["eps_diss"]), steps=steps, tol=1e-12 * steps)
+
+
+def test_wave1_256_sampled(oracle):
+    """The paper's Sample-1 system at 256^3, O8 + KO, Gaussian pulse of width 16 cells, 2 RK4 steps; 1e-12 per step."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1307_6488_b200 import binding
+    n, g, dx = 256, 4, 1.0 / 256
+    dt, steps = 0.25 * dx, 2
+    u0 = inputs.wave1_gaussian(n, n, n, width_cells=16.0)
+    h = binding.Chemora(n, n, n, g, 8, binding.SYS_WAVE1, dx)
+    h.set_param("eps_diss", 0.1)
+    h.set_state(u0)
+    h.autotune()
+    for _ in range(steps):
+        h.rk4_step(dt)
+    got = h.get_state()
+    h.destroy()
+    centres = [(128, 128, 128), (140, 128, 120), (0, 0, 0), (255, 130, 3), (110, 150, 128)]
+    check_samples(oracle, oracle.SYS_WAVE1, u0, got, centres, reach=16 * steps, core=4, g=g, order=8, dx=dx, dt=dt,
+                  prm=oracle.params(eps_diss=0.1), steps=steps, tol=1e-12 * steps)

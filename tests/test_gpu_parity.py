@@ -130,6 +130,37 @@ def test_wave_config1_shape_at_48(chem, oracle):
     h.destroy()
 
 
+# ------------------------------------------------------------------------- first-order wave system (Sample 1)
+@pytest.mark.parametrize("order,g,eps,dims", [(4, 2, 0.0, (37, 21, 19)), (8, 4, 0.1, (70, 33, 18)),
+                                              (4, 3, 0.1, (16, 16, 16)), (8, 4, 0.0, (33, 9, 12))])
+def test_wave1_rhs_all_tiles(chem, oracle, order, g, eps, dims):
+    nx, ny, nz = dims
+    u = np.random.default_rng(12).standard_normal((5, nz, ny, nx))
+    dx = 1.0 / 32
+    want = oracle_rhs(oracle, 2, u, g, order, dx, eps_diss=eps)
+    h = chem.Chemora(nx, ny, nz, g, order, chem.SYS_WAVE1, dx)
+    h.set_param("eps_diss", eps)
+    for tile in range(6):
+        h.set_variant(1, tile)
+        assert relerr(gpu_rhs(h, u), want) < TOL_RHS, tile
+    h.destroy()
+
+
+def test_wave1_gaussian_pulse_20_steps(chem, oracle):
+    """the paper's Sample-1 initial data (u = 0, rho = Gaussian, v = 0) at 32^3, O4, 20 RK4 steps"""
+    n, g, order = 32, 2, 4
+    u0 = inputs.wave1_gaussian(n, n, n)
+    dx = 1.0 / n
+    dt = 0.25 * dx
+    h = chem.Chemora(n, n, n, g, order, chem.SYS_WAVE1, dx)
+    h.set_state(u0)
+    for _ in range(20):
+        h.rk4_step(dt)
+    st = oracle.rk4(2, oracle.with_ghosts(u0, g), g, order, dx, dt, oracle.params(), 20)
+    assert relerr(h.get_state(), oracle.interior(st, g)) < TOL_WAVE_PER_STEP * 20
+    h.destroy()
+
+
 # ------------------------------------------------------------------------------------------------ BSSN
 def strong_field(nx, ny, nz, seed=21):
     """far-from-flat random data exercising every nonlinear term (gt = delta + 0.1 noise, etc.)."""
@@ -224,7 +255,9 @@ def test_autotune_and_kernel_info(chem):
     u = inputs.bssn_noise(n, n, n)
     h.set_state(u)
     fused, tile, ms = h.autotune()
-    assert fused in (0, 1) and 0 <= tile < chem.NUM_TILES and all(m > 0 for m in ms)
+    nt = chem.NUM_TILES
+    assert fused in (0, 1) and 0 <= tile < nt
+    assert all(m > 0 for m in ms[nt:]) and all(m > 0 for m in ms[:6])   # every fused id, the six split tiles
     assert (fused, tile) == h.get_variant()
     assert np.array_equal(h.get_state(), u)        # U is not modified by the sweep
     info = h.kernel_info()
