@@ -21,7 +21,9 @@
 // Pins (tests/test_oracle_*.py): polynomial exactness of every stencil (O1), the exact
 // discrete Fourier solution of the wave system (O2), convergence order (O3), flat stays
 // flat bitwise (O4), Kasner (O5), linearised BSSN (O6), Schwarzschild in isotropic (O7) and
-// Kerr-Schild (O8) coordinates.  "Parity unpinned" (conventions of this build that the
+// Kerr-Schild (O8) coordinates; for system 2 (the paper's Sample 1) the exact
+// discrete Fourier solution, the discrete energy identity and the energy of the Gaussian pulse
+// (W1-W3, tests/test_oracle_wave1.py).  "Parity unpinned" (conventions of this build that the
 // paper does not fix, so nothing external can pin them): eta, eps_diss, dx, the inert 25th
 // slot A, KO order 5 on BSSN.
 //
