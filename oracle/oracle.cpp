@@ -553,6 +553,70 @@ void rk4_step(int system, double* U, const Grid& G, const Params& P, double dt) 
 // C entry points for the ctypes harness (oracle/oracle.py).  All arrays are host memory in
 // the oracle layout described at the top.  params = {eps_diss, eta, shift_gamma_coeff}.
 // ---------------------------------------------------------------------------------------
+// ---------------------------------------------------------------------------------------
+// RK3 (reading S9b; the paper's runs use "RK3", without a formula): the third-order
+// strong-stability-preserving scheme of Shu and Osher,
+//   U1 = U + dt f(U) ;  U2 = 3/4 U + 1/4 (U1 + dt f(U1)) ;  U+ = 1/3 U + 2/3 (U2 + dt f(U2)),
+// every stage written as  a*U + b*(Y + dt*k)  with each product and sum rounded once.
+// Ghost fill before every RHS evaluation.
+// ---------------------------------------------------------------------------------------
+static void rk3_step(int system, double* U, const Grid& G, const Params& P, double dt) {
+  const int V = nvars_of(system);
+  const long n = G.npts(), tot = V * n;
+  std::vector<double> Ya(tot, 0.0), Yb(tot, 0.0), kk(tot, 0.0);
+  auto fill_all = [&](double* st) { for (int v = 0; v < V; ++v) fill_ghosts(st + v * n, G); };
+  auto stage = [&](const double* Y, double* out, double a, double b) {
+    rhs_any(system, Y, kk.data(), G, P);
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < G.nz; ++k)
+      for (int v = 0; v < V; ++v)
+        for (int j = 0; j < G.ny; ++j)
+          for (int i = 0; i < G.nx; ++i) {
+            long q = v * n + idx(G, i, j, k);
+            out[q] = a * U[q] + b * (Y[q] + dt * kk[q]);
+          }
+  };
+  fill_all(U);
+  stage(U, Ya.data(), 0.0, 1.0);
+  fill_all(Ya.data());
+  stage(Ya.data(), Yb.data(), 3.0 / 4.0, 1.0 / 4.0);
+  fill_all(Yb.data());
+  stage(Yb.data(), U, 1.0 / 3.0, 2.0 / 3.0);
+}
+
+// ---------------------------------------------------------------------------------------
+// Algebraic constraint enforcement of the BSSN variables (reading S10b; not in the paper, the
+// standard companion of the evolution in its production runs): at every interior point
+//   gt_ij <- gt_ij / det(gt)^(1/3)          (det gt = 1)
+//   At_ij <- At_ij - 1/3 gt_ij gtu^{kl} At_kl (tr At = 0), with the new gt and its inverse.
+// ---------------------------------------------------------------------------------------
+static void enforce_constraints(double* state, const Grid& G) {
+  const long n = G.npts();
+#pragma omp parallel for schedule(static)
+  for (int k = 0; k < G.nz; ++k)
+    for (int j = 0; j < G.ny; ++j)
+      for (int i = 0; i < G.nx; ++i) {
+        long p = idx(G, i, j, k);
+        double g[6], A[6];
+        for (int s = 0; s < 6; ++s) { g[s] = state[(1 + s) * n + p]; A[s] = state[(8 + s) * n + p]; }
+        // packed order 11 12 13 22 23 33
+        double det = g[0] * (g[3] * g[5] - g[4] * g[4]) - g[1] * (g[1] * g[5] - g[4] * g[2]) +
+                     g[2] * (g[1] * g[4] - g[3] * g[2]);
+        double f = 1.0 / std::cbrt(det);
+        for (int s = 0; s < 6; ++s) g[s] *= f;
+        // inverse of the rescaled metric (its determinant is 1 up to rounding; divide by it anyway)
+        double c00 = g[3] * g[5] - g[4] * g[4], c01 = g[2] * g[4] - g[1] * g[5], c02 = g[1] * g[4] - g[2] * g[3];
+        double d = g[0] * c00 + g[1] * c01 + g[2] * c02;
+        double u[6] = {c00 / d, c01 / d, c02 / d, (g[0] * g[5] - g[2] * g[2]) / d, (g[1] * g[2] - g[0] * g[4]) / d,
+                       (g[0] * g[3] - g[1] * g[1]) / d};
+        double tr = (u[0] * A[0] + u[3] * A[3] + u[5] * A[5]) + 2.0 * (u[1] * A[1] + u[2] * A[2] + u[4] * A[4]);
+        for (int s = 0; s < 6; ++s) {
+          state[(1 + s) * n + p] = g[s];
+          state[(8 + s) * n + p] = A[s] - (tr / 3.0) * g[s];
+        }
+      }
+}
+
 extern "C" {
 
 void oracle_set_threads(int n) {
@@ -607,6 +671,23 @@ void oracle_rk4(int system, double* U, int nx, int ny, int nz, int g, int order,
   Grid G = make_grid(nx, ny, nz, g, order, h);
   Params P = {params[0], params[1], params[2]};
   for (int s = 0; s < nsteps; ++s) rk4_step(system, U, G, P, dt);
+}
+
+// U (ghosted) is advanced in place by `nsteps` RK3 steps (reading S9b); with enforce != 0 (BSSN only) the algebraic
+// constraints are enforced after every step.
+void oracle_rk3(int system, double* U, int nx, int ny, int nz, int g, int order, double h, double dt,
+                const double* params, int nsteps, int enforce) {
+  Grid G = make_grid(nx, ny, nz, g, order, h);
+  Params P = {params[0], params[1], params[2]};
+  for (int s = 0; s < nsteps; ++s) {
+    rk3_step(system, U, G, P, dt);
+    if (enforce && system == SYS_BSSN) enforce_constraints(U, G);
+  }
+}
+
+void oracle_enforce(double* U, int nx, int ny, int nz, int g) {
+  Grid G = make_grid(nx, ny, nz, g, 4, 1.0);
+  enforce_constraints(U, G);
 }
 
 }  // extern "C"

@@ -41,6 +41,10 @@ def lib():
         _lib.oracle_fill_ghosts.argtypes = [dp, i, i, i, i, i]
         _lib.oracle_rhs.argtypes = [i, dp, dp, i, i, i, i, i, d, dp]
         _lib.oracle_rk4.argtypes = [i, dp, i, i, i, i, i, d, d, dp, i]
+        _lib.oracle_rk3.argtypes = [i, dp, i, i, i, i, i, d, d, dp, i, i]
+        _lib.oracle_enforce.argtypes = [dp, i, i, i, i]
+        _lib.oracle_rk3.restype = None
+        _lib.oracle_enforce.restype = None
         _lib.oracle_set_threads.argtypes = [i]
         _lib.oracle_max_threads.restype = i
         for f in (_lib.oracle_apply_op, _lib.oracle_fill_ghosts, _lib.oracle_rhs, _lib.oracle_rk4,
@@ -109,4 +113,21 @@ def rk4(system, state, g, order, h, dt, prm, nsteps=1):
     assert V == NVARS[system]
     lib().oracle_rk4(system, _p(state), tx - 2 * g, ty - 2 * g, tz - 2 * g, g, order, float(h), float(dt), _p(prm),
                      int(nsteps))
+    return state
+
+
+def rk3(system, state, g, order, h, dt, prm, nsteps=1, enforce=False):
+    """Shu-Osher RK3 (reading S9b), in place; enforce=True applies the BSSN algebraic constraints after each step."""
+    V, tz, ty, tx = state.shape
+    assert V == NVARS[system]
+    lib().oracle_rk3(system, _p(state), tx - 2 * g, ty - 2 * g, tz - 2 * g, g, order, float(h), float(dt), _p(prm),
+                     int(nsteps), int(bool(enforce)))
+    return state
+
+
+def enforce(state, g):
+    """det gt -> 1, tr At -> 0 on the interior of a ghosted BSSN state (reading S10b), in place."""
+    V, tz, ty, tx = state.shape
+    assert V == 25
+    lib().oracle_enforce(_p(state), tx - 2 * g, ty - 2 * g, tz - 2 * g, g)
     return state
