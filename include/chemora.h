@@ -100,6 +100,16 @@ int chemora_rhs(chemora_t* h, const double* dev_state, double* dev_rhs);
  * the four RHS evaluations; asynchronous on the stream. */
 int chemora_rk4_step(chemora_t* h, double dt);
 
+/* U <- U(t + dt) with the third-order Shu-Osher Runge-Kutta scheme (reading S9b; the paper's own runs use RK3,
+ * PAPER.md:338): U1 = U + dt f(U); U2 = 3/4 U + 1/4 (U1 + dt f(U1)); U+ = 1/3 U + 2/3 (U2 + dt f(U2)); ghost fill
+ * before each of the three RHS evaluations; uses buffers U, YA, YB; asynchronous on the stream. */
+int chemora_rk3_step(chemora_t* h, double dt);
+
+/* Algebraic constraint enforcement on the interior of a BSSN state in the padded layout (dev_state == NULL: U):
+ * gt_ij <- gt_ij / det(gt)^(1/3), At_ij <- At_ij - 1/3 gt_ij gtu^kl At_kl (reading S10b).  In place, asynchronous.
+ * CHEMORA_EINVAL for the wave systems. */
+int chemora_enforce_constraints(chemora_t* h, double* dev_state);
+
 /* Kernel variant: fused (1: derivatives + RHS + RK stage update in one kernel) or split (0: derivatives
  * written to global arrays by one kernel, RHS + stage update by a second), and tile_id in
  * [0, CHEMORA_NUM_TILES).  chemora_tile_shape reports the (x, y, z) extent of a tile id: for the fused BSSN

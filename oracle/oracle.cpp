@@ -587,7 +587,7 @@ static void rk3_step(int system, double* U, const Grid& G, const Params& P, doub
 // ---------------------------------------------------------------------------------------
 // Algebraic constraint enforcement of the BSSN variables (reading S10b; not in the paper, the
 // standard companion of the evolution in its production runs): at every interior point
-//   gt_ij <- gt_ij / det(gt)^(1/3)          (det gt = 1)
+//   gt_ij <- gt_ij + gt_ij (det(gt)^(-1/3) - 1)   (det gt = 1)
 //   At_ij <- At_ij - 1/3 gt_ij gtu^{kl} At_kl (tr At = 0), with the new gt and its inverse.
 // ---------------------------------------------------------------------------------------
 static void enforce_constraints(double* state, const Grid& G) {
@@ -602,8 +602,10 @@ static void enforce_constraints(double* state, const Grid& G) {
         // packed order 11 12 13 22 23 33
         double det = g[0] * (g[3] * g[5] - g[4] * g[4]) - g[1] * (g[1] * g[5] - g[4] * g[2]) +
                      g[2] * (g[1] * g[4] - g[3] * g[2]);
-        double f = 1.0 / std::cbrt(det);
-        for (int s = 0; s < 6; ++s) g[s] *= f;
+        // rounding-aware form (reading R-H1): the correction factor minus one, det^(-1/3) - 1, is a small number
+        // known to full relative accuracy, and gt_ij is rounded once at its own magnitude when it is added
+        double f1 = std::expm1(-std::log(det) / 3.0);
+        for (int s = 0; s < 6; ++s) g[s] = g[s] + g[s] * f1;
         // inverse of the rescaled metric (its determinant is 1 up to rounding; divide by it anyway)
         double c00 = g[3] * g[5] - g[4] * g[4], c01 = g[2] * g[4] - g[1] * g[5], c02 = g[1] * g[4] - g[2] * g[3];
         double d = g[0] * c00 + g[1] * c01 + g[2] * c02;

@@ -21,7 +21,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 # every symbol include/chemora.h declares (tests check that the library exports all of them)
 SYMBOLS = ["chemora_create", "chemora_set_param", "chemora_get_param", "chemora_layout", "chemora_state_ptr",
            "chemora_set_state", "chemora_get_state", "chemora_set_state_dev", "chemora_get_state_dev",
-           "chemora_fill_ghosts", "chemora_rhs", "chemora_rk4_step", "chemora_set_variant",
+           "chemora_fill_ghosts", "chemora_rhs", "chemora_rk4_step", "chemora_rk3_step", "chemora_enforce_constraints", "chemora_set_variant",
            "chemora_get_variant", "chemora_tile_shape", "chemora_autotune", "chemora_launch_count",
            "chemora_kernel_info", "chemora_timing", "chemora_timing_read", "chemora_measure_fp64_peak", "chemora_last_error", "chemora_destroy"]
 
@@ -58,6 +58,8 @@ def load():
         "chemora_set_state_dev": [vp, vp], "chemora_get_state_dev": [vp, vp],
         "chemora_fill_ghosts": [vp, vp], "chemora_rhs": [vp, vp, vp],
         "chemora_rk4_step": [vp, d],
+        "chemora_rk3_step": [vp, d],
+        "chemora_enforce_constraints": [vp, vp],
         "chemora_set_variant": [vp, i, i], "chemora_get_variant": [vp, ip, ip],
         "chemora_tile_shape": [i, i, i, ip, ip, ip],
         "chemora_autotune": [vp, ip, ip, ctypes.POINTER(ctypes.c_float)],
@@ -201,6 +203,13 @@ class Chemora:
 
     def rk4_step(self, dt):
         self._ck(self.lib.chemora_rk4_step(self._h, float(dt)))
+
+    def rk3_step(self, dt):
+        self._ck(self.lib.chemora_rk3_step(self._h, float(dt)))
+
+    def enforce_constraints(self, state=None):
+        """in place on a padded device state tensor (default: U)"""
+        self._ck(self.lib.chemora_enforce_constraints(self._h, None if state is None else state.data_ptr()))
 
     def set_variant(self, fused, tile_id):
         self._ck(self.lib.chemora_set_variant(self._h, int(fused), int(tile_id)))

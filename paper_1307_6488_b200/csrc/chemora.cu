@@ -320,6 +320,30 @@ int chemora_rk4_step(chemora_t* h, double dt) {
   return CHEMORA_OK;
 }
 
+int chemora_rk3_step(chemora_t* h, double dt) {
+  if (!h || !(dt == dt)) return CHEMORA_EINVAL;
+  double *U = h->buf[0], *Ya = h->buf[1], *Yb = h->buf[2];
+  int rc;
+  // U1 = U + dt f(U)
+  if ((rc = fill(h, U))) return rc;
+  if ((rc = run_rhs(h, Stage{U, U, nullptr, Ya, dt, MODE_SSP, 0.0, 1.0}))) return rc;
+  // U2 = 3/4 U + 1/4 (U1 + dt f(U1))
+  if ((rc = fill(h, Ya))) return rc;
+  if ((rc = run_rhs(h, Stage{Ya, U, nullptr, Yb, dt, MODE_SSP, 3.0 / 4.0, 1.0 / 4.0}))) return rc;
+  // U+ = 1/3 U + 2/3 (U2 + dt f(U2)), written over U point by point
+  if ((rc = fill(h, Yb))) return rc;
+  if ((rc = run_rhs(h, Stage{Yb, U, nullptr, U, dt, MODE_SSP, 1.0 / 3.0, 2.0 / 3.0}))) return rc;
+  return CHEMORA_OK;
+}
+
+int chemora_enforce_constraints(chemora_t* h, double* dev_state) {
+  if (!h) return CHEMORA_EINVAL;
+  if (h->system != CHEMORA_SYS_BSSN) return fail(h, CHEMORA_EINVAL, "constraint enforcement is defined for the BSSN system only");
+  CK(h, launch_enforce(h->L, dev_state ? dev_state : h->buf[0], h->stream), "constraint enforcement launch");
+  h->launches += 1;
+  return CHEMORA_OK;
+}
+
 int chemora_set_variant(chemora_t* h, int fused, int tile_id) {
   if (!h || tile_id < 0 || tile_id >= CHEMORA_NUM_TILES || (fused != 0 && fused != 1)) return CHEMORA_EINVAL;
   if (!fused && h->system != CHEMORA_SYS_BSSN) return fail(h, CHEMORA_EINVAL, "wave systems have no split variant");

@@ -42,7 +42,9 @@ struct Coef {
 //   MODE_FIRST : S = k          ; Y = U + a k        (U == the input state)
 //   MODE_MID   : S = S + 2 k    ; Y = U + a k
 //   MODE_LAST  : U = U + a (S + k)                   (a = dt/6)
-enum { MODE_RHS = 0, MODE_FIRST = 1, MODE_MID = 2, MODE_LAST = 3 };
+// and of the Shu-Osher RK3 (reading S9b):
+//   MODE_SSP   : out = ca U + cb (in + a k)          (a = dt; out may be U itself: each point is read, then written)
+enum { MODE_RHS = 0, MODE_FIRST = 1, MODE_MID = 2, MODE_LAST = 3, MODE_SSP = 4 };
 
 struct Stage {
   const double* in;      // state the RHS is evaluated on (ghosts filled)
@@ -51,7 +53,13 @@ struct Stage {
   double* out;           // MODE_RHS: rhs ; MODE_FIRST/MID: next stage state Y
   double a;              // dt/2, dt/2, dt, dt/6
   int mode;
+  double ca, cb;         // MODE_SSP only
 };
+
+// a U + b (Y + dt k), every product and sum rounded once
+__device__ __forceinline__ double ssp_combine(const Stage& st, double u, double y, double k) {
+  return __dadd_rn(__dmul_rn(st.ca, u), __dmul_rn(st.cb, __dadd_rn(y, __dmul_rn(st.a, k))));
+}
 
 // The stage combination, one rounding per operation and no FMA contraction, so that it is
 // bit-identical to the association written in reading S9 for a given k.
@@ -64,8 +72,10 @@ __device__ __forceinline__ void stage_emit(const Stage& st, long q, double k) {
   } else if (st.mode == MODE_MID) {
     st.S[q] = __dadd_rn(st.S[q], __dmul_rn(2.0, k));
     st.out[q] = __dadd_rn(st.U[q], __dmul_rn(st.a, k));
-  } else {
+  } else if (st.mode == MODE_LAST) {
     st.U[q] = __dadd_rn(st.U[q], __dmul_rn(st.a, __dadd_rn(st.S[q], k)));
+  } else {
+    st.out[q] = ssp_combine(st, st.U[q], st.in[q], k);
   }
 }
 
@@ -73,6 +83,7 @@ __device__ __forceinline__ void stage_emit(const Stage& st, long q, double k) {
 struct StagePre { double u, s; };
 __device__ __forceinline__ void stage_prefetch(const Stage& st, long q, StagePre& r) {
   if (st.mode == MODE_FIRST) r.u = st.in[q];
+  else if (st.mode == MODE_SSP) { r.u = st.U[q]; r.s = st.in[q]; }
   else if (st.mode != MODE_RHS) { r.u = st.U[q]; r.s = st.S[q]; }
 }
 __device__ __forceinline__ void stage_emit(const Stage& st, long q, double k, const StagePre& pr) {
@@ -84,8 +95,10 @@ __device__ __forceinline__ void stage_emit(const Stage& st, long q, double k, co
   } else if (st.mode == MODE_MID) {
     CHM_ST(&st.S[q], __dadd_rn(pr.s, __dmul_rn(2.0, k)));
     CHM_ST(&st.out[q], __dadd_rn(pr.u, __dmul_rn(st.a, k)));
-  } else {
+  } else if (st.mode == MODE_LAST) {
     CHM_ST(&st.U[q], __dadd_rn(pr.u, __dmul_rn(st.a, __dadd_rn(pr.s, k))));
+  } else {
+    CHM_ST(&st.out[q], ssp_combine(st, pr.u, pr.s, k));
   }
 }
 
@@ -101,9 +114,12 @@ __device__ __forceinline__ void stage_emit_t(const Stage& st, long q, double k, 
   } else if (MODE == MODE_MID) {
     const double s2 = __dadd_rn(pr.s, __dmul_rn(2.0, k)), y = __dadd_rn(pr.u, __dmul_rn(st.a, k));
     if (valid) { CHM_ST(&st.S[q], s2); CHM_ST(&st.out[q], y); }
-  } else {
+  } else if (MODE == MODE_LAST) {
     const double u = __dadd_rn(pr.u, __dmul_rn(st.a, __dadd_rn(pr.s, k)));
     if (valid) CHM_ST(&st.U[q], u);
+  } else {
+    const double y = ssp_combine(st, pr.u, pr.s, k);   // pr.u = U, pr.s = the evaluated state at the point
+    if (valid) CHM_ST(&st.out[q], y);
   }
 }
 
@@ -118,6 +134,7 @@ static const TileShape kTilesMarch[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64
 
 // launchers implemented in the kernel translation units; each returns the cudaError_t of the launch
 cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s);
+cudaError_t launch_enforce(const Layout& L, double* state, cudaStream_t s);
 cudaError_t launch_pack(const Layout& L, const double* packed, double* state, bool to_state, cudaStream_t s);
 cudaError_t launch_wave(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
 cudaError_t launch_wave1(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);

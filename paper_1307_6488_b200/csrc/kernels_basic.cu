@@ -66,6 +66,47 @@ cudaError_t launch_pack(const Layout& L, const double* packed, double* state, bo
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Algebraic constraint enforcement of a BSSN state (reading S10b): gt_ij <- gt_ij + gt_ij (det(gt)^(-1/3) - 1),
+// At_ij <- At_ij - 1/3 gt_ij gtu^{kl} At_kl with the rescaled metric.  Pointwise over the interior.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) enforce_kernel(Layout L, double* __restrict__ state) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= L.nx) return;
+  const long p = (long)(blockIdx.z + L.g) * L.plane + (long)(blockIdx.y + L.g) * L.pitch + (i + L.xo);
+  double g[6], A[6];
+#pragma unroll
+  for (int s = 0; s < 6; ++s) { g[s] = state[(1 + s) * L.vstride + p]; A[s] = state[(8 + s) * L.vstride + p]; }
+  // The determinant and the rescaling are written without FMA contraction, one rounding per operation, in the
+  // association of reading S10b: values near 1 are rounded exactly as any other implementation of that reading
+  // rounds them (reading R-H1: a 1-ulp difference in gt_ii ~ 1 reappears as a 1e-6 relative one in At_ij).
+  auto mul = [](double a, double b) { return __dmul_rn(a, b); };
+  auto sub = [](double a, double b) { return __dsub_rn(a, b); };
+  const double det = __dadd_rn(sub(mul(g[0], sub(mul(g[3], g[5]), mul(g[4], g[4]))),
+                                   mul(g[1], sub(mul(g[1], g[5]), mul(g[4], g[2])))),
+                               mul(g[2], sub(mul(g[1], g[4]), mul(g[3], g[2]))));
+  const double f1 = expm1(-log(det) / 3.0);   // det^(-1/3) - 1: small, known to full relative accuracy
+#pragma unroll
+  for (int s = 0; s < 6; ++s) g[s] = __dadd_rn(g[s], mul(g[s], f1));
+  const double c00 = g[3] * g[5] - g[4] * g[4], c01 = g[2] * g[4] - g[1] * g[5], c02 = g[1] * g[4] - g[2] * g[3];
+  const double id = 1.0 / (g[0] * c00 + g[1] * c01 + g[2] * c02);
+  const double u[6] = {c00 * id, c01 * id, c02 * id, (g[0] * g[5] - g[2] * g[2]) * id,
+                       (g[1] * g[2] - g[0] * g[4]) * id, (g[0] * g[3] - g[1] * g[1]) * id};
+  const double tr3 = ((u[0] * A[0] + u[3] * A[3] + u[5] * A[5]) + 2.0 * (u[1] * A[1] + u[2] * A[2] + u[4] * A[4])) *
+                     (1.0 / 3.0);
+#pragma unroll
+  for (int s = 0; s < 6; ++s) {
+    state[(1 + s) * L.vstride + p] = g[s];
+    state[(8 + s) * L.vstride + p] = A[s] - tr3 * g[s];
+  }
+}
+
+cudaError_t launch_enforce(const Layout& L, double* state, cudaStream_t s) {
+  dim3 grid((L.nx + 255) / 256, L.ny, L.nz);
+  enforce_kernel<<<grid, 256, 0, s>>>(L, state);
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Wave system (reading S1): d_t phi = pi (+KO), d_t pi = (d_xx + d_yy + d_zz) phi (+KO).
 // Block = TX x TY threads; each thread marches TZ consecutive z-planes.
 // ---------------------------------------------------------------------------------------------------

@@ -777,6 +777,7 @@ static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, 
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   };
   // RK4 operands: MODE_FIRST reads U == in; MODE_MID / MODE_LAST read U and S; MODE_RHS none (maps unused)
+  // MODE_SSP reads U and the evaluated state itself
   const double* ubase = st->mode == MODE_FIRST || st->mode == MODE_RHS ? st->in : st->U;
   const double* sbase = st->mode == MODE_MID || st->mode == MODE_LAST ? st->S : st->in;
   if (tile_map(&tmCen, st->in, 7) != CUDA_SUCCESS || tile_map(&tmU, ubase, 1) != CUDA_SUCCESS ||
@@ -809,6 +810,7 @@ static cudaError_t tma_go(const Layout& L, const Coef& C, const Stage* st, cudaS
     case MODE_FIRST: return tma_go_mode<TX, TY, TZ, MODE_FIRST>(L, C, st, s, a);
     case MODE_MID: return tma_go_mode<TX, TY, TZ, MODE_MID>(L, C, st, s, a);
     case MODE_LAST: return tma_go_mode<TX, TY, TZ, MODE_LAST>(L, C, st, s, a);
+    case MODE_SSP: return tma_go_mode<TX, TY, TZ, MODE_SSP>(L, C, st, s, a);
   }
   return cudaErrorInvalidValue;
 }

@@ -232,6 +232,7 @@ bssn_ws_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ C
       StagePre pr{0.0, 0.0};
       const long qq = q + v * L.vstride;
       if (st.mode == MODE_FIRST) pr.u = __ldg(st.in + qq);
+      else if (st.mode == MODE_SSP) { pr.u = __ldcs(st.U + qq); pr.s = __ldg(st.in + qq); }
       else if (st.mode != MODE_RHS) { pr.u = __ldcs(st.U + qq); pr.s = __ldcs(st.S + qq); }
       return pr;
     };

@@ -114,3 +114,42 @@ def test_wave1_256_sampled(oracle):
     centres = [(128, 128, 128), (140, 128, 120), (0, 0, 0), (255, 130, 3), (110, 150, 128)]
     check_samples(oracle, oracle.SYS_WAVE1, u0, got, centres, reach=16 * steps, core=4, g=g, order=8, dx=dx, dt=dt,
                   prm=oracle.params(eps_diss=0.1), steps=steps, tol=1e-12 * steps)
+
+
+def test_bssn_rk3_enforced_256_sampled(oracle):
+    """The paper's integrator at full size: BSSN 256^3 (configs[3] data), RK3 + constraint enforcement, 2 steps."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1307_6488_b200 import binding
+    c = inputs.config(3)
+    n, g, dx = 256, c["ghost"], c["dx"]
+    dt, steps = 0.25 * dx, 2
+    u0 = c["state"]()
+    h = binding.Chemora(n, n, n, g, c["order"], binding.SYS_BSSN, dx)
+    h.set_param("eps_diss", c["eps_diss"])
+    h.set_state(u0)
+    for _ in range(steps):
+        h.rk3_step(dt)
+        h.enforce_constraints()
+    got = h.get_state()
+    h.destroy()
+    ga = np.abs(np.gradient(u0[17, :, :, :], axis=2))
+    k, j, i = np.unravel_index(int(np.argmax(ga)), ga.shape)
+    centres = [(0, 0, 0), (255, 128, 3), (int(i), int(j), int(k))]
+    V = 25
+    scale = [float(np.max(np.abs(got[v]))) for v in range(V)]
+    reach, core, worst = 9 * steps, 4, 0.0
+    for cpt in centres:
+        blk = cut(u0, cpt, core + reach)
+        st = oracle.rk3(oracle.SYS_BSSN, oracle.with_ghosts(blk, g), g, 4, dx, dt, oracle.params(eps_diss=c["eps_diss"]),
+                        steps, True)
+        want = oracle.interior(st, g)[:, reach:reach + 2 * core, reach:reach + 2 * core, reach:reach + 2 * core]
+        have = cut(got, cpt, core)
+        for v in range(V):
+            err = float(np.max(np.abs(have[v] - want[v])))
+            if scale[v] == 0.0:
+                assert err == 0.0
+            else:
+                worst = max(worst, err / scale[v])
+    assert worst < 2e-11, worst

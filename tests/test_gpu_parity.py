@@ -264,3 +264,75 @@ def test_autotune_and_kernel_info(chem):
     assert 0 < info["regs"] <= 255
     assert h.launch_count() > 0
     h.destroy()
+
+
+# --------------------------------------------------------------------- RK3 + constraint enforcement
+@pytest.mark.parametrize("system,order,g,V", [(0, 8, 4, 2), (2, 4, 3, 5)])
+def test_rk3_wave_systems(chem, oracle, system, order, g, V):
+    nx, ny, nz = 37, 21, 19
+    u0 = np.random.default_rng(31).standard_normal((V, nz, ny, nx))
+    dx = 1.0 / 32
+    dt = 0.25 * dx
+    h = chem.Chemora(nx, ny, nz, g, order, system, dx)
+    h.set_param("eps_diss", 0.1)
+    h.set_state(u0)
+    for _ in range(5):
+        h.rk3_step(dt)
+    st = oracle.rk3(system, oracle.with_ghosts(u0, g), g, order, dx, dt, oracle.params(eps_diss=0.1), 5)
+    assert relerr(h.get_state(), oracle.interior(st, g)) < TOL_WAVE_PER_STEP * 5
+    h.destroy()
+
+
+def test_enforce_constraints(chem, oracle):
+    nx, ny, nz, g = 21, 9, 10, 3
+    u = strong_field(nx, ny, nz, seed=33)
+    h = chem.Chemora(nx, ny, nz, g, 4, 1, 0.05)
+    h.set_state(u)
+    h.enforce_constraints()
+    got = h.get_state()
+    want = oracle.interior(oracle.enforce(oracle.with_ghosts(u, g), g), g)
+    assert relerr(got, want) < 1e-14
+    for v in [0, 7] + list(range(14, 25)):
+        assert np.array_equal(got[v], u[v])            # only gt_ij and At_ij are touched
+    flat = inputs.bssn_minkowski(nx, ny, nz)
+    h.set_state(flat)
+    h.enforce_constraints()
+    assert np.array_equal(h.get_state(), flat)
+    h.destroy()
+    w = chem.Chemora(8, 8, 8, 2, 4, 0, 0.1)
+    with pytest.raises(chem.ChemoraError):
+        w.enforce_constraints()
+    w.destroy()
+
+
+@pytest.mark.parametrize("tile", [0, 1, 4, 6, 9])
+def test_bssn_rk3_with_enforcement_10_steps(chem, oracle, tile):
+    """the paper's integrator (RK3) with constraint enforcement after every step, configs[2] data at 24x20x18"""
+    nx, ny, nz = 24, 20, 18
+    u0 = inputs.bssn_noise(nx, ny, nz)
+    dx, dt, eps = 0.05, 0.0125, 0.1
+    h = chem.Chemora(nx, ny, nz, 3, 4, 1, dx)
+    h.set_param("eps_diss", eps)
+    h.set_variant(1, tile)
+    h.set_state(u0)
+    for _ in range(10):
+        h.rk3_step(dt)
+        h.enforce_constraints()
+    st = oracle.rk3(1, oracle.with_ghosts(u0, 3), 3, 4, dx, dt, oracle.params(eps_diss=eps), 10, True)
+    assert relerr(h.get_state(), oracle.interior(st, 3)) < TOL_BSSN_10_STEPS
+    h.destroy()
+
+
+def test_bssn_rk3_split_variant(chem, oracle):
+    nx, ny, nz = 24, 20, 18
+    u0 = inputs.bssn_gaussians(nx, ny, nz, width_cells=4.0)
+    dx, dt, eps = 0.05, 0.0125, 0.1
+    h = chem.Chemora(nx, ny, nz, 3, 4, 1, dx)
+    h.set_param("eps_diss", eps)
+    h.set_variant(0, 1)
+    h.set_state(u0)
+    for _ in range(3):
+        h.rk3_step(dt)
+    st = oracle.rk3(1, oracle.with_ghosts(u0, 3), 3, 4, dx, dt, oracle.params(eps_diss=eps), 3)
+    assert relerr(h.get_state(), oracle.interior(st, 3)) < TOL_BSSN_10_STEPS
+    h.destroy()
