@@ -52,14 +52,23 @@ def _roll(f, axis, m):          # value at offset +m along axis (0=x,1=y,2=z) on
     return np.roll(f, -m, axis=2 - axis)
 
 
+ORDER = [4]                     # FD order the linearised evaluator uses (set by the O6 tests)
+
+
 def _d1(f, a, h):
-    return (8 * (_roll(f, a, 1) - _roll(f, a, -1)) - (_roll(f, a, 2) - _roll(f, a, -2))) / (12 * h)
+    e = [_roll(f, a, m) - _roll(f, a, -m) for m in range(5)]
+    if ORDER[0] == 4:
+        return (8 * e[1] - e[2]) / (12 * h)
+    return (672 * e[1] - 168 * e[2] + 32 * e[3] - 3 * e[4]) / (840 * h)
 
 
 def _dd(f, a, b, h):
     if a != b:
         return _d1(_d1(f, a, h), b, h)
-    return (-30 * f + 16 * (_roll(f, a, 1) + _roll(f, a, -1)) - (_roll(f, a, 2) + _roll(f, a, -2))) / (12 * h * h)
+    s = [_roll(f, a, m) + _roll(f, a, -m) for m in range(5)]
+    if ORDER[0] == 4:
+        return (-30 * f + 16 * s[1] - s[2]) / (12 * h * h)
+    return (-14350 * f + 8064 * s[1] - 1008 * s[2] + 128 * s[3] - 9 * s[4]) / (5040 * h * h)
 
 
 def _ko(f, eps, h):
@@ -106,11 +115,17 @@ def linearised_rhs(u, h, eps, eta):
     return r
 
 
-def test_O6_linearised_bssn_on_config2_data(oracle):
+@pytest.mark.parametrize("order,g", [(4, 3), (8, 5)])
+def test_O6_linearised_bssn_on_config2_data(oracle, order, g):
+    """order 8 with 5 ghost zones is the paper's own configuration"""
     n, h, eps, eta = 16, 0.05, 0.1, 1.0
     u = inputs.bssn_noise(n, n, n, amp=1e-10)
-    got = rhs_periodic(oracle, u, h=h, eps_diss=eps, eta=eta)
-    want = linearised_rhs(u, h, eps, eta)
+    got = rhs_periodic(oracle, u, g=g, order=order, h=h, eps_diss=eps, eta=eta)
+    ORDER[0] = order
+    try:
+        want = linearised_rhs(u, h, eps, eta)
+    finally:
+        ORDER[0] = 4
     for v in range(25):
         scale = np.max(np.abs(want[v]))
         assert scale > 0
