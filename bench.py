@@ -277,6 +277,38 @@ def run_sweep(args):
     print(json.dumps({"metric": "BSSN RHS variant sweep (configs[4])", "unit": "ms per RHS evaluation", "rows": table}))
 
 
+def run_paper_shape(args):
+    """The shape of the paper's own single-GPU benchmark: BSSN, 8th-order FD, 5 ghost zones,
+    RK3 (+ constraint enforcement), 100^3 evolved points; synthetic Minkowski + 1e-4 Gaussians.  Context line, not the
+    headline: 8th-order BSSN runs through the derivative-split variant only."""
+    import torch
+    from paper_1307_6488_b200 import binding, inputs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device and no CPU fallback")
+    rows = []
+    for n in (100, args.size):
+        h = binding.Chemora(n, n, n, 5, 8, binding.SYS_BSSN, 0.05)
+        h.set_param("eps_diss", 0.1)
+        h.set_state(inputs.bssn_gaussians(n, n, n, width_cells=n / 16.0))
+        fused, tile, _ = h.autotune()
+        dt = 0.0125
+        for _ in range(max(args.warmup, 3)):
+            h.rk3_step(dt); h.enforce_constraints()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            h.rk3_step(dt); h.enforce_constraints()
+        e1.record(); torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        rows.append({"grid": n, "ms_per_rk3_step": ms, "updates_per_s": n ** 3 / (ms * 1e-3),
+                     "variant": {"fused": fused, "tile": list(binding.tile_shape(tile, binding.SYS_BSSN, fused))}})
+        h.destroy()
+    print(json.dumps({"metric": "BSSN O8 (5 ghosts) RK3 + enforcement grid-point updates/sec, fp64", "unit": UNIT,
+                      "rows": rows, "paper_context": {"value": 1.05e6, "hardware": "NVIDIA M2050, 100^3, derived from "
+                                                      "25 GFlop/s / 7900 flop / 3 substeps (PAPER.md:55, :338, :388)"}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -289,9 +321,12 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=64)
     ap.add_argument("--ref-sample", type=int, default=64)
     ap.add_argument("--sweep", action="store_true", help="configs[4] variant/tile sweep instead of the headline run")
+    ap.add_argument("--paper-shape", action="store_true", help="BSSN O8 + RK3 at 100^3 (the paper's own benchmark shape)")
     args = ap.parse_args()
     if args.sweep:
         run_sweep(args)
+    elif args.paper_shape:
+        run_paper_shape(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

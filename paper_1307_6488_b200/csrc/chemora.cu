@@ -122,7 +122,7 @@ int run_rhs_inner(chemora_t* h, const Stage& st) {
   } else {
     int rc = ensure_derivs(h);
     if (rc) return rc;
-    CK(h, launch_bssn_derivs(h->L, C, h->tile % 6, st.in, h->derivs, h->stream), "bssn derivative kernel launch");
+    CK(h, launch_bssn_derivs(h->L, C, h->order, h->tile % 6, st.in, h->derivs, h->stream), "bssn derivative kernel launch");
     CK(h, launch_bssn_from_derivs(h->L, C, h->tile % 6, h->derivs, st, h->stream), "bssn rhs kernel launch");
     h->launches += 2;
   }
@@ -155,7 +155,6 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
   const int need = system_id == CHEMORA_SYS_BSSN ? fd_order / 2 + 1 : fd_order / 2;
   if (ghost < need) return CHEMORA_EINVAL;
   if (nx < ghost || ny < ghost || nz < ghost) return CHEMORA_EINVAL;
-  if (system_id == CHEMORA_SYS_BSSN && fd_order != 4) return CHEMORA_EINVAL;  // 8th-order BSSN: not built yet
 
   chemora_t* h = new (std::nothrow) chemora_t();
   if (!h) return CHEMORA_ENOMEM;
@@ -173,7 +172,8 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
   h->stream = (cudaStream_t)cuda_stream;
   h->alloc = alloc; h->dealloc = dealloc; h->actx = alloc_ctx;
   h->derivs = nullptr; h->staging = nullptr;
-  h->fused = 1; h->tile = 1;
+  // 8th-order BSSN (the paper's configuration, 5 ghost zones) runs through the derivative-split variant only
+  h->fused = (system_id == CHEMORA_SYS_BSSN && fd_order == 8) ? 0 : 1; h->tile = 1;
   h->launches = 0;
   h->timing = false;
   h->ev_launches[0] = h->ev_launches[1] = 0;
@@ -347,6 +347,8 @@ int chemora_enforce_constraints(chemora_t* h, double* dev_state) {
 int chemora_set_variant(chemora_t* h, int fused, int tile_id) {
   if (!h || tile_id < 0 || tile_id >= CHEMORA_NUM_TILES || (fused != 0 && fused != 1)) return CHEMORA_EINVAL;
   if (!fused && h->system != CHEMORA_SYS_BSSN) return fail(h, CHEMORA_EINVAL, "wave systems have no split variant");
+  if (fused && h->system == CHEMORA_SYS_BSSN && h->order == 8)
+    return fail(h, CHEMORA_EINVAL, "8th-order BSSN has the derivative-split variant only");
   h->fused = fused;
   h->tile = tile_id;
   return CHEMORA_OK;
@@ -381,7 +383,8 @@ int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out)
   for (int f = 1; f >= 0 && !rc; --f)
     for (int t = 0; t < CHEMORA_NUM_TILES && !rc; ++t) {
       float ms = -1.f;
-      if ((f == 1 && (h->system == CHEMORA_SYS_BSSN || t < 6)) || (f == 0 && h->system == CHEMORA_SYS_BSSN && t < 6)) {
+      const bool bssn = h->system == CHEMORA_SYS_BSSN, o8 = bssn && h->order == 8;   // O8 BSSN: split variant only
+      if ((f == 1 && !o8 && (bssn || t < 6)) || (f == 0 && bssn && t < 6)) {
         h->fused = f; h->tile = t;
         // a middle RK4 stage (the common case) on scratch operands: k = f(U); S += 2k; Ya = U + a k.
         // S and Ya are scratch between steps (stage 1 overwrites them); U is only read.

@@ -142,7 +142,7 @@ cudaError_t kernel_info_wave1(int order, int tile, cudaFuncAttributes* a);
 cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int tile, const Stage& st, cudaStream_t s);
 cudaError_t launch_bssn_ws(const Layout& L, const Coef& C, int which, const Stage& st, cudaStream_t s);
 cudaError_t kernel_info_bssn_ws(int which, cudaFuncAttributes* a);
-cudaError_t launch_bssn_derivs(const Layout& L, const Coef& C, int tile, const double* in, double* derivs,
+cudaError_t launch_bssn_derivs(const Layout& L, const Coef& C, int order, int tile, const double* in, double* derivs,
                                cudaStream_t s);
 cudaError_t launch_bssn_from_derivs(const Layout& L, const Coef& C, int tile, const double* derivs,
                                     const Stage& st, cudaStream_t s);

@@ -19,21 +19,25 @@ __device__ __forceinline__ constexpr int slot_d2(int v, int a, int b) {
 __device__ __forceinline__ constexpr int slot_ad(int v) { return 111 + v; }
 
 // differentiates on the fly from a point accessor P
-template <class P>
+template <class P, int ORDER = 4>
 struct OnTheFly {
   P pt;
   Coef C;
   double beta[3];
   __device__ __forceinline__ double f(int v) const { return pt.at(v, 0, 0, 0); }
-  __device__ __forceinline__ double d1(int v, int a) const { return d1_o4(pt, v, a, C.inv_h); }
+  __device__ __forceinline__ double d1(int v, int a) const {
+    return ORDER == 4 ? d1_o4(pt, v, a, C.inv_h) : d1_o8(pt, v, a, C.inv_h);
+  }
   __device__ __forceinline__ double d2(int v, int a, int b) const {
-    return a == b ? d2_o4(pt, v, a, C.inv_h2) : dmix_o4(pt, v, a, b, C.inv_h2);
+    if (ORDER == 4) return a == b ? d2_o4(pt, v, a, C.inv_h2) : dmix_o4(pt, v, a, b, C.inv_h2);
+    return a == b ? d2_o8(pt, v, a, C.inv_h2) : dmix_o8(pt, v, a, b, C.inv_h2);
+  }
+  __device__ __forceinline__ double adv(int v, int a) const {
+    return ORDER == 4 ? adv_o4(pt, v, a, beta[a], C.inv_h) : adv_o8(pt, v, a, beta[a], C.inv_h);
   }
   __device__ __forceinline__ double ad(int v) const {
     double r = ko5(pt, v, C.ko);
-    if (v != V_A)
-      r += (adv_o4(pt, v, 0, beta[0], C.inv_h) + adv_o4(pt, v, 1, beta[1], C.inv_h)) +
-           adv_o4(pt, v, 2, beta[2], C.inv_h);
+    if (v != V_A) r += (adv(v, 0) + adv(v, 1)) + adv(v, 2);
     return r;
   }
 };
@@ -55,7 +59,7 @@ __host__ __device__ inline long packed_stride(const Layout& L) {
   return (n + 15) / 16 * 16;
 }
 
-template <int TX, int TY, int TZ>
+template <int TX, int TY, int TZ, int ORDER>
 __global__ void __launch_bounds__(TX* TY) bssn_derivs_kernel(Layout L, Coef C, const double* __restrict__ in,
                                                             double* __restrict__ derivs) {
   const int i = blockIdx.x * TX + threadIdx.x, j = blockIdx.y * TY + threadIdx.y;
@@ -68,7 +72,7 @@ __global__ void __launch_bounds__(TX* TY) bssn_derivs_kernel(Layout L, Coef C, c
     if (k >= L.nz) break;
     const long q = (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.xo);
     double* o = derivs + ((long)k * L.ny + j) * L.nx + i;
-    OnTheFly<GlobalPoint> D{{in + q, L.pitch, L.plane, L.vstride}, C, {0, 0, 0}};
+    OnTheFly<GlobalPoint, ORDER> D{{in + q, L.pitch, L.plane, L.vstride}, C, {0, 0, 0}};
     D.beta[0] = D.f(V_BETA); D.beta[1] = D.f(V_BETA + 1); D.beta[2] = D.f(V_BETA + 2);
 #pragma unroll
     for (int v = 0; v < 25; ++v) {
@@ -112,7 +116,11 @@ static cudaError_t bssn_go(int which, const Layout& L, const Coef& C, const Stag
                            double* derivs, cudaStream_t s, cudaFuncAttributes* a) {
   dim3 grid((L.nx + TX - 1) / TX, (L.ny + TY - 1) / TY, (L.nz + TZ - 1) / TZ), block(TX, TY);
   if (which == 1) {
-    auto kern = bssn_derivs_kernel<TX, TY, TZ>;
+    auto kern = bssn_derivs_kernel<TX, TY, TZ, 4>;
+    if (a) return cudaFuncGetAttributes(a, kern);
+    kern<<<grid, block, 0, s>>>(L, C, in, derivs);
+  } else if (which == 3) {   // 8th-order derivatives (the paper's configuration; split variant only)
+    auto kern = bssn_derivs_kernel<TX, TY, TZ, 8>;
     if (a) return cudaFuncGetAttributes(a, kern);
     kern<<<grid, block, 0, s>>>(L, C, in, derivs);
   } else {
@@ -136,9 +144,9 @@ static cudaError_t bssn_dispatch(int which, int tile, const Layout& L, const Coe
   return cudaErrorInvalidValue;
 }
 
-cudaError_t launch_bssn_derivs(const Layout& L, const Coef& C, int tile, const double* in, double* derivs,
+cudaError_t launch_bssn_derivs(const Layout& L, const Coef& C, int order, int tile, const double* in, double* derivs,
                                cudaStream_t s) {
-  return bssn_dispatch(1, tile, L, C, nullptr, in, derivs, s, nullptr);
+  return bssn_dispatch(order == 8 ? 3 : 1, tile, L, C, nullptr, in, derivs, s, nullptr);
 }
 cudaError_t launch_bssn_from_derivs(const Layout& L, const Coef& C, int tile, const double* derivs, const Stage& st,
                                     cudaStream_t s) {

@@ -99,6 +99,38 @@ __device__ __forceinline__ double d1_o8(const P& f, int v, int a, double inv_h) 
   return ((672.0 * e1 - 168.0 * e2) + (32.0 * e3 - 3.0 * e4)) * (inv_h * (1.0 / 840.0));
 }
 
+// mixed derivative: the 1-D first-derivative stencil along a applied to the one along b (64 points)
+template <class P>
+__device__ __forceinline__ double dmix_o8(const P& f, int v, int a, int b, double inv_h2) {
+  double r[8];
+  const int off[8] = {1, -1, 2, -2, 3, -3, 4, -4};
+#pragma unroll
+  for (int t = 0; t < 8; ++t) {
+    const int m = off[t];
+    const double e1 = f.ax2(v, a, m, b, 1) - f.ax2(v, a, m, b, -1);
+    const double e2 = f.ax2(v, a, m, b, 2) - f.ax2(v, a, m, b, -2);
+    const double e3 = f.ax2(v, a, m, b, 3) - f.ax2(v, a, m, b, -3);
+    const double e4 = f.ax2(v, a, m, b, 4) - f.ax2(v, a, m, b, -4);
+    r[t] = (672.0 * e1 - 168.0 * e2) + (32.0 * e3 - 3.0 * e4);
+  }
+  return ((672.0 * (r[0] - r[1]) - 168.0 * (r[2] - r[3])) + (32.0 * (r[4] - r[5]) - 3.0 * (r[6] - r[7]))) *
+         (inv_h2 * (1.0 / (840.0 * 840.0)));
+}
+
+// beta^a * upwinded d_a f at 8th order: offsets -3..+5 on the side of beta,
+// (-5, 60, -420, -378, 1050, -420, 140, -30, 3)/840h, in differences from the centre value (5 ghosts)
+template <class P>
+__device__ __forceinline__ double adv_o8(const P& f, int v, int a, double beta, double inv_h) {
+  const double f0 = f.at(v, 0, 0, 0);
+  const int s = beta > 0.0 ? 1 : -1;
+  const double m3 = f.ax(v, a, -3 * s) - f0, m2 = f.ax(v, a, -2 * s) - f0, m1 = f.ax(v, a, -s) - f0;
+  const double p1 = f.ax(v, a, s) - f0, p2 = f.ax(v, a, 2 * s) - f0, p3 = f.ax(v, a, 3 * s) - f0;
+  const double p4 = f.ax(v, a, 4 * s) - f0, p5 = f.ax(v, a, 5 * s) - f0;
+  const double r = ((1050.0 * p1 - 420.0 * m1) + (60.0 * m2 - 420.0 * p2)) + ((140.0 * p3 - 5.0 * m3) + (3.0 * p5 - 30.0 * p4));
+  const double sb = beta > 0.0 ? beta : -beta;   // beta * side = |beta|
+  return sb * r * (inv_h * (1.0 / 840.0));
+}
+
 // 2nd derivative (-9,128,-1008,8064,-14350,8064,-1008,128,-9)/5040h^2
 template <class P>
 __device__ __forceinline__ double d2_o8(const P& f, int v, int a, double inv_h2) {

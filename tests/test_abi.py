@@ -42,6 +42,7 @@ def test_tile_table(binding):
     (8, 8, 8, 1, 4, 0, 0.1),      # wave O4 needs g >= 2
     (8, 8, 8, 3, 8, 0, 0.1),      # wave O8 needs g >= 4
     (8, 8, 8, 2, 4, 1, 0.1),      # BSSN O4 upwinded needs g >= 3 (PAPER.md:382 rule order/2+1)
+    (8, 8, 8, 4, 8, 1, 0.1),      # BSSN O8 upwinded needs g >= 5
     (8, 8, 8, 3, 6, 1, 0.1),      # order not in {4,8}
     (8, 8, 8, 3, 4, 3, 0.1),      # unknown system
     (8, 8, 8, 3, 8, 2, 0.1),      # first-order wave system O8 needs g >= 4

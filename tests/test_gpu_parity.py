@@ -336,3 +336,42 @@ def test_bssn_rk3_split_variant(chem, oracle):
     st = oracle.rk3(1, oracle.with_ghosts(u0, 3), 3, 4, dx, dt, oracle.params(eps_diss=eps), 3)
     assert relerr(h.get_state(), oracle.interior(st, 3)) < TOL_BSSN_10_STEPS
     h.destroy()
+
+
+# ------------------------------------------------------------------ 8th-order BSSN, 5 ghost zones
+@pytest.mark.parametrize("data", ["noise1e-10", "strong"])
+def test_bssn_o8_rhs(chem, oracle, data):
+    """the paper's configuration: 8th-order centred FD, upwinded advection over offsets -3..+5"""
+    nx, ny, nz, g = 21, 14, 11, 5
+    u = inputs.bssn_noise(nx, ny, nz) if data == "noise1e-10" else strong_field(nx, ny, nz, seed=41)
+    dx, eps = 0.05, 0.1
+    want = oracle_rhs(oracle, 1, u, g, 8, dx, eps_diss=eps)
+    h = chem.Chemora(nx, ny, nz, g, 8, 1, dx)
+    h.set_param("eps_diss", eps)
+    assert h.get_variant()[0] == 0                      # split variant only
+    with pytest.raises(chem.ChemoraError):
+        h.set_variant(1, 0)
+    for tile in range(6):
+        h.set_variant(0, tile)
+        assert relerr(gpu_rhs(h, u), want) < TOL_RHS, tile
+    h.destroy()
+
+
+def test_bssn_o8_rk4_10_steps_and_rk3_enforced(chem, oracle):
+    nx, ny, nz, g = 20, 16, 12, 5
+    u0 = inputs.bssn_noise(nx, ny, nz)
+    dx, dt, eps = 0.05, 0.0125, 0.1
+    h = chem.Chemora(nx, ny, nz, g, 8, 1, dx)
+    h.set_param("eps_diss", eps)
+    h.set_state(u0)
+    for _ in range(10):
+        h.rk4_step(dt)
+    st = oracle.rk4(1, oracle.with_ghosts(u0, g), g, 8, dx, dt, oracle.params(eps_diss=eps), 10)
+    assert relerr(h.get_state(), oracle.interior(st, g)) < TOL_BSSN_10_STEPS
+    h.set_state(u0)
+    for _ in range(5):
+        h.rk3_step(dt)
+        h.enforce_constraints()
+    st = oracle.rk3(1, oracle.with_ghosts(u0, g), g, 8, dx, dt, oracle.params(eps_diss=eps), 5, True)
+    assert relerr(h.get_state(), oracle.interior(st, g)) < TOL_BSSN_10_STEPS
+    h.destroy()
