@@ -687,6 +687,20 @@ void oracle_rk3(int system, double* U, int nx, int ny, int nz, int g, int order,
   }
 }
 
+// The "Energy" calculation of the paper's Sample 1: eps = 1/2 (rho^2 + delta^ij v_i v_j) at every
+// interior point of a ghosted system-2 state, written to a packed nz x ny x nx array.
+void oracle_energy(const double* U, int nx, int ny, int nz, int g, double* eps) {
+  Grid G = make_grid(nx, ny, nz, g, 4, 1.0);
+  const long n = G.npts();
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) {
+        long p = idx(G, i, j, k);
+        double rho = U[n + p], v1 = U[2 * n + p], v2 = U[3 * n + p], v3 = U[4 * n + p];
+        eps[((long)k * ny + j) * nx + i] = 0.5 * (rho * rho + ((v1 * v1 + v2 * v2) + v3 * v3));
+      }
+}
+
 void oracle_enforce(double* U, int nx, int ny, int nz, int g) {
   Grid G = make_grid(nx, ny, nz, g, 4, 1.0);
   enforce_constraints(U, G);

@@ -43,6 +43,8 @@ def lib():
         _lib.oracle_rk4.argtypes = [i, dp, i, i, i, i, i, d, d, dp, i]
         _lib.oracle_rk3.argtypes = [i, dp, i, i, i, i, i, d, d, dp, i, i]
         _lib.oracle_enforce.argtypes = [dp, i, i, i, i]
+        _lib.oracle_energy.argtypes = [dp, i, i, i, i, dp]
+        _lib.oracle_energy.restype = None
         _lib.oracle_rk3.restype = None
         _lib.oracle_enforce.restype = None
         _lib.oracle_set_threads.argtypes = [i]
@@ -131,3 +133,12 @@ def enforce(state, g):
     assert V == 25
     lib().oracle_enforce(_p(state), tx - 2 * g, ty - 2 * g, tz - 2 * g, g)
     return state
+
+
+def energy(state, g):
+    """eps = 1/2 (rho^2 + v_i v_i) of a ghosted system-2 state on its interior: array [nz, ny, nx]."""
+    V, tz, ty, tx = state.shape
+    assert V == 5
+    out = np.empty((tz - 2 * g, ty - 2 * g, tx - 2 * g), dtype=np.float64)
+    lib().oracle_energy(_p(state), tx - 2 * g, ty - 2 * g, tz - 2 * g, g, _p(out))
+    return out

@@ -74,3 +74,18 @@ def test_W3_gaussian_pulse_keeps_energy(oracle):
     u1 = oracle.interior(st, g)
     e1 = 0.5 * (u1[1] ** 2 + (u1[2:] ** 2).sum(0)).sum()
     assert abs(e1 / e0 - 1.0) < 1e-6 and np.abs(u1[2:]).max() > 1e-3     # conserved, and something did propagate
+
+
+def test_W4_energy_closed_forms(oracle):
+    """eps = 1/2 (rho^2 + v_i v_i): u does not enter, every v_i enters once with weight 1/2"""
+    g = 2
+    u = np.zeros((5, 4, 5, 6))
+    u[0] = 7.0                                   # u must not contribute
+    u[1], u[2], u[3], u[4] = 3.0, 1.0, 2.0, 2.0
+    assert np.array_equal(oracle.energy(oracle.with_ghosts(u, g), g), np.full((4, 5, 6), 9.0))
+    for c, val in [(1, 2.0), (2, 4.0), (3, 6.0), (4, 8.0)]:
+        e = np.zeros((5, 4, 5, 6)); e[c] = val
+        assert np.array_equal(oracle.energy(oracle.with_ghosts(e, g), g), np.full((4, 5, 6), 0.5 * val * val))
+    # the energy the conservation pin W3 sums is this field
+    w = inputs.wave1_gaussian(8, 8, 8)
+    assert np.isclose(oracle.energy(oracle.with_ghosts(w, g), g).sum(), 0.5 * (w[1] ** 2).sum(), rtol=1e-15)
