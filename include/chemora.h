@@ -111,6 +111,12 @@ int chemora_rk3_step(chemora_t* h, double dt);
  * CHEMORA_EINVAL for the wave systems. */
 int chemora_enforce_constraints(chemora_t* h, double* dev_state);
 
+/* The "Energy" calculation of the paper's Sample 1 for the first-order wave system:
+ * eps = 1/2 (rho^2 + delta^ij v_i v_j) at every interior point of dev_state (padded layout; NULL: U).
+ * dev_eps, if not NULL, receives the field packed nz x ny x nx (device); host_sum, if not NULL, the sum of eps over
+ * the grid (then the call synchronises the stream).  CHEMORA_EINVAL for the other systems. */
+int chemora_energy(chemora_t* h, const double* dev_state, double* dev_eps, double* host_sum);
+
 /* Kernel variant: fused (1: derivatives + RHS + RK stage update in one kernel) or split (0: derivatives
  * written to global arrays by one kernel, RHS + stage update by a second), and tile_id in
  * [0, CHEMORA_NUM_TILES).  chemora_tile_shape reports the (x, y, z) extent of a tile id: for the fused BSSN

@@ -21,7 +21,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 # every symbol include/chemora.h declares (tests check that the library exports all of them)
 SYMBOLS = ["chemora_create", "chemora_set_param", "chemora_get_param", "chemora_layout", "chemora_state_ptr",
            "chemora_set_state", "chemora_get_state", "chemora_set_state_dev", "chemora_get_state_dev",
-           "chemora_fill_ghosts", "chemora_rhs", "chemora_rk4_step", "chemora_rk3_step", "chemora_enforce_constraints", "chemora_set_variant",
+           "chemora_fill_ghosts", "chemora_rhs", "chemora_rk4_step", "chemora_rk3_step", "chemora_enforce_constraints", "chemora_energy", "chemora_set_variant",
            "chemora_get_variant", "chemora_tile_shape", "chemora_autotune", "chemora_launch_count",
            "chemora_kernel_info", "chemora_timing", "chemora_timing_read", "chemora_measure_fp64_peak", "chemora_last_error", "chemora_destroy"]
 
@@ -60,6 +60,7 @@ def load():
         "chemora_rk4_step": [vp, d],
         "chemora_rk3_step": [vp, d],
         "chemora_enforce_constraints": [vp, vp],
+        "chemora_energy": [vp, vp, vp, dp],
         "chemora_set_variant": [vp, i, i], "chemora_get_variant": [vp, ip, ip],
         "chemora_tile_shape": [i, i, i, ip, ip, ip],
         "chemora_autotune": [vp, ip, ip, ctypes.POINTER(ctypes.c_float)],
@@ -210,6 +211,16 @@ class Chemora:
     def enforce_constraints(self, state=None):
         """in place on a padded device state tensor (default: U)"""
         self._ck(self.lib.chemora_enforce_constraints(self._h, None if state is None else state.data_ptr()))
+
+    def energy(self, state=None, field=False):
+        """Sample-1 energy of a padded device state (default U): the grid sum, and the packed field if asked."""
+        import torch
+        total = ctypes.c_double()
+        nx, ny, nz = self.dims
+        eps = torch.empty((nz, ny, nx), dtype=torch.float64, device=self.device) if field else None
+        self._ck(self.lib.chemora_energy(self._h, None if state is None else state.data_ptr(),
+                                         None if eps is None else eps.data_ptr(), ctypes.byref(total)))
+        return (total.value, eps) if field else total.value
 
     def set_variant(self, fused, tile_id):
         self._ck(self.lib.chemora_set_variant(self._h, int(fused), int(tile_id)))

@@ -344,6 +344,21 @@ int chemora_enforce_constraints(chemora_t* h, double* dev_state) {
   return CHEMORA_OK;
 }
 
+int chemora_energy(chemora_t* h, const double* dev_state, double* dev_eps, double* host_sum) {
+  if (!h) return CHEMORA_EINVAL;
+  if (h->system != CHEMORA_SYS_WAVE1) return fail(h, CHEMORA_EINVAL, "the energy calculation belongs to the first-order wave system");
+  int rc = ensure_staging(h);   // first 8 bytes of the staging buffer hold the sum
+  if (rc) return rc;
+  CK(h, cudaMemsetAsync(h->staging, 0, sizeof(double), h->stream), "energy memset");
+  CK(h, launch_energy(h->L, dev_state ? dev_state : h->buf[0], dev_eps, h->staging, h->stream), "energy launch");
+  h->launches += 1;
+  if (host_sum) {
+    CK(h, cudaMemcpyAsync(host_sum, h->staging, sizeof(double), cudaMemcpyDeviceToHost, h->stream), "energy D2H");
+    CK(h, cudaStreamSynchronize(h->stream), "energy sync");
+  }
+  return CHEMORA_OK;
+}
+
 int chemora_set_variant(chemora_t* h, int fused, int tile_id) {
   if (!h || tile_id < 0 || tile_id >= CHEMORA_NUM_TILES || (fused != 0 && fused != 1)) return CHEMORA_EINVAL;
   if (!fused && h->system != CHEMORA_SYS_BSSN) return fail(h, CHEMORA_EINVAL, "wave systems have no split variant");

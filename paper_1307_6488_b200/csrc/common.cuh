@@ -134,6 +134,7 @@ static const TileShape kTilesMarch[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64
 
 // launchers implemented in the kernel translation units; each returns the cudaError_t of the launch
 cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s);
+cudaError_t launch_energy(const Layout& L, const double* state, double* eps_out, double* sum, cudaStream_t s);
 cudaError_t launch_enforce(const Layout& L, double* state, cudaStream_t s);
 cudaError_t launch_pack(const Layout& L, const double* packed, double* state, bool to_state, cudaStream_t s);
 cudaError_t launch_wave(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);

@@ -241,6 +241,41 @@ cudaError_t kernel_info_wave1(int order, int tile, cudaFuncAttributes* a) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// "Energy" calculation of the paper's Sample 1: eps = 1/2 (rho^2 + v_i v_i) at every interior
+// point of a system-2 state (optionally stored, packed nz x ny x nx) and its sum over the grid.
+// One rounding per operation in the association of the definition, so the field is reproducible bit for bit.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) energy_kernel(Layout L, const double* __restrict__ state,
+                                                     double* __restrict__ eps_out, double* __restrict__ sum) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  double e = 0.0;
+  if (i < L.nx) {
+    const long p = (long)(k + L.g) * L.plane + (long)(j + L.g) * L.pitch + (i + L.xo);
+    const double rho = state[L.vstride + p], v1 = state[2 * L.vstride + p], v2 = state[3 * L.vstride + p],
+                 v3 = state[4 * L.vstride + p];
+    e = __dmul_rn(0.5, __dadd_rn(__dmul_rn(rho, rho),
+                                 __dadd_rn(__dadd_rn(__dmul_rn(v1, v1), __dmul_rn(v2, v2)), __dmul_rn(v3, v3))));
+    if (eps_out) eps_out[((long)k * L.ny + j) * L.nx + i] = e;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) e += __shfl_down_sync(0xffffffffu, e, o);
+  __shared__ double part[8];
+  if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = e;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += part[w];
+    atomicAdd(sum, t);
+  }
+}
+
+cudaError_t launch_energy(const Layout& L, const double* state, double* eps_out, double* sum, cudaStream_t s) {
+  dim3 grid((L.nx + 255) / 256, L.ny, L.nz);
+  energy_kernel<<<grid, 256, 0, s>>>(L, state, eps_out, sum);
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------
 // FP64 peak probe: 8 independent register-resident DFMA chains per thread.
 // flops = blocks * threads * iters * 8 chains * 2.
 // ---------------------------------------------------------------------------------------------------

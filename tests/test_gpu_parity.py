@@ -375,3 +375,29 @@ def test_bssn_o8_rk4_10_steps_and_rk3_enforced(chem, oracle):
     st = oracle.rk3(1, oracle.with_ghosts(u0, g), g, 8, dx, dt, oracle.params(eps_diss=eps), 5, True)
     assert relerr(h.get_state(), oracle.interior(st, g)) < TOL_BSSN_10_STEPS
     h.destroy()
+
+
+def test_wave1_energy(chem, oracle):
+    """the Energy calculation of the paper's Sample 1: field bit-exact, grid sum to summation-order accuracy, and
+    conserved by the evolution of the paper's Gaussian pulse"""
+    n, g = 32, 2
+    u = np.random.default_rng(71).standard_normal((5, 9, 11, 37))
+    h = chem.Chemora(37, 11, 9, g, 4, chem.SYS_WAVE1, 0.1)
+    h.set_state(u)
+    total, eps = h.energy(field=True)
+    want = oracle.energy(oracle.with_ghosts(u, g), g)
+    assert np.array_equal(eps.cpu().numpy(), want)
+    assert abs(total - want.sum()) < 1e-13 * want.sum()
+    h.destroy()
+    u0 = inputs.wave1_gaussian(n, n, n)
+    h = chem.Chemora(n, n, n, g, 4, chem.SYS_WAVE1, 1.0 / n)
+    h.set_state(u0)
+    e0 = h.energy()
+    for _ in range(20):
+        h.rk4_step(0.25 / n)
+    assert abs(h.energy() / e0 - 1.0) < 1e-6
+    h.destroy()
+    b = chem.Chemora(8, 8, 8, 3, 4, chem.SYS_BSSN, 0.1)
+    with pytest.raises(chem.ChemoraError):
+        b.energy()
+    b.destroy()
