@@ -277,6 +277,44 @@ def run_sweep(args):
     print(json.dumps({"metric": "BSSN RHS variant sweep (configs[4])", "unit": "ms per RHS evaluation", "rows": table}))
 
 
+def run_wave(args):
+    """configs[1]: wave (phi, pi) 256^3, O8 + KO eps=0.1, 8 plane waves; RK4 steps; HBM roofline at 272 B per update."""
+    import torch
+    from paper_1307_6488_b200 import binding, inputs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device and no CPU fallback")
+    c = inputs.config(1, scale=args.size)
+    n = args.size
+    h = binding.Chemora(n, n, n, c["ghost"], c["order"], binding.SYS_WAVE, c["dx"])
+    h.set_param("eps_diss", c["eps_diss"])
+    h.set_state(c["state"]())
+    fused, tile, sweep_ms = h.autotune()
+    dt = 0.25 * c["dx"]
+    for _ in range(max(args.warmup, 3)):
+        h.rk4_step(dt)
+    torch.cuda.synchronize()
+    h.timing(1)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        h.rk4_step(dt)
+    e1.record(); torch.cuda.synchronize()
+    kt = h.timing_read(); h.timing(0)
+    ms = e0.elapsed_time(e1) / args.steps
+    pk, pk_src = peaks()
+    rhs_ms = kt["rhs_ms"] / max(kt["rhs_launches"], 1)
+    ach = 68.0 * n ** 3 / (rhs_ms * 1e-3) / 1e9
+    print(json.dumps({"metric": "wave (phi, pi) RHS+RK4 grid-point updates/sec, fp64 8th-order + KO, %d^3" % n,
+                      "value": n ** 3 / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms,
+                      "config": {"workload": "configs[1]", "tile_id": tile, "tile": list(binding.tile_shape(tile, binding.SYS_WAVE, 1)),
+                                 "sweep_ms": sweep_ms[binding.NUM_TILES:]},
+                      "roofline": {"bound": "hbm", "kernel": "wave_tma_kernel" if 6 <= tile < 9 else "wave_kernel",
+                                   "achieved": ach, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": ach / pk["hbm_gbs"],
+                                   "ms_per_launch": rhs_ms, "algorithmic_bytes_per_point_per_launch": 68.0,
+                                   "peak_source": pk_src, "fill_share_of_step": kt["fill_ms"] / (ms * args.steps)}}))
+    h.destroy()
+
+
 def run_paper_shape(args):
     """The shape of the paper's own single-GPU benchmark: BSSN, 8th-order FD, 5 ghost zones,
     RK3 (+ constraint enforcement), 100^3 evolved points; synthetic Minkowski + 1e-4 Gaussians.  Context line, not the
@@ -321,10 +359,13 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=64)
     ap.add_argument("--ref-sample", type=int, default=64)
     ap.add_argument("--sweep", action="store_true", help="configs[4] variant/tile sweep instead of the headline run")
+    ap.add_argument("--wave", action="store_true", help="configs[1]: the (phi, pi) wave system at 256^3, O8 + KO")
     ap.add_argument("--paper-shape", action="store_true", help="BSSN O8 + RK3 at 100^3 (the paper's own benchmark shape)")
     args = ap.parse_args()
     if args.sweep:
         run_sweep(args)
+    elif args.wave:
+        run_wave(args)
     elif args.paper_shape:
         run_paper_shape(args)
     elif args.impl == "reference":

@@ -110,7 +110,10 @@ int run_rhs_inner(chemora_t* h, const Stage& st) {
   if (h->eps_diss != 0.0 && h->L.g < 3) return fail(h, CHEMORA_EINVAL, "eps_diss != 0 needs ghost >= 3 (KO order 5)");
   Coef C = make_coef(h);
   if (h->system == CHEMORA_SYS_WAVE) {
-    CK(h, launch_wave(h->L, C, h->order, h->tile % 6, st, h->stream), "wave kernel launch");
+    if (h->tile >= 6 && h->tile < 9 && wave_tma_ok(h->L, h->order, C.ko != 0.0))
+      CK(h, launch_wave_tma(h->L, C, h->order, h->tile - 6, st, h->stream), "wave plane-ring kernel launch");
+    else
+      CK(h, launch_wave(h->L, C, h->order, h->tile % 6, st, h->stream), "wave kernel launch");
     h->launches += 1;
   } else if (h->system == CHEMORA_SYS_WAVE1) {
     CK(h, launch_wave1(h->L, C, h->order, h->tile % 6, st, h->stream), "first-order wave kernel launch");
@@ -379,7 +382,9 @@ int chemora_get_variant(const chemora_t* h, int* fused, int* tile_id) {
 int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, int* tz) {
   if (tile_id < 0 || tile_id >= CHEMORA_NUM_TILES) return CHEMORA_EINVAL;
   const bool f = system_id == CHEMORA_SYS_BSSN && fused;
-  const TileShape T = f ? kTilesFused[tile_id] : kTilesMarch[tile_id % 6];
+  const TileShape T = f ? kTilesFused[tile_id]
+                      : (system_id == CHEMORA_SYS_WAVE && tile_id >= 6 && tile_id < 9) ? kTilesWaveTma[tile_id - 6]
+                                                                                        : kTilesMarch[tile_id % 6];
   if (tx) *tx = T.tx;
   if (ty) *ty = T.ty;
   if (tz) *tz = T.tz;
@@ -399,7 +404,8 @@ int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out)
     for (int t = 0; t < CHEMORA_NUM_TILES && !rc; ++t) {
       float ms = -1.f;
       const bool bssn = h->system == CHEMORA_SYS_BSSN, o8 = bssn && h->order == 8;   // O8 BSSN: split variant only
-      if ((f == 1 && !o8 && (bssn || t < 6)) || (f == 0 && bssn && t < 6)) {
+      const int nwave = h->system == CHEMORA_SYS_WAVE ? 9 : 6;   // (phi, pi) has three more ids: the plane-ring kernel
+      if ((f == 1 && !o8 && (bssn || t < nwave)) || (f == 0 && bssn && t < 6)) {
         h->fused = f; h->tile = t;
         // a middle RK4 stage (the common case) on scratch operands: k = f(U); S += 2k; Ya = U + a k.
         // S and Ya are scratch between steps (stage 1 overwrites them); U is only read.
@@ -462,7 +468,8 @@ int chemora_timing_read(chemora_t* h, double* rhs_ms, long* rhs_launches, double
 int chemora_kernel_info(const chemora_t* h, int* regs, int* local_bytes, int* smem_bytes) {
   if (!h) return CHEMORA_EINVAL;
   cudaFuncAttributes a;
-  cudaError_t e = h->system == CHEMORA_SYS_WAVE ? kernel_info_wave(h->order, h->tile % 6, &a)
+  cudaError_t e = h->system == CHEMORA_SYS_WAVE && h->tile >= 6 && h->tile < 9 ? kernel_info_wave_tma(h->order, h->tile - 6, &a)
+                  : h->system == CHEMORA_SYS_WAVE ? kernel_info_wave(h->order, h->tile % 6, &a)
                   : h->system == CHEMORA_SYS_WAVE1 ? kernel_info_wave1(h->order, h->tile % 6, &a)
                   : !h->fused              ? kernel_info_bssn_split(1, h->tile % 6, &a)
                   : h->tile >= 6 && h->tile < 9 ? kernel_info_bssn_ws(h->tile - 6, &a)

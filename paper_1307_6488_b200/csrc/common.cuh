@@ -130,6 +130,8 @@ struct TileShape { int tx, ty, tz; };
 // ids 9..10: the uniform kernel on 384-point tiles (12 warps, live values parked in tensor memory)
 static const TileShape kTilesFused[11] = {{16, 4, 4}, {16, 8, 2}, {8, 8, 4}, {8, 4, 8}, {16, 2, 8}, {16, 4, 2},
                                           {16, 4, 4}, {16, 8, 2}, {16, 2, 8}, {16, 4, 6}, {16, 6, 4}};
+// wave system ids 6..8: the TMA plane-ring kernel (x, y = thread block, z = planes per work item)
+static const TileShape kTilesWaveTma[3] = {{32, 16, 32}, {32, 16, 64}, {64, 8, 32}};
 static const TileShape kTilesMarch[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64, 4, 8}, {128, 2, 8}, {16, 16, 8}};
 
 // launchers implemented in the kernel translation units; each returns the cudaError_t of the launch
@@ -138,6 +140,9 @@ cudaError_t launch_energy(const Layout& L, const double* state, double* eps_out,
 cudaError_t launch_enforce(const Layout& L, double* state, cudaStream_t s);
 cudaError_t launch_pack(const Layout& L, const double* packed, double* state, bool to_state, cudaStream_t s);
 cudaError_t launch_wave(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
+cudaError_t launch_wave_tma(const Layout& L, const Coef& C, int order, int which, const Stage& st, cudaStream_t s);
+cudaError_t kernel_info_wave_tma(int order, int which, cudaFuncAttributes* a);
+bool wave_tma_ok(const Layout& L, int order, bool ko);
 cudaError_t launch_wave1(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
 cudaError_t kernel_info_wave1(int order, int tile, cudaFuncAttributes* a);
 cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int tile, const Stage& st, cudaStream_t s);
