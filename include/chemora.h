@@ -54,8 +54,8 @@ enum { CHEMORA_NUM_TILES = 11 };
  * fd_order (4 or 8), system system_id and grid spacing dx (same in x, y, z).
  * Rejects (CHEMORA_EINVAL): non-positive dims, dims < ghost (periodic images would overlap),
  * fd_order not in {4,8}, ghost < fd_order/2 (wave), ghost < fd_order/2 + 1 (BSSN: upwinded advection,
- * 5 ghost zones at 8th order, the paper's configuration), dx <= 0.  8th-order BSSN runs through the
- * derivative-split variant only (chemora_set_variant(h, 1, ...) is rejected for it).  Dissipation (eps_diss != 0, KO order 5)
+ * 5 ghost zones at 8th order, the paper's configuration), dx <= 0.  For 8th-order BSSN the fused kernel
+ * exists for tile id 0 only (other fused ids are rejected by chemora_set_variant); all six split tiles work.  Dissipation (eps_diss != 0, KO order 5)
  * needs ghost >= 3; that is checked when the parameter is set and again at launch.
  * cuda_stream: a cudaStream_t (may be NULL = default stream).
  * alloc/dealloc: optional device allocator callbacks (e.g. torch's caching allocator); alloc(bytes, ctx)

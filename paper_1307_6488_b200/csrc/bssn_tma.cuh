@@ -263,6 +263,73 @@ __device__ __forceinline__ double var_ad(const P& p, const AdvW& w) {
   return ad;
 }
 
+// ---- 8th order (the paper's configuration: 5 ghost zones) -------------------------------------
+// Centred: d1 (3,-32,168,-672,0,672,-168,32,-3)/840h, d2 (-9,128,-1008,8064,-14350,...)/5040h^2.  The two one-sided
+// upwind stencils over offsets -3..+5 (-5,60,-420,-378,1050,-420,140,-30,3)/840h split into an antisymmetric part
+//   A = 735 e1 - 240 e2 + 72.5 e3 - 15 e4 + 1.5 e5   and a symmetric part   S = 315 s1 - 180 s2 + 67.5 s3 - 15 s4 + 1.5 s5
+// (e_k = u[+k] - u[-k], s_k = (u[+k]-u0) + (u[-k]-u0)):  up(+-) = (A +- S)/840h, so
+//   beta d^up u + KO(u) = ws A + wq S + ko q5,   ws = beta/840h, wq = |beta|/840h, q5 = s3 - 6 s2 + 15 s1.
+template <class P, bool D1, bool D2>
+__device__ __forceinline__ void axis8(const P& p, double f0, int a, const Coef& C, const AdvW& w, double& d1, double& d2,
+                                      double& ad) {
+  double e[6], s[6];
+#pragma unroll
+  for (int k = 1; k <= 5; ++k) {
+    const double pk = p.ax(a, k), mk = p.ax(a, -k);
+    e[k] = pk - mk;
+    s[k] = (pk - f0) + (mk - f0);
+  }
+  if (D1) d1 = ((672.0 * e[1] - 168.0 * e[2]) + (32.0 * e[3] - 3.0 * e[4])) * (C.inv_h * (1.0 / 840.0));
+  if (D2) d2 = ((8064.0 * s[1] - 1008.0 * s[2]) + (128.0 * s[3] - 9.0 * s[4])) * (C.inv_h2 * (1.0 / 5040.0));
+  const double A = ((735.0 * e[1] - 240.0 * e[2]) + (72.5 * e[3] - 15.0 * e[4])) + 1.5 * e[5];
+  const double S = ((315.0 * s[1] - 180.0 * s[2]) + (67.5 * s[3] - 15.0 * s[4])) + 1.5 * s[5];
+  const double q5 = (s[3] - 6.0 * s[2]) + 15.0 * s[1];
+  const double c = (w.ws[a] * A + w.wq[a] * S) + C.ko * q5;
+  ad = a == 0 ? c : ad + c;
+}
+// mixed derivative d_a d_b (a != b) at 8th order, 64 reads
+template <class P>
+__device__ __forceinline__ double mixed8(const P& p, int a, int b, const Coef& C) {
+  double r[8];
+  const int off[8] = {1, -1, 2, -2, 3, -3, 4, -4};
+#pragma unroll
+  for (int t = 0; t < 8; ++t) {
+    const int m = off[t];
+    const double e1 = p.ax2(a, m, b, 1) - p.ax2(a, m, b, -1), e2 = p.ax2(a, m, b, 2) - p.ax2(a, m, b, -2);
+    const double e3 = p.ax2(a, m, b, 3) - p.ax2(a, m, b, -3), e4 = p.ax2(a, m, b, 4) - p.ax2(a, m, b, -4);
+    r[t] = (672.0 * e1 - 168.0 * e2) + (32.0 * e3 - 3.0 * e4);
+  }
+  return ((672.0 * (r[0] - r[1]) - 168.0 * (r[2] - r[3])) + (32.0 * (r[4] - r[5]) - 3.0 * (r[6] - r[7]))) *
+         (C.inv_h2 * (1.0 / (840.0 * 840.0)));
+}
+template <class P>
+__device__ __forceinline__ void var_full8(const P& p, const Coef& C, const AdvW& w, double* d1, double* d2, double& ad) {
+  const double f0 = p.at(0, 0, 0);
+  axis8<P, true, true>(p, f0, 0, C, w, d1[0], d2[0], ad);
+  axis8<P, true, true>(p, f0, 1, C, w, d1[1], d2[3], ad);
+  axis8<P, true, true>(p, f0, 2, C, w, d1[2], d2[5], ad);
+  d2[1] = mixed8(p, 0, 1, C);
+  d2[2] = mixed8(p, 0, 2, C);
+  d2[4] = mixed8(p, 1, 2, C);
+}
+template <class P>
+__device__ __forceinline__ void var_d1_ad8(const P& p, const Coef& C, const AdvW& w, double* d1, double& ad) {
+  const double f0 = p.at(0, 0, 0);
+  double dummy;
+  axis8<P, true, false>(p, f0, 0, C, w, d1[0], dummy, ad);
+  axis8<P, true, false>(p, f0, 1, C, w, d1[1], dummy, ad);
+  axis8<P, true, false>(p, f0, 2, C, w, d1[2], dummy, ad);
+}
+template <class P>
+__device__ __forceinline__ double var_ad8(const P& p, const Coef& C, const AdvW& w) {
+  const double f0 = p.at(0, 0, 0);
+  double ad, dummy;
+  axis8<P, false, false>(p, f0, 0, C, w, dummy, dummy, ad);
+  axis8<P, false, false>(p, f0, 1, C, w, dummy, dummy, ad);
+  axis8<P, false, false>(p, f0, 2, C, w, dummy, dummy, ad);
+  return ad;
+}
+
 // consumption order of the 25 variables (slot of order index o is o % 5)
 __device__ __forceinline__ constexpr int order_var(int o) {
   return o < 3 ? V_BETA + o : o < 9 ? V_GT + (o - 3) : o < 12 ? V_GAM + (o - 9) : o == 12 ? V_CHI : o == 13 ? V_ALPHA

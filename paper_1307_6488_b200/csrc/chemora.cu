@@ -120,7 +120,7 @@ int run_rhs_inner(chemora_t* h, const Stage& st) {
     h->launches += 1;
   } else if (h->fused) {
     if (h->tile >= 6 && h->tile < 9) CK(h, launch_bssn_ws(h->L, C, h->tile - 6, st, h->stream), "bssn warp-specialised kernel launch");
-    else CK(h, launch_bssn_fused(h->L, C, h->tile, st, h->stream), "bssn fused kernel launch");
+    else CK(h, launch_bssn_fused(h->L, C, h->order, h->tile, st, h->stream), "bssn fused kernel launch");
     h->launches += 1;
   } else {
     int rc = ensure_derivs(h);
@@ -175,8 +175,8 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
   h->stream = (cudaStream_t)cuda_stream;
   h->alloc = alloc; h->dealloc = dealloc; h->actx = alloc_ctx;
   h->derivs = nullptr; h->staging = nullptr;
-  // 8th-order BSSN (the paper's configuration, 5 ghost zones) runs through the derivative-split variant only
-  h->fused = (system_id == CHEMORA_SYS_BSSN && fd_order == 8) ? 0 : 1; h->tile = 1;
+  // 8th-order BSSN (the paper's configuration, 5 ghost zones): fused kernel on tile id 0 only
+  h->fused = 1; h->tile = (system_id == CHEMORA_SYS_BSSN && fd_order == 8) ? 0 : 1;
   h->launches = 0;
   h->timing = false;
   h->ev_launches[0] = h->ev_launches[1] = 0;
@@ -365,8 +365,8 @@ int chemora_energy(chemora_t* h, const double* dev_state, double* dev_eps, doubl
 int chemora_set_variant(chemora_t* h, int fused, int tile_id) {
   if (!h || tile_id < 0 || tile_id >= CHEMORA_NUM_TILES || (fused != 0 && fused != 1)) return CHEMORA_EINVAL;
   if (!fused && h->system != CHEMORA_SYS_BSSN) return fail(h, CHEMORA_EINVAL, "wave systems have no split variant");
-  if (fused && h->system == CHEMORA_SYS_BSSN && h->order == 8)
-    return fail(h, CHEMORA_EINVAL, "8th-order BSSN has the derivative-split variant only");
+  if (fused && h->system == CHEMORA_SYS_BSSN && h->order == 8 && tile_id != 0)
+    return fail(h, CHEMORA_EINVAL, "8th-order BSSN: the fused kernel has tile id 0 (16x4x4) only");
   h->fused = fused;
   h->tile = tile_id;
   return CHEMORA_OK;
@@ -403,7 +403,7 @@ int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out)
   for (int f = 1; f >= 0 && !rc; --f)
     for (int t = 0; t < CHEMORA_NUM_TILES && !rc; ++t) {
       float ms = -1.f;
-      const bool bssn = h->system == CHEMORA_SYS_BSSN, o8 = bssn && h->order == 8;   // O8 BSSN: split variant only
+      const bool bssn = h->system == CHEMORA_SYS_BSSN, o8 = bssn && h->order == 8 && t != 0;   // O8 BSSN: one fused tile
       const int nwave = h->system == CHEMORA_SYS_WAVE ? 9 : 6;   // (phi, pi) has three more ids: the plane-ring kernel
       if ((f == 1 && !o8 && (bssn || t < nwave)) || (f == 0 && bssn && t < 6)) {
         h->fused = f; h->tile = t;
@@ -473,7 +473,7 @@ int chemora_kernel_info(const chemora_t* h, int* regs, int* local_bytes, int* sm
                   : h->system == CHEMORA_SYS_WAVE1 ? kernel_info_wave1(h->order, h->tile % 6, &a)
                   : !h->fused              ? kernel_info_bssn_split(1, h->tile % 6, &a)
                   : h->tile >= 6 && h->tile < 9 ? kernel_info_bssn_ws(h->tile - 6, &a)
-                                           : kernel_info_bssn_fused(h->tile, &a);
+                                           : kernel_info_bssn_fused(h->order, h->tile, &a);
   if (e != cudaSuccess) return cuda_fail(const_cast<chemora_t*>(h), e, "cudaFuncGetAttributes");
   if (regs) *regs = a.numRegs;
   if (local_bytes) *local_bytes = (int)a.localSizeBytes;

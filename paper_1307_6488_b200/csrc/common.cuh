@@ -145,7 +145,7 @@ cudaError_t kernel_info_wave_tma(int order, int which, cudaFuncAttributes* a);
 bool wave_tma_ok(const Layout& L, int order, bool ko);
 cudaError_t launch_wave1(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
 cudaError_t kernel_info_wave1(int order, int tile, cudaFuncAttributes* a);
-cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int tile, const Stage& st, cudaStream_t s);
+cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
 cudaError_t launch_bssn_ws(const Layout& L, const Coef& C, int which, const Stage& st, cudaStream_t s);
 cudaError_t kernel_info_bssn_ws(int which, cudaFuncAttributes* a);
 cudaError_t launch_bssn_derivs(const Layout& L, const Coef& C, int order, int tile, const double* in, double* derivs,
@@ -153,7 +153,7 @@ cudaError_t launch_bssn_derivs(const Layout& L, const Coef& C, int order, int ti
 cudaError_t launch_bssn_from_derivs(const Layout& L, const Coef& C, int tile, const double* derivs,
                                     const Stage& st, cudaStream_t s);
 cudaError_t kernel_info_wave(int order, int tile, cudaFuncAttributes* a);
-cudaError_t kernel_info_bssn_fused(int tile, cudaFuncAttributes* a);
+cudaError_t kernel_info_bssn_fused(int order, int tile, cudaFuncAttributes* a);
 cudaError_t kernel_info_bssn_split(int which, int tile, cudaFuncAttributes* a);
 cudaError_t launch_dfma_peak(int blocks, int threads, int iters, double* sink, cudaStream_t s);
 

@@ -37,17 +37,18 @@ __device__ __forceinline__ constexpr int emit_var(int o, int n) {
          : o < 24 ? (n == 0 ? V_GAM + (o - 21) : V_B + (o - 21)) : (n == 0 ? V_A : -1);
 }
 
-template <int TX, int TY, int TZ>
+template <int TX, int TY, int TZ, int ORDER = 4>
 struct TmaCfg {
+  static constexpr int H = ORDER == 8 ? 5 : 3;    // halo: upwinded stencils reach order/2 + 1 cells
   static_assert(TX % 2 == 0 && ((TX + 2) * TY * TZ) % 16 == 0, "tile boxes must stay 128-byte aligned in smem");
-  static constexpr int BX = TX + 6, BY = TY + 6, BZ = TZ + 6;
+  static constexpr int BX = TX + 2 * H, BY = TY + 2 * H, BZ = TZ + 2 * H;
   static constexpr int SLOT = (BX * BY * BZ + 15) / 16 * 16;          // doubles, 128-byte multiple
   static constexpr uint32_t BOX_BYTES = (uint32_t)BX * BY * BZ * 8u;
   static constexpr int THREADS = TX * TY * TZ;
   static constexpr bool HEAVY = THREADS > 256;    // 12 warps at 168 registers: live values parked in tensor memory
   // ring slots (a 6-slot ring fits the 16x4x4 tile but its run-time slot index costs more than the depth gains:
   // 8.2 ms vs 6.3 ms)
-  static constexpr int NS = HEAVY ? 4 : 5;
+  static constexpr int NS = ORDER == 8 ? 3 : HEAVY ? 4 : 5;   // 8th order: 41 KB boxes, three fit
   static constexpr bool PARK = HEAVY || CHM_TMEM;
   static constexpr int TILE = (TX + 2) * TY * TZ;                      // doubles in one (TX+2,TY,TZ) tile box
   static constexpr uint32_t TILE_BYTES = (uint32_t)TILE * 8u;
@@ -58,18 +59,19 @@ struct TmaCfg {
   static constexpr int DYX = TX + 4;
   static constexpr int DY_N = DYX * TY * TZ, DZ_N = DYX * (TY + 4) * TZ;
   // (planes of 128 threads: measured no gain over the one-pass form)
-  static constexpr bool TWOPASS = !HEAVY && (CHM_TWOPASS == 2 || (CHM_TWOPASS == 1 && (TX * TY == 64 || TX * TY == 32)));
+  static constexpr bool TWOPASS = ORDER == 4 && !HEAVY && (CHM_TWOPASS == 2 || (CHM_TWOPASS == 1 && (TX * TY == 64 || TX * TY == 32)));
   static constexpr int DB = TWOPASS ? (DY_N + DZ_N + 15) / 16 * 16 : 0;
   static constexpr size_t SMEM = (size_t)(NS * SLOTX + CEN + 2 * DB) * 8 + (NS + 1) * 8 + (NS + 1) * 8 + 64 + 16 + 64 + 128;
   static constexpr int NWARPS = THREADS / 32;
 };
 
-template <int TX, int TY, int TZ, int MODE>
+template <int TX, int TY, int TZ, int MODE, int ORDER>
 __global__ void __launch_bounds__(TX* TY* TZ, 1)
 bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ CUtensorMap tmCen,
                 const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS, Layout L, Coef C,
                 Stage st, int ntx, int nty, int ntz, int cy) {
-  using Cfg = TmaCfg<TX, TY, TZ>;
+  using Cfg = TmaCfg<TX, TY, TZ, ORDER>;
+  constexpr int H = Cfg::H;
   constexpr int BX = Cfg::BX, BY = Cfg::BY, SLOT = Cfg::SLOT, SLOTX = Cfg::SLOTX, TILE = Cfg::TILE, CEN = Cfg::CEN;
   constexpr unsigned NW = Cfg::NWARPS;
   constexpr int kSlots = Cfg::NS;
@@ -88,11 +90,11 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 
   const int tid = threadIdx.x, lane = tid & 31;
   const int lx = tid % TX, ly = (tid / TX) % TY, lz = tid / (TX * TY);
-  const int coff = ((lz + 3) * BY + (ly + 3)) * BX + lx + 3;
+  const int coff = ((lz + H) * BY + (ly + H)) * BX + lx + H;
   // halo-box origin relative to the tile origin in padded coordinates.  TMA needs every row of a box to start
   // on a 16-byte boundary: the layout makes L.xo - 3 even, and the (TX,TY,TZ) tile boxes (point values, RK4
   // operands) are loaded two columns wider, from x0 + 2, and read at column + 1.
-  const int goffx = L.xo - 3, goff = L.g - 3;
+  const int goffx = L.xo - H, goff = L.g - H;
   const uint64_t pol_stream = CHM_L2HINT ? l2_policy_evict_first() : l2_policy_normal();   // U, S: read once per launch
 
   if (tid == 0) {
@@ -146,17 +148,17 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     const int nem = (v0 >= 0) + (v1 >= 0);
     mbar_expect_tx(&full[slot], Cfg::BOX_BYTES + (uint32_t)(nops * nem) * Cfg::TILE_BYTES);
     tma_load_4d(dst, &tm, &full[slot], x0, y0, z0, order_var(o));
-    if (v0 >= 0 && nops >= 1) tma_load_4d_hint(dst + SLOT, &tmU, &full[slot], x0 + 2, y0 + 3, z0 + 3, v0, pol_stream);
-    if (v0 >= 0 && nops == 2) tma_load_4d_hint(dst + SLOT + TILE, &tmS, &full[slot], x0 + 2, y0 + 3, z0 + 3, v0, pol_stream);
-    if (v1 >= 0 && nops >= 1) tma_load_4d_hint(dst + SLOT + 2 * TILE, &tmU, &full[slot], x0 + 2, y0 + 3, z0 + 3, v1, pol_stream);
-    if (v1 >= 0 && nops == 2) tma_load_4d_hint(dst + SLOT + 3 * TILE, &tmS, &full[slot], x0 + 2, y0 + 3, z0 + 3, v1, pol_stream);
+    if (v0 >= 0 && nops >= 1) tma_load_4d_hint(dst + SLOT, &tmU, &full[slot], x0 + H - 1, y0 + H, z0 + H, v0, pol_stream);
+    if (v0 >= 0 && nops == 2) tma_load_4d_hint(dst + SLOT + TILE, &tmS, &full[slot], x0 + H - 1, y0 + H, z0 + H, v0, pol_stream);
+    if (v1 >= 0 && nops >= 1) tma_load_4d_hint(dst + SLOT + 2 * TILE, &tmU, &full[slot], x0 + H - 1, y0 + H, z0 + H, v1, pol_stream);
+    if (v1 >= 0 && nops == 2) tma_load_4d_hint(dst + SLOT + 3 * TILE, &tmS, &full[slot], x0 + H - 1, y0 + H, z0 + H, v1, pol_stream);
   };
   // point values of a tile (three 7-variable boxes: vars 0..6, 7..13, 17..23)
   auto issue_cen = [&](int x0, int y0, int z0) {
     mbar_expect_tx(cfull, (uint32_t)kCenVars * Cfg::TILE_BYTES);
-    tma_load_4d(cbuf, &tmCen, cfull, x0 + 2, y0 + 3, z0 + 3, 0);
-    tma_load_4d(cbuf + 7 * TILE, &tmCen, cfull, x0 + 2, y0 + 3, z0 + 3, 7);
-    tma_load_4d(cbuf + 14 * TILE, &tmCen, cfull, x0 + 2, y0 + 3, z0 + 3, 17);
+    tma_load_4d(cbuf, &tmCen, cfull, x0 + H - 1, y0 + H, z0 + H, 0);
+    tma_load_4d(cbuf + 7 * TILE, &tmCen, cfull, x0 + H - 1, y0 + H, z0 + H, 7);
+    tma_load_4d(cbuf + 14 * TILE, &tmCen, cfull, x0 + H - 1, y0 + H, z0 + H, 17);
   };
   // one warp leaves buffer b (all its reads of it are done); true for lane 0 of the last of the NW warps
   auto leave = [&](int b) {
@@ -330,7 +332,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       d2[2] = (8.0 * (z[1] - z[-1]) - (z[2] - z[-2])) * c12;
       d2[4] = (8.0 * (z[DYX] - z[-DYX]) - (z[2 * DYX] - z[-2 * DYX])) * c12;
       } else {
-        var_full(p, C, w, d1, d2, ad);
+        if (ORDER == 4) var_full(p, C, w, d1, d2, ad); else var_full8(p, C, w, d1, d2, ad);
         done(o);
       }
     };
@@ -353,8 +355,13 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       const double b = cen(V_BETA + a);
-      w.ws[a] = b * (C.inv_h * (1.0 / 24.0));
-      w.wq[a] = fabs(b) * (C.inv_h * (1.0 / 24.0)) + C.ko;
+      if (ORDER == 4) {
+        w.ws[a] = b * (C.inv_h * (1.0 / 24.0));
+        w.wq[a] = fabs(b) * (C.inv_h * (1.0 / 24.0)) + C.ko;
+      } else {   // 8th order: KO is added separately (its stencil is not the symmetric part of the upwind one)
+        w.ws[a] = b * (C.inv_h * (1.0 / 840.0));
+        w.wq[a] = fabs(b) * (C.inv_h * (1.0 / 840.0));
+      }
     }
     const double alpha = cen(V_ALPHA), trK = cen(V_K), chi = cen(V_CHI);
 
@@ -539,7 +546,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     for (int k2 = 0; k2 < 3; ++k2) {
       auto p = box(9 + k2);
       double d1[3];
-      var_d1_ad(p, C, w, d1, adG[k2]);
+      if (ORDER == 4) var_d1_ad(p, C, w, d1, adG[k2]); else var_d1_ad8(p, C, w, d1, adG[k2]);
       done(9 + k2);
 #pragma unroll
       for (int i2 = 0; i2 < 3; ++i2)
@@ -646,7 +653,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       auto p = box(14);
       const StagePre pr = pre(14, 0);
       double ad;
-      var_d1_ad(p, C, w, dK, ad);
+      if (ORDER == 4) var_d1_ad(p, C, w, dK, ad); else var_d1_ad8(p, C, w, dK, ad);
       done(14);
       emit(V_K, (alpha * (sdot(Au, At) + third * trK * trK) - lap_alpha) + ad, pr);
     }
@@ -671,7 +678,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
           const int s = sym(i2, j2);
           auto p = box(15 + s);
           const StagePre pr = pre(15 + s, 0);
-          const double ad = var_ad(p, w);
+          const double ad = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
           done(15 + s);
           double AA, lie;
 #pragma unroll
@@ -704,7 +711,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       auto p = box(21 + i2);
       const StagePre prG = pre(21 + i2, 0), prB = pre(21 + i2, 1);
       const double Bi = p.at(0, 0, 0);
-      const double adB = var_ad(p, w);
+      const double adB = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
       done(21 + i2);
       double r = lapb[i2];
       if constexpr (PARK) tmem_unpark<6>(park, P_CU + 6 * i2, &Cu[i2][0]);
@@ -754,10 +761,10 @@ static EncodeTiledFn encode_fn() {
   return fn;
 }
 
-template <int TX, int TY, int TZ, int MODE>
+template <int TX, int TY, int TZ, int MODE, int ORDER>
 static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
-  using Cfg = TmaCfg<TX, TY, TZ>;
-  auto kern = bssn_tma_kernel<TX, TY, TZ, MODE>;
+  using Cfg = TmaCfg<TX, TY, TZ, ORDER>;
+  auto kern = bssn_tma_kernel<TX, TY, TZ, MODE, ORDER>;
   if (a) return cudaFuncGetAttributes(a, kern);
   EncodeTiledFn enc = encode_fn();
   if (!enc) return cudaErrorNotSupported;
@@ -803,20 +810,21 @@ static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, 
   return cudaGetLastError();
 }
 
-template <int TX, int TY, int TZ>
+template <int TX, int TY, int TZ, int ORDER = 4>
 static cudaError_t tma_go(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
   switch (st ? st->mode : MODE_MID) {   // kernel_info reports the common (middle-stage) instance
-    case MODE_RHS: return tma_go_mode<TX, TY, TZ, MODE_RHS>(L, C, st, s, a);
-    case MODE_FIRST: return tma_go_mode<TX, TY, TZ, MODE_FIRST>(L, C, st, s, a);
-    case MODE_MID: return tma_go_mode<TX, TY, TZ, MODE_MID>(L, C, st, s, a);
-    case MODE_LAST: return tma_go_mode<TX, TY, TZ, MODE_LAST>(L, C, st, s, a);
-    case MODE_SSP: return tma_go_mode<TX, TY, TZ, MODE_SSP>(L, C, st, s, a);
+    case MODE_RHS: return tma_go_mode<TX, TY, TZ, MODE_RHS, ORDER>(L, C, st, s, a);
+    case MODE_FIRST: return tma_go_mode<TX, TY, TZ, MODE_FIRST, ORDER>(L, C, st, s, a);
+    case MODE_MID: return tma_go_mode<TX, TY, TZ, MODE_MID, ORDER>(L, C, st, s, a);
+    case MODE_LAST: return tma_go_mode<TX, TY, TZ, MODE_LAST, ORDER>(L, C, st, s, a);
+    case MODE_SSP: return tma_go_mode<TX, TY, TZ, MODE_SSP, ORDER>(L, C, st, s, a);
   }
   return cudaErrorInvalidValue;
 }
 
-static cudaError_t tma_dispatch(int tile, const Layout& L, const Coef& C, const Stage* st, cudaStream_t s,
+static cudaError_t tma_dispatch(int order, int tile, const Layout& L, const Coef& C, const Stage* st, cudaStream_t s,
                                 cudaFuncAttributes* a) {
+  if (order == 8) return tile == 0 ? tma_go<16, 4, 4, 8>(L, C, st, s, a) : cudaErrorInvalidValue;   // one 8th-order tile
   switch (tile) {
     case 0: return tma_go<16, 4, 4>(L, C, st, s, a);
     case 1: return tma_go<16, 8, 2>(L, C, st, s, a);
@@ -830,12 +838,12 @@ static cudaError_t tma_dispatch(int tile, const Layout& L, const Coef& C, const 
   return cudaErrorInvalidValue;
 }
 
-cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int tile, const Stage& st, cudaStream_t s) {
-  return tma_dispatch(tile, L, C, &st, s, nullptr);
+cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s) {
+  return tma_dispatch(order, tile, L, C, &st, s, nullptr);
 }
-cudaError_t kernel_info_bssn_fused(int tile, cudaFuncAttributes* a) {
+cudaError_t kernel_info_bssn_fused(int order, int tile, cudaFuncAttributes* a) {
   Layout L{}; Coef C{};
-  return tma_dispatch(tile, L, C, nullptr, 0, a);
+  return tma_dispatch(order, tile, L, C, nullptr, 0, a);
 }
 
 }  // namespace chm

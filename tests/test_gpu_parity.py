@@ -348,21 +348,24 @@ def test_bssn_o8_rhs(chem, oracle, data):
     want = oracle_rhs(oracle, 1, u, g, 8, dx, eps_diss=eps)
     h = chem.Chemora(nx, ny, nz, g, 8, 1, dx)
     h.set_param("eps_diss", eps)
-    assert h.get_variant()[0] == 0                      # split variant only
+    assert h.get_variant() == (1, 0)                    # the fused 8th-order kernel has one tile shape
     with pytest.raises(chem.ChemoraError):
-        h.set_variant(1, 0)
+        h.set_variant(1, 1)
+    assert relerr(gpu_rhs(h, u), want) < TOL_RHS
     for tile in range(6):
         h.set_variant(0, tile)
         assert relerr(gpu_rhs(h, u), want) < TOL_RHS, tile
     h.destroy()
 
 
-def test_bssn_o8_rk4_10_steps_and_rk3_enforced(chem, oracle):
+@pytest.mark.parametrize("fused", [1, 0])
+def test_bssn_o8_rk4_10_steps_and_rk3_enforced(chem, oracle, fused):
     nx, ny, nz, g = 20, 16, 12, 5
     u0 = inputs.bssn_noise(nx, ny, nz)
     dx, dt, eps = 0.05, 0.0125, 0.1
     h = chem.Chemora(nx, ny, nz, g, 8, 1, dx)
     h.set_param("eps_diss", eps)
+    h.set_variant(fused, 0)
     h.set_state(u0)
     for _ in range(10):
         h.rk4_step(dt)
