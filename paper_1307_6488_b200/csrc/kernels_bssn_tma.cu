@@ -56,10 +56,10 @@ struct TmaCfg {
   static constexpr int CEN = kCenVars * TILE;     // point values needed ahead of their own boxes
   // first derivatives shared between threads for the mixed second derivatives (two buffers, alternating):
   // D_y f on the tile + 2 columns of x-halo, D_z f on the tile + 2 columns of x-halo + 2 rows of y-halo
-  static constexpr int DYX = TX + 4;
-  static constexpr int DY_N = DYX * TY * TZ, DZ_N = DYX * (TY + 4) * TZ;
+  static constexpr int DYX = TX + ORDER;             // x-halo = reach of the centred first derivative (order/2) on each side
+  static constexpr int DY_N = DYX * TY * TZ, DZ_N = DYX * (TY + ORDER) * TZ;
   // (planes of 128 threads: measured no gain over the one-pass form)
-  static constexpr bool TWOPASS = ORDER == 4 && !HEAVY && (CHM_TWOPASS == 2 || (CHM_TWOPASS == 1 && (TX * TY == 64 || TX * TY == 32)));
+  static constexpr bool TWOPASS = !HEAVY && (CHM_TWOPASS == 2 || (CHM_TWOPASS == 1 && (TX * TY == 64 || TX * TY == 32)));
   static constexpr int DB = TWOPASS ? (DY_N + DZ_N + 15) / 16 * 16 : 0;
   static constexpr size_t SMEM = (size_t)(NS * SLOTX + CEN + 2 * DB) * 8 + (NS + 1) * 8 + (NS + 1) * 8 + 64 + 16 + 64 + 128;
   static constexpr int NWARPS = THREADS / 32;
@@ -245,16 +245,27 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     // d_xy = D_x(D_y f), d_xz = D_x(D_z f), d_yz = D_y(D_z f) cost 4 reads each instead of 16.
     auto full_var = [&](const BoxPoint<BX, BY>& p, const AdvW& w, int o, int n, double* d1, double* d2, double& ad) {
       if constexpr (Cfg::TWOPASS) {
-      constexpr int DYX = Cfg::DYX, ZS = BX * BY;
+      constexpr int DYX = Cfg::DYX, ZS = BX * BY, HM = ORDER / 2;   // HM: reach of the centred first derivative
       const double f0 = p.at(0, 0, 0);
-      axis_full(p, f0, 0, C, w, d1[0], d2[0], ad);
-      axis_full(p, f0, 1, C, w, d1[1], d2[3], ad);
-      axis_full(p, f0, 2, C, w, d1[2], d2[5], ad);
+      if (ORDER == 4) {
+        axis_full(p, f0, 0, C, w, d1[0], d2[0], ad);
+        axis_full(p, f0, 1, C, w, d1[1], d2[3], ad);
+        axis_full(p, f0, 2, C, w, d1[2], d2[5], ad);
+      } else {
+        axis8<BoxPoint<BX, BY>, true, true>(p, f0, 0, C, w, d1[0], d2[0], ad);
+        axis8<BoxPoint<BX, BY>, true, true>(p, f0, 1, C, w, d1[1], d2[3], ad);
+        axis8<BoxPoint<BX, BY>, true, true>(p, f0, 2, C, w, d1[2], d2[5], ad);
+      }
       double* Dy = dbuf + ((t + n) & 1) * Cfg::DB;
       double* Dz = Dy + Cfg::DY_N;
-      const double c12 = C.inv_h * (1.0 / 12.0);
-      Dy[(lz * TY + ly) * DYX + lx + 2] = d1[1];
-      Dz[(lz * (TY + 4) + ly + 2) * DYX + lx + 2] = d1[2];
+      const double cD = C.inv_h * (ORDER == 4 ? 1.0 / 12.0 : 1.0 / 840.0);
+      // centred first derivative along the direction with element stride s, from a pointer to the point
+      auto D1 = [&](const double* c, int s) {
+        if (ORDER == 4) return (8.0 * (c[s] - c[-s]) - (c[2 * s] - c[-2 * s])) * cD;
+        return ((672.0 * (c[s] - c[-s]) - 168.0 * (c[2 * s] - c[-2 * s])) + (32.0 * (c[3 * s] - c[-3 * s]) - 3.0 * (c[4 * s] - c[-4 * s]))) * cD;
+      };
+      Dy[(lz * TY + ly) * DYX + lx + HM] = d1[1];
+      Dz[(lz * (TY + 2 * HM) + ly + HM) * DYX + lx + HM] = d1[2];
       const double* sb = p.c - coff;   // slot base
       if constexpr (TX * TY == 64 || TX * TY == 128) {
         // One z-plane of the tile = PLANE threads = two or four warps, and every first derivative a thread reads
@@ -262,75 +273,75 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
         // PLANE-thread named barrier instead of a block barrier.
         constexpr int PLANE = TX * TY, WPP = PLANE / 32;
         const int u0 = tid % PLANE;
-        for (int u = u0; u < TX * 4; u += PLANE) {                       // D_z f on the y-halo rows -2,-1,TY,TY+1
+        for (int u = u0; u < TX * 2 * HM; u += PLANE) {                       // D_z f on the y-halo rows -2,-1,TY,TY+1
           const int hx = u % TX, hyi = u / TX;
-          const int yy = hyi < 2 ? hyi - 2 : TY + hyi - 2;
-          const double* c = sb + ((lz + 3) * BY + (yy + 3)) * BX + hx + 3;
-          Dz[(lz * (TY + 4) + yy + 2) * DYX + hx + 2] = (8.0 * (c[ZS] - c[-ZS]) - (c[2 * ZS] - c[-2 * ZS])) * c12;
+          const int yy = hyi < HM ? hyi - HM : TY + hyi - HM;
+          const double* c = sb + ((lz + H) * BY + (yy + H)) * BX + hx + H;
+          Dz[(lz * (TY + 2 * HM) + yy + HM) * DYX + hx + HM] = D1(c, ZS);
         }
         // D_y f, D_z f on the 4 x-halo columns: 8 * TY evaluations per plane, started at a warp of the plane
         // chosen so that every scheduler (warp w runs on scheduler w % 4) gets the same share
         const int start = WPP == 2 ? (((lz + 1) >> 1) & 1) : (2 * lz) % WPP;
-        for (int l = (u0 - 32 * start + PLANE) % PLANE; l < 8 * TY; l += PLANE) {
-          const int kind = l / (4 * TY), hh = l % (4 * TY);
-          const int hxi = hh % 4, hy = hh / 4;
-          const int xx = hxi < 2 ? hxi - 2 : TX + hxi - 2;
-          const double* c = sb + ((lz + 3) * BY + (hy + 3)) * BX + xx + 3;
+        for (int l = (u0 - 32 * start + PLANE) % PLANE; l < 4 * HM * TY; l += PLANE) {
+          const int kind = l / (2 * HM * TY), hh = l % (2 * HM * TY);
+          const int hxi = hh % (2 * HM), hy = hh / (2 * HM);
+          const int xx = hxi < HM ? hxi - HM : TX + hxi - HM;
+          const double* c = sb + ((lz + H) * BY + (hy + H)) * BX + xx + H;
           const int st1 = kind == 0 ? BX : ZS;
-          const double v = (8.0 * (c[st1] - c[-st1]) - (c[2 * st1] - c[-2 * st1])) * c12;
-          if (kind == 0) Dy[(lz * TY + hy) * DYX + xx + 2] = v;
-          else Dz[(lz * (TY + 4) + hy + 2) * DYX + xx + 2] = v;
+          const double v = D1(c, st1);
+          if (kind == 0) Dy[(lz * TY + hy) * DYX + xx + HM] = v;
+          else Dz[(lz * (TY + 2 * HM) + hy + HM) * DYX + xx + HM] = v;
         }
         done(o);
         asm volatile("bar.sync %0, %1;" ::"r"(1 + lz), "n"(PLANE) : "memory");
       } else if constexpr (TX * TY == 32) {
         // One z-plane of the tile = one warp: the warp fills its own plane's halo entries; no barrier at all.
 #pragma unroll
-        for (int e = 0; e < (TX * 4) / 32; ++e) {                         // D_z f on the y-halo rows
+        for (int e = 0; e < (TX * 2 * HM) / 32; ++e) {                         // D_z f on the y-halo rows
           const int u = lane + 32 * e, hx = u % TX, hyi = u / TX;
-          const int yy = hyi < 2 ? hyi - 2 : TY + hyi - 2;
-          const double* c = sb + ((lz + 3) * BY + (yy + 3)) * BX + hx + 3;
-          Dz[(lz * (TY + 4) + yy + 2) * DYX + hx + 2] = (8.0 * (c[ZS] - c[-ZS]) - (c[2 * ZS] - c[-2 * ZS])) * c12;
+          const int yy = hyi < HM ? hyi - HM : TY + hyi - HM;
+          const double* c = sb + ((lz + H) * BY + (yy + H)) * BX + hx + H;
+          Dz[(lz * (TY + 2 * HM) + yy + HM) * DYX + hx + HM] = D1(c, ZS);
         }
         if (lane < 8 * TY) {                                              // D_y f, D_z f on the 4 x-halo columns
           const int kind = lane / (4 * TY), hh = lane % (4 * TY);
-          const int hxi = hh % 4, hy = hh / 4;
-          const int xx = hxi < 2 ? hxi - 2 : TX + hxi - 2;
-          const double* c = sb + ((lz + 3) * BY + (hy + 3)) * BX + xx + 3;
+          const int hxi = hh % (2 * HM), hy = hh / (2 * HM);
+          const int xx = hxi < HM ? hxi - HM : TX + hxi - HM;
+          const double* c = sb + ((lz + H) * BY + (hy + H)) * BX + xx + H;
           const int st1 = kind == 0 ? BX : ZS;
-          const double v = (8.0 * (c[st1] - c[-st1]) - (c[2 * st1] - c[-2 * st1])) * c12;
-          if (kind == 0) Dy[(lz * TY + hy) * DYX + xx + 2] = v;
-          else Dz[(lz * (TY + 4) + hy + 2) * DYX + xx + 2] = v;
+          const double v = D1(c, st1);
+          if (kind == 0) Dy[(lz * TY + hy) * DYX + xx + HM] = v;
+          else Dz[(lz * (TY + 2 * HM) + hy + HM) * DYX + xx + HM] = v;
         }
         done(o);
         __syncwarp();
       } else {
-      for (int h = tid; h < TX * 4 * TZ; h += Cfg::THREADS) {          // D_z f on the y-halo rows -2,-1,TY,TY+1
-        const int hx = h % TX, hyi = (h / TX) % 4, hz = h / (TX * 4);
-        const int yy = hyi < 2 ? hyi - 2 : TY + hyi - 2;
-        const double* c = sb + ((hz + 3) * BY + (yy + 3)) * BX + hx + 3;
-        Dz[(hz * (TY + 4) + yy + 2) * DYX + hx + 2] = (8.0 * (c[ZS] - c[-ZS]) - (c[2 * ZS] - c[-2 * ZS])) * c12;
+      for (int h = tid; h < TX * 2 * HM * TZ; h += Cfg::THREADS) {          // D_z f on the y-halo rows -2,-1,TY,TY+1
+        const int hx = h % TX, hyi = (h / TX) % (2 * HM), hz = h / (TX * 2 * HM);
+        const int yy = hyi < HM ? hyi - HM : TY + hyi - HM;
+        const double* c = sb + ((hz + H) * BY + (yy + H)) * BX + hx + H;
+        Dz[(hz * (TY + 2 * HM) + yy + HM) * DYX + hx + HM] = D1(c, ZS);
       }
       // D_y f and D_z f on the 4 x-halo columns: 2 * 4 * TY * TZ single evaluations, spread over the first
       // warps so that every scheduler (warp w runs on scheduler w % 4) gets the same share
-      for (int h = tid; h < 8 * TY * TZ; h += Cfg::THREADS) {
-        const int kind = h / (4 * TY * TZ), hh = h - kind * (4 * TY * TZ);
-        const int hxi = hh % 4, hy = (hh / 4) % TY, hz = hh / (4 * TY);
-        const int xx = hxi < 2 ? hxi - 2 : TX + hxi - 2;
-        const double* c = sb + ((hz + 3) * BY + (hy + 3)) * BX + xx + 3;
+      for (int h = tid; h < 4 * HM * TY * TZ; h += Cfg::THREADS) {
+        const int kind = h / (2 * HM * TY * TZ), hh = h - kind * (2 * HM * TY * TZ);
+        const int hxi = hh % (2 * HM), hy = (hh / (2 * HM)) % TY, hz = hh / (2 * HM * TY);
+        const int xx = hxi < HM ? hxi - HM : TX + hxi - HM;
+        const double* c = sb + ((hz + H) * BY + (hy + H)) * BX + xx + H;
         const int st1 = kind == 0 ? BX : ZS;
-        const double v = (8.0 * (c[st1] - c[-st1]) - (c[2 * st1] - c[-2 * st1])) * c12;
-        if (kind == 0) Dy[(hz * TY + hy) * DYX + xx + 2] = v;
-        else Dz[(hz * (TY + 4) + hy + 2) * DYX + xx + 2] = v;
+        const double v = D1(c, st1);
+        if (kind == 0) Dy[(hz * TY + hy) * DYX + xx + HM] = v;
+        else Dz[(hz * (TY + 2 * HM) + hy + HM) * DYX + xx + HM] = v;
       }
       done(o);
       __syncthreads();
       }
-      const double* y = Dy + (lz * TY + ly) * DYX + lx + 2;
-      const double* z = Dz + (lz * (TY + 4) + ly + 2) * DYX + lx + 2;
-      d2[1] = (8.0 * (y[1] - y[-1]) - (y[2] - y[-2])) * c12;
-      d2[2] = (8.0 * (z[1] - z[-1]) - (z[2] - z[-2])) * c12;
-      d2[4] = (8.0 * (z[DYX] - z[-DYX]) - (z[2 * DYX] - z[-2 * DYX])) * c12;
+      const double* y = Dy + (lz * TY + ly) * DYX + lx + HM;
+      const double* z = Dz + (lz * (TY + 2 * HM) + ly + HM) * DYX + lx + HM;
+      d2[1] = D1(y, 1);
+      d2[2] = D1(z, 1);
+      d2[4] = D1(z, DYX);
       } else {
         if (ORDER == 4) var_full(p, C, w, d1, d2, ad); else var_full8(p, C, w, d1, d2, ad);
         done(o);
