@@ -86,3 +86,31 @@ def test_product_never_touches_the_oracle():
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_1307_6488_b200" not in src and "from paper_1307_6488_b200" not in src
             assert "libchemora" not in src and "csrc" not in src
+
+
+def test_flop_counts_of_the_fused_kernels(binding):
+    """the paper's ~7900 flop per grid point and RHS evaluation at 8th order is an
+    order-of-magnitude check on the 8th-order kernel's own FP64 work, and the 4th-order count must be lower.
+    Counted from the SASS of the middle-stage instances (DADD + DMUL + 2 DFMA, straight-line code executed once per
+    point)."""
+    import shutil
+    import subprocess
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([cuobjdump, "-sass", binding.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    counts, cur = {}, None
+    for line in sass.splitlines():
+        if "Function :" in line:
+            cur = None
+            for order in (4, 8):
+                if "bssn_tma_kernelILi16ELi4ELi4ELi2ELi%dE" % order in line:
+                    cur = order
+                    counts[cur] = 0
+        elif cur is not None:
+            for op, w in (("DADD", 1), ("DMUL", 1), ("DFMA", 2)):
+                if " %s " % op in line or " %s." % op in line:
+                    counts[cur] += w
+    assert set(counts) == {4, 8}, counts
+    assert 3000 < counts[4] < counts[8]
+    assert 7900 / 2 < counts[8] < 7900 * 2
