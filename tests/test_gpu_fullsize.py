@@ -153,3 +153,39 @@ def test_bssn_rk3_enforced_256_sampled(oracle):
             else:
                 worst = max(worst, err / scale[v])
     assert worst < 2e-11, worst
+
+
+def test_bssn_o8_rk3_enforced_256_sampled(oracle):
+    """The paper's configuration at full size: BSSN 256^3, 8th order, 5 ghost zones, RK3 + enforcement, 1 step."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1307_6488_b200 import binding
+    n, g, dx = 256, 5, 0.05
+    dt, steps = 0.25 * dx, 1
+    u0 = inputs.bssn_gaussians(n, n, n)
+    h = binding.Chemora(n, n, n, g, 8, binding.SYS_BSSN, dx)
+    h.set_param("eps_diss", 0.1)
+    h.set_state(u0)
+    h.autotune()
+    h.rk3_step(dt)
+    h.enforce_constraints()
+    got = h.get_state()
+    h.destroy()
+    ga = np.abs(np.gradient(u0[17, :, :, :], axis=2))
+    k, j, i = np.unravel_index(int(np.argmax(ga)), ga.shape)
+    centres = [(0, 0, 0), (255, 128, 3), (int(i), int(j), int(k))]
+    scale = [float(np.max(np.abs(got[v]))) for v in range(25)]
+    reach, core, worst = 15 * steps, 4, 0.0
+    for cpt in centres:
+        blk = cut(u0, cpt, core + reach)
+        st = oracle.rk3(oracle.SYS_BSSN, oracle.with_ghosts(blk, g), g, 8, dx, dt, oracle.params(eps_diss=0.1), steps, True)
+        want = oracle.interior(st, g)[:, reach:reach + 2 * core, reach:reach + 2 * core, reach:reach + 2 * core]
+        have = cut(got, cpt, core)
+        for v in range(25):
+            err = float(np.max(np.abs(have[v] - want[v])))
+            if scale[v] == 0.0:
+                assert err == 0.0
+            else:
+                worst = max(worst, err / scale[v])
+    assert worst < 1e-11, worst
