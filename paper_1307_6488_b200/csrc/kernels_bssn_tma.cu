@@ -20,6 +20,18 @@
 #ifndef CHM_TMEM
 #define CHM_TMEM 0      // park long-lived per-point values (the 18 Christoffel symbols) in tensor memory
 #endif
+// further sections of one kind as one loop body (tables in tensor memory): 1 = beta^i, 2 = gt_ij, 4 = Gt^i,
+// 8 = B^i.  Measured at 8th order, 256^3, ms per launch: 0 -> 8.79, 4 -> 8.80, 8 -> 8.87, 12 -> 8.86, 2 -> 8.95,
+// 13 -> 8.87, 15 -> 9.09 (code 132 KB -> 80 KB): once the At_ij loop is in, code size no longer binds.
+#ifndef CHM_LOOPS8
+#define CHM_LOOPS8 0
+#endif
+#ifndef CHM_LOOPS4
+#define CHM_LOOPS4 0
+#endif
+#ifndef CHM_ATLOOP
+#define CHM_ATLOOP 1   // 4th order too: the At_ij sections as one loop body (6.29 -> 6.19 ms per launch at 256^3)
+#endif
 #ifndef CHM_L2HINT
 #define CHM_L2HINT 1
 #endif
@@ -76,6 +88,14 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
   constexpr unsigned NW = Cfg::NWARPS;
   constexpr int kSlots = Cfg::NS;
   constexpr bool PARK = Cfg::PARK;
+  // Sections of the same kind as ONE loop body each, with a run-time section index.  The 8th-order kernel was
+  // bound by instruction fetch at 150 KB of code; the At_ij loop (always on, table in shared memory, see there)
+  // brought it to 132 KB and 27 % less time.  The further loops (beta^i, gt_ij, Gt^i, B^i; CHM_LOOPS8/4) hand
+  // values to and from the statically indexed code around them through small per-thread tables in tensor memory
+  // (run-time column address); measured no further gain, off by default.
+  constexpr int LOOPS = Cfg::TWOPASS && TX * TY == 64 && !PARK ? (ORDER == 8 ? CHM_LOOPS8 : CHM_LOOPS4) : 0;
+  constexpr bool TMEM = PARK || LOOPS != 0;
+  constexpr int T_TAB = 0, T_OUT = 12;   // LOOPS: tables (doubles): 6 pairs handed to a loop, up to 30 values handed back
   // parking map (offsets in doubles inside the thread's 84-double area)
   constexpr int P_CU = 0, P_DG = 18, P_DB = 42, P_LG = 52, P_AT = 58, P_ADG = 64, P_GN = 68, P_DCA = 72, P_AU = 78;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -106,7 +126,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(empty + kSlots + 1);
   int* org = reinterpret_cast<int*>((reinterpret_cast<uintptr_t>(tmem_slot + 1) + 15) & ~uintptr_t(15));   // [4][4]
   uint32_t park = 0;   // this thread's parking area in tensor memory: its lane, 168 columns (84 doubles)
-  if constexpr (PARK) {
+  if constexpr (TMEM) {
     if (tid < 32) {   // warp 0 allocates all 512 columns (one CTA per SM)
       asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
       asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -403,6 +423,34 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       }
     }
 #else
+    if constexpr (LOOPS & 1) {
+      {
+        const double tb[6] = {C.sgc * cen(V_B + 0), 0.0, C.sgc * cen(V_B + 1), 0.0, C.sgc * cen(V_B + 2), 0.0};
+        tmem_park<6>(park, T_TAB, tb);
+      }
+#pragma unroll 1
+      for (int i2 = 0; i2 < 3; ++i2) {
+        auto p = box(i2);
+        const StagePre pr = pre(i2, 0);
+        double d1[3], d2[6], ad, r2[2];
+        full_var(p, w, i2, i2, d1, d2, ad);
+        tmem_unpark<2>(park, T_TAB + 2 * i2, r2);
+        emit(V_BETA + i2, r2[0] + ad, pr);
+        const double o10[10] = {d1[0], d1[1], d1[2], sdot(gu, d2), d2[0], d2[1], d2[2], d2[3], d2[4], d2[5]};
+        tmem_park<10>(park, T_OUT + 10 * i2, o10);
+      }
+#pragma unroll
+      for (int i2 = 0; i2 < 3; ++i2) {
+        double o10[10];
+        tmem_unpark<10>(park, T_OUT + 10 * i2, o10);
+        lapb[i2] = o10[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+          db[a][i2] = o10[a];
+          gdiv[a] = i2 == 0 ? o10[4 + sym(a, i2)] : gdiv[a] + o10[4 + sym(a, i2)];
+        }
+      }
+    } else
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2) {
       const double Bc = cen(V_B + i2);
@@ -453,6 +501,43 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       }
     }
 #else
+    if constexpr (LOOPS & 2) {
+      {
+        double tb[12];
+#pragma unroll
+        for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+          for (int j2 = i2; j2 < 3; ++j2) {
+            const int s = sym(i2, j2);
+            double lie;
+#pragma unroll
+            for (int k2 = 0; k2 < 3; ++k2) {
+              const double c = g[sym(i2, k2)] * db[j2][k2] + g[sym(j2, k2)] * db[i2][k2];
+              lie = k2 == 0 ? c : lie + c;
+            }
+            tb[2 * s] = (lie - two_thirds * g[s] * divb) - 2.0 * alpha * At[s];
+            tb[2 * s + 1] = 0.0;
+          }
+        tmem_park<12>(park, T_TAB, tb);
+      }
+#pragma unroll 1
+      for (int s = 0; s < 6; ++s) {
+        auto p = box(3 + s);
+        const StagePre pr = pre(3 + s, 0);
+        double d1[3], d2[6], ad, r2[2];
+        full_var(p, w, 3 + s, 3 + s, d1, d2, ad);
+        tmem_unpark<2>(park, T_TAB + 2 * s, r2);
+        emit(V_GT + s, r2[0] + ad, pr);
+        const double d4[4] = {d1[0], d1[1], d1[2], -0.5 * sdot(gu, d2)};
+        tmem_park<4>(park, T_OUT + 4 * s, d4);
+      }
+#pragma unroll
+      for (int s = 0; s < 6; ++s) {
+        double d4[4];
+        tmem_unpark<4>(park, T_OUT + 4 * s, d4);
+        dg[0][s] = d4[0]; dg[1][s] = d4[1]; dg[2][s] = d4[2]; Rt[s] = d4[3];
+      }
+    } else
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2)
 #pragma unroll
@@ -553,6 +638,27 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     }
     // ---- o = 9..11: Gt^k : R~_ij += 1/2 (gt_ki d_j Gt^k + gt_kj d_i Gt^k); advection kept for the end ------
     double adG[3];
+    if constexpr (LOOPS & 4) {
+#pragma unroll 1
+      for (int k2 = 0; k2 < 3; ++k2) {
+        auto p = box(9 + k2);
+        double d4[4];
+        if (ORDER == 4) var_d1_ad(p, C, w, d4, d4[3]); else var_d1_ad8(p, C, w, d4, d4[3]);
+        done(9 + k2);
+        tmem_park<4>(park, T_OUT + 4 * k2, d4);
+      }
+#pragma unroll
+      for (int k2 = 0; k2 < 3; ++k2) {
+        double d4[4];
+        tmem_unpark<4>(park, T_OUT + 4 * k2, d4);
+        adG[k2] = d4[3];
+#pragma unroll
+        for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+          for (int j2 = i2; j2 < 3; ++j2)
+            Rt[sym(i2, j2)] += 0.5 * (g[sym(k2, i2)] * d4[j2] + g[sym(k2, j2)] * d4[i2]);
+      }
+    } else
 #pragma unroll
     for (int k2 = 0; k2 < 3; ++k2) {
       auto p = box(9 + k2);
@@ -680,7 +786,49 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
         for (int b = 0; b < 3; ++b) db[a][b] = t10[3 * a + b];
       divb = t10[9];
     }
-    {
+    if constexpr ((ORDER == 8 || CHM_ATLOOP) && Cfg::TWOPASS && TX * TY == 64) {
+      // The kernel is bound by instruction fetch at 8th order (150 KB of code), so the six advection stencils are
+      // ONE loop body.  The box-independent part of each right-hand side goes through a per-thread table laid
+      // over this thread's OWN z-plane of the shared first-derivative buffers (components 0..2 in the buffer of
+      // chi, n = 9; components 3..5 in the buffer of alpha, n = 10): a plane's entries are touched by the
+      // plane's two warps only, and the plane barrier below orders the partner's last reads before these
+      // writes; the next tile's first full variables write the buffers only after every warp has left
+      // section 20 (the table is read before a section's slot is released).
+      constexpr int PLANE = TX * TY, HM = ORDER / 2, NY = TY * Cfg::DYX, NZ = (TY + 2 * HM) * Cfg::DYX;
+      static_assert(3 * PLANE <= NY + NZ, "table does not fit the plane's share of a buffer");
+      const int u0 = tid % PLANE;
+      auto tab = [&](int s) {
+        double* b = dbuf + ((t + (s < 3 ? 1 : 0)) & 1) * Cfg::DB;
+        const int e = (s < 3 ? s : s - 3) * PLANE + u0;
+        return e < NY ? b + lz * NY + e : b + Cfg::DY_N + lz * NZ + (e - NY);
+      };
+      asm volatile("bar.sync %0, %1;" ::"r"(1 + lz), "n"(PLANE) : "memory");
+      const double trX = sdot(gu, Rt);
+#pragma unroll
+      for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+        for (int j2 = i2; j2 < 3; ++j2) {
+          const int s = sym(i2, j2);
+          double AA, lie;
+#pragma unroll
+          for (int k2 = 0; k2 < 3; ++k2) {
+            const double c = At[sym(i2, k2)] * db[j2][k2] + At[sym(j2, k2)] * db[i2][k2];
+            AA = k2 == 0 ? At[sym(i2, k2)] * Am[k2][j2] : AA + At[sym(i2, k2)] * Am[k2][j2];
+            lie = k2 == 0 ? c : lie + c;
+          }
+          *tab(s) = chi * (Rt[s] - third * g[s] * trX) + alpha * (trK * At[s] - 2.0 * AA) +
+                    (lie - two_thirds * At[s] * divb);
+        }
+#pragma unroll 1
+      for (int s = 0; s < 6; ++s) {
+        auto p = box(15 + s);
+        const StagePre pr = pre(15 + s, 0);
+        const double ad = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
+        const double rest = *tab(s);
+        done(15 + s);
+        emit(V_AT + s, rest + ad, pr);
+      }
+    } else {
       const double trX = sdot(gu, Rt);
 #pragma unroll
       for (int i2 = 0; i2 < 3; ++i2)
@@ -717,6 +865,38 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 #pragma unroll
       for (int a = 0; a < 3; ++a) { Gn[a] = g4[a]; dchi[a] = dc[a]; dal[a] = dc[3 + a]; }
     }
+    if constexpr (LOOPS & 8) {
+      {
+        double tb[6];
+#pragma unroll
+        for (int i2 = 0; i2 < 3; ++i2) {
+          double r = lapb[i2];
+          double t2 = sdot(Cu[i2], Au);
+#pragma unroll
+          for (int j2 = 0; j2 < 3; ++j2) {
+            r += third * gu[sym(i2, j2)] * gdiv[j2];
+            t2 -= two_thirds * gu[sym(i2, j2)] * dK[j2] + 1.5 * ichi * Au[sym(i2, j2)] * dchi[j2];
+            r -= 2.0 * Au[sym(i2, j2)] * dal[j2] + Gn[j2] * db[j2][i2];
+          }
+          r += 2.0 * alpha * t2 + two_thirds * Gn[i2] * divb;
+          tb[2 * i2] = r;
+          tb[2 * i2 + 1] = adG[i2];
+        }
+        tmem_park<6>(park, T_TAB, tb);
+      }
+#pragma unroll 1
+      for (int i2 = 0; i2 < 3; ++i2) {
+        auto p = box(21 + i2);
+        const StagePre prG = pre(21 + i2, 0), prB = pre(21 + i2, 1);
+        const double Bi = p.at(0, 0, 0);
+        const double adB = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
+        done(21 + i2);
+        double r2[2];
+        tmem_unpark<2>(park, T_TAB + 2 * i2, r2);
+        emit(V_GAM + i2, r2[0] + r2[1], prG);
+        emit(V_B + i2, (r2[0] - C.eta * Bi) + adB, prB);
+      }
+    } else
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2) {
       auto p = box(21 + i2);
@@ -748,7 +928,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       emit(V_A, C.ko * qsum, pr);
     }
   }
-  if constexpr (PARK) {
+  if constexpr (TMEM) {
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(*tmem_slot) : "memory");
