@@ -168,6 +168,24 @@ double ko5(const double* f, const Grid& G, int i, int j, int k, double eps) {
   return eps * total / (64.0 * G.h);
 }
 
+// Kreiss-Oliger dissipation of order p=9 (reading S6b; SURVEY 8(f)-1 "9th-order KO (11-point)", the operator
+// that goes with 8th-order differencing and 5 ghost zones), summed over the three axes:
+//   + (eps/1024h) sum_axes (u[-5] - 10u[-4] + 45u[-3] - 120u[-2] + 210u[-1] - 252u0 + 210u[+1] - ... + u[+5])
+// = + (eps/1024h) h^10 (D+ D-)^5 u, written in difference form like ko5 (the coefficients sum to zero).
+double ko9(const double* f, const Grid& G, int i, int j, int k, double eps) {
+  double f0 = f[idx(G, i, j, k)];
+  double total = 0.0;
+  for (int axis = 0; axis < 3; ++axis) {
+    double s1 = (at(f, G, i, j, k, axis, +1) - f0) + (at(f, G, i, j, k, axis, -1) - f0);
+    double s2 = (at(f, G, i, j, k, axis, +2) - f0) + (at(f, G, i, j, k, axis, -2) - f0);
+    double s3 = (at(f, G, i, j, k, axis, +3) - f0) + (at(f, G, i, j, k, axis, -3) - f0);
+    double s4 = (at(f, G, i, j, k, axis, +4) - f0) + (at(f, G, i, j, k, axis, -4) - f0);
+    double s5 = (at(f, G, i, j, k, axis, +5) - f0) + (at(f, G, i, j, k, axis, -5) - f0);
+    total += s5 - 10.0 * s4 + 45.0 * s3 - 120.0 * s2 + 210.0 * s1;
+  }
+  return eps * total / (1024.0 * G.h);
+}
+
 // advective term beta^k d^{up}_k u, side chosen by the sign of beta^k at the point (S2);
 // beta^k == 0 contributes exactly 0.
 double advect(const double* u, const double* const beta[3], const Grid& G, int i, int j, int k) {
@@ -206,7 +224,12 @@ struct Params {
   double eps_diss;  // KO strength; 0 switches the KO term off (and its +-3 reads)
   double eta;       // Gamma-driver damping (S5)
   double shift_gamma_coeff;  // 3/4 (S5)
+  int ko_order;     // 5 (S6, the default) or 9 (S6b: needs 5 ghost zones)
 };
+// the dissipation operator the parameters select
+inline double ko(const double* f, const Grid& G, int i, int j, int k, const Params& P) {
+  return P.ko_order == 9 ? ko9(f, G, i, j, k, P.eps_diss) : ko5(f, G, i, j, k, P.eps_diss);
+}
 
 void wave_rhs(const double* state, double* rhs, const Grid& G, const Params& P) {
   const long n = G.npts();
@@ -220,8 +243,8 @@ void wave_rhs(const double* state, double* rhs, const Grid& G, const Params& P) 
         double rphi = pi[p];
         double rpi = (d2(phi, G, i, j, k, 0) + d2(phi, G, i, j, k, 1)) + d2(phi, G, i, j, k, 2);
         if (P.eps_diss != 0.0) {
-          rphi += ko5(phi, G, i, j, k, P.eps_diss);
-          rpi += ko5(pi, G, i, j, k, P.eps_diss);
+          rphi += ko(phi, G, i, j, k, P);
+          rpi += ko(pi, G, i, j, k, P);
         }
         rhs[p] = rphi;
         rhs[n + p] = rpi;
@@ -249,9 +272,9 @@ void wave1_rhs(const double* state, double* rhs, const Grid& G, const Params& P)
         r[1] = (d1(v[0], G, i, j, k, 0) + d1(v[1], G, i, j, k, 1)) + d1(v[2], G, i, j, k, 2);
         for (int a = 0; a < 3; ++a) r[2 + a] = d1(rho, G, i, j, k, a);
         if (P.eps_diss != 0.0) {
-          r[0] += ko5(u, G, i, j, k, P.eps_diss);
-          r[1] += ko5(rho, G, i, j, k, P.eps_diss);
-          for (int a = 0; a < 3; ++a) r[2 + a] += ko5(v[a], G, i, j, k, P.eps_diss);
+          r[0] += ko(u, G, i, j, k, P);
+          r[1] += ko(rho, G, i, j, k, P);
+          for (int a = 0; a < 3; ++a) r[2 + a] += ko(v[a], G, i, j, k, P);
         }
         for (int c = 0; c < 5; ++c) rhs[c * n + p] = r[c];
       }
@@ -360,7 +383,7 @@ void bssn_rhs_point(const double* const u[25], double* const r[25], const Grid& 
   double divbeta = (dbeta[0][0] + dbeta[1][1]) + dbeta[2][2];
 
   // dissipation + advection of variable v
-  auto diss = [&](int v) { return P.eps_diss != 0.0 ? ko5(u[v], G, i, j, k, P.eps_diss) : 0.0; };
+  auto diss = [&](int v) { return P.eps_diss != 0.0 ? ko(u[v], G, i, j, k, P) : 0.0; };
   auto adv = [&](int v) { return advect(u[v], beta_f, G, i, j, k); };
 
   // d_t chi = 2/3 chi (alpha K - d_k beta^k) + adv
@@ -551,7 +574,7 @@ void rk4_step(int system, double* U, const Grid& G, const Params& P, double dt) 
 
 // ---------------------------------------------------------------------------------------
 // C entry points for the ctypes harness (oracle/oracle.py).  All arrays are host memory in
-// the oracle layout described at the top.  params = {eps_diss, eta, shift_gamma_coeff}.
+// the oracle layout described at the top.  params = {eps_diss, eta, shift_gamma_coeff, ko_order}.
 // ---------------------------------------------------------------------------------------
 // ---------------------------------------------------------------------------------------
 // RK3 (reading S9b; the paper's runs use "RK3", without a formula): the third-order
@@ -637,7 +660,7 @@ int oracle_max_threads() {
 #endif
 }
 
-// op: 0 d1(axis a) | 1 dd(a,b) | 2 dupw(axis a, side b=+-1) | 3 ko5(eps) ; `f` has ghosts,
+// op: 0 d1(axis a) | 1 dd(a,b) | 2 dupw(axis a, side b=+-1) | 3 ko5(eps) | 4 ko9(eps) ; `f` has ghosts,
 // `out` is interior-packed nz*ny*nx.
 void oracle_apply_op(int op, const double* f, double* out, int nx, int ny, int nz, int g, int order,
                      double h, int a, int b, double eps) {
@@ -650,6 +673,7 @@ void oracle_apply_op(int op, const double* f, double* out, int nx, int ny, int n
         else if (op == 1) v = dd(f, G, i, j, k, a, b);
         else if (op == 2) v = dupw(f, G, i, j, k, a, b);
         else if (op == 3) v = ko5(f, G, i, j, k, eps);
+        else if (op == 4) v = ko9(f, G, i, j, k, eps);
         out[((long)k * ny + j) * nx + i] = v;
       }
 }
@@ -663,7 +687,7 @@ void oracle_fill_ghosts(double* state, int nvars, int nx, int ny, int nz, int g)
 void oracle_rhs(int system, const double* state, double* rhs, int nx, int ny, int nz, int g, int order,
                 double h, const double* params) {
   Grid G = make_grid(nx, ny, nz, g, order, h);
-  Params P = {params[0], params[1], params[2]};
+  Params P = {params[0], params[1], params[2], (int)params[3]};
   rhs_any(system, state, rhs, G, P);
 }
 
@@ -671,7 +695,7 @@ void oracle_rhs(int system, const double* state, double* rhs, int nx, int ny, in
 void oracle_rk4(int system, double* U, int nx, int ny, int nz, int g, int order, double h, double dt,
                 const double* params, int nsteps) {
   Grid G = make_grid(nx, ny, nz, g, order, h);
-  Params P = {params[0], params[1], params[2]};
+  Params P = {params[0], params[1], params[2], (int)params[3]};
   for (int s = 0; s < nsteps; ++s) rk4_step(system, U, G, P, dt);
 }
 
@@ -680,7 +704,7 @@ void oracle_rk4(int system, double* U, int nx, int ny, int nz, int g, int order,
 void oracle_rk3(int system, double* U, int nx, int ny, int nz, int g, int order, double h, double dt,
                 const double* params, int nsteps, int enforce) {
   Grid G = make_grid(nx, ny, nz, g, order, h);
-  Params P = {params[0], params[1], params[2]};
+  Params P = {params[0], params[1], params[2], (int)params[3]};
   for (int s = 0; s < nsteps; ++s) {
     rk3_step(system, U, G, P, dt);
     if (enforce && system == SYS_BSSN) enforce_constraints(U, G);

@@ -16,7 +16,7 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 
 SYS_WAVE, SYS_BSSN, SYS_WAVE1 = 0, 1, 2
 NVARS = {SYS_WAVE: 2, SYS_BSSN: 25, SYS_WAVE1: 5}
-OP_D1, OP_DD, OP_UPW, OP_KO = 0, 1, 2, 3
+OP_D1, OP_DD, OP_UPW, OP_KO, OP_KO9 = 0, 1, 2, 3, 4
 
 _lib = None
 
@@ -60,8 +60,9 @@ def _p(a):
     return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
 
 
-def params(eps_diss=0.0, eta=1.0, shift_gamma_coeff=0.75):
-    return np.array([eps_diss, eta, shift_gamma_coeff], dtype=np.float64)
+def params(eps_diss=0.0, eta=1.0, shift_gamma_coeff=0.75, ko_order=5):
+    assert ko_order in (5, 9)
+    return np.array([eps_diss, eta, shift_gamma_coeff, ko_order], dtype=np.float64)
 
 
 def set_threads(n):

@@ -53,6 +53,7 @@ def _roll(f, axis, m):          # value at offset +m along axis (0=x,1=y,2=z) on
 
 
 ORDER = [4]                     # FD order the linearised evaluator uses (set by the O6 tests)
+KO_ORDER = [5]                  # dissipation order it uses (S6; 9 = S6b)
 
 
 def _d1(f, a, h):
@@ -73,6 +74,13 @@ def _dd(f, a, b, h):
 
 def _ko(f, eps, h):
     s = 0
+    if KO_ORDER[0] == 9:
+        w = (210, -120, 45, -10, 1)
+        for a in range(3):
+            s = s - 252 * f
+            for m in range(1, 6):
+                s = s + w[m - 1] * (_roll(f, a, m) + _roll(f, a, -m))
+        return eps * s / (1024 * h)
     for a in range(3):
         s = s + (_roll(f, a, 3) + _roll(f, a, -3) - 6 * (_roll(f, a, 2) + _roll(f, a, -2))
                  + 15 * (_roll(f, a, 1) + _roll(f, a, -1)) - 20 * f)
@@ -115,17 +123,17 @@ def linearised_rhs(u, h, eps, eta):
     return r
 
 
-@pytest.mark.parametrize("order,g", [(4, 3), (8, 5)])
-def test_O6_linearised_bssn_on_config2_data(oracle, order, g):
-    """order 8 with 5 ghost zones is the paper's own configuration"""
+@pytest.mark.parametrize("order,g,ko_order", [(4, 3, 5), (8, 5, 5), (8, 5, 9)])
+def test_O6_linearised_bssn_on_config2_data(oracle, order, g, ko_order):
+    """order 8 with 5 ghost zones is the paper's own configuration; ko_order 9 is S6b"""
     n, h, eps, eta = 16, 0.05, 0.1, 1.0
     u = inputs.bssn_noise(n, n, n, amp=1e-10)
-    got = rhs_periodic(oracle, u, g=g, order=order, h=h, eps_diss=eps, eta=eta)
-    ORDER[0] = order
+    got = rhs_periodic(oracle, u, g=g, order=order, h=h, eps_diss=eps, eta=eta, ko_order=ko_order)
+    ORDER[0], KO_ORDER[0] = order, ko_order
     try:
         want = linearised_rhs(u, h, eps, eta)
     finally:
-        ORDER[0] = 4
+        ORDER[0], KO_ORDER[0] = 4, 5
     for v in range(25):
         scale = np.max(np.abs(want[v]))
         assert scale > 0

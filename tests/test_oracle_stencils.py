@@ -142,6 +142,50 @@ def test_ko5_symbol(oracle):
     assert np.max(np.abs(got - want)) < 1e-13 * (eps / h)
 
 
+def test_ko9_annihilates_degree9_and_sees_degree10(oracle):
+    """S6b: the 11-point operator is (eps/1024h) times the 10th undivided central difference."""
+    rng = np.random.default_rng(501)
+    g, n, eps = 5, 4, 0.1
+    c = [rand_poly(rng, 9), rand_poly(rng, 9), rand_poly(rng, 9)]
+    f, idx = poly_grid(*c, n, g, H)
+    got = oracle.apply_op(oracle.OP_KO9, np.ascontiguousarray(f), g, 8, H, eps=eps)
+    assert np.max(np.abs(got)) <= 1e-9 * np.max(np.abs(f)) / H
+    # on a10 x^10 the 10th undivided difference is 10! a10 h^10: KO9 = eps * 3628800 a10 h^9 / 1024
+    a10 = 0.7
+    for axis in range(3):
+        c = [np.ones(1), np.ones(1), np.ones(1)]
+        c[axis] = np.array([0.0] * 10 + [a10])
+        f, idx = poly_grid(*c, n, g, H)
+        got = oracle.apply_op(oracle.OP_KO9, np.ascontiguousarray(f), g, 8, H, eps=eps)
+        want = eps * 3628800.0 * a10 * H ** 9 / 1024.0
+        assert np.allclose(got, want, rtol=1e-6, atol=0.0)
+
+
+def test_ko9_symbol_and_single_point_weights(oracle):
+    """S6b: on exp(i theta i) KO9 multiplies by -(eps/h) sin^10(theta/2) per axis; a unit spike at offset k along
+    an axis returns eps/(1024 h) * (-1)^(k+1) C(10, 5+k) (a wrong coefficient or sign fails here)."""
+    from math import comb
+    n, g, eps, h = 16, 5, 0.1, 1.0 / 16
+    i = np.arange(-g, n + g)
+    for m in (1, 3, 8):
+        theta = 2 * np.pi * m / n
+        f = np.cos(theta * i)[None, None, :] * np.ones((n + 2 * g, n + 2 * g, 1))
+        got = oracle.apply_op(oracle.OP_KO9, np.ascontiguousarray(f), g, 8, h, eps=eps)
+        want = -(eps / h) * np.sin(theta / 2) ** 10 * f[g:-g, g:-g, g:-g]
+        assert np.max(np.abs(got - want)) < 1e-13 * (eps / h)
+    for axis in range(3):
+        for k in range(-5, 6):
+            z = np.zeros((3 + 2 * g,) * 3)
+            q = [g + 1, g + 1, g + 1]
+            q[axis] += k
+            z[q[2], q[1], q[0]] = 1.0
+            got = oracle.apply_op(oracle.OP_KO9, z, g, 8, h, eps=eps)[1, 1, 1]
+            w = (-1) ** (abs(k) + 1) * comb(10, 5 + k)
+            if k == 0:
+                w *= 3      # the centre belongs to all three axes
+            assert got == pytest.approx(eps / (1024.0 * h) * w, rel=1e-13)
+
+
 def test_flat_field_gives_exact_zero(oracle):
     """difference form (reading R-H1): a constant field differentiates to exactly 0.0."""
     g = 5

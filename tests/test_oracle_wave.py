@@ -16,13 +16,14 @@ def lam(theta, order):
             + (16.0 / 315) * np.cos(3 * theta) - (1.0 / 280) * np.cos(4 * theta))
 
 
-def exact_discrete(state, order, h, dt, eps, nsteps):
+def exact_discrete(state, order, h, dt, eps, nsteps, ko_order=5):
     """Each Fourier mode evolves by P(dt M)^n, M = [[-s, 1], [-L, -s]], P = RK4 stability polynomial."""
     _, nz, ny, nx = state.shape
     th = [2 * np.pi * np.fft.fftfreq(n) for n in (nz, ny, nx)]
     TZ, TY, TX = np.meshgrid(*th, indexing="ij")
     L = -(lam(TX, order) + lam(TY, order) + lam(TZ, order)) / h ** 2
-    s = (eps / h) * (np.sin(TX / 2) ** 6 + np.sin(TY / 2) ** 6 + np.sin(TZ / 2) ** 6)
+    p = ko_order + 1   # S6: sin^6 ; S6b: sin^10
+    s = (eps / h) * (np.sin(TX / 2) ** p + np.sin(TY / 2) ** p + np.sin(TZ / 2) ** p)
     M = np.empty(L.shape + (2, 2))
     M[..., 0, 0] = -s; M[..., 0, 1] = 1.0; M[..., 1, 0] = -L; M[..., 1, 1] = -s
     Z = dt * M
@@ -54,6 +55,21 @@ def test_O2_exact_discrete_solution(oracle, order, g, eps, dims):
                                      oracle.params(eps_diss=eps), nsteps), g)
     want = exact_discrete(u0, order, h, dt, eps, nsteps)
     assert relerr(got, want) < 2e-13
+
+
+def test_O2_exact_discrete_solution_ko9(oracle):
+    """S6b through the whole path: 8th order, 5 ghost zones, 9th-order KO, against the per-mode solution."""
+    nx, ny, nz = 16, 12, 20
+    rng = np.random.default_rng(43)
+    u0 = rng.standard_normal((2, nz, ny, nx))
+    h, nsteps, g, eps = 1.0 / 16, 5, 5, 0.1
+    dt = 0.25 * h
+    got = oracle.interior(oracle.rk4(oracle.SYS_WAVE, oracle.with_ghosts(u0, g), g, 8, h, dt,
+                                     oracle.params(eps_diss=eps, ko_order=9), nsteps), g)
+    want = exact_discrete(u0, 8, h, dt, eps, nsteps, ko_order=9)
+    assert relerr(got, want) < 2e-13
+    # and it is not the 5th-order operator
+    assert relerr(got, exact_discrete(u0, 8, h, dt, eps, nsteps, ko_order=5)) > 1e-4
 
 
 def test_O2_config0_and_config1_shapes(oracle):
