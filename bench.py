@@ -317,8 +317,9 @@ def run_wave(args):
 
 def run_paper_shape(args):
     """The shape of the paper's own single-GPU benchmark: BSSN, 8th-order FD, 5 ghost zones,
-    RK3 (+ constraint enforcement), 100^3 evolved points; synthetic Minkowski + 1e-4 Gaussians.  Context line, not the
-    headline: 8th-order BSSN runs through the derivative-split variant only."""
+    RK3 (+ constraint enforcement), 9th-order KO (reading S6b), 100^3 evolved points; synthetic Minkowski +
+    1e-4 Gaussians.  Context line, not the headline; variant picked by the runtime sweep (fused 8th-order kernel or
+    the derivative-split variant)."""
     import torch
     from paper_1307_6488_b200 import binding, inputs
     if not torch.cuda.is_available():
@@ -327,6 +328,7 @@ def run_paper_shape(args):
     for n in (100, args.size):
         h = binding.Chemora(n, n, n, 5, 8, binding.SYS_BSSN, 0.05)
         h.set_param("eps_diss", 0.1)
+        h.set_param("ko_order", args.ko_order)
         h.set_state(inputs.bssn_gaussians(n, n, n, width_cells=n / 16.0))
         fused, tile, _ = h.autotune()
         dt = 0.0125
@@ -343,7 +345,7 @@ def run_paper_shape(args):
                      "variant": {"fused": fused, "tile": list(binding.tile_shape(tile, binding.SYS_BSSN, fused))}})
         h.destroy()
     print(json.dumps({"metric": "BSSN O8 (5 ghosts) RK3 + enforcement grid-point updates/sec, fp64", "unit": UNIT,
-                      "rows": rows, "paper_context": {"value": 1.05e6, "hardware": "NVIDIA M2050, 100^3, derived from "
+                      "ko_order": args.ko_order, "rows": rows, "paper_context": {"value": 1.05e6, "hardware": "NVIDIA M2050, 100^3, derived from "
                                                       "25 GFlop/s / 7900 flop / 3 substeps (PAPER.md:55, :338, :388)"}}))
 
 
@@ -361,6 +363,7 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="configs[4] variant/tile sweep instead of the headline run")
     ap.add_argument("--wave", action="store_true", help="configs[1]: the (phi, pi) wave system at 256^3, O8 + KO")
     ap.add_argument("--paper-shape", action="store_true", help="BSSN O8 + RK3 at 100^3 (the paper's own benchmark shape)")
+    ap.add_argument("--ko-order", type=int, default=9, choices=[5, 9], help="--paper-shape: dissipation order")
     args = ap.parse_args()
     if args.sweep:
         run_sweep(args)

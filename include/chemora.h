@@ -66,7 +66,9 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
                    void* alloc_ctx);
 
 /* Named parameters: "eps_diss" (KO strength, default 0), "eta" (default 1), "shift_gamma_coeff"
- * (default 0.75); tuning: "col_rows" (default 32: y-extent in grid rows of the columns in which the fused BSSN
+ * (default 0.75), "ko_order" (5, the default, or 9: the 11-point operator (eps/1024h) h^10 (D+D-)^5 that goes
+ * with the paper's 8th-order, 5-ghost-zone configuration; accepted for the 8th-order BSSN
+ * system only); tuning: "col_rows" (default 32: y-extent in grid rows of the columns in which the fused BSSN
  * kernel visits its tiles, chosen so the halo planes shared by z-neighbour tiles stay in L2).
  * Unknown name or invalid value -> CHEMORA_EINVAL. */
 int chemora_set_param(chemora_t* h, const char* name, double value);

@@ -268,7 +268,8 @@ __device__ __forceinline__ double var_ad(const P& p, const AdvW& w) {
 // upwind stencils over offsets -3..+5 (-5,60,-420,-378,1050,-420,140,-30,3)/840h split into an antisymmetric part
 //   A = 735 e1 - 240 e2 + 72.5 e3 - 15 e4 + 1.5 e5   and a symmetric part   S = 315 s1 - 180 s2 + 67.5 s3 - 15 s4 + 1.5 s5
 // (e_k = u[+k] - u[-k], s_k = (u[+k]-u0) + (u[-k]-u0)):  up(+-) = (A +- S)/840h, so
-//   beta d^up u + KO(u) = ws A + wq S + ko q5,   ws = beta/840h, wq = |beta|/840h, q5 = s3 - 6 s2 + 15 s1.
+//   beta d^up u + KO(u) = ws A + wq S + sum_k kq_k s_k,   ws = beta/840h, wq = |beta|/840h,
+// kq = the dissipation weights of Coef (order 5: ko (15, -6, 1, 0, 0); order 9, reading S6b: all five).
 template <class P, bool D1, bool D2>
 __device__ __forceinline__ void axis8(const P& p, double f0, int a, const Coef& C, const AdvW& w, double& d1, double& d2,
                                       double& ad) {
@@ -283,9 +284,17 @@ __device__ __forceinline__ void axis8(const P& p, double f0, int a, const Coef& 
   if (D2) d2 = ((8064.0 * s[1] - 1008.0 * s[2]) + (128.0 * s[3] - 9.0 * s[4])) * (C.inv_h2 * (1.0 / 5040.0));
   const double A = ((735.0 * e[1] - 240.0 * e[2]) + (72.5 * e[3] - 15.0 * e[4])) + 1.5 * e[5];
   const double S = ((315.0 * s[1] - 180.0 * s[2]) + (67.5 * s[3] - 15.0 * s[4])) + 1.5 * s[5];
-  const double q5 = (s[3] - 6.0 * s[2]) + 15.0 * s[1];
-  const double c = (w.ws[a] * A + w.wq[a] * S) + C.ko * q5;
+  const double q = ((C.kq[4] * s[5] + C.kq[3] * s[4]) + (C.kq[2] * s[3] + C.kq[1] * s[2])) + C.kq[0] * s[1];
+  const double c = (w.ws[a] * A + w.wq[a] * S) + q;
   ad = a == 0 ? c : ad + c;
+}
+// dissipation alone along one axis (the inert slot A)
+template <class P>
+__device__ __forceinline__ double axis_ko8(const P& p, double f0, int a, const Coef& C) {
+  double s[6];
+#pragma unroll
+  for (int k = 1; k <= 5; ++k) s[k] = (p.ax(a, k) - f0) + (p.ax(a, -k) - f0);
+  return ((C.kq[4] * s[5] + C.kq[3] * s[4]) + (C.kq[2] * s[3] + C.kq[1] * s[2])) + C.kq[0] * s[1];
 }
 // mixed derivative d_a d_b (a != b) at 8th order, 64 reads
 template <class P>

@@ -19,6 +19,7 @@ struct chemora {
   int order, system;
   double dx;
   double eps_diss, eta, sgc;
+  int ko_order;          // 5, or 9 (8th-order BSSN only)
   cudaStream_t stream;
   void* (*alloc)(size_t, void*);
   void (*dealloc)(void*, void*);
@@ -73,6 +74,14 @@ Coef make_coef(const chemora_t* h) {
   C.inv_h = 1.0 / h->dx;
   C.inv_h2 = 1.0 / (h->dx * h->dx);
   C.ko = h->eps_diss / (64.0 * h->dx);
+  if (h->ko_order == 9) {
+    const double k9 = h->eps_diss / (1024.0 * h->dx);
+    const double w9[5] = {210.0, -120.0, 45.0, -10.0, 1.0};
+    for (int k = 0; k < 5; ++k) C.kq[k] = k9 * w9[k];
+  } else {
+    const double w5[5] = {15.0, -6.0, 1.0, 0.0, 0.0};
+    for (int k = 0; k < 5; ++k) C.kq[k] = C.ko * w5[k];
+  }
   C.eta = h->eta;
   C.sgc = h->sgc;
   return C;
@@ -172,6 +181,7 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
   L.col_rows = 32;
   h->order = fd_order; h->system = system_id; h->dx = dx;
   h->eps_diss = 0.0; h->eta = 1.0; h->sgc = 0.75;
+  h->ko_order = 5;
   h->stream = (cudaStream_t)cuda_stream;
   h->alloc = alloc; h->dealloc = dealloc; h->actx = alloc_ctx;
   h->derivs = nullptr; h->staging = nullptr;
@@ -212,6 +222,11 @@ int chemora_set_param(chemora_t* h, const char* name, double v) {
     if (v < 0.0) return fail(h, CHEMORA_EINVAL, "eps_diss must be >= 0");
     if (v != 0.0 && h->L.g < 3) return fail(h, CHEMORA_EINVAL, "eps_diss != 0 needs ghost >= 3 (KO order 5)");
     h->eps_diss = v;
+  } else if (!strcmp(name, "ko_order")) {
+    if (v != 5.0 && v != 9.0) return fail(h, CHEMORA_EINVAL, "ko_order must be 5 or 9");
+    if (v == 9.0 && !(h->system == CHEMORA_SYS_BSSN && h->order == 8))
+      return fail(h, CHEMORA_EINVAL, "ko_order 9 is built for the 8th-order BSSN system only");
+    h->ko_order = (int)v;
   } else if (!strcmp(name, "eta")) h->eta = v;
   else if (!strcmp(name, "shift_gamma_coeff")) h->sgc = v;
   else if (!strcmp(name, "col_rows")) {
@@ -224,6 +239,7 @@ int chemora_set_param(chemora_t* h, const char* name, double v) {
 int chemora_get_param(const chemora_t* h, const char* name, double* v) {
   if (!h || !name || !v) return CHEMORA_EINVAL;
   if (!strcmp(name, "eps_diss")) *v = h->eps_diss;
+  else if (!strcmp(name, "ko_order")) *v = h->ko_order;
   else if (!strcmp(name, "eta")) *v = h->eta;
   else if (!strcmp(name, "shift_gamma_coeff")) *v = h->sgc;
   else if (!strcmp(name, "col_rows")) *v = h->L.col_rows;

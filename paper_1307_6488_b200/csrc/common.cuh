@@ -33,6 +33,8 @@ struct Coef {
   double inv_h;          // 1/h
   double inv_h2;         // 1/h^2
   double ko;             // eps_diss / (64 h); 0 => dissipation off (no +-3 reads)
+  double kq[5];          // 8th-order BSSN kernels: dissipation = sum_k kq[k-1] s_k, s_k = (u[+k]-u0) + (u[-k]-u0);
+                         // KO order 5: ko * (15, -6, 1, 0, 0); order 9 (reading S6b): eps/(1024 h) * (210, -120, 45, -10, 1)
   double eta;            // Gamma-driver damping
   double sgc;            // shift_gamma_coeff (3/4)
 };

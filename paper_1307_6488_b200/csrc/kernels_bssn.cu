@@ -36,7 +36,7 @@ struct OnTheFly {
     return ORDER == 4 ? adv_o4(pt, v, a, beta[a], C.inv_h) : adv_o8(pt, v, a, beta[a], C.inv_h);
   }
   __device__ __forceinline__ double ad(int v) const {
-    double r = ko5(pt, v, C.ko);
+    double r = ORDER == 4 ? ko5(pt, v, C.ko) : ko_kq(pt, v, C.kq);
     if (v != V_A) r += (adv(v, 0) + adv(v, 1)) + adv(v, 2);
     return r;
   }

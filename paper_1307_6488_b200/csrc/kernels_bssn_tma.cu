@@ -923,9 +923,11 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       auto p = box(24);
       const StagePre pr = pre(24, 0);
       const double f0 = p.at(0, 0, 0);
-      const double qsum = (axis_q(p, f0, 0) + axis_q(p, f0, 1)) + axis_q(p, f0, 2);
+      double rA;
+      if (ORDER == 4) rA = C.ko * ((axis_q(p, f0, 0) + axis_q(p, f0, 1)) + axis_q(p, f0, 2));
+      else rA = (axis_ko8(p, f0, 0, C) + axis_ko8(p, f0, 1, C)) + axis_ko8(p, f0, 2, C);
       done(24);
-      emit(V_A, C.ko * qsum, pr);
+      emit(V_A, rA, pr);
     }
   }
   if constexpr (TMEM) {

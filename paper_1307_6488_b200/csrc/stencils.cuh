@@ -87,6 +87,21 @@ template <class P>
 __device__ __forceinline__ double ko5(const P& f, int v, double ko) {
   return ko * ((ko5_axis(f, v, 0) + ko5_axis(f, v, 1)) + ko5_axis(f, v, 2));
 }
+// dissipation with the five weights of Coef::kq (order 5 or 9; needs 5 ghost zones): 8th-order BSSN kernels
+template <class P>
+__device__ __forceinline__ double ko_kq(const P& f, int v, const double* kq) {
+  const double f0 = f.at(v, 0, 0, 0);
+  double r = 0.0;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    double s[6];
+#pragma unroll
+    for (int k = 1; k <= 5; ++k) s[k] = (f.ax(v, a, k) - f0) + (f.ax(v, a, -k) - f0);
+    const double q = ((kq[4] * s[5] + kq[3] * s[4]) + (kq[2] * s[3] + kq[1] * s[2])) + kq[0] * s[1];
+    r = a == 0 ? q : r + q;
+  }
+  return r;
+}
 
 // ---- 8th order (wave systems) ------------------------------------------------------------------------
 // 1st derivative (3,-32,168,-672,0,672,-168,32,-3)/840h

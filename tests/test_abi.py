@@ -93,8 +93,8 @@ def test_flop_counts_of_the_fused_kernels(binding):
     order-of-magnitude check on the 8th-order kernel's own FP64 work, and the 4th-order count must be lower.
     Counted from the SASS of the middle-stage instances (DADD + DMUL + 2 DFMA).  The code is straight-line and runs
     once per point, except the loop over the six At_ij advection stencils, whose body appears once and runs six
-    times: the static count (3708 / 5848) is the executed one (4088 / 6588, what bench.py uses) minus five such
-    stencils (76 / 148 flops each)."""
+    times: the static count (3708 / 6108) is the executed one (4088 / 6908; bench.py uses the 4th-order figure) minus
+    five such stencils (76 / 160 flops each; the 8th-order one carries the five dissipation weights of S6b)."""
     import shutil
     import subprocess
     cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
@@ -114,6 +114,6 @@ def test_flop_counts_of_the_fused_kernels(binding):
                 if " %s " % op in line or " %s." % op in line:
                     counts[cur] += w
     assert set(counts) == {4, 8}, counts
-    executed = {4: counts[4] + 5 * 76, 8: counts[8] + 5 * 148}
+    executed = {4: counts[4] + 5 * 76, 8: counts[8] + 5 * 160}
     assert 3000 < executed[4] < executed[8]
     assert 7900 / 2 < executed[8] < 7900 * 2

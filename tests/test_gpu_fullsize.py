@@ -155,8 +155,10 @@ def test_bssn_rk3_enforced_256_sampled(oracle):
     assert worst < 2e-11, worst
 
 
-def test_bssn_o8_rk3_enforced_256_sampled(oracle):
-    """The paper's configuration at full size: BSSN 256^3, 8th order, 5 ghost zones, RK3 + enforcement, 1 step."""
+@pytest.mark.parametrize("ko_order", [5, 9])
+def test_bssn_o8_rk3_enforced_256_sampled(oracle, ko_order):
+    """The paper's configuration at full size: BSSN 256^3, 8th order, 5 ghost zones, RK3 + enforcement, 1 step;
+    dissipation of order 5 (S6) and 9 (S6b)."""
     import torch
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
@@ -166,6 +168,7 @@ def test_bssn_o8_rk3_enforced_256_sampled(oracle):
     u0 = inputs.bssn_gaussians(n, n, n)
     h = binding.Chemora(n, n, n, g, 8, binding.SYS_BSSN, dx)
     h.set_param("eps_diss", 0.1)
+    h.set_param("ko_order", ko_order)
     h.set_state(u0)
     h.autotune()
     h.rk3_step(dt)
@@ -179,7 +182,8 @@ def test_bssn_o8_rk3_enforced_256_sampled(oracle):
     reach, core, worst = 15 * steps, 4, 0.0
     for cpt in centres:
         blk = cut(u0, cpt, core + reach)
-        st = oracle.rk3(oracle.SYS_BSSN, oracle.with_ghosts(blk, g), g, 8, dx, dt, oracle.params(eps_diss=0.1), steps, True)
+        st = oracle.rk3(oracle.SYS_BSSN, oracle.with_ghosts(blk, g), g, 8, dx, dt,
+                        oracle.params(eps_diss=0.1, ko_order=ko_order), steps, True)
         want = oracle.interior(st, g)[:, reach:reach + 2 * core, reach:reach + 2 * core, reach:reach + 2 * core]
         have = cut(got, cpt, core)
         for v in range(25):

@@ -380,6 +380,40 @@ def test_bssn_o8_rk4_10_steps_and_rk3_enforced(chem, oracle, fused):
     h.destroy()
 
 
+@pytest.mark.parametrize("fused", [1, 0])
+def test_bssn_o8_ko9(chem, oracle, fused):
+    """reading S6b: 8th-order BSSN with the 11-point 9th-order KO operator -- RHS on noise and on
+    strong fields, then RK3 + enforcement; and the parameter is refused where it is not built"""
+    nx, ny, nz, g = 21, 14, 11, 5
+    dx, dt, eps = 0.05, 0.0125, 0.1
+    h = chem.Chemora(nx, ny, nz, g, 8, 1, dx)
+    h.set_param("eps_diss", eps)
+    h.set_param("ko_order", 9)
+    assert h.get_param("ko_order") == 9.0
+    h.set_variant(fused, 0)
+    for u in (inputs.bssn_noise(nx, ny, nz), strong_field(nx, ny, nz, seed=43)):
+        want = oracle_rhs(oracle, 1, u, g, 8, dx, eps_diss=eps, ko_order=9)
+        assert relerr(gpu_rhs(h, u), want) < TOL_RHS
+        # and it is not the 5th-order operator
+        assert relerr(oracle_rhs(oracle, 1, u, g, 8, dx, eps_diss=eps), want) > 1e-6
+    u0 = inputs.bssn_noise(nx, ny, nz)
+    h.set_state(u0)
+    for _ in range(5):
+        h.rk3_step(dt)
+        h.enforce_constraints()
+    st = oracle.rk3(1, oracle.with_ghosts(u0, g), g, 8, dx, dt, oracle.params(eps_diss=eps, ko_order=9), 5, True)
+    assert relerr(h.get_state(), oracle.interior(st, g)) < TOL_BSSN_10_STEPS
+    with pytest.raises(chem.ChemoraError):
+        h.set_param("ko_order", 7)
+    h.destroy()
+    for args in ((16, 16, 16, 3, 4, 1, dx), (16, 16, 16, 5, 8, 0, dx)):   # 4th-order BSSN, 8th-order wave
+        b = chem.Chemora(*args)
+        with pytest.raises(chem.ChemoraError):
+            b.set_param("ko_order", 9)
+        b.set_param("ko_order", 5)
+        b.destroy()
+
+
 def test_wave1_energy(chem, oracle):
     """the Energy calculation of the paper's Sample 1: field bit-exact, grid sum to summation-order accuracy, and
     conserved by the evolution of the paper's Gaussian pulse"""
