@@ -86,6 +86,15 @@ int chemora_state_ptr(chemora_t* h, int which, double** dev);
  * synchronised before returning).  Ghosts of U are left untouched by set_state. */
 int chemora_set_state(chemora_t* h, const double* host_packed);
 int chemora_get_state(chemora_t* h, double* host_packed);
+/* The same two copies without the final synchronisation, for pipelining independent handles on different
+ * streams (one handle's copies run under another's kernels): host_packed should be page-locked (with pageable
+ * memory the copy degrades to a synchronous one), must stay valid and, for set, unmodified until
+ * chemora_synchronize(h) returns; each handle stages through its own device buffer, so a handle has at most one
+ * such copy in flight per direction between two synchronisations of the same kind.  chemora_synchronize waits
+ * for everything queued on the handle's stream and returns the first asynchronous error, if any. */
+int chemora_set_state_async(chemora_t* h, const double* host_packed);
+int chemora_get_state_async(chemora_t* h, double* host_packed);
+int chemora_synchronize(chemora_t* h);
 /* Same for a device buffer in the padded layout: pack/unpack between a DEVICE packed array and U
  * (asynchronous on the stream; used by the device-resident benchmark path). */
 int chemora_set_state_dev(chemora_t* h, const double* dev_packed);

@@ -20,7 +20,8 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 
 # every symbol include/chemora.h declares (tests check that the library exports all of them)
 SYMBOLS = ["chemora_create", "chemora_set_param", "chemora_get_param", "chemora_layout", "chemora_state_ptr",
-           "chemora_set_state", "chemora_get_state", "chemora_set_state_dev", "chemora_get_state_dev",
+           "chemora_set_state", "chemora_get_state", "chemora_set_state_async", "chemora_get_state_async",
+           "chemora_synchronize", "chemora_set_state_dev", "chemora_get_state_dev",
            "chemora_fill_ghosts", "chemora_rhs", "chemora_rk4_step", "chemora_rk3_step", "chemora_enforce_constraints", "chemora_energy", "chemora_set_variant",
            "chemora_get_variant", "chemora_tile_shape", "chemora_autotune", "chemora_launch_count",
            "chemora_kernel_info", "chemora_timing", "chemora_timing_read", "chemora_measure_fp64_peak", "chemora_last_error", "chemora_destroy"]
@@ -189,6 +190,31 @@ class Chemora:
             out = np.empty((self.nvars, nz, ny, nx), dtype=np.float64)
         self._ck(self.lib.chemora_get_state(self._h, ctypes.c_void_p(out.ctypes.data)))
         return out
+
+    def _host_ptr(self, a):
+        """host pointer of a numpy array or a (pinned) CPU torch tensor, kept alive until synchronize()"""
+        if not hasattr(self, "_inflight"):
+            self._inflight = []
+        self._inflight.append(a)
+        if isinstance(a, np.ndarray):
+            assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+            n, p = a.size, a.ctypes.data
+        else:
+            assert a.dtype == self._torch.float64 and a.is_contiguous() and not a.is_cuda
+            n, p = a.numel(), a.data_ptr()
+        assert n == self.nvars * self.dims[0] * self.dims[1] * self.dims[2]
+        return ctypes.c_void_p(p)
+
+    def set_state_async(self, host_packed):
+        """queue the copy of a packed host state (page-locked for a real overlap) into U; see chemora.h"""
+        self._ck(self.lib.chemora_set_state_async(self._h, self._host_ptr(host_packed)))
+
+    def get_state_async(self, out):
+        self._ck(self.lib.chemora_get_state_async(self._h, self._host_ptr(out)))
+
+    def synchronize(self):
+        self._ck(self.lib.chemora_synchronize(self._h))
+        self._inflight = []
 
     def set_state_dev(self, dev_packed):
         self._ck(self.lib.chemora_set_state_dev(self._h, self._ptr(dev_packed)))

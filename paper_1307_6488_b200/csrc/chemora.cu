@@ -285,19 +285,16 @@ int chemora_get_state_dev(chemora_t* h, double* dev_packed) {
   return CHEMORA_OK;
 }
 
-int chemora_set_state(chemora_t* h, const double* host_packed) {
+int chemora_set_state_async(chemora_t* h, const double* host_packed) {
   if (!h || !host_packed) return CHEMORA_EINVAL;
   int rc = ensure_staging(h);
   if (rc) return rc;
   CK(h, cudaMemcpyAsync(h->staging, host_packed, packed_count(h) * sizeof(double), cudaMemcpyHostToDevice, h->stream),
      "H2D copy");
-  rc = chemora_set_state_dev(h, h->staging);
-  if (rc) return rc;
-  CK(h, cudaStreamSynchronize(h->stream), "set_state sync");
-  return CHEMORA_OK;
+  return chemora_set_state_dev(h, h->staging);
 }
 
-int chemora_get_state(chemora_t* h, double* host_packed) {
+int chemora_get_state_async(chemora_t* h, double* host_packed) {
   if (!h || !host_packed) return CHEMORA_EINVAL;
   int rc = ensure_staging(h);
   if (rc) return rc;
@@ -305,8 +302,23 @@ int chemora_get_state(chemora_t* h, double* host_packed) {
   if (rc) return rc;
   CK(h, cudaMemcpyAsync(host_packed, h->staging, packed_count(h) * sizeof(double), cudaMemcpyDeviceToHost, h->stream),
      "D2H copy");
-  CK(h, cudaStreamSynchronize(h->stream), "get_state sync");
   return CHEMORA_OK;
+}
+
+int chemora_synchronize(chemora_t* h) {
+  if (!h) return CHEMORA_EINVAL;
+  CK(h, cudaStreamSynchronize(h->stream), "stream synchronisation");
+  return CHEMORA_OK;
+}
+
+int chemora_set_state(chemora_t* h, const double* host_packed) {
+  int rc = chemora_set_state_async(h, host_packed);
+  return rc ? rc : chemora_synchronize(h);
+}
+
+int chemora_get_state(chemora_t* h, double* host_packed) {
+  int rc = chemora_get_state_async(h, host_packed);
+  return rc ? rc : chemora_synchronize(h);
 }
 
 int chemora_fill_ghosts(chemora_t* h, double* dev_state) {

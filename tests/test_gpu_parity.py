@@ -414,6 +414,36 @@ def test_bssn_o8_ko9(chem, oracle, fused):
         b.destroy()
 
 
+def test_async_state_copies_pipeline_two_handles(chem, oracle):
+    """chemora_set_state_async / get_state_async / synchronize: two handles on two streams, pinned host buffers;
+    the results are those of the synchronous calls, bit for bit, and of the oracle to tolerance"""
+    import torch
+    nx, ny, nz, g = 24, 20, 18, 3
+    dx, dt, eps = 0.05, 0.0125, 0.1
+    u = [inputs.bssn_gaussians(nx, ny, nz, width_cells=4.0, seed=s) for s in (5, 6)]
+    side = torch.cuda.Stream()
+    hs = [chem.Chemora(nx, ny, nz, g, 4, 1, dx)]
+    with torch.cuda.stream(side):
+        hs.append(chem.Chemora(nx, ny, nz, g, 4, 1, dx))
+    ins = [torch.from_numpy(x).pin_memory() for x in u]
+    outs = [torch.empty_like(x).pin_memory() for x in ins]
+    for rep in range(3):                      # several rounds through the same staging buffers
+        for h, i, o in zip(hs, ins, outs):
+            h.set_param("eps_diss", eps)
+            h.set_state_async(i)
+            h.rk4_step(dt)
+            h.get_state_async(o)
+        for h in hs:
+            h.synchronize()
+    for h, x, o in zip(hs, u, outs):
+        h.set_state(x)
+        h.rk4_step(dt)
+        assert np.array_equal(h.get_state(), o.numpy())
+        st = oracle.rk4(1, oracle.with_ghosts(x, g), g, 4, dx, dt, oracle.params(eps_diss=eps), 1)
+        assert relerr(o.numpy(), oracle.interior(st, g)) < TOL_BSSN_10_STEPS
+        h.destroy()
+
+
 def test_wave1_energy(chem, oracle):
     """the Energy calculation of the paper's Sample 1: field bit-exact, grid sum to summation-order accuracy, and
     conserved by the evolution of the paper's Gaussian pulse"""
