@@ -122,6 +122,29 @@ def bssn_gaussians(nx, ny, nz, amp=1e-4, width_cells=16.0, seed=SEED_BASE + 3):
 
 
 # The five BASELINE.json configs as (system, dims, ghost, fd_order, dx, eps_diss, generator)
+def bssn_waves_slab(nx, ny, nz, z0, z1, amp=1e-4, seed=SEED_BASE + 6):
+    """Planes z0 <= k < z1 (k taken mod nz) of a periodic near-Minkowski state that can be generated slab by slab:
+    every slot = its Minkowski value + amp * sin(2 pi (mx i/nx + my j/ny + mz k/nz) + phase), with seeded integer
+    mode numbers per slot (wavelength nx/mx >= 8 cells in x and y, about 16..32 cells in z).  Used for blocks too
+    large to build on the host in one piece (more than 2^31 elements per buffer)."""
+    rng = np.random.default_rng(seed)
+    mx = rng.integers(1, max(nx // 8, 1) + 1, size=25)
+    my = rng.integers(1, max(ny // 8, 1) + 1, size=25)
+    mz = rng.integers(max(nz // 32, 1), max(nz // 16, 1) + 1, size=25)
+    ph = rng.uniform(0.0, 2 * np.pi, size=25)
+    k = np.arange(z0, z1, dtype=np.int64) % nz
+    j = np.arange(ny, dtype=np.int64)
+    i = np.arange(nx, dtype=np.int64)
+    out = np.empty((25, z1 - z0, ny, nx), dtype=np.float64)
+    base = bssn_minkowski(1, 1, 1)[:, 0, 0, 0]
+    for v in range(25):
+        # integer products reduced modulo the period first, so the phase keeps full precision at large nz
+        arg = (2 * np.pi) * (((mz[v] * k) % nz)[:, None, None] / nz + ((my[v] * j) % ny)[None, :, None] / ny
+                             + ((mx[v] * i) % nx)[None, None, :] / nx) + ph[v]
+        out[v] = base[v] + amp * np.sin(arg)
+    return out
+
+
 def config(index, scale=None):
     """Returns a dict describing BASELINE.json configs[index]; `scale` overrides the cube size
     (for parity tests at sizes the oracle finishes in seconds)."""

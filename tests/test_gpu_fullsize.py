@@ -193,3 +193,53 @@ def test_bssn_o8_rk3_enforced_256_sampled(oracle, ko_order):
             else:
                 worst = max(worst, err / scale[v])
     assert worst < 1e-11, worst
+
+
+def test_bssn_more_than_2_31_elements_per_buffer(oracle):
+    """Maximum-size edge: a 32 x 32 x 48000 BSSN block has 2.19e9 doubles per state buffer (17.5 GB; four buffers
+    70 GB), so element offsets of the later variables exceed 2^31 and every kernel's 64-bit indexing is exercised
+    (ghost fill, the fused kernel's TMA coordinates and operand maps, the stores).  State built slab by slab from
+    the seeded analytic generator; one RK4 step on two fused tile shapes; windows compared with the oracle, among
+    them the last planes of the last variables and the wrap-around in z."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    if torch.cuda.get_device_properties(0).total_memory < 100e9:
+        pytest.skip("needs 80 GB of device memory")
+    from paper_1307_6488_b200 import binding
+    nx, ny, nz, g, dx = 32, 32, 48000, 3, 0.05
+    dt, eps = 0.25 * dx, 0.1
+    h = binding.Chemora(nx, ny, nz, g, 4, binding.SYS_BSSN, dx)
+    assert h.nvars * h.var_stride > 2 ** 31
+    h.set_param("eps_diss", eps)
+    U = h.interior(h.state_view())               # [25, nz, ny, nx] view of the library's buffer
+    slab = 2000
+
+    def load():
+        for z0 in range(0, nz, slab):
+            U[:, z0:z0 + slab] = torch.from_numpy(inputs.bssn_waves_slab(nx, ny, nz, z0, z0 + slab)).to(U.device)
+
+    reach, core = 12, 4
+    half = reach + core
+    centres = [nz - core, 0, nz // 2 + 7, 31337]      # the end (wraps), the start (wraps), two inside
+    load()
+    U0 = U.clone()                                # 9.8 GB: the initial interior, kept on the device
+    for tile in (0, 4):
+        U.copy_(U0)
+        h.set_variant(1, tile)
+        h.rk4_step(dt)
+        torch.cuda.synchronize()
+        scale = [float(U[v].abs().max()) for v in range(25)]
+        worst = 0.0
+        for zc in centres:
+            blk = inputs.bssn_waves_slab(nx, ny, nz, zc - half, zc + half)     # full x, y extent: periodic as is
+            st = oracle.rk4(oracle.SYS_BSSN, oracle.with_ghosts(blk, g), g, 4, dx, dt, oracle.params(eps_diss=eps), 1)
+            want = oracle.interior(st, g)[:, reach:reach + 2 * core]
+            idx = torch.arange(zc - core, zc + core, device=U.device) % nz
+            have = U[:, idx].cpu().numpy()
+            for v in range(25):
+                err = float(np.max(np.abs(have[v] - want[v])))
+                worst = max(worst, err / scale[v]) if scale[v] > 0 else worst
+                assert scale[v] > 0 or err == 0.0
+        assert worst < 1e-11, (tile, worst)
+    h.destroy()
