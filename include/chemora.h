@@ -69,7 +69,10 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
  * (default 0.75), "ko_order" (5, the default, or 9: the 11-point operator (eps/1024h) h^10 (D+D-)^5 that goes
  * with the paper's 8th-order, 5-ghost-zone configuration; accepted for the 8th-order BSSN
  * system only); tuning: "col_rows" (default 32: y-extent in grid rows of the columns in which the fused BSSN
- * kernel visits its tiles, chosen so the halo planes shared by z-neighbour tiles stay in L2).
+ * kernel visits its tiles, chosen so the halo planes shared by z-neighbour tiles stay in L2), "x_images" (default 0;
+ * 1: inside chemora_rk4_step / chemora_rk3_step the fused BSSN kernel also writes the x-ghost images of the stage
+ * states it produces, and the ghost fill of those states leaves the x-ghost columns of the interior rows out;
+ * results are bit-identical either way; measured no net gain at 256^3).
  * Unknown name or invalid value -> CHEMORA_EINVAL. */
 int chemora_set_param(chemora_t* h, const char* name, double value);
 int chemora_get_param(const chemora_t* h, const char* name, double* value);

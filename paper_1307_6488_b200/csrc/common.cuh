@@ -14,6 +14,14 @@ namespace chm {
 #else
 #define CHM_ST(p, v) (*(p) = (v))
 #endif
+#ifndef CHM_IMG_PLAIN
+#define CHM_IMG_PLAIN 1
+#endif
+#if CHM_IMG_PLAIN
+#define CHM_IMG(p, v) (*(p) = (v))   // x-ghost images share their sector with points another CTA writes: keep it in L2
+#else
+#define CHM_IMG(p, v) CHM_ST(p, v)
+#endif
 
 // Device-side view of the padded SoA layout (include/chemora.h "Conventions").
 struct Layout {
@@ -56,6 +64,9 @@ struct Stage {
   double a;              // dt/2, dt/2, dt, dt/6
   int mode;
   double ca, cb;         // MODE_SSP only
+  int xg;                // fused BSSN kernel: != 0 (= nx) => it also writes the x-ghost images of the new state's
+                         // points (columns i < g to i + nx, i >= nx - g to i - nx), so that the next ghost fill can
+                         // leave the x-ghost columns of the interior rows out; needs nx >= 2 g
 };
 
 // a U + b (Y + dt k), every product and sum rounded once
@@ -105,23 +116,30 @@ __device__ __forceinline__ void stage_emit(const Stage& st, long q, double k, co
 }
 
 // Same with the mode as a compile-time constant (no branches in the epilogue of the fused BSSN kernel).
+// xgo: offset of the point's x-ghost image (0: it has none, or Stage::xg is off); see Stage::xg
 template <int MODE>
-__device__ __forceinline__ void stage_emit_t(const Stage& st, long q, double k, const StagePre& pr, bool valid) {
+__device__ __forceinline__ void stage_emit_t(const Stage& st, long q, double k, const StagePre& pr, bool valid,
+                                             long xgo = 0) {
   // values first, stores under one predicate (no divergent region around the arithmetic)
+  const bool img = valid && xgo != 0;
   if (MODE == MODE_RHS) {
     if (valid) CHM_ST(&st.out[q], k);
   } else if (MODE == MODE_FIRST) {
     const double y = __dadd_rn(pr.u, __dmul_rn(st.a, k));
     if (valid) { CHM_ST(&st.S[q], k); CHM_ST(&st.out[q], y); }
+    if (img) CHM_IMG(&st.out[q + xgo], y);
   } else if (MODE == MODE_MID) {
     const double s2 = __dadd_rn(pr.s, __dmul_rn(2.0, k)), y = __dadd_rn(pr.u, __dmul_rn(st.a, k));
     if (valid) { CHM_ST(&st.S[q], s2); CHM_ST(&st.out[q], y); }
+    if (img) CHM_IMG(&st.out[q + xgo], y);
   } else if (MODE == MODE_LAST) {
     const double u = __dadd_rn(pr.u, __dmul_rn(st.a, __dadd_rn(pr.s, k)));
     if (valid) CHM_ST(&st.U[q], u);
+    if (img) CHM_IMG(&st.U[q + xgo], u);
   } else {
     const double y = ssp_combine(st, pr.u, pr.s, k);   // pr.u = U, pr.s = the evaluated state at the point
     if (valid) CHM_ST(&st.out[q], y);
+    if (img) CHM_IMG(&st.out[q + xgo], y);
   }
 }
 
@@ -137,7 +155,8 @@ static const TileShape kTilesWaveTma[3] = {{32, 16, 32}, {32, 16, 64}, {64, 8, 3
 static const TileShape kTilesMarch[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64, 4, 8}, {128, 2, 8}, {16, 16, 8}};
 
 // launchers implemented in the kernel translation units; each returns the cudaError_t of the launch
-cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s);
+// skip_x: leave the x-ghost columns of the interior rows out (their producer wrote them, Stage::xg)
+cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s, bool skip_x = false);
 cudaError_t launch_energy(const Layout& L, const double* state, double* eps_out, double* sum, cudaStream_t s);
 cudaError_t launch_enforce(const Layout& L, double* state, cudaStream_t s);
 cudaError_t launch_pack(const Layout& L, const double* packed, double* state, bool to_state, cudaStream_t s);

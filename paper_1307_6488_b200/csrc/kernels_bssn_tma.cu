@@ -235,7 +235,8 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       const double* op = sm + slot_of(o) * SLOTX + SLOT + 2 * n * TILE + toff;
       return StagePre{op[0], op[TILE]};
     };
-    auto emit = [&](int v, double k, const StagePre& pr) { stage_emit_t<MODE>(st, q + v * L.vstride, k, pr, valid); };
+    const long xgo = st.xg == 0 ? 0 : (i < L.g ? st.xg : (i >= L.nx - L.g ? -st.xg : 0));   // x-ghost image, Stage::xg
+    auto emit = [&](int v, double k, const StagePre& pr) { stage_emit_t<MODE>(st, q + v * L.vstride, k, pr, valid, xgo); };
 
     // section o: wait for its box, hand out the accessor; done(o): this warp leaves the slot; the last warp to
     // leave refills it with the box 5 loads ahead (of this tile, or of this CTA's next tile)

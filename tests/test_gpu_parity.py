@@ -414,6 +414,26 @@ def test_bssn_o8_ko9(chem, oracle, fused):
         b.destroy()
 
 
+@pytest.mark.parametrize("order,g,dims", [(4, 3, (37, 21, 19)), (4, 3, (6, 9, 7)), (8, 5, (21, 14, 11))])
+def test_x_ghost_images_are_bit_identical(chem, order, g, dims):
+    """tuning switch x_images: the fused kernel writes the x-ghost images itself and the fills skip those columns;
+    RK4 and RK3 give the same bits either way (ragged tiles, nx = 2g, 8th order)"""
+    nx, ny, nz = dims
+    u0 = strong_field(nx, ny, nz, seed=77)
+    h = chem.Chemora(nx, ny, nz, g, order, 1, 0.05)
+    h.set_param("eps_diss", 0.1)
+    res = []
+    for x in (0, 1):
+        h.set_param("x_images", x)
+        h.set_state(u0)
+        for _ in range(2):
+            h.rk4_step(0.0125)
+            h.rk3_step(0.0125)
+        res.append(h.get_state())
+    assert np.array_equal(res[0], res[1])
+    h.destroy()
+
+
 def test_async_state_copies_pipeline_two_handles(chem, oracle):
     """chemora_set_state_async / get_state_async / synchronize: two handles on two streams, pinned host buffers;
     the results are those of the synchronous calls, bit for bit, and of the oracle to tolerance"""
