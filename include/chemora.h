@@ -75,6 +75,19 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
  * results are bit-identical either way; measured no net gain at 256^3).
  * Unknown name or invalid value -> CHEMORA_EINVAL. */
 int chemora_set_param(chemora_t* h, const char* name, double value);
+
+/* The paper's tile cost model re-targeted at this design, for the uniform fused BSSN kernel
+ * (fused tile ids 0..5, 9, 10; 8th order: id 0).  Host arithmetic only, no device needed.
+ *   requests r = the 32-byte L2 sectors one interior tile of a middle RK4 stage requests: the (tx+2H)(ty+2H)(tz+2H)
+ *     halo boxes of the 25 variables (H = fd_order/2 + 1), the point-value and Runge-Kutta operand boxes
+ *     ((tx+2) x ty x tz, 21 + 2*25 of them) and the 2*25 stored tiles, every row counted with its alignment in
+ *     the padded layout ("all lines survive" is exact here: each sector is staged once per tile);
+ *   points = I tx ty tz with I = 1 iteration per thread;
+ *   sigma = (r / points) * (1 + 256 / (tx ty tz)): the request size per grid point, divided by the paper's
+ *     empirical efficiency 1 / (1 + 256/(tx ty tz)) of small tiles (reading S15: the printed formula
+ *     divides by (1 + 256/...), which would favour small tiles against the sentence that introduces it).
+ * Any out pointer may be NULL.  CHEMORA_EINVAL for ids the model does not cover. */
+int chemora_tile_cost(int fd_order, int ghost, int tile_id, double* sigma, long* requests, long* points);
 int chemora_get_param(const chemora_t* h, const char* name, double* value);
 
 /* Layout in units of doubles; any out pointer may be NULL.  interior_offset = offset of interior (0,0,0)

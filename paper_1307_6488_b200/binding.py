@@ -23,7 +23,7 @@ SYMBOLS = ["chemora_create", "chemora_set_param", "chemora_get_param", "chemora_
            "chemora_set_state", "chemora_get_state", "chemora_set_state_async", "chemora_get_state_async",
            "chemora_synchronize", "chemora_set_state_dev", "chemora_get_state_dev",
            "chemora_fill_ghosts", "chemora_rhs", "chemora_rk4_step", "chemora_rk3_step", "chemora_enforce_constraints", "chemora_energy", "chemora_set_variant",
-           "chemora_get_variant", "chemora_tile_shape", "chemora_autotune", "chemora_launch_count",
+           "chemora_get_variant", "chemora_tile_shape", "chemora_tile_cost", "chemora_autotune", "chemora_launch_count",
            "chemora_kernel_info", "chemora_timing", "chemora_timing_read", "chemora_measure_fp64_peak", "chemora_last_error", "chemora_destroy"]
 
 _ALLOC_T = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
@@ -87,6 +87,15 @@ def tile_shape(tile_id, system_id=SYS_BSSN, fused=1):
     if rc:
         raise ChemoraError(rc)
     return a.value, b.value, c.value
+
+
+def tile_cost(fd_order, ghost, tile_id):
+    """(sigma, requests, points) of the paper's tile cost model for a fused BSSN tile id; host arithmetic only"""
+    s, r, n = ctypes.c_double(), ctypes.c_long(), ctypes.c_long()
+    rc = load().chemora_tile_cost(fd_order, ghost, tile_id, ctypes.byref(s), ctypes.byref(r), ctypes.byref(n))
+    if rc:
+        raise ChemoraError(rc)
+    return s.value, r.value, n.value
 
 
 class Chemora:

@@ -435,6 +435,29 @@ int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, 
   return CHEMORA_OK;
 }
 
+// The paper's tile cost model for the uniform fused BSSN kernel; see include/chemora.h.
+int chemora_tile_cost(int fd_order, int ghost, int tile_id, double* sigma, long* requests, long* points) {
+  if (fd_order != 4 && fd_order != 8) return CHEMORA_EINVAL;
+  if (tile_id < 0 || tile_id >= CHEMORA_NUM_TILES || (tile_id >= 6 && tile_id < 9)) return CHEMORA_EINVAL;
+  if (fd_order == 8 && tile_id != 0) return CHEMORA_EINVAL;
+  const int H = fd_order / 2 + 1;
+  if (ghost < H) return CHEMORA_EINVAL;
+  const TileShape T = kTilesFused[tile_id];
+  const int xo = ((ghost - 3) & 1) ? ghost + 1 : ghost;   // the layout rule of chemora_create
+  // 32-byte sectors (4 doubles) covered by `len` doubles from column x0 of a row (rows start 128-byte aligned)
+  auto sectors = [](long x0, long len) { return (x0 + len - 1) / 4 - x0 / 4 + 1; };
+  const long V = 25, rows_box = (long)(T.ty + 2 * H) * (T.tz + 2 * H), rows_tile = (long)T.ty * T.tz;
+  const long r = V * rows_box * sectors(xo - H, T.tx + 2 * H)           // the halo boxes of the 25 variables
+                 + 21 * rows_tile * sectors(xo - 1, T.tx + 2)           // point values needed ahead of their boxes
+                 + 2 * V * rows_tile * sectors(xo - 1, T.tx + 2)        // Runge-Kutta operands U, S
+                 + 2 * V * rows_tile * sectors(xo, T.tx);               // stores S, Y
+  const long n = (long)T.tx * T.ty * T.tz;   // I = 1: one point per thread
+  if (requests) *requests = r;
+  if (points) *points = n;
+  if (sigma) *sigma = ((double)r / (double)n) * (1.0 + 256.0 / (double)n);
+  return CHEMORA_OK;
+}
+
 int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out) {
   if (!h) return CHEMORA_EINVAL;
   const int save_f = h->fused, save_t = h->tile;
