@@ -133,6 +133,21 @@ int chemora_rk4_step(chemora_t* h, double dt);
  * before each of the three RHS evaluations; uses buffers U, YA, YB; asynchronous on the stream. */
 int chemora_rk3_step(chemora_t* h, double dt);
 
+/* Multi-block interface, the second boundary kind (the paper's domains are sets of blocks whose ghost zones are
+ * synchronised from their neighbours): slab decomposition along z.  After
+ * chemora_link_z(h, lower, upper) the ghost z-planes of block h are copied from the top `ghost` interior planes of
+ * `lower` and the bottom `ghost` interior planes of `upper` (the same one of the four buffers), x and y stay
+ * periodic; NULL = the block's own periodic image on that side.  Neighbours have the same nx, ny, ghost width,
+ * system, order, spacing and stream (else CHEMORA_EINVAL) and their own nz >= ghost.  The library keeps the
+ * pointers: unlink (NULL, NULL) before destroying a neighbour.
+ * Linked blocks step together: chemora_rk4_step_group / chemora_rk3_step_group run, stage by stage, every block's
+ * ghost fill and then every block's right-hand side (n <= 64 blocks, all links inside the group, one stream);
+ * chemora_rk4_step / chemora_rk3_step / chemora_fill_ghosts of a foreign buffer return CHEMORA_ESTATE on a linked
+ * block.  A ring of blocks linked periodically gives bit for bit the single-block result. */
+int chemora_link_z(chemora_t* h, chemora_t* lower, chemora_t* upper);
+int chemora_rk4_step_group(chemora_t* const* blocks, int n, double dt);
+int chemora_rk3_step_group(chemora_t* const* blocks, int n, double dt);
+
 /* Algebraic constraint enforcement on the interior of a BSSN state in the padded layout (dev_state == NULL: U):
  * gt_ij <- gt_ij / det(gt)^(1/3), At_ij <- At_ij - 1/3 gt_ij gtu^kl At_kl (reading S10b).  In place, asynchronous.
  * CHEMORA_EINVAL for the wave systems. */

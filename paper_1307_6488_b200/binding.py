@@ -22,7 +22,8 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 SYMBOLS = ["chemora_create", "chemora_set_param", "chemora_get_param", "chemora_layout", "chemora_state_ptr",
            "chemora_set_state", "chemora_get_state", "chemora_set_state_async", "chemora_get_state_async",
            "chemora_synchronize", "chemora_set_state_dev", "chemora_get_state_dev",
-           "chemora_fill_ghosts", "chemora_rhs", "chemora_rk4_step", "chemora_rk3_step", "chemora_enforce_constraints", "chemora_energy", "chemora_set_variant",
+           "chemora_fill_ghosts", "chemora_rhs", "chemora_rk4_step", "chemora_rk3_step", "chemora_link_z",
+           "chemora_rk4_step_group", "chemora_rk3_step_group", "chemora_enforce_constraints", "chemora_energy", "chemora_set_variant",
            "chemora_get_variant", "chemora_tile_shape", "chemora_tile_cost", "chemora_autotune", "chemora_launch_count",
            "chemora_kernel_info", "chemora_timing", "chemora_timing_read", "chemora_measure_fp64_peak", "chemora_last_error", "chemora_destroy"]
 
@@ -60,6 +61,10 @@ def load():
         "chemora_fill_ghosts": [vp, vp], "chemora_rhs": [vp, vp, vp],
         "chemora_rk4_step": [vp, d],
         "chemora_rk3_step": [vp, d],
+        "chemora_set_state_async": [vp, vp], "chemora_get_state_async": [vp, vp], "chemora_synchronize": [vp],
+        "chemora_link_z": [vp, vp, vp],
+        "chemora_rk4_step_group": [ctypes.POINTER(vp), i, d], "chemora_rk3_step_group": [ctypes.POINTER(vp), i, d],
+        "chemora_tile_cost": [i, i, i, dp, lp, lp],
         "chemora_enforce_constraints": [vp, vp],
         "chemora_energy": [vp, vp, vp, dp],
         "chemora_set_variant": [vp, i, i], "chemora_get_variant": [vp, ip, ip],
@@ -87,6 +92,13 @@ def tile_shape(tile_id, system_id=SYS_BSSN, fused=1):
     if rc:
         raise ChemoraError(rc)
     return a.value, b.value, c.value
+
+
+def step_group(blocks, dt, rk3=False):
+    """one RK4 (or RK3) step of a group of z-linked blocks: chemora_rk4_step_group / chemora_rk3_step_group"""
+    arr = (ctypes.c_void_p * len(blocks))(*[b._h for b in blocks])
+    fn = blocks[0].lib.chemora_rk3_step_group if rk3 else blocks[0].lib.chemora_rk4_step_group
+    blocks[0]._ck(fn(arr, len(blocks), float(dt)))
 
 
 def tile_cost(fd_order, ghost, tile_id):
@@ -242,6 +254,11 @@ class Chemora:
 
     def rk3_step(self, dt):
         self._ck(self.lib.chemora_rk3_step(self._h, float(dt)))
+
+    def link_z(self, lower=None, upper=None):
+        """multi-block interface: the ghost z-planes come from the neighbour blocks' interiors (None: own images)"""
+        self._ck(self.lib.chemora_link_z(self._h, lower._h if lower is not None else None,
+                                         upper._h if upper is not None else None))
 
     def enforce_constraints(self, state=None):
         """in place on a padded device state tensor (default: U)"""

@@ -29,6 +29,8 @@ struct chemora {
   double* derivs;       // split variant scratch (lazy)
   double* staging;      // device packed staging for set/get_state (lazy)
   int fused, tile;
+  chemora* nb_lo;        // z-neighbours of a linked block (chemora_link_z); nullptr: periodic in itself
+  chemora* nb_hi;
   long launches;
   // optional per-kernel timing (chemora_timing): event pairs around every RHS evaluation / ghost fill
   bool timing;
@@ -151,8 +153,21 @@ int stage_xg(const chemora_t* h) {
 }
 
 int fill(chemora_t* h, double* state, bool skip_x = false) {
+  FillLink link, *lp = nullptr;
+  if (h->nb_lo || h->nb_hi) {
+    // a linked block takes its ghost z-planes from the SAME buffer of its neighbours, so the state must be one of
+    // the library's four buffers
+    int which = -1;
+    for (int b = 0; b < 4; ++b)
+      if (state == h->buf[b]) which = b;
+    if (which < 0) return fail(h, CHEMORA_ESTATE, "a z-linked block can fill only its own four buffers");
+    chemora_t* lo = h->nb_lo ? h->nb_lo : h;
+    chemora_t* hi = h->nb_hi ? h->nb_hi : h;
+    link = FillLink{lo->buf[which], lo->L.vstride, lo->L.nz, hi->buf[which], hi->L.vstride};
+    lp = &link;
+  }
   tick(h, 1);
-  CK(h, launch_fill_ghosts(h->L, state, h->stream, skip_x), "ghost fill launch");
+  CK(h, launch_fill_ghosts(h->L, state, h->stream, skip_x, lp), "ghost fill launch");
   tick(h, 1);
   h->launches += 1;
   if (h->timing) h->ev_launches[1] += 1;
@@ -191,6 +206,7 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
   h->order = fd_order; h->system = system_id; h->dx = dx;
   h->eps_diss = 0.0; h->eta = 1.0; h->sgc = 0.75;
   h->ko_order = 5;
+  h->nb_lo = h->nb_hi = nullptr;
   h->x_images = 0;   // measured at 256^3: the fills save 0.10 ms each, the fused kernel loses 0.15-0.2 ms per launch
   h->stream = (cudaStream_t)cuda_stream;
   h->alloc = alloc; h->dealloc = dealloc; h->actx = alloc_ctx;
@@ -346,40 +362,91 @@ int chemora_rhs(chemora_t* h, const double* dev_state, double* dev_rhs) {
   return run_rhs(h, st);
 }
 
-int chemora_rk4_step(chemora_t* h, double dt) {
-  if (!h || !(dt == dt)) return CHEMORA_EINVAL;
+// The steppers as stage tables: stage s fills buffer `in` (ghosts), then evaluates the right-hand side with the
+// Runge-Kutta epilogue `st`.  One block: stage after stage.  A group of z-linked blocks: every block's fill of a
+// stage, then every block's evaluation (a fill reads the neighbours' interiors of the same stage buffer).
+struct StagePlan { int in; Stage st; bool skip_x; };
+
+static int rk4_plan(chemora_t* h, double dt, StagePlan* p) {
   double *U = h->buf[0], *Ya = h->buf[1], *Yb = h->buf[2], *S = h->buf[3];
   const int xg = stage_xg(h);   // stages 1..3 write the x-ghost images of the state the next stage evaluates
-  int rc;
   // stage 1: k1 = f(U);  S = k1;  Yb = U + dt/2 k1      (U may have been touched by the caller: full fill)
-  if ((rc = fill(h, U))) return rc;
-  if ((rc = run_rhs(h, Stage{U, U, S, Yb, dt / 2.0, MODE_FIRST, 0.0, 0.0, xg}))) return rc;
+  p[0] = {0, Stage{U, U, S, Yb, dt / 2.0, MODE_FIRST, 0.0, 0.0, xg}, false};
   // stage 2: k2 = f(Yb); S += 2 k2; Ya = U + dt/2 k2
-  if ((rc = fill(h, Yb, xg != 0))) return rc;
-  if ((rc = run_rhs(h, Stage{Yb, U, S, Ya, dt / 2.0, MODE_MID, 0.0, 0.0, xg}))) return rc;
+  p[1] = {2, Stage{Yb, U, S, Ya, dt / 2.0, MODE_MID, 0.0, 0.0, xg}, xg != 0};
   // stage 3: k3 = f(Ya); S += 2 k3; Yb = U + dt k3
-  if ((rc = fill(h, Ya, xg != 0))) return rc;
-  if ((rc = run_rhs(h, Stage{Ya, U, S, Yb, dt, MODE_MID, 0.0, 0.0, xg}))) return rc;
+  p[2] = {1, Stage{Ya, U, S, Yb, dt, MODE_MID, 0.0, 0.0, xg}, xg != 0};
   // stage 4: k4 = f(Yb); U = U + dt/6 (S + k4)
-  if ((rc = fill(h, Yb, xg != 0))) return rc;
-  if ((rc = run_rhs(h, Stage{Yb, U, S, nullptr, dt / 6.0, MODE_LAST, 0.0, 0.0, 0}))) return rc;
+  p[3] = {2, Stage{Yb, U, S, nullptr, dt / 6.0, MODE_LAST, 0.0, 0.0, 0}, xg != 0};
+  return 4;
+}
+
+static int rk3_plan(chemora_t* h, double dt, StagePlan* p) {
+  double *U = h->buf[0], *Ya = h->buf[1], *Yb = h->buf[2];
+  const int xg = stage_xg(h);
+  // U1 = U + dt f(U)
+  p[0] = {0, Stage{U, U, nullptr, Ya, dt, MODE_SSP, 0.0, 1.0, xg}, false};
+  // U2 = 3/4 U + 1/4 (U1 + dt f(U1))
+  p[1] = {1, Stage{Ya, U, nullptr, Yb, dt, MODE_SSP, 3.0 / 4.0, 1.0 / 4.0, xg}, xg != 0};
+  // U+ = 1/3 U + 2/3 (U2 + dt f(U2)), written over U point by point
+  p[2] = {2, Stage{Yb, U, nullptr, U, dt, MODE_SSP, 1.0 / 3.0, 2.0 / 3.0, 0}, xg != 0};
+  return 3;
+}
+
+static int step_one(chemora_t* h, double dt, bool rk3) {
+  if (!h || !(dt == dt)) return CHEMORA_EINVAL;
+  if (h->nb_lo || h->nb_hi) return fail(h, CHEMORA_ESTATE, "a z-linked block steps through the *_step_group calls");
+  StagePlan p[4];
+  const int ns = rk3 ? rk3_plan(h, dt, p) : rk4_plan(h, dt, p);
+  for (int s = 0; s < ns; ++s) {
+    int rc;
+    if ((rc = fill(h, h->buf[p[s].in], p[s].skip_x))) return rc;
+    if ((rc = run_rhs(h, p[s].st))) return rc;
+  }
   return CHEMORA_OK;
 }
 
-int chemora_rk3_step(chemora_t* h, double dt) {
-  if (!h || !(dt == dt)) return CHEMORA_EINVAL;
-  double *U = h->buf[0], *Ya = h->buf[1], *Yb = h->buf[2];
-  const int xg = stage_xg(h);
-  int rc;
-  // U1 = U + dt f(U)
-  if ((rc = fill(h, U))) return rc;
-  if ((rc = run_rhs(h, Stage{U, U, nullptr, Ya, dt, MODE_SSP, 0.0, 1.0, xg}))) return rc;
-  // U2 = 3/4 U + 1/4 (U1 + dt f(U1))
-  if ((rc = fill(h, Ya, xg != 0))) return rc;
-  if ((rc = run_rhs(h, Stage{Ya, U, nullptr, Yb, dt, MODE_SSP, 3.0 / 4.0, 1.0 / 4.0, xg}))) return rc;
-  // U+ = 1/3 U + 2/3 (U2 + dt f(U2)), written over U point by point
-  if ((rc = fill(h, Yb, xg != 0))) return rc;
-  if ((rc = run_rhs(h, Stage{Yb, U, nullptr, U, dt, MODE_SSP, 1.0 / 3.0, 2.0 / 3.0, 0}))) return rc;
+static int step_group(chemora_t* const* hs, int n, double dt, bool rk3) {
+  if (!hs || n < 1 || n > 64 || !(dt == dt)) return CHEMORA_EINVAL;
+  for (int b = 0; b < n; ++b) {
+    chemora_t* h = hs[b];
+    if (!h) return CHEMORA_EINVAL;
+    if (h->stream != hs[0]->stream) return fail(h, CHEMORA_EINVAL, "the blocks of a group share one stream");
+    for (chemora_t* nb : {h->nb_lo, h->nb_hi}) {
+      bool in_group = nb == nullptr;
+      for (int c = 0; c < n; ++c) in_group = in_group || hs[c] == nb;
+      if (!in_group) return fail(h, CHEMORA_EINVAL, "a block of the group is linked to a block outside it");
+    }
+  }
+  StagePlan p[64][4];
+  int ns = 0;
+  for (int b = 0; b < n; ++b) ns = rk3 ? rk3_plan(hs[b], dt, p[b]) : rk4_plan(hs[b], dt, p[b]);
+  for (int s = 0; s < ns; ++s) {
+    int rc;
+    for (int b = 0; b < n; ++b)
+      if ((rc = fill(hs[b], hs[b]->buf[p[b][s].in], p[b][s].skip_x))) return rc;
+    for (int b = 0; b < n; ++b)
+      if ((rc = run_rhs(hs[b], p[b][s].st))) return rc;
+  }
+  return CHEMORA_OK;
+}
+
+int chemora_rk4_step(chemora_t* h, double dt) { return step_one(h, dt, false); }
+int chemora_rk3_step(chemora_t* h, double dt) { return step_one(h, dt, true); }
+int chemora_rk4_step_group(chemora_t* const* hs, int n, double dt) { return step_group(hs, n, dt, false); }
+int chemora_rk3_step_group(chemora_t* const* hs, int n, double dt) { return step_group(hs, n, dt, true); }
+
+int chemora_link_z(chemora_t* h, chemora_t* lower, chemora_t* upper) {
+  if (!h) return CHEMORA_EINVAL;
+  for (chemora_t* nb : {lower, upper}) {
+    if (!nb) continue;
+    if (nb->L.nx != h->L.nx || nb->L.ny != h->L.ny || nb->L.g != h->L.g || nb->system != h->system ||
+        nb->order != h->order || nb->dx != h->dx)
+      return fail(h, CHEMORA_EINVAL, "a z-neighbour has the same nx, ny, ghost width, system, order and spacing");
+    if (nb->stream != h->stream) return fail(h, CHEMORA_EINVAL, "z-neighbours share the block's stream");
+  }
+  h->nb_lo = lower;
+  h->nb_hi = upper;
   return CHEMORA_OK;
 }
 

@@ -155,8 +155,16 @@ static const TileShape kTilesWaveTma[3] = {{32, 16, 32}, {32, 16, 64}, {64, 8, 3
 static const TileShape kTilesMarch[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64, 4, 8}, {128, 2, 8}, {16, 16, 8}};
 
 // launchers implemented in the kernel translation units; each returns the cudaError_t of the launch
-// skip_x: leave the x-ghost columns of the interior rows out (their producer wrote them, Stage::xg)
-cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s, bool skip_x = false);
+// Source of the ghost z-planes when the block is linked to z-neighbours (multi-block interface): the same state
+// buffer of the lower / upper neighbour block (same nx, ny, ghost width and row layout; its own nz).
+struct FillLink {
+  const double* lo;  long lo_vstride;  int lo_nz;    // lower neighbour: its top g interior planes
+  const double* hi;  long hi_vstride;                // upper neighbour: its bottom g interior planes
+};
+// skip_x: leave the x-ghost columns of the interior rows out (their producer wrote them, Stage::xg);
+// link: where the ghost z-planes come from (nullptr: the block's own periodic images)
+cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s, bool skip_x = false,
+                               const FillLink* link = nullptr);
 cudaError_t launch_energy(const Layout& L, const double* state, double* eps_out, double* sum, cudaStream_t s);
 cudaError_t launch_enforce(const Layout& L, double* state, cudaStream_t s);
 cudaError_t launch_pack(const Layout& L, const double* packed, double* state, bool to_state, cudaStream_t s);

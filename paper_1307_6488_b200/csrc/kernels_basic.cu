@@ -14,7 +14,7 @@ namespace chm {
 // decode was bound by the divisions, not by memory: 0.285 ms per fill at 256^3 x 25 variables, 1.7 TB/s).
 // ---------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) fill_ghosts_kernel(Layout L, double* __restrict__ state, int rowsA, int rowsAB,
-                                                          int lpr_shift) {
+                                                          int lpr_shift, FillLink link) {
   const int g = L.g, tx = L.nx + 2 * g, lane = threadIdx.x & 31;
   const int task = blockIdx.x * 8 + (threadIdx.x >> 5);
   auto wrap = [g](int c, int n) { int r = (c - g) % n; return (r < 0 ? r + n : r) + g; };
@@ -32,6 +32,11 @@ __global__ void __launch_bounds__(256) fill_ghosts_kernel(Layout L, double* __re
       j = jj < g ? jj : jj + L.ny;
     }
     const double* src = p + (long)wrap(k, L.nz) * L.plane + (long)wrap(j, L.ny) * L.pitch;
+    if (task < rowsA) {   // ghost z-plane: from the linked neighbour (the block itself when it is not linked)
+      src = k < g ? link.lo + (long)blockIdx.y * link.lo_vstride + (L.xo - g) + (long)(link.lo_nz + k) * L.plane
+                  : link.hi + (long)blockIdx.y * link.hi_vstride + (L.xo - g) + (long)(k - L.nz) * L.plane;
+      src += (long)wrap(j, L.ny) * L.pitch;
+    }
     double* dst = p + (long)k * L.plane + (long)j * L.pitch;
     for (int i = lane; i < tx; i += 32) dst[i] = src[wrap(i, L.nx)];
   } else {
@@ -48,7 +53,7 @@ __global__ void __launch_bounds__(256) fill_ghosts_kernel(Layout L, double* __re
   }
 }
 
-cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s, bool skip_x) {
+cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s, bool skip_x, const FillLink* link) {
   const int g = L.g;
   if (g == 0) return cudaSuccess;
   const long rowsA = 2L * g * L.tot_y, rowsAB = rowsA + 2L * g * L.nz, rowsC = skip_x ? 0 : (long)L.nz * L.ny;
@@ -57,7 +62,8 @@ cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s, b
   const long tasks = rowsAB + (rowsC + (32 >> lpr_shift) - 1) / (32 >> lpr_shift);
   if (tasks > 0x7fffffffL - 8 || rowsC > 0x7fffffffL) return cudaErrorInvalidValue;
   dim3 grid((unsigned)((tasks + 7) / 8), L.nvars);
-  fill_ghosts_kernel<<<grid, 256, 0, s>>>(L, state, (int)rowsA, (int)rowsAB, lpr_shift);
+  const FillLink self{state, L.vstride, L.nz, state, L.vstride};
+  fill_ghosts_kernel<<<grid, 256, 0, s>>>(L, state, (int)rowsA, (int)rowsAB, lpr_shift, link ? *link : self);
   return cudaGetLastError();
 }
 

@@ -434,6 +434,51 @@ def test_x_ghost_images_are_bit_identical(chem, order, g, dims):
     h.destroy()
 
 
+@pytest.mark.parametrize("system,order,g,rk3", [(1, 4, 3, False), (1, 4, 3, True), (0, 8, 4, False), (2, 4, 3, False),
+                                                (1, 8, 5, True)])
+def test_z_linked_blocks_equal_the_single_block(chem, oracle, system, order, g, rk3):
+    """multi-block interface (chemora_link_z + step_group): a periodic ring of three slabs of different thickness
+    evolves bit for bit like the single block it decomposes; the single block is checked against the oracle"""
+    nx, ny, cuts = 20, 14, (0, 13, 19, 30)
+    nz = cuts[-1]
+    dx, dt, eps, steps = 0.05, 0.0125, 0.1, 3
+    V = {0: 2, 1: 25, 2: 5}[system]
+    u0 = strong_field(nx, ny, nz, seed=91) if system == 1 else np.random.default_rng(91).standard_normal((V, nz, ny, nx))
+    one = chem.Chemora(nx, ny, nz, g, order, system, dx)
+    one.set_param("eps_diss", eps)
+    one.set_state(u0)
+    blocks = []
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        h = chem.Chemora(nx, ny, b - a, g, order, system, dx)
+        h.set_param("eps_diss", eps)
+        h.set_state(np.ascontiguousarray(u0[:, a:b]))
+        blocks.append(h)
+    for n, h in enumerate(blocks):
+        h.link_z(lower=blocks[n - 1], upper=blocks[(n + 1) % len(blocks)])
+    with pytest.raises(chem.ChemoraError):
+        blocks[0].rk4_step(dt)                       # a linked block does not step alone
+    for _ in range(steps):
+        (one.rk3_step if rk3 else one.rk4_step)(dt)
+        chem.step_group(blocks, dt, rk3=rk3)
+    want = one.get_state()
+    got = np.concatenate([h.get_state() for h in blocks], axis=1)
+    assert np.array_equal(got, want)
+    orc = (oracle.rk3 if rk3 else oracle.rk4)(system, oracle.with_ghosts(u0, g), g, order, dx, dt,
+                                              oracle.params(eps_diss=eps), steps)
+    assert relerr(want, oracle.interior(orc, g)) < (TOL_BSSN_10_STEPS if system == 1 else 1e-12 * steps)
+    with pytest.raises(chem.ChemoraError):
+        chem.step_group(blocks[:2], dt)              # a link leaves the group
+    other = chem.Chemora(nx + 2, ny, 8, g, order, system, dx)
+    with pytest.raises(chem.ChemoraError):
+        blocks[0].link_z(lower=other)
+    other.destroy()
+    for h in blocks:
+        h.link_z()
+    blocks[0].rk4_step(dt)                           # unlinked again: steps alone
+    for h in blocks + [one]:
+        h.destroy()
+
+
 def test_async_state_copies_pipeline_two_handles(chem, oracle):
     """chemora_set_state_async / get_state_async / synchronize: two handles on two streams, pinned host buffers;
     the results are those of the synchronous calls, bit for bit, and of the oracle to tolerance"""
