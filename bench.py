@@ -34,8 +34,8 @@ BYTES_PER_POINT_PER_LAUNCH = BYTES_PER_UPDATE / 4.0
 # middle-stage instance of the default tile).  An upper bound on the paper's convention.
 FLOPS_PER_RHS_POINT = 4088.0
 # dram__bytes_read.sum + dram__bytes_write.sum of the fused kernel at 256^3, mean over the 4 launches of an RK4 step
-# (ncu --set full, profiles/r01_d_fused_ncu_full.md); None for other variants / sizes
-NCU_TRAFFIC_BYTES_256 = 18.25e9
+# (ncu --set full, profiles/r01_j_fused_ncu_full.md; capture D had 18.25e9); None for other variants / sizes
+NCU_TRAFFIC_BYTES_256 = 19.60e9
 
 
 def peaks():
