@@ -128,7 +128,10 @@ int run_rhs_inner(chemora_t* h, const Stage& st) {
       CK(h, launch_wave(h->L, C, h->order, h->tile % 6, st, h->stream), "wave kernel launch");
     h->launches += 1;
   } else if (h->system == CHEMORA_SYS_WAVE1) {
-    CK(h, launch_wave1(h->L, C, h->order, h->tile % 6, st, h->stream), "first-order wave kernel launch");
+    if (h->tile >= 6 && h->tile < 9 && wave1_tma_ok(h->L, h->order, C.ko != 0.0, h->tile - 6))
+      CK(h, launch_wave1_tma(h->L, C, h->order, h->tile - 6, st, h->stream), "first-order wave plane-ring kernel launch");
+    else
+      CK(h, launch_wave1(h->L, C, h->order, h->tile % 6, st, h->stream), "first-order wave kernel launch");
     h->launches += 1;
   } else if (h->fused) {
     if (h->tile >= 6 && h->tile < 9) CK(h, launch_bssn_ws(h->L, C, h->tile - 6, st, h->stream), "bssn warp-specialised kernel launch");
@@ -495,6 +498,7 @@ int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, 
   const bool f = system_id == CHEMORA_SYS_BSSN && fused;
   const TileShape T = f ? kTilesFused[tile_id]
                       : (system_id == CHEMORA_SYS_WAVE && tile_id >= 6 && tile_id < 9) ? kTilesWaveTma[tile_id - 6]
+                      : (system_id == CHEMORA_SYS_WAVE1 && tile_id >= 6 && tile_id < 9) ? kTilesWave1Tma[tile_id - 6]
                                                                                         : kTilesMarch[tile_id % 6];
   if (tx) *tx = T.tx;
   if (ty) *ty = T.ty;
@@ -538,7 +542,7 @@ int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out)
     for (int t = 0; t < CHEMORA_NUM_TILES && !rc; ++t) {
       float ms = -1.f;
       const bool bssn = h->system == CHEMORA_SYS_BSSN, o8 = bssn && h->order == 8 && t != 0;   // O8 BSSN: one fused tile
-      const int nwave = h->system == CHEMORA_SYS_WAVE ? 9 : 6;   // (phi, pi) has three more ids: the plane-ring kernel
+      const int nwave = 9;   // the wave systems have three more ids: the plane-ring kernel
       if ((f == 1 && !o8 && (bssn || t < nwave)) || (f == 0 && bssn && t < 6)) {
         h->fused = f; h->tile = t;
         // a middle RK4 stage (the common case) on scratch operands: k = f(U); S += 2k; Ya = U + a k.
@@ -604,6 +608,9 @@ int chemora_kernel_info(const chemora_t* h, int* regs, int* local_bytes, int* sm
   cudaFuncAttributes a;
   cudaError_t e = h->system == CHEMORA_SYS_WAVE && h->tile >= 6 && h->tile < 9 ? kernel_info_wave_tma(h->order, h->tile - 6, &a)
                   : h->system == CHEMORA_SYS_WAVE ? kernel_info_wave(h->order, h->tile % 6, &a)
+                  : h->system == CHEMORA_SYS_WAVE1 && h->tile >= 6 && h->tile < 9 &&
+                            wave1_tma_ok(h->L, h->order, true, h->tile - 6)
+                      ? kernel_info_wave1_tma(h->order, h->tile - 6, &a)
                   : h->system == CHEMORA_SYS_WAVE1 ? kernel_info_wave1(h->order, h->tile % 6, &a)
                   : !h->fused              ? kernel_info_bssn_split(1, h->tile % 6, &a)
                   : h->tile >= 6 && h->tile < 9 ? kernel_info_bssn_ws(h->tile - 6, &a)

@@ -152,6 +152,8 @@ static const TileShape kTilesFused[11] = {{16, 4, 4}, {16, 8, 2}, {8, 8, 4}, {8,
                                           {16, 4, 4}, {16, 8, 2}, {16, 2, 8}, {16, 4, 6}, {16, 6, 4}};
 // wave system ids 6..8: the TMA plane-ring kernel (x, y = thread block, z = planes per work item)
 static const TileShape kTilesWaveTma[3] = {{32, 16, 32}, {32, 16, 64}, {64, 8, 32}};
+// Sample-1 system ids 6..8: the same plane-ring kernel with five variables (smaller tiles: the ring holds 5 boxes a plane)
+static const TileShape kTilesWave1Tma[3] = {{16, 8, 32}, {16, 16, 32}, {32, 8, 32}};
 static const TileShape kTilesMarch[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64, 4, 8}, {128, 2, 8}, {16, 16, 8}};
 
 // launchers implemented in the kernel translation units; each returns the cudaError_t of the launch
@@ -172,6 +174,9 @@ cudaError_t launch_wave(const Layout& L, const Coef& C, int order, int tile, con
 cudaError_t launch_wave_tma(const Layout& L, const Coef& C, int order, int which, const Stage& st, cudaStream_t s);
 cudaError_t kernel_info_wave_tma(int order, int which, cudaFuncAttributes* a);
 bool wave_tma_ok(const Layout& L, int order, bool ko);
+cudaError_t launch_wave1_tma(const Layout& L, const Coef& C, int order, int which, const Stage& st, cudaStream_t s);
+cudaError_t kernel_info_wave1_tma(int order, int which, cudaFuncAttributes* a);
+bool wave1_tma_ok(const Layout& L, int order, bool ko, int which);
 cudaError_t launch_wave1(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
 cudaError_t kernel_info_wave1(int order, int tile, cudaFuncAttributes* a);
 cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);

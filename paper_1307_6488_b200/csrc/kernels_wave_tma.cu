@@ -13,17 +13,22 @@ namespace chm {
 
 namespace wv {
 
-template <int ORDER, bool KO, int TX, int TY>
+// NV = 2: the (phi, pi) system; NV = 5: the paper's Sample-1 system (u, rho, v_i), reading S1b
+template <int ORDER, bool KO, int TX, int TY, int NV = 2>
 struct Cfg {
   static constexpr int R0 = ORDER / 2, R = (KO && R0 < 3) ? 3 : R0;
   static constexpr int ROW = TX + 2 * R, COLS = TY + 2 * R;
   static constexpr int PB = ROW * COLS;                       // doubles per variable in one plane box
-  static constexpr int SLOT = (2 * PB + 15) / 16 * 16;        // both variables, 128-byte multiple
-  static constexpr uint32_t BYTES = 2u * PB * 8u;
-  static constexpr int PF = TX * TY == 512 && TX == 32 ? 5 : 3;   // planes in flight ahead of the one being evaluated
+  static constexpr int SLOT = (NV * PB + 15) / 16 * 16;       // all variables, 128-byte multiple
+  static constexpr uint32_t BYTES = (uint32_t)NV * PB * 8u;
+  static constexpr size_t smem_of(int pf) { return (size_t)(2 * R + 1 + pf) * SLOT * 8 + 2 * (2 * R + 1 + pf) * 8 + 128; }
+  // planes in flight ahead of the one being evaluated: as many as fit (five variables leave room for fewer)
+  static constexpr int PF0 = TX * TY == 512 && TX == 32 ? 5 : 3;
+  static constexpr int PF = NV == 2 ? PF0 : (smem_of(3) <= 227 * 1024 ? 3 : (smem_of(2) <= 227 * 1024 ? 2 : 1));
   static constexpr int NP = 2 * R + 1 + PF;                   // ring slots
   static constexpr int THREADS = TX * TY, NW = THREADS / 32;
-  static constexpr size_t SMEM = (size_t)NP * SLOT * 8 + 2 * NP * 8 + 128;
+  static constexpr size_t SMEM = smem_of(PF);
+  static constexpr bool FITS = SMEM <= 227 * 1024;
   static_assert(TX % 2 == 0, "TMA rows start on 16-byte boundaries");
 };
 
@@ -40,10 +45,10 @@ struct RingPoint {
 
 }  // namespace wv
 
-template <int ORDER, bool KO, int TX, int TY, int ZC>
+template <int ORDER, bool KO, int TX, int TY, int ZC, int NV>
 __global__ void __launch_bounds__(TX* TY, 1)
 wave_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage st, int ntx, int nty, int ntz) {
-  using K = wv::Cfg<ORDER, KO, TX, TY>;
+  using K = wv::Cfg<ORDER, KO, TX, TY, NV>;
   constexpr int R = K::R, ROW = K::ROW, PB = K::PB, SLOT = K::SLOT, NP = K::NP, PF = K::PF;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double* sm = reinterpret_cast<double*>(smem_raw);
@@ -89,12 +94,12 @@ wave_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
     const bool inxy = i < L.nx && j < L.ny;
     long q = (long)(k0 + L.g) * L.plane + (long)((inxy ? j : 0) + L.g) * L.pitch + ((inxy ? i : 0) + L.xo);
     // RK operands (U, S) of planes k, k+1, k+2 travel in registers: loaded two planes before they are used
-    StagePre pr[2], n1[2], n2[2];
-    stage_prefetch(st, q, pr[0]);
-    stage_prefetch(st, q + L.vstride, pr[1]);
+    StagePre pr[NV], n1[NV], n2[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) stage_prefetch(st, q + v * L.vstride, pr[v]);
     if (k0 + 1 < k1) {
-      stage_prefetch(st, q + L.plane, n1[0]);
-      stage_prefetch(st, q + L.plane + L.vstride, n1[1]);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) stage_prefetch(st, q + L.plane + v * L.vstride, n1[v]);
     }
     for (int k = k0; k < k1; ++k) {
       const int pc = (k - k0) + R;                                  // centre plane number inside the item
@@ -109,15 +114,28 @@ wave_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
 #pragma unroll
       for (int d = 0; d <= 2 * R; ++d) zp[d] = sm + ((nbase + pc - R + d) % NP) * SLOT + poff;
       if (k + 2 < k1) {
-        stage_prefetch(st, q + 2 * L.plane, n2[0]);
-        stage_prefetch(st, q + 2 * L.plane + L.vstride, n2[1]);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) stage_prefetch(st, q + 2 * L.plane + v * L.vstride, n2[v]);
       }
       wv::RingPoint<R> P{zp, ROW, PB};
-      double lap;
-      if (ORDER == 4) lap = (d2_o4(P, 0, 0, C.inv_h2) + d2_o4(P, 0, 1, C.inv_h2)) + d2_o4(P, 0, 2, C.inv_h2);
-      else lap = (d2_o8(P, 0, 0, C.inv_h2) + d2_o8(P, 0, 1, C.inv_h2)) + d2_o8(P, 0, 2, C.inv_h2);
-      double rphi = P.at(1, 0, 0, 0), rpi = lap;
-      if (KO) { rphi += ko5(P, 0, C.ko); rpi += ko5(P, 1, C.ko); }
+      double r[NV];
+      if constexpr (NV == 2) {
+        double lap;
+        if (ORDER == 4) lap = (d2_o4(P, 0, 0, C.inv_h2) + d2_o4(P, 0, 1, C.inv_h2)) + d2_o4(P, 0, 2, C.inv_h2);
+        else lap = (d2_o8(P, 0, 0, C.inv_h2) + d2_o8(P, 0, 1, C.inv_h2)) + d2_o8(P, 0, 2, C.inv_h2);
+        r[0] = P.at(1, 0, 0, 0);
+        r[1] = lap;
+      } else {   // D_t u = rho ; D_t rho = d_i v_i ; D_t v_i = d_i rho
+        auto d1 = [&](int v, int a) { return ORDER == 4 ? d1_o4(P, v, a, C.inv_h) : d1_o8(P, v, a, C.inv_h); };
+        r[0] = P.at(1, 0, 0, 0);
+        r[1] = (d1(2, 0) + d1(3, 1)) + d1(4, 2);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) r[2 + a] = d1(1, a);
+      }
+      if (KO) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) r[v] += ko5(P, v, C.ko);
+      }
       // the oldest plane (k - R) is not needed after this step: release it; the last warp out refills its slot
       __syncwarp();
       if (lane == 0) {
@@ -128,11 +146,11 @@ wave_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
         }
       }
       if (inxy) {
-        stage_emit(st, q, rphi, pr[0]);
-        stage_emit(st, q + L.vstride, rpi, pr[1]);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) stage_emit(st, q + v * L.vstride, r[v], pr[v]);
       }
-      pr[0] = n1[0]; pr[1] = n1[1];
-      n1[0] = n2[0]; n1[1] = n2[1];
+#pragma unroll
+      for (int v = 0; v < NV; ++v) { pr[v] = n1[v]; n1[v] = n2[v]; }
       q += L.plane;
     }
     // release the 2R planes of the item that were never "oldest" (its last planes), so the next item can reuse them
@@ -159,17 +177,19 @@ static WvEncodeFn wv_encode_fn() {
   return fn;
 }
 
-template <int ORDER, bool KO, int TX, int TY, int ZC>
+template <int ORDER, bool KO, int TX, int TY, int ZC, int NV = 2>
 static cudaError_t wv_go(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
-  using K = wv::Cfg<ORDER, KO, TX, TY>;
-  auto kern = wave_tma_kernel<ORDER, KO, TX, TY, ZC>;
+  using K = wv::Cfg<ORDER, KO, TX, TY, NV>;
+  if constexpr (!K::FITS) return cudaErrorInvalidConfiguration;   // ring does not fit: the caller falls back
+  else {
+  auto kern = wave_tma_kernel<ORDER, KO, TX, TY, ZC, NV>;
   if (a) return cudaFuncGetAttributes(a, kern);
   WvEncodeFn enc = wv_encode_fn();
   if (!enc) return cudaErrorNotSupported;
   CUtensorMap tm;
   cuuint64_t dims[4] = {(cuuint64_t)L.pitch, (cuuint64_t)L.tot_y, (cuuint64_t)L.tot_z, (cuuint64_t)L.nvars};
   cuuint64_t strides[3] = {(cuuint64_t)L.pitch * 8, (cuuint64_t)L.plane * 8, (cuuint64_t)L.vstride * 8};
-  cuuint32_t box[4] = {(cuuint32_t)K::ROW, (cuuint32_t)K::COLS, 1, 2};
+  cuuint32_t box[4] = {(cuuint32_t)K::ROW, (cuuint32_t)K::COLS, 1, (cuuint32_t)NV};
   cuuint32_t estr[4] = {1, 1, 1, 1};
   if (enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(st->in), dims, strides, box, estr,
           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -189,6 +209,7 @@ static cudaError_t wv_go(const Layout& L, const Coef& C, const Stage* st, cudaSt
   const int grid = nitems < sms ? nitems : sms;   // persistent, one CTA per SM
   kern<<<grid, dim3(TX, TY), K::SMEM, s>>>(tm, L, C, *st, ntx, nty, ntz);
   return cudaGetLastError();
+  }
 }
 
 // which: 0 = 32x16 threads, 32-plane chunks; 1 = 32x16, 64-plane chunks; 2 = 64x8, 32-plane chunks
@@ -201,6 +222,40 @@ static cudaError_t wv_tile(int which, const Layout& L, const Coef& C, const Stag
     case 2: return wv_go<ORDER, KO, 64, 8, 32>(L, C, st, s, a);
   }
   return cudaErrorInvalidValue;
+}
+
+// Sample-1 system (five variables): which: 0 = 16x8 threads, 1 = 16x16 (at 8th order with one plane of prefetch),
+// 2 = 32x8 (fits at 4th order only); 32-plane chunks
+template <int ORDER, bool KO>
+static cudaError_t wv1_tile(int which, const Layout& L, const Coef& C, const Stage* st, cudaStream_t s,
+                            cudaFuncAttributes* a) {
+  switch (which) {
+    case 0: return wv_go<ORDER, KO, 16, 8, 32, 5>(L, C, st, s, a);
+    case 1: return wv_go<ORDER, KO, 16, 16, 32, 5>(L, C, st, s, a);
+    case 2: return wv_go<ORDER, KO, 32, 8, 32, 5>(L, C, st, s, a);
+  }
+  return cudaErrorInvalidValue;
+}
+static cudaError_t wv1_dispatch(int order, bool ko, int which, const Layout& L, const Coef& C, const Stage* st,
+                                cudaStream_t s, cudaFuncAttributes* a) {
+  if (order == 4) return ko ? wv1_tile<4, true>(which, L, C, st, s, a) : wv1_tile<4, false>(which, L, C, st, s, a);
+  if (order == 8) return ko ? wv1_tile<8, true>(which, L, C, st, s, a) : wv1_tile<8, false>(which, L, C, st, s, a);
+  return cudaErrorInvalidValue;
+}
+// true when plane-ring variant `which` of the Sample-1 system exists for this order / dissipation (its ring fits
+// shared memory) and the layout suits TMA
+bool wave1_tma_ok(const Layout& L, int order, bool ko, int which) {
+  if (!wave_tma_ok(L, order, ko)) return false;
+  cudaFuncAttributes fa;
+  Layout L0{}; Coef C0{};
+  return wv1_dispatch(order, ko, which, L0, C0, nullptr, 0, &fa) == cudaSuccess;
+}
+cudaError_t launch_wave1_tma(const Layout& L, const Coef& C, int order, int which, const Stage& st, cudaStream_t s) {
+  return wv1_dispatch(order, C.ko != 0.0, which, L, C, &st, s, nullptr);
+}
+cudaError_t kernel_info_wave1_tma(int order, int which, cudaFuncAttributes* a) {
+  Layout L{}; Coef C{};
+  return wv1_dispatch(order, true, which, L, C, nullptr, 0, a);
 }
 
 // true when the TMA form can serve this layout: plane-box rows must start on 16-byte boundaries

@@ -140,9 +140,38 @@ def test_wave1_rhs_all_tiles(chem, oracle, order, g, eps, dims):
     want = oracle_rhs(oracle, 2, u, g, order, dx, eps_diss=eps)
     h = chem.Chemora(nx, ny, nz, g, order, chem.SYS_WAVE1, dx)
     h.set_param("eps_diss", eps)
-    for tile in range(6):
+    for tile in range(9):           # ids 6..8: the TMA plane-ring kernel (where its ring fits; else the L1 kernel)
         h.set_variant(1, tile)
         assert relerr(gpu_rhs(h, u), want) < TOL_RHS, tile
+    h.destroy()
+
+
+@pytest.mark.parametrize("order,g,eps", [(8, 4, 0.1), (4, 3, 0.1), (4, 2, 0.0)])
+def test_wave1_plane_ring_kernel_steps(chem, oracle, order, g, eps):
+    """ids 6..8 of the Sample-1 system: RK4 and RK3 over a grid with ragged tiles and two z chunks (nz > 32);
+    same stencil arithmetic as the L1-path kernel (agreement to rounding), and within tolerance of the oracle"""
+    nx, ny, nz = 37, 21, 45
+    u0 = np.random.default_rng(13).standard_normal((5, nz, ny, nx))
+    dx, steps = 1.0 / 32, 3
+    dt = 0.25 * dx
+    h = chem.Chemora(nx, ny, nz, g, order, chem.SYS_WAVE1, dx)
+    h.set_param("eps_diss", eps)
+    res = {}
+    for tile in (0, 6, 7, 8):
+        h.set_variant(1, tile)
+        h.set_state(u0)
+        for _ in range(steps):
+            h.rk4_step(dt)
+            h.rk3_step(dt)
+        res[tile] = h.get_state()
+    st = oracle.with_ghosts(u0, g)
+    for _ in range(steps):
+        st = oracle.rk4(2, st, g, order, dx, dt, oracle.params(eps_diss=eps), 1)
+        st = oracle.rk3(2, st, g, order, dx, dt, oracle.params(eps_diss=eps), 1)
+    want = oracle.interior(st, g)
+    for tile in (0, 6, 7, 8):
+        assert relerr(res[tile], want) < TOL_WAVE_PER_STEP * 2 * steps, tile
+        assert relerr(res[tile], res[0]) < 1e-13, tile
     h.destroy()
 
 
