@@ -168,9 +168,9 @@ int chemora_energy(chemora_t* h, const double* dev_state, double* dev_eps, doubl
  * 384-point tiles (12 warps per CTA at 168 registers, long-lived per-point values parked in tensor memory).
  * For the split BSSN kernels and the wave kernels a tile is an x*y thread block marching z planes; there an id
  * >= 6 repeats id - 6, except ids 6..8 of the wave systems: the TMA plane-ring kernel (CHEMORA_SYS_WAVE: 32x16x32,
- * 32x16x64, 64x8x32; CHEMORA_SYS_WAVE1, five variables a plane: 16x8x32, 16x16x32, 32x8x32; falls back to id - 6
+ * 32x16x64, 64x8x32; CHEMORA_SYS_WAVE1, five variables a plane: 16x8x64, 16x16x64, 32x8x64; falls back to id - 6
  * when the layout does not give 16-byte aligned plane boxes or the ring of planes does not fit shared memory,
- * as 32x8x32 at 8th order). */
+ * as 32x8x64 at 8th order). */
 int chemora_set_variant(chemora_t* h, int fused, int tile_id);
 int chemora_get_variant(const chemora_t* h, int* fused, int* tile_id);
 int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, int* tz);

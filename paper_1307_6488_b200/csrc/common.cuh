@@ -153,7 +153,7 @@ static const TileShape kTilesFused[11] = {{16, 4, 4}, {16, 8, 2}, {8, 8, 4}, {8,
 // wave system ids 6..8: the TMA plane-ring kernel (x, y = thread block, z = planes per work item)
 static const TileShape kTilesWaveTma[3] = {{32, 16, 32}, {32, 16, 64}, {64, 8, 32}};
 // Sample-1 system ids 6..8: the same plane-ring kernel with five variables (smaller tiles: the ring holds 5 boxes a plane)
-static const TileShape kTilesWave1Tma[3] = {{16, 8, 32}, {16, 16, 32}, {32, 8, 32}};
+static const TileShape kTilesWave1Tma[3] = {{16, 8, 64}, {16, 16, 64}, {32, 8, 64}};
 static const TileShape kTilesMarch[6] = {{32, 4, 8}, {32, 8, 8}, {64, 2, 8}, {64, 4, 8}, {128, 2, 8}, {16, 16, 8}};
 
 // launchers implemented in the kernel translation units; each returns the cudaError_t of the launch

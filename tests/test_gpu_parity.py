@@ -148,9 +148,9 @@ def test_wave1_rhs_all_tiles(chem, oracle, order, g, eps, dims):
 
 @pytest.mark.parametrize("order,g,eps", [(8, 4, 0.1), (4, 3, 0.1), (4, 2, 0.0)])
 def test_wave1_plane_ring_kernel_steps(chem, oracle, order, g, eps):
-    """ids 6..8 of the Sample-1 system: RK4 and RK3 over a grid with ragged tiles and two z chunks (nz > 32);
+    """ids 6..8 of the Sample-1 system: RK4 and RK3 over a grid with ragged tiles and two z chunks (nz > 64);
     same stencil arithmetic as the L1-path kernel (agreement to rounding), and within tolerance of the oracle"""
-    nx, ny, nz = 37, 21, 45
+    nx, ny, nz = 37, 21, 75
     u0 = np.random.default_rng(13).standard_normal((5, nz, ny, nx))
     dx, steps = 1.0 / 32, 3
     dt = 0.25 * dx
