@@ -170,6 +170,16 @@ struct BoxPoint {
   }
 };
 
+// Star-shaped staging (sections that need only the three axis stencils: first derivatives, advection, dissipation):
+// three slab boxes instead of the cuboid -- the tile + x-halo, the tile + y-halo, the tile + z-halo -- each a pointer
+// to this thread's own point in it; SY, SZ are the y- and z-strides of the y- and z-slab (rows of TX + 2).
+template <int SY, int SZ>
+struct StarPoint {
+  const double *cx, *cy, *cz;
+  __device__ __forceinline__ double at(int, int, int) const { return cx[0]; }   // only ever the point itself
+  __device__ __forceinline__ double ax(int a, int m) const { return a == 0 ? cx[m] : (a == 1 ? cy[m * SY] : cz[m * SZ]); }
+};
+
 // Per-point upwind/dissipation weights: beta^a d^up_a u + KO(u) = sum_a  wq[a] * q_a(u) + ws[a] * sp_a(u)
 //   q_a  = s3 - 6 s2 + 15 s1   (s_k = (u[+k]-u0) + (u[-k]-u0))      symmetric 7-point (the KO stencil)
 //   sp_a = 21 e1 - 6 e2 + e3   (e_k = u[+k] - u[-k])                 antisymmetric 7-point

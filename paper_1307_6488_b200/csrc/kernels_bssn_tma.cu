@@ -32,6 +32,13 @@
 #ifndef CHM_ATLOOP
 #define CHM_ATLOOP 1   // 4th order too: the At_ij sections as one loop body (6.29 -> 6.19 ms per launch at 256^3)
 #endif
+#ifndef CHM_STAR
+#define CHM_STAR 0     // advection / first-derivative-only sections (Gt^i, K, At_ij, B^i, A) stage a 3-D star (three slab
+#endif                 // boxes: tile + x-halo, + y-halo, + z-halo) instead of the cuboid: 1792 instead of 2200 doubles out
+                       // of L2 per section at 4th order, 2432 instead of 5096 at 8th.  Bit-identical; measured SLOWER
+                       // (256^3, ms per launch: 16x4x4 6.09 -> 6.64, 16x2x8 6.12 -> 6.62; 8th order 100^3 RK3 step
+                       // 2.12 -> 2.56): the slabs have as many rows (96 vs 100) as the cuboid and three TMA
+                       // instructions per refill instead of one -- the box fill is bound by rows, not bytes.  Off.
 #ifndef CHM_L2HINT
 #define CHM_L2HINT 1
 #endif
@@ -75,13 +82,21 @@ struct TmaCfg {
   static constexpr int DB = TWOPASS ? (DY_N + DZ_N + 15) / 16 * 16 : 0;
   static constexpr size_t SMEM = (size_t)(NS * SLOTX + CEN + 2 * DB) * 8 + (NS + 1) * 8 + (NS + 1) * 8 + 64 + 16 + 64 + 128;
   static constexpr int NWARPS = THREADS / 32;
+  // star staging: x-slab (BX,TY,TZ), y-slab (TX+2,BY,TZ), z-slab (TX+2,TY,BZ), back to back inside the slot
+  // (only on the tile shapes whose slabs keep every box 128-byte aligned in the slot)
+  static constexpr int SX_N = BX * TY * TZ, SY_N = (TX + 2) * BY * TZ, SZ_N = (TX + 2) * TY * BZ;
+  static constexpr bool STAR = CHM_STAR && !HEAVY && SX_N % 16 == 0 && SY_N % 16 == 0 && SX_N + SY_N + SZ_N <= SLOT;
+  static constexpr uint32_t STAR_BYTES = (uint32_t)(SX_N + SY_N + SZ_N) * 8u;
 };
+// sections (consumption order) that read only axis stencils: Gt^i 9..11, K 14, At_ij 15..20, B^i 21..23, A 24
+__device__ __forceinline__ constexpr bool star_section(int o) { return (o >= 9 && o <= 11) || o >= 14; }
 
 template <int TX, int TY, int TZ, int MODE, int ORDER>
 __global__ void __launch_bounds__(TX* TY* TZ, 1)
 bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ CUtensorMap tmCen,
-                const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS, Layout L, Coef C,
-                Stage st, int ntx, int nty, int ntz, int cy) {
+                const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS,
+                const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmY,
+                const __grid_constant__ CUtensorMap tmZ, Layout L, Coef C, Stage st, int ntx, int nty, int ntz, int cy) {
   using Cfg = TmaCfg<TX, TY, TZ, ORDER>;
   constexpr int H = Cfg::H;
   constexpr int BX = Cfg::BX, BY = Cfg::BY, SLOT = Cfg::SLOT, SLOTX = Cfg::SLOTX, TILE = Cfg::TILE, CEN = Cfg::CEN;
@@ -166,8 +181,15 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     double* dst = sm + slot * SLOTX;
     const int v0 = emit_var(o, 0), v1 = emit_var(o, 1);
     const int nem = (v0 >= 0) + (v1 >= 0);
-    mbar_expect_tx(&full[slot], Cfg::BOX_BYTES + (uint32_t)(nops * nem) * Cfg::TILE_BYTES);
-    tma_load_4d(dst, &tm, &full[slot], x0, y0, z0, order_var(o));
+    const bool star = Cfg::STAR && star_section(o);
+    mbar_expect_tx(&full[slot], (star ? Cfg::STAR_BYTES : Cfg::BOX_BYTES) + (uint32_t)(nops * nem) * Cfg::TILE_BYTES);
+    if (star) {
+      tma_load_4d(dst, &tmX, &full[slot], x0, y0 + H, z0 + H, order_var(o));
+      tma_load_4d(dst + Cfg::SX_N, &tmY, &full[slot], x0 + H - 1, y0, z0 + H, order_var(o));
+      tma_load_4d(dst + Cfg::SX_N + Cfg::SY_N, &tmZ, &full[slot], x0 + H - 1, y0 + H, z0, order_var(o));
+    } else {
+      tma_load_4d(dst, &tm, &full[slot], x0, y0, z0, order_var(o));
+    }
     if (v0 >= 0 && nops >= 1) tma_load_4d_hint(dst + SLOT, &tmU, &full[slot], x0 + H - 1, y0 + H, z0 + H, v0, pol_stream);
     if (v0 >= 0 && nops == 2) tma_load_4d_hint(dst + SLOT + TILE, &tmS, &full[slot], x0 + H - 1, y0 + H, z0 + H, v0, pol_stream);
     if (v1 >= 0 && nops >= 1) tma_load_4d_hint(dst + SLOT + 2 * TILE, &tmU, &full[slot], x0 + H - 1, y0 + H, z0 + H, v1, pol_stream);
@@ -243,6 +265,18 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     auto box = [&](int o) {
       mbar_wait(&full[slot_of(o)], parity_of(o));
       return BoxPoint<BX, BY>{sm + slot_of(o) * SLOTX + coff};
+    };
+    // the same for a star section: pointers to the point in the x-, y- and z-slab
+    auto sbox = [&](int o) {
+      if constexpr (Cfg::STAR) {
+        mbar_wait(&full[slot_of(o)], parity_of(o));
+        const double* b = sm + slot_of(o) * SLOTX;
+        return StarPoint<TX + 2, (TX + 2) * TY>{b + (lz * TY + ly) * BX + lx + H,
+                                                b + Cfg::SX_N + (lz * BY + ly + H) * (TX + 2) + lx + 1,
+                                                b + Cfg::SX_N + Cfg::SY_N + ((lz + H) * TY + ly) * (TX + 2) + lx + 1};
+      } else {
+        return box(o);
+      }
     };
     auto done = [&](int o) {
       if (leave(slot_of(o))) {   // the refill is load number 25 t + o + kSlots: same slot
@@ -642,7 +676,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     if constexpr (LOOPS & 4) {
 #pragma unroll 1
       for (int k2 = 0; k2 < 3; ++k2) {
-        auto p = box(9 + k2);
+        auto p = sbox(9 + k2);
         double d4[4];
         if (ORDER == 4) var_d1_ad(p, C, w, d4, d4[3]); else var_d1_ad8(p, C, w, d4, d4[3]);
         done(9 + k2);
@@ -662,7 +696,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     } else
 #pragma unroll
     for (int k2 = 0; k2 < 3; ++k2) {
-      auto p = box(9 + k2);
+      auto p = sbox(9 + k2);
       double d1[3];
       if (ORDER == 4) var_d1_ad(p, C, w, d1, adG[k2]); else var_d1_ad8(p, C, w, d1, adG[k2]);
       done(9 + k2);
@@ -768,7 +802,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     // ---- o = 14: K -------------------------------------------------------------------------------------------
     double dK[3];
     {
-      auto p = box(14);
+      auto p = sbox(14);
       const StagePre pr = pre(14, 0);
       double ad;
       if (ORDER == 4) var_d1_ad(p, C, w, dK, ad); else var_d1_ad8(p, C, w, dK, ad);
@@ -822,7 +856,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
         }
 #pragma unroll 1
       for (int s = 0; s < 6; ++s) {
-        auto p = box(15 + s);
+        auto p = sbox(15 + s);
         const StagePre pr = pre(15 + s, 0);
         const double ad = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
         const double rest = *tab(s);
@@ -836,7 +870,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 #pragma unroll
         for (int j2 = i2; j2 < 3; ++j2) {
           const int s = sym(i2, j2);
-          auto p = box(15 + s);
+          auto p = sbox(15 + s);
           const StagePre pr = pre(15 + s, 0);
           const double ad = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
           done(15 + s);
@@ -887,7 +921,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       }
 #pragma unroll 1
       for (int i2 = 0; i2 < 3; ++i2) {
-        auto p = box(21 + i2);
+        auto p = sbox(21 + i2);
         const StagePre prG = pre(21 + i2, 0), prB = pre(21 + i2, 1);
         const double Bi = p.at(0, 0, 0);
         const double adB = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
@@ -900,7 +934,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     } else
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2) {
-      auto p = box(21 + i2);
+      auto p = sbox(21 + i2);
       const StagePre prG = pre(21 + i2, 0), prB = pre(21 + i2, 1);
       const double Bi = p.at(0, 0, 0);
       const double adB = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
@@ -921,7 +955,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 
     // ---- o = 24: A (inert slot, dissipation only) -----------------------------------------------------------------
     {
-      auto p = box(24);
+      auto p = sbox(24);
       const StagePre pr = pre(24, 0);
       const double f0 = p.at(0, 0, 0);
       double rA;
@@ -984,6 +1018,18 @@ static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, 
   if (tile_map(&tmCen, st->in, 7) != CUDA_SUCCESS || tile_map(&tmU, ubase, 1) != CUDA_SUCCESS ||
       tile_map(&tmS, sbase, 1) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
+  CUtensorMap tmX = tm, tmY = tm, tmZ = tm;   // star staging: the three slab boxes of the evaluated state
+  if (Cfg::STAR) {
+    auto slab_map = [&](CUtensorMap* m, int bx, int by, int bz) {
+      cuuint32_t b[4] = {(cuuint32_t)bx, (cuuint32_t)by, (cuuint32_t)bz, 1};
+      return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(st->in), dims, strides, b, estr,
+                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    };
+    if (slab_map(&tmX, Cfg::BX, TY, TZ) != CUDA_SUCCESS || slab_map(&tmY, TX + 2, Cfg::BY, TZ) != CUDA_SUCCESS ||
+        slab_map(&tmZ, TX + 2, TY, Cfg::BZ) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+  }
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
@@ -1000,7 +1046,7 @@ static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, 
   if (blocks_per_sm < 1) blocks_per_sm = 1;
   const int grid = ntiles < sms * blocks_per_sm ? ntiles : sms * blocks_per_sm;
   const int cy = L.col_rows / TY > 0 ? L.col_rows / TY : 1;   // tile rows per traversal column
-  kern<<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, L, C, *st, ntx, nty, ntz, cy);
+  kern<<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, tmX, tmY, tmZ, L, C, *st, ntx, nty, ntz, cy);
   return cudaGetLastError();
 }
 
