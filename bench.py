@@ -243,7 +243,7 @@ def run_ours(args):
                    "variant": {"fused": fused, "tile": list(binding.tile_shape(tile, binding.SYS_BSSN, fused)), "sweep_ms": sweep_ms},
                    "kernel": info, "multi_gpu": "replicas only",
                    "l2": "inputs larger than L2 (%.2f GB per state buffer vs 126 MB)" % (h.nvars * h.var_stride * 8 / 1e9)},
-        "roofline": {"bound": "hbm", "kernel": ("bssn_ws_kernel" if tile >= 6 else "bssn_tma_kernel") if fused else "bssn_derivs+from_derivs",
+        "roofline": {"bound": "hbm", "kernel": ("bssn_ws_kernel" if 6 <= tile <= 8 else "bssn_tma_kernel") if fused else "bssn_derivs+from_derivs",
                      "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
                      "traffic": NCU_TRAFFIC_BYTES_256 if (fused and tile < 6 and n == 256) else None, "traffic_unit": "bytes per launch (ncu)",
                      "algorithmic_bytes_per_launch": BYTES_PER_POINT_PER_LAUNCH * n ** 3, "peak_source": pk_src, "ms_per_launch": rhs_launch_ms,
