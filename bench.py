@@ -23,19 +23,25 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-METRIC = "BSSN RHS+RK4 grid-point updates/sec, fp64 4th-order 256^3"
+METRIC = "BSSN RHS+RK4 grid-point updates/sec, fp64 4th-order 256^3; % HBM/FP64 roofline"   # BASELINE.json, byte for byte
 UNIT = "grid-point updates/s"
 # algorithmic HBM traffic of the fused 4-buffer RK4 scheme (reading S9), V = 25:
 # stage 1 reads U, writes S,Yb (75 doubles); stages 2-3 read Y,U,S write S,Y' (125 each); stage 4 reads
 # Y,S,U writes U (100): 425 doubles = 3400 B per grid-point update, i.e. 850 B per RHS-kernel launch and point.
 BYTES_PER_UPDATE = 3400.0
 BYTES_PER_POINT_PER_LAUNCH = BYTES_PER_UPDATE / 4.0
-# FP64 work the fused kernel executes per point and RHS evaluation: 1365 DADD + 671 DMUL + 2 x 1026 DFMA (SASS of the
-# middle-stage instance of the default tile).  An upper bound on the paper's convention.
+# CONSTANTS from earlier captures, printed as such (never measured by this script):
+# FP64 work the fused kernel executes per point and RHS evaluation: 1365 DADD + 671 DMUL + 2 x 1026 DFMA thread
+# instructions (SASS of the middle-stage 16x4x4 instance, static count + 5 more trips of the At_ij loop;
+# tests/test_abi.py::test_flop_counts_of_the_fused_kernels re-counts it from the built library).  An upper bound on the
+# paper's convention.
 FLOPS_PER_RHS_POINT = 4088.0
-# dram__bytes_read.sum + dram__bytes_write.sum of the fused kernel at 256^3, mean over the 4 launches of an RK4 step
-# (ncu --set full, profiles/r01_j_fused_ncu_full.md; capture D had 18.25e9); None for other variants / sizes
+FLOPS_SOURCE = "constant: SASS count of bssn_tma_kernel<16,4,4,MODE_MID,4>, DESIGN.md section 6 / tests/test_abi.py"
+# dram__bytes_read.sum + dram__bytes_write.sum of the fused kernel at 256^3, mean over the 4 launches of an RK4 step,
+# from the one ncu --set full capture named here; reported under "traffic_constant", "traffic" itself stays null
+# because this script does not run under ncu.
 NCU_TRAFFIC_BYTES_256 = 19.60e9
+NCU_TRAFFIC_SOURCE = "profiles/r01_j_fused_ncu_full.md"
 
 
 def peaks():
@@ -243,13 +249,18 @@ def run_ours(args):
                    "variant": {"fused": fused, "tile": list(binding.tile_shape(tile, binding.SYS_BSSN, fused)), "sweep_ms": sweep_ms},
                    "kernel": info, "multi_gpu": "replicas only",
                    "l2": "inputs larger than L2 (%.2f GB per state buffer vs 126 MB)" % (h.nvars * h.var_stride * 8 / 1e9)},
-        "roofline": {"bound": "hbm", "kernel": ("bssn_ws_kernel" if 6 <= tile <= 8 else "bssn_tma_kernel") if fused else "bssn_derivs+from_derivs",
+        "roofline": {"bound": "hbm", "kernel": "bssn_tma_kernel" if fused else "bssn_derivs+from_derivs",
                      "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
-                     "traffic": NCU_TRAFFIC_BYTES_256 if (fused and tile < 6 and n == 256) else None, "traffic_unit": "bytes per launch (ncu)",
+                     "traffic": None,
+                     "traffic_constant": {"bytes_per_launch": NCU_TRAFFIC_BYTES_256, "source": NCU_TRAFFIC_SOURCE}
+                                         if (fused and n == 256) else None,
                      "algorithmic_bytes_per_launch": BYTES_PER_POINT_PER_LAUNCH * n ** 3, "peak_source": pk_src, "ms_per_launch": rhs_launch_ms,
+                     # the whole step (4 fills + 4 launches, the driver-timed number) against the same roof
+                     "step_frac": BYTES_PER_UPDATE * n ** 3 / (ms / args.steps * 1e-3) / 1e9 / hbm_peak,
                      "share_of_step": kt["rhs_ms"] / ms, "fill_share_of_step": kt["fill_ms"] / ms},
         "roofline_fp64": {"bound": "alu", "achieved": gf, "peak": fp64_gf, "unit": "GFLOP/s",
                           "frac": gf / fp64_gf if fp64_gf else None, "flops_per_rhs_point": FLOPS_PER_RHS_POINT,
+                          "flops_source": FLOPS_SOURCE,
                           "peak_source": "measured in this run: DFMA chains on all SMs (chemora_measure_fp64_peak)"},
         "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle",
                          "sample": "3 RK4 steps of the configs[3] recipe on a %d^3 periodic block (%.1f s)" % (
@@ -274,11 +285,12 @@ def run_sweep(args):
         h = binding.Chemora(nx, ny, nz, 3, 4, binding.SYS_BSSN, 0.05)
         h.set_param("eps_diss", 0.1)
         h.set_state(inputs.bssn_noise(nx, ny, nz))
+        h.set_param("autotune_split", 1)        # configs[4] asks for both variants
         fused, tile, ms = h.autotune()
         for f in (1, 0):
-            for t in range(binding.NUM_TILES):
+            for t in binding.variants(binding.SYS_BSSN, 4, f):
                 m = ms[f * binding.NUM_TILES + t]
-                if m <= 0 or (f == 0 and t >= 6):
+                if m <= 0:
                     continue
                 h.set_variant(f, t)
                 info = h.kernel_info()
@@ -289,7 +301,7 @@ def run_sweep(args):
                               "updates_per_s": npts / (4 * m * 1e-3), "regs": info["regs"],
                               "spill_bytes": info["local_bytes"], "hbm_gbs_algorithmic": bytes_pt * npts / (m * 1e-3) / 1e9,
                               "best": (f, t) == (fused, tile)})
-                if f == 1 and not 6 <= t < 9:     # the paper's tile cost model next to the measurement
+                if f == 1:     # the paper's tile cost model next to the measurement
                     table[-1]["sigma_model"] = binding.tile_cost(4, 3, t)[0]
         h.destroy()
         rows = [r for r in table if r["grid"] == [nx, ny, nz] and "sigma_model" in r]

@@ -48,7 +48,7 @@ enum { CHEMORA_SYS_WAVE = 0, CHEMORA_SYS_BSSN = 1, CHEMORA_SYS_WAVE1 = 2 };
 enum { CHEMORA_BUF_U = 0, CHEMORA_BUF_YA = 1, CHEMORA_BUF_YB = 2, CHEMORA_BUF_S = 3 };
 
 /* kernel variant axes (PAPER.md:215-216 fused vs derivative-split; :248-266 tile shape) */
-enum { CHEMORA_NUM_TILES = 11 };
+enum { CHEMORA_NUM_TILES = 9 };
 
 /* Create a handle for an nx x ny x nz interior block with `ghost` ghost layers per face, centred FD order
  * fd_order (4 or 8), system system_id and grid spacing dx (same in x, y, z).
@@ -69,15 +69,13 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
  * (default 0.75), "ko_order" (5, the default, or 9: the 11-point operator (eps/1024h) h^10 (D+D-)^5 that goes
  * with the paper's 8th-order, 5-ghost-zone configuration; accepted for the 8th-order BSSN
  * system only); tuning: "col_rows" (default 32: y-extent in grid rows of the columns in which the fused BSSN
- * kernel visits its tiles, chosen so the halo planes shared by z-neighbour tiles stay in L2), "x_images" (default 0;
- * 1: inside chemora_rk4_step / chemora_rk3_step the fused BSSN kernel also writes the x-ghost images of the stage
- * states it produces, and the ghost fill of those states leaves the x-ghost columns of the interior rows out;
- * results are bit-identical either way; measured no net gain at 256^3).
+ * kernel visits its tiles, chosen so the halo planes shared by z-neighbour tiles stay in L2), "autotune_split"
+ * (default 0; 1: chemora_autotune also times the derivative-split variant, which allocates its derivative scratch).
  * Unknown name or invalid value -> CHEMORA_EINVAL. */
 int chemora_set_param(chemora_t* h, const char* name, double value);
 
 /* The paper's tile cost model re-targeted at this design, for the uniform fused BSSN kernel
- * (fused tile ids 0..5, 9, 10; 8th order: id 0).  Host arithmetic only, no device needed.
+ * (fused tile ids 0..4; 8th order: id 0).  Host arithmetic only, no device needed.
  *   requests r = the 32-byte L2 sectors one interior tile of a middle RK4 stage requests: the (tx+2H)(ty+2H)(tz+2H)
  *     halo boxes of the 25 variables (H = fd_order/2 + 1), the point-value and Runge-Kutta operand boxes
  *     ((tx+2) x ty x tz, 21 + 2*25 of them) and the 2*25 stored tiles, every row counted with its alignment in
@@ -149,7 +147,10 @@ int chemora_rk4_step_group(chemora_t* const* blocks, int n, double dt);
 int chemora_rk3_step_group(chemora_t* const* blocks, int n, double dt);
 
 /* Algebraic constraint enforcement on the interior of a BSSN state in the padded layout (dev_state == NULL: U):
- * gt_ij <- gt_ij / det(gt)^(1/3), At_ij <- At_ij - 1/3 gt_ij gtu^kl At_kl (reading S10b).  In place, asynchronous.
+ * gt_ij <- gt_ij + gt_ij (det(gt)^(-1/3) - 1), the bracket evaluated as expm1(-log(det)/3) and det in a fixed
+ * association without FMA contraction (reading S10b: mathematically gt_ij / det^(1/3); this form rounds the O(1)
+ * values identically in any implementation), then At_ij <- At_ij - 1/3 gt_ij gtu^kl At_kl with the new metric.
+ * In place, asynchronous.
  * CHEMORA_EINVAL for the wave systems. */
 int chemora_enforce_constraints(chemora_t* h, double* dev_state);
 
@@ -161,26 +162,42 @@ int chemora_energy(chemora_t* h, const double* dev_state, double* dev_eps, doubl
 
 /* Kernel variant: fused (1: derivatives + RHS + RK stage update in one kernel) or split (0: derivatives
  * written to global arrays by one kernel, RHS + stage update by a second), and tile_id in
- * [0, CHEMORA_NUM_TILES).  chemora_tile_shape reports the (x, y, z) extent of a tile id: for the fused BSSN
- * kernel a 3-D tile with one grid point per thread (staged with a 3-cell halo by TMA); ids 0..5 are six
- * shapes of the uniform kernel (every warp does the same work), ids 6..8 the warp-specialised kernel
- * (8 point warps + 4 stencil warps per CTA) on the shapes of ids 0, 1 and 4, ids 9..10 the uniform kernel on
- * 384-point tiles (12 warps per CTA at 168 registers, long-lived per-point values parked in tensor memory).
- * For the split BSSN kernels and the wave kernels a tile is an x*y thread block marching z planes; there an id
- * >= 6 repeats id - 6, except ids 6..8 of the wave systems: the TMA plane-ring kernel (CHEMORA_SYS_WAVE: 32x16x32,
- * 32x16x64, 64x8x32; CHEMORA_SYS_WAVE1, five variables a plane: 16x8x64, 16x16x64, 32x8x64; falls back to id - 6
+ * [0, CHEMORA_NUM_TILES); chemora_variant_available says (host only, 1/0) which ids exist for a system and order.
+ * chemora_tile_shape reports the (x, y, z) extent of a tile id.  Fused BSSN kernel: a 3-D tile with one grid point
+ * per thread, staged with an (order/2 + 1)-cell halo by TMA; ids 0..4 = 16x4x4, 16x8x2, 8x4x8, 16x2x8, 16x4x2 at 4th
+ * order, id 0 only at 8th order.  Split BSSN kernels (ids 0..5) and the L1-path wave kernels (ids 0..5): an x*y thread
+ * block marching z planes.  Ids 6..8 of the wave systems: the TMA plane-ring kernel (CHEMORA_SYS_WAVE: 32x16x32,
+ * 32x16x64, 64x8x32; CHEMORA_SYS_WAVE1, five variables a plane: 16x8x64, 16x16x64, 32x8x64; runs id - 6 instead
  * when the layout does not give 16-byte aligned plane boxes or the ring of planes does not fit shared memory,
- * as 32x8x64 at 8th order). */
+ * as 32x8x64 at 8th order).  chemora_set_variant returns CHEMORA_EINVAL for an id that does not exist. */
 int chemora_set_variant(chemora_t* h, int fused, int tile_id);
 int chemora_get_variant(const chemora_t* h, int* fused, int* tile_id);
+int chemora_variant_available(int system_id, int fd_order, int fused, int tile_id);
 int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, int* tz);
 
-/* Runtime sweep (the paper's model-based choice, replaced by measurement): times every
- * (fused, tile) once on the handle's own grid (one middle RK4 stage evaluated on the current U, results
- * into the scratch buffers S and Ya), keeps the fastest, returns it.
+/* Runtime sweep (the paper's model-based choice, replaced by measurement): times every available
+ * fused tile id (and, with the parameter "autotune_split" = 1, the six split tiles) on the handle's own grid -- one
+ * middle RK4 stage evaluated on the current U, results into the scratch buffers S and Ya; one warm-up run, then the
+ * median of three timed runs -- keeps the fastest, returns it.  A variant that cannot run here (CHEMORA_ENOMEM for
+ * its scratch, CHEMORA_EINVAL from its launch check) is skipped, not fatal.
  * ms_out, if not NULL, receives 2*CHEMORA_NUM_TILES timings in milliseconds ([fused*NUM_TILES + tile];
- * negative = variant unavailable).  U is not modified.  Synchronous. */
+ * negative = variant unavailable or not timed).  U is not modified.  Synchronous. */
 int chemora_autotune(chemora_t* h, int* fused, int* tile_id, float* ms_out);
+
+/* Launch safety (the paper's run-time path that edits, compiles and loads kernels is its failure surface,
+ * PAPER.md:246; here the equivalent is a TMA launch with a bad box or byte count).
+ * chemora_selfcheck: host only, no device: builds the launch plan (shared-memory destinations, box extents, x-coordinate
+ * parity, mbarrier byte counts, shared-memory total, threads) of EVERY TMA kernel instance in the library for every
+ * ghost width and Runge-Kutta mode and validates it with the same checker every launcher runs before <<<>>>.
+ * Returns the number of plans checked (> 0), or CHEMORA_EINVAL if one is rejected; buf (may be NULL) gets a one-line
+ * report.  A launch whose plan or layout is rejected is never issued: the call returns CHEMORA_ECUDA and
+ * chemora_last_error names the rule.
+ * Device error word: every wait on a TMA mbarrier inside the kernels is bounded (seconds); a wait that gives up records
+ * a code in the handle's device error word and the kernel runs on without the data (memory-safe: no address depends on
+ * loaded values).  chemora_synchronize (and chemora_get_state) read the word: non-zero -> CHEMORA_ECUDA, the message
+ * from chemora_describe_device_error(code) (host only), and the word is cleared. */
+int chemora_selfcheck(char* buf, size_t n);
+int chemora_describe_device_error(unsigned code, char* buf, size_t n);
 
 /* Number of kernel launches issued through this handle so far (for benchmarks' gpu_launches). */
 long chemora_launch_count(const chemora_t* h);

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libchemora.so")
 
 SYS_WAVE, SYS_BSSN, SYS_WAVE1 = 0, 1, 2
 BUF_U, BUF_YA, BUF_YB, BUF_S = 0, 1, 2, 3
-NUM_TILES = 11
+NUM_TILES = 9
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 
 # every symbol include/chemora.h declares (tests check that the library exports all of them)
@@ -24,7 +24,7 @@ SYMBOLS = ["chemora_create", "chemora_set_param", "chemora_get_param", "chemora_
            "chemora_synchronize", "chemora_set_state_dev", "chemora_get_state_dev",
            "chemora_fill_ghosts", "chemora_rhs", "chemora_rk4_step", "chemora_rk3_step", "chemora_link_z",
            "chemora_rk4_step_group", "chemora_rk3_step_group", "chemora_enforce_constraints", "chemora_energy", "chemora_set_variant",
-           "chemora_get_variant", "chemora_tile_shape", "chemora_tile_cost", "chemora_autotune", "chemora_launch_count",
+           "chemora_get_variant", "chemora_variant_available", "chemora_selfcheck", "chemora_describe_device_error", "chemora_tile_shape", "chemora_tile_cost", "chemora_autotune", "chemora_launch_count",
            "chemora_kernel_info", "chemora_timing", "chemora_timing_read", "chemora_measure_fp64_peak", "chemora_last_error", "chemora_destroy"]
 
 _ALLOC_T = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
@@ -69,6 +69,9 @@ def load():
         "chemora_energy": [vp, vp, vp, dp],
         "chemora_set_variant": [vp, i, i], "chemora_get_variant": [vp, ip, ip],
         "chemora_tile_shape": [i, i, i, ip, ip, ip],
+        "chemora_variant_available": [i, i, i, i],
+        "chemora_selfcheck": [ctypes.c_char_p, ctypes.c_size_t],
+        "chemora_describe_device_error": [ctypes.c_uint, ctypes.c_char_p, ctypes.c_size_t],
         "chemora_autotune": [vp, ip, ip, ctypes.POINTER(ctypes.c_float)],
         "chemora_launch_count": [vp],
         "chemora_kernel_info": [vp, ip, ip, ip],
@@ -92,6 +95,32 @@ def tile_shape(tile_id, system_id=SYS_BSSN, fused=1):
     if rc:
         raise ChemoraError(rc)
     return a.value, b.value, c.value
+
+
+def variant_available(system_id, fd_order, fused, tile_id):
+    return bool(load().chemora_variant_available(system_id, fd_order, fused, tile_id))
+
+
+def variants(system_id, fd_order, fused=1):
+    """the tile ids that exist for a system, order and variant axis"""
+    return [t for t in range(NUM_TILES) if variant_available(system_id, fd_order, fused, t)]
+
+
+def selfcheck():
+    """(number of launch plans checked, report line); raises if the validator rejects one.  Host only."""
+    buf = ctypes.create_string_buffer(512)
+    rc = load().chemora_selfcheck(buf, len(buf))
+    if rc <= 0:
+        raise ChemoraError(rc, buf.value.decode())
+    return rc, buf.value.decode()
+
+
+def describe_device_error(code):
+    buf = ctypes.create_string_buffer(256)
+    rc = load().chemora_describe_device_error(code, buf, len(buf))
+    if rc:
+        raise ChemoraError(rc)
+    return buf.value.decode()
 
 
 def step_group(blocks, dt, rk3=False):

@@ -23,16 +23,35 @@ __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+__device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
   asm volatile(
       "{\n"
       ".reg .pred p;\n"
-      "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE_%=;\n"
-      "bra WAIT_%=;\n"
-      "DONE_%=:\n"
-      "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
+// Bounded wait.  A wrong expect_tx byte count, a TMA load that never lands or a refill that is never issued must
+// end as an error code, not as a hung device: after kWaitBudget clock cycles (seconds; a whole launch takes
+// milliseconds) the waiter records `code` in the handle's device error word and carries on WITHOUT the data --
+// every address these kernels form depends on the tile index only, never on loaded values, so running on is
+// memory-safe; the results are garbage and chemora_synchronize reports CHEMORA_ECUDA.  Once the word is set,
+// every later wait of the launch gives up after its first 256 polls.
+constexpr long long kWaitBudget = 4000000000LL;
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, unsigned* err, unsigned code) {
+  const uint32_t b = smem_u32(bar);
+  if (mbar_try(b, parity)) return;
+  const long long t0 = clock64();
+#pragma unroll 1
+  for (unsigned it = 1;; ++it) {
+    if (mbar_try(b, parity)) return;
+    if ((it & 255u) == 0u) {
+      if (*reinterpret_cast<volatile unsigned*>(err) != 0u) return;
+      if (clock64() - t0 > kWaitBudget) { atomicCAS(err, 0u, code); return; }
+    }
+  }
 }
 __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, uint64_t* bar, int x, int y, int z,
                                             int v) {
@@ -350,7 +369,7 @@ __device__ __forceinline__ double var_ad8(const P& p, const Coef& C, const AdvW&
 }
 
 // consumption order of the 25 variables (slot of order index o is o % 5)
-__device__ __forceinline__ constexpr int order_var(int o) {
+__host__ __device__ __forceinline__ constexpr int order_var(int o) {
   return o < 3 ? V_BETA + o : o < 9 ? V_GT + (o - 3) : o < 12 ? V_GAM + (o - 9) : o == 12 ? V_CHI : o == 13 ? V_ALPHA
          : o == 14 ? V_K : o < 21 ? V_AT + (o - 15) : o < 24 ? V_B + (o - 21) : V_A;
 }

@@ -3,6 +3,7 @@
 // every compute entry point enqueues CUDA kernels and reports CHEMORA_ECUDA if that fails.
 #include "../../include/chemora.h"
 
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -11,6 +12,7 @@
 #include <vector>
 
 #include "common.cuh"
+#include "tma_check.cuh"
 
 using namespace chm;
 
@@ -20,7 +22,6 @@ struct chemora {
   double dx;
   double eps_diss, eta, sgc;
   int ko_order;          // 5, or 9 (8th-order BSSN only)
-  int x_images;          // tuning: the fused BSSN kernel writes the x-ghost images of the states it produces
   cudaStream_t stream;
   void* (*alloc)(size_t, void*);
   void (*dealloc)(void*, void*);
@@ -28,13 +29,17 @@ struct chemora {
   double* buf[4];
   double* derivs;       // split variant scratch (lazy)
   double* staging;      // device packed staging for set/get_state (lazy)
+  unsigned* dev_err;    // device error word the kernels' bounded waits write (Layout::err)
   int fused, tile;
+  int autotune_split;   // tuning: chemora_autotune also times the derivative-split variant
   chemora* nb_lo;        // z-neighbours of a linked block (chemora_link_z); nullptr: periodic in itself
   chemora* nb_hi;
   long launches;
   // optional per-kernel timing (chemora_timing): event pairs around every RHS evaluation / ghost fill
   bool timing;
-  std::vector<cudaEvent_t> ev[2];   // [0] rhs, [1] fill; consecutive (start, stop) pairs
+  std::vector<cudaEvent_t> ev[2];   // [0] rhs, [1] fill: a fixed pool of kEvPool events, consecutive (start, stop) pairs
+  int ev_used[2];                   // events of the pool recorded since the last drain
+  double ev_ms[2];                  // time drained from the pool so far
   long ev_launches[2];
   std::string err;
 };
@@ -46,7 +51,9 @@ int fail(chemora_t* h, int code, const std::string& msg) {
   return code;
 }
 int cuda_fail(chemora_t* h, cudaError_t e, const char* what) {
-  return fail(h, CHEMORA_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+  std::string msg = std::string(what) + ": " + cudaGetErrorString(e);
+  if (!last_refusal().empty()) { msg += " (launch refused by the validator: " + last_refusal() + ")"; last_refusal().clear(); }
+  return fail(h, CHEMORA_ECUDA, msg);
 }
 #define CK(h, call, what)                                   \
   do {                                                      \
@@ -98,12 +105,23 @@ int ensure_derivs(chemora_t* h) {
   return CHEMORA_OK;
 }
 
+constexpr int kEvPool = 512;   // 256 (start, stop) pairs per category
+
+// add the recorded pairs' durations to ev_ms and make the pool empty again (waits for the last recorded event)
+void drain(chemora_t* h, int cat) {
+  const int n = h->ev_used[cat] & ~1;
+  if (n >= 2 && cudaEventSynchronize(h->ev[cat][n - 1]) == cudaSuccess)
+    for (int i = 0; i < n; i += 2) {
+      float ms = 0.f;
+      if (cudaEventElapsedTime(&ms, h->ev[cat][i], h->ev[cat][i + 1]) == cudaSuccess) h->ev_ms[cat] += ms;
+    }
+  h->ev_used[cat] = 0;
+}
+
 void tick(chemora_t* h, int cat) {
   if (!h->timing) return;
-  cudaEvent_t e;
-  if (cudaEventCreate(&e) != cudaSuccess) return;
-  cudaEventRecord(e, h->stream);
-  h->ev[cat].push_back(e);
+  if (h->ev_used[cat] == kEvPool) drain(h, cat);   // pool full: one wait per 256 timed launches
+  cudaEventRecord(h->ev[cat][h->ev_used[cat]++], h->stream);
 }
 
 int run_rhs_inner(chemora_t* h, const Stage& st);
@@ -134,8 +152,7 @@ int run_rhs_inner(chemora_t* h, const Stage& st) {
       CK(h, launch_wave1(h->L, C, h->order, h->tile % 6, st, h->stream), "first-order wave kernel launch");
     h->launches += 1;
   } else if (h->fused) {
-    if (h->tile >= 6 && h->tile < 9) CK(h, launch_bssn_ws(h->L, C, h->tile - 6, st, h->stream), "bssn warp-specialised kernel launch");
-    else CK(h, launch_bssn_fused(h->L, C, h->order, h->tile, st, h->stream), "bssn fused kernel launch");
+    CK(h, launch_bssn_fused(h->L, C, h->order, h->tile, st, h->stream), "bssn fused kernel launch");
     h->launches += 1;
   } else {
     int rc = ensure_derivs(h);
@@ -147,15 +164,7 @@ int run_rhs_inner(chemora_t* h, const Stage& st) {
   return CHEMORA_OK;
 }
 
-// Stage::xg for the steppers: the uniform fused BSSN kernel also writes the x-ghost images of the state it
-// produces, and the fill of that state (inside the same step call, so nobody else can have touched it) leaves the
-// x-ghost columns of the interior rows out.  Returns nx when that applies, else 0.
-int stage_xg(const chemora_t* h) {
-  const bool uniform_fused = h->system == CHEMORA_SYS_BSSN && h->fused && !(h->tile >= 6 && h->tile < 9);
-  return h->x_images && uniform_fused && h->L.nx >= 2 * h->L.g ? h->L.nx : 0;
-}
-
-int fill(chemora_t* h, double* state, bool skip_x = false) {
+int fill(chemora_t* h, double* state) {
   FillLink link, *lp = nullptr;
   if (h->nb_lo || h->nb_hi) {
     // a linked block takes its ghost z-planes from the SAME buffer of its neighbours, so the state must be one of
@@ -170,7 +179,7 @@ int fill(chemora_t* h, double* state, bool skip_x = false) {
     lp = &link;
   }
   tick(h, 1);
-  CK(h, launch_fill_ghosts(h->L, state, h->stream, skip_x, lp), "ghost fill launch");
+  CK(h, launch_fill_ghosts(h->L, state, h->stream, lp), "ghost fill launch");
   tick(h, 1);
   h->launches += 1;
   if (h->timing) h->ev_launches[1] += 1;
@@ -210,15 +219,15 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
   h->eps_diss = 0.0; h->eta = 1.0; h->sgc = 0.75;
   h->ko_order = 5;
   h->nb_lo = h->nb_hi = nullptr;
-  h->x_images = 0;   // measured at 256^3: the fills save 0.10 ms each, the fused kernel loses 0.15-0.2 ms per launch
   h->stream = (cudaStream_t)cuda_stream;
   h->alloc = alloc; h->dealloc = dealloc; h->actx = alloc_ctx;
-  h->derivs = nullptr; h->staging = nullptr;
+  h->derivs = nullptr; h->staging = nullptr; h->dev_err = nullptr;
   // 8th-order BSSN (the paper's configuration, 5 ghost zones): fused kernel on tile id 0 only
   h->fused = 1; h->tile = (system_id == CHEMORA_SYS_BSSN && fd_order == 8) ? 0 : 1;
   h->launches = 0;
+  h->autotune_split = 0;
   h->timing = false;
-  h->ev_launches[0] = h->ev_launches[1] = 0;
+  for (int c = 0; c < 2; ++c) { h->ev_used[c] = 0; h->ev_ms[c] = 0.0; h->ev_launches[c] = 0; }
   for (int b = 0; b < 4; ++b) h->buf[b] = nullptr;
 
   int ndev = 0;
@@ -240,6 +249,14 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
       return CHEMORA_ECUDA;
     }
   }
+  h->dev_err = (unsigned*)dev_alloc(h, 128);
+  if (!h->dev_err || cudaMemsetAsync(h->dev_err, 0, 128, h->stream) != cudaSuccess) {
+    dev_free(h, h->dev_err);
+    for (int c = 0; c < 4; ++c) dev_free(h, h->buf[c]);
+    delete h;
+    return CHEMORA_ENOMEM;
+  }
+  L.err = h->dev_err;
   *out = h;
   return CHEMORA_OK;
 }
@@ -261,9 +278,9 @@ int chemora_set_param(chemora_t* h, const char* name, double v) {
   else if (!strcmp(name, "col_rows")) {
     if (v < 1.0 || v > 1e6) return fail(h, CHEMORA_EINVAL, "col_rows must be >= 1");
     h->L.col_rows = (int)v;
-  } else if (!strcmp(name, "x_images")) {
-    if (v != 0.0 && v != 1.0) return fail(h, CHEMORA_EINVAL, "x_images must be 0 or 1");
-    h->x_images = (int)v;
+  } else if (!strcmp(name, "autotune_split")) {
+    if (v != 0.0 && v != 1.0) return fail(h, CHEMORA_EINVAL, "autotune_split must be 0 or 1");
+    h->autotune_split = (int)v;
   } else return fail(h, CHEMORA_EINVAL, std::string("unknown parameter: ") + name);
   return CHEMORA_OK;
 }
@@ -275,7 +292,7 @@ int chemora_get_param(const chemora_t* h, const char* name, double* v) {
   else if (!strcmp(name, "eta")) *v = h->eta;
   else if (!strcmp(name, "shift_gamma_coeff")) *v = h->sgc;
   else if (!strcmp(name, "col_rows")) *v = h->L.col_rows;
-  else if (!strcmp(name, "x_images")) *v = h->x_images;
+  else if (!strcmp(name, "autotune_split")) *v = h->autotune_split;
   else return CHEMORA_EINVAL;
   return CHEMORA_OK;
 }
@@ -340,8 +357,41 @@ int chemora_get_state_async(chemora_t* h, double* host_packed) {
 
 int chemora_synchronize(chemora_t* h) {
   if (!h) return CHEMORA_EINVAL;
+  unsigned code = 0;
+  CK(h, cudaMemcpyAsync(&code, h->dev_err, sizeof code, cudaMemcpyDeviceToHost, h->stream), "error word D2H");
   CK(h, cudaStreamSynchronize(h->stream), "stream synchronisation");
+  if (code != 0) {   // a bounded wait inside a kernel gave up: the results since the last synchronisation are invalid
+    char msg[160];
+    chemora_describe_device_error(code, msg, sizeof msg);
+    cudaMemsetAsync(h->dev_err, 0, sizeof code, h->stream);
+    return fail(h, CHEMORA_ECUDA, msg);
+  }
   return CHEMORA_OK;
+}
+
+int chemora_describe_device_error(unsigned code, char* buf, size_t n) {
+  if (!buf || n == 0) return CHEMORA_EINVAL;
+  const unsigned family = code >> 16, where = code & 0xffffu;
+  if (code == 0) snprintf(buf, n, "no device error");
+  else if (family == 1 && where == 0x80) snprintf(buf, n, "fused BSSN kernel: wait for the point-value tiles timed out (code 0x%x)", code);
+  else if (family == 1) snprintf(buf, n, "fused BSSN kernel: wait for the box of section %u timed out (code 0x%x)", where - 1, code);
+  else if (family == 2) snprintf(buf, n, "wave plane-ring kernel: wait %u for a plane timed out (code 0x%x)", where, code);
+  else snprintf(buf, n, "unknown device error code 0x%x", code);
+  return CHEMORA_OK;
+}
+
+int chemora_selfcheck(char* buf, size_t n) {
+  std::vector<TmaPlan> plans;
+  plans_bssn_fused(plans);
+  plans_wave_tma(plans);
+  int bad = 0;
+  std::string first;
+  for (const TmaPlan& p : plans) {
+    const std::string why = check_tma_plan(p);
+    if (!why.empty() && bad++ == 0) first = why;
+  }
+  if (buf && n) snprintf(buf, n, "%zu launch plans checked, %d rejected%s%s", plans.size(), bad, bad ? ": " : "", first.c_str());
+  return bad ? CHEMORA_EINVAL : (int)plans.size();
 }
 
 int chemora_set_state(chemora_t* h, const double* host_packed) {
@@ -368,31 +418,29 @@ int chemora_rhs(chemora_t* h, const double* dev_state, double* dev_rhs) {
 // The steppers as stage tables: stage s fills buffer `in` (ghosts), then evaluates the right-hand side with the
 // Runge-Kutta epilogue `st`.  One block: stage after stage.  A group of z-linked blocks: every block's fill of a
 // stage, then every block's evaluation (a fill reads the neighbours' interiors of the same stage buffer).
-struct StagePlan { int in; Stage st; bool skip_x; };
+struct StagePlan { int in; Stage st; };
 
 static int rk4_plan(chemora_t* h, double dt, StagePlan* p) {
   double *U = h->buf[0], *Ya = h->buf[1], *Yb = h->buf[2], *S = h->buf[3];
-  const int xg = stage_xg(h);   // stages 1..3 write the x-ghost images of the state the next stage evaluates
-  // stage 1: k1 = f(U);  S = k1;  Yb = U + dt/2 k1      (U may have been touched by the caller: full fill)
-  p[0] = {0, Stage{U, U, S, Yb, dt / 2.0, MODE_FIRST, 0.0, 0.0, xg}, false};
+  // stage 1: k1 = f(U);  S = k1;  Yb = U + dt/2 k1
+  p[0] = {0, Stage{U, U, S, Yb, dt / 2.0, MODE_FIRST, 0.0, 0.0}};
   // stage 2: k2 = f(Yb); S += 2 k2; Ya = U + dt/2 k2
-  p[1] = {2, Stage{Yb, U, S, Ya, dt / 2.0, MODE_MID, 0.0, 0.0, xg}, xg != 0};
+  p[1] = {2, Stage{Yb, U, S, Ya, dt / 2.0, MODE_MID, 0.0, 0.0}};
   // stage 3: k3 = f(Ya); S += 2 k3; Yb = U + dt k3
-  p[2] = {1, Stage{Ya, U, S, Yb, dt, MODE_MID, 0.0, 0.0, xg}, xg != 0};
+  p[2] = {1, Stage{Ya, U, S, Yb, dt, MODE_MID, 0.0, 0.0}};
   // stage 4: k4 = f(Yb); U = U + dt/6 (S + k4)
-  p[3] = {2, Stage{Yb, U, S, nullptr, dt / 6.0, MODE_LAST, 0.0, 0.0, 0}, xg != 0};
+  p[3] = {2, Stage{Yb, U, S, nullptr, dt / 6.0, MODE_LAST, 0.0, 0.0}};
   return 4;
 }
 
 static int rk3_plan(chemora_t* h, double dt, StagePlan* p) {
   double *U = h->buf[0], *Ya = h->buf[1], *Yb = h->buf[2];
-  const int xg = stage_xg(h);
   // U1 = U + dt f(U)
-  p[0] = {0, Stage{U, U, nullptr, Ya, dt, MODE_SSP, 0.0, 1.0, xg}, false};
+  p[0] = {0, Stage{U, U, nullptr, Ya, dt, MODE_SSP, 0.0, 1.0}};
   // U2 = 3/4 U + 1/4 (U1 + dt f(U1))
-  p[1] = {1, Stage{Ya, U, nullptr, Yb, dt, MODE_SSP, 3.0 / 4.0, 1.0 / 4.0, xg}, xg != 0};
+  p[1] = {1, Stage{Ya, U, nullptr, Yb, dt, MODE_SSP, 3.0 / 4.0, 1.0 / 4.0}};
   // U+ = 1/3 U + 2/3 (U2 + dt f(U2)), written over U point by point
-  p[2] = {2, Stage{Yb, U, nullptr, U, dt, MODE_SSP, 1.0 / 3.0, 2.0 / 3.0, 0}, xg != 0};
+  p[2] = {2, Stage{Yb, U, nullptr, U, dt, MODE_SSP, 1.0 / 3.0, 2.0 / 3.0}};
   return 3;
 }
 
@@ -403,7 +451,7 @@ static int step_one(chemora_t* h, double dt, bool rk3) {
   const int ns = rk3 ? rk3_plan(h, dt, p) : rk4_plan(h, dt, p);
   for (int s = 0; s < ns; ++s) {
     int rc;
-    if ((rc = fill(h, h->buf[p[s].in], p[s].skip_x))) return rc;
+    if ((rc = fill(h, h->buf[p[s].in]))) return rc;
     if ((rc = run_rhs(h, p[s].st))) return rc;
   }
   return CHEMORA_OK;
@@ -427,7 +475,7 @@ static int step_group(chemora_t* const* hs, int n, double dt, bool rk3) {
   for (int s = 0; s < ns; ++s) {
     int rc;
     for (int b = 0; b < n; ++b)
-      if ((rc = fill(hs[b], hs[b]->buf[p[b][s].in], p[b][s].skip_x))) return rc;
+      if ((rc = fill(hs[b], hs[b]->buf[p[b][s].in]))) return rc;
     for (int b = 0; b < n; ++b)
       if ((rc = run_rhs(hs[b], p[b][s].st))) return rc;
   }
@@ -479,11 +527,20 @@ int chemora_energy(chemora_t* h, const double* dev_state, double* dev_eps, doubl
 int chemora_set_variant(chemora_t* h, int fused, int tile_id) {
   if (!h || tile_id < 0 || tile_id >= CHEMORA_NUM_TILES || (fused != 0 && fused != 1)) return CHEMORA_EINVAL;
   if (!fused && h->system != CHEMORA_SYS_BSSN) return fail(h, CHEMORA_EINVAL, "wave systems have no split variant");
-  if (fused && h->system == CHEMORA_SYS_BSSN && h->order == 8 && tile_id != 0)
-    return fail(h, CHEMORA_EINVAL, "8th-order BSSN: the fused kernel has tile id 0 (16x4x4) only");
+  if (!chemora_variant_available(h->system, h->order, fused, tile_id))
+    return fail(h, CHEMORA_EINVAL, "no such kernel variant for this system and order (chemora_variant_available)");
   h->fused = fused;
   h->tile = tile_id;
   return CHEMORA_OK;
+}
+
+int chemora_variant_available(int system_id, int fd_order, int fused, int tile_id) {
+  if (tile_id < 0 || tile_id >= CHEMORA_NUM_TILES || (fd_order != 4 && fd_order != 8)) return 0;
+  if (system_id == CHEMORA_SYS_WAVE || system_id == CHEMORA_SYS_WAVE1) return fused == 1;   // ids 6..8: plane-ring kernel
+  if (system_id != CHEMORA_SYS_BSSN) return 0;
+  if (fused == 0) return tile_id < 6;                      // six split tiles, both orders
+  if (fused != 1) return 0;
+  return fd_order == 8 ? tile_id == 0 : tile_id < kNumFused;
 }
 
 int chemora_get_variant(const chemora_t* h, int* fused, int* tile_id) {
@@ -496,6 +553,7 @@ int chemora_get_variant(const chemora_t* h, int* fused, int* tile_id) {
 int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, int* tz) {
   if (tile_id < 0 || tile_id >= CHEMORA_NUM_TILES) return CHEMORA_EINVAL;
   const bool f = system_id == CHEMORA_SYS_BSSN && fused;
+  if (f && tile_id >= kNumFused) return CHEMORA_EINVAL;
   const TileShape T = f ? kTilesFused[tile_id]
                       : (system_id == CHEMORA_SYS_WAVE && tile_id >= 6 && tile_id < 9) ? kTilesWaveTma[tile_id - 6]
                       : (system_id == CHEMORA_SYS_WAVE1 && tile_id >= 6 && tile_id < 9) ? kTilesWave1Tma[tile_id - 6]
@@ -509,7 +567,7 @@ int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, 
 // The paper's tile cost model for the uniform fused BSSN kernel; see include/chemora.h.
 int chemora_tile_cost(int fd_order, int ghost, int tile_id, double* sigma, long* requests, long* points) {
   if (fd_order != 4 && fd_order != 8) return CHEMORA_EINVAL;
-  if (tile_id < 0 || tile_id >= CHEMORA_NUM_TILES || (tile_id >= 6 && tile_id < 9)) return CHEMORA_EINVAL;
+  if (tile_id < 0 || tile_id >= kNumFused) return CHEMORA_EINVAL;
   if (fd_order == 8 && tile_id != 0) return CHEMORA_EINVAL;
   const int H = fd_order / 2 + 1;
   if (ghost < H) return CHEMORA_EINVAL;
@@ -532,36 +590,42 @@ int chemora_tile_cost(int fd_order, int ghost, int tile_id, double* sigma, long*
 int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out) {
   if (!h) return CHEMORA_EINVAL;
   const int save_f = h->fused, save_t = h->tile;
+  if (ms_out) for (int n = 0; n < 2 * CHEMORA_NUM_TILES; ++n) ms_out[n] = -1.f;
   float best = -1.f;
   int bf = save_f, bt = save_t;
-  cudaEvent_t e0, e1;
-  CK(h, cudaEventCreate(&e0), "event create");
-  CK(h, cudaEventCreate(&e1), "event create");
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  for (int n = 0; n < 4; ++n)
+    if (cudaEventCreate(&ev[n]) != cudaSuccess) {
+      for (int m = 0; m < n; ++m) cudaEventDestroy(ev[m]);
+      return cuda_fail(h, cudaGetLastError(), "event create");
+    }
   int rc = fill(h, h->buf[0]);
-  for (int f = 1; f >= 0 && !rc; --f)
+  // fused variants always; the derivative-split variant (about 18 GB of scratch at 256^3, never the pick in any
+  // measured sweep) only when the tuning parameter "autotune_split" is 1
+  for (int f = 1; f >= (h->autotune_split ? 0 : 1) && !rc; --f)
     for (int t = 0; t < CHEMORA_NUM_TILES && !rc; ++t) {
-      float ms = -1.f;
-      const bool bssn = h->system == CHEMORA_SYS_BSSN, o8 = bssn && h->order == 8 && t != 0;   // O8 BSSN: one fused tile
-      const int nwave = 9;   // the wave systems have three more ids: the plane-ring kernel
-      if ((f == 1 && !o8 && (bssn || t < nwave)) || (f == 0 && bssn && t < 6)) {
-        h->fused = f; h->tile = t;
-        // a middle RK4 stage (the common case) on scratch operands: k = f(U); S += 2k; Ya = U + a k.
-        // S and Ya are scratch between steps (stage 1 overwrites them); U is only read.
-        Stage st{h->buf[0], h->buf[0], h->buf[3], h->buf[1], 1e-3, MODE_MID};
-        rc = run_rhs(h, st);                                               // warm-up
-        if (!rc) {
-          cudaEventRecord(e0, h->stream);
-          rc = run_rhs(h, st);
-          cudaEventRecord(e1, h->stream);
-          if (cudaEventSynchronize(e1) != cudaSuccess) rc = fail(h, CHEMORA_ECUDA, "autotune sync failed");
-          else cudaEventElapsedTime(&ms, e0, e1);
-        }
-        if (!rc && (best < 0.f || ms < best)) { best = ms; bf = f; bt = t; }
+      if (!chemora_variant_available(h->system, h->order, f, t)) continue;
+      h->fused = f; h->tile = t;
+      // a middle RK4 stage (the common case) on scratch operands: k = f(U); S += 2k; Ya = U + a k.
+      // S and Ya are scratch between steps (stage 1 overwrites them); U is only read.
+      Stage st{h->buf[0], h->buf[0], h->buf[3], h->buf[1], 1e-3, MODE_MID};
+      int vrc = run_rhs(h, st);                                            // warm-up
+      for (int n = 0; n < 3 && !vrc; ++n) {                                // three timed runs, the median counts
+        cudaEventRecord(ev[n], h->stream);
+        vrc = run_rhs(h, st);
       }
+      if (vrc == CHEMORA_ENOMEM || vrc == CHEMORA_EINVAL) continue;        // variant not usable here: ms stays -1
+      if (vrc) { rc = vrc; break; }
+      cudaEventRecord(ev[3], h->stream);
+      if (cudaEventSynchronize(ev[3]) != cudaSuccess) { rc = cuda_fail(h, cudaGetLastError(), "autotune sync"); break; }
+      float m[3];
+      for (int n = 0; n < 3; ++n) cudaEventElapsedTime(&m[n], ev[n], ev[n + 1]);
+      const float lo = fminf(m[0], fminf(m[1], m[2])), hi = fmaxf(m[0], fmaxf(m[1], m[2]));
+      const float ms = m[0] + m[1] + m[2] - lo - hi;
+      if (best < 0.f || ms < best) { best = ms; bf = f; bt = t; }
       if (ms_out) ms_out[f * CHEMORA_NUM_TILES + t] = ms;
     }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
+  for (int n = 0; n < 4; ++n) cudaEventDestroy(ev[n]);
   h->fused = rc ? save_f : bf;
   h->tile = rc ? save_t : bt;
   if (fused_out) *fused_out = h->fused;
@@ -575,29 +639,36 @@ static void drop_events(chemora_t* h) {
   for (int c = 0; c < 2; ++c) {
     for (cudaEvent_t e : h->ev[c]) cudaEventDestroy(e);
     h->ev[c].clear();
+    h->ev_used[c] = 0;
+    h->ev_ms[c] = 0.0;
     h->ev_launches[c] = 0;
   }
 }
 
 int chemora_timing(chemora_t* h, int enable) {
   if (!h) return CHEMORA_EINVAL;
+  h->timing = false;
   drop_events(h);
-  h->timing = enable != 0;
+  if (!enable) return CHEMORA_OK;
+  for (int c = 0; c < 2; ++c)
+    for (int i = 0; i < kEvPool; ++i) {
+      cudaEvent_t e;
+      if (cudaEventCreate(&e) != cudaSuccess) {
+        drop_events(h);
+        return cuda_fail(h, cudaGetLastError(), "event create");
+      }
+      h->ev[c].push_back(e);
+    }
+  h->timing = true;
   return CHEMORA_OK;
 }
 
 int chemora_timing_read(chemora_t* h, double* rhs_ms, long* rhs_launches, double* fill_ms, long* fill_launches) {
   if (!h) return CHEMORA_EINVAL;
   CK(h, cudaStreamSynchronize(h->stream), "timing sync");
-  double tot[2] = {0.0, 0.0};
-  for (int c = 0; c < 2; ++c)
-    for (size_t i = 0; i + 1 < h->ev[c].size(); i += 2) {
-      float ms = 0.f;
-      CK(h, cudaEventElapsedTime(&ms, h->ev[c][i], h->ev[c][i + 1]), "event elapsed");
-      tot[c] += ms;
-    }
-  if (rhs_ms) *rhs_ms = tot[0];
-  if (fill_ms) *fill_ms = tot[1];
+  for (int c = 0; c < 2; ++c) drain(h, c);
+  if (rhs_ms) *rhs_ms = h->ev_ms[0];
+  if (fill_ms) *fill_ms = h->ev_ms[1];
   if (rhs_launches) *rhs_launches = h->ev_launches[0];
   if (fill_launches) *fill_launches = h->ev_launches[1];
   return CHEMORA_OK;
@@ -613,7 +684,6 @@ int chemora_kernel_info(const chemora_t* h, int* regs, int* local_bytes, int* sm
                       ? kernel_info_wave1_tma(h->order, h->tile - 6, &a)
                   : h->system == CHEMORA_SYS_WAVE1 ? kernel_info_wave1(h->order, h->tile % 6, &a)
                   : !h->fused              ? kernel_info_bssn_split(1, h->tile % 6, &a)
-                  : h->tile >= 6 && h->tile < 9 ? kernel_info_bssn_ws(h->tile - 6, &a)
                                            : kernel_info_bssn_fused(h->order, h->tile, &a);
   if (e != cudaSuccess) return cuda_fail(const_cast<chemora_t*>(h), e, "cudaFuncGetAttributes");
   if (regs) *regs = a.numRegs;
@@ -661,6 +731,7 @@ int chemora_destroy(chemora_t* h) {
   for (int b = 0; b < 4; ++b) dev_free(h, h->buf[b]);
   dev_free(h, h->derivs);
   dev_free(h, h->staging);
+  dev_free(h, h->dev_err);
   delete h;
   return CHEMORA_OK;
 }

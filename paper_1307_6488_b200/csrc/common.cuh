@@ -14,15 +14,6 @@ namespace chm {
 #else
 #define CHM_ST(p, v) (*(p) = (v))
 #endif
-#ifndef CHM_IMG_PLAIN
-#define CHM_IMG_PLAIN 1
-#endif
-#if CHM_IMG_PLAIN
-#define CHM_IMG(p, v) (*(p) = (v))   // x-ghost images share their sector with points another CTA writes: keep it in L2
-#else
-#define CHM_IMG(p, v) CHM_ST(p, v)
-#endif
-
 // Device-side view of the padded SoA layout (include/chemora.h "Conventions").
 struct Layout {
   int nx, ny, nz, g;     // interior dims, ghost width
@@ -34,6 +25,7 @@ struct Layout {
   long vstride;          // plane * tot_z
   int tot_y, tot_z;
   int col_rows;          // fused BSSN kernel: y-extent (grid rows) of a tile-traversal column (L2 reuse of halos)
+  unsigned* err;         // the handle's device error word (0 = fine): bounded mbarrier waits record a code here
 };
 
 // Stencil scale factors and model parameters, precomputed on the host once per launch.
@@ -64,9 +56,6 @@ struct Stage {
   double a;              // dt/2, dt/2, dt, dt/6
   int mode;
   double ca, cb;         // MODE_SSP only
-  int xg;                // fused BSSN kernel: != 0 (= nx) => it also writes the x-ghost images of the new state's
-                         // points (columns i < g to i + nx, i >= nx - g to i - nx), so that the next ghost fill can
-                         // leave the x-ghost columns of the interior rows out; needs nx >= 2 g
 };
 
 // a U + b (Y + dt k), every product and sum rounded once
@@ -115,41 +104,32 @@ __device__ __forceinline__ void stage_emit(const Stage& st, long q, double k, co
   }
 }
 
-// Same with the mode as a compile-time constant (no branches in the epilogue of the fused BSSN kernel).
-// xgo: offset of the point's x-ghost image (0: it has none, or Stage::xg is off); see Stage::xg
+// Same with the mode as a compile-time constant (no branches in the epilogue of the fused BSSN kernel):
+// values first, stores under one predicate (no divergent region around the arithmetic)
 template <int MODE>
-__device__ __forceinline__ void stage_emit_t(const Stage& st, long q, double k, const StagePre& pr, bool valid,
-                                             long xgo = 0) {
-  // values first, stores under one predicate (no divergent region around the arithmetic)
-  const bool img = valid && xgo != 0;
+__device__ __forceinline__ void stage_emit_t(const Stage& st, long q, double k, const StagePre& pr, bool valid) {
   if (MODE == MODE_RHS) {
     if (valid) CHM_ST(&st.out[q], k);
   } else if (MODE == MODE_FIRST) {
     const double y = __dadd_rn(pr.u, __dmul_rn(st.a, k));
     if (valid) { CHM_ST(&st.S[q], k); CHM_ST(&st.out[q], y); }
-    if (img) CHM_IMG(&st.out[q + xgo], y);
   } else if (MODE == MODE_MID) {
     const double s2 = __dadd_rn(pr.s, __dmul_rn(2.0, k)), y = __dadd_rn(pr.u, __dmul_rn(st.a, k));
     if (valid) { CHM_ST(&st.S[q], s2); CHM_ST(&st.out[q], y); }
-    if (img) CHM_IMG(&st.out[q + xgo], y);
   } else if (MODE == MODE_LAST) {
     const double u = __dadd_rn(pr.u, __dmul_rn(st.a, __dadd_rn(pr.s, k)));
     if (valid) CHM_ST(&st.U[q], u);
-    if (img) CHM_IMG(&st.U[q + xgo], u);
   } else {
     const double y = ssp_combine(st, pr.u, pr.s, k);   // pr.u = U, pr.s = the evaluated state at the point
     if (valid) CHM_ST(&st.out[q], y);
-    if (img) CHM_IMG(&st.out[q + xgo], y);
   }
 }
 
 // Tile shapes of the variant sweep.  Fused kernel: 3-D tile, one point per thread.  Split kernels and the wave
 // kernel: x,y = thread block, z = planes marched per block.
 struct TileShape { int tx, ty, tz; };
-// ids 6..8: the warp-specialised fused kernel (kernels_bssn_ws.cu) on the three 256-point shapes;
-// ids 9..10: the uniform kernel on 384-point tiles (12 warps, live values parked in tensor memory)
-static const TileShape kTilesFused[11] = {{16, 4, 4}, {16, 8, 2}, {8, 8, 4}, {8, 4, 8}, {16, 2, 8}, {16, 4, 2},
-                                          {16, 4, 4}, {16, 8, 2}, {16, 2, 8}, {16, 4, 6}, {16, 6, 4}};
+constexpr int kNumFused = 5;   // fused BSSN tile ids 0..4 (8th order: id 0 only)
+static const TileShape kTilesFused[kNumFused] = {{16, 4, 4}, {16, 8, 2}, {8, 4, 8}, {16, 2, 8}, {16, 4, 2}};
 // wave system ids 6..8: the TMA plane-ring kernel (x, y = thread block, z = planes per work item)
 static const TileShape kTilesWaveTma[3] = {{32, 16, 32}, {32, 16, 64}, {64, 8, 32}};
 // Sample-1 system ids 6..8: the same plane-ring kernel with five variables (smaller tiles: the ring holds 5 boxes a plane)
@@ -163,10 +143,8 @@ struct FillLink {
   const double* lo;  long lo_vstride;  int lo_nz;    // lower neighbour: its top g interior planes
   const double* hi;  long hi_vstride;                // upper neighbour: its bottom g interior planes
 };
-// skip_x: leave the x-ghost columns of the interior rows out (their producer wrote them, Stage::xg);
 // link: where the ghost z-planes come from (nullptr: the block's own periodic images)
-cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s, bool skip_x = false,
-                               const FillLink* link = nullptr);
+cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s, const FillLink* link = nullptr);
 cudaError_t launch_energy(const Layout& L, const double* state, double* eps_out, double* sum, cudaStream_t s);
 cudaError_t launch_enforce(const Layout& L, double* state, cudaStream_t s);
 cudaError_t launch_pack(const Layout& L, const double* packed, double* state, bool to_state, cudaStream_t s);
@@ -180,8 +158,6 @@ bool wave1_tma_ok(const Layout& L, int order, bool ko, int which);
 cudaError_t launch_wave1(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
 cudaError_t kernel_info_wave1(int order, int tile, cudaFuncAttributes* a);
 cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
-cudaError_t launch_bssn_ws(const Layout& L, const Coef& C, int which, const Stage& st, cudaStream_t s);
-cudaError_t kernel_info_bssn_ws(int which, cudaFuncAttributes* a);
 cudaError_t launch_bssn_derivs(const Layout& L, const Coef& C, int order, int tile, const double* in, double* derivs,
                                cudaStream_t s);
 cudaError_t launch_bssn_from_derivs(const Layout& L, const Coef& C, int tile, const double* derivs,

@@ -53,10 +53,10 @@ __global__ void __launch_bounds__(256) fill_ghosts_kernel(Layout L, double* __re
   }
 }
 
-cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s, bool skip_x, const FillLink* link) {
+cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s, const FillLink* link) {
   const int g = L.g;
   if (g == 0) return cudaSuccess;
-  const long rowsA = 2L * g * L.tot_y, rowsAB = rowsA + 2L * g * L.nz, rowsC = skip_x ? 0 : (long)L.nz * L.ny;
+  const long rowsA = 2L * g * L.tot_y, rowsAB = rowsA + 2L * g * L.nz, rowsC = (long)L.nz * L.ny;
   int lpr_shift = 0;
   while ((1 << lpr_shift) < 2 * g && lpr_shift < 5) ++lpr_shift;
   const long tasks = rowsAB + (rowsC + (32 >> lpr_shift) - 1) / (32 >> lpr_shift);

@@ -7,38 +7,8 @@
 // above it is processed; the read-once RK4 operands carry an L2 evict-first policy and stores are streaming.
 // See bssn_tma.cuh for the design; DESIGN.md "Kernels" for the roofline that bounds it.
 #include "bssn_tma.cuh"
+#include "tma_check.cuh"
 
-#ifndef CHM_BLOCKSYNC   // experiment switch: block barrier per variable instead of warp-wise slot release
-#define CHM_BLOCKSYNC 0
-#endif
-#ifndef CHM_TWOPASS
-#define CHM_TWOPASS 1   // mixed second derivatives as D_x(D_y f), D_x(D_z f), D_y(D_z f) through shared memory, on the
-#endif                  // tiles whose z-planes are one or two warps (plane-local barrier); 2 = on every 256-point tile
-#ifndef CHM_PAIR
-#define CHM_PAIR 0      // evaluate the stencils of 3 (beta^i) / 2 (gt_ij) staged boxes in one block: more independent
-#endif                  // LDS and FP64 chains in flight per warp while few values are live (early sections)
-#ifndef CHM_TMEM
-#define CHM_TMEM 0      // park long-lived per-point values (the 18 Christoffel symbols) in tensor memory
-#endif
-// further sections of one kind as one loop body (tables in tensor memory): 1 = beta^i, 2 = gt_ij, 4 = Gt^i,
-// 8 = B^i.  Measured at 8th order, 256^3, ms per launch: 0 -> 8.79, 4 -> 8.80, 8 -> 8.87, 12 -> 8.86, 2 -> 8.95,
-// 13 -> 8.87, 15 -> 9.09 (code 132 KB -> 80 KB): once the At_ij loop is in, code size no longer binds.
-#ifndef CHM_LOOPS8
-#define CHM_LOOPS8 0
-#endif
-#ifndef CHM_LOOPS4
-#define CHM_LOOPS4 0
-#endif
-#ifndef CHM_ATLOOP
-#define CHM_ATLOOP 1   // 4th order too: the At_ij sections as one loop body (6.29 -> 6.19 ms per launch at 256^3)
-#endif
-#ifndef CHM_STAR
-#define CHM_STAR 0     // advection / first-derivative-only sections (Gt^i, K, At_ij, B^i, A) stage a 3-D star (three slab
-#endif                 // boxes: tile + x-halo, + y-halo, + z-halo) instead of the cuboid: 1792 instead of 2200 doubles out
-                       // of L2 per section at 4th order, 2432 instead of 5096 at 8th.  Bit-identical; measured SLOWER
-                       // (256^3, ms per launch: 16x4x4 6.09 -> 6.64, 16x2x8 6.12 -> 6.62; 8th order 100^3 RK3 step
-                       // 2.12 -> 2.56): the slabs have as many rows (96 vs 100) as the cuboid and three TMA
-                       // instructions per refill instead of one -- the box fill is bound by rows, not bytes.  Off.
 #ifndef CHM_L2HINT
 #define CHM_L2HINT 1
 #endif
@@ -51,7 +21,7 @@ namespace chm {
 constexpr int kCenVars = 21;
 __device__ __forceinline__ constexpr int cen_index(int v) { return v < 14 ? v : v - 3; }
 // variables whose right-hand side leaves in section o (first, second; -1 = none)
-__device__ __forceinline__ constexpr int emit_var(int o, int n) {
+__host__ __device__ __forceinline__ constexpr int emit_var(int o, int n) {
   return o < 9 ? (n == 0 ? order_var(o) : -1) : o < 12 ? -1 : o < 21 ? (n == 0 ? order_var(o) : -1)
          : o < 24 ? (n == 0 ? V_GAM + (o - 21) : V_B + (o - 21)) : (n == 0 ? V_A : -1);
 }
@@ -68,7 +38,7 @@ struct TmaCfg {
   // ring slots (a 6-slot ring fits the 16x4x4 tile but its run-time slot index costs more than the depth gains:
   // 8.2 ms vs 6.3 ms)
   static constexpr int NS = ORDER == 8 ? 3 : HEAVY ? 4 : 5;   // 8th order: 41 KB boxes, three fit
-  static constexpr bool PARK = HEAVY || CHM_TMEM;
+  static constexpr bool PARK = HEAVY;
   static constexpr int TILE = (TX + 2) * TY * TZ;                      // doubles in one (TX+2,TY,TZ) tile box
   static constexpr uint32_t TILE_BYTES = (uint32_t)TILE * 8u;
   static constexpr int SLOTX = SLOT + 4 * TILE;   // box + RK4 operands (U,S) of up to two emitted variables
@@ -78,46 +48,35 @@ struct TmaCfg {
   static constexpr int DYX = TX + ORDER;             // x-halo = reach of the centred first derivative (order/2) on each side
   static constexpr int DY_N = DYX * TY * TZ, DZ_N = DYX * (TY + ORDER) * TZ;
   // (planes of 128 threads: measured no gain over the one-pass form)
-  static constexpr bool TWOPASS = !HEAVY && (CHM_TWOPASS == 2 || (CHM_TWOPASS == 1 && (TX * TY == 64 || TX * TY == 32)));
+  static constexpr bool TWOPASS = !HEAVY && (TX * TY == 64 || TX * TY == 32);
   static constexpr int DB = TWOPASS ? (DY_N + DZ_N + 15) / 16 * 16 : 0;
   static constexpr size_t SMEM = (size_t)(NS * SLOTX + CEN + 2 * DB) * 8 + (NS + 1) * 8 + (NS + 1) * 8 + 64 + 16 + 64 + 128;
   static constexpr int NWARPS = THREADS / 32;
-  // star staging: x-slab (BX,TY,TZ), y-slab (TX+2,BY,TZ), z-slab (TX+2,TY,BZ), back to back inside the slot
-  // (only on the tile shapes whose slabs keep every box 128-byte aligned in the slot)
-  static constexpr int SX_N = BX * TY * TZ, SY_N = (TX + 2) * BY * TZ, SZ_N = (TX + 2) * TY * BZ;
-  static constexpr bool STAR = CHM_STAR && !HEAVY && SX_N % 16 == 0 && SY_N % 16 == 0 && SX_N + SY_N + SZ_N <= SLOT;
-  static constexpr uint32_t STAR_BYTES = (uint32_t)(SX_N + SY_N + SZ_N) * 8u;
+  // shared-memory map in doubles from the dynamic base (the kernel and the host-side validator both use these)
+  __host__ __device__ static constexpr int box_off(int slot) { return slot * SLOTX; }
+  __host__ __device__ static constexpr int op_off(int slot, int n) { return slot * SLOTX + SLOT + n * TILE; }   // n: U0, S0, U1, S1
+  __host__ __device__ static constexpr int cen_off(int group) { return NS * SLOTX + 7 * group * TILE; }        // three 7-variable groups
+  __host__ __device__ static constexpr int dbuf_off() { return NS * SLOTX + CEN; }
+  __host__ __device__ static constexpr int bar_off() { return NS * SLOTX + CEN + 2 * DB; }                      // full[NS], cfull, empty[NS + 1]
 };
-// sections (consumption order) that read only axis stencils: Gt^i 9..11, K 14, At_ij 15..20, B^i 21..23, A 24
-__device__ __forceinline__ constexpr bool star_section(int o) { return (o >= 9 && o <= 11) || o >= 14; }
-
 template <int TX, int TY, int TZ, int MODE, int ORDER>
 __global__ void __launch_bounds__(TX* TY* TZ, 1)
 bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ CUtensorMap tmCen,
-                const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS,
-                const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmY,
-                const __grid_constant__ CUtensorMap tmZ, Layout L, Coef C, Stage st, int ntx, int nty, int ntz, int cy) {
+                const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS, Layout L, Coef C, Stage st, int ntx, int nty, int ntz, int cy) {
   using Cfg = TmaCfg<TX, TY, TZ, ORDER>;
   constexpr int H = Cfg::H;
   constexpr int BX = Cfg::BX, BY = Cfg::BY, SLOT = Cfg::SLOT, SLOTX = Cfg::SLOTX, TILE = Cfg::TILE, CEN = Cfg::CEN;
   constexpr unsigned NW = Cfg::NWARPS;
   constexpr int kSlots = Cfg::NS;
   constexpr bool PARK = Cfg::PARK;
-  // Sections of the same kind as ONE loop body each, with a run-time section index.  The 8th-order kernel was
-  // bound by instruction fetch at 150 KB of code; the At_ij loop (always on, table in shared memory, see there)
-  // brought it to 132 KB and 27 % less time.  The further loops (beta^i, gt_ij, Gt^i, B^i; CHM_LOOPS8/4) hand
-  // values to and from the statically indexed code around them through small per-thread tables in tensor memory
-  // (run-time column address); measured no further gain, off by default.
-  constexpr int LOOPS = Cfg::TWOPASS && TX * TY == 64 && !PARK ? (ORDER == 8 ? CHM_LOOPS8 : CHM_LOOPS4) : 0;
-  constexpr bool TMEM = PARK || LOOPS != 0;
-  constexpr int T_TAB = 0, T_OUT = 12;   // LOOPS: tables (doubles): 6 pairs handed to a loop, up to 30 values handed back
+  constexpr bool TMEM = PARK;
   // parking map (offsets in doubles inside the thread's 84-double area)
   constexpr int P_CU = 0, P_DG = 18, P_DB = 42, P_LG = 52, P_AT = 58, P_ADG = 64, P_GN = 68, P_DCA = 72, P_AU = 78;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double* sm = reinterpret_cast<double*>(smem_raw);   // dynamic smem base: 128-byte aligned (no static smem)
-  double* cbuf = sm + kSlots * SLOTX;                                  // [kCenVars][TILE]
-  double* dbuf = cbuf + CEN;                                           // [2][DB] shared first derivatives
-  uint64_t* full = reinterpret_cast<uint64_t*>(dbuf + 2 * Cfg::DB);    // [kSlots] boxes, then [1] point values
+  double* cbuf = sm + Cfg::cen_off(0);                                 // [kCenVars][TILE]
+  double* dbuf = sm + Cfg::dbuf_off();                                 // [2][DB] shared first derivatives
+  uint64_t* full = reinterpret_cast<uint64_t*>(sm + Cfg::bar_off());   // [kSlots] boxes, then [1] point values
   uint64_t* cfull = full + kSlots;
   uint64_t* empty = cfull + 1;                                         // [kSlots] + [1]: warps that left a buffer
   constexpr int nops = MODE == MODE_RHS ? 0 : (MODE == MODE_FIRST ? 1 : 2);   // RK4 operands per emitted var
@@ -178,36 +137,24 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
   };
   // box of variable order o of the tile whose origin (padded, minus halo) is (x0,y0,z0); issued by one thread
   auto issue = [&](int o, int slot, int x0, int y0, int z0) {
-    double* dst = sm + slot * SLOTX;
     const int v0 = emit_var(o, 0), v1 = emit_var(o, 1);
     const int nem = (v0 >= 0) + (v1 >= 0);
-    const bool star = Cfg::STAR && star_section(o);
-    mbar_expect_tx(&full[slot], (star ? Cfg::STAR_BYTES : Cfg::BOX_BYTES) + (uint32_t)(nops * nem) * Cfg::TILE_BYTES);
-    if (star) {
-      tma_load_4d(dst, &tmX, &full[slot], x0, y0 + H, z0 + H, order_var(o));
-      tma_load_4d(dst + Cfg::SX_N, &tmY, &full[slot], x0 + H - 1, y0, z0 + H, order_var(o));
-      tma_load_4d(dst + Cfg::SX_N + Cfg::SY_N, &tmZ, &full[slot], x0 + H - 1, y0 + H, z0, order_var(o));
-    } else {
-      tma_load_4d(dst, &tm, &full[slot], x0, y0, z0, order_var(o));
-    }
-    if (v0 >= 0 && nops >= 1) tma_load_4d_hint(dst + SLOT, &tmU, &full[slot], x0 + H - 1, y0 + H, z0 + H, v0, pol_stream);
-    if (v0 >= 0 && nops == 2) tma_load_4d_hint(dst + SLOT + TILE, &tmS, &full[slot], x0 + H - 1, y0 + H, z0 + H, v0, pol_stream);
-    if (v1 >= 0 && nops >= 1) tma_load_4d_hint(dst + SLOT + 2 * TILE, &tmU, &full[slot], x0 + H - 1, y0 + H, z0 + H, v1, pol_stream);
-    if (v1 >= 0 && nops == 2) tma_load_4d_hint(dst + SLOT + 3 * TILE, &tmS, &full[slot], x0 + H - 1, y0 + H, z0 + H, v1, pol_stream);
+    mbar_expect_tx(&full[slot], Cfg::BOX_BYTES + (uint32_t)(nops * nem) * Cfg::TILE_BYTES);
+    tma_load_4d(sm + Cfg::box_off(slot), &tm, &full[slot], x0, y0, z0, order_var(o));
+    if (v0 >= 0 && nops >= 1) tma_load_4d_hint(sm + Cfg::op_off(slot, 0), &tmU, &full[slot], x0 + H - 1, y0 + H, z0 + H, v0, pol_stream);
+    if (v0 >= 0 && nops == 2) tma_load_4d_hint(sm + Cfg::op_off(slot, 1), &tmS, &full[slot], x0 + H - 1, y0 + H, z0 + H, v0, pol_stream);
+    if (v1 >= 0 && nops >= 1) tma_load_4d_hint(sm + Cfg::op_off(slot, 2), &tmU, &full[slot], x0 + H - 1, y0 + H, z0 + H, v1, pol_stream);
+    if (v1 >= 0 && nops == 2) tma_load_4d_hint(sm + Cfg::op_off(slot, 3), &tmS, &full[slot], x0 + H - 1, y0 + H, z0 + H, v1, pol_stream);
   };
   // point values of a tile (three 7-variable boxes: vars 0..6, 7..13, 17..23)
   auto issue_cen = [&](int x0, int y0, int z0) {
     mbar_expect_tx(cfull, (uint32_t)kCenVars * Cfg::TILE_BYTES);
-    tma_load_4d(cbuf, &tmCen, cfull, x0 + H - 1, y0 + H, z0 + H, 0);
-    tma_load_4d(cbuf + 7 * TILE, &tmCen, cfull, x0 + H - 1, y0 + H, z0 + H, 7);
-    tma_load_4d(cbuf + 14 * TILE, &tmCen, cfull, x0 + H - 1, y0 + H, z0 + H, 17);
+    tma_load_4d(sm + Cfg::cen_off(0), &tmCen, cfull, x0 + H - 1, y0 + H, z0 + H, 0);
+    tma_load_4d(sm + Cfg::cen_off(1), &tmCen, cfull, x0 + H - 1, y0 + H, z0 + H, 7);
+    tma_load_4d(sm + Cfg::cen_off(2), &tmCen, cfull, x0 + H - 1, y0 + H, z0 + H, 17);
   };
   // one warp leaves buffer b (all its reads of it are done); true for lane 0 of the last of the NW warps
   auto leave = [&](int b) {
-#if CHM_BLOCKSYNC
-    __syncthreads();
-    return tid == 0;
-#endif
     __syncwarp();
     bool last = false;
     if (lane == 0) {
@@ -257,26 +204,13 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       const double* op = sm + slot_of(o) * SLOTX + SLOT + 2 * n * TILE + toff;
       return StagePre{op[0], op[TILE]};
     };
-    const long xgo = st.xg == 0 ? 0 : (i < L.g ? st.xg : (i >= L.nx - L.g ? -st.xg : 0));   // x-ghost image, Stage::xg
-    auto emit = [&](int v, double k, const StagePre& pr) { stage_emit_t<MODE>(st, q + v * L.vstride, k, pr, valid, xgo); };
+    auto emit = [&](int v, double k, const StagePre& pr) { stage_emit_t<MODE>(st, q + v * L.vstride, k, pr, valid); };
 
     // section o: wait for its box, hand out the accessor; done(o): this warp leaves the slot; the last warp to
     // leave refills it with the box 5 loads ahead (of this tile, or of this CTA's next tile)
     auto box = [&](int o) {
-      mbar_wait(&full[slot_of(o)], parity_of(o));
+      mbar_wait(&full[slot_of(o)], parity_of(o), L.err, 0x10000u + (unsigned)o + 1u);
       return BoxPoint<BX, BY>{sm + slot_of(o) * SLOTX + coff};
-    };
-    // the same for a star section: pointers to the point in the x-, y- and z-slab
-    auto sbox = [&](int o) {
-      if constexpr (Cfg::STAR) {
-        mbar_wait(&full[slot_of(o)], parity_of(o));
-        const double* b = sm + slot_of(o) * SLOTX;
-        return StarPoint<TX + 2, (TX + 2) * TY>{b + (lz * TY + ly) * BX + lx + H,
-                                                b + Cfg::SX_N + (lz * BY + ly + H) * (TX + 2) + lx + 1,
-                                                b + Cfg::SX_N + Cfg::SY_N + ((lz + H) * TY + ly) * (TX + 2) + lx + 1};
-      } else {
-        return box(o);
-      }
     };
     auto done = [&](int o) {
       if (leave(slot_of(o))) {   // the refill is load number 25 t + o + kSlots: same slot
@@ -404,7 +338,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     };
 
     const double third = 1.0 / 3.0, two_thirds = 2.0 / 3.0;
-    mbar_wait(cfull, (uint32_t)(t & 1));
+    mbar_wait(cfull, (uint32_t)(t & 1), L.err, 0x10080u);
     // ---- point values needed before their own boxes arrive: metric, shift ----------------------------------
     double g[6], gu[6];
 #pragma unroll
@@ -433,59 +367,6 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 
     // ---- o = 0..2: beta^i : d_j beta^i, gtu^{jk} d_j d_k beta^i, d_j (d_k beta^k) ----------------------------
     double db[3][3], lapb[3], gdiv[3];   // db[j][i] = d_j beta^i ; gdiv[j] = d_j d_k beta^k
-#if CHM_PAIR && CHM_TWOPASS == 0
-    {
-      double d1[3][3], d2[3][6], ad[3], Bc[3];
-      StagePre pr[3];
-#pragma unroll
-      for (int i2 = 0; i2 < 3; ++i2) Bc[i2] = cen(V_B + i2);
-      const BoxPoint<BX, BY> p0 = box(0), p1 = box(1), p2 = box(2);
-#pragma unroll
-      for (int i2 = 0; i2 < 3; ++i2) pr[i2] = pre(i2, 0);
-      var_full(p0, C, w, d1[0], d2[0], ad[0]);
-      var_full(p1, C, w, d1[1], d2[1], ad[1]);
-      var_full(p2, C, w, d1[2], d2[2], ad[2]);
-      done(0); done(1); done(2);
-#pragma unroll
-      for (int i2 = 0; i2 < 3; ++i2) {
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-          db[a][i2] = d1[i2][a];
-          gdiv[a] = i2 == 0 ? d2[i2][sym(a, i2)] : gdiv[a] + d2[i2][sym(a, i2)];
-        }
-        lapb[i2] = sdot(gu, d2[i2]);
-        emit(V_BETA + i2, C.sgc * Bc[i2] + ad[i2], pr[i2]);
-      }
-    }
-#else
-    if constexpr (LOOPS & 1) {
-      {
-        const double tb[6] = {C.sgc * cen(V_B + 0), 0.0, C.sgc * cen(V_B + 1), 0.0, C.sgc * cen(V_B + 2), 0.0};
-        tmem_park<6>(park, T_TAB, tb);
-      }
-#pragma unroll 1
-      for (int i2 = 0; i2 < 3; ++i2) {
-        auto p = box(i2);
-        const StagePre pr = pre(i2, 0);
-        double d1[3], d2[6], ad, r2[2];
-        full_var(p, w, i2, i2, d1, d2, ad);
-        tmem_unpark<2>(park, T_TAB + 2 * i2, r2);
-        emit(V_BETA + i2, r2[0] + ad, pr);
-        const double o10[10] = {d1[0], d1[1], d1[2], sdot(gu, d2), d2[0], d2[1], d2[2], d2[3], d2[4], d2[5]};
-        tmem_park<10>(park, T_OUT + 10 * i2, o10);
-      }
-#pragma unroll
-      for (int i2 = 0; i2 < 3; ++i2) {
-        double o10[10];
-        tmem_unpark<10>(park, T_OUT + 10 * i2, o10);
-        lapb[i2] = o10[3];
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-          db[a][i2] = o10[a];
-          gdiv[a] = i2 == 0 ? o10[4 + sym(a, i2)] : gdiv[a] + o10[4 + sym(a, i2)];
-        }
-      }
-    } else
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2) {
       const double Bc = cen(V_B + i2);
@@ -498,7 +379,6 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       lapb[i2] = sdot(gu, d2);
       emit(V_BETA + i2, C.sgc * Bc + ad, pr);
     }
-#endif
     double divb = (db[0][0] + db[1][1]) + db[2][2];
     if constexpr (PARK) {   // needed again only by the Gt^i right-hand side (sections 21..23)
       const double lg[6] = {lapb[0], lapb[1], lapb[2], gdiv[0], gdiv[1], gdiv[2]};
@@ -510,69 +390,6 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 #pragma unroll
     for (int s = 0; s < 6; ++s) At[s] = cen(V_AT + s);
     done_cen();
-#if CHM_PAIR && CHM_TWOPASS == 0
-#pragma unroll
-    for (int pp = 0; pp < 3; ++pp) {
-      constexpr int I2[6] = {0, 0, 0, 1, 1, 2}, J2[6] = {0, 1, 2, 1, 2, 2};   // packed index -> (i, j)
-      const int sa = 2 * pp, sb = 2 * pp + 1;
-      const BoxPoint<BX, BY> pa = box(3 + sa), pb = box(3 + sb);
-      const StagePre pra = pre(3 + sa, 0), prb = pre(3 + sb, 0);
-      double d1[2][3], d2[2][6], ad[2];
-      var_full(pa, C, w, d1[0], d2[0], ad[0]);
-      var_full(pb, C, w, d1[1], d2[1], ad[1]);
-      done(3 + sa); done(3 + sb);
-#pragma unroll
-      for (int h2 = 0; h2 < 2; ++h2) {
-        const int s = 2 * pp + h2, i2 = I2[s], j2 = J2[s];
-        dg[0][s] = d1[h2][0]; dg[1][s] = d1[h2][1]; dg[2][s] = d1[h2][2];
-        Rt[s] = -0.5 * sdot(gu, d2[h2]);
-        double lie;
-#pragma unroll
-        for (int k2 = 0; k2 < 3; ++k2) {
-          const double c = g[sym(i2, k2)] * db[j2][k2] + g[sym(j2, k2)] * db[i2][k2];
-          lie = k2 == 0 ? c : lie + c;
-        }
-        emit(V_GT + s, (lie - two_thirds * g[s] * divb) - 2.0 * alpha * At[s] + ad[h2], h2 == 0 ? pra : prb);
-      }
-    }
-#else
-    if constexpr (LOOPS & 2) {
-      {
-        double tb[12];
-#pragma unroll
-        for (int i2 = 0; i2 < 3; ++i2)
-#pragma unroll
-          for (int j2 = i2; j2 < 3; ++j2) {
-            const int s = sym(i2, j2);
-            double lie;
-#pragma unroll
-            for (int k2 = 0; k2 < 3; ++k2) {
-              const double c = g[sym(i2, k2)] * db[j2][k2] + g[sym(j2, k2)] * db[i2][k2];
-              lie = k2 == 0 ? c : lie + c;
-            }
-            tb[2 * s] = (lie - two_thirds * g[s] * divb) - 2.0 * alpha * At[s];
-            tb[2 * s + 1] = 0.0;
-          }
-        tmem_park<12>(park, T_TAB, tb);
-      }
-#pragma unroll 1
-      for (int s = 0; s < 6; ++s) {
-        auto p = box(3 + s);
-        const StagePre pr = pre(3 + s, 0);
-        double d1[3], d2[6], ad, r2[2];
-        full_var(p, w, 3 + s, 3 + s, d1, d2, ad);
-        tmem_unpark<2>(park, T_TAB + 2 * s, r2);
-        emit(V_GT + s, r2[0] + ad, pr);
-        const double d4[4] = {d1[0], d1[1], d1[2], -0.5 * sdot(gu, d2)};
-        tmem_park<4>(park, T_OUT + 4 * s, d4);
-      }
-#pragma unroll
-      for (int s = 0; s < 6; ++s) {
-        double d4[4];
-        tmem_unpark<4>(park, T_OUT + 4 * s, d4);
-        dg[0][s] = d4[0]; dg[1][s] = d4[1]; dg[2][s] = d4[2]; Rt[s] = d4[3];
-      }
-    } else
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2)
 #pragma unroll
@@ -597,8 +414,6 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
         }
         emit(V_GT + s, (lie - two_thirds * g[s] * divb) - 2.0 * alpha * At[s] + ad, pr);
       }
-
-#endif
 
     // ---- Christoffels: Cl[k][s(i,j)] = Gamma~_kij, Cu[k][s] = Gamma~^k_ij, Gn[k] = gtu^{ij} Gamma~^k_ij ----
     double Cu[3][6], Gn[3];
@@ -673,30 +488,9 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     }
     // ---- o = 9..11: Gt^k : R~_ij += 1/2 (gt_ki d_j Gt^k + gt_kj d_i Gt^k); advection kept for the end ------
     double adG[3];
-    if constexpr (LOOPS & 4) {
-#pragma unroll 1
-      for (int k2 = 0; k2 < 3; ++k2) {
-        auto p = sbox(9 + k2);
-        double d4[4];
-        if (ORDER == 4) var_d1_ad(p, C, w, d4, d4[3]); else var_d1_ad8(p, C, w, d4, d4[3]);
-        done(9 + k2);
-        tmem_park<4>(park, T_OUT + 4 * k2, d4);
-      }
-#pragma unroll
-      for (int k2 = 0; k2 < 3; ++k2) {
-        double d4[4];
-        tmem_unpark<4>(park, T_OUT + 4 * k2, d4);
-        adG[k2] = d4[3];
-#pragma unroll
-        for (int i2 = 0; i2 < 3; ++i2)
-#pragma unroll
-          for (int j2 = i2; j2 < 3; ++j2)
-            Rt[sym(i2, j2)] += 0.5 * (g[sym(k2, i2)] * d4[j2] + g[sym(k2, j2)] * d4[i2]);
-      }
-    } else
 #pragma unroll
     for (int k2 = 0; k2 < 3; ++k2) {
-      auto p = sbox(9 + k2);
+      auto p = box(9 + k2);
       double d1[3];
       if (ORDER == 4) var_d1_ad(p, C, w, d1, adG[k2]); else var_d1_ad8(p, C, w, d1, adG[k2]);
       done(9 + k2);
@@ -802,7 +596,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     // ---- o = 14: K -------------------------------------------------------------------------------------------
     double dK[3];
     {
-      auto p = sbox(14);
+      auto p = box(14);
       const StagePre pr = pre(14, 0);
       double ad;
       if (ORDER == 4) var_d1_ad(p, C, w, dK, ad); else var_d1_ad8(p, C, w, dK, ad);
@@ -821,7 +615,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
         for (int b = 0; b < 3; ++b) db[a][b] = t10[3 * a + b];
       divb = t10[9];
     }
-    if constexpr ((ORDER == 8 || CHM_ATLOOP) && Cfg::TWOPASS && TX * TY == 64) {
+    if constexpr (Cfg::TWOPASS && TX * TY == 64) {
       // The kernel is bound by instruction fetch at 8th order (150 KB of code), so the six advection stencils are
       // ONE loop body.  The box-independent part of each right-hand side goes through a per-thread table laid
       // over this thread's OWN z-plane of the shared first-derivative buffers (components 0..2 in the buffer of
@@ -856,7 +650,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
         }
 #pragma unroll 1
       for (int s = 0; s < 6; ++s) {
-        auto p = sbox(15 + s);
+        auto p = box(15 + s);
         const StagePre pr = pre(15 + s, 0);
         const double ad = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
         const double rest = *tab(s);
@@ -870,7 +664,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 #pragma unroll
         for (int j2 = i2; j2 < 3; ++j2) {
           const int s = sym(i2, j2);
-          auto p = sbox(15 + s);
+          auto p = box(15 + s);
           const StagePre pr = pre(15 + s, 0);
           const double ad = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
           done(15 + s);
@@ -900,41 +694,9 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 #pragma unroll
       for (int a = 0; a < 3; ++a) { Gn[a] = g4[a]; dchi[a] = dc[a]; dal[a] = dc[3 + a]; }
     }
-    if constexpr (LOOPS & 8) {
-      {
-        double tb[6];
-#pragma unroll
-        for (int i2 = 0; i2 < 3; ++i2) {
-          double r = lapb[i2];
-          double t2 = sdot(Cu[i2], Au);
-#pragma unroll
-          for (int j2 = 0; j2 < 3; ++j2) {
-            r += third * gu[sym(i2, j2)] * gdiv[j2];
-            t2 -= two_thirds * gu[sym(i2, j2)] * dK[j2] + 1.5 * ichi * Au[sym(i2, j2)] * dchi[j2];
-            r -= 2.0 * Au[sym(i2, j2)] * dal[j2] + Gn[j2] * db[j2][i2];
-          }
-          r += 2.0 * alpha * t2 + two_thirds * Gn[i2] * divb;
-          tb[2 * i2] = r;
-          tb[2 * i2 + 1] = adG[i2];
-        }
-        tmem_park<6>(park, T_TAB, tb);
-      }
-#pragma unroll 1
-      for (int i2 = 0; i2 < 3; ++i2) {
-        auto p = sbox(21 + i2);
-        const StagePre prG = pre(21 + i2, 0), prB = pre(21 + i2, 1);
-        const double Bi = p.at(0, 0, 0);
-        const double adB = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
-        done(21 + i2);
-        double r2[2];
-        tmem_unpark<2>(park, T_TAB + 2 * i2, r2);
-        emit(V_GAM + i2, r2[0] + r2[1], prG);
-        emit(V_B + i2, (r2[0] - C.eta * Bi) + adB, prB);
-      }
-    } else
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2) {
-      auto p = sbox(21 + i2);
+      auto p = box(21 + i2);
       const StagePre prG = pre(21 + i2, 0), prB = pre(21 + i2, 1);
       const double Bi = p.at(0, 0, 0);
       const double adB = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
@@ -955,7 +717,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 
     // ---- o = 24: A (inert slot, dissipation only) -----------------------------------------------------------------
     {
-      auto p = sbox(24);
+      auto p = box(24);
       const StagePre pr = pre(24, 0);
       const double f0 = p.at(0, 0, 0);
       double rA;
@@ -989,11 +751,45 @@ static EncodeTiledFn encode_fn() {
   return fn;
 }
 
+// What one launch of bssn_tma_kernel<TX,TY,TZ,MODE,ORDER> issues, for the validator: every section's box and
+// operand loads with the mbarrier byte count the kernel announces for it (one "barrier" entry per section, one for
+// the point-value tiles).  xo: Layout::xo (decides the parity of the x coordinates).
+template <int TX, int TY, int TZ, int ORDER>
+static TmaPlan bssn_plan(int mode, int xo) {
+  using Cfg = TmaCfg<TX, TY, TZ, ORDER>;
+  char name[64];
+  snprintf(name, sizeof name, "bssn_tma_kernel<%d,%d,%d,order %d>", TX, TY, TZ, ORDER);
+  TmaPlan p;
+  p.kernel = name;
+  p.smem_bytes = Cfg::SMEM;
+  p.threads = Cfg::THREADS;
+  p.tmem_cols = Cfg::PARK ? 512 : 0;
+  p.barrier_off = (size_t)Cfg::bar_off() * 8;
+  p.n_barriers = 2 * (Cfg::NS + 1);
+  const int nops = mode == MODE_RHS ? 0 : (mode == MODE_FIRST ? 1 : 2);
+  const int par_box = (xo - Cfg::H) & 1, par_tile = (xo - 1) & 1;
+  for (int o = 0; o < 25; ++o) {
+    const int slot = o % Cfg::NS, v0 = emit_var(o, 0), v1 = emit_var(o, 1), nem = (v0 >= 0) + (v1 >= 0);
+    p.expect.push_back(Cfg::BOX_BYTES + (uint32_t)(nops * nem) * Cfg::TILE_BYTES);
+    p.loads.push_back({"halo box", (size_t)Cfg::box_off(slot) * 8, {(uint32_t)Cfg::BX, (uint32_t)Cfg::BY, (uint32_t)Cfg::BZ, 1}, o, par_box});
+    for (int n = 0; n < 4; ++n) {
+      const bool has = (n < 2 ? v0 >= 0 : v1 >= 0) && ((n & 1) ? nops == 2 : nops >= 1);
+      if (has) p.loads.push_back({"RK operand tile", (size_t)Cfg::op_off(slot, n) * 8, {(uint32_t)(TX + 2), (uint32_t)TY, (uint32_t)TZ, 1}, o, par_tile});
+    }
+  }
+  p.expect.push_back((uint32_t)kCenVars * Cfg::TILE_BYTES);
+  for (int grp = 0; grp < 3; ++grp)
+    p.loads.push_back({"point-value tiles", (size_t)Cfg::cen_off(grp) * 8, {(uint32_t)(TX + 2), (uint32_t)TY, (uint32_t)TZ, 7}, 25, par_tile});
+  return p;
+}
+
 template <int TX, int TY, int TZ, int MODE, int ORDER>
 static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
   using Cfg = TmaCfg<TX, TY, TZ, ORDER>;
   auto kern = bssn_tma_kernel<TX, TY, TZ, MODE, ORDER>;
   if (a) return cudaFuncGetAttributes(a, kern);
+  // nothing is launched unless the validator accepts what this instance will issue on this layout
+  if (!launch_allowed(bssn_plan<TX, TY, TZ, ORDER>(MODE, L.xo), L, st->in, L.xo - Cfg::H, Cfg::H)) return cudaErrorInvalidValue;
   EncodeTiledFn enc = encode_fn();
   if (!enc) return cudaErrorNotSupported;
   CUtensorMap tm, tmCen, tmU, tmS;
@@ -1015,27 +811,13 @@ static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, 
   // MODE_SSP reads U and the evaluated state itself
   const double* ubase = st->mode == MODE_FIRST || st->mode == MODE_RHS ? st->in : st->U;
   const double* sbase = st->mode == MODE_MID || st->mode == MODE_LAST ? st->S : st->in;
+  if (!ubase || !sbase || (reinterpret_cast<uintptr_t>(ubase) | reinterpret_cast<uintptr_t>(sbase)) % 128) return cudaErrorInvalidValue;
   if (tile_map(&tmCen, st->in, 7) != CUDA_SUCCESS || tile_map(&tmU, ubase, 1) != CUDA_SUCCESS ||
       tile_map(&tmS, sbase, 1) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
-  CUtensorMap tmX = tm, tmY = tm, tmZ = tm;   // star staging: the three slab boxes of the evaluated state
-  if (Cfg::STAR) {
-    auto slab_map = [&](CUtensorMap* m, int bx, int by, int bz) {
-      cuuint32_t b[4] = {(cuuint32_t)bx, (cuuint32_t)by, (cuuint32_t)bz, 1};
-      return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(st->in), dims, strides, b, estr,
-                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    };
-    if (slab_map(&tmX, Cfg::BX, TY, TZ) != CUDA_SUCCESS || slab_map(&tmY, TX + 2, Cfg::BY, TZ) != CUDA_SUCCESS ||
-        slab_map(&tmZ, TX + 2, TY, Cfg::BZ) != CUDA_SUCCESS)
-      return cudaErrorInvalidValue;
-  }
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  // per launch: function attributes are per device, and the call is cheap
+  cudaError_t ea = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
+  if (ea != cudaSuccess) return ea;
   int dev = 0, sms = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -1046,7 +828,7 @@ static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, 
   if (blocks_per_sm < 1) blocks_per_sm = 1;
   const int grid = ntiles < sms * blocks_per_sm ? ntiles : sms * blocks_per_sm;
   const int cy = L.col_rows / TY > 0 ? L.col_rows / TY : 1;   // tile rows per traversal column
-  kern<<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, tmX, tmY, tmZ, L, C, *st, ntx, nty, ntz, cy);
+  kern<<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, L, C, *st, ntx, nty, ntz, cy);
   return cudaGetLastError();
 }
 
@@ -1068,12 +850,9 @@ static cudaError_t tma_dispatch(int order, int tile, const Layout& L, const Coef
   switch (tile) {
     case 0: return tma_go<16, 4, 4>(L, C, st, s, a);
     case 1: return tma_go<16, 8, 2>(L, C, st, s, a);
-    case 2: return tma_go<8, 8, 4>(L, C, st, s, a);
-    case 3: return tma_go<8, 4, 8>(L, C, st, s, a);
-    case 4: return tma_go<16, 2, 8>(L, C, st, s, a);
-    case 5: return tma_go<16, 4, 2>(L, C, st, s, a);
-    case 9: return tma_go<16, 4, 6>(L, C, st, s, a);     // 12 warps, 168 registers, tensor-memory parking
-    case 10: return tma_go<16, 6, 4>(L, C, st, s, a);
+    case 2: return tma_go<8, 4, 8>(L, C, st, s, a);
+    case 3: return tma_go<16, 2, 8>(L, C, st, s, a);
+    case 4: return tma_go<16, 4, 2>(L, C, st, s, a);
   }
   return cudaErrorInvalidValue;
 }
@@ -1081,6 +860,19 @@ static cudaError_t tma_dispatch(int order, int tile, const Layout& L, const Coef
 cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s) {
   return tma_dispatch(order, tile, L, C, &st, s, nullptr);
 }
+void plans_bssn_fused(std::vector<TmaPlan>& out) {
+  for (int mode = MODE_RHS; mode <= MODE_SSP; ++mode)
+    for (int g = 3; g <= 6; ++g) {   // every ghost width the layout rule gives a different xo for
+      const int xo = ((g - 3) & 1) ? g + 1 : g;
+      out.push_back(bssn_plan<16, 4, 4, 4>(mode, xo));
+      out.push_back(bssn_plan<16, 8, 2, 4>(mode, xo));
+      out.push_back(bssn_plan<8, 4, 8, 4>(mode, xo));
+      out.push_back(bssn_plan<16, 2, 8, 4>(mode, xo));
+      out.push_back(bssn_plan<16, 4, 2, 4>(mode, xo));
+      if (g >= 5) out.push_back(bssn_plan<16, 4, 4, 8>(mode, xo));
+    }
+}
+
 cudaError_t kernel_info_bssn_fused(int order, int tile, cudaFuncAttributes* a) {
   Layout L{}; Coef C{};
   return tma_dispatch(order, tile, L, C, nullptr, 0, a);

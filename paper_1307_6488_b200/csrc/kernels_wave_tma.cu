@@ -8,6 +8,7 @@
 // whose returned state tells the last arriver, see bssn_tma.cuh); the last warp out issues the slot's next load.
 #include "bssn_tma.cuh"
 #include "stencils.cuh"
+#include "tma_check.cuh"
 
 namespace chm {
 
@@ -86,7 +87,7 @@ wave_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
       const int first = nplanes < NP ? nplanes : NP;               // fill the whole ring
       for (int p = 0; p < first; ++p) {
         const int m = nbase + p;
-        if (m >= NP) mbar_wait(&empty[m % NP], (uint32_t)(((m / NP) - 1) & 1));
+        if (m >= NP) mbar_wait(&empty[m % NP], (uint32_t)(((m / NP) - 1) & 1), L.err, 0x20001u);
         issue(p);
       }
     }
@@ -105,10 +106,10 @@ wave_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
       const int pc = (k - k0) + R;                                  // centre plane number inside the item
       // wait for the newest plane this step needs (older ones were waited for in earlier steps / below)
       if (k == k0) {
-        for (int p = 0; p <= pc + R; ++p) { const int m = nbase + p; mbar_wait(&full[m % NP], (uint32_t)((m / NP) & 1)); }
+        for (int p = 0; p <= pc + R; ++p) { const int m = nbase + p; mbar_wait(&full[m % NP], (uint32_t)((m / NP) & 1), L.err, 0x20002u); }
       } else {
         const int m = nbase + pc + R;
-        mbar_wait(&full[m % NP], (uint32_t)((m / NP) & 1));
+        mbar_wait(&full[m % NP], (uint32_t)((m / NP) & 1), L.err, 0x20003u);
       }
       const double* zp[2 * R + 1];
 #pragma unroll
@@ -177,6 +178,25 @@ static WvEncodeFn wv_encode_fn() {
   return fn;
 }
 
+// what one launch of wave_tma_kernel issues, for the validator: one plane box per ring slot
+template <int ORDER, bool KO, int TX, int TY, int NV>
+static TmaPlan wv_plan(int xo) {
+  using K = wv::Cfg<ORDER, KO, TX, TY, NV>;
+  char name[80];
+  snprintf(name, sizeof name, "wave_tma_kernel<order %d,ko %d,%dx%d,%d vars>", ORDER, (int)KO, TX, TY, NV);
+  TmaPlan p;
+  p.kernel = name;
+  p.smem_bytes = K::SMEM;
+  p.threads = K::THREADS;
+  p.barrier_off = (size_t)K::NP * K::SLOT * 8;
+  p.n_barriers = 2 * K::NP;
+  for (int slot = 0; slot < K::NP; ++slot) {
+    p.expect.push_back(K::BYTES);
+    p.loads.push_back({"plane box", (size_t)slot * K::SLOT * 8, {(uint32_t)K::ROW, (uint32_t)K::COLS, 1, (uint32_t)NV}, slot, (xo - K::R) & 1});
+  }
+  return p;
+}
+
 template <int ORDER, bool KO, int TX, int TY, int ZC, int NV = 2>
 static cudaError_t wv_go(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
   using K = wv::Cfg<ORDER, KO, TX, TY, NV>;
@@ -184,6 +204,7 @@ static cudaError_t wv_go(const Layout& L, const Coef& C, const Stage* st, cudaSt
   else {
   auto kern = wave_tma_kernel<ORDER, KO, TX, TY, ZC, NV>;
   if (a) return cudaFuncGetAttributes(a, kern);
+  if (L.nvars != NV || !launch_allowed(wv_plan<ORDER, KO, TX, TY, NV>(L.xo), L, st->in, L.xo - K::R, K::R)) return cudaErrorInvalidValue;
   WvEncodeFn enc = wv_encode_fn();
   if (!enc) return cudaErrorNotSupported;
   CUtensorMap tm;
@@ -195,12 +216,9 @@ static cudaError_t wv_go(const Layout& L, const Coef& C, const Stage* st, cudaSt
           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SMEM);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  // per launch: function attributes are per device, and the call is cheap
+  cudaError_t ea = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SMEM);
+  if (ea != cudaSuccess) return ea;
   int dev = 0, sms = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -273,6 +291,26 @@ static cudaError_t wv_dispatch(int order, bool ko, int which, const Layout& L, c
   if (order == 4) return ko ? wv_tile<4, true>(which, L, C, st, s, a) : wv_tile<4, false>(which, L, C, st, s, a);
   if (order == 8) return ko ? wv_tile<8, true>(which, L, C, st, s, a) : wv_tile<8, false>(which, L, C, st, s, a);
   return cudaErrorInvalidValue;
+}
+
+template <int ORDER, bool KO>
+static void wv_plans_of(std::vector<TmaPlan>& out, int xo) {
+  out.push_back(wv_plan<ORDER, KO, 32, 16, 2>(xo));
+  out.push_back(wv_plan<ORDER, KO, 64, 8, 2>(xo));
+  if (wv::Cfg<ORDER, KO, 16, 8, 5>::FITS) out.push_back(wv_plan<ORDER, KO, 16, 8, 5>(xo));
+  if (wv::Cfg<ORDER, KO, 16, 16, 5>::FITS) out.push_back(wv_plan<ORDER, KO, 16, 16, 5>(xo));
+  if (wv::Cfg<ORDER, KO, 32, 8, 5>::FITS) out.push_back(wv_plan<ORDER, KO, 32, 8, 5>(xo));
+}
+// every instance, on every ghost width wave_tma_ok admits (xo = g for the wave systems)
+void plans_wave_tma(std::vector<TmaPlan>& out) {
+  for (int g = 2; g <= 6; ++g) {
+    Layout L{};
+    L.xo = g; L.g = g;
+    if (wave_tma_ok(L, 4, false)) wv_plans_of<4, false>(out, g);
+    if (wave_tma_ok(L, 4, true)) wv_plans_of<4, true>(out, g);
+    if (wave_tma_ok(L, 8, false)) wv_plans_of<8, false>(out, g);
+    if (wave_tma_ok(L, 8, true)) wv_plans_of<8, true>(out, g);
+  }
 }
 
 cudaError_t launch_wave_tma(const Layout& L, const Coef& C, int order, int which, const Stage& st, cudaStream_t s) {

@@ -47,3 +47,16 @@ def test_product_arm_refuses_to_run_without_a_gpu():
     r = _run("--steps", "1", "--warmup", "0")
     assert r.returncode != 0
     assert "no CUDA device" in (r.stderr + r.stdout)
+
+
+def test_metric_string_is_baseline_jsons_byte_for_byte():
+    """a mechanical comparison of the bench line with BASELINE.json must not trip on the metric name"""
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("bench_mod", os.path.join(ROOT, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    base = json.load(open(os.path.join(ROOT, "BASELINE.json")))
+    assert bench.METRIC == base["metric"]
+    # constants the roofline objects print are labelled as constants, with the capture they come from
+    assert os.path.exists(os.path.join(ROOT, bench.NCU_TRAFFIC_SOURCE))
+    assert "constant" in bench.FLOPS_SOURCE

@@ -32,6 +32,31 @@ def relerr(a, b):
     return worst
 
 
+BG_SLOTS = (0, 1, 4, 6, 17)      # chi, gt11, gt22, gt33, alpha: the slots whose flat-space value is 1
+ULP1 = 2.220446049250313e-16
+
+
+def relerr_bg(a, b):
+    """DESIGN.md reading S11b: the O(1) slots carry a perturbation of 1e-10..1e-4 on a background of 1, where S11's
+    denominator max|oracle| = 1 cannot see an error the size of the perturbation.  Second norm on those slots,
+    background-subtracted (both subtractions are exact, Sterbenz): max|(a-1) - (b-1)| / max|b-1|.  Returns (worst
+    ratio, its tolerance): the evolved perturbation must agree to the north_star's 1e-10 or to 8 ulp of the O(1)
+    value it is stored on (a value of 1 + 1e-10 holds its perturbation to 2e-6 only), whichever is larger."""
+    worst, tol = 0.0, 0.0
+    for v in BG_SLOTS:
+        amp = max(np.max(np.abs(b[v] - 1.0)), 1e-300)
+        r = np.max(np.abs((a[v] - 1.0) - (b[v] - 1.0))) / amp
+        if r >= worst:
+            worst, tol = r, max(1e-10, 8 * ULP1 / amp)
+    return worst, tol
+
+
+def assert_bssn_close(got, want, tol):
+    assert relerr(got, want) < tol
+    r, t = relerr_bg(got, want)
+    assert r < t, (r, t)
+
+
 def to_padded(h, packed):
     import torch
     st = h.new_state()
@@ -91,7 +116,7 @@ def test_wave_rhs_all_tiles(chem, oracle, order, g, eps, dims):
     want = oracle_rhs(oracle, 0, u, g, order, dx, eps_diss=eps)
     h = chem.Chemora(nx, ny, nz, g, order, 0, dx)
     h.set_param("eps_diss", eps)
-    for tile in range(chem.NUM_TILES):
+    for tile in chem.variants(chem.SYS_WAVE, order):
         h.set_variant(1, tile)
         assert relerr(gpu_rhs(h, u), want) < TOL_RHS, tile
     h.destroy()
@@ -210,7 +235,7 @@ def test_bssn_rhs_all_variants_and_tiles(chem, oracle, data):
     h = chem.Chemora(nx, ny, nz, 3, 4, 1, dx)
     h.set_param("eps_diss", eps)
     for fused in (1, 0):
-        for tile in range(chem.NUM_TILES):
+        for tile in chem.variants(chem.SYS_BSSN, 4, fused):
             h.set_variant(fused, tile)
             got = gpu_rhs(h, u)
             assert relerr(got, want) < TOL_RHS, (fused, tile)
@@ -258,7 +283,29 @@ def test_bssn_rk4_10_steps_small(chem, oracle, fused):
     for _ in range(10):
         h.rk4_step(dt)
     st = oracle.rk4(1, oracle.with_ghosts(u0, 3), 3, 4, dx, dt, oracle.params(eps_diss=eps), 10)
-    assert relerr(h.get_state(), oracle.interior(st, 3)) < TOL_BSSN_10_STEPS
+    assert_bssn_close(h.get_state(), oracle.interior(st, 3), TOL_BSSN_10_STEPS)
+    h.destroy()
+
+
+@pytest.mark.parametrize("data", ["gaussians", "strong"])
+def test_bssn_rk4_10_steps_every_slot_moves(chem, oracle, data):
+    """10 RK4 steps on data where every slot evolves by far more than 1e-10 of its size (Gaussians of amplitude 1e-4;
+    0.02-amplitude strong field), every fused tile id and one split tile: 1e-10 is then meaningful on all 25 slots"""
+    nx, ny, nz = 24, 20, 18
+    u0 = inputs.bssn_gaussians(nx, ny, nz, width_cells=4.0) if data == "gaussians" else \
+        inputs.bssn_minkowski(nx, ny, nz) + 0.02 * np.random.default_rng(23).uniform(-1, 1, size=(25, nz, ny, nx))
+    dx, dt, eps = 0.05, 0.0125, 0.1
+    st = oracle.rk4(1, oracle.with_ghosts(u0, 3), 3, 4, dx, dt, oracle.params(eps_diss=eps), 10)
+    want = oracle.interior(st, 3)
+    assert all(np.max(np.abs(want[v] - u0[v])) > 1e-8 * max(np.max(np.abs(want[v])), 1e-300) for v in range(24))
+    h = chem.Chemora(nx, ny, nz, 3, 4, 1, dx)
+    h.set_param("eps_diss", eps)
+    for fused, tile in [(1, t) for t in chem.variants(chem.SYS_BSSN, 4)] + [(0, 1)]:
+        h.set_variant(fused, tile)
+        h.set_state(u0)
+        for _ in range(10):
+            h.rk4_step(dt)
+        assert_bssn_close(h.get_state(), want, TOL_BSSN_10_STEPS)
     h.destroy()
 
 
@@ -273,7 +320,7 @@ def test_bssn_config2_full_size_10_steps(chem, oracle):
     for _ in range(10):
         h.rk4_step(0.25 * dx)
     st = oracle.rk4(1, oracle.with_ghosts(u0, 3), 3, 4, dx, 0.25 * dx, oracle.params(eps_diss=c["eps_diss"]), 10)
-    assert relerr(h.get_state(), oracle.interior(st, 3)) < TOL_BSSN_10_STEPS
+    assert_bssn_close(h.get_state(), oracle.interior(st, 3), TOL_BSSN_10_STEPS)
     h.destroy()
 
 
@@ -285,8 +332,12 @@ def test_autotune_and_kernel_info(chem):
     h.set_state(u)
     fused, tile, ms = h.autotune()
     nt = chem.NUM_TILES
-    assert fused in (0, 1) and 0 <= tile < nt
-    assert all(m > 0 for m in ms[nt:]) and all(m > 0 for m in ms[:6])   # every fused id, the six split tiles
+    assert fused == 1 and tile in chem.variants(chem.SYS_BSSN, 4)
+    assert all((ms[nt + t] > 0) == (t < 5) for t in range(nt))          # the five fused ids, nothing else
+    assert all(m < 0 for m in ms[:nt])                                  # split variant: only on request
+    h.set_param("autotune_split", 1)
+    fused2, tile2, ms2 = h.autotune()
+    assert all(m > 0 for m in ms2[:6]) and fused2 == 1                  # the six split tiles timed; never the pick
     assert (fused, tile) == h.get_variant()
     assert np.array_equal(h.get_state(), u)        # U is not modified by the sweep
     info = h.kernel_info()
@@ -334,7 +385,7 @@ def test_enforce_constraints(chem, oracle):
     w.destroy()
 
 
-@pytest.mark.parametrize("tile", [0, 1, 4, 6, 9])
+@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4])
 def test_bssn_rk3_with_enforcement_10_steps(chem, oracle, tile):
     """the paper's integrator (RK3) with constraint enforcement after every step, configs[2] data at 24x20x18"""
     nx, ny, nz = 24, 20, 18
@@ -348,7 +399,7 @@ def test_bssn_rk3_with_enforcement_10_steps(chem, oracle, tile):
         h.rk3_step(dt)
         h.enforce_constraints()
     st = oracle.rk3(1, oracle.with_ghosts(u0, 3), 3, 4, dx, dt, oracle.params(eps_diss=eps), 10, True)
-    assert relerr(h.get_state(), oracle.interior(st, 3)) < TOL_BSSN_10_STEPS
+    assert_bssn_close(h.get_state(), oracle.interior(st, 3), TOL_BSSN_10_STEPS)
     h.destroy()
 
 
@@ -399,7 +450,7 @@ def test_bssn_o8_rk4_10_steps_and_rk3_enforced(chem, oracle, fused):
     for _ in range(10):
         h.rk4_step(dt)
     st = oracle.rk4(1, oracle.with_ghosts(u0, g), g, 8, dx, dt, oracle.params(eps_diss=eps), 10)
-    assert relerr(h.get_state(), oracle.interior(st, g)) < TOL_BSSN_10_STEPS
+    assert_bssn_close(h.get_state(), oracle.interior(st, g), TOL_BSSN_10_STEPS)
     h.set_state(u0)
     for _ in range(5):
         h.rk3_step(dt)
@@ -441,26 +492,6 @@ def test_bssn_o8_ko9(chem, oracle, fused):
             b.set_param("ko_order", 9)
         b.set_param("ko_order", 5)
         b.destroy()
-
-
-@pytest.mark.parametrize("order,g,dims", [(4, 3, (37, 21, 19)), (4, 3, (6, 9, 7)), (8, 5, (21, 14, 11))])
-def test_x_ghost_images_are_bit_identical(chem, order, g, dims):
-    """tuning switch x_images: the fused kernel writes the x-ghost images itself and the fills skip those columns;
-    RK4 and RK3 give the same bits either way (ragged tiles, nx = 2g, 8th order)"""
-    nx, ny, nz = dims
-    u0 = strong_field(nx, ny, nz, seed=77)
-    h = chem.Chemora(nx, ny, nz, g, order, 1, 0.05)
-    h.set_param("eps_diss", 0.1)
-    res = []
-    for x in (0, 1):
-        h.set_param("x_images", x)
-        h.set_state(u0)
-        for _ in range(2):
-            h.rk4_step(0.0125)
-            h.rk3_step(0.0125)
-        res.append(h.get_state())
-    assert np.array_equal(res[0], res[1])
-    h.destroy()
 
 
 @pytest.mark.parametrize("system,order,g,rk3", [(1, 4, 3, False), (1, 4, 3, True), (0, 8, 4, False), (2, 4, 3, False),

@@ -276,3 +276,72 @@ def test_advection_side_follows_sign_of_shift(oracle, axis, sign):
             assert got == pytest.approx(sign * b * sign / (12 * h), rel=1e-13)
         else:
             assert got == 0.0
+
+
+# ------------------------------------------------------- S5: advection of the gauge variables (task 2)
+def _up_symbol(theta, sign, order, h):
+    """Fourier symbol of the one-sided advection stencil of reading S2 on e^{i theta j}: offsets -1..+3 (O4) or
+    -3..+5 (O8) for a positive shift, the mirror image (coefficients negated) for a negative one."""
+    if order == 4:
+        off, c, den = np.arange(-1, 4), np.array([-3.0, -10.0, 18.0, -6.0, 1.0]), 12.0
+    else:
+        off, c, den = np.arange(-3, 6), np.array([-5.0, 60.0, -420.0, -378.0, 1050.0, -420.0, 140.0, -30.0, 3.0]), 840.0
+    if sign < 0:
+        off, c = -off, -c
+    return np.sum(c * np.exp(1j * theta * off)) / (den * h)
+
+
+def _d2_symbol(theta, order, h):
+    if order == 4:
+        return (-30.0 + 32.0 * np.cos(theta) - 2.0 * np.cos(2 * theta)) / (12.0 * h * h)
+    return (-14350.0 + 2 * (8064.0 * np.cos(theta) - 1008.0 * np.cos(2 * theta) + 128.0 * np.cos(3 * theta)
+                            - 9.0 * np.cos(4 * theta))) / (5040.0 * h * h)
+
+
+@pytest.mark.parametrize("order,g", [(4, 3), (8, 5)])
+@pytest.mark.parametrize("axis", [0, 1, 2])
+@pytest.mark.parametrize("sign", [+1.0, -1.0])
+def test_gauge_advection_closed_form(oracle, order, g, axis, sign):
+    """Flat space, uniform shift beta^axis = +-c, one Fourier mode (along `axis`) in alpha, then in each beta^i, then
+    in each B^i: every term of the gauge right-hand sides (slots 17..23, reading S5) is then a closed form --
+        d_t alpha = c D^up alpha + KO;   d_t beta^i = 3/4 B^i + beta^k D^up_k beta^i + KO;
+        d_t B^i = [d_j d_j beta^i + 1/3 d_i d_k beta^k] - eta B^i + c D^up B^i + KO
+    with D^up's symbol (one-sided, side by the sign of the shift), the centred second-derivative symbol and
+    -(eps/h) sin^6(theta/2) for the dissipation.  A dropped adv(21+a), an advection of B^i with another slot, the
+    wrong side or a wrong axis all fail here (they pass O4..O8, where the shift is zero, linear or only the tensor
+    slots are checked)."""
+    n, h, c, A, eps, eta, sgc = 10, 0.05, 0.3, 1e-3, 0.1, 1.3, 0.6
+    m, phase = 3, 0.7
+    theta = 2 * np.pi * m / n
+    idx = np.arange(n)
+    shape = [1, 1, 1]
+    shape[2 - axis] = n                      # arrays are [z, y, x]
+    wave = np.cos(theta * idx + phase).reshape(shape) * np.ones((n, n, n))
+    up, d2 = _up_symbol(theta, sign, order, h), _d2_symbol(theta, order, h)
+    ko = -(eps / h) * np.sin(theta / 2) ** 6
+
+    def apply(symbol):                       # symbol applied to A cos(theta j + phase)
+        z = A * symbol * np.exp(1j * (theta * idx + phase))
+        return z.real.reshape(shape) * np.ones((n, n, n))
+
+    for slot in [17] + [18 + i for i in range(3)] + [21 + i for i in range(3)]:
+        u = inputs.bssn_minkowski(n, n, n)
+        u[18 + axis] = sign * c
+        u[slot] = u[slot] + A * wave
+        st = oracle.fill_ghosts(oracle.with_ghosts(u, g), g)
+        r = oracle.interior(oracle.rhs(oracle.SYS_BSSN, st, g, order, h,
+                                       oracle.params(eps_diss=eps, eta=eta, shift_gamma_coeff=sgc)), g)
+        want = {v: np.zeros((n, n, n)) for v in range(17, 24)}
+        if slot == 17:
+            want[17] = sign * c * apply(up) + apply(ko)
+        elif slot < 21:
+            i = slot - 18
+            want[slot] = u[18 + axis] * apply(up) + apply(ko)       # beta^axis itself carries the mode when i == axis
+            want[21 + i] = apply(d2) + (apply(d2) / 3.0 if i == axis else 0.0)      # d_t Gt^i|_0 of flat space
+        else:
+            i = slot - 21
+            want[18 + i] = sgc * A * wave
+            want[slot] = -eta * A * wave + sign * c * apply(up) + apply(ko)
+        for v in range(17, 24):
+            scale = max(np.max(np.abs(want[v])), A)
+            assert np.max(np.abs(r[v] - want[v])) < 1e-13 * scale * (4 if order == 8 else 1), (slot, v)

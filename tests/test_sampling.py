@@ -3,7 +3,7 @@ a sample reproduces, bit for bit, the centre of the oracle run on the whole grid
 import numpy as np
 
 from paper_1307_6488_b200 import inputs
-from tests.test_gpu_fullsize import cut
+from tests.test_gpu_z_fullsize import cut
 
 
 def test_cut_block_reproduces_full_run(oracle):
