@@ -44,6 +44,10 @@ enum { CHEMORA_OK = 0, CHEMORA_EINVAL = -1, CHEMORA_ENOMEM = -2, CHEMORA_ECUDA =
  * D_t v_i = D_i rho, with centred first derivatives of order fd_order (needs ghost >= fd_order/2). */
 enum { CHEMORA_SYS_WAVE = 0, CHEMORA_SYS_BSSN = 1, CHEMORA_SYS_WAVE1 = 2 };
 
+/* boundary kind of a block (chemora_set_boundary): periodic ghost fill (reading S8, the default) or radiative outer
+ * boundary (reading S16) */
+enum { CHEMORA_BC_PERIODIC = 0, CHEMORA_BC_RADIATIVE = 1 };
+
 /* which buffer of the four RK4 buffers (reading S9) */
 enum { CHEMORA_BUF_U = 0, CHEMORA_BUF_YA = 1, CHEMORA_BUF_YB = 2, CHEMORA_BUF_S = 3 };
 
@@ -145,6 +149,24 @@ int chemora_rk3_step(chemora_t* h, double dt);
 int chemora_link_z(chemora_t* h, chemora_t* lower, chemora_t* upper);
 int chemora_rk4_step_group(chemora_t* const* blocks, int n, double dt);
 int chemora_rk3_step_group(chemora_t* const* blocks, int n, double dt);
+
+/* Radiative (Sommerfeld) outer boundary, the outer-face half of the second boundary kind (the paper's
+ * blocks have outer faces as well as inter-block faces, and it prints no boundary condition:
+ * DESIGN.md reading S16).  With CHEMORA_BC_RADIATIVE the g ghost layers of the block are evolved BOUNDARY POINTS:
+ * chemora_rk4_step / chemora_rk3_step fill nothing and run, after every interior right-hand side, a face kernel that
+ * applies  d_t u = -[ n^i D_i u + (u - u_inf)/r ]  (n^i = x^i/r, block centred on the origin, x^i = (i - (N_i-1)/2) dx,
+ * u_inf = 1 on chi, gt11, gt22, gt33, alpha of the BSSN system and 0 elsewhere, D_i second order: centred, one-sided
+ * three-point at the two ends of the padded array) with the same Runge-Kutta stage update.  Needs ghost >= 2; not
+ * combinable with chemora_link_z (CHEMORA_ESTATE).  The caller provides the boundary-point values of the initial state
+ * (chemora_set_state_ghosted, or chemora_fill_ghosts once after chemora_set_state).
+ * chemora_radiative_rhs: dev_rhs boundary points <- the radiative right-hand side of dev_state (interior untouched).
+ * chemora_set_state_ghosted / chemora_get_state_ghosted: U's whole padded block as one packed host array
+ * V x (nz+2g) x (ny+2g) x (nx+2g), x fastest.  Synchronous. */
+int chemora_set_boundary(chemora_t* h, int kind);
+int chemora_get_boundary(const chemora_t* h, int* kind);
+int chemora_radiative_rhs(chemora_t* h, const double* dev_state, double* dev_rhs);
+int chemora_set_state_ghosted(chemora_t* h, const double* host_ghosted);
+int chemora_get_state_ghosted(chemora_t* h, double* host_ghosted);
 
 /* Algebraic constraint enforcement on the interior of a BSSN state in the padded layout (dev_state == NULL: U):
  * gt_ij <- gt_ij + gt_ij (det(gt)^(-1/3) - 1), the bracket evaluated as expm1(-log(det)/3) and det in a fixed

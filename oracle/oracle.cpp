@@ -570,6 +570,76 @@ void rk4_step(int system, double* U, const Grid& G, const Params& P, double dt) 
   interior_loop([&](long q) { U[q] = U[q] + (dt / 6.0) * (S[q] + kk[q]); });
 }
 
+// ---------------------------------------------------------------------------------------
+// Second boundary kind (the paper's blocks have outer faces as well as inter-block
+// faces; it prints no boundary condition): radiative (Sommerfeld) outer
+// boundary, reading S16 of DESIGN.md.  Every point of the padded block outside the interior (the g
+// ghost layers: faces, edges, corners) is a BOUNDARY POINT that is evolved, not filled:
+//     d_t u = - v [ n^i D_i u + (u - u_inf) / r ],   n^i = x^i / r,   v = 1,
+// with the block centred on the origin, x^i = (i - (N_i - 1)/2) h for i in [-g, N_i + g), r = |x|,
+// u_inf = 1 for chi, gt11, gt22, gt33, alpha of the BSSN system and 0 for every other variable, and
+// D_i the second-order first derivative: centred (u[+1] - u[-1]) / 2h where both neighbours exist in
+// the padded array, else the one-sided three-point formula pointing into the block,
+//     lowest index:  (-3 u[0] + 4 u[+1] - u[+2]) / 2h ;   highest:  (3 u[0] - 4 u[-1] + u[-2]) / 2h .
+// No dissipation at boundary points.  The interior right-hand side is unchanged (it reads the
+// boundary points as its stencil neighbours); there is no ghost fill.
+// ---------------------------------------------------------------------------------------
+double u_infinity(int system, int v) {
+  if (system != SYS_BSSN) return 0.0;
+  return (v == 0 || v == 1 || v == 4 || v == 6 || v == 17) ? 1.0 : 0.0;
+}
+
+inline bool is_interior(const Grid& G, int i, int j, int k) {
+  return i >= 0 && i < G.nx && j >= 0 && j < G.ny && k >= 0 && k < G.nz;
+}
+
+// second-order first derivative along `axis` at a point of the padded array (centred, or one-sided at its two ends)
+double d1_boundary(const double* f, const Grid& G, int i, int j, int k, int axis) {
+  const int c = axis == 0 ? i : axis == 1 ? j : k;
+  const int n = axis == 0 ? G.nx : axis == 1 ? G.ny : G.nz;
+  const double u0 = at(f, G, i, j, k, axis, 0);
+  if (c == -G.g) return (-3.0 * u0 + 4.0 * at(f, G, i, j, k, axis, 1) - at(f, G, i, j, k, axis, 2)) / (2.0 * G.h);
+  if (c == n + G.g - 1) return (3.0 * u0 - 4.0 * at(f, G, i, j, k, axis, -1) + at(f, G, i, j, k, axis, -2)) / (2.0 * G.h);
+  return (at(f, G, i, j, k, axis, 1) - at(f, G, i, j, k, axis, -1)) / (2.0 * G.h);
+}
+
+double radiative_rhs_point(const double* f, const Grid& G, int i, int j, int k, double uinf) {
+  const double x = (i - 0.5 * (G.nx - 1)) * G.h, y = (j - 0.5 * (G.ny - 1)) * G.h, z = (k - 0.5 * (G.nz - 1)) * G.h;
+  const double r = std::sqrt(x * x + y * y + z * z);
+  const double nd = (x * d1_boundary(f, G, i, j, k, 0) + y * d1_boundary(f, G, i, j, k, 1) +
+                     z * d1_boundary(f, G, i, j, k, 2)) / r;
+  return -(nd + (f[idx(G, i, j, k)] - uinf) / r);
+}
+
+// rhs at every boundary point of every variable (interior entries untouched)
+void radiative_rhs(int system, const double* state, double* rhs, const Grid& G) {
+  const int V = nvars_of(system);
+  const long n = G.npts();
+  for (int v = 0; v < V; ++v)
+    for (int k = -G.g; k < G.nz + G.g; ++k)
+      for (int j = -G.g; j < G.ny + G.g; ++j)
+        for (int i = -G.g; i < G.nx + G.g; ++i)
+          if (!is_interior(G, i, j, k))
+            rhs[v * n + idx(G, i, j, k)] = radiative_rhs_point(state + v * n, G, i, j, k, u_infinity(system, v));
+}
+
+// RK4 (reading S9, same association) on a block with radiative outer boundaries: the stage updates run over ALL
+// points of the padded array, the right-hand side is the system's in the interior and the radiative one outside.
+void rk4_step_radiative(int system, double* U, const Grid& G, const Params& P, double dt) {
+  const int V = nvars_of(system);
+  const long tot = V * G.npts();
+  std::vector<double> Y(tot, 0.0), S(tot, 0.0), kk(tot, 0.0);
+  auto rhs_all = [&](const double* st) { rhs_any(system, st, kk.data(), G, P); radiative_rhs(system, st, kk.data(), G); };
+  rhs_all(U);
+  for (long q = 0; q < tot; ++q) { S[q] = kk[q]; Y[q] = U[q] + (dt / 2.0) * kk[q]; }
+  rhs_all(Y.data());
+  for (long q = 0; q < tot; ++q) { S[q] = S[q] + 2.0 * kk[q]; Y[q] = U[q] + (dt / 2.0) * kk[q]; }
+  rhs_all(Y.data());
+  for (long q = 0; q < tot; ++q) { S[q] = S[q] + 2.0 * kk[q]; Y[q] = U[q] + dt * kk[q]; }
+  rhs_all(Y.data());
+  for (long q = 0; q < tot; ++q) U[q] = U[q] + (dt / 6.0) * (S[q] + kk[q]);
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------------------
@@ -728,6 +798,20 @@ void oracle_energy(const double* U, int nx, int ny, int nz, int g, double* eps) 
 void oracle_enforce(double* U, int nx, int ny, int nz, int g) {
   Grid G = make_grid(nx, ny, nz, g, 4, 1.0);
   enforce_constraints(U, G);
+}
+
+// Radiative outer boundary (reading S16): rhs at the boundary points of a ghosted state (interior entries of `rhs`
+// are left as they are), and RK4 steps of a block whose ghost layers are evolved boundary points.
+void oracle_radiative_rhs(int system, const double* state, double* rhs, int nx, int ny, int nz, int g, double h) {
+  Grid G = make_grid(nx, ny, nz, g, 4, h);
+  radiative_rhs(system, state, rhs, G);
+}
+
+void oracle_rk4_radiative(int system, double* U, int nx, int ny, int nz, int g, int order, double h, double dt,
+                          const double* params, int nsteps) {
+  Grid G = make_grid(nx, ny, nz, g, order, h);
+  Params P = {params[0], params[1], params[2], (int)params[3]};
+  for (int s = 0; s < nsteps; ++s) rk4_step_radiative(system, U, G, P, dt);
 }
 
 }  // extern "C"

@@ -42,6 +42,10 @@ def lib():
         _lib.oracle_rhs.argtypes = [i, dp, dp, i, i, i, i, i, d, dp]
         _lib.oracle_rk4.argtypes = [i, dp, i, i, i, i, i, d, d, dp, i]
         _lib.oracle_rk3.argtypes = [i, dp, i, i, i, i, i, d, d, dp, i, i]
+        _lib.oracle_radiative_rhs.argtypes = [i, dp, dp, i, i, i, i, d]
+        _lib.oracle_radiative_rhs.restype = None
+        _lib.oracle_rk4_radiative.argtypes = [i, dp, i, i, i, i, i, d, d, dp, i]
+        _lib.oracle_rk4_radiative.restype = None
         _lib.oracle_enforce.argtypes = [dp, i, i, i, i]
         _lib.oracle_energy.argtypes = [dp, i, i, i, i, dp]
         _lib.oracle_energy.restype = None
@@ -125,6 +129,27 @@ def rk3(system, state, g, order, h, dt, prm, nsteps=1, enforce=False):
     assert V == NVARS[system]
     lib().oracle_rk3(system, _p(state), tx - 2 * g, ty - 2 * g, tz - 2 * g, g, order, float(h), float(dt), _p(prm),
                      int(nsteps), int(bool(enforce)))
+    return state
+
+
+def radiative_rhs(system, state, g, h, out=None):
+    """Reading S16: the radiative (Sommerfeld) right-hand side at every boundary point (the g ghost layers) of a
+    ghosted state; interior entries of the result are those of `out` (zeros when not given)."""
+    V, tz, ty, tx = state.shape
+    assert V == NVARS[system]
+    if out is None:
+        out = np.zeros_like(state)
+    lib().oracle_radiative_rhs(system, _p(state), _p(out), tx - 2 * g, ty - 2 * g, tz - 2 * g, g, float(h))
+    return out
+
+
+def rk4_radiative(system, state, g, order, h, dt, prm, nsteps=1):
+    """RK4 (S9) of a block with radiative outer boundaries: `state` is the whole padded block (its ghost layers are
+    evolved boundary points, nothing is filled); advanced in place."""
+    V, tz, ty, tx = state.shape
+    assert V == NVARS[system]
+    lib().oracle_rk4_radiative(system, _p(state), tx - 2 * g, ty - 2 * g, tz - 2 * g, g, order, float(h), float(dt),
+                               _p(prm), int(nsteps))
     return state
 
 

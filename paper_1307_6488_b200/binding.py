@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libchemora.so")
 
 SYS_WAVE, SYS_BSSN, SYS_WAVE1 = 0, 1, 2
 BUF_U, BUF_YA, BUF_YB, BUF_S = 0, 1, 2, 3
+BC_PERIODIC, BC_RADIATIVE = 0, 1
 NUM_TILES = 9
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 
@@ -23,7 +24,8 @@ SYMBOLS = ["chemora_create", "chemora_set_param", "chemora_get_param", "chemora_
            "chemora_set_state", "chemora_get_state", "chemora_set_state_async", "chemora_get_state_async",
            "chemora_synchronize", "chemora_set_state_dev", "chemora_get_state_dev",
            "chemora_fill_ghosts", "chemora_rhs", "chemora_rk4_step", "chemora_rk3_step", "chemora_link_z",
-           "chemora_rk4_step_group", "chemora_rk3_step_group", "chemora_enforce_constraints", "chemora_energy", "chemora_set_variant",
+           "chemora_rk4_step_group", "chemora_rk3_step_group", "chemora_set_boundary", "chemora_get_boundary", "chemora_radiative_rhs",
+           "chemora_set_state_ghosted", "chemora_get_state_ghosted", "chemora_enforce_constraints", "chemora_energy", "chemora_set_variant",
            "chemora_get_variant", "chemora_variant_available", "chemora_selfcheck", "chemora_describe_device_error", "chemora_tile_shape", "chemora_tile_cost", "chemora_autotune", "chemora_launch_count",
            "chemora_kernel_info", "chemora_timing", "chemora_timing_read", "chemora_measure_fp64_peak", "chemora_last_error", "chemora_destroy"]
 
@@ -63,6 +65,8 @@ def load():
         "chemora_rk3_step": [vp, d],
         "chemora_set_state_async": [vp, vp], "chemora_get_state_async": [vp, vp], "chemora_synchronize": [vp],
         "chemora_link_z": [vp, vp, vp],
+        "chemora_set_boundary": [vp, i], "chemora_get_boundary": [vp, ip], "chemora_radiative_rhs": [vp, vp, vp],
+        "chemora_set_state_ghosted": [vp, vp], "chemora_get_state_ghosted": [vp, vp],
         "chemora_rk4_step_group": [ctypes.POINTER(vp), i, d], "chemora_rk3_step_group": [ctypes.POINTER(vp), i, d],
         "chemora_tile_cost": [i, i, i, dp, lp, lp],
         "chemora_enforce_constraints": [vp, vp],
@@ -288,6 +292,29 @@ class Chemora:
         """multi-block interface: the ghost z-planes come from the neighbour blocks' interiors (None: own images)"""
         self._ck(self.lib.chemora_link_z(self._h, lower._h if lower is not None else None,
                                          upper._h if upper is not None else None))
+
+    def set_boundary(self, kind):
+        self._ck(self.lib.chemora_set_boundary(self._h, int(kind)))
+
+    def get_boundary(self):
+        k = ctypes.c_int()
+        self._ck(self.lib.chemora_get_boundary(self._h, ctypes.byref(k)))
+        return k.value
+
+    def radiative_rhs(self, dev_state, dev_rhs):
+        self._ck(self.lib.chemora_radiative_rhs(self._h, self._ptr(dev_state), self._ptr(dev_rhs)))
+
+    def set_state_ghosted(self, host_ghosted):
+        g, (nx, ny, nz) = self.ghost, self.dims
+        a = np.ascontiguousarray(host_ghosted, dtype=np.float64)
+        assert a.shape == (self.nvars, nz + 2 * g, ny + 2 * g, nx + 2 * g)
+        self._ck(self.lib.chemora_set_state_ghosted(self._h, a.ctypes.data_as(ctypes.c_void_p)))
+
+    def get_state_ghosted(self):
+        g, (nx, ny, nz) = self.ghost, self.dims
+        out = np.empty((self.nvars, nz + 2 * g, ny + 2 * g, nx + 2 * g), dtype=np.float64)
+        self._ck(self.lib.chemora_get_state_ghosted(self._h, out.ctypes.data_as(ctypes.c_void_p)))
+        return out
 
     def enforce_constraints(self, state=None):
         """in place on a padded device state tensor (default: U)"""

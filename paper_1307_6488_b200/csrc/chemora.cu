@@ -31,6 +31,7 @@ struct chemora {
   double* staging;      // device packed staging for set/get_state (lazy)
   unsigned* dev_err;    // device error word the kernels' bounded waits write (Layout::err)
   int fused, tile;
+  int boundary;         // CHEMORA_BC_PERIODIC (ghost fill) or CHEMORA_BC_RADIATIVE (ghost layers are evolved boundary points)
   int autotune_split;   // tuning: chemora_autotune also times the derivative-split variant
   chemora* nb_lo;        // z-neighbours of a linked block (chemora_link_z); nullptr: periodic in itself
   chemora* nb_hi;
@@ -186,6 +187,17 @@ int fill(chemora_t* h, double* state) {
   return CHEMORA_OK;
 }
 
+// the radiative face kernel with the Runge-Kutta epilogue `st` (reading S16); u_inf = 1 on chi, gt11, gt22, gt33, alpha
+int radiative(chemora_t* h, const Stage& st) {
+  const unsigned mask = h->system == CHEMORA_SYS_BSSN ? (1u << 0) | (1u << 1) | (1u << 4) | (1u << 6) | (1u << 17) : 0u;
+  tick(h, 1);
+  CK(h, launch_radiative(h->L, st, h->dx, mask, h->stream), "radiative boundary launch");
+  tick(h, 1);
+  h->launches += 1;
+  if (h->timing) h->ev_launches[1] += 1;
+  return CHEMORA_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -226,6 +238,7 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
   h->fused = 1; h->tile = (system_id == CHEMORA_SYS_BSSN && fd_order == 8) ? 0 : 1;
   h->launches = 0;
   h->autotune_split = 0;
+  h->boundary = CHEMORA_BC_PERIODIC;
   h->timing = false;
   for (int c = 0; c < 2; ++c) { h->ev_used[c] = 0; h->ev_ms[c] = 0.0; h->ev_launches[c] = 0; }
   for (int b = 0; b < 4; ++b) h->buf[b] = nullptr;
@@ -317,7 +330,9 @@ int chemora_state_ptr(chemora_t* h, int which, double** dev) {
 
 static int ensure_staging(chemora_t* h) {
   if (h->staging) return CHEMORA_OK;
-  h->staging = (double*)dev_alloc(h, packed_count(h) * sizeof(double));
+  // sized for the ghosted block too (chemora_set_state_ghosted / chemora_get_state_ghosted)
+  const size_t ghosted = (size_t)h->L.nvars * (h->L.nx + 2 * h->L.g) * (h->L.ny + 2 * h->L.g) * (h->L.nz + 2 * h->L.g);
+  h->staging = (double*)dev_alloc(h, ghosted * sizeof(double));
   return h->staging ? CHEMORA_OK : fail(h, CHEMORA_ENOMEM, "staging allocation failed");
 }
 
@@ -451,8 +466,13 @@ static int step_one(chemora_t* h, double dt, bool rk3) {
   const int ns = rk3 ? rk3_plan(h, dt, p) : rk4_plan(h, dt, p);
   for (int s = 0; s < ns; ++s) {
     int rc;
-    if ((rc = fill(h, h->buf[p[s].in]))) return rc;
-    if ((rc = run_rhs(h, p[s].st))) return rc;
+    if (h->boundary == CHEMORA_BC_RADIATIVE) {   // nothing is filled: the ghost layers are evolved by the face kernel
+      if ((rc = run_rhs(h, p[s].st))) return rc;
+      if ((rc = radiative(h, p[s].st))) return rc;
+    } else {
+      if ((rc = fill(h, h->buf[p[s].in]))) return rc;
+      if ((rc = run_rhs(h, p[s].st))) return rc;
+    }
   }
   return CHEMORA_OK;
 }
@@ -489,6 +509,8 @@ int chemora_rk3_step_group(chemora_t* const* hs, int n, double dt) { return step
 
 int chemora_link_z(chemora_t* h, chemora_t* lower, chemora_t* upper) {
   if (!h) return CHEMORA_EINVAL;
+  if ((lower || upper) && h->boundary != CHEMORA_BC_PERIODIC)
+    return fail(h, CHEMORA_ESTATE, "a block with radiative boundaries cannot be z-linked");
   for (chemora_t* nb : {lower, upper}) {
     if (!nb) continue;
     if (nb->L.nx != h->L.nx || nb->L.ny != h->L.ny || nb->L.g != h->L.g || nb->system != h->system ||
@@ -499,6 +521,63 @@ int chemora_link_z(chemora_t* h, chemora_t* lower, chemora_t* upper) {
   h->nb_lo = lower;
   h->nb_hi = upper;
   return CHEMORA_OK;
+}
+
+int chemora_set_boundary(chemora_t* h, int kind) {
+  if (!h) return CHEMORA_EINVAL;
+  if (kind != CHEMORA_BC_PERIODIC && kind != CHEMORA_BC_RADIATIVE) return fail(h, CHEMORA_EINVAL, "unknown boundary kind");
+  if (kind == CHEMORA_BC_RADIATIVE && (h->nb_lo || h->nb_hi))
+    return fail(h, CHEMORA_ESTATE, "a z-linked block cannot have radiative boundaries");
+  if (kind == CHEMORA_BC_RADIATIVE && h->L.g < 2) return fail(h, CHEMORA_EINVAL, "radiative boundaries need ghost >= 2");
+  h->boundary = kind;
+  return CHEMORA_OK;
+}
+
+int chemora_get_boundary(const chemora_t* h, int* kind) {
+  if (!h || !kind) return CHEMORA_EINVAL;
+  *kind = h->boundary;
+  return CHEMORA_OK;
+}
+
+int chemora_radiative_rhs(chemora_t* h, const double* dev_state, double* dev_rhs) {
+  if (!h || !dev_state || !dev_rhs || dev_state == dev_rhs) return CHEMORA_EINVAL;
+  if (h->L.g < 2) return fail(h, CHEMORA_EINVAL, "radiative boundaries need ghost >= 2");
+  Stage st{dev_state, nullptr, nullptr, dev_rhs, 0.0, MODE_RHS};
+  return radiative(h, st);
+}
+
+// the whole padded block as one packed array [V][nz+2g][ny+2g][nx+2g]: the pack kernel on a layout whose "interior" is
+// the padded block (ghost width 0, first column xo - g)
+static Layout ghosted_layout(const chemora_t* h) {
+  Layout G = h->L;
+  G.nx += 2 * G.g; G.ny += 2 * G.g; G.nz += 2 * G.g;
+  G.xo -= G.g;
+  G.g = 0;
+  return G;
+}
+
+int chemora_set_state_ghosted(chemora_t* h, const double* host_ghosted) {
+  if (!h || !host_ghosted) return CHEMORA_EINVAL;
+  int rc = ensure_staging(h);
+  if (rc) return rc;
+  const Layout G = ghosted_layout(h);
+  const size_t n = (size_t)G.nvars * G.nx * G.ny * G.nz;
+  CK(h, cudaMemcpyAsync(h->staging, host_ghosted, n * sizeof(double), cudaMemcpyHostToDevice, h->stream), "H2D copy");
+  CK(h, launch_pack(G, h->staging, h->buf[0], true, h->stream), "unpack launch");
+  h->launches += 1;
+  return chemora_synchronize(h);
+}
+
+int chemora_get_state_ghosted(chemora_t* h, double* host_ghosted) {
+  if (!h || !host_ghosted) return CHEMORA_EINVAL;
+  int rc = ensure_staging(h);
+  if (rc) return rc;
+  const Layout G = ghosted_layout(h);
+  const size_t n = (size_t)G.nvars * G.nx * G.ny * G.nz;
+  CK(h, launch_pack(G, h->staging, h->buf[0], false, h->stream), "pack launch");
+  h->launches += 1;
+  CK(h, cudaMemcpyAsync(host_ghosted, h->staging, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream), "D2H copy");
+  return chemora_synchronize(h);
 }
 
 int chemora_enforce_constraints(chemora_t* h, double* dev_state) {
