@@ -580,7 +580,8 @@ void rk4_step(int system, double* U, const Grid& G, const Params& P, double dt) 
 // u_inf = 1 for chi, gt11, gt22, gt33, alpha of the BSSN system and 0 for every other variable, and
 // D_i the second-order first derivative: centred (u[+1] - u[-1]) / 2h where both neighbours exist in
 // the padded array, else the one-sided three-point formula pointing into the block,
-//     lowest index:  (-3 u[0] + 4 u[+1] - u[+2]) / 2h ;   highest:  (3 u[0] - 4 u[-1] + u[-2]) / 2h .
+//     lowest index:  (-3 u[0] + 4 u[+1] - u[+2]) / 2h ;   highest:  (3 u[0] - 4 u[-1] + u[-2]) / 2h ,
+// both evaluated in difference form (reading R-H1).
 // No dissipation at boundary points.  The interior right-hand side is unchanged (it reads the
 // boundary points as its stencil neighbours); there is no ghost fill.
 // ---------------------------------------------------------------------------------------
@@ -597,9 +598,11 @@ inline bool is_interior(const Grid& G, int i, int j, int k) {
 double d1_boundary(const double* f, const Grid& G, int i, int j, int k, int axis) {
   const int c = axis == 0 ? i : axis == 1 ? j : k;
   const int n = axis == 0 ? G.nx : axis == 1 ? G.ny : G.nz;
+  // difference form (reading R-H1): -3 u0 + 4 u1 - u2 = 4 (u1 - u0) - (u2 - u0), every subtraction of near-equal
+  // values exact, so near-flat data keeps its relative accuracy and flat data gives exactly 0
   const double u0 = at(f, G, i, j, k, axis, 0);
-  if (c == -G.g) return (-3.0 * u0 + 4.0 * at(f, G, i, j, k, axis, 1) - at(f, G, i, j, k, axis, 2)) / (2.0 * G.h);
-  if (c == n + G.g - 1) return (3.0 * u0 - 4.0 * at(f, G, i, j, k, axis, -1) + at(f, G, i, j, k, axis, -2)) / (2.0 * G.h);
+  if (c == -G.g) return (4.0 * (at(f, G, i, j, k, axis, 1) - u0) - (at(f, G, i, j, k, axis, 2) - u0)) / (2.0 * G.h);
+  if (c == n + G.g - 1) return -(4.0 * (at(f, G, i, j, k, axis, -1) - u0) - (at(f, G, i, j, k, axis, -2) - u0)) / (2.0 * G.h);
   return (at(f, G, i, j, k, axis, 1) - at(f, G, i, j, k, axis, -1)) / (2.0 * G.h);
 }
 

@@ -85,8 +85,9 @@ __global__ void __launch_bounds__(256) radiative_kernel(Layout L, Stage st, doub
   const double ih2 = 1.0 / (2.0 * h);
   // second-order first derivative along a direction with element stride s, at padded coordinate c of n
   auto d1 = [&](const double* c0, long s, int c, int n) {
-    if (c == 0) return (-3.0 * c0[0] + 4.0 * c0[s] - c0[2 * s]) * ih2;
-    if (c == n - 1) return (3.0 * c0[0] - 4.0 * c0[-s] + c0[-2 * s]) * ih2;
+    // difference form (reading R-H1): -3 u0 + 4 u1 - u2 = 4 (u1 - u0) - (u2 - u0)
+    if (c == 0) return (4.0 * (c0[s] - c0[0]) - (c0[2 * s] - c0[0])) * ih2;
+    if (c == n - 1) return -(4.0 * (c0[-s] - c0[0]) - (c0[-2 * s] - c0[0])) * ih2;
     return (c0[s] - c0[-s]) * ih2;
   };
   auto point = [&](int i, int j, int k) {   // padded coordinates
