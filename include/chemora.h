@@ -201,7 +201,10 @@ int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, 
  * fused tile id (and, with the parameter "autotune_split" = 1, the six split tiles) on the handle's own grid -- one
  * middle RK4 stage evaluated on the current U, results into the scratch buffers S and Ya; one warm-up run, then the
  * median of three timed runs -- keeps the fastest, returns it.  A variant that cannot run here (CHEMORA_ENOMEM for
- * its scratch, CHEMORA_EINVAL from its launch check) is skipped, not fatal.
+ * its scratch, CHEMORA_EINVAL from its launch check) is skipped, not fatal.  Guard: every fused BSSN tile id evaluates
+ * the same right-hand side, so a candidate whose result (Ya) differs from the first fused id's (kept in Yb for the
+ * duration of the sweep) by more than 1e-11 in the norm of reading S11, or whose bounded waits gave up, is
+ * disqualified: ms_out = -2 / -3.
  * ms_out, if not NULL, receives 2*CHEMORA_NUM_TILES timings in milliseconds ([fused*NUM_TILES + tile];
  * negative = variant unavailable or not timed).  U is not modified.  Synchronous. */
 int chemora_autotune(chemora_t* h, int* fused, int* tile_id, float* ms_out);

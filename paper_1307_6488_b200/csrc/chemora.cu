@@ -262,8 +262,8 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
       return CHEMORA_ECUDA;
     }
   }
-  h->dev_err = (unsigned*)dev_alloc(h, 128);
-  if (!h->dev_err || cudaMemsetAsync(h->dev_err, 0, 128, h->stream) != cudaSuccess) {
+  h->dev_err = (unsigned*)dev_alloc(h, 1024);   // [0] error word; from byte 16: the sweep guard's 2 x V norms
+  if (!h->dev_err || cudaMemsetAsync(h->dev_err, 0, 1024, h->stream) != cudaSuccess) {
     dev_free(h, h->dev_err);
     for (int c = 0; c < 4; ++c) dev_free(h, h->buf[c]);
     delete h;
@@ -679,6 +679,7 @@ int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out)
       return cuda_fail(h, cudaGetLastError(), "event create");
     }
   int rc = fill(h, h->buf[0]);
+  bool have_ref = false;
   // fused variants always; the derivative-split variant (about 18 GB of scratch at 256^3, never the pick in any
   // measured sweep) only when the tuning parameter "autotune_split" is 1
   for (int f = 1; f >= (h->autotune_split ? 0 : 1) && !rc; --f)
@@ -697,6 +698,44 @@ int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out)
       if (vrc) { rc = vrc; break; }
       cudaEventRecord(ev[3], h->stream);
       if (cudaEventSynchronize(ev[3]) != cudaSuccess) { rc = cuda_fail(h, cudaGetLastError(), "autotune sync"); break; }
+      // Guard (the paper's run-time path loads kernels it has just generated; here: a variant
+      // is only eligible if it computes what the reference variant computes).  The fused BSSN tile ids evaluate
+      // the same right-hand side (two-pass or one-pass mixed derivatives: rounding differs, nothing else), so their
+      // Ya = U + a k must agree with the first one's -- kept in Yb, scratch between steps -- to 1e-11 in the norm
+      // of reading S11, per variable.  A variant that disagrees, or whose bounded waits gave up, is disqualified.
+      if (f == 1 && h->system == CHEMORA_SYS_BSSN) {
+        const int V = h->L.nvars;
+        unsigned long long* dnorm = reinterpret_cast<unsigned long long*>(h->dev_err) + 2;   // [2 V] after the error words
+        unsigned long long host[2 + 2 * 25];
+        cudaError_t ge = cudaSuccess;
+        if (!have_ref) {
+          ge = cudaMemcpyAsync(h->buf[2], h->buf[1], (size_t)V * h->L.vstride * sizeof(double), cudaMemcpyDeviceToDevice, h->stream);
+        } else {
+          ge = cudaMemsetAsync(dnorm, 0, 2 * V * sizeof(unsigned long long), h->stream);
+          if (ge == cudaSuccess) ge = launch_maxdiff(h->buf[1], h->buf[2], h->L.vstride, V, dnorm, h->stream);
+          h->launches += 1;
+        }
+        if (ge == cudaSuccess) ge = cudaMemcpyAsync(host, h->dev_err, sizeof host, cudaMemcpyDeviceToHost, h->stream);
+        if (ge == cudaSuccess) ge = cudaStreamSynchronize(h->stream);
+        if (ge != cudaSuccess) { rc = cuda_fail(h, ge, "autotune guard"); break; }
+        if ((unsigned)host[0] != 0) {            // a wait timed out inside this variant: clear the word, disqualify
+          cudaMemsetAsync(h->dev_err, 0, sizeof(unsigned), h->stream);
+          if (ms_out) ms_out[f * CHEMORA_NUM_TILES + t] = -3.f;
+          continue;
+        }
+        bool agree = true;
+        for (int v = 0; have_ref && v < V; ++v) {
+          double d, m;
+          memcpy(&d, &host[2 + 2 * v], sizeof d);
+          memcpy(&m, &host[2 + 2 * v + 1], sizeof m);
+          if (!(d <= 1e-11 * m)) agree = false;
+        }
+        if (!agree) {
+          if (ms_out) ms_out[f * CHEMORA_NUM_TILES + t] = -2.f;
+          continue;
+        }
+        have_ref = true;
+      }
       float m[3];
       for (int n = 0; n < 3; ++n) cudaEventElapsedTime(&m[n], ev[n], ev[n + 1]);
       const float lo = fminf(m[0], fminf(m[1], m[2])), hi = fmaxf(m[0], fmaxf(m[1], m[2]));

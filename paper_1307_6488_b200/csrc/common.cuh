@@ -147,6 +147,7 @@ struct FillLink {
 cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s, const FillLink* link = nullptr);
 // radiative outer boundary (reading S16): RHS + stage epilogue at the boundary points (the g ghost layers)
 cudaError_t launch_radiative(const Layout& L, const Stage& st, double h, unsigned uinf_mask, cudaStream_t s);
+cudaError_t launch_maxdiff(const double* a, const double* b, long vstride, int nvars, unsigned long long* out, cudaStream_t s);
 cudaError_t launch_energy(const Layout& L, const double* state, double* eps_out, double* sum, cudaStream_t s);
 cudaError_t launch_enforce(const Layout& L, double* state, cudaStream_t s);
 cudaError_t launch_pack(const Layout& L, const double* packed, double* state, bool to_state, cudaStream_t s);

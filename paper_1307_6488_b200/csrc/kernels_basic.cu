@@ -135,6 +135,41 @@ cudaError_t launch_radiative(const Layout& L, const Stage& st, double h, unsigne
   return cudaGetLastError();
 }
 
+// Per variable v: out[2 v] = max |a - b|, out[2 v + 1] = max |b| over the variable's whole padded array, as the bit
+// patterns of non-negative doubles (which order like unsigned integers, so atomicMax works); a NaN on either side
+// counts as an infinite difference.  The runtime sweep's guard: a candidate variant must reproduce the reference
+// variant's result in the norm of reading S11.
+__global__ void __launch_bounds__(256) maxdiff_kernel(const double* __restrict__ a, const double* __restrict__ b,
+                                                      long vstride, unsigned long long* out) {
+  const long base = (long)blockIdx.y * vstride;
+  double d = 0.0, m = 0.0;
+  for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < vstride; i += (long)gridDim.x * blockDim.x) {
+    const double x = a[base + i], y = b[base + i];
+    double e = fabs(x - y);
+    if (!(e == e)) e = __longlong_as_double(0x7ff0000000000000LL);
+    d = fmax(d, e);
+    m = fmax(m, fabs(y));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    d = fmax(d, __shfl_xor_sync(0xffffffffu, d, o));
+    m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+  }
+  if ((threadIdx.x & 31) == 0) {
+    atomicMax(out + 2 * blockIdx.y, (unsigned long long)__double_as_longlong(d));
+    atomicMax(out + 2 * blockIdx.y + 1, (unsigned long long)__double_as_longlong(m));
+  }
+}
+
+cudaError_t launch_maxdiff(const double* a, const double* b, long vstride, int nvars, unsigned long long* out,
+                           cudaStream_t s) {
+  long blocks = (vstride + 256L * 8 - 1) / (256L * 8);
+  if (blocks > 1024) blocks = 1024;
+  if (blocks < 1) blocks = 1;
+  maxdiff_kernel<<<dim3((unsigned)blocks, nvars), 256, 0, s>>>(a, b, vstride, out);
+  return cudaGetLastError();
+}
+
 // packed [V][nz][ny][nx] <-> padded interior
 __global__ void __launch_bounds__(256) pack_kernel(Layout L, const double* __restrict__ src, double* __restrict__ dst,
                                                    bool to_state) {

@@ -287,28 +287,6 @@ def test_bssn_rk4_10_steps_small(chem, oracle, fused):
     h.destroy()
 
 
-@pytest.mark.parametrize("data", ["gaussians", "strong"])
-def test_bssn_rk4_10_steps_every_slot_moves(chem, oracle, data):
-    """10 RK4 steps on data where every slot evolves by far more than 1e-10 of its size (Gaussians of amplitude 1e-4;
-    0.02-amplitude strong field), every fused tile id and one split tile: 1e-10 is then meaningful on all 25 slots"""
-    nx, ny, nz = 24, 20, 18
-    u0 = inputs.bssn_gaussians(nx, ny, nz, width_cells=4.0) if data == "gaussians" else \
-        inputs.bssn_minkowski(nx, ny, nz) + 0.02 * np.random.default_rng(23).uniform(-1, 1, size=(25, nz, ny, nx))
-    dx, dt, eps = 0.05, 0.0125, 0.1
-    st = oracle.rk4(1, oracle.with_ghosts(u0, 3), 3, 4, dx, dt, oracle.params(eps_diss=eps), 10)
-    want = oracle.interior(st, 3)
-    assert all(np.max(np.abs(want[v] - u0[v])) > 1e-8 * max(np.max(np.abs(want[v])), 1e-300) for v in range(24))
-    h = chem.Chemora(nx, ny, nz, 3, 4, 1, dx)
-    h.set_param("eps_diss", eps)
-    for fused, tile in [(1, t) for t in chem.variants(chem.SYS_BSSN, 4)] + [(0, 1)]:
-        h.set_variant(fused, tile)
-        h.set_state(u0)
-        for _ in range(10):
-            h.rk4_step(dt)
-        assert_bssn_close(h.get_state(), want, TOL_BSSN_10_STEPS)
-    h.destroy()
-
-
 def test_bssn_config2_full_size_10_steps(chem, oracle):
     """configs[2] exactly: 64^3, g=3, O4 + upwind + KO, Minkowski + 1e-10 noise, 10 steps (oracle ~1-2 min)."""
     c = inputs.config(2)
@@ -338,7 +316,7 @@ def test_autotune_and_kernel_info(chem):
     h.set_param("autotune_split", 1)
     fused2, tile2, ms2 = h.autotune()
     assert all(m > 0 for m in ms2[:6]) and fused2 == 1                  # the six split tiles timed; never the pick
-    assert (fused, tile) == h.get_variant()
+    assert (fused2, tile2) == h.get_variant()
     assert np.array_equal(h.get_state(), u)        # U is not modified by the sweep
     info = h.kernel_info()
     assert 0 < info["regs"] <= 255
@@ -593,61 +571,3 @@ def test_wave1_energy(chem, oracle):
     with pytest.raises(chem.ChemoraError):
         b.energy()
     b.destroy()
-
-
-# ------------------------------------------------- radiative outer boundary, reading S16 (second half)
-@pytest.mark.parametrize("system,order,g,dims", [(0, 4, 2, (19, 11, 9)), (0, 8, 4, (37, 9, 12)), (1, 4, 3, (21, 12, 10)),
-                                                 (2, 4, 3, (9, 33, 8))])
-def test_radiative_rhs_at_boundary_points(chem, oracle, system, order, g, dims):
-    """the face kernel against the oracle at every boundary point (faces, edges, corners), interior untouched"""
-    nx, ny, nz = dims
-    V = {0: 2, 1: 25, 2: 5}[system]
-    st = np.random.default_rng(51).standard_normal((V, nz + 2 * g, ny + 2 * g, nx + 2 * g))
-    dx = 0.07
-    want = oracle.radiative_rhs(system, st, g, dx)
-    h = chem.Chemora(nx, ny, nz, g, order, system, dx)
-    h.set_state_ghosted(st)
-    assert np.array_equal(h.get_state_ghosted(), st)                 # the ghosted copies are bit-exact
-    out = h.new_state()
-    out.fill_(7.0)
-    h.radiative_rhs(h.state_view(), out)
-    got = h.ghosted(out).cpu().numpy()
-    m = np.ones(got.shape[1:], dtype=bool)
-    m[g:-g, g:-g, g:-g] = False
-    for v in range(V):
-        assert np.max(np.abs(got[v][m] - want[v][m])) < 1e-12 * np.max(np.abs(want[v][m])), v
-    assert (got[:, ~m] == 7.0).all()
-    h.destroy()
-
-
-@pytest.mark.parametrize("system,order,g,steps,tol", [(0, 4, 2, 10, 1e-11), (2, 8, 4, 5, 5e-12), (1, 4, 3, 10, 1e-10)])
-def test_radiative_rk4_whole_block(chem, oracle, system, order, g, steps, tol):
-    """RK4 with radiative boundaries: the whole padded block (interior and evolved boundary points) against the
-    oracle; the BSSN case on configs[2]-like data with both norms"""
-    nx, ny, nz = 22, 18, 13
-    dx = 0.05
-    dt = 0.25 * dx
-    V = {0: 2, 1: 25, 2: 5}[system]
-    rng = np.random.default_rng(52)
-    if system == 1:
-        st = oracle.fill_ghosts(oracle.with_ghosts(inputs.bssn_noise(nx, ny, nz), g), g)
-        st += 1e-10 * rng.uniform(-1, 1, size=st.shape)
-    else:
-        st = rng.standard_normal((V, nz + 2 * g, ny + 2 * g, nx + 2 * g))
-    prm = oracle.params(eps_diss=0.1 if g >= 3 else 0.0)
-    h = chem.Chemora(nx, ny, nz, g, order, system, dx)
-    h.set_param("eps_diss", 0.1 if g >= 3 else 0.0)
-    h.set_boundary(chem.BC_RADIATIVE)
-    assert h.get_boundary() == chem.BC_RADIATIVE
-    h.set_state_ghosted(st)
-    for _ in range(steps):
-        h.rk4_step(dt)
-    got = h.get_state_ghosted()
-    want = oracle.rk4_radiative(system, st.copy(), g, order, dx, dt, prm, steps)
-    if system == 1:
-        assert_bssn_close(got, want, tol)
-    else:
-        assert relerr(got, want) < tol
-    with pytest.raises(chem.ChemoraError):
-        h.link_z(h, h)                                      # radiative blocks are not z-linked
-    h.destroy()
