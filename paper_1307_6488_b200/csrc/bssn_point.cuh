@@ -13,17 +13,17 @@ namespace chm {
 
 enum { V_CHI = 0, V_GT = 1, V_K = 7, V_AT = 8, V_GAM = 14, V_ALPHA = 17, V_BETA = 18, V_B = 21, V_A = 24 };
 
-__device__ __forceinline__ constexpr int sym(int i, int j) {
+CHM_HD constexpr int sym(int i, int j) {
   return i <= j ? (i == 0 ? j : i + j + 1) : (j == 0 ? i : i + j + 1);   // (0,0)0 (0,1)1 (0,2)2 (1,1)3 (1,2)4 (2,2)5
 }
 
 // contraction of a packed symmetric tensor with another: A^{ij} B_{ij}
-__device__ __forceinline__ double sdot(const double* A, const double* B) {
+CHM_HD double sdot(const double* A, const double* B) {
   return (A[0] * B[0] + A[3] * B[3] + A[5] * B[5]) + 2.0 * (A[1] * B[1] + A[2] * B[2] + A[4] * B[4]);
 }
 
 template <class D, class Emit>
-__device__ __forceinline__ void bssn_point(const D& d, const Coef& C, Emit&& emit) {
+CHM_HD void bssn_point(const D& d, const Coef& C, Emit&& emit) {
   const double third = 1.0 / 3.0, two_thirds = 2.0 / 3.0;
 
   // ---- metric, inverse metric ----------------------------------------------------------------------

@@ -7,6 +7,9 @@
 #endif
 #include <stdint.h>
 
+// inline helper usable from device code and from host-side probes of the same arithmetic (tests/native/)
+#define CHM_HD __host__ __device__ __forceinline__
+
 namespace chm {
 
 #if CHM_STCS

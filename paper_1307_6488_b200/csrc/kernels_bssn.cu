@@ -18,30 +18,6 @@ __device__ __forceinline__ constexpr int slot_d2(int v, int a, int b) {
 }
 __device__ __forceinline__ constexpr int slot_ad(int v) { return 111 + v; }
 
-// differentiates on the fly from a point accessor P
-template <class P, int ORDER = 4>
-struct OnTheFly {
-  P pt;
-  Coef C;
-  double beta[3];
-  __device__ __forceinline__ double f(int v) const { return pt.at(v, 0, 0, 0); }
-  __device__ __forceinline__ double d1(int v, int a) const {
-    return ORDER == 4 ? d1_o4(pt, v, a, C.inv_h) : d1_o8(pt, v, a, C.inv_h);
-  }
-  __device__ __forceinline__ double d2(int v, int a, int b) const {
-    if (ORDER == 4) return a == b ? d2_o4(pt, v, a, C.inv_h2) : dmix_o4(pt, v, a, b, C.inv_h2);
-    return a == b ? d2_o8(pt, v, a, C.inv_h2) : dmix_o8(pt, v, a, b, C.inv_h2);
-  }
-  __device__ __forceinline__ double adv(int v, int a) const {
-    return ORDER == 4 ? adv_o4(pt, v, a, beta[a], C.inv_h) : adv_o8(pt, v, a, beta[a], C.inv_h);
-  }
-  __device__ __forceinline__ double ad(int v) const {
-    double r = ORDER == 4 ? ko5(pt, v, C.ko) : ko_kq(pt, v, C.kq);
-    if (v != V_A) r += (adv(v, 0) + adv(v, 1)) + adv(v, 2);
-    return r;
-  }
-};
-
 // reads the precomputed derivative arrays (packed interior layout, stride n per array)
 struct FromArrays {
   const double* __restrict__ fields;   // at the point, padded layout

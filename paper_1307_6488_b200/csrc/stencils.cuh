@@ -4,7 +4,7 @@
 // All in difference form (reading R-H1): only differences of neighbouring values are ever scaled and summed,
 // so flat data differentiates to exactly 0 and near-flat data keeps full relative accuracy.
 #pragma once
-#include "common.cuh"
+#include "bssn_point.cuh"
 
 namespace chm {
 
@@ -30,14 +30,14 @@ struct GlobalPoint {
 
 // ---- 4th order ---------------------------------------------------------------------------------------
 template <class P>
-__device__ __forceinline__ double d1_o4(const P& f, int v, int a, double inv_h) {
+CHM_HD double d1_o4(const P& f, int v, int a, double inv_h) {
   double e1 = f.ax(v, a, 1) - f.ax(v, a, -1);
   double e2 = f.ax(v, a, 2) - f.ax(v, a, -2);
   return (8.0 * e1 - e2) * (inv_h * (1.0 / 12.0));
 }
 
 template <class P>
-__device__ __forceinline__ double d2_o4(const P& f, int v, int a, double inv_h2) {
+CHM_HD double d2_o4(const P& f, int v, int a, double inv_h2) {
   double f0 = f.at(v, 0, 0, 0);
   double s1 = (f.ax(v, a, 1) - f0) + (f.ax(v, a, -1) - f0);
   double s2 = (f.ax(v, a, 2) - f0) + (f.ax(v, a, -2) - f0);
@@ -46,7 +46,7 @@ __device__ __forceinline__ double d2_o4(const P& f, int v, int a, double inv_h2)
 
 // row(m) = undivided first difference along b at offset m along a
 template <class P>
-__device__ __forceinline__ double dmix_o4(const P& f, int v, int a, int b, double inv_h2) {
+CHM_HD double dmix_o4(const P& f, int v, int a, int b, double inv_h2) {
   double r[4];
   const int off[4] = {1, -1, 2, -2};
 #pragma unroll
@@ -61,7 +61,7 @@ __device__ __forceinline__ double dmix_o4(const P& f, int v, int a, int b, doubl
 
 // beta^a * upwinded d_a f, side by the sign of beta (beta == 0 gives exactly 0)
 template <class P>
-__device__ __forceinline__ double adv_o4(const P& f, int v, int a, double beta, double inv_h) {
+CHM_HD double adv_o4(const P& f, int v, int a, double beta, double inv_h) {
   double f0 = f.at(v, 0, 0, 0);
   int s = beta > 0.0 ? 1 : -1;
   double m1 = f.ax(v, a, -s) - f0;
@@ -75,7 +75,7 @@ __device__ __forceinline__ double adv_o4(const P& f, int v, int a, double beta, 
 
 // Kreiss-Oliger dissipation along one axis, undivided: s3 - 6 s2 + 15 s1
 template <class P>
-__device__ __forceinline__ double ko5_axis(const P& f, int v, int a) {
+CHM_HD double ko5_axis(const P& f, int v, int a) {
   double f0 = f.at(v, 0, 0, 0);
   double s1 = (f.ax(v, a, 1) - f0) + (f.ax(v, a, -1) - f0);
   double s2 = (f.ax(v, a, 2) - f0) + (f.ax(v, a, -2) - f0);
@@ -84,12 +84,12 @@ __device__ __forceinline__ double ko5_axis(const P& f, int v, int a) {
 }
 
 template <class P>
-__device__ __forceinline__ double ko5(const P& f, int v, double ko) {
+CHM_HD double ko5(const P& f, int v, double ko) {
   return ko * ((ko5_axis(f, v, 0) + ko5_axis(f, v, 1)) + ko5_axis(f, v, 2));
 }
 // dissipation with the five weights of Coef::kq (order 5 or 9; needs 5 ghost zones): 8th-order BSSN kernels
 template <class P>
-__device__ __forceinline__ double ko_kq(const P& f, int v, const double* kq) {
+CHM_HD double ko_kq(const P& f, int v, const double* kq) {
   const double f0 = f.at(v, 0, 0, 0);
   double r = 0.0;
 #pragma unroll
@@ -106,7 +106,7 @@ __device__ __forceinline__ double ko_kq(const P& f, int v, const double* kq) {
 // ---- 8th order (wave systems) ------------------------------------------------------------------------
 // 1st derivative (3,-32,168,-672,0,672,-168,32,-3)/840h
 template <class P>
-__device__ __forceinline__ double d1_o8(const P& f, int v, int a, double inv_h) {
+CHM_HD double d1_o8(const P& f, int v, int a, double inv_h) {
   double e1 = f.ax(v, a, 1) - f.ax(v, a, -1);
   double e2 = f.ax(v, a, 2) - f.ax(v, a, -2);
   double e3 = f.ax(v, a, 3) - f.ax(v, a, -3);
@@ -116,7 +116,7 @@ __device__ __forceinline__ double d1_o8(const P& f, int v, int a, double inv_h) 
 
 // mixed derivative: the 1-D first-derivative stencil along a applied to the one along b (64 points)
 template <class P>
-__device__ __forceinline__ double dmix_o8(const P& f, int v, int a, int b, double inv_h2) {
+CHM_HD double dmix_o8(const P& f, int v, int a, int b, double inv_h2) {
   double r[8];
   const int off[8] = {1, -1, 2, -2, 3, -3, 4, -4};
 #pragma unroll
@@ -135,7 +135,7 @@ __device__ __forceinline__ double dmix_o8(const P& f, int v, int a, int b, doubl
 // beta^a * upwinded d_a f at 8th order: offsets -3..+5 on the side of beta,
 // (-5, 60, -420, -378, 1050, -420, 140, -30, 3)/840h, in differences from the centre value (5 ghosts)
 template <class P>
-__device__ __forceinline__ double adv_o8(const P& f, int v, int a, double beta, double inv_h) {
+CHM_HD double adv_o8(const P& f, int v, int a, double beta, double inv_h) {
   const double f0 = f.at(v, 0, 0, 0);
   const int s = beta > 0.0 ? 1 : -1;
   const double m3 = f.ax(v, a, -3 * s) - f0, m2 = f.ax(v, a, -2 * s) - f0, m1 = f.ax(v, a, -s) - f0;
@@ -148,7 +148,7 @@ __device__ __forceinline__ double adv_o8(const P& f, int v, int a, double beta, 
 
 // 2nd derivative (-9,128,-1008,8064,-14350,8064,-1008,128,-9)/5040h^2
 template <class P>
-__device__ __forceinline__ double d2_o8(const P& f, int v, int a, double inv_h2) {
+CHM_HD double d2_o8(const P& f, int v, int a, double inv_h2) {
   double f0 = f.at(v, 0, 0, 0);
   double s1 = (f.ax(v, a, 1) - f0) + (f.ax(v, a, -1) - f0);
   double s2 = (f.ax(v, a, 2) - f0) + (f.ax(v, a, -2) - f0);
@@ -156,5 +156,29 @@ __device__ __forceinline__ double d2_o8(const P& f, int v, int a, double inv_h2)
   double s4 = (f.ax(v, a, 4) - f0) + (f.ax(v, a, -4) - f0);
   return ((8064.0 * s1 - 1008.0 * s2) + (128.0 * s3 - 9.0 * s4)) * (inv_h2 * (1.0 / 5040.0));
 }
+
+// differentiates on the fly from a point accessor P
+template <class P, int ORDER = 4>
+struct OnTheFly {
+  P pt;
+  Coef C;
+  double beta[3];
+  CHM_HD double f(int v) const { return pt.at(v, 0, 0, 0); }
+  CHM_HD double d1(int v, int a) const {
+    return ORDER == 4 ? d1_o4(pt, v, a, C.inv_h) : d1_o8(pt, v, a, C.inv_h);
+  }
+  CHM_HD double d2(int v, int a, int b) const {
+    if (ORDER == 4) return a == b ? d2_o4(pt, v, a, C.inv_h2) : dmix_o4(pt, v, a, b, C.inv_h2);
+    return a == b ? d2_o8(pt, v, a, C.inv_h2) : dmix_o8(pt, v, a, b, C.inv_h2);
+  }
+  CHM_HD double adv(int v, int a) const {
+    return ORDER == 4 ? adv_o4(pt, v, a, beta[a], C.inv_h) : adv_o8(pt, v, a, beta[a], C.inv_h);
+  }
+  CHM_HD double ad(int v) const {
+    double r = ORDER == 4 ? ko5(pt, v, C.ko) : ko_kq(pt, v, C.kq);
+    if (v != V_A) r += (adv(v, 0) + adv(v, 1)) + adv(v, 2);
+    return r;
+  }
+};
 
 }  // namespace chm
