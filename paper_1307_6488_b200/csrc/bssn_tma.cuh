@@ -8,12 +8,44 @@
 // it is complete.  Mathematics: readings S2-S6, S10 of DESIGN.md (same system as bssn_point.cuh; that file
 // serves the split variant).
 #pragma once
+#ifndef CHM_EMULATE
 #include <cuda.h>
+#endif
 
 #include "bssn_point.cuh"
 
 namespace chm {
 
+// ---- TMA / mbarrier: host emulation (tests/native/cta_emu.hpp; the kernel source is compiled unchanged) ------------
+#ifdef CHM_EMULATE
+#define CHM_DYNAMIC_SMEM(name) unsigned char* name = chm_emu::t_cta->smem
+inline uint32_t smem_u32(const void* p) { return chm_emu::smem_offset(p); }
+inline void mbar_init(uint64_t* bar, int count) { chm_emu::mbar_init(bar, count); }
+inline void mbar_expect_tx(uint64_t* bar, uint32_t bytes) { chm_emu::mbar_expect_tx(bar, bytes); }
+inline bool mbar_try(uint32_t bar, uint32_t parity) { return chm_emu::mbar_try_wait(chm_emu::smem_at(bar), parity); }
+constexpr long long kWaitBudget = 120000000000LL;   // nanoseconds here: 256 OS threads on a few cores are slow
+inline void mbar_wait(uint64_t* bar, uint32_t parity, unsigned* err, unsigned code) {
+  const uint32_t b = smem_u32(bar);
+  const long long t0 = clock64();
+  for (unsigned it = 1;; ++it) {
+    if (mbar_try(b, parity)) return;
+    if (*reinterpret_cast<volatile unsigned*>(err) != 0u) return;
+    if (clock64() - t0 > kWaitBudget) { atomicCAS(err, 0u, code); return; }
+  }
+}
+inline void tma_load_4d(void* dst, const CUtensorMap* tm, uint64_t* bar, int x, int y, int z, int v) {
+  chm_emu::tma_load_4d(dst, tm, bar, x, y, z, v);
+}
+inline uint64_t l2_policy_evict_first() { return 0; }
+inline uint64_t l2_policy_normal() { return 0; }
+inline void tma_load_4d_hint(void* dst, const CUtensorMap* tm, uint64_t* bar, int x, int y, int z, int v, uint64_t) {
+  chm_emu::tma_load_4d(dst, tm, bar, x, y, z, v);
+}
+inline bool mbar_arrive_is_last(uint64_t* bar) { return chm_emu::mbar_arrive(bar) == 1; }
+inline void fence_mbar_init() {}
+template <int COUNT> inline void named_barrier(int id) { chm_emu::sync_named(id, COUNT); }
+#else
+#define CHM_DYNAMIC_SMEM(name) extern __shared__ __align__(128) unsigned char name[]
 // ---- TMA / mbarrier PTX wrappers ----------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -98,6 +130,22 @@ __device__ __forceinline__ unsigned smem_add_relaxed(unsigned* p, unsigned v) {
   return old;
 }
 
+// mbarrier initialisation made visible to the async proxy (TMA) before the first load is issued
+__device__ __forceinline__ void fence_mbar_init() {
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+// named barrier `id` (1..15) over COUNT threads
+template <int COUNT>
+__device__ __forceinline__ void named_barrier(int id) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(COUNT) : "memory");
+}
+#endif   // CHM_EMULATE
+
+#ifdef CHM_EMULATE   // tensor memory is not emulated: no instantiated tile parks values (TmaCfg::HEAVY is false for all)
+template <int N> inline void tmem_park(uint32_t, int, const double*) { abort(); }
+template <int N> inline void tmem_unpark(uint32_t, int, double*) { abort(); }
+#else
 // ---- tensor memory as a per-thread parking area (tcgen05.st / tcgen05.ld, shape 32x32b: lane i of warp w owns TMEM
 // lane 32*(w%4)+i; a double takes two 32-bit columns).  All 32 lanes of the warp must execute these together.
 // The wait after a load names the loaded registers as in/out operands, so no use of them can be scheduled above it.
@@ -172,6 +220,8 @@ __device__ __forceinline__ void tmem_unpark(uint32_t base, int first, double* x)
   if (N - i >= 4) { tmem_ld4(base + 2 * (first + i), x + i); i += 4; }
   if (N - i >= 2) tmem_ld2(base + 2 * (first + i), x + i);
 }
+
+#endif   // CHM_EMULATE
 
 // ---- stencil reads from the staged box -------------------------------------------------------------------------
 // `c` points at this thread's own grid point inside the current slot; BX, BY are the box row / plane extents.

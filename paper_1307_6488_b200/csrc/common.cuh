@@ -1,7 +1,9 @@
 // common.cuh -- shared declarations of libchemora's translation units (host + device).
 // Part of the CUDA product path; shares nothing with oracle/.
 #pragma once
+#ifndef CHM_EMULATE   // tests/native/cta_emu.hpp stands in for the CUDA headers when the kernel source is compiled for the host
 #include <cuda_runtime.h>
+#endif
 #ifndef CHM_STCS
 #define CHM_STCS 1
 #endif

@@ -7,7 +7,9 @@
 // above it is processed; the read-once RK4 operands carry an L2 evict-first policy and stores are streaming.
 // See bssn_tma.cuh for the design; DESIGN.md "Kernels" for the roofline that bounds it.
 #include "bssn_tma.cuh"
+#ifndef CHM_EMULATE
 #include "tma_check.cuh"
+#endif
 
 #ifndef CHM_L2HINT
 #define CHM_L2HINT 1
@@ -72,7 +74,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
   constexpr bool TMEM = PARK;
   // parking map (offsets in doubles inside the thread's 84-double area)
   constexpr int P_CU = 0, P_DG = 18, P_DB = 42, P_LG = 52, P_AT = 58, P_ADG = 64, P_GN = 68, P_DCA = 72, P_AU = 78;
-  extern __shared__ __align__(128) unsigned char smem_raw[];
+  CHM_DYNAMIC_SMEM(smem_raw);
   double* sm = reinterpret_cast<double*>(smem_raw);   // dynamic smem base: 128-byte aligned (no static smem)
   double* cbuf = sm + Cfg::cen_off(0);                                 // [kCenVars][TILE]
   double* dbuf = sm + Cfg::dbuf_off();                                 // [2][DB] shared first derivatives
@@ -94,8 +96,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < kSlots + 1; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NW); }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    fence_mbar_init();
   }
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(empty + kSlots + 1);
   int* org = reinterpret_cast<int*>((reinterpret_cast<uintptr_t>(tmem_slot + 1) + 15) & ~uintptr_t(15));   // [4][4]
@@ -282,7 +283,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
           else Dz[(lz * (TY + 2 * HM) + hy + HM) * DYX + xx + HM] = v;
         }
         done(o);
-        asm volatile("bar.sync %0, %1;" ::"r"(1 + lz), "n"(PLANE) : "memory");
+        named_barrier<PLANE>(1 + lz);
       } else if constexpr (TX * TY == 32) {
         // One z-plane of the tile = one warp: the warp fills its own plane's halo entries; no barrier at all.
 #pragma unroll
@@ -631,7 +632,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
         const int e = (s < 3 ? s : s - 3) * PLANE + u0;
         return e < NY ? b + lz * NY + e : b + Cfg::DY_N + lz * NZ + (e - NY);
       };
-      asm volatile("bar.sync %0, %1;" ::"r"(1 + lz), "n"(PLANE) : "memory");
+      named_barrier<PLANE>(1 + lz);
       const double trX = sdot(gu, Rt);
 #pragma unroll
       for (int i2 = 0; i2 < 3; ++i2)
@@ -734,6 +735,7 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
   }
 }
 
+#ifndef CHM_EMULATE
 // ---- host side: tensor map + launch -----------------------------------------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -877,5 +879,7 @@ cudaError_t kernel_info_bssn_fused(int order, int tile, cudaFuncAttributes* a) {
   Layout L{}; Coef C{};
   return tma_dispatch(order, tile, L, C, nullptr, 0, a);
 }
+
+#endif   // CHM_EMULATE
 
 }  // namespace chm

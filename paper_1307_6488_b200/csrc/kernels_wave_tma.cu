@@ -8,7 +8,9 @@
 // whose returned state tells the last arriver, see bssn_tma.cuh); the last warp out issues the slot's next load.
 #include "bssn_tma.cuh"
 #include "stencils.cuh"
+#ifndef CHM_EMULATE
 #include "tma_check.cuh"
+#endif
 
 namespace chm {
 
@@ -51,7 +53,7 @@ __global__ void __launch_bounds__(TX* TY, 1)
 wave_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage st, int ntx, int nty, int ntz) {
   using K = wv::Cfg<ORDER, KO, TX, TY, NV>;
   constexpr int R = K::R, ROW = K::ROW, PB = K::PB, SLOT = K::SLOT, NP = K::NP, PF = K::PF;
-  extern __shared__ __align__(128) unsigned char smem_raw[];
+  CHM_DYNAMIC_SMEM(smem_raw);
   double* sm = reinterpret_cast<double*>(smem_raw);
   uint64_t* full = reinterpret_cast<uint64_t*>(sm + NP * SLOT);   // [NP] plane arrived
   uint64_t* empty = full + NP;                                     // [NP] plane released by all warps
@@ -60,8 +62,7 @@ wave_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < NP; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], K::NW); }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    fence_mbar_init();
   }
   __syncthreads();
 
@@ -162,6 +163,7 @@ wave_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
   }
 }
 
+#ifndef CHM_EMULATE
 // ---- host side ------------------------------------------------------------------------------------------------
 typedef CUresult (*WvEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -320,5 +322,7 @@ cudaError_t kernel_info_wave_tma(int order, int which, cudaFuncAttributes* a) {
   Layout L{}; Coef C{};
   return wv_dispatch(order, true, which, L, C, nullptr, 0, a);
 }
+
+#endif   // CHM_EMULATE
 
 }  // namespace chm
