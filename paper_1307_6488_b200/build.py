@@ -10,7 +10,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libchemora.so")
-SOURCES = ["chemora.cu", "kernels_basic.cu", "kernels_bssn.cu", "kernels_bssn_tma.cu", "kernels_wave_tma.cu"]
+SOURCES = ["chemora.cu", "kernels_basic.cu", "kernels_boundary.cu", "kernels_bssn.cu", "kernels_bssn_tma.cu", "kernels_wave_tma.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

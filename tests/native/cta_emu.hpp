@@ -97,6 +97,7 @@ struct Cta {
   int nthreads = 0;
   Barrier all;
   std::vector<std::unique_ptr<Barrier>> warp, named;
+  std::vector<double> shfl;                       // one slot per thread: warp shuffles
   std::mutex bars_m;
   std::map<size_t, std::unique_ptr<MBar>> bars;   // keyed by shared-memory offset
   long tma_loads = 0, tma_bytes = 0;              // statistics
@@ -183,17 +184,27 @@ inline void tma_load_4d(void* dst, const CUtensorMap* tm, void* bar, int x, int 
 inline void sync_all() { t_cta->all.wait(t_cta->nthreads); }
 inline void sync_warp() { t_cta->warp[(t_threadIdx.y * t_blockDim.x + t_threadIdx.x) / 32]->wait(32); }
 inline void sync_named(int id, int count) { t_cta->named[id]->wait(count); }
+inline double shfl_xor(double v, int lane_mask) {   // all 32 threads of the warp call it together
+  const int t = t_threadIdx.y * t_blockDim.x + t_threadIdx.x;
+  t_cta->shfl[t] = v;
+  sync_warp();
+  const double r = t_cta->shfl[(t & ~31) | ((t ^ lane_mask) & 31)];
+  sync_warp();
+  return r;
+}
 
 // run `grid` CTAs of `threads` (x * y) threads one after the other; body() is the kernel call
 struct Stats { long tma_loads = 0, tma_bytes = 0; };
-inline Stats run_grid(int grid, int bx, int by, size_t smem_bytes, const std::function<void()>& body) {
+inline Stats run_grid(int grid, int bx, int by, size_t smem_bytes, const std::function<void()>& body, int grid_y = 1) {
   Stats st;
+  for (int by_ = 0; by_ < grid_y; ++by_)
   for (int b = 0; b < grid; ++b) {
     Cta cta;
     cta.smem_bytes = smem_bytes;
     cta.smem = (unsigned char*)aligned_alloc(128, (smem_bytes + 127) / 128 * 128);
     memset(cta.smem, 0xff, smem_bytes);   // NaN pattern: reading what was never loaded shows up
     cta.nthreads = bx * by;
+    cta.shfl.assign(cta.nthreads, 0.0);
     for (int w = 0; w < (cta.nthreads + 31) / 32; ++w) cta.warp.emplace_back(new Barrier());
     for (int i = 0; i < 16; ++i) cta.named.emplace_back(new Barrier());
     std::vector<std::thread> th;
@@ -201,8 +212,8 @@ inline Stats run_grid(int grid, int bx, int by, size_t smem_bytes, const std::fu
       th.emplace_back([&, t] {
         t_cta = &cta;
         t_threadIdx = Idx3{(unsigned)(t % bx), (unsigned)(t / bx), 0};
-        t_blockIdx = Idx3{(unsigned)b, 0, 0};
-        t_gridDim = Idx3{(unsigned)grid, 1, 1};
+        t_blockIdx = Idx3{(unsigned)b, (unsigned)by_, 0};
+        t_gridDim = Idx3{(unsigned)grid, (unsigned)grid_y, 1};
         t_blockDim = Idx3{(unsigned)bx, (unsigned)by, 1};
         body();
       });
@@ -227,6 +238,14 @@ inline double __dsub_rn(double a, double b) { return a - b; }
 inline double __dmul_rn(double a, double b) { return a * b; }
 template <class T> inline void __stcs(T* p, T v) { *p = v; }
 template <class T> inline T __ldg(const T* p) { return *p; }
+inline double __shfl_xor_sync(unsigned, double v, int lane_mask) { return chm_emu::shfl_xor(v, lane_mask); }
+inline double __longlong_as_double(long long x) { double d; memcpy(&d, &x, 8); return d; }
+inline long long __double_as_longlong(double d) { long long x; memcpy(&x, &d, 8); return x; }
+inline unsigned long long atomicMax(unsigned long long* p, unsigned long long v) {
+  unsigned long long old = __atomic_load_n(p, __ATOMIC_SEQ_CST);
+  while (old < v && !__atomic_compare_exchange_n(p, &old, v, false, __ATOMIC_SEQ_CST, __ATOMIC_SEQ_CST)) {}
+  return old;
+}
 inline long long clock64() {
   return std::chrono::duration_cast<std::chrono::nanoseconds>(std::chrono::steady_clock::now().time_since_epoch()).count();
 }
