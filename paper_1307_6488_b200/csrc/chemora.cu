@@ -646,7 +646,7 @@ int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, 
 // The paper's tile cost model for the uniform fused BSSN kernel; see include/chemora.h.
 int chemora_tile_cost(int fd_order, int ghost, int tile_id, double* sigma, long* requests, long* points) {
   if (fd_order != 4 && fd_order != 8) return CHEMORA_EINVAL;
-  if (tile_id < 0 || tile_id >= kNumFused) return CHEMORA_EINVAL;
+  if (tile_id < 0 || tile_id >= 5) return CHEMORA_EINVAL;   // the five tile shapes of the plain section layout
   if (fd_order == 8 && tile_id != 0) return CHEMORA_EINVAL;
   const int H = fd_order / 2 + 1;
   if (ghost < H) return CHEMORA_EINVAL;

@@ -133,8 +133,8 @@ __device__ __forceinline__ void stage_emit_t(const Stage& st, long q, double k, 
 // Tile shapes of the variant sweep.  Fused kernel: 3-D tile, one point per thread.  Split kernels and the wave
 // kernel: x,y = thread block, z = planes marched per block.
 struct TileShape { int tx, ty, tz; };
-constexpr int kNumFused = 5;   // fused BSSN tile ids 0..4 (8th order: id 0 only)
-static const TileShape kTilesFused[kNumFused] = {{16, 4, 4}, {16, 8, 2}, {8, 4, 8}, {16, 2, 8}, {16, 4, 2}};
+constexpr int kNumFused = 6;   // fused BSSN tile ids 0..5 (8th order: id 0 only); id 5: 16x4x4 with the interleaved section layout
+static const TileShape kTilesFused[kNumFused] = {{16, 4, 4}, {16, 8, 2}, {8, 4, 8}, {16, 2, 8}, {16, 4, 2}, {16, 4, 4}};
 // wave system ids 6..8: the TMA plane-ring kernel (x, y = thread block, z = planes per work item)
 static const TileShape kTilesWaveTma[3] = {{32, 16, 32}, {32, 16, 64}, {64, 8, 32}};
 // Sample-1 system ids 6..8: the same plane-ring kernel with five variables (smaller tiles: the ring holds 5 boxes a plane)

@@ -6,6 +6,8 @@
 // (full x extent, Layout::col_rows rows of y, all z) so that the z-halo of a box is still in L2 when the tile
 // above it is processed; the read-once RK4 operands carry an L2 evict-first policy and stores are streaming.
 // See bssn_tma.cuh for the design; DESIGN.md "Kernels" for the roofline that bounds it.
+#include <type_traits>
+
 #include "bssn_tma.cuh"
 #ifndef CHM_EMULATE
 #include "tma_check.cuh"
@@ -28,8 +30,51 @@ __host__ __device__ __forceinline__ constexpr int emit_var(int o, int n) {
          : o < 24 ? (n == 0 ? V_GAM + (o - 21) : V_B + (o - 21)) : (n == 0 ? V_A : -1);
 }
 
-template <int TX, int TY, int TZ, int ORDER = 4>
+// ---- interleaved section layout (IL) -----------------------------------------------------
+// The plain layout ends every tile with ten cheap sections (At_ij x6, B^i x3, A: 18 reads and ~57 FP64 each) that
+// consume a 17.6 KB box every ~500 cycles and outrun the TMA fill (profiles/r01_l: 14 % of all warp-stall samples
+// wait for those boxes).  IL evaluates the advection + dissipation stencil of At_ij and B^i EARLY, between the
+// expensive beta^i / gt_ij sections, parks the one double per point it yields in a per-thread table in shared
+// memory, and ends the tile with three box-less EMIT sections that only fetch Runge-Kutta operand tiles (eight per
+// section, requested five sections ahead, i.e. under the expensive chi / alpha / K sections) plus two empty ones:
+//   o:  0 b1 | 1 At11* | 2 b2 | 3 At12* | 4 b3 | 5 At13* | 6 gt11 | 7 At22* | 8 gt12 | 9 At23* | 10 gt13 | 11 At33* |
+//       12 gt22 | 13 B1* | 14 gt23 | 15 B2* | 16 gt33 | 17 B3* | 18 Gt1 | 19 A | 20 Gt2 | 21 Gt3 | 22 chi | 23 alpha |
+//       24 K | 25 emit At11..At22 | 26 emit At23, At33, Gt1, Gt2 | 27 emit Gt3, B1..B3 | 28, 29 empty
+// 30 = 6 x 5 sections: slot = o mod 5 and parity = (o / 5) & 1 are compile-time constants of a section.
+struct SecIL {
+  static constexpr int N = 30;
+  __host__ __device__ static constexpr int beta(int i) { return 2 * i; }
+  __host__ __device__ static constexpr int at(int s) { return s < 3 ? 1 + 2 * s : 7 + 2 * (s - 3); }
+  __host__ __device__ static constexpr int gt(int s) { return 6 + 2 * s; }
+  __host__ __device__ static constexpr int b(int i) { return 13 + 2 * i; }
+  __host__ __device__ static constexpr int gam(int k) { return k == 0 ? 18 : 19 + k; }
+  static constexpr int a = 19, chi = 22, alpha = 23, k = 24, emit0 = 25;
+  // variable whose box section o stages (-1: none)
+  __host__ __device__ static constexpr int var(int o) {
+    return o < 6 ? ((o & 1) ? V_AT + o / 2 : V_BETA + o / 2)
+           : o < 12 ? ((o & 1) ? V_AT + 3 + (o - 7) / 2 : V_GT + (o - 6) / 2)
+           : o < 18 ? ((o & 1) ? V_B + (o - 13) / 2 : V_GT + (o - 6) / 2)
+           : o == 18 ? V_GAM : o == 19 ? V_A : o < 22 ? V_GAM + (o - 19) : o == 22 ? V_CHI : o == 23 ? V_ALPHA
+           : o == 24 ? V_K : -1;
+  }
+  // variable whose right-hand side leaves in box section o, with its operand tiles next to the box (-1: none)
+  __host__ __device__ static constexpr int emit(int o) {
+    return o < 18 ? ((o & 1) ? -1 : var(o)) : (o == 19 || o == 22 || o == 23 || o == 24) ? var(o) : -1;
+  }
+};
+struct SecPlain {
+  static constexpr int N = 25;
+  __host__ __device__ static constexpr int beta(int i) { return i; }
+  __host__ __device__ static constexpr int gt(int s) { return 3 + s; }
+  __host__ __device__ static constexpr int gam(int k) { return 9 + k; }
+  __host__ __device__ static constexpr int at(int s) { return 15 + s; }
+  __host__ __device__ static constexpr int b(int i) { return 21 + i; }
+  static constexpr int chi = 12, alpha = 13, k = 14, a = 24;
+};
+
+template <int TX, int TY, int TZ, int ORDER = 4, bool IL = false>
 struct TmaCfg {
+  static_assert(!IL || (ORDER == 4 && TX * TY * TZ == 256), "the interleaved layout is built for 4th order, 256-point tiles");
   static constexpr int H = ORDER == 8 ? 5 : 3;    // halo: upwinded stencils reach order/2 + 1 cells
   static_assert(TX % 2 == 0 && ((TX + 2) * TY * TZ) % 16 == 0, "tile boxes must stay 128-byte aligned in smem");
   static constexpr int BX = TX + 2 * H, BY = TY + 2 * H, BZ = TZ + 2 * H;
@@ -52,32 +97,42 @@ struct TmaCfg {
   // (planes of 128 threads: measured no gain over the one-pass form)
   static constexpr bool TWOPASS = !HEAVY && (TX * TY == 64 || TX * TY == 32);
   static constexpr int DB = TWOPASS ? (DY_N + DZ_N + 15) / 16 * 16 : 0;
-  static constexpr size_t SMEM = (size_t)(NS * SLOTX + CEN + 2 * DB) * 8 + (NS + 1) * 8 + (NS + 1) * 8 + 64 + 16 + 64 + 128;
+  // IL: per-thread table of parked values: the advection + dissipation results of At_ij (6) and B^i (3), and B^i (3)
+  static constexpr int TAB = IL ? 12 * THREADS : 0;
+  static_assert(!IL || 8 * TILE <= SLOTX, "the eight operand tiles of an emit section must fit one ring slot");
+  static constexpr size_t SMEM = (size_t)(NS * SLOTX + CEN + 2 * DB + TAB) * 8 + (NS + 1) * 8 + (NS + 1) * 8 + 64 + 16 + 64 + 128;
   static constexpr int NWARPS = THREADS / 32;
   // shared-memory map in doubles from the dynamic base (the kernel and the host-side validator both use these)
   __host__ __device__ static constexpr int box_off(int slot) { return slot * SLOTX; }
   __host__ __device__ static constexpr int op_off(int slot, int n) { return slot * SLOTX + SLOT + n * TILE; }   // n: U0, S0, U1, S1
   __host__ __device__ static constexpr int cen_off(int group) { return NS * SLOTX + 7 * group * TILE; }        // three 7-variable groups
   __host__ __device__ static constexpr int dbuf_off() { return NS * SLOTX + CEN; }
-  __host__ __device__ static constexpr int bar_off() { return NS * SLOTX + CEN + 2 * DB; }                      // full[NS], cfull, empty[NS + 1]
+  __host__ __device__ static constexpr int tab_off() { return NS * SLOTX + CEN + 2 * DB; }
+  __host__ __device__ static constexpr int eop_off(int slot, int n) { return slot * SLOTX + n * TILE; }   // IL emit sections: U0..U3, S0..S3
+  __host__ __device__ static constexpr int bar_off() { return NS * SLOTX + CEN + 2 * DB + TAB; }                      // full[NS], cfull, empty[NS + 1]
 };
-template <int TX, int TY, int TZ, int MODE, int ORDER>
-__global__ void __launch_bounds__(TX* TY* TZ, 1)
-bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ CUtensorMap tmCen,
-                const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS, Layout L, Coef C, Stage st, int ntx, int nty, int ntz, int cy) {
-  using Cfg = TmaCfg<TX, TY, TZ, ORDER>;
+// the kernel body; tmU4 / tmS4 / tmU3 / tmS3: operand maps with 4 and 3 consecutive variables per box (IL emit sections)
+template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL>
+__device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUtensorMap& tmCen, const CUtensorMap& tmU,
+                                              const CUtensorMap& tmS, const CUtensorMap& tmU4, const CUtensorMap& tmS4,
+                                              const CUtensorMap& tmU3, const CUtensorMap& tmS3, const Layout& L,
+                                              const Coef& C, const Stage& st, int ntx, int nty, int ntz, int cy) {
+  using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL>;
   constexpr int H = Cfg::H;
   constexpr int BX = Cfg::BX, BY = Cfg::BY, SLOT = Cfg::SLOT, SLOTX = Cfg::SLOTX, TILE = Cfg::TILE, CEN = Cfg::CEN;
   constexpr unsigned NW = Cfg::NWARPS;
   constexpr int kSlots = Cfg::NS;
   constexpr bool PARK = Cfg::PARK;
   constexpr bool TMEM = PARK;
+  using Sec = std::conditional_t<IL, SecIL, SecPlain>;
+  constexpr int NSEC = Sec::N;   // sections per tile: the ring position of section o of tile t is NSEC t + o
   // parking map (offsets in doubles inside the thread's 84-double area)
   constexpr int P_CU = 0, P_DG = 18, P_DB = 42, P_LG = 52, P_AT = 58, P_ADG = 64, P_GN = 68, P_DCA = 72, P_AU = 78;
   CHM_DYNAMIC_SMEM(smem_raw);
   double* sm = reinterpret_cast<double*>(smem_raw);   // dynamic smem base: 128-byte aligned (no static smem)
   double* cbuf = sm + Cfg::cen_off(0);                                 // [kCenVars][TILE]
   double* dbuf = sm + Cfg::dbuf_off();                                 // [2][DB] shared first derivatives
+  double* tabp = sm + Cfg::tab_off() + threadIdx.x;                    // IL: this thread's parked values, entry e at e * THREADS
   uint64_t* full = reinterpret_cast<uint64_t*>(sm + Cfg::bar_off());   // [kSlots] boxes, then [1] point values
   uint64_t* cfull = full + kSlots;
   uint64_t* empty = cfull + 1;                                         // [kSlots] + [1]: warps that left a buffer
@@ -138,6 +193,36 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
   };
   // box of variable order o of the tile whose origin (padded, minus halo) is (x0,y0,z0); issued by one thread
   auto issue = [&](int o, int slot, int x0, int y0, int z0) {
+    if constexpr (IL) {
+      const int tx0 = x0 + H - 1, ty0 = y0 + H, tz0 = z0 + H;   // tile-box origin
+      if (o >= SecIL::emit0) {
+        // emit sections: eight operand tiles (U of four variables, then S of the same four) and no box; the two
+        // empty sections, and the emit sections of a plain right-hand-side evaluation (no operands), complete
+        // their phase with the issuer's arrival alone
+        if (o >= SecIL::emit0 + 3 || nops == 0) { mbar_arrive_is_last(&full[slot]); return; }
+        mbar_expect_tx(&full[slot], (uint32_t)(4 * nops) * Cfg::TILE_BYTES);
+        const int e = o - SecIL::emit0;
+        double* base = sm + Cfg::eop_off(slot, 0);
+        if (e < 2) {        // At11..At22 (variables 8..11) / At23, At33, Gt1, Gt2 (variables 12..15): one box each
+          tma_load_4d_hint(base, &tmU4, &full[slot], tx0, ty0, tz0, V_AT + 4 * e, pol_stream);
+          if (nops == 2) tma_load_4d_hint(base + 4 * TILE, &tmS4, &full[slot], tx0, ty0, tz0, V_AT + 4 * e, pol_stream);
+        } else {            // Gt3 (variable 16), then B1..B3 (variables 21..23)
+          tma_load_4d_hint(base, &tmU, &full[slot], tx0, ty0, tz0, V_GAM + 2, pol_stream);
+          tma_load_4d_hint(base + TILE, &tmU3, &full[slot], tx0, ty0, tz0, V_B, pol_stream);
+          if (nops == 2) {
+            tma_load_4d_hint(base + 4 * TILE, &tmS, &full[slot], tx0, ty0, tz0, V_GAM + 2, pol_stream);
+            tma_load_4d_hint(base + 5 * TILE, &tmS3, &full[slot], tx0, ty0, tz0, V_B, pol_stream);
+          }
+        }
+        return;
+      }
+      const int ve = SecIL::emit(o);
+      mbar_expect_tx(&full[slot], Cfg::BOX_BYTES + (uint32_t)(ve >= 0 ? nops : 0) * Cfg::TILE_BYTES);
+      tma_load_4d(sm + Cfg::box_off(slot), &tm, &full[slot], x0, y0, z0, SecIL::var(o));
+      if (ve >= 0 && nops >= 1) tma_load_4d_hint(sm + Cfg::op_off(slot, 0), &tmU, &full[slot], tx0, ty0, tz0, ve, pol_stream);
+      if (ve >= 0 && nops == 2) tma_load_4d_hint(sm + Cfg::op_off(slot, 1), &tmS, &full[slot], tx0, ty0, tz0, ve, pol_stream);
+      return;
+    }
     const int v0 = emit_var(o, 0), v1 = emit_var(o, 1);
     const int nem = (v0 >= 0) + (v1 >= 0);
     mbar_expect_tx(&full[slot], Cfg::BOX_BYTES + (uint32_t)(nops * nem) * Cfg::TILE_BYTES);
@@ -200,7 +285,15 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     // read after box(o) and before done(o)
     // ring slot and mbarrier parity of section o of this CTA's t-th tile (load number 25 t + o)
     auto slot_of = [&](int o) { return kSlots == 5 ? o % 5 : (25 * t + o) % kSlots; };
-    auto parity_of = [&](int o) { return (uint32_t)(kSlots == 5 ? (t + o / 5) & 1 : ((25 * t + o) / kSlots) & 1); };
+    auto parity_of = [&](int o) {
+      if constexpr (IL) return (uint32_t)(o / 5) & 1u;   // 30 sections = 6 phases of a slot per tile: no dependence on t
+      else return (uint32_t)(kSlots == 5 ? (t + o / 5) & 1 : ((25 * t + o) / kSlots) & 1);
+    };
+    // IL emit sections: operands (U, S) of the n-th variable of the section (U tiles 0..3, S tiles 4..7 of the slot)
+    auto pre_e = [&](int o, int n) {
+      const double* op = sm + Cfg::eop_off(slot_of(o), n) + toff;
+      return StagePre{op[0], op[4 * TILE]};
+    };
     auto pre = [&](int o, int n) {
       const double* op = sm + slot_of(o) * SLOTX + SLOT + 2 * n * TILE + toff;
       return StagePre{op[0], op[TILE]};
@@ -215,10 +308,10 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     };
     auto done = [&](int o) {
       if (leave(slot_of(o))) {   // the refill is load number 25 t + o + kSlots: same slot
-        const int4 a = !Cfg::HEAVY ? (o + kSlots < 25 ? own : nxt)
-                                   : *reinterpret_cast<const int4*>(org + 4 * ((o + kSlots < 25 ? t : t + 1) & 3));
-        if (o + kSlots < 25) issue(o + kSlots, slot_of(o), a.x, a.y, a.z);
-        else if (a.w) issue(o + kSlots - 25, slot_of(o), a.x, a.y, a.z);
+        const int4 a = !Cfg::HEAVY ? (o + kSlots < NSEC ? own : nxt)
+                                   : *reinterpret_cast<const int4*>(org + 4 * ((o + kSlots < NSEC ? t : t + 1) & 3));
+        if (o + kSlots < NSEC) issue(o + kSlots, slot_of(o), a.x, a.y, a.z);
+        else if (a.w) issue(o + kSlots - NSEC, slot_of(o), a.x, a.y, a.z);
       }
     };
     // the point values are last read just before section 3 (At)
@@ -338,6 +431,17 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       }
     };
 
+    // IL: the advection + dissipation stencil of the variable staged by section o, parked in table entry e
+    // (a thread reads back only what it wrote itself: no synchronisation, no hazard across tiles)
+    auto park_ad = [&](int o, int e, const AdvW& w) {
+      auto p = box(o);
+      const double ad = var_ad(p, w);
+      done(o);
+      tabp[e * Cfg::THREADS] = ad;
+    };
+    // IL: wait for a box-less section (operand tiles only, or nothing)
+    auto wait_sec = [&](int o) { mbar_wait(&full[slot_of(o)], parity_of(o), L.err, 0x10000u + (unsigned)o + 1u); };
+
     const double third = 1.0 / 3.0, two_thirds = 2.0 / 3.0;
     mbar_wait(cfull, (uint32_t)(t & 1), L.err, 0x10080u);
     // ---- point values needed before their own boxes arrive: metric, shift ----------------------------------
@@ -371,14 +475,15 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2) {
       const double Bc = cen(V_B + i2);
-      auto p = box(i2);
-      const StagePre pr = pre(i2, 0);
+      auto p = box(Sec::beta(i2));
+      const StagePre pr = pre(Sec::beta(i2), 0);
       double d1[3], d2[6], ad;
-      full_var(p, w, i2, i2, d1, d2, ad);
+      full_var(p, w, Sec::beta(i2), i2, d1, d2, ad);
 #pragma unroll
       for (int a = 0; a < 3; ++a) { db[a][i2] = d1[a]; gdiv[a] = i2 == 0 ? d2[sym(a, i2)] : gdiv[a] + d2[sym(a, i2)]; }
       lapb[i2] = sdot(gu, d2);
       emit(V_BETA + i2, C.sgc * Bc + ad, pr);
+      if constexpr (IL) park_ad(SecIL::at(i2), i2, w);   // At11, At12, At13
     }
     double divb = (db[0][0] + db[1][1]) + db[2][2];
     if constexpr (PARK) {   // needed again only by the Gt^i right-hand side (sections 21..23)
@@ -396,10 +501,10 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 #pragma unroll
       for (int j2 = i2; j2 < 3; ++j2) {
         const int s = sym(i2, j2);
-        auto p = box(3 + s);
-        const StagePre pr = pre(3 + s, 0);
+        auto p = box(Sec::gt(s));
+        const StagePre pr = pre(Sec::gt(s), 0);
         double d1[3], d2[6], ad;
-        full_var(p, w, 3 + s, 3 + s, d1, d2, ad);
+        full_var(p, w, Sec::gt(s), 3 + s, d1, d2, ad);
         if constexpr (PARK) {
           const double d4[4] = {d1[0], d1[1], d1[2], 0.0};
           tmem_park<4>(park, P_DG + 4 * s, d4);
@@ -414,6 +519,16 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
           lie = k2 == 0 ? c : lie + c;
         }
         emit(V_GT + s, (lie - two_thirds * g[s] * divb) - 2.0 * alpha * At[s] + ad, pr);
+        if constexpr (IL) {
+          if (s < 3) park_ad(SecIL::at(3 + s), 3 + s, w);   // At22, At23, At33
+          else {                                             // B1, B2, B3: the stencil result and the point value
+            auto pb = box(SecIL::b(s - 3));
+            const double Bi = pb.at(0, 0, 0), adB = var_ad(pb, w);
+            done(SecIL::b(s - 3));
+            tabp[(6 + s - 3) * Cfg::THREADS] = adB;
+            tabp[(9 + s - 3) * Cfg::THREADS] = Bi;
+          }
+        }
       }
 
     // ---- Christoffels: Cl[k][s(i,j)] = Gamma~_kij, Cu[k][s] = Gamma~^k_ij, Gn[k] = gtu^{ij} Gamma~^k_ij ----
@@ -487,14 +602,27 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
       const double g4[4] = {Gn[0], Gn[1], Gn[2], 0.0};
       tmem_park<4>(park, P_GN, g4);
     }
+    // A (inert slot, dissipation only): the last section of the plain layout, between Gt1 and Gt2 in the interleaved one
+    auto section_A = [&]() {
+      auto p = box(Sec::a);
+      const StagePre pr = pre(Sec::a, 0);
+      const double f0 = p.at(0, 0, 0);
+      double rA;
+      if (ORDER == 4) rA = C.ko * ((axis_q(p, f0, 0) + axis_q(p, f0, 1)) + axis_q(p, f0, 2));
+      else rA = (axis_ko8(p, f0, 0, C) + axis_ko8(p, f0, 1, C)) + axis_ko8(p, f0, 2, C);
+      done(Sec::a);
+      emit(V_A, rA, pr);
+    };
+
     // ---- o = 9..11: Gt^k : R~_ij += 1/2 (gt_ki d_j Gt^k + gt_kj d_i Gt^k); advection kept for the end ------
     double adG[3];
 #pragma unroll
     for (int k2 = 0; k2 < 3; ++k2) {
-      auto p = box(9 + k2);
+      auto p = box(Sec::gam(k2));
       double d1[3];
       if (ORDER == 4) var_d1_ad(p, C, w, d1, adG[k2]); else var_d1_ad8(p, C, w, d1, adG[k2]);
-      done(9 + k2);
+      done(Sec::gam(k2));
+      if constexpr (IL) { if (k2 == 0) section_A(); }
 #pragma unroll
       for (int i2 = 0; i2 < 3; ++i2)
 #pragma unroll
@@ -510,10 +638,10 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     const double ichi = 1.0 / chi;
     double dchi[3];
     {
-      auto p = box(12);
-      const StagePre pr = pre(12, 0);
+      auto p = box(Sec::chi);
+      const StagePre pr = pre(Sec::chi, 0);
       double d2[6], ad;
-      full_var(p, w, 12, 9, dchi, d2, ad);
+      full_var(p, w, Sec::chi, 9, dchi, d2, ad);
       emit(V_CHI, two_thirds * chi * (alpha * trK - divb) + ad, pr);
       double cd[6], cc[6];   // D~_i D~_j chi ; d_i chi d_j chi
       if constexpr (PARK) {   // Gamma~^k_ij one k at a time from tensor memory
@@ -544,10 +672,10 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     // ---- o = 13: alpha : X_ij = alpha R_ij - D_i D_j alpha ; D^2 alpha -----------------------------------------
     double dal[3], lap_alpha;
     {
-      auto p = box(13);
-      const StagePre pr = pre(13, 0);
+      auto p = box(Sec::alpha);
+      const StagePre pr = pre(Sec::alpha, 0);
       double d2[6], ad;
-      full_var(p, w, 13, 10, dal, d2, ad);
+      full_var(p, w, Sec::alpha, 10, dal, d2, ad);
       emit(V_ALPHA, -2.0 * alpha * trK + ad, pr);
       double cd[6], ca[6];   // d_i d_j alpha - Gamma~^k_ij d_k alpha ; d_i chi d_j alpha + d_j chi d_i alpha
       if constexpr (PARK) {
@@ -597,11 +725,11 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     // ---- o = 14: K -------------------------------------------------------------------------------------------
     double dK[3];
     {
-      auto p = box(14);
-      const StagePre pr = pre(14, 0);
+      auto p = box(Sec::k);
+      const StagePre pr = pre(Sec::k, 0);
       double ad;
       if (ORDER == 4) var_d1_ad(p, C, w, dK, ad); else var_d1_ad8(p, C, w, dK, ad);
-      done(14);
+      done(Sec::k);
       emit(V_K, (alpha * (sdot(Au, At) + third * trK * trK) - lap_alpha) + ad, pr);
     }
     if constexpr (PARK) tmem_park<6>(park, P_AU, Au);
@@ -615,6 +743,58 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 #pragma unroll
         for (int b = 0; b < 3; ++b) db[a][b] = t10[3 * a + b];
       divb = t10[9];
+    }
+    if constexpr (IL) {
+      // Interleaved layout: the stencil results of At_ij and B^i were parked early; what is left is pointwise.  All
+      // twelve right-hand sides are formed here, then leave through the three emit sections (operand tiles only).
+      double kAt[6], kG[3], kB[3];
+      const double trX = sdot(gu, Rt);
+#pragma unroll
+      for (int i2 = 0; i2 < 3; ++i2)
+#pragma unroll
+        for (int j2 = i2; j2 < 3; ++j2) {
+          const int s = sym(i2, j2);
+          double AA, lie;
+#pragma unroll
+          for (int k2 = 0; k2 < 3; ++k2) {
+            const double c = At[sym(i2, k2)] * db[j2][k2] + At[sym(j2, k2)] * db[i2][k2];
+            AA = k2 == 0 ? At[sym(i2, k2)] * Am[k2][j2] : AA + At[sym(i2, k2)] * Am[k2][j2];
+            lie = k2 == 0 ? c : lie + c;
+          }
+          const double rest = chi * (Rt[s] - third * g[s] * trX) + alpha * (trK * At[s] - 2.0 * AA) +
+                              (lie - two_thirds * At[s] * divb);
+          kAt[s] = rest + tabp[s * Cfg::THREADS];
+        }
+#pragma unroll
+      for (int i2 = 0; i2 < 3; ++i2) {
+        double r = lapb[i2];
+        double t2 = sdot(Cu[i2], Au);   // Gamma~^i_jk At^{jk}
+#pragma unroll
+        for (int j2 = 0; j2 < 3; ++j2) {
+          r += third * gu[sym(i2, j2)] * gdiv[j2];
+          t2 -= two_thirds * gu[sym(i2, j2)] * dK[j2] + 1.5 * ichi * Au[sym(i2, j2)] * dchi[j2];
+          r -= 2.0 * Au[sym(i2, j2)] * dal[j2] + Gn[j2] * db[j2][i2];
+        }
+        r += 2.0 * alpha * t2 + two_thirds * Gn[i2] * divb;
+        kG[i2] = r + adG[i2];
+        kB[i2] = (r - C.eta * tabp[(9 + i2) * Cfg::THREADS]) + tabp[(6 + i2) * Cfg::THREADS];
+      }
+      constexpr int E = SecIL::emit0;
+      wait_sec(E);          // At11, At12, At13, At22 (variables 8..11)
+      { const StagePre p0 = pre_e(E, 0), p1 = pre_e(E, 1), p2 = pre_e(E, 2), p3 = pre_e(E, 3);
+        done(E);
+        emit(V_AT + 0, kAt[0], p0); emit(V_AT + 1, kAt[1], p1); emit(V_AT + 2, kAt[2], p2); emit(V_AT + 3, kAt[3], p3); }
+      wait_sec(E + 1);      // At23, At33, Gt1, Gt2 (variables 12..15)
+      { const StagePre p0 = pre_e(E + 1, 0), p1 = pre_e(E + 1, 1), p2 = pre_e(E + 1, 2), p3 = pre_e(E + 1, 3);
+        done(E + 1);
+        emit(V_AT + 4, kAt[4], p0); emit(V_AT + 5, kAt[5], p1); emit(V_GAM + 0, kG[0], p2); emit(V_GAM + 1, kG[1], p3); }
+      wait_sec(E + 2);      // Gt3 (variable 16), B1, B2, B3 (variables 21..23)
+      { const StagePre p0 = pre_e(E + 2, 0), p1 = pre_e(E + 2, 1), p2 = pre_e(E + 2, 2), p3 = pre_e(E + 2, 3);
+        done(E + 2);
+        emit(V_GAM + 2, kG[2], p0); emit(V_B + 0, kB[0], p1); emit(V_B + 1, kB[1], p2); emit(V_B + 2, kB[2], p3); }
+      wait_sec(E + 3); done(E + 3);   // the two empty sections keep slot = o mod 5: their release refills the slots
+      wait_sec(E + 4); done(E + 4);   // with the next tile's sections 3 and 4
+      continue;
     }
     if constexpr (Cfg::TWOPASS && TX * TY == 64) {
       // The kernel is bound by instruction fetch at 8th order (150 KB of code), so the six advection stencils are
@@ -651,11 +831,11 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
         }
 #pragma unroll 1
       for (int s = 0; s < 6; ++s) {
-        auto p = box(15 + s);
-        const StagePre pr = pre(15 + s, 0);
+        auto p = box(SecPlain::at(s));
+        const StagePre pr = pre(SecPlain::at(s), 0);
         const double ad = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
         const double rest = *tab(s);
-        done(15 + s);
+        done(SecPlain::at(s));
         emit(V_AT + s, rest + ad, pr);
       }
     } else {
@@ -665,10 +845,10 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
 #pragma unroll
         for (int j2 = i2; j2 < 3; ++j2) {
           const int s = sym(i2, j2);
-          auto p = box(15 + s);
-          const StagePre pr = pre(15 + s, 0);
+          auto p = box(SecPlain::at(s));
+          const StagePre pr = pre(SecPlain::at(s), 0);
           const double ad = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
-          done(15 + s);
+          done(SecPlain::at(s));
           double AA, lie;
 #pragma unroll
           for (int k2 = 0; k2 < 3; ++k2) {
@@ -697,11 +877,11 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     }
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2) {
-      auto p = box(21 + i2);
-      const StagePre prG = pre(21 + i2, 0), prB = pre(21 + i2, 1);
+      auto p = box(SecPlain::b(i2));
+      const StagePre prG = pre(SecPlain::b(i2), 0), prB = pre(SecPlain::b(i2), 1);
       const double Bi = p.at(0, 0, 0);
       const double adB = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
-      done(21 + i2);
+      done(SecPlain::b(i2));
       double r = lapb[i2];
       if constexpr (PARK) tmem_unpark<6>(park, P_CU + 6 * i2, &Cu[i2][0]);
       double t2 = sdot(Cu[i2], Au);   // Gamma~^i_jk At^{jk}
@@ -717,22 +897,31 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
     }
 
     // ---- o = 24: A (inert slot, dissipation only) -----------------------------------------------------------------
-    {
-      auto p = box(24);
-      const StagePre pr = pre(24, 0);
-      const double f0 = p.at(0, 0, 0);
-      double rA;
-      if (ORDER == 4) rA = C.ko * ((axis_q(p, f0, 0) + axis_q(p, f0, 1)) + axis_q(p, f0, 2));
-      else rA = (axis_ko8(p, f0, 0, C) + axis_ko8(p, f0, 1, C)) + axis_ko8(p, f0, 2, C);
-      done(24);
-      emit(V_A, rA, pr);
-    }
+    section_A();
   }
   if constexpr (TMEM) {
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(*tmem_slot) : "memory");
   }
+}
+
+// plain section layout: fused tile ids 0..4 (and the 8th-order instance)
+template <int TX, int TY, int TZ, int MODE, int ORDER>
+__global__ void __launch_bounds__(TX* TY* TZ, 1)
+bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ CUtensorMap tmCen,
+                const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS, Layout L, Coef C, Stage st, int ntx, int nty, int ntz, int cy) {
+  bssn_tma_body<TX, TY, TZ, MODE, ORDER, false>(tm, tmCen, tmU, tmS, tmU, tmS, tmU, tmS, L, C, st, ntx, nty, ntz, cy);
+}
+// interleaved section layout (4th order, 256-point tiles)
+template <int TX, int TY, int TZ, int MODE>
+__global__ void __launch_bounds__(TX* TY* TZ, 1)
+bssn_tma_il_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ CUtensorMap tmCen,
+                   const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS,
+                   const __grid_constant__ CUtensorMap tmU4, const __grid_constant__ CUtensorMap tmS4,
+                   const __grid_constant__ CUtensorMap tmU3, const __grid_constant__ CUtensorMap tmS3, Layout L, Coef C,
+                   Stage st, int ntx, int nty, int ntz, int cy) {
+  bssn_tma_body<TX, TY, TZ, MODE, 4, true>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C, st, ntx, nty, ntz, cy);
 }
 
 #ifndef CHM_EMULATE
@@ -756,11 +945,11 @@ static EncodeTiledFn encode_fn() {
 // What one launch of bssn_tma_kernel<TX,TY,TZ,MODE,ORDER> issues, for the validator: every section's box and
 // operand loads with the mbarrier byte count the kernel announces for it (one "barrier" entry per section, one for
 // the point-value tiles).  xo: Layout::xo (decides the parity of the x coordinates).
-template <int TX, int TY, int TZ, int ORDER>
+template <int TX, int TY, int TZ, int ORDER, bool IL = false>
 static TmaPlan bssn_plan(int mode, int xo) {
-  using Cfg = TmaCfg<TX, TY, TZ, ORDER>;
+  using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL>;
   char name[64];
-  snprintf(name, sizeof name, "bssn_tma_kernel<%d,%d,%d,order %d>", TX, TY, TZ, ORDER);
+  snprintf(name, sizeof name, "bssn_tma%s_kernel<%d,%d,%d,order %d>", IL ? "_il" : "", TX, TY, TZ, ORDER);
   TmaPlan p;
   p.kernel = name;
   p.smem_bytes = Cfg::SMEM;
@@ -770,7 +959,27 @@ static TmaPlan bssn_plan(int mode, int xo) {
   p.n_barriers = 2 * (Cfg::NS + 1);
   const int nops = mode == MODE_RHS ? 0 : (mode == MODE_FIRST ? 1 : 2);
   const int par_box = (xo - Cfg::H) & 1, par_tile = (xo - 1) & 1;
-  for (int o = 0; o < 25; ++o) {
+  const auto tile_load = [&](const char* what, int off, int nv, int bar) {
+    p.loads.push_back({what, (size_t)off * 8, {(uint32_t)(TX + 2), (uint32_t)TY, (uint32_t)TZ, (uint32_t)nv}, bar, par_tile});
+  };
+  for (int o = 0; IL && o < SecIL::N; ++o) {   // interleaved layout: 25 box sections, 3 emit sections, 2 empty ones
+    const int slot = o % Cfg::NS;
+    if (o >= SecIL::emit0) {
+      const int e = o - SecIL::emit0;
+      p.expect.push_back(e < 3 ? (uint32_t)(4 * nops) * Cfg::TILE_BYTES : 0u);
+      if (e < 2 && nops >= 1) tile_load("operand tiles U x4", Cfg::eop_off(slot, 0), 4, o);
+      if (e < 2 && nops == 2) tile_load("operand tiles S x4", Cfg::eop_off(slot, 4), 4, o);
+      if (e == 2 && nops >= 1) { tile_load("operand tile U", Cfg::eop_off(slot, 0), 1, o); tile_load("operand tiles U x3", Cfg::eop_off(slot, 1), 3, o); }
+      if (e == 2 && nops == 2) { tile_load("operand tile S", Cfg::eop_off(slot, 4), 1, o); tile_load("operand tiles S x3", Cfg::eop_off(slot, 5), 3, o); }
+      continue;
+    }
+    const bool em = SecIL::emit(o) >= 0;
+    p.expect.push_back(Cfg::BOX_BYTES + (uint32_t)(em ? nops : 0) * Cfg::TILE_BYTES);
+    p.loads.push_back({"halo box", (size_t)Cfg::box_off(slot) * 8, {(uint32_t)Cfg::BX, (uint32_t)Cfg::BY, (uint32_t)Cfg::BZ, 1}, o, par_box});
+    if (em && nops >= 1) tile_load("RK operand tile", Cfg::op_off(slot, 0), 1, o);
+    if (em && nops == 2) tile_load("RK operand tile", Cfg::op_off(slot, 1), 1, o);
+  }
+  for (int o = 0; !IL && o < 25; ++o) {
     const int slot = o % Cfg::NS, v0 = emit_var(o, 0), v1 = emit_var(o, 1), nem = (v0 >= 0) + (v1 >= 0);
     p.expect.push_back(Cfg::BOX_BYTES + (uint32_t)(nops * nem) * Cfg::TILE_BYTES);
     p.loads.push_back({"halo box", (size_t)Cfg::box_off(slot) * 8, {(uint32_t)Cfg::BX, (uint32_t)Cfg::BY, (uint32_t)Cfg::BZ, 1}, o, par_box});
@@ -780,21 +989,22 @@ static TmaPlan bssn_plan(int mode, int xo) {
     }
   }
   p.expect.push_back((uint32_t)kCenVars * Cfg::TILE_BYTES);
-  for (int grp = 0; grp < 3; ++grp)
-    p.loads.push_back({"point-value tiles", (size_t)Cfg::cen_off(grp) * 8, {(uint32_t)(TX + 2), (uint32_t)TY, (uint32_t)TZ, 7}, 25, par_tile});
+  for (int grp = 0; grp < 3; ++grp) tile_load("point-value tiles", Cfg::cen_off(grp), 7, (int)p.expect.size() - 1);
   return p;
 }
 
-template <int TX, int TY, int TZ, int MODE, int ORDER>
+template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL = false>
 static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
-  using Cfg = TmaCfg<TX, TY, TZ, ORDER>;
-  auto kern = bssn_tma_kernel<TX, TY, TZ, MODE, ORDER>;
+  using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL>;
+  const void* kern;
+  if constexpr (IL) kern = (const void*)bssn_tma_il_kernel<TX, TY, TZ, MODE>;
+  else kern = (const void*)bssn_tma_kernel<TX, TY, TZ, MODE, ORDER>;
   if (a) return cudaFuncGetAttributes(a, kern);
   // nothing is launched unless the validator accepts what this instance will issue on this layout
-  if (!launch_allowed(bssn_plan<TX, TY, TZ, ORDER>(MODE, L.xo), L, st->in, L.xo - Cfg::H, Cfg::H)) return cudaErrorInvalidValue;
+  if (!launch_allowed(bssn_plan<TX, TY, TZ, ORDER, IL>(MODE, L.xo), L, st->in, L.xo - Cfg::H, Cfg::H)) return cudaErrorInvalidValue;
   EncodeTiledFn enc = encode_fn();
   if (!enc) return cudaErrorNotSupported;
-  CUtensorMap tm, tmCen, tmU, tmS;
+  CUtensorMap tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3;
   cuuint64_t dims[4] = {(cuuint64_t)L.pitch, (cuuint64_t)L.tot_y, (cuuint64_t)L.tot_z, (cuuint64_t)L.nvars};
   cuuint64_t strides[3] = {(cuuint64_t)L.pitch * 8, (cuuint64_t)L.plane * 8, (cuuint64_t)L.vstride * 8};
   cuuint32_t box[4] = {(cuuint32_t)Cfg::BX, (cuuint32_t)Cfg::BY, (cuuint32_t)Cfg::BZ, 1};
@@ -817,6 +1027,9 @@ static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, 
   if (tile_map(&tmCen, st->in, 7) != CUDA_SUCCESS || tile_map(&tmU, ubase, 1) != CUDA_SUCCESS ||
       tile_map(&tmS, sbase, 1) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
+  if (IL && (tile_map(&tmU4, ubase, 4) != CUDA_SUCCESS || tile_map(&tmS4, sbase, 4) != CUDA_SUCCESS ||
+             tile_map(&tmU3, ubase, 3) != CUDA_SUCCESS || tile_map(&tmS3, sbase, 3) != CUDA_SUCCESS))
+    return cudaErrorInvalidValue;
   // per launch: function attributes are per device, and the call is cheap
   cudaError_t ea = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
   if (ea != cudaSuccess) return ea;
@@ -830,18 +1043,22 @@ static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, 
   if (blocks_per_sm < 1) blocks_per_sm = 1;
   const int grid = ntiles < sms * blocks_per_sm ? ntiles : sms * blocks_per_sm;
   const int cy = L.col_rows / TY > 0 ? L.col_rows / TY : 1;   // tile rows per traversal column
-  kern<<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, L, C, *st, ntx, nty, ntz, cy);
+  if constexpr (IL)
+    bssn_tma_il_kernel<TX, TY, TZ, MODE><<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C,
+                                                                                *st, ntx, nty, ntz, cy);
+  else
+    bssn_tma_kernel<TX, TY, TZ, MODE, ORDER><<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, L, C, *st, ntx, nty, ntz, cy);
   return cudaGetLastError();
 }
 
-template <int TX, int TY, int TZ, int ORDER = 4>
+template <int TX, int TY, int TZ, int ORDER = 4, bool IL = false>
 static cudaError_t tma_go(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
   switch (st ? st->mode : MODE_MID) {   // kernel_info reports the common (middle-stage) instance
-    case MODE_RHS: return tma_go_mode<TX, TY, TZ, MODE_RHS, ORDER>(L, C, st, s, a);
-    case MODE_FIRST: return tma_go_mode<TX, TY, TZ, MODE_FIRST, ORDER>(L, C, st, s, a);
-    case MODE_MID: return tma_go_mode<TX, TY, TZ, MODE_MID, ORDER>(L, C, st, s, a);
-    case MODE_LAST: return tma_go_mode<TX, TY, TZ, MODE_LAST, ORDER>(L, C, st, s, a);
-    case MODE_SSP: return tma_go_mode<TX, TY, TZ, MODE_SSP, ORDER>(L, C, st, s, a);
+    case MODE_RHS: return tma_go_mode<TX, TY, TZ, MODE_RHS, ORDER, IL>(L, C, st, s, a);
+    case MODE_FIRST: return tma_go_mode<TX, TY, TZ, MODE_FIRST, ORDER, IL>(L, C, st, s, a);
+    case MODE_MID: return tma_go_mode<TX, TY, TZ, MODE_MID, ORDER, IL>(L, C, st, s, a);
+    case MODE_LAST: return tma_go_mode<TX, TY, TZ, MODE_LAST, ORDER, IL>(L, C, st, s, a);
+    case MODE_SSP: return tma_go_mode<TX, TY, TZ, MODE_SSP, ORDER, IL>(L, C, st, s, a);
   }
   return cudaErrorInvalidValue;
 }
@@ -855,6 +1072,7 @@ static cudaError_t tma_dispatch(int order, int tile, const Layout& L, const Coef
     case 2: return tma_go<8, 4, 8>(L, C, st, s, a);
     case 3: return tma_go<16, 2, 8>(L, C, st, s, a);
     case 4: return tma_go<16, 4, 2>(L, C, st, s, a);
+    case 5: return tma_go<16, 4, 4, 4, true>(L, C, st, s, a);   // interleaved section layout
   }
   return cudaErrorInvalidValue;
 }
@@ -871,6 +1089,7 @@ void plans_bssn_fused(std::vector<TmaPlan>& out) {
       out.push_back(bssn_plan<8, 4, 8, 4>(mode, xo));
       out.push_back(bssn_plan<16, 2, 8, 4>(mode, xo));
       out.push_back(bssn_plan<16, 4, 2, 4>(mode, xo));
+      out.push_back(bssn_plan<16, 4, 4, 4, true>(mode, xo));
       if (g >= 5) out.push_back(bssn_plan<16, 4, 4, 8>(mode, xo));
     }
 }

@@ -46,7 +46,7 @@ static void from_padded(const Layout& L, const double* p, std::vector<double>& g
 
 template <int TX, int TY, int TZ, int MODE, int ORDER, int IL = 0>
 static chm_emu::Stats run(const Layout& L, const Coef& C, const Stage& st, int grid_req) {
-  using Cfg = TmaCfg<TX, TY, TZ, ORDER>;
+  using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL != 0>;
   auto map = [&](const double* base, uint32_t bx, uint32_t by, uint32_t bz, uint32_t bv) {
     CUtensorMap m;
     m.base = base;
@@ -63,19 +63,27 @@ static chm_emu::Stats run(const Layout& L, const Coef& C, const Stage& st, int g
   const int ntx = (L.nx + TX - 1) / TX, nty = (L.ny + TY - 1) / TY, ntz = (L.nz + TZ - 1) / TZ;
   const int ntiles = ntx * nty * ntz, grid = ntiles < grid_req ? ntiles : grid_req;
   const int cy = L.col_rows / TY > 0 ? L.col_rows / TY : 1;
-  return chm_emu::run_grid(grid, Cfg::THREADS, 1, Cfg::SMEM, [&] {
-    bssn_tma_kernel<TX, TY, TZ, MODE, ORDER>(tm, tmCen, tmU, tmS, L, C, st, ntx, nty, ntz, cy);
-  });
+  if constexpr (IL != 0) {   // the interleaved layout's operand maps: 4 and 3 consecutive variables a box
+    const CUtensorMap tmU4 = map(ubase, TX + 2, TY, TZ, 4), tmS4 = map(sbase, TX + 2, TY, TZ, 4),
+                      tmU3 = map(ubase, TX + 2, TY, TZ, 3), tmS3 = map(sbase, TX + 2, TY, TZ, 3);
+    return chm_emu::run_grid(grid, Cfg::THREADS, 1, Cfg::SMEM, [&] {
+      bssn_tma_il_kernel<TX, TY, TZ, MODE>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C, st, ntx, nty, ntz, cy);
+    });
+  } else {
+    return chm_emu::run_grid(grid, Cfg::THREADS, 1, Cfg::SMEM, [&] {
+      bssn_tma_kernel<TX, TY, TZ, MODE, ORDER>(tm, tmCen, tmU, tmS, L, C, st, ntx, nty, ntz, cy);
+    });
+  }
 }
 
-template <int TX, int TY, int TZ, int ORDER>
+template <int TX, int TY, int TZ, int ORDER, int IL = 0>
 static chm_emu::Stats run_mode(int mode, const Layout& L, const Coef& C, const Stage& st, int grid) {
   switch (mode) {
-    case MODE_RHS: return run<TX, TY, TZ, MODE_RHS, ORDER>(L, C, st, grid);
-    case MODE_FIRST: return run<TX, TY, TZ, MODE_FIRST, ORDER>(L, C, st, grid);
-    case MODE_MID: return run<TX, TY, TZ, MODE_MID, ORDER>(L, C, st, grid);
-    case MODE_LAST: return run<TX, TY, TZ, MODE_LAST, ORDER>(L, C, st, grid);
-    case MODE_SSP: return run<TX, TY, TZ, MODE_SSP, ORDER>(L, C, st, grid);
+    case MODE_RHS: return run<TX, TY, TZ, MODE_RHS, ORDER, IL>(L, C, st, grid);
+    case MODE_FIRST: return run<TX, TY, TZ, MODE_FIRST, ORDER, IL>(L, C, st, grid);
+    case MODE_MID: return run<TX, TY, TZ, MODE_MID, ORDER, IL>(L, C, st, grid);
+    case MODE_LAST: return run<TX, TY, TZ, MODE_LAST, ORDER, IL>(L, C, st, grid);
+    case MODE_SSP: return run<TX, TY, TZ, MODE_SSP, ORDER, IL>(L, C, st, grid);
   }
   abort();
 }
@@ -111,6 +119,7 @@ int main(int argc, char** argv) {
   else if (order == 4 && tile == 0) s = run_mode<16, 4, 4, 4>(mode, L, C, st, grid);
   else if (order == 4 && tile == 1) s = run_mode<16, 8, 2, 4>(mode, L, C, st, grid);
   else if (order == 4 && tile == 3) s = run_mode<16, 2, 8, 4>(mode, L, C, st, grid);
+  else if (order == 4 && tile == 5) s = run_mode<16, 4, 4, 4, 1>(mode, L, C, st, grid);
   else { fprintf(stderr, "instance not built into the emulator\n"); return 5; }
   std::vector<double> o(ng), so(ng), uo(ng);
   from_padded(L, out.data(), o); from_padded(L, S.data(), so); from_padded(L, (mode == MODE_FIRST ? in : U).data(), uo);

@@ -55,7 +55,8 @@ def strong(nx, ny, nz, seed=21, amp=0.1):
 
 
 @pytest.mark.parametrize("order,g,tile,dims,grid", [(4, 3, 0, (20, 9, 6), 3), (4, 3, 1, (20, 9, 6), 2), (4, 3, 3, (17, 5, 11), 1),
-                                                    (4, 4, 0, (18, 6, 5), 2), (8, 5, 0, (19, 6, 7), 2)])
+                                                    (4, 4, 0, (18, 6, 5), 2), (8, 5, 0, (19, 6, 7), 2),
+                                                    (4, 3, 5, (20, 9, 6), 3), (4, 4, 5, (18, 6, 9), 1)])
 @pytest.mark.parametrize("data", ["strong", "noise1e-10"])
 def test_rhs_against_the_oracle(oracle, emu, tmp_path, order, g, tile, dims, grid, data):
     nx, ny, nz = dims
@@ -69,9 +70,24 @@ def test_rhs_against_the_oracle(oracle, emu, tmp_path, order, g, tile, dims, gri
     m = np.ones(out.shape[1:], dtype=bool)
     m[g:-g, g:-g, g:-g] = False
     assert not out[:, m].any()                                  # nothing is written outside the interior
-    tx, ty, tz = {0: (16, 4, 4), 1: (16, 8, 2), 3: (16, 2, 8)}[tile]
+    tx, ty, tz = {0: (16, 4, 4), 1: (16, 8, 2), 3: (16, 2, 8), 5: (16, 4, 4)}[tile]
     ntiles = -(-nx // tx) * -(-ny // ty) * -(-nz // tz)
     assert stats["loads"] == ntiles * (25 + 3)                  # one box per section + three point-value groups
+
+
+def test_interleaved_layout_is_bit_identical_to_the_plain_one(oracle, emu, tmp_path):
+    """tile id 5 evaluates the arithmetic of tile id 0 in another section order: a middle RK4 stage gives the same bits
+    (Y and S), and loads the same boxes plus the same operand tiles in fewer, larger requests"""
+    nx, ny, nz, g, h, eps = 20, 9, 6, 3, 0.05, 0.1
+    st = oracle.fill_ghosts(oracle.with_ghosts(strong(nx, ny, nz), g), g)
+    U = oracle.fill_ghosts(oracle.with_ghosts(strong(nx, ny, nz, seed=7), g), g)
+    S = oracle.fill_ghosts(oracle.with_ghosts(strong(nx, ny, nz, seed=8), g), g)
+    a0 = launch(emu, tmp_path, 4, 0, MODE_MID, st, U, S, g, h, eps, a=0.00625)
+    a5 = launch(emu, tmp_path, 4, 5, MODE_MID, st, U, S, g, h, eps, a=0.00625)
+    assert np.array_equal(a0[0], a5[0]) and np.array_equal(a0[1], a5[1]) and np.array_equal(a0[2], a5[2])
+    assert a0[3]["bytes"] == a5[3]["bytes"]
+    ntiles = 2 * 3 * 2
+    assert a0[3]["loads"] == ntiles * (25 + 50 + 3) and a5[3]["loads"] == ntiles * (25 + 2 * 13 + 2 * 2 + 4 + 3)
 
 
 def test_flat_space_gives_exactly_zero(oracle, emu, tmp_path):
@@ -81,7 +97,7 @@ def test_flat_space_gives_exactly_zero(oracle, emu, tmp_path):
     assert not out.any()
 
 
-@pytest.mark.parametrize("tile", [0, 3])
+@pytest.mark.parametrize("tile", [0, 3, 5])
 def test_one_rk4_step_through_the_four_epilogues(oracle, emu, tmp_path, tile):
     """FIRST, MID, MID, LAST chained as chemora_rk4_step chains them (the periodic fill between the stages done by the
     oracle's fill): equals the oracle's RK4 step in both norms of DESIGN.md S11 / S11b"""
@@ -103,12 +119,13 @@ def test_one_rk4_step_through_the_four_epilogues(oracle, emu, tmp_path, tile):
         assert np.max(np.abs((got[v] - 1.0) - (want[v] - 1.0))) < max(1e-11, 8 * 2.3e-16 / amp) * amp
 
 
-def test_ssp_epilogue(oracle, emu, tmp_path):
+@pytest.mark.parametrize("tile", [0, 5])
+def test_ssp_epilogue(oracle, emu, tmp_path, tile):
     """MODE_SSP: out = ca U + cb (in + dt k), the Shu-Osher stage"""
     nx, ny, nz, g, h, eps = 16, 8, 4, 3, 0.05, 0.1
     st = oracle.fill_ghosts(oracle.with_ghosts(strong(nx, ny, nz, seed=5, amp=0.02), g), g)
     U = oracle.fill_ghosts(oracle.with_ghosts(strong(nx, ny, nz, seed=6, amp=0.02), g), g)
-    out, _, _, _ = launch(emu, tmp_path, 4, 0, MODE_SSP, st, U, np.zeros_like(U), g, h, eps, a=0.01, ca=0.75, cb=0.25)
+    out, _, _, _ = launch(emu, tmp_path, 4, tile, MODE_SSP, st, U, np.zeros_like(U), g, h, eps, a=0.01, ca=0.75, cb=0.25)
     k = oracle.rhs(oracle.SYS_BSSN, st, g, 4, h, oracle.params(eps_diss=eps))
     want = 0.75 * U + 0.25 * (st + 0.01 * k)
     assert relerr(oracle.interior(out, g), oracle.interior(want, g)) < 1e-13

@@ -311,7 +311,7 @@ def test_autotune_and_kernel_info(chem):
     fused, tile, ms = h.autotune()
     nt = chem.NUM_TILES
     assert fused == 1 and tile in chem.variants(chem.SYS_BSSN, 4)
-    assert all((ms[nt + t] > 0) == (t < 5) for t in range(nt))          # the five fused ids, nothing else
+    assert all((ms[nt + t] > 0) == (t < 6) for t in range(nt))          # the six fused ids, nothing else
     assert all(m < 0 for m in ms[:nt])                                  # split variant: only on request
     h.set_param("autotune_split", 1)
     fused2, tile2, ms2 = h.autotune()
@@ -363,7 +363,7 @@ def test_enforce_constraints(chem, oracle):
     w.destroy()
 
 
-@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5])
 def test_bssn_rk3_with_enforcement_10_steps(chem, oracle, tile):
     """the paper's integrator (RK3) with constraint enforcement after every step, configs[2] data at 24x20x18"""
     nx, ny, nz = 24, 20, 18
