@@ -53,6 +53,7 @@ __global__ void __launch_bounds__(256) fill_ghosts_kernel(Layout L, double* __re
   }
 }
 
+#ifndef CHM_EMULATE
 cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s, const FillLink* link) {
   const int g = L.g;
   if (g == 0) return cudaSuccess;
@@ -66,6 +67,7 @@ cudaError_t launch_fill_ghosts(const Layout& L, double* state, cudaStream_t s, c
   fill_ghosts_kernel<<<grid, 256, 0, s>>>(L, state, (int)rowsA, (int)rowsAB, lpr_shift, link ? *link : self);
   return cudaGetLastError();
 }
+#endif   // CHM_EMULATE
 
 // packed [V][nz][ny][nx] <-> padded interior
 __global__ void __launch_bounds__(256) pack_kernel(Layout L, const double* __restrict__ src, double* __restrict__ dst,
@@ -78,12 +80,14 @@ __global__ void __launch_bounds__(256) pack_kernel(Layout L, const double* __res
   if (to_state) dst[q] = src[r]; else dst[r] = src[q];
 }
 
+#ifndef CHM_EMULATE
 cudaError_t launch_pack(const Layout& L, const double* packed, double* state, bool to_state, cudaStream_t s) {
   dim3 grid((L.nx + 255) / 256, L.ny, L.nz * L.nvars);
   if (to_state) pack_kernel<<<grid, 256, 0, s>>>(L, packed, state, true);
   else pack_kernel<<<grid, 256, 0, s>>>(L, state, const_cast<double*>(packed), false);
   return cudaGetLastError();
 }
+#endif   // CHM_EMULATE
 
 // ---------------------------------------------------------------------------------------------------
 // Algebraic constraint enforcement of a BSSN state (reading S10b): gt_ij <- gt_ij + gt_ij (det(gt)^(-1/3) - 1),
@@ -120,11 +124,13 @@ __global__ void __launch_bounds__(256) enforce_kernel(Layout L, double* __restri
   }
 }
 
+#ifndef CHM_EMULATE
 cudaError_t launch_enforce(const Layout& L, double* state, cudaStream_t s) {
   dim3 grid((L.nx + 255) / 256, L.ny, L.nz);
   enforce_kernel<<<grid, 256, 0, s>>>(L, state);
   return cudaGetLastError();
 }
+#endif   // CHM_EMULATE
 
 // ---------------------------------------------------------------------------------------------------
 // Wave system (reading S1): d_t phi = pi (+KO), d_t pi = (d_xx + d_yy + d_zz) phi (+KO).
@@ -151,6 +157,7 @@ __global__ void __launch_bounds__(TX* TY) wave_kernel(Layout L, Coef C, Stage st
   }
 }
 
+#ifndef CHM_EMULATE
 template <int ORDER, bool KO, int TX, int TY, int TZ>
 static cudaError_t wave_go(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
   auto kern = wave_kernel<ORDER, KO, TX, TY, TZ>;
@@ -159,7 +166,9 @@ static cudaError_t wave_go(const Layout& L, const Coef& C, const Stage* st, cuda
   kern<<<grid, dim3(TX, TY), 0, s>>>(L, C, *st);
   return cudaGetLastError();
 }
+#endif   // CHM_EMULATE
 
+#ifndef CHM_EMULATE
 template <int ORDER, bool KO>
 static cudaError_t wave_tile(int tile, const Layout& L, const Coef& C, const Stage* st, cudaStream_t s,
                              cudaFuncAttributes* a) {
@@ -173,22 +182,29 @@ static cudaError_t wave_tile(int tile, const Layout& L, const Coef& C, const Sta
   }
   return cudaErrorInvalidValue;
 }
+#endif   // CHM_EMULATE
 
+#ifndef CHM_EMULATE
 static cudaError_t wave_dispatch(int order, bool ko, int tile, const Layout& L, const Coef& C, const Stage* st,
                                  cudaStream_t s, cudaFuncAttributes* a) {
   if (order == 4) return ko ? wave_tile<4, true>(tile, L, C, st, s, a) : wave_tile<4, false>(tile, L, C, st, s, a);
   if (order == 8) return ko ? wave_tile<8, true>(tile, L, C, st, s, a) : wave_tile<8, false>(tile, L, C, st, s, a);
   return cudaErrorInvalidValue;
 }
+#endif   // CHM_EMULATE
 
+#ifndef CHM_EMULATE
 cudaError_t launch_wave(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s) {
   return wave_dispatch(order, C.ko != 0.0, tile, L, C, &st, s, nullptr);
 }
+#endif   // CHM_EMULATE
 
+#ifndef CHM_EMULATE
 cudaError_t kernel_info_wave(int order, int tile, cudaFuncAttributes* a) {
   Layout L{}; Coef C{};
   return wave_dispatch(order, true, tile, L, C, nullptr, 0, a);
 }
+#endif   // CHM_EMULATE
 
 // ---------------------------------------------------------------------------------------------------
 // First-order wave system of the paper's Sample 1, V = 5: (u, rho, v_1, v_2, v_3):
@@ -221,6 +237,7 @@ __global__ void __launch_bounds__(TX* TY) wave1_kernel(Layout L, Coef C, Stage s
   }
 }
 
+#ifndef CHM_EMULATE
 template <int ORDER, bool KO, int TX, int TY, int TZ>
 static cudaError_t wave1_go(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
   auto kern = wave1_kernel<ORDER, KO, TX, TY, TZ>;
@@ -229,7 +246,9 @@ static cudaError_t wave1_go(const Layout& L, const Coef& C, const Stage* st, cud
   kern<<<grid, dim3(TX, TY), 0, s>>>(L, C, *st);
   return cudaGetLastError();
 }
+#endif   // CHM_EMULATE
 
+#ifndef CHM_EMULATE
 template <int ORDER, bool KO>
 static cudaError_t wave1_tile(int tile, const Layout& L, const Coef& C, const Stage* st, cudaStream_t s,
                               cudaFuncAttributes* a) {
@@ -243,22 +262,29 @@ static cudaError_t wave1_tile(int tile, const Layout& L, const Coef& C, const St
   }
   return cudaErrorInvalidValue;
 }
+#endif   // CHM_EMULATE
 
+#ifndef CHM_EMULATE
 static cudaError_t wave1_dispatch(int order, bool ko, int tile, const Layout& L, const Coef& C, const Stage* st,
                                   cudaStream_t s, cudaFuncAttributes* a) {
   if (order == 4) return ko ? wave1_tile<4, true>(tile, L, C, st, s, a) : wave1_tile<4, false>(tile, L, C, st, s, a);
   if (order == 8) return ko ? wave1_tile<8, true>(tile, L, C, st, s, a) : wave1_tile<8, false>(tile, L, C, st, s, a);
   return cudaErrorInvalidValue;
 }
+#endif   // CHM_EMULATE
 
+#ifndef CHM_EMULATE
 cudaError_t launch_wave1(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s) {
   return wave1_dispatch(order, C.ko != 0.0, tile, L, C, &st, s, nullptr);
 }
+#endif   // CHM_EMULATE
 
+#ifndef CHM_EMULATE
 cudaError_t kernel_info_wave1(int order, int tile, cudaFuncAttributes* a) {
   Layout L{}; Coef C{};
   return wave1_dispatch(order, true, tile, L, C, nullptr, 0, a);
 }
+#endif   // CHM_EMULATE
 
 // ---------------------------------------------------------------------------------------------------
 // "Energy" calculation of the paper's Sample 1: eps = 1/2 (rho^2 + v_i v_i) at every interior
@@ -289,11 +315,13 @@ __global__ void __launch_bounds__(256) energy_kernel(Layout L, const double* __r
   }
 }
 
+#ifndef CHM_EMULATE
 cudaError_t launch_energy(const Layout& L, const double* state, double* eps_out, double* sum, cudaStream_t s) {
   dim3 grid((L.nx + 255) / 256, L.ny, L.nz);
   energy_kernel<<<grid, 256, 0, s>>>(L, state, eps_out, sum);
   return cudaGetLastError();
 }
+#endif   // CHM_EMULATE
 
 // ---------------------------------------------------------------------------------------------------
 // FP64 peak probe: 8 independent register-resident DFMA chains per thread.
@@ -312,9 +340,11 @@ __global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, double* sink)
   if (r == 12345.678) sink[0] = r;   // never true; keeps the chains alive
 }
 
+#ifndef CHM_EMULATE
 cudaError_t launch_dfma_peak(int blocks, int threads, int iters, double* sink, cudaStream_t s) {
   dfma_peak_kernel<<<blocks, threads, 0, s>>>(iters, sink);
   return cudaGetLastError();
 }
+#endif   // CHM_EMULATE
 
 }  // namespace chm

@@ -87,6 +87,7 @@ __global__ void __launch_bounds__(TX* TY) bssn_from_derivs_kernel(Layout L, Coef
 }
 
 // which: 1 derivs, 2 from_derivs
+#ifndef CHM_EMULATE
 template <int TX, int TY, int TZ>
 static cudaError_t bssn_go(int which, const Layout& L, const Coef& C, const Stage* st, const double* in,
                            double* derivs, cudaStream_t s, cudaFuncAttributes* a) {
@@ -106,7 +107,9 @@ static cudaError_t bssn_go(int which, const Layout& L, const Coef& C, const Stag
   }
   return cudaGetLastError();
 }
+#endif   // CHM_EMULATE
 
+#ifndef CHM_EMULATE
 static cudaError_t bssn_dispatch(int which, int tile, const Layout& L, const Coef& C, const Stage* st,
                                  const double* in, double* derivs, cudaStream_t s, cudaFuncAttributes* a) {
   switch (tile) {
@@ -119,18 +122,25 @@ static cudaError_t bssn_dispatch(int which, int tile, const Layout& L, const Coe
   }
   return cudaErrorInvalidValue;
 }
+#endif   // CHM_EMULATE
 
+#ifndef CHM_EMULATE
 cudaError_t launch_bssn_derivs(const Layout& L, const Coef& C, int order, int tile, const double* in, double* derivs,
                                cudaStream_t s) {
   return bssn_dispatch(order == 8 ? 3 : 1, tile, L, C, nullptr, in, derivs, s, nullptr);
 }
+#endif   // CHM_EMULATE
+#ifndef CHM_EMULATE
 cudaError_t launch_bssn_from_derivs(const Layout& L, const Coef& C, int tile, const double* derivs, const Stage& st,
                                     cudaStream_t s) {
   return bssn_dispatch(2, tile, L, C, &st, nullptr, const_cast<double*>(derivs), s, nullptr);
 }
+#endif   // CHM_EMULATE
+#ifndef CHM_EMULATE
 cudaError_t kernel_info_bssn_split(int which, int tile, cudaFuncAttributes* a) {
   Layout L{}; Coef C{};
   return bssn_dispatch(which, tile, L, C, nullptr, nullptr, nullptr, 0, a);
 }
+#endif   // CHM_EMULATE
 
 }  // namespace chm

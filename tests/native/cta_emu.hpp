@@ -31,6 +31,7 @@
 #include <map>
 #include <memory>
 #include <mutex>
+#include <string>
 #include <thread>
 #include <vector>
 
@@ -41,6 +42,7 @@
 #define __launch_bounds__(...)
 #define __grid_constant__
 #define __align__(n) alignas(n)
+#define __shared__ static   // static shared arrays: one CTA runs at a time, so one instance per kernel is per-CTA storage
 
 using std::max;
 using std::min;
@@ -184,6 +186,14 @@ inline void tma_load_4d(void* dst, const CUtensorMap* tm, void* bar, int x, int 
 inline void sync_all() { t_cta->all.wait(t_cta->nthreads); }
 inline void sync_warp() { t_cta->warp[(t_threadIdx.y * t_blockDim.x + t_threadIdx.x) / 32]->wait(32); }
 inline void sync_named(int id, int count) { t_cta->named[id]->wait(count); }
+inline double shfl_down(double v, int delta) {   // all 32 threads of the warp call it together
+  const int t = t_threadIdx.y * t_blockDim.x + t_threadIdx.x;
+  t_cta->shfl[t] = v;
+  sync_warp();
+  const double r = (t & 31) + delta < 32 ? t_cta->shfl[t + delta] : v;
+  sync_warp();
+  return r;
+}
 inline double shfl_xor(double v, int lane_mask) {   // all 32 threads of the warp call it together
   const int t = t_threadIdx.y * t_blockDim.x + t_threadIdx.x;
   t_cta->shfl[t] = v;
@@ -195,8 +205,10 @@ inline double shfl_xor(double v, int lane_mask) {   // all 32 threads of the war
 
 // run `grid` CTAs of `threads` (x * y) threads one after the other; body() is the kernel call
 struct Stats { long tma_loads = 0, tma_bytes = 0; };
-inline Stats run_grid(int grid, int bx, int by, size_t smem_bytes, const std::function<void()>& body, int grid_y = 1) {
+inline Stats run_grid(int grid, int bx, int by, size_t smem_bytes, const std::function<void()>& body, int grid_y = 1,
+                      int grid_z = 1) {
   Stats st;
+  for (int bz_ = 0; bz_ < grid_z; ++bz_)
   for (int by_ = 0; by_ < grid_y; ++by_)
   for (int b = 0; b < grid; ++b) {
     Cta cta;
@@ -212,8 +224,8 @@ inline Stats run_grid(int grid, int bx, int by, size_t smem_bytes, const std::fu
       th.emplace_back([&, t] {
         t_cta = &cta;
         t_threadIdx = Idx3{(unsigned)(t % bx), (unsigned)(t / bx), 0};
-        t_blockIdx = Idx3{(unsigned)b, (unsigned)by_, 0};
-        t_gridDim = Idx3{(unsigned)grid, (unsigned)grid_y, 1};
+        t_blockIdx = Idx3{(unsigned)b, (unsigned)by_, (unsigned)bz_};
+        t_gridDim = Idx3{(unsigned)grid, (unsigned)grid_y, (unsigned)grid_z};
         t_blockDim = Idx3{(unsigned)bx, (unsigned)by, 1};
         body();
       });
@@ -222,6 +234,22 @@ inline Stats run_grid(int grid, int bx, int by, size_t smem_bytes, const std::fu
     free(cta.smem);
   }
   return st;
+}
+
+// kernels without any inter-thread synchronisation (no barrier, no shuffle): every thread of every block in turn, on
+// the calling OS thread
+inline void run_grid_serial(int gx, int gy, int gz, int bx, int by, const std::function<void()>& body) {
+  for (int z = 0; z < gz; ++z)
+    for (int y = 0; y < gy; ++y)
+      for (int x = 0; x < gx; ++x)
+        for (int t = 0; t < bx * by; ++t) {
+          t_cta = nullptr;
+          t_threadIdx = Idx3{(unsigned)(t % bx), (unsigned)(t / bx), 0};
+          t_blockIdx = Idx3{(unsigned)x, (unsigned)y, (unsigned)z};
+          t_gridDim = Idx3{(unsigned)gx, (unsigned)gy, (unsigned)gz};
+          t_blockDim = Idx3{(unsigned)bx, (unsigned)by, 1};
+          body();
+        }
 }
 
 }  // namespace chm_emu
@@ -239,6 +267,14 @@ inline double __dmul_rn(double a, double b) { return a * b; }
 template <class T> inline void __stcs(T* p, T v) { *p = v; }
 template <class T> inline T __ldg(const T* p) { return *p; }
 inline double __shfl_xor_sync(unsigned, double v, int lane_mask) { return chm_emu::shfl_xor(v, lane_mask); }
+inline double __shfl_down_sync(unsigned, double v, int delta) { return chm_emu::shfl_down(v, delta); }
+inline double atomicAdd(double* p, double v) {   // CTAs run one at a time and one thread per CTA adds: plain
+  static std::mutex m;
+  std::lock_guard<std::mutex> lk(m);
+  const double old = *p;
+  *p = old + v;
+  return old;
+}
 inline double __longlong_as_double(long long x) { double d; memcpy(&d, &x, 8); return d; }
 inline long long __double_as_longlong(double d) { long long x; memcpy(&x, &d, 8); return x; }
 inline unsigned long long atomicMax(unsigned long long* p, unsigned long long v) {
