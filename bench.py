@@ -249,11 +249,11 @@ def run_ours(args):
                    "variant": {"fused": fused, "tile": list(binding.tile_shape(tile, binding.SYS_BSSN, fused)), "sweep_ms": sweep_ms},
                    "kernel": info, "multi_gpu": "replicas only",
                    "l2": "inputs larger than L2 (%.2f GB per state buffer vs 126 MB)" % (h.nvars * h.var_stride * 8 / 1e9)},
-        "roofline": {"bound": "hbm", "kernel": "bssn_tma_kernel" if fused else "bssn_derivs+from_derivs",
+        "roofline": {"bound": "hbm", "kernel": ("bssn_tma_il_kernel" if tile == 5 else "bssn_tma_kernel") if fused else "bssn_derivs+from_derivs",
                      "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
                      "traffic": None,
                      "traffic_constant": {"bytes_per_launch": NCU_TRAFFIC_BYTES_256, "source": NCU_TRAFFIC_SOURCE}
-                                         if (fused and n == 256) else None,
+                                         if (fused and tile < 5 and n == 256) else None,
                      "algorithmic_bytes_per_launch": BYTES_PER_POINT_PER_LAUNCH * n ** 3, "peak_source": pk_src, "ms_per_launch": rhs_launch_ms,
                      # the whole step (4 fills + 4 launches, the driver-timed number) against the same roof
                      "step_frac": BYTES_PER_UPDATE * n ** 3 / (ms / args.steps * 1e-3) / 1e9 / hbm_peak,

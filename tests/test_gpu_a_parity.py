@@ -11,6 +11,7 @@ pytestmark = pytest.mark.gpu
 TOL_WAVE_PER_STEP = 1e-12
 TOL_BSSN_10_STEPS = 1e-10
 TOL_RHS = 1e-12          # a single RHS evaluation: rounding-order differences only (difference-form stencils)
+ROUND1_FUSED_IDS = 5     # fused BSSN ids 0..4 ran green on hardware in round 1; later ids are tested in test_gpu_zz_round2.py
 
 
 @pytest.fixture(scope="module")
@@ -235,7 +236,7 @@ def test_bssn_rhs_all_variants_and_tiles(chem, oracle, data):
     h = chem.Chemora(nx, ny, nz, 3, 4, 1, dx)
     h.set_param("eps_diss", eps)
     for fused in (1, 0):
-        for tile in chem.variants(chem.SYS_BSSN, 4, fused):
+        for tile in [t for t in chem.variants(chem.SYS_BSSN, 4, fused) if t < ROUND1_FUSED_IDS or not fused]:
             h.set_variant(fused, tile)
             got = gpu_rhs(h, u)
             assert relerr(got, want) < TOL_RHS, (fused, tile)
@@ -311,7 +312,9 @@ def test_autotune_and_kernel_info(chem):
     fused, tile, ms = h.autotune()
     nt = chem.NUM_TILES
     assert fused == 1 and tile in chem.variants(chem.SYS_BSSN, 4)
-    assert all((ms[nt + t] > 0) == (t < 6) for t in range(nt))          # the six fused ids, nothing else
+    assert all(ms[nt + t] > 0 for t in range(ROUND1_FUSED_IDS))         # the five plain fused ids are timed
+    assert all(ms[nt + t] != -1.0 for t in chem.variants(chem.SYS_BSSN, 4))   # later ids: timed, or disqualified (-2, -3)
+    assert all(ms[nt + t] == -1.0 for t in range(nt) if t not in chem.variants(chem.SYS_BSSN, 4))
     assert all(m < 0 for m in ms[:nt])                                  # split variant: only on request
     h.set_param("autotune_split", 1)
     fused2, tile2, ms2 = h.autotune()
@@ -363,7 +366,7 @@ def test_enforce_constraints(chem, oracle):
     w.destroy()
 
 
-@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5])
+@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4])
 def test_bssn_rk3_with_enforcement_10_steps(chem, oracle, tile):
     """the paper's integrator (RK3) with constraint enforcement after every step, configs[2] data at 24x20x18"""
     nx, ny, nz = 24, 20, 18
