@@ -53,5 +53,45 @@ def build(force=False, verbose=False):
     return LIB
 
 
+def report():
+    """Static per-kernel report of the built library (the paper's run-time prints one per kernel at the end of a run,
+    PAPER.md:272-276; this is its compile-time part): registers and spill bytes from ptxas, SASS instruction counts from
+    cuobjdump.  Markdown table on stdout.  Needs a build made by this process or an earlier one (build/ptxas.log)."""
+    import collections
+    import re
+    cuda_bin = os.path.dirname(os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc"))
+    sass = subprocess.run([os.path.join(cuda_bin, "cuobjdump"), "-sass", LIB], capture_output=True, text=True,
+                          check=True).stdout
+    log = open(os.path.join(HERE, "build", "ptxas.log")).read()
+    regs = {}
+    for m in re.finditer(r"Compiling entry function '(\S+)' for 'sm_100a'\nptxas info\s+: Function properties for \S+\n"
+                         r"\s+\d+ bytes stack frame, (\d+) bytes spill stores, \d+ bytes spill loads\n"
+                         r"ptxas info\s+: Used (\d+) registers", log):
+        regs[m.group(1)] = (int(m.group(3)), int(m.group(2)))
+    cur, cnt = None, collections.defaultdict(collections.Counter)
+    for line in sass.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            cur = m.group(1)
+            continue
+        m = re.match(r"\s+/\*[0-9a-f]{4,6}\*/\s+(@!?U?P[0-9T]+ )?([A-Z0-9_]+)", line)
+        if m and cur:
+            cnt[cur][m.group(2)] += 1
+    names = sorted(cnt)
+    dem = subprocess.run(["c++filt"] + names, capture_output=True, text=True).stdout.splitlines()
+    rows = []
+    for n, d in zip(names, dem):
+        c, r = cnt[n], regs.get(n, ("?", "?"))
+        d = re.sub(r"\(.*", "", d).replace("void chm::", "").replace("chm::", "")
+        rows.append((d, r[0], r[1], sum(c.values()), c["DADD"] + c["DMUL"] + c["DFMA"], c["LDS"], c["STS"],
+                     c["UTMALDG"], c["SYNCS"], c["LDG"], c["STG"]))
+    print("| kernel | regs | spill B | SASS instr | FP64 | LDS | STS | UTMALDG | SYNCS | LDG | STG |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|")
+    for r in sorted(rows):
+        print("| `%s` | %s |" % (r[0], " | ".join(str(x) for x in r[1:])))
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--report" in sys.argv:
+        report()
