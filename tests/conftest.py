@@ -17,3 +17,19 @@ def oracle():
     from oracle import oracle as o
     o.lib()
     return o
+
+
+_EMU = {}
+
+
+def build_emulator(name):
+    """g++ -DCHM_EMULATE build of tests/native/<name>.cpp (a kernel source on top of cta_emu.hpp), once per session"""
+    import subprocess
+    import tempfile
+    if name not in _EMU:
+        d = tempfile.mkdtemp(prefix="chm_emu_")
+        exe = os.path.join(d, name)
+        subprocess.run(["g++", "-std=c++17", "-O1", "-DCHM_EMULATE", "-pthread", "-o", exe,
+                        os.path.join(ROOT, "tests", "native", name + ".cpp")], check=True, capture_output=True)
+        _EMU[name] = exe
+    return _EMU[name]

@@ -16,11 +16,9 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 @pytest.fixture(scope="module")
-def emu(tmp_path_factory):
-    exe = str(tmp_path_factory.mktemp("emu") / "basic_emu")
-    subprocess.run(["g++", "-std=c++17", "-O1", "-DCHM_EMULATE", "-pthread", "-o", exe,
-                    os.path.join(ROOT, "tests", "native", "basic_emu.cpp")], check=True, capture_output=True)
-    return exe
+def emu():
+    from tests.conftest import build_emulator
+    return build_emulator("basic_emu")
 
 
 def run(exe, tmp, op, system, order, st, g, h=0.05, eps=0.0, tile=0, mode=0, a=0.0, ko_order=5, raw=False):

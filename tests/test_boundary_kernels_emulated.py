@@ -14,11 +14,9 @@ MODE_RHS, MODE_FIRST, MODE_MID, MODE_LAST, MODE_SSP = range(5)
 
 
 @pytest.fixture(scope="module")
-def emu(tmp_path_factory):
-    exe = str(tmp_path_factory.mktemp("emu") / "boundary_emu")
-    subprocess.run(["g++", "-std=c++17", "-O1", "-DCHM_EMULATE", "-pthread", "-o", exe,
-                    os.path.join(ROOT, "tests", "native", "boundary_emu.cpp")], check=True, capture_output=True)
-    return exe
+def emu():
+    from tests.conftest import build_emulator
+    return build_emulator("boundary_emu")
 
 
 def rad(exe, tmp, system, st_in, U, S, g, h, mode, a=0.0, ca=0.0, cb=0.0):

@@ -13,11 +13,9 @@ MODE_RHS, MODE_FIRST, MODE_MID, MODE_LAST, MODE_SSP = range(5)
 
 
 @pytest.fixture(scope="module")
-def emu(tmp_path_factory):
-    exe = str(tmp_path_factory.mktemp("emu") / "wave_emu")
-    subprocess.run(["g++", "-std=c++17", "-O1", "-DCHM_EMULATE", "-pthread", "-o", exe,
-                    os.path.join(ROOT, "tests", "native", "wave_emu.cpp")], check=True, capture_output=True)
-    return exe
+def emu():
+    from tests.conftest import build_emulator
+    return build_emulator("wave_emu")
 
 
 def launch(exe, tmp, V, order, ko, which, mode, st_in, U, S, g, h, eps, a=0.0, ca=0.0, cb=0.0, grid=2):
