@@ -112,7 +112,10 @@ struct TmaCfg {
   __host__ __device__ static constexpr int bar_off() { return NS * SLOTX + CEN + 2 * DB + TAB; }                      // full[NS], cfull, empty[NS + 1]
 };
 // the kernel body; tmU4 / tmS4 / tmU3 / tmS3: operand maps with 4 and 3 consecutive variables per box (IL emit sections)
-template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL>
+// EARLY: a full variable's own right-hand side (which needs none of its mixed derivatives) leaves BEFORE the plane
+// barrier of the two-pass mixed derivatives instead of after it, so the time a warp would spend waiting for its
+// plane partner is spent on the operand reads, the stage update and the stores (capture L: 4 % of stall samples)
+template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL, bool EARLY = false>
 __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUtensorMap& tmCen, const CUtensorMap& tmU,
                                               const CUtensorMap& tmS, const CUtensorMap& tmU4, const CUtensorMap& tmS4,
                                               const CUtensorMap& tmU3, const CUtensorMap& tmS3, const Layout& L,
@@ -326,7 +329,8 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
     // Two-pass mixed derivatives: every thread publishes D_y f and D_z f of its own point (it has them already),
     // the block adds them on the 2-cell x-halo (and D_z f on the 2-cell y-halo), and after one block barrier
     // d_xy = D_x(D_y f), d_xz = D_x(D_z f), d_yz = D_y(D_z f) cost 4 reads each instead of 16.
-    auto full_var = [&](const BoxPoint<BX, BY>& p, const AdvW& w, int o, int n, double* d1, double* d2, double& ad) {
+    auto full_var = [&](const BoxPoint<BX, BY>& p, const AdvW& w, int o, int n, double* d1, double* d2, double& ad,
+                        auto&& early) {
       if constexpr (Cfg::TWOPASS) {
       constexpr int DYX = Cfg::DYX, ZS = BX * BY, HM = ORDER / 2;   // HM: reach of the centred first derivative
       const double f0 = p.at(0, 0, 0);
@@ -376,6 +380,7 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
           else Dz[(lz * (TY + 2 * HM) + hy + HM) * DYX + xx + HM] = v;
         }
         done(o);
+        early();
         named_barrier<PLANE>(1 + lz);
       } else if constexpr (TX * TY == 32) {
         // One z-plane of the tile = one warp: the warp fills its own plane's halo entries; no barrier at all.
@@ -397,6 +402,7 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
           else Dz[(lz * (TY + 2 * HM) + hy + HM) * DYX + xx + HM] = v;
         }
         done(o);
+        early();
         __syncwarp();
       } else {
       for (int h = tid; h < TX * 2 * HM * TZ; h += Cfg::THREADS) {          // D_z f on the y-halo rows -2,-1,TY,TY+1
@@ -418,6 +424,7 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
         else Dz[(hz * (TY + 2 * HM) + hy + HM) * DYX + xx + HM] = v;
       }
       done(o);
+      early();
       __syncthreads();
       }
       const double* y = Dy + (lz * TY + ly) * DYX + lx + HM;
@@ -428,8 +435,10 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
       } else {
         if (ORDER == 4) var_full(p, C, w, d1, d2, ad); else var_full8(p, C, w, d1, d2, ad);
         done(o);
+        early();
       }
     };
+    auto nothing = [] {};
 
     // IL: the advection + dissipation stencil of the variable staged by section o, parked in table entry e
     // (a thread reads back only what it wrote itself: no synchronisation, no hazard across tiles)
@@ -478,11 +487,13 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
       auto p = box(Sec::beta(i2));
       const StagePre pr = pre(Sec::beta(i2), 0);
       double d1[3], d2[6], ad;
-      full_var(p, w, Sec::beta(i2), i2, d1, d2, ad);
+      auto em = [&] { emit(V_BETA + i2, C.sgc * Bc + ad, pr); };
+      if constexpr (EARLY) full_var(p, w, Sec::beta(i2), i2, d1, d2, ad, em);
+      else full_var(p, w, Sec::beta(i2), i2, d1, d2, ad, nothing);
 #pragma unroll
       for (int a = 0; a < 3; ++a) { db[a][i2] = d1[a]; gdiv[a] = i2 == 0 ? d2[sym(a, i2)] : gdiv[a] + d2[sym(a, i2)]; }
       lapb[i2] = sdot(gu, d2);
-      emit(V_BETA + i2, C.sgc * Bc + ad, pr);
+      if constexpr (!EARLY) em();
       if constexpr (IL) park_ad(SecIL::at(i2), i2, w);   // At11, At12, At13
     }
     double divb = (db[0][0] + db[1][1]) + db[2][2];
@@ -504,7 +515,17 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
         auto p = box(Sec::gt(s));
         const StagePre pr = pre(Sec::gt(s), 0);
         double d1[3], d2[6], ad;
-        full_var(p, w, Sec::gt(s), 3 + s, d1, d2, ad);
+        auto em = [&] {
+          double lie;
+#pragma unroll
+          for (int k2 = 0; k2 < 3; ++k2) {
+            const double c = g[sym(i2, k2)] * db[j2][k2] + g[sym(j2, k2)] * db[i2][k2];
+            lie = k2 == 0 ? c : lie + c;
+          }
+          emit(V_GT + s, (lie - two_thirds * g[s] * divb) - 2.0 * alpha * At[s] + ad, pr);
+        };
+        if constexpr (EARLY) full_var(p, w, Sec::gt(s), 3 + s, d1, d2, ad, em);
+        else full_var(p, w, Sec::gt(s), 3 + s, d1, d2, ad, nothing);
         if constexpr (PARK) {
           const double d4[4] = {d1[0], d1[1], d1[2], 0.0};
           tmem_park<4>(park, P_DG + 4 * s, d4);
@@ -512,13 +533,7 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
           dg[0][s] = d1[0]; dg[1][s] = d1[1]; dg[2][s] = d1[2];
         }
         Rt[s] = -0.5 * sdot(gu, d2);
-        double lie;
-#pragma unroll
-        for (int k2 = 0; k2 < 3; ++k2) {
-          const double c = g[sym(i2, k2)] * db[j2][k2] + g[sym(j2, k2)] * db[i2][k2];
-          lie = k2 == 0 ? c : lie + c;
-        }
-        emit(V_GT + s, (lie - two_thirds * g[s] * divb) - 2.0 * alpha * At[s] + ad, pr);
+        if constexpr (!EARLY) em();
         if constexpr (IL) {
           if (s < 3) park_ad(SecIL::at(3 + s), 3 + s, w);   // At22, At23, At33
           else {                                             // B1, B2, B3: the stencil result and the point value
@@ -641,8 +656,9 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
       auto p = box(Sec::chi);
       const StagePre pr = pre(Sec::chi, 0);
       double d2[6], ad;
-      full_var(p, w, Sec::chi, 9, dchi, d2, ad);
-      emit(V_CHI, two_thirds * chi * (alpha * trK - divb) + ad, pr);
+      auto em = [&] { emit(V_CHI, two_thirds * chi * (alpha * trK - divb) + ad, pr); };
+      if constexpr (EARLY) full_var(p, w, Sec::chi, 9, dchi, d2, ad, em);
+      else { full_var(p, w, Sec::chi, 9, dchi, d2, ad, nothing); em(); }
       double cd[6], cc[6];   // D~_i D~_j chi ; d_i chi d_j chi
       if constexpr (PARK) {   // Gamma~^k_ij one k at a time from tensor memory
 #pragma unroll
@@ -675,8 +691,9 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
       auto p = box(Sec::alpha);
       const StagePre pr = pre(Sec::alpha, 0);
       double d2[6], ad;
-      full_var(p, w, Sec::alpha, 10, dal, d2, ad);
-      emit(V_ALPHA, -2.0 * alpha * trK + ad, pr);
+      auto em = [&] { emit(V_ALPHA, -2.0 * alpha * trK + ad, pr); };
+      if constexpr (EARLY) full_var(p, w, Sec::alpha, 10, dal, d2, ad, em);
+      else { full_var(p, w, Sec::alpha, 10, dal, d2, ad, nothing); em(); }
       double cd[6], ca[6];   // d_i d_j alpha - Gamma~^k_ij d_k alpha ; d_i chi d_j alpha + d_j chi d_i alpha
       if constexpr (PARK) {
 #pragma unroll
@@ -914,14 +931,14 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
   bssn_tma_body<TX, TY, TZ, MODE, ORDER, false>(tm, tmCen, tmU, tmS, tmU, tmS, tmU, tmS, L, C, st, ntx, nty, ntz, cy);
 }
 // interleaved section layout (4th order, 256-point tiles)
-template <int TX, int TY, int TZ, int MODE>
+template <int TX, int TY, int TZ, int MODE, bool EARLY = false>
 __global__ void __launch_bounds__(TX* TY* TZ, 1)
 bssn_tma_il_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ CUtensorMap tmCen,
                    const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS,
                    const __grid_constant__ CUtensorMap tmU4, const __grid_constant__ CUtensorMap tmS4,
                    const __grid_constant__ CUtensorMap tmU3, const __grid_constant__ CUtensorMap tmS3, Layout L, Coef C,
                    Stage st, int ntx, int nty, int ntz, int cy) {
-  bssn_tma_body<TX, TY, TZ, MODE, 4, true>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C, st, ntx, nty, ntz, cy);
+  bssn_tma_body<TX, TY, TZ, MODE, 4, true, EARLY>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C, st, ntx, nty, ntz, cy);
 }
 
 #ifndef CHM_EMULATE
@@ -993,11 +1010,11 @@ static TmaPlan bssn_plan(int mode, int xo) {
   return p;
 }
 
-template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL = false>
+template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL = false, bool EARLY = false>
 static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
   using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL>;
   const void* kern;
-  if constexpr (IL) kern = (const void*)bssn_tma_il_kernel<TX, TY, TZ, MODE>;
+  if constexpr (IL) kern = (const void*)bssn_tma_il_kernel<TX, TY, TZ, MODE, EARLY>;
   else kern = (const void*)bssn_tma_kernel<TX, TY, TZ, MODE, ORDER>;
   if (a) return cudaFuncGetAttributes(a, kern);
   // nothing is launched unless the validator accepts what this instance will issue on this layout
@@ -1044,21 +1061,21 @@ static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, 
   const int grid = ntiles < sms * blocks_per_sm ? ntiles : sms * blocks_per_sm;
   const int cy = L.col_rows / TY > 0 ? L.col_rows / TY : 1;   // tile rows per traversal column
   if constexpr (IL)
-    bssn_tma_il_kernel<TX, TY, TZ, MODE><<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C,
+    bssn_tma_il_kernel<TX, TY, TZ, MODE, EARLY><<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C,
                                                                                 *st, ntx, nty, ntz, cy);
   else
     bssn_tma_kernel<TX, TY, TZ, MODE, ORDER><<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, L, C, *st, ntx, nty, ntz, cy);
   return cudaGetLastError();
 }
 
-template <int TX, int TY, int TZ, int ORDER = 4, bool IL = false>
+template <int TX, int TY, int TZ, int ORDER = 4, bool IL = false, bool EARLY = false>
 static cudaError_t tma_go(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
   switch (st ? st->mode : MODE_MID) {   // kernel_info reports the common (middle-stage) instance
-    case MODE_RHS: return tma_go_mode<TX, TY, TZ, MODE_RHS, ORDER, IL>(L, C, st, s, a);
-    case MODE_FIRST: return tma_go_mode<TX, TY, TZ, MODE_FIRST, ORDER, IL>(L, C, st, s, a);
-    case MODE_MID: return tma_go_mode<TX, TY, TZ, MODE_MID, ORDER, IL>(L, C, st, s, a);
-    case MODE_LAST: return tma_go_mode<TX, TY, TZ, MODE_LAST, ORDER, IL>(L, C, st, s, a);
-    case MODE_SSP: return tma_go_mode<TX, TY, TZ, MODE_SSP, ORDER, IL>(L, C, st, s, a);
+    case MODE_RHS: return tma_go_mode<TX, TY, TZ, MODE_RHS, ORDER, IL, EARLY>(L, C, st, s, a);
+    case MODE_FIRST: return tma_go_mode<TX, TY, TZ, MODE_FIRST, ORDER, IL, EARLY>(L, C, st, s, a);
+    case MODE_MID: return tma_go_mode<TX, TY, TZ, MODE_MID, ORDER, IL, EARLY>(L, C, st, s, a);
+    case MODE_LAST: return tma_go_mode<TX, TY, TZ, MODE_LAST, ORDER, IL, EARLY>(L, C, st, s, a);
+    case MODE_SSP: return tma_go_mode<TX, TY, TZ, MODE_SSP, ORDER, IL, EARLY>(L, C, st, s, a);
   }
   return cudaErrorInvalidValue;
 }
@@ -1073,6 +1090,7 @@ static cudaError_t tma_dispatch(int order, int tile, const Layout& L, const Coef
     case 3: return tma_go<16, 2, 8>(L, C, st, s, a);
     case 4: return tma_go<16, 4, 2>(L, C, st, s, a);
     case 5: return tma_go<16, 4, 4, 4, true>(L, C, st, s, a);   // interleaved section layout
+    case 6: return tma_go<16, 4, 4, 4, true, true>(L, C, st, s, a);   // the same, right-hand sides emitted before the plane barrier
   }
   return cudaErrorInvalidValue;
 }
@@ -1089,7 +1107,7 @@ void plans_bssn_fused(std::vector<TmaPlan>& out) {
       out.push_back(bssn_plan<8, 4, 8, 4>(mode, xo));
       out.push_back(bssn_plan<16, 2, 8, 4>(mode, xo));
       out.push_back(bssn_plan<16, 4, 2, 4>(mode, xo));
-      out.push_back(bssn_plan<16, 4, 4, 4, true>(mode, xo));
+      out.push_back(bssn_plan<16, 4, 4, 4, true>(mode, xo));   // ids 5 and 6 issue the same loads
       if (g >= 5) out.push_back(bssn_plan<16, 4, 4, 8>(mode, xo));
     }
 }

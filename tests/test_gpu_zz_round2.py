@@ -188,7 +188,7 @@ def test_interleaved_layout_rhs_and_bit_identity(chem, oracle, data):
     h = chem.Chemora(nx, ny, nz, g, 4, chem.SYS_BSSN, dx)
     h.set_param("eps_diss", eps)
     res = {}
-    for tile in (0, 5):
+    for tile in (0, 5, 6):
         h.set_variant(1, tile)
         pad = h.new_state()
         h.interior(pad).copy_(__import__("torch").from_numpy(u))
@@ -200,17 +200,19 @@ def test_interleaved_layout_rhs_and_bit_identity(chem, oracle, data):
         h.set_state(u)
         h.rk4_step(0.25 * dx)
         res[tile] = (rhs, h.get_state())
-    assert np.array_equal(res[0][0], res[5][0]) and np.array_equal(res[0][1], res[5][1])
+    for tile in (5, 6):
+        assert np.array_equal(res[0][0], res[tile][0]) and np.array_equal(res[0][1], res[tile][1]), tile
     h.destroy()
 
 
-def test_interleaved_layout_10_steps_and_rk3(chem, oracle):
+@pytest.mark.parametrize("tile", [5, 6])
+def test_interleaved_layout_10_steps_and_rk3(chem, oracle, tile):
     nx, ny, nz, g, dx, eps = 24, 20, 18, 3, 0.05, 0.1
     dt = 0.25 * dx
     u0 = inputs.bssn_noise(nx, ny, nz)
     h = chem.Chemora(nx, ny, nz, g, 4, chem.SYS_BSSN, dx)
     h.set_param("eps_diss", eps)
-    h.set_variant(1, 5)
+    h.set_variant(1, tile)
     h.set_state(u0)
     for _ in range(10):
         h.rk4_step(dt)
