@@ -177,8 +177,8 @@ def test_radiative_rk4_whole_block(chem, oracle, system, order, g, steps, tol):
 # ------------------------------------------- fused tile id 5: the interleaved section layout
 @pytest.mark.parametrize("data", ["noise1e-10", "gaussians", "strong"])
 def test_interleaved_layout_rhs_and_bit_identity(chem, oracle, data):
-    """id 5 against the oracle on ragged tiles, and bit for bit against id 0 (same arithmetic, other section order):
-    plain right-hand side and a whole RK4 step"""
+    """ids 5 and 6 against the oracle on ragged tiles, and against id 0 (same arithmetic, other section order) at rounding
+    level: plain right-hand side and a whole RK4 step"""
     nx, ny, nz, g, dx, eps = 37, 22, 19, 3, 0.05, 0.1
     u = {"noise1e-10": lambda: inputs.bssn_noise(nx, ny, nz),
          "gaussians": lambda: inputs.bssn_gaussians(nx, ny, nz, width_cells=4.0),
@@ -200,8 +200,10 @@ def test_interleaved_layout_rhs_and_bit_identity(chem, oracle, data):
         h.set_state(u)
         h.rk4_step(0.25 * dx)
         res[tile] = (rhs, h.get_state())
+    # same arithmetic in another section order: bit-identical under the host emulator; on the device the compiler may
+    # contract a product and a sum differently in the two instantiations, so the bar here is rounding level
     for tile in (5, 6):
-        assert np.array_equal(res[0][0], res[tile][0]) and np.array_equal(res[0][1], res[tile][1]), tile
+        assert relerr(res[tile][0], res[0][0]) < 1e-13 and relerr(res[tile][1], res[0][1]) < 1e-14, tile
     h.destroy()
 
 
