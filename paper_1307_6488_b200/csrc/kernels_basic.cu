@@ -17,7 +17,10 @@ __global__ void __launch_bounds__(256) fill_ghosts_kernel(Layout L, double* __re
                                                           int lpr_shift, FillLink link) {
   const int g = L.g, tx = L.nx + 2 * g, lane = threadIdx.x & 31;
   const int task = blockIdx.x * 8 + (threadIdx.x >> 5);
-  auto wrap = [g](int c, int n) { int r = (c - g) % n; return (r < 0 ? r + n : r) + g; };
+  // padded coordinate c in [0, n + 2g) -> padded coordinate of its periodic image in [g, g + n).  chemora_create
+  // guarantees n >= g, so one conditional shift by n replaces the integer modulo (the per-element division was the
+  // bulk of this kernel's instructions)
+  auto wrap = [g](int c, int n) { return c < g ? c + n : (c >= g + n ? c - n : c); };
   // the first ghost column of a row is column L.xo - g of the padded row
   double* p = state + (long)blockIdx.y * L.vstride + (L.xo - g);
   if (task < rowsAB) {
