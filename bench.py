@@ -172,6 +172,7 @@ def run_ours(args):
         h.set_variant(fused, tile)
         sweep_ms = None
     info = h.kernel_info()
+    col_rows = int(h.get_param("col_rows"))
 
     # ---- device-resident timing: W warm-up, then exactly K steps ------------------------------------------
     for _ in range(args.warmup):
@@ -207,6 +208,7 @@ def run_ours(args):
         h2 = binding.Chemora(n, n, n, g, c["order"], binding.SYS_BSSN, dx, device="cuda:%d" % local)
     h2.set_param("eps_diss", c["eps_diss"])
     h2.set_variant(*h.get_variant())
+    h2.set_param("col_rows", col_rows)
     pipe.append(h2)
     outs = [torch.empty_like(host).pin_memory() for _ in pipe]
     for hh, o in zip(pipe, outs):   # warm-up (staging allocation)
@@ -246,7 +248,8 @@ def run_ours(args):
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": "BSSN (25 vars) O4 centred FD + upwind advection + KO5, fp64, %d^3 interior, g=3, "
                                "RK4 4-buffer, configs[3] recipe (Minkowski + 1e-4 Gaussians)" % n,
-                   "variant": {"fused": fused, "tile": list(binding.tile_shape(tile, binding.SYS_BSSN, fused)), "sweep_ms": sweep_ms},
+                   "variant": {"fused": fused, "tile_id": tile, "tile": list(binding.tile_shape(tile, binding.SYS_BSSN, fused)),
+                               "col_rows": col_rows, "sweep_ms": sweep_ms},
                    "kernel": info, "multi_gpu": "replicas only",
                    "l2": "inputs larger than L2 (%.2f GB per state buffer vs 126 MB)" % (h.nvars * h.var_stride * 8 / 1e9)},
         "roofline": {"bound": "hbm", "kernel": ("bssn_tma_il_kernel" if tile == 5 else "bssn_tma_kernel") if fused else "bssn_derivs+from_derivs",

@@ -207,6 +207,8 @@ int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, 
  * the same right-hand side, so a candidate whose result (Ya) differs from the first fused id's (kept in Yb for the
  * duration of the sweep) by more than 1e-11 in the norm of reading S11, or whose bounded waits gave up, is
  * disqualified: ms_out = -2 / -3.
+ * For the fused BSSN kernel the pick is then timed with half and twice the current "col_rows" and the fastest
+ * extent is kept (chemora_get_param tells which; results do not depend on it).
  * ms_out, if not NULL, receives 2*CHEMORA_NUM_TILES timings in milliseconds ([fused*NUM_TILES + tile];
  * negative = variant unavailable or not timed).  U is not modified.  Synchronous. */
 int chemora_autotune(chemora_t* h, int* fused, int* tile_id, float* ms_out);

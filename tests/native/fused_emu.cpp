@@ -21,7 +21,7 @@ static Layout make_layout(int nx, int ny, int nz, int g) {   // the rule of chem
   L.tot_y = ny + 2 * g; L.tot_z = nz + 2 * g;
   L.plane = L.pitch * L.tot_y;
   L.vstride = L.plane * L.tot_z;
-  L.col_rows = 32;
+  L.col_rows = getenv("CHM_COL_ROWS") ? atoi(getenv("CHM_COL_ROWS")) : 32;   // tile traversal: any value, same result
   return L;
 }
 

@@ -90,6 +90,19 @@ def test_interleaved_layout_is_bit_identical_to_the_plain_one(oracle, emu, tmp_p
     assert a0[3]["loads"] == ntiles * (25 + 50 + 3) and a5[3]["loads"] == ntiles * (25 + 2 * 13 + 2 * 2 + 4 + 3)
 
 
+@pytest.mark.parametrize("col_rows", [2, 4, 8, 64])
+def test_tile_traversal_order_does_not_change_the_result(oracle, emu, tmp_path, col_rows, monkeypatch):
+    """the tuning parameter col_rows (y-extent of the columns in which the persistent CTAs visit the tiles; the runtime
+    sweep tries half and twice its value) only permutes the tiles: same bits, every tile visited once"""
+    nx, ny, nz, g, h, eps = 20, 13, 6, 3, 0.05, 0.1
+    st = oracle.fill_ghosts(oracle.with_ghosts(strong(nx, ny, nz), g), g)
+    z = np.zeros_like(st)
+    ref = launch(emu, tmp_path, 4, 0, MODE_RHS, st, z, z, g, h, eps, grid=3)
+    monkeypatch.setenv("CHM_COL_ROWS", str(col_rows))
+    got = launch(emu, tmp_path, 4, 5, MODE_RHS, st, z, z, g, h, eps, grid=3)
+    assert np.array_equal(ref[0], got[0]) and ref[3]["loads"] == got[3]["loads"]
+
+
 def test_flat_space_gives_exactly_zero(oracle, emu, tmp_path):
     st = oracle.fill_ghosts(oracle.with_ghosts(inputs.bssn_minkowski(16, 8, 8), 3), 3)
     z = np.zeros_like(st)
