@@ -189,7 +189,9 @@ int chemora_energy(chemora_t* h, const double* dev_state, double* dev_eps, doubl
  * per thread, staged with an (order/2 + 1)-cell halo by TMA; ids 0..4 = 16x4x4, 16x8x2, 8x4x8, 16x2x8, 16x4x2 at 4th
  * order, id 5 = 16x4x4 with the interleaved section layout (the cheap advection-only stencils evaluated between the
  * expensive sections, box-less emit sections at the end of a tile), id 6 = id 5 with a full
- * variable's own right-hand side emitted before the plane barrier of its mixed derivatives; id 0 only at 8th order.  Split BSSN kernels (ids 0..5) and the L1-path wave kernels (ids 0..5): an x*y thread
+ * variable's own right-hand side emitted before the plane barrier of its mixed derivatives, id 7 = id 6 with a six-slot box ring
+ * (a box section of that layout needs two operand tiles, not four: six slots fit the shared memory of five); id 0 only
+ * at 8th order.  Split BSSN kernels (ids 0..5) and the L1-path wave kernels (ids 0..5): an x*y thread
  * block marching z planes.  Ids 6..8 of the wave systems: the TMA plane-ring kernel (CHEMORA_SYS_WAVE: 32x16x32,
  * 32x16x64, 64x8x32; CHEMORA_SYS_WAVE1, five variables a plane: 16x8x64, 16x16x64, 32x8x64; runs id - 6 instead
  * when the layout does not give 16-byte aligned plane boxes or the ring of planes does not fit shared memory,

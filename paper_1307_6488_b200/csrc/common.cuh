@@ -134,9 +134,10 @@ __device__ __forceinline__ void stage_emit_t(const Stage& st, long q, double k, 
 // kernel: x,y = thread block, z = planes marched per block.
 struct TileShape { int tx, ty, tz; };
 // fused BSSN tile ids 0..6 (8th order: id 0 only); id 5: 16x4x4 with the interleaved section layout; id 6: the same
-// with a full variable's own right-hand side emitted before the plane barrier of its mixed derivatives
-constexpr int kNumFused = 7;
-static const TileShape kTilesFused[kNumFused] = {{16, 4, 4}, {16, 8, 2}, {8, 4, 8}, {16, 2, 8}, {16, 4, 2}, {16, 4, 4}, {16, 4, 4}};
+// with a full variable's own right-hand side emitted before the plane barrier of its mixed derivatives; id 7: id 6
+// with a six-slot box ring
+constexpr int kNumFused = 8;
+static const TileShape kTilesFused[kNumFused] = {{16, 4, 4}, {16, 8, 2}, {8, 4, 8}, {16, 2, 8}, {16, 4, 2}, {16, 4, 4}, {16, 4, 4}, {16, 4, 4}};
 // wave system ids 6..8: the TMA plane-ring kernel (x, y = thread block, z = planes per work item)
 static const TileShape kTilesWaveTma[3] = {{32, 16, 32}, {32, 16, 64}, {64, 8, 32}};
 // Sample-1 system ids 6..8: the same plane-ring kernel with five variables (smaller tiles: the ring holds 5 boxes a plane)

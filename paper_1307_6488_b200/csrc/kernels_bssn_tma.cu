@@ -72,8 +72,12 @@ struct SecPlain {
   static constexpr int chi = 12, alpha = 13, k = 14, a = 24;
 };
 
-template <int TX, int TY, int TZ, int ORDER = 4, bool IL = false>
+// DEEP (interleaved layout only): six ring slots instead of five in the same shared memory -- a box section of the
+// interleaved layout emits at most one variable, so a slot needs two operand tiles instead of four, and 30 sections
+// divide by six as well as by five (the slot stays a compile-time constant of a section)
+template <int TX, int TY, int TZ, int ORDER = 4, bool IL = false, bool DEEP = false>
 struct TmaCfg {
+  static_assert(!DEEP || IL, "the six-slot ring belongs to the interleaved layout");
   static_assert(!IL || (ORDER == 4 && TX * TY * TZ == 256), "the interleaved layout is built for 4th order, 256-point tiles");
   static constexpr int H = ORDER == 8 ? 5 : 3;    // halo: upwinded stencils reach order/2 + 1 cells
   static_assert(TX % 2 == 0 && ((TX + 2) * TY * TZ) % 16 == 0, "tile boxes must stay 128-byte aligned in smem");
@@ -84,11 +88,11 @@ struct TmaCfg {
   static constexpr bool HEAVY = THREADS > 256;    // 12 warps at 168 registers: live values parked in tensor memory
   // ring slots (a 6-slot ring fits the 16x4x4 tile but its run-time slot index costs more than the depth gains:
   // 8.2 ms vs 6.3 ms)
-  static constexpr int NS = ORDER == 8 ? 3 : HEAVY ? 4 : 5;   // 8th order: 41 KB boxes, three fit
+  static constexpr int NS = DEEP ? 6 : ORDER == 8 ? 3 : HEAVY ? 4 : 5;   // 8th order: 41 KB boxes, three fit
   static constexpr bool PARK = HEAVY;
   static constexpr int TILE = (TX + 2) * TY * TZ;                      // doubles in one (TX+2,TY,TZ) tile box
   static constexpr uint32_t TILE_BYTES = (uint32_t)TILE * 8u;
-  static constexpr int SLOTX = SLOT + 4 * TILE;   // box + RK4 operands (U,S) of up to two emitted variables
+  static constexpr int SLOTX = SLOT + (DEEP ? 2 : 4) * TILE;   // box + RK4 operands (U,S) of up to two emitted variables
   static constexpr int CEN = kCenVars * TILE;     // point values needed ahead of their own boxes
   // first derivatives shared between threads for the mixed second derivatives (two buffers, alternating):
   // D_y f on the tile + 2 columns of x-halo, D_z f on the tile + 2 columns of x-halo + 2 rows of y-halo
@@ -115,12 +119,12 @@ struct TmaCfg {
 // EARLY: a full variable's own right-hand side (which needs none of its mixed derivatives) leaves BEFORE the plane
 // barrier of the two-pass mixed derivatives instead of after it, so the time a warp would spend waiting for its
 // plane partner is spent on the operand reads, the stage update and the stores (capture L: 4 % of stall samples)
-template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL, bool EARLY = false>
+template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL, bool EARLY = false, bool DEEP = false>
 __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUtensorMap& tmCen, const CUtensorMap& tmU,
                                               const CUtensorMap& tmS, const CUtensorMap& tmU4, const CUtensorMap& tmS4,
                                               const CUtensorMap& tmU3, const CUtensorMap& tmS3, const Layout& L,
                                               const Coef& C, const Stage& st, int ntx, int nty, int ntz, int cy) {
-  using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL>;
+  using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL, DEEP>;
   constexpr int H = Cfg::H;
   constexpr int BX = Cfg::BX, BY = Cfg::BY, SLOT = Cfg::SLOT, SLOTX = Cfg::SLOTX, TILE = Cfg::TILE, CEN = Cfg::CEN;
   constexpr unsigned NW = Cfg::NWARPS;
@@ -287,9 +291,10 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
     // RK4 stage operands (U, S) of the n-th variable emitted by section o: staged by TMA next to the box;
     // read after box(o) and before done(o)
     // ring slot and mbarrier parity of section o of this CTA's t-th tile (load number 25 t + o)
-    auto slot_of = [&](int o) { return kSlots == 5 ? o % 5 : (25 * t + o) % kSlots; };
+    auto slot_of = [&](int o) { return (kSlots == 5 || IL) ? o % kSlots : (25 * t + o) % kSlots; };
     auto parity_of = [&](int o) {
-      if constexpr (IL) return (uint32_t)(o / 5) & 1u;   // 30 sections = 6 phases of a slot per tile: no dependence on t
+      // 30 sections: 6 phases of a slot per tile with five slots (no dependence on t), 5 with six slots
+      if constexpr (IL) return (uint32_t)((NSEC / kSlots) * t + o / kSlots) & 1u;
       else return (uint32_t)(kSlots == 5 ? (t + o / 5) & 1 : ((25 * t + o) / kSlots) & 1);
     };
     // IL emit sections: operands (U, S) of the n-th variable of the section (U tiles 0..3, S tiles 4..7 of the slot)
@@ -931,14 +936,14 @@ bssn_tma_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ 
   bssn_tma_body<TX, TY, TZ, MODE, ORDER, false>(tm, tmCen, tmU, tmS, tmU, tmS, tmU, tmS, L, C, st, ntx, nty, ntz, cy);
 }
 // interleaved section layout (4th order, 256-point tiles)
-template <int TX, int TY, int TZ, int MODE, bool EARLY = false>
+template <int TX, int TY, int TZ, int MODE, bool EARLY = false, bool DEEP = false>
 __global__ void __launch_bounds__(TX* TY* TZ, 1)
 bssn_tma_il_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ CUtensorMap tmCen,
                    const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS,
                    const __grid_constant__ CUtensorMap tmU4, const __grid_constant__ CUtensorMap tmS4,
                    const __grid_constant__ CUtensorMap tmU3, const __grid_constant__ CUtensorMap tmS3, Layout L, Coef C,
                    Stage st, int ntx, int nty, int ntz, int cy) {
-  bssn_tma_body<TX, TY, TZ, MODE, 4, true, EARLY>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C, st, ntx, nty, ntz, cy);
+  bssn_tma_body<TX, TY, TZ, MODE, 4, true, EARLY, DEEP>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C, st, ntx, nty, ntz, cy);
 }
 
 #ifndef CHM_EMULATE
@@ -962,11 +967,11 @@ static EncodeTiledFn encode_fn() {
 // What one launch of bssn_tma_kernel<TX,TY,TZ,MODE,ORDER> issues, for the validator: every section's box and
 // operand loads with the mbarrier byte count the kernel announces for it (one "barrier" entry per section, one for
 // the point-value tiles).  xo: Layout::xo (decides the parity of the x coordinates).
-template <int TX, int TY, int TZ, int ORDER, bool IL = false>
+template <int TX, int TY, int TZ, int ORDER, bool IL = false, bool DEEP = false>
 static TmaPlan bssn_plan(int mode, int xo) {
-  using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL>;
+  using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL, DEEP>;
   char name[64];
-  snprintf(name, sizeof name, "bssn_tma%s_kernel<%d,%d,%d,order %d>", IL ? "_il" : "", TX, TY, TZ, ORDER);
+  snprintf(name, sizeof name, "bssn_tma%s_kernel<%d,%d,%d,order %d%s>", IL ? "_il" : "", TX, TY, TZ, ORDER, DEEP ? ",6 slots" : "");
   TmaPlan p;
   p.kernel = name;
   p.smem_bytes = Cfg::SMEM;
@@ -1010,15 +1015,15 @@ static TmaPlan bssn_plan(int mode, int xo) {
   return p;
 }
 
-template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL = false, bool EARLY = false>
+template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL = false, bool EARLY = false, bool DEEP = false>
 static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
-  using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL>;
+  using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL, DEEP>;
   const void* kern;
-  if constexpr (IL) kern = (const void*)bssn_tma_il_kernel<TX, TY, TZ, MODE, EARLY>;
+  if constexpr (IL) kern = (const void*)bssn_tma_il_kernel<TX, TY, TZ, MODE, EARLY, DEEP>;
   else kern = (const void*)bssn_tma_kernel<TX, TY, TZ, MODE, ORDER>;
   if (a) return cudaFuncGetAttributes(a, kern);
   // nothing is launched unless the validator accepts what this instance will issue on this layout
-  if (!launch_allowed(bssn_plan<TX, TY, TZ, ORDER, IL>(MODE, L.xo), L, st->in, L.xo - Cfg::H, Cfg::H)) return cudaErrorInvalidValue;
+  if (!launch_allowed(bssn_plan<TX, TY, TZ, ORDER, IL, DEEP>(MODE, L.xo), L, st->in, L.xo - Cfg::H, Cfg::H)) return cudaErrorInvalidValue;
   EncodeTiledFn enc = encode_fn();
   if (!enc) return cudaErrorNotSupported;
   CUtensorMap tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3;
@@ -1061,21 +1066,21 @@ static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, 
   const int grid = ntiles < sms * blocks_per_sm ? ntiles : sms * blocks_per_sm;
   const int cy = L.col_rows / TY > 0 ? L.col_rows / TY : 1;   // tile rows per traversal column
   if constexpr (IL)
-    bssn_tma_il_kernel<TX, TY, TZ, MODE, EARLY><<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C,
+    bssn_tma_il_kernel<TX, TY, TZ, MODE, EARLY, DEEP><<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C,
                                                                                 *st, ntx, nty, ntz, cy);
   else
     bssn_tma_kernel<TX, TY, TZ, MODE, ORDER><<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, L, C, *st, ntx, nty, ntz, cy);
   return cudaGetLastError();
 }
 
-template <int TX, int TY, int TZ, int ORDER = 4, bool IL = false, bool EARLY = false>
+template <int TX, int TY, int TZ, int ORDER = 4, bool IL = false, bool EARLY = false, bool DEEP = false>
 static cudaError_t tma_go(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
   switch (st ? st->mode : MODE_MID) {   // kernel_info reports the common (middle-stage) instance
-    case MODE_RHS: return tma_go_mode<TX, TY, TZ, MODE_RHS, ORDER, IL, EARLY>(L, C, st, s, a);
-    case MODE_FIRST: return tma_go_mode<TX, TY, TZ, MODE_FIRST, ORDER, IL, EARLY>(L, C, st, s, a);
-    case MODE_MID: return tma_go_mode<TX, TY, TZ, MODE_MID, ORDER, IL, EARLY>(L, C, st, s, a);
-    case MODE_LAST: return tma_go_mode<TX, TY, TZ, MODE_LAST, ORDER, IL, EARLY>(L, C, st, s, a);
-    case MODE_SSP: return tma_go_mode<TX, TY, TZ, MODE_SSP, ORDER, IL, EARLY>(L, C, st, s, a);
+    case MODE_RHS: return tma_go_mode<TX, TY, TZ, MODE_RHS, ORDER, IL, EARLY, DEEP>(L, C, st, s, a);
+    case MODE_FIRST: return tma_go_mode<TX, TY, TZ, MODE_FIRST, ORDER, IL, EARLY, DEEP>(L, C, st, s, a);
+    case MODE_MID: return tma_go_mode<TX, TY, TZ, MODE_MID, ORDER, IL, EARLY, DEEP>(L, C, st, s, a);
+    case MODE_LAST: return tma_go_mode<TX, TY, TZ, MODE_LAST, ORDER, IL, EARLY, DEEP>(L, C, st, s, a);
+    case MODE_SSP: return tma_go_mode<TX, TY, TZ, MODE_SSP, ORDER, IL, EARLY, DEEP>(L, C, st, s, a);
   }
   return cudaErrorInvalidValue;
 }
@@ -1091,6 +1096,7 @@ static cudaError_t tma_dispatch(int order, int tile, const Layout& L, const Coef
     case 4: return tma_go<16, 4, 2>(L, C, st, s, a);
     case 5: return tma_go<16, 4, 4, 4, true>(L, C, st, s, a);   // interleaved section layout
     case 6: return tma_go<16, 4, 4, 4, true, true>(L, C, st, s, a);   // the same, right-hand sides emitted before the plane barrier
+    case 7: return tma_go<16, 4, 4, 4, true, true, true>(L, C, st, s, a);   // the same with a six-slot ring
   }
   return cudaErrorInvalidValue;
 }
@@ -1108,6 +1114,7 @@ void plans_bssn_fused(std::vector<TmaPlan>& out) {
       out.push_back(bssn_plan<16, 2, 8, 4>(mode, xo));
       out.push_back(bssn_plan<16, 4, 2, 4>(mode, xo));
       out.push_back(bssn_plan<16, 4, 4, 4, true>(mode, xo));   // ids 5 and 6 issue the same loads
+      out.push_back(bssn_plan<16, 4, 4, 4, true, true>(mode, xo));
       if (g >= 5) out.push_back(bssn_plan<16, 4, 4, 8>(mode, xo));
     }
 }

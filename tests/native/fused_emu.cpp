@@ -46,7 +46,7 @@ static void from_padded(const Layout& L, const double* p, std::vector<double>& g
 
 template <int TX, int TY, int TZ, int MODE, int ORDER, int IL = 0>
 static chm_emu::Stats run(const Layout& L, const Coef& C, const Stage& st, int grid_req) {
-  using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL != 0>;
+  using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL != 0, IL == 3>;
   auto map = [&](const double* base, uint32_t bx, uint32_t by, uint32_t bz, uint32_t bv) {
     CUtensorMap m;
     m.base = base;
@@ -67,7 +67,7 @@ static chm_emu::Stats run(const Layout& L, const Coef& C, const Stage& st, int g
     const CUtensorMap tmU4 = map(ubase, TX + 2, TY, TZ, 4), tmS4 = map(sbase, TX + 2, TY, TZ, 4),
                       tmU3 = map(ubase, TX + 2, TY, TZ, 3), tmS3 = map(sbase, TX + 2, TY, TZ, 3);
     return chm_emu::run_grid(grid, Cfg::THREADS, 1, Cfg::SMEM, [&] {
-      bssn_tma_il_kernel<TX, TY, TZ, MODE, IL == 2>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C, st, ntx, nty, ntz, cy);
+      bssn_tma_il_kernel<TX, TY, TZ, MODE, IL >= 2, IL == 3>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C, st, ntx, nty, ntz, cy);
     });
   } else {
     return chm_emu::run_grid(grid, Cfg::THREADS, 1, Cfg::SMEM, [&] {
@@ -121,6 +121,7 @@ int main(int argc, char** argv) {
   else if (order == 4 && tile == 3) s = run_mode<16, 2, 8, 4>(mode, L, C, st, grid);
   else if (order == 4 && tile == 5) s = run_mode<16, 4, 4, 4, 1>(mode, L, C, st, grid);
   else if (order == 4 && tile == 6) s = run_mode<16, 4, 4, 4, 2>(mode, L, C, st, grid);
+  else if (order == 4 && tile == 7) s = run_mode<16, 4, 4, 4, 3>(mode, L, C, st, grid);
   else { fprintf(stderr, "instance not built into the emulator\n"); return 5; }
   std::vector<double> o(ng), so(ng), uo(ng);
   from_padded(L, out.data(), o); from_padded(L, S.data(), so); from_padded(L, (mode == MODE_FIRST ? in : U).data(), uo);

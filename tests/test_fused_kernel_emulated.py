@@ -54,7 +54,7 @@ def strong(nx, ny, nz, seed=21, amp=0.1):
 
 @pytest.mark.parametrize("order,g,tile,dims,grid", [(4, 3, 0, (20, 9, 6), 3), (4, 3, 1, (20, 9, 6), 2), (4, 3, 3, (17, 5, 11), 1),
                                                     (4, 4, 0, (18, 6, 5), 2), (8, 5, 0, (19, 6, 7), 2),
-                                                    (4, 3, 5, (20, 9, 6), 3), (4, 4, 5, (18, 6, 9), 1), (4, 3, 6, (20, 9, 6), 2)])
+                                                    (4, 3, 5, (20, 9, 6), 3), (4, 4, 5, (18, 6, 9), 1), (4, 3, 6, (20, 9, 6), 2), (4, 3, 7, (20, 9, 6), 3), (4, 4, 7, (18, 6, 9), 1)])
 @pytest.mark.parametrize("data", ["strong", "noise1e-10"])
 def test_rhs_against_the_oracle(oracle, emu, tmp_path, order, g, tile, dims, grid, data):
     nx, ny, nz = dims
@@ -68,7 +68,7 @@ def test_rhs_against_the_oracle(oracle, emu, tmp_path, order, g, tile, dims, gri
     m = np.ones(out.shape[1:], dtype=bool)
     m[g:-g, g:-g, g:-g] = False
     assert not out[:, m].any()                                  # nothing is written outside the interior
-    tx, ty, tz = {0: (16, 4, 4), 1: (16, 8, 2), 3: (16, 2, 8), 5: (16, 4, 4), 6: (16, 4, 4)}[tile]
+    tx, ty, tz = {0: (16, 4, 4), 1: (16, 8, 2), 3: (16, 2, 8), 5: (16, 4, 4), 6: (16, 4, 4), 7: (16, 4, 4)}[tile]
     ntiles = -(-nx // tx) * -(-ny // ty) * -(-nz // tz)
     assert stats["loads"] == ntiles * (25 + 3)                  # one box per section + three point-value groups
 
@@ -84,7 +84,9 @@ def test_interleaved_layout_is_bit_identical_to_the_plain_one(oracle, emu, tmp_p
     a5 = launch(emu, tmp_path, 4, 5, MODE_MID, st, U, S, g, h, eps, a=0.00625)
     a6 = launch(emu, tmp_path, 4, 6, MODE_MID, st, U, S, g, h, eps, a=0.00625)
     assert np.array_equal(a0[0], a5[0]) and np.array_equal(a0[1], a5[1]) and np.array_equal(a0[2], a5[2])
+    a7 = launch(emu, tmp_path, 4, 7, MODE_MID, st, U, S, g, h, eps, a=0.00625)
     assert np.array_equal(a0[0], a6[0]) and np.array_equal(a0[1], a6[1]) and a5[3] == a6[3]
+    assert np.array_equal(a0[0], a7[0]) and np.array_equal(a0[1], a7[1]) and a5[3] == a7[3]
     assert a0[3]["bytes"] == a5[3]["bytes"]
     ntiles = 2 * 3 * 2
     assert a0[3]["loads"] == ntiles * (25 + 50 + 3) and a5[3]["loads"] == ntiles * (25 + 2 * 13 + 2 * 2 + 4 + 3)
@@ -110,7 +112,7 @@ def test_flat_space_gives_exactly_zero(oracle, emu, tmp_path):
     assert not out.any()
 
 
-@pytest.mark.parametrize("tile", [0, 3, 5, 6])
+@pytest.mark.parametrize("tile", [0, 3, 5, 6, 7])
 def test_one_rk4_step_through_the_four_epilogues(oracle, emu, tmp_path, tile):
     """FIRST, MID, MID, LAST chained as chemora_rk4_step chains them (the periodic fill between the stages done by the
     oracle's fill): equals the oracle's RK4 step in both norms of DESIGN.md S11 / S11b"""
@@ -132,7 +134,7 @@ def test_one_rk4_step_through_the_four_epilogues(oracle, emu, tmp_path, tile):
         assert np.max(np.abs((got[v] - 1.0) - (want[v] - 1.0))) < max(1e-11, 8 * 2.3e-16 / amp) * amp
 
 
-@pytest.mark.parametrize("tile", [0, 5])
+@pytest.mark.parametrize("tile", [0, 5, 7])
 def test_ssp_epilogue(oracle, emu, tmp_path, tile):
     """MODE_SSP: out = ca U + cb (in + dt k), the Shu-Osher stage"""
     nx, ny, nz, g, h, eps = 16, 8, 4, 3, 0.05, 0.1

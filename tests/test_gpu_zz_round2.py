@@ -188,7 +188,7 @@ def test_interleaved_layout_rhs_and_bit_identity(chem, oracle, data):
     h = chem.Chemora(nx, ny, nz, g, 4, chem.SYS_BSSN, dx)
     h.set_param("eps_diss", eps)
     res = {}
-    for tile in (0, 5, 6):
+    for tile in (0, 5, 6, 7):
         h.set_variant(1, tile)
         pad = h.new_state()
         h.interior(pad).copy_(__import__("torch").from_numpy(u))
@@ -202,12 +202,12 @@ def test_interleaved_layout_rhs_and_bit_identity(chem, oracle, data):
         res[tile] = (rhs, h.get_state())
     # same arithmetic in another section order: bit-identical under the host emulator; on the device the compiler may
     # contract a product and a sum differently in the two instantiations, so the bar here is rounding level
-    for tile in (5, 6):
+    for tile in (5, 6, 7):
         assert relerr(res[tile][0], res[0][0]) < 1e-13 and relerr(res[tile][1], res[0][1]) < 1e-14, tile
     h.destroy()
 
 
-@pytest.mark.parametrize("tile", [5, 6])
+@pytest.mark.parametrize("tile", [5, 6, 7])
 def test_interleaved_layout_10_steps_and_rk3(chem, oracle, tile):
     nx, ny, nz, g, dx, eps = 24, 20, 18, 3, 0.05, 0.1
     dt = 0.25 * dx

@@ -1,7 +1,7 @@
 """Two whole RK4 steps with nothing but emulated kernels: the stage table of chemora_rk4_step (csrc/chemora.cu,
 rk4_plan: fill(U) FIRST -> fill(Yb) MID -> fill(Ya) MID -> fill(Yb) LAST on the buffers U, Ya, Yb, S) driven from
 Python, every launch the library's own kernel source under the CTA emulator -- fill_ghosts_kernel, then the fused
-kernel (plain layout id 0 and interleaved layout id 5).  Against the oracle's RK4, both norms of DESIGN.md S11/S11b."""
+kernel (plain layout id 0 and interleaved layout with the six-slot ring, id 7).  Against the oracle's RK4, both norms of DESIGN.md S11/S11b."""
 import os
 import subprocess
 
@@ -21,7 +21,7 @@ def emus():
     return build_emulator("basic_emu"), build_emulator("fused_emu")
 
 
-@pytest.mark.parametrize("tile", [0, 5])
+@pytest.mark.parametrize("tile", [0, 7])
 def test_two_rk4_steps_all_kernels_emulated(oracle, emus, tmp_path, tile):
     basic, fused = emus
     nx, ny, nz, g, h, eps = 18, 7, 6, 3, 0.05, 0.1
