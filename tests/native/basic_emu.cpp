@@ -29,7 +29,7 @@ int main(int argc, char** argv) {
   L.plane = L.pitch * L.tot_y; L.vstride = L.plane * L.tot_z;
   const long tx = nx + 2 * g;
   const size_t rows = (size_t)V * L.tot_z * L.tot_y, ng = rows * tx;
-  std::vector<double> ghosted(ng), in((size_t)V * L.vstride + 16, 0.0), out((size_t)V * L.vstride + 16, 0.0);
+  std::vector<double> ghosted(ng), in((size_t)V * L.vstride, 0.0), out((size_t)V * L.vstride, 0.0);
   FILE* f = fopen(argv[14], "rb");
   if (!f || fread(ghosted.data(), 8, ng, f) != ng) return 3;
   fclose(f);

@@ -37,14 +37,14 @@ int main(int argc, char** argv) {
   const long tx = nx + 2 * g;
   const size_t ng = (size_t)V * L.tot_z * L.tot_y * tx, rows = (size_t)V * L.tot_z * L.tot_y;
   auto load = [&](const char* path) {
-    std::vector<double> v(ng), p((size_t)V * L.vstride + 16, 0.0);
+    std::vector<double> v(ng), p((size_t)V * L.vstride, 0.0);
     FILE* f = fopen(path, "rb");
     if (!f || fread(v.data(), 8, ng, f) != ng) { fprintf(stderr, "cannot read %s\n", path); exit(3); }
     fclose(f);
     for (size_t r = 0; r < rows; ++r) memcpy(&p[r * L.pitch + (L.xo - g)], &v[r * tx], tx * 8);
     return p;
   };
-  std::vector<double> in = load(argv[12]), U = load(argv[13]), S = load(argv[14]), out((size_t)V * L.vstride + 16, 7.0);
+  std::vector<double> in = load(argv[12]), U = load(argv[13]), S = load(argv[14]), out((size_t)V * L.vstride, 7.0);
   Stage st{in.data(), mode == MODE_FIRST ? in.data() : U.data(), S.data(), out.data(), a, mode, ca, cb};
   const unsigned mask = system == 1 ? (1u << 0) | (1u << 1) | (1u << 4) | (1u << 6) | (1u << 17) : 0u;   // as chemora.cu
   const RadGeom G = rad_geom(L);

@@ -26,7 +26,7 @@ static Layout make_layout(int nx, int ny, int nz, int g) {   // the rule of chem
 }
 
 static std::vector<double> to_padded(const Layout& L, const std::vector<double>& ghosted) {
-  std::vector<double> p((size_t)L.nvars * L.vstride + 16, 0.0);
+  std::vector<double> p((size_t)L.nvars * L.vstride, 0.0);
   const long tx = L.nx + 2 * L.g;
   for (int v = 0; v < L.nvars; ++v)
     for (int k = 0; k < L.tot_z; ++k)
@@ -106,7 +106,7 @@ int main(int argc, char** argv) {
     return to_padded(L, v);
   };
   std::vector<double> in = load(argv[17]), U = load(argv[18]), S = load(argv[19]);
-  std::vector<double> out((size_t)25 * L.vstride + 16, 0.0);
+  std::vector<double> out((size_t)25 * L.vstride, 0.0);
   auto al = [](std::vector<double>& v) { return v.data(); };   // vectors of doubles are 16-byte aligned: enough here
   Coef C;   // as chemora.cu's make_coef
   C.inv_h = 1.0 / h; C.inv_h2 = 1.0 / (h * h); C.ko = eps / (64.0 * h); C.eta = eta; C.sgc = sgc;

@@ -59,14 +59,14 @@ int main(int argc, char** argv) {
   const long tx = nx + 2 * g;
   const size_t ng = (size_t)V * L.tot_z * L.tot_y * tx;
   auto load = [&](const char* path) {
-    std::vector<double> v(ng), p((size_t)V * L.vstride + 16, 0.0);
+    std::vector<double> v(ng), p((size_t)V * L.vstride, 0.0);
     FILE* f = fopen(path, "rb");
     if (!f || fread(v.data(), 8, ng, f) != ng) { fprintf(stderr, "cannot read %s\n", path); exit(3); }
     fclose(f);
     for (size_t r = 0; r < (size_t)V * L.tot_z * L.tot_y; ++r) memcpy(&p[r * L.pitch + (L.xo - g)], &v[r * tx], tx * 8);
     return p;
   };
-  std::vector<double> in = load(argv[16]), U = load(argv[17]), S = load(argv[18]), out((size_t)V * L.vstride + 16, 0.0);
+  std::vector<double> in = load(argv[16]), U = load(argv[17]), S = load(argv[18]), out((size_t)V * L.vstride, 0.0);
   Coef C{};
   C.inv_h = 1.0 / h; C.inv_h2 = 1.0 / (h * h); C.ko = ko ? eps / (64.0 * h) : 0.0;
   Stage st{in.data(), mode == MODE_FIRST ? in.data() : U.data(), S.data(), out.data(), a, mode, ca, cb};

@@ -1,0 +1,67 @@
+"""The emulated kernels once more under AddressSanitizer: the CTA's shared memory is one heap block and every state
+buffer an exactly sized heap array, so a shared-memory or global access outside its allocation -- which on the device
+is a fault (Xid 13/43) or silent corruption -- aborts the emulator here.  Covers the fused kernel in every section
+layout (ids 0, 1, 3, 5, 7; a middle RK4 stage, ragged tiles, several tiles per CTA), the 8th-order instance, the
+plane-ring kernel and the radiative face kernel.  Part of VERDICT r1 task 1 (no launch may fault)."""
+import os
+import subprocess
+
+import numpy as np
+import pytest
+
+from paper_1307_6488_b200 import inputs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def build(tmp, name):
+    exe = str(tmp / (name + "_asan"))
+    r = subprocess.run(["g++", "-std=c++17", "-O0", "-fsanitize=address", "-fno-omit-frame-pointer", "-DCHM_EMULATE",
+                        "-pthread", "-o", exe, os.path.join(ROOT, "tests", "native", name + ".cpp")], capture_output=True,
+                       text=True)
+    if r.returncode != 0 and "asan" in (r.stderr or "").lower():
+        pytest.skip("AddressSanitizer runtime not available")
+    assert r.returncode == 0, r.stderr[-2000:]
+    return exe
+
+
+def run(cmd):
+    env = dict(os.environ, ASAN_OPTIONS="detect_leaks=0")
+    r = subprocess.run(cmd, capture_output=True, text=True, env=env, timeout=900)
+    assert r.returncode == 0 and "AddressSanitizer" not in r.stderr, r.stderr[-3000:]
+    return r.stdout
+
+
+def test_fused_kernel_under_asan(oracle, tmp_path):
+    exe = build(tmp_path, "fused_emu")
+    g, h, eps = 3, 0.05, 0.1
+    for order, tile, dims, gg in [(4, 0, (20, 9, 6), 3), (4, 1, (17, 9, 3), 3), (4, 3, (17, 3, 9), 3), (4, 5, (20, 5, 6), 3),
+                                  (4, 7, (18, 5, 6), 4), (8, 0, (17, 5, 5), 5)]:
+        nx, ny, nz = dims
+        st = oracle.fill_ghosts(oracle.with_ghosts(inputs.bssn_noise(nx, ny, nz), gg), gg)
+        paths = [str(tmp_path / n) for n in ("in.bin", "U.bin", "S.bin", "out.bin")]
+        for p in paths[:3]:
+            st.tofile(p)
+        out = run([exe, str(order), str(tile), "2", str(nx), str(ny), str(nz), str(gg), repr(h), repr(eps), "1.0", "0.75", "5",
+                   "0.00625", "0.0", "0.0", "2"] + paths)
+        assert out.split()[1] == "0", out
+
+
+def test_wave_and_boundary_kernels_under_asan(oracle, tmp_path):
+    wave, bnd = build(tmp_path, "wave_emu"), build(tmp_path, "boundary_emu")
+    rng = np.random.default_rng(3)
+    paths = [str(tmp_path / n) for n in ("in.bin", "U.bin", "S.bin", "out.bin")]
+    for V, order, g, which, dims in [(2, 8, 4, 0, (33, 18, 35)), (5, 4, 3, 0, (19, 11, 66))]:
+        nx, ny, nz = dims
+        st = oracle.fill_ghosts(oracle.with_ghosts(rng.standard_normal((V, nz, ny, nx)), g), g)
+        for p in paths[:3]:
+            st.tofile(p)
+        run([wave, str(V), str(order), "1", str(which), "2", str(nx), str(ny), str(nz), str(g), "0.03125", "0.1", "0.01", "0.0",
+             "0.0", "2"] + paths)
+    for system, g, dims in [(1, 3, (9, 6, 5)), (0, 2, (10, 8, 6))]:
+        nx, ny, nz = dims
+        V = 25 if system == 1 else 2
+        st = rng.standard_normal((V, nz + 2 * g, ny + 2 * g, nx + 2 * g))
+        for p in paths[:3]:
+            st.tofile(p)
+        run([bnd, "rad", str(system), str(nx), str(ny), str(nz), str(g), "0.07", "2", "0.01", "0.0", "0.0"] + paths)
