@@ -189,11 +189,11 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
   // Origins (padded coordinates minus halo) of this CTA's tiles t and t+1 live in a 4-entry shared-memory ring
   // (entry t & 3: x0, y0, z0, valid), written one tile ahead by lane 0 of every warp (identical values), so the
   // refill path needs no registers for them.  Warps drift less than one tile apart, so entries t, t+1 are stable.
-  auto put_origin = [&](int e, int tl) {
+  auto put_origin = [&](int e, int tl, bool one_writer = false) {
     int b0 = 0, b1 = 0, b2 = 0;
     const bool ok = tl < ntiles;
     if (ok) decode(tl, b0, b1, b2);
-    if (lane == 0) {
+    if (one_writer ? tid == 0 : lane == 0) {
       int4 v = make_int4(b0 * TX + goffx, b1 * TY + goff, b2 * TZ + goff, ok ? 1 : 0);
       *reinterpret_cast<int4*>(org + 4 * (e & 3)) = v;
     }
@@ -255,7 +255,7 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
     }
     return last;
   };
-  put_origin(0, blockIdx.x);
+  put_origin(0, blockIdx.x, true);   // one writer: the block barrier below publishes it
   __syncthreads();
   if (tid == 0 && (int)blockIdx.x < ntiles) {
     const int x0 = org[0], y0 = org[1], z0 = org[2];

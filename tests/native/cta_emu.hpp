@@ -185,7 +185,11 @@ inline void tma_load_4d(void* dst, const CUtensorMap* tm, void* bar, int x, int 
 
 inline void sync_all() { t_cta->all.wait(t_cta->nthreads); }
 inline void sync_warp() { t_cta->warp[(t_threadIdx.y * t_blockDim.x + t_threadIdx.x) / 32]->wait(32); }
+#ifdef CHM_EMU_DROP_NAMED_BARRIERS   // self-test of the race detection: bar.sync id, n becomes a no-op
+inline void sync_named(int, int) {}
+#else
 inline void sync_named(int id, int count) { t_cta->named[id]->wait(count); }
+#endif
 inline double shfl_down(double v, int delta) {   // all 32 threads of the warp call it together
   const int t = t_threadIdx.y * t_blockDim.x + t_threadIdx.x;
   t_cta->shfl[t] = v;

@@ -65,3 +65,44 @@ def test_wave_and_boundary_kernels_under_asan(oracle, tmp_path):
         for p in paths[:3]:
             st.tofile(p)
         run([bnd, "rad", str(system), str(nx), str(ny), str(nz), str(g), "0.07", "2", "0.01", "0.0", "0.0"] + paths)
+
+
+def build_tsan(tmp, name, *defines):
+    exe = str(tmp / (name + "_tsan" + str(len(defines))))
+    r = subprocess.run(["g++", "-std=c++17", "-O0", "-fsanitize=thread", "-DCHM_EMULATE", "-pthread"] + list(defines) +
+                       ["-o", exe, os.path.join(ROOT, "tests", "native", name + ".cpp")], capture_output=True, text=True)
+    if r.returncode != 0 and "tsan" in (r.stderr or "").lower():
+        pytest.skip("ThreadSanitizer runtime not available")
+    assert r.returncode == 0, r.stderr[-2000:]
+    return exe
+
+
+def test_fused_kernel_under_thread_sanitizer(oracle, tmp_path):
+    """Race detection at the granularity of the emulator's barriers: the emulated CUDA threads are OS threads whose only
+    ordering comes from the kernel's own __syncthreads / __syncwarp / bar.sync / mbarrier calls, so a shared-memory
+    access pair the kernel's protocol leaves unordered (a slot refilled while a warp still reads it, a first-derivative
+    buffer rewritten before the plane's readers are through, the At_ij table laid over those buffers) is a
+    ThreadSanitizer report.  Every section layout of the fused kernel runs a middle RK4 stage clean; and, as a
+    self-test of the detector, the same kernel with its plane barriers compiled out (CHM_EMU_DROP_NAMED_BARRIERS) IS
+    reported."""
+    exe = build_tsan(tmp_path, "fused_emu")
+    h, eps = 0.05, 0.1
+    paths = [str(tmp_path / n) for n in ("in.bin", "U.bin", "S.bin", "out.bin")]
+    env = dict(os.environ, TSAN_OPTIONS="halt_on_error=0 report_signal_unsafe=0")
+
+    def go(binary, order, tile, dims, g):
+        nx, ny, nz = dims
+        st = oracle.fill_ghosts(oracle.with_ghosts(inputs.bssn_noise(nx, ny, nz), g), g)
+        for p in paths[:3]:
+            st.tofile(p)
+        return subprocess.run([binary, str(order), str(tile), "2", str(nx), str(ny), str(nz), str(g), repr(h), repr(eps), "1.0",
+                               "0.75", "5", "0.00625", "0.0", "0.0", "2"] + paths, capture_output=True, text=True, env=env,
+                              timeout=900)
+
+    for order, tile, dims, g in [(4, 0, (20, 9, 6), 3), (4, 1, (17, 9, 3), 3), (4, 3, (17, 3, 9), 3), (4, 5, (20, 5, 6), 3),
+                                 (4, 6, (20, 5, 6), 3), (4, 7, (18, 5, 6), 4), (8, 0, (17, 5, 5), 5)]:
+        r = go(exe, order, tile, dims, g)
+        assert "ThreadSanitizer" not in r.stderr and r.stdout.split()[1] == "0", (tile, r.stderr[-3000:])
+    broken = build_tsan(tmp_path, "fused_emu", "-DCHM_EMU_DROP_NAMED_BARRIERS")
+    r = go(broken, 4, 0, (20, 9, 6), 3)
+    assert "ThreadSanitizer: data race" in r.stderr
