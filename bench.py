@@ -165,8 +165,15 @@ def run_ours(args):
     h.set_param("eps_diss", c["eps_diss"])
     host = torch.from_numpy(u0).pin_memory()
     h.set_state(host.numpy())
+    sweep_error = None
     if args.variant == "auto":
-        fused, tile, sweep_ms = h.autotune()
+        try:
+            fused, tile, sweep_ms = h.autotune()
+        except binding.ChemoraError as e:     # the sweep must not cost the headline run: fall back to the default tile
+            sweep_error, sweep_ms = str(e), None
+            h.synchronize_quietly()
+            fused, tile = 1, 0
+            h.set_variant(fused, tile)
     else:
         fused, tile = [int(x) for x in args.variant.split(",")]
         h.set_variant(fused, tile)
@@ -249,7 +256,7 @@ def run_ours(args):
         "config": {"workload": "BSSN (25 vars) O4 centred FD + upwind advection + KO5, fp64, %d^3 interior, g=3, "
                                "RK4 4-buffer, configs[3] recipe (Minkowski + 1e-4 Gaussians)" % n,
                    "variant": {"fused": fused, "tile_id": tile, "tile": list(binding.tile_shape(tile, binding.SYS_BSSN, fused)),
-                               "col_rows": col_rows, "sweep_ms": sweep_ms},
+                               "col_rows": col_rows, "sweep_ms": sweep_ms, "sweep_error": sweep_error},
                    "kernel": info, "multi_gpu": "replicas only",
                    "l2": "inputs larger than L2 (%.2f GB per state buffer vs 126 MB)" % (h.nvars * h.var_stride * 8 / 1e9)},
         "roofline": {"bound": "hbm", "kernel": ("bssn_tma_il_kernel" if tile == 5 else "bssn_tma_kernel") if fused else "bssn_derivs+from_derivs",

@@ -270,6 +270,10 @@ class Chemora:
         self._ck(self.lib.chemora_synchronize(self._h))
         self._inflight = []
 
+    def synchronize_quietly(self):
+        """chemora_synchronize, return code instead of an exception (clears a pending device error word)"""
+        return self.lib.chemora_synchronize(self._h)
+
     def set_state_dev(self, dev_packed):
         self._ck(self.lib.chemora_set_state_dev(self._h, self._ptr(dev_packed)))
 
