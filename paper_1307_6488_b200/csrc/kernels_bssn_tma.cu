@@ -8,10 +8,10 @@
 // See bssn_tma.cuh for the design; DESIGN.md "Kernels" for the roofline that bounds it.
 #include <type_traits>
 
+#include <cstdio>
+
 #include "bssn_tma.cuh"
-#ifndef CHM_EMULATE
 #include "tma_check.cuh"
-#endif
 
 #ifndef CHM_L2HINT
 #define CHM_L2HINT 1
@@ -946,24 +946,7 @@ bssn_tma_il_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant
   bssn_tma_body<TX, TY, TZ, MODE, 4, true, EARLY, DEEP>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C, st, ntx, nty, ntz, cy);
 }
 
-#ifndef CHM_EMULATE
-// ---- host side: tensor map + launch -----------------------------------------------------------------------------
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-static EncodeTiledFn encode_fn() {
-  static EncodeTiledFn fn = nullptr;
-  if (!fn) {
-    void* p = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
-        qres == cudaDriverEntryPointSuccess)
-      fn = (EncodeTiledFn)p;
-  }
-  return fn;
-}
-
+// ---- launch plans (pure host code: also compiled when the kernel source is built for the CTA emulator) ------------
 // What one launch of bssn_tma_kernel<TX,TY,TZ,MODE,ORDER> issues, for the validator: every section's box and
 // operand loads with the mbarrier byte count the kernel announces for it (one "barrier" entry per section, one for
 // the point-value tiles).  xo: Layout::xo (decides the parity of the x coordinates).
@@ -1013,6 +996,54 @@ static TmaPlan bssn_plan(int mode, int xo) {
   p.expect.push_back((uint32_t)kCenVars * Cfg::TILE_BYTES);
   for (int grp = 0; grp < 3; ++grp) tile_load("point-value tiles", Cfg::cen_off(grp), 7, (int)p.expect.size() - 1);
   return p;
+}
+
+void plans_bssn_fused(std::vector<TmaPlan>& out) {
+  for (int mode = MODE_RHS; mode <= MODE_SSP; ++mode)
+    for (int g = 3; g <= 6; ++g) {   // every ghost width the layout rule gives a different xo for
+      const int xo = ((g - 3) & 1) ? g + 1 : g;
+      out.push_back(bssn_plan<16, 4, 4, 4>(mode, xo));
+      out.push_back(bssn_plan<16, 8, 2, 4>(mode, xo));
+      out.push_back(bssn_plan<8, 4, 8, 4>(mode, xo));
+      out.push_back(bssn_plan<16, 2, 8, 4>(mode, xo));
+      out.push_back(bssn_plan<16, 4, 2, 4>(mode, xo));
+      out.push_back(bssn_plan<16, 4, 4, 4, true>(mode, xo));   // ids 5 and 6 issue the same loads
+      out.push_back(bssn_plan<16, 4, 4, 4, true, true>(mode, xo));
+      if (g >= 5) out.push_back(bssn_plan<16, 4, 4, 8>(mode, xo));
+    }
+}
+
+// the plan of fused tile id `tile` at FD order `order` (the dispatch of tma_dispatch below); false: no such variant
+inline bool bssn_plan_for(int order, int tile, int mode, int xo, TmaPlan* out) {
+  if (order == 8) { if (tile != 0) return false; *out = bssn_plan<16, 4, 4, 8>(mode, xo); return true; }
+  switch (tile) {
+    case 0: *out = bssn_plan<16, 4, 4, 4>(mode, xo); return true;
+    case 1: *out = bssn_plan<16, 8, 2, 4>(mode, xo); return true;
+    case 2: *out = bssn_plan<8, 4, 8, 4>(mode, xo); return true;
+    case 3: *out = bssn_plan<16, 2, 8, 4>(mode, xo); return true;
+    case 4: *out = bssn_plan<16, 4, 2, 4>(mode, xo); return true;
+    case 5: case 6: *out = bssn_plan<16, 4, 4, 4, true>(mode, xo); return true;
+    case 7: *out = bssn_plan<16, 4, 4, 4, true, true>(mode, xo); return true;
+  }
+  return false;
+}
+
+#ifndef CHM_EMULATE
+// ---- host side: tensor map + launch -----------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  }
+  return fn;
 }
 
 template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL = false, bool EARLY = false, bool DEEP = false>
@@ -1104,21 +1135,6 @@ static cudaError_t tma_dispatch(int order, int tile, const Layout& L, const Coef
 cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s) {
   return tma_dispatch(order, tile, L, C, &st, s, nullptr);
 }
-void plans_bssn_fused(std::vector<TmaPlan>& out) {
-  for (int mode = MODE_RHS; mode <= MODE_SSP; ++mode)
-    for (int g = 3; g <= 6; ++g) {   // every ghost width the layout rule gives a different xo for
-      const int xo = ((g - 3) & 1) ? g + 1 : g;
-      out.push_back(bssn_plan<16, 4, 4, 4>(mode, xo));
-      out.push_back(bssn_plan<16, 8, 2, 4>(mode, xo));
-      out.push_back(bssn_plan<8, 4, 8, 4>(mode, xo));
-      out.push_back(bssn_plan<16, 2, 8, 4>(mode, xo));
-      out.push_back(bssn_plan<16, 4, 2, 4>(mode, xo));
-      out.push_back(bssn_plan<16, 4, 4, 4, true>(mode, xo));   // ids 5 and 6 issue the same loads
-      out.push_back(bssn_plan<16, 4, 4, 4, true, true>(mode, xo));
-      if (g >= 5) out.push_back(bssn_plan<16, 4, 4, 8>(mode, xo));
-    }
-}
-
 cudaError_t kernel_info_bssn_fused(int order, int tile, cudaFuncAttributes* a) {
   Layout L{}; Coef C{};
   return tma_dispatch(order, tile, L, C, nullptr, 0, a);

@@ -7,10 +7,10 @@
 // are prefetched into registers while the current plane is evaluated.  Slots are released warp by warp (mbarrier
 // whose returned state tells the last arriver, see bssn_tma.cuh); the last warp out issues the slot's next load.
 #include "bssn_tma.cuh"
+#include <cstdio>
+
 #include "stencils.cuh"
-#ifndef CHM_EMULATE
 #include "tma_check.cuh"
-#endif
 
 namespace chm {
 
@@ -163,23 +163,7 @@ wave_tma_kernel(const __grid_constant__ CUtensorMap tm, Layout L, Coef C, Stage 
   }
 }
 
-#ifndef CHM_EMULATE
-// ---- host side ------------------------------------------------------------------------------------------------
-typedef CUresult (*WvEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-static WvEncodeFn wv_encode_fn() {
-  static WvEncodeFn fn = nullptr;
-  if (!fn) {
-    void* p = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
-        qres == cudaDriverEntryPointSuccess)
-      fn = (WvEncodeFn)p;
-  }
-  return fn;
-}
-
+// ---- launch plans and layout test (pure host code: also compiled for the CTA emulator) ----------------------------
 // what one launch of wave_tma_kernel issues, for the validator: one plane box per ring slot
 template <int ORDER, bool KO, int TX, int TY, int NV>
 static TmaPlan wv_plan(int xo) {
@@ -197,6 +181,49 @@ static TmaPlan wv_plan(int xo) {
     p.loads.push_back({"plane box", (size_t)slot * K::SLOT * 8, {(uint32_t)K::ROW, (uint32_t)K::COLS, 1, (uint32_t)NV}, slot, (xo - K::R) & 1});
   }
   return p;
+}
+
+// true when the TMA form can serve this layout: plane-box rows must start on 16-byte boundaries
+bool wave_tma_ok(const Layout& L, int order, bool ko) {
+  const int r0 = order / 2, r = (ko && r0 < 3) ? 3 : r0;
+  return ((L.xo - r) % 2) == 0 && L.g >= r;
+}
+
+template <int ORDER, bool KO>
+static void wv_plans_of(std::vector<TmaPlan>& out, int xo) {
+  out.push_back(wv_plan<ORDER, KO, 32, 16, 2>(xo));
+  out.push_back(wv_plan<ORDER, KO, 64, 8, 2>(xo));
+  if (wv::Cfg<ORDER, KO, 16, 8, 5>::FITS) out.push_back(wv_plan<ORDER, KO, 16, 8, 5>(xo));
+  if (wv::Cfg<ORDER, KO, 16, 16, 5>::FITS) out.push_back(wv_plan<ORDER, KO, 16, 16, 5>(xo));
+  if (wv::Cfg<ORDER, KO, 32, 8, 5>::FITS) out.push_back(wv_plan<ORDER, KO, 32, 8, 5>(xo));
+}
+// every instance, on every ghost width wave_tma_ok admits (xo = g for the wave systems)
+void plans_wave_tma(std::vector<TmaPlan>& out) {
+  for (int g = 2; g <= 6; ++g) {
+    Layout L{};
+    L.xo = g; L.g = g;
+    if (wave_tma_ok(L, 4, false)) wv_plans_of<4, false>(out, g);
+    if (wave_tma_ok(L, 4, true)) wv_plans_of<4, true>(out, g);
+    if (wave_tma_ok(L, 8, false)) wv_plans_of<8, false>(out, g);
+    if (wave_tma_ok(L, 8, true)) wv_plans_of<8, true>(out, g);
+  }
+}
+
+#ifndef CHM_EMULATE
+// ---- host side ------------------------------------------------------------------------------------------------
+typedef CUresult (*WvEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static WvEncodeFn wv_encode_fn() {
+  static WvEncodeFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = (WvEncodeFn)p;
+  }
+  return fn;
 }
 
 template <int ORDER, bool KO, int TX, int TY, int ZC, int NV = 2>
@@ -282,37 +309,11 @@ cudaError_t kernel_info_wave1_tma(int order, int which, cudaFuncAttributes* a) {
   return wv1_dispatch(order, true, which, L, C, nullptr, 0, a);
 }
 
-// true when the TMA form can serve this layout: plane-box rows must start on 16-byte boundaries
-bool wave_tma_ok(const Layout& L, int order, bool ko) {
-  const int r0 = order / 2, r = (ko && r0 < 3) ? 3 : r0;
-  return ((L.xo - r) % 2) == 0 && L.g >= r;
-}
-
 static cudaError_t wv_dispatch(int order, bool ko, int which, const Layout& L, const Coef& C, const Stage* st,
                                cudaStream_t s, cudaFuncAttributes* a) {
   if (order == 4) return ko ? wv_tile<4, true>(which, L, C, st, s, a) : wv_tile<4, false>(which, L, C, st, s, a);
   if (order == 8) return ko ? wv_tile<8, true>(which, L, C, st, s, a) : wv_tile<8, false>(which, L, C, st, s, a);
   return cudaErrorInvalidValue;
-}
-
-template <int ORDER, bool KO>
-static void wv_plans_of(std::vector<TmaPlan>& out, int xo) {
-  out.push_back(wv_plan<ORDER, KO, 32, 16, 2>(xo));
-  out.push_back(wv_plan<ORDER, KO, 64, 8, 2>(xo));
-  if (wv::Cfg<ORDER, KO, 16, 8, 5>::FITS) out.push_back(wv_plan<ORDER, KO, 16, 8, 5>(xo));
-  if (wv::Cfg<ORDER, KO, 16, 16, 5>::FITS) out.push_back(wv_plan<ORDER, KO, 16, 16, 5>(xo));
-  if (wv::Cfg<ORDER, KO, 32, 8, 5>::FITS) out.push_back(wv_plan<ORDER, KO, 32, 8, 5>(xo));
-}
-// every instance, on every ghost width wave_tma_ok admits (xo = g for the wave systems)
-void plans_wave_tma(std::vector<TmaPlan>& out) {
-  for (int g = 2; g <= 6; ++g) {
-    Layout L{};
-    L.xo = g; L.g = g;
-    if (wave_tma_ok(L, 4, false)) wv_plans_of<4, false>(out, g);
-    if (wave_tma_ok(L, 4, true)) wv_plans_of<4, true>(out, g);
-    if (wave_tma_ok(L, 8, false)) wv_plans_of<8, false>(out, g);
-    if (wave_tma_ok(L, 8, true)) wv_plans_of<8, true>(out, g);
-  }
 }
 
 cudaError_t launch_wave_tma(const Layout& L, const Coef& C, int order, int which, const Stage& st, cudaStream_t s) {

@@ -22,14 +22,15 @@ def oracle():
 _EMU = {}
 
 
-def build_emulator(name):
-    """g++ -DCHM_EMULATE build of tests/native/<name>.cpp (a kernel source on top of cta_emu.hpp), once per session"""
+def build_emulator(name, shared=False):
+    """g++ -DCHM_EMULATE build of tests/native/<name>.cpp (a kernel source on top of cta_emu.hpp), once per session;
+    shared=True: as a shared library"""
     import subprocess
     import tempfile
     if name not in _EMU:
         d = tempfile.mkdtemp(prefix="chm_emu_")
-        exe = os.path.join(d, name)
-        subprocess.run(["g++", "-std=c++17", "-O1", "-DCHM_EMULATE", "-pthread", "-o", exe,
+        exe = os.path.join(d, name + (".so" if shared else ""))
+        subprocess.run(["g++", "-std=c++17", "-O1", "-DCHM_EMULATE", "-pthread"] + (["-shared", "-fPIC"] if shared else []) + ["-o", exe,
                         os.path.join(ROOT, "tests", "native", name + ".cpp")], check=True, capture_output=True)
         _EMU[name] = exe
     return _EMU[name]

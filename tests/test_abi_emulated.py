@@ -1,0 +1,186 @@
+"""The library's real C ABI on a box without a GPU: csrc/chemora.cu itself (handle, layout, stage plans, the runtime
+sweep with its agreement guard and col_rows sweep, the timing event pool, ghosted state copies, the radiative step
+order, the device error word) compiled with g++ on top of the emulated kernels and a stub of the few CUDA runtime
+calls it makes (tests/native/libchemora_emu.cpp), driven through the normal Python binding by (a) the same test
+FUNCTIONS that run on the GPU (tests/test_gpu_a_parity.py, tests/test_gpu_zz_round2.py), called with the emulated
+library behind `chem`, and (b) small clones of the heavy ones.
+
+Why: GPU access was closed for all of round 2, and that host code -- which sits on bench.py's default path -- had
+never executed.  This is test infrastructure: the package never loads the emulated library (no CPU fallback exists:
+tests/test_abi.py::test_no_cpu_fallback), and the -m gpu tests remain the proof on the device."""
+import ctypes
+import types
+
+import numpy as np
+import pytest
+
+from paper_1307_6488_b200 import inputs
+
+
+@pytest.fixture(scope="module")
+def chem():
+    import torch
+    from paper_1307_6488_b200 import binding
+    from tests.conftest import build_emulator
+    lib = build_emulator("libchemora_emu", shared=True)
+    saved = (binding.LIB_PATH, binding._lib, torch.cuda.is_available)
+    binding.LIB_PATH, binding._lib = lib, None
+    torch.cuda.is_available = lambda: False          # the binding must use host memory here, on a GPU box too
+    binding.load()
+
+    class EmuChemora(binding.Chemora):
+        """host tensors standing in for device tensors: 128-byte aligned like CUDA allocations (torch's CPU
+        allocator gives 64), and a view of the library's own buffers without the torch allocator callbacks"""
+
+        def new_state(self):
+            n = self.nvars * self.tot_z * self.tot_y * self.pitch
+            raw = torch.zeros(n + 16, dtype=torch.float64)
+            off = ((-raw.data_ptr()) % 128) // 8
+            return raw[off:off + n].view(self.nvars, self.tot_z, self.tot_y, self.pitch)
+
+        def state_view(self, which=0):
+            n = self.nvars * self.var_stride
+            a = np.ctypeslib.as_array((ctypes.c_double * n).from_address(self.state_ptr(which)))
+            return torch.from_numpy(a).view(self.nvars, self.tot_z, self.tot_y, self.pitch)
+
+    ns = types.SimpleNamespace(**{k: getattr(binding, k) for k in dir(binding) if not k.startswith("__")})
+    ns.Chemora = EmuChemora
+    yield ns
+    binding.LIB_PATH, binding._lib, torch.cuda.is_available = saved
+
+
+def relerr(a, b):
+    return max(np.max(np.abs(a[v] - b[v])) / max(np.max(np.abs(b[v])), 1e-300) for v in range(a.shape[0]))
+
+
+def test_gpu_test_functions_against_the_emulated_library(chem, oracle):
+    """the cheap ones of the -m gpu tests, as they are (the Energy kernel, one 256-thread CTA per grid row and slow
+    under emulation, has its own emulated test in tests/test_basic_kernels_emulated.py)"""
+    from tests import test_gpu_a_parity as A
+    from tests import test_gpu_zz_round2 as Z
+    A.test_fill_ghosts_bit_exact(chem, oracle, (16, 16, 16), 2, 0)
+    A.test_fill_ghosts_bit_exact(chem, oracle, (9, 6, 7), 4, 1)
+    A.test_set_get_state_roundtrip(chem)
+    A.test_bssn_even_ghost_width(chem, oracle)
+    A.test_enforce_constraints(chem, oracle)
+    A.test_rk3_wave_systems(chem, oracle, 2, 4, 3, 5)
+    Z.test_radiative_rhs_at_boundary_points(chem, oracle, 1, 4, 3, (21, 12, 10))
+    Z.test_radiative_rhs_at_boundary_points(chem, oracle, 0, 8, 4, (37, 9, 12))
+    Z.test_radiative_rk4_whole_block(chem, oracle, 0, 4, 2, 10, 1e-11)
+
+
+def test_z_linked_blocks_through_the_step_group_calls(chem, oracle):
+    """chemora_link_z / chemora_rk4_step_group on the wave system (L1 kernels: cheap under emulation)"""
+    from tests import test_gpu_a_parity as A
+    A.test_z_linked_blocks_equal_the_single_block(chem, oracle, 0, 8, 4, False)
+
+
+@pytest.mark.parametrize("fused,tile", [(1, 0), (1, 3), (1, 5), (1, 7), (0, 1)])
+def test_bssn_steps_through_the_abi(chem, oracle, fused, tile):
+    """chemora_rk4_step, then chemora_rk3_step + chemora_enforce_constraints, on 16 x 8 x 8: the stage plans, the
+    buffer rotation and the fills as the library issues them, both norms of DESIGN.md S11 / S11b"""
+    from tests.test_gpu_a_parity import assert_bssn_close
+    nx, ny, nz, g, dx, eps = 16, 8, 8, 3, 0.05, 0.1
+    dt = 0.25 * dx
+    u0 = inputs.bssn_gaussians(nx, ny, nz, width_cells=3.0) + 1e-10 * np.random.default_rng(2).uniform(-1, 1, size=(25, nz, ny, nx))
+    h = chem.Chemora(nx, ny, nz, g, 4, chem.SYS_BSSN, dx)
+    h.set_param("eps_diss", eps)
+    h.set_variant(fused, tile)
+    h.set_state(u0)
+    l0 = h.launch_count()
+    for _ in range(2):
+        h.rk4_step(dt)
+    assert h.launch_count() - l0 == 2 * (8 if fused else 12)          # 4 fills + 4 (split: 8) kernels per step
+    want = oracle.interior(oracle.rk4(1, oracle.with_ghosts(u0, g), g, 4, dx, dt, oracle.params(eps_diss=eps), 2), g)
+    assert_bssn_close(h.get_state(), want, 1e-12)
+    h.set_state(u0)
+    for _ in range(2):
+        h.rk3_step(dt)
+        h.enforce_constraints()
+    want = oracle.interior(oracle.rk3(1, oracle.with_ghosts(u0, g), g, 4, dx, dt, oracle.params(eps_diss=eps), 2, True), g)
+    assert_bssn_close(h.get_state(), want, 1e-12)
+    assert h.lib.chemora_synchronize(h._h) == 0
+    h.destroy()
+
+
+def test_radiative_bssn_step_through_the_abi(chem, oracle):
+    """CHEMORA_BC_RADIATIVE: no fill, interior kernel then face kernel per stage; whole padded block vs the oracle"""
+    from tests.test_gpu_a_parity import assert_bssn_close
+    nx, ny, nz, g, dx = 16, 8, 8, 3, 0.05
+    dt = 0.25 * dx
+    st = oracle.fill_ghosts(oracle.with_ghosts(inputs.bssn_noise(nx, ny, nz), g), g)
+    st += 1e-10 * np.random.default_rng(52).uniform(-1, 1, size=st.shape)
+    h = chem.Chemora(nx, ny, nz, g, 4, chem.SYS_BSSN, dx)
+    h.set_param("eps_diss", 0.1)
+    h.set_boundary(chem.BC_RADIATIVE)
+    h.set_state_ghosted(st)
+    l0 = h.launch_count()
+    for _ in range(2):
+        h.rk4_step(dt)
+    assert h.launch_count() - l0 == 16
+    want = oracle.rk4_radiative(1, st.copy(), g, 4, dx, dt, oracle.params(eps_diss=0.1), 2)
+    assert_bssn_close(h.get_state_ghosted(), want, 1e-10)
+    h.destroy()
+
+
+def test_runtime_sweep_guard_and_col_rows(chem, monkeypatch):
+    """chemora_autotune as bench.py calls it: every fused id timed and eligible, the split variant only on request,
+    U untouched, the pick in force.  Then with two faults injected into the emulated launcher: a variant that computes
+    something else is disqualified (-2), one whose bounded wait gave up is disqualified (-3) and the error word is
+    cleared; neither is the pick.  (Which variant is FASTEST under emulation means nothing and is not asserted.)"""
+    nx, ny, nz = 16, 4, 4
+    h = chem.Chemora(nx, ny, nz, 3, 4, chem.SYS_BSSN, 0.05)
+    h.set_param("eps_diss", 0.1)
+    u = inputs.bssn_minkowski(nx, ny, nz) + 0.05 * np.random.default_rng(3).uniform(-1, 1, size=(25, nz, ny, nx))
+    h.set_state(u)
+    nt = chem.NUM_TILES
+    ids = chem.variants(chem.SYS_BSSN, 4)
+    fused, tile, ms = h.autotune()
+    assert fused == 1 and tile in ids and (fused, tile) == h.get_variant()
+    assert all(ms[nt + t] > 0 for t in ids) and all(ms[nt + t] == -1.0 for t in range(nt) if t not in ids)
+    assert all(m == -1.0 for m in ms[:nt])                             # split variant: only on request
+    assert h.get_param("col_rows") in (16.0, 32.0, 64.0)
+    assert np.array_equal(h.get_state(), u)
+    monkeypatch.setenv("CHM_EMU_BREAK_TILE", "5")
+    monkeypatch.setenv("CHM_EMU_TIMEOUT_TILE", "3")
+    h.set_param("autotune_split", 1)
+    fused, tile, ms = h.autotune()
+    assert ms[nt + 5] == -2.0 and ms[nt + 3] == -3.0 and (fused, tile) not in ((1, 5), (1, 3))
+    assert all(ms[nt + t] > 0 for t in ids if t not in (3, 5)) and all(m > 0 for m in ms[:6])
+    assert (fused, tile) == h.get_variant() and np.array_equal(h.get_state(), u)
+    monkeypatch.delenv("CHM_EMU_BREAK_TILE")
+    monkeypatch.delenv("CHM_EMU_TIMEOUT_TILE")
+    assert h.lib.chemora_synchronize(h._h) == 0                        # the sweep cleared the word
+    h.destroy()
+
+
+def test_device_error_word_reaches_the_caller(chem, monkeypatch):
+    """a wait that gave up inside a kernel: chemora_synchronize / chemora_get_state return CHEMORA_ECUDA, the message
+    names the section, and the word is cleared for the next call"""
+    h = chem.Chemora(16, 8, 8, 3, 4, chem.SYS_BSSN, 0.05)
+    h.set_variant(1, 0)
+    h.set_state(inputs.bssn_minkowski(16, 8, 8))
+    monkeypatch.setenv("CHM_EMU_TIMEOUT_TILE", "0")
+    h.rk4_step(0.0125)
+    monkeypatch.delenv("CHM_EMU_TIMEOUT_TILE")
+    with pytest.raises(chem.ChemoraError) as e:
+        h.get_state()
+    assert e.value.code == chem.ECUDA and "section 12" in str(e.value)
+    h.get_state()                                                       # cleared
+    h.destroy()
+
+
+def test_timing_pool_wraps_without_losing_launches(chem):
+    """chemora_timing: more timed launches than the pool holds event pairs (256 per category)"""
+    n = 8
+    h = chem.Chemora(n, n, n, 2, 4, chem.SYS_WAVE, 1.0 / n)
+    h.set_variant(1, 0)
+    h.set_state(np.random.default_rng(1).standard_normal((2, n, n, n)))
+    h.timing(1)
+    for _ in range(70):
+        h.rk4_step(0.01)
+    t = h.timing_read()
+    assert t["rhs_launches"] == 280 and t["fill_launches"] == 280 and t["rhs_ms"] > 0 and t["fill_ms"] > 0
+    h.timing(0)
+    assert h.timing_read()["rhs_launches"] == 0
+    h.destroy()
