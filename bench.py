@@ -323,6 +323,31 @@ def run_sweep(args):
                       "tile_cost_model": picks}))
 
 
+def run_fill_floor(args):
+    """DESIGN.md 6.5's box-fill floor through the library (chemora_measure_box_fill): for every fused 4th-order BSSN
+    tile id at the headline size, ms of a fill-only launch (all TMA traffic of a middle RK4 stage, no arithmetic, no
+    stores) next to ms of the full middle-stage launch as the runtime sweep times it."""
+    import torch
+    from paper_1307_6488_b200 import binding, inputs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device and no CPU fallback")
+    n = args.size
+    h = binding.Chemora(n, n, n, 3, 4, binding.SYS_BSSN, 0.05)
+    h.set_param("eps_diss", 0.1)
+    h.set_state(inputs.bssn_gaussians(n, n, n))
+    _, _, ms = h.autotune()
+    rows = []
+    for t in binding.variants(binding.SYS_BSSN, 4):
+        fill_ms = h.measure_box_fill(t)
+        full_ms = ms[binding.NUM_TILES + t]
+        rows.append({"tile_id": t, "tile": list(binding.tile_shape(t, binding.SYS_BSSN, 1)), "fill_only_ms": fill_ms,
+                     "full_mid_stage_ms": full_ms if full_ms > 0 else None,
+                     "fill_share": fill_ms / full_ms if full_ms > 0 else None})
+    h.destroy()
+    print(json.dumps({"metric": "fused BSSN kernel: fill-only vs full middle-stage launch, %d^3" % n, "unit": "ms per launch",
+                      "rows": rows}))
+
+
 def run_wave(args):
     """configs[1]: wave (phi, pi) 256^3, O8 + KO eps=0.1, 8 plane waves; RK4 steps; HBM roofline at 272 B per update."""
     import torch
@@ -414,6 +439,7 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=128)
     ap.add_argument("--ref-sample", type=int, default=64)
     ap.add_argument("--sweep", action="store_true", help="configs[4] variant/tile sweep instead of the headline run")
+    ap.add_argument("--fill-floor", action="store_true", help="fill-only vs full launch per fused id (DESIGN.md 6.5)")
     ap.add_argument("--wave", action="store_true", help="configs[1]: the (phi, pi) wave system at 256^3, O8 + KO")
     ap.add_argument("--wave1", action="store_true", help="the paper's Sample-1 wave system (u, rho, v_i) at 256^3, O8 + KO")
     ap.add_argument("--paper-shape", action="store_true", help="BSSN O8 + RK3 at 100^3 (the paper's own benchmark shape)")
@@ -421,6 +447,8 @@ def main():
     args = ap.parse_args()
     if args.sweep:
         run_sweep(args)
+    elif args.fill_floor:
+        run_fill_floor(args)
     elif args.wave or args.wave1:
         run_wave(args)
     elif args.paper_shape:

@@ -230,6 +230,14 @@ int chemora_autotune(chemora_t* h, int* fused, int* tile_id, float* ms_out);
 int chemora_selfcheck(char* buf, size_t n);
 int chemora_describe_device_error(unsigned code, char* buf, size_t n);
 
+/* Benchmark mode: the cost of moving one launch's data into shared memory.  Runs the fused 4th-order BSSN kernel of
+ * tile_id in FILL-ONLY mode on the current U: every TMA box, Runge-Kutta operand tile and point-value tile of a middle
+ * RK4 stage is requested, awaited, released and refilled by the code the full kernel uses (same launch plan, same
+ * validator), and no arithmetic is done and nothing is written.  *ms = median of three launches after a warm-up.
+ * This is the tracked form of the stand-alone probe behind DESIGN.md section 6.5's box-fill floor.  Fills U's ghosts;
+ * S and YA are not modified.  CHEMORA_EINVAL for other systems / orders / ids.  Synchronous. */
+int chemora_measure_box_fill(chemora_t* h, int tile_id, float* ms);
+
 /* Number of kernel launches issued through this handle so far (for benchmarks' gpu_launches). */
 long chemora_launch_count(const chemora_t* h);
 

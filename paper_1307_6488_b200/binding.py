@@ -27,7 +27,7 @@ SYMBOLS = ["chemora_create", "chemora_set_param", "chemora_get_param", "chemora_
            "chemora_rk4_step_group", "chemora_rk3_step_group", "chemora_set_boundary", "chemora_get_boundary", "chemora_radiative_rhs",
            "chemora_set_state_ghosted", "chemora_get_state_ghosted", "chemora_enforce_constraints", "chemora_energy", "chemora_set_variant",
            "chemora_get_variant", "chemora_variant_available", "chemora_selfcheck", "chemora_describe_device_error", "chemora_tile_shape", "chemora_tile_cost", "chemora_autotune", "chemora_launch_count",
-           "chemora_kernel_info", "chemora_timing", "chemora_timing_read", "chemora_measure_fp64_peak", "chemora_last_error", "chemora_destroy"]
+           "chemora_kernel_info", "chemora_measure_box_fill", "chemora_timing", "chemora_timing_read", "chemora_measure_fp64_peak", "chemora_last_error", "chemora_destroy"]
 
 _ALLOC_T = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
 _DEALLOC_T = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p)
@@ -80,6 +80,7 @@ def load():
         "chemora_launch_count": [vp],
         "chemora_kernel_info": [vp, ip, ip, ip],
         "chemora_measure_fp64_peak": [vp, dp],
+        "chemora_measure_box_fill": [vp, i, ctypes.POINTER(ctypes.c_float)],
         "chemora_timing": [vp, i], "chemora_timing_read": [vp, dp, lp, dp, lp],
         "chemora_last_error": [vp], "chemora_destroy": [vp],
     }
@@ -363,6 +364,12 @@ class Chemora:
         a, b, c, d = ctypes.c_double(), ctypes.c_long(), ctypes.c_double(), ctypes.c_long()
         self._ck(self.lib.chemora_timing_read(self._h, a, b, c, d))
         return dict(rhs_ms=a.value, rhs_launches=b.value, fill_ms=c.value, fill_launches=d.value)
+
+    def measure_box_fill(self, tile_id):
+        """ms of one fill-only launch of fused tile id `tile_id` (chemora_measure_box_fill)"""
+        ms = ctypes.c_float()
+        self._ck(self.lib.chemora_measure_box_fill(self._h, int(tile_id), ctypes.byref(ms)))
+        return ms.value
 
     def measure_fp64_peak(self):
         v = ctypes.c_double()

@@ -774,6 +774,40 @@ int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out)
   return rc;
 }
 
+int chemora_measure_box_fill(chemora_t* h, int tile_id, float* ms) {
+  if (!h || !ms) return CHEMORA_EINVAL;
+  if (h->system != CHEMORA_SYS_BSSN || h->order != 4 || !chemora_variant_available(h->system, h->order, 1, tile_id))
+    return fail(h, CHEMORA_EINVAL, "the fill-only mode exists for the fused 4th-order BSSN tile ids");
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  for (int n = 0; n < 4; ++n)
+    if (cudaEventCreate(&ev[n]) != cudaSuccess) {
+      for (int m = 0; m < n; ++m) cudaEventDestroy(ev[m]);
+      return cuda_fail(h, cudaGetLastError(), "event create");
+    }
+  int rc = fill(h, h->buf[0]);
+  // what a middle RK4 stage loads: boxes of U, operand tiles of U and S; nothing is written
+  Stage st{h->buf[0], h->buf[0], h->buf[3], h->buf[1], 1e-3, MODE_MID};
+  const Coef C = make_coef(h);
+  cudaError_t e = rc ? cudaSuccess : launch_bssn_fill(h->L, C, tile_id, st, h->stream);   // warm-up
+  for (int n = 0; n < 3 && !rc && e == cudaSuccess; ++n) {
+    cudaEventRecord(ev[n], h->stream);
+    e = launch_bssn_fill(h->L, C, tile_id, st, h->stream);
+  }
+  if (!rc && e != cudaSuccess) rc = cuda_fail(h, e, "fill-only kernel launch");
+  if (!rc) {
+    h->launches += 4;
+    cudaEventRecord(ev[3], h->stream);
+    if (cudaEventSynchronize(ev[3]) != cudaSuccess) rc = cuda_fail(h, cudaGetLastError(), "fill-only sync");
+  }
+  if (!rc) {
+    float m[3];
+    for (int n = 0; n < 3; ++n) cudaEventElapsedTime(&m[n], ev[n], ev[n + 1]);
+    *ms = m[0] + m[1] + m[2] - fminf(m[0], fminf(m[1], m[2])) - fmaxf(m[0], fmaxf(m[1], m[2]));
+  }
+  for (int n = 0; n < 4; ++n) cudaEventDestroy(ev[n]);
+  return rc ? rc : chemora_synchronize(h);
+}
+
 long chemora_launch_count(const chemora_t* h) { return h ? h->launches : 0; }
 
 static void drop_events(chemora_t* h) {

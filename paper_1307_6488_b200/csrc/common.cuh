@@ -169,6 +169,7 @@ bool wave1_tma_ok(const Layout& L, int order, bool ko, int which);
 cudaError_t launch_wave1(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
 cudaError_t kernel_info_wave1(int order, int tile, cudaFuncAttributes* a);
 cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s);
+cudaError_t launch_bssn_fill(const Layout& L, const Coef& C, int tile, const Stage& st, cudaStream_t s);   // fill-only mode
 cudaError_t launch_bssn_derivs(const Layout& L, const Coef& C, int order, int tile, const double* in, double* derivs,
                                cudaStream_t s);
 cudaError_t launch_bssn_from_derivs(const Layout& L, const Coef& C, int tile, const double* derivs,

@@ -119,7 +119,8 @@ struct TmaCfg {
 // EARLY: a full variable's own right-hand side (which needs none of its mixed derivatives) leaves BEFORE the plane
 // barrier of the two-pass mixed derivatives instead of after it, so the time a warp would spend waiting for its
 // plane partner is spent on the operand reads, the stage update and the stores (capture L: 4 % of stall samples)
-template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL, bool EARLY = false, bool DEEP = false>
+// FILL: fill-only mode, see the branch at the top of the tile loop and chemora_measure_box_fill
+template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL, bool EARLY = false, bool DEEP = false, bool FILL = false>
 __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUtensorMap& tmCen, const CUtensorMap& tmU,
                                               const CUtensorMap& tmS, const CUtensorMap& tmU4, const CUtensorMap& tmS4,
                                               const CUtensorMap& tmU3, const CUtensorMap& tmS3, const Layout& L,
@@ -458,6 +459,27 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
 
     const double third = 1.0 / 3.0, two_thirds = 2.0 / 3.0;
     mbar_wait(cfull, (uint32_t)(t & 1), L.err, 0x10080u);
+    if constexpr (FILL) {
+      // Fill-only mode (chemora_measure_box_fill): the whole TMA protocol of a launch -- every box, operand tile and
+      // point-value tile requested, awaited, released and refilled by the code the full kernel uses -- and no
+      // arithmetic: a thread reads its own point of every box.  What remains is the cost of moving the data into
+      // shared memory, the "third floor" of DESIGN.md section 6.5, measured through the validated launch path.
+      double acc = cen(V_CHI);
+      done_cen();
+#pragma unroll
+      for (int o = 0; o < NSEC; ++o) {
+        if (IL && o >= SecIL::emit0) {
+          wait_sec(o);
+          if (nops != 0 && o < SecIL::emit0 + 3) acc += pre_e(o, 0).u;
+        } else {
+          const auto p = box(o);
+          acc += p.at(0, 0, 0);
+        }
+        done(o);
+      }
+      if (acc == 1.2345678e300 && valid) st.S[q] = acc;   // never true: keeps the reads alive
+      continue;
+    }
     // ---- point values needed before their own boxes arrive: metric, shift ----------------------------------
     double g[6], gu[6];
 #pragma unroll
@@ -946,6 +968,17 @@ bssn_tma_il_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant
   bssn_tma_body<TX, TY, TZ, MODE, 4, true, EARLY, DEEP>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C, st, ntx, nty, ntz, cy);
 }
 
+// fill-only mode of either layout (chemora_measure_box_fill): same arguments, same launch plan, no arithmetic
+template <int TX, int TY, int TZ, int MODE, bool IL, bool DEEP>
+__global__ void __launch_bounds__(TX* TY* TZ, 1)
+bssn_fill_kernel(const __grid_constant__ CUtensorMap tm, const __grid_constant__ CUtensorMap tmCen,
+                 const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmS,
+                 const __grid_constant__ CUtensorMap tmU4, const __grid_constant__ CUtensorMap tmS4,
+                 const __grid_constant__ CUtensorMap tmU3, const __grid_constant__ CUtensorMap tmS3, Layout L, Coef C,
+                 Stage st, int ntx, int nty, int ntz, int cy) {
+  bssn_tma_body<TX, TY, TZ, MODE, 4, IL, false, DEEP, true>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C, st, ntx, nty, ntz, cy);
+}
+
 // ---- launch plans (pure host code: also compiled when the kernel source is built for the CTA emulator) ------------
 // What one launch of bssn_tma_kernel<TX,TY,TZ,MODE,ORDER> issues, for the validator: every section's box and
 // operand loads with the mbarrier byte count the kernel announces for it (one "barrier" entry per section, one for
@@ -1046,11 +1079,12 @@ static EncodeTiledFn encode_fn() {
   return fn;
 }
 
-template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL = false, bool EARLY = false, bool DEEP = false>
+template <int TX, int TY, int TZ, int MODE, int ORDER, bool IL = false, bool EARLY = false, bool DEEP = false, bool FILL = false>
 static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, cudaStream_t s, cudaFuncAttributes* a) {
   using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL, DEEP>;
   const void* kern;
-  if constexpr (IL) kern = (const void*)bssn_tma_il_kernel<TX, TY, TZ, MODE, EARLY, DEEP>;
+  if constexpr (FILL) kern = (const void*)bssn_fill_kernel<TX, TY, TZ, MODE, IL, DEEP>;
+  else if constexpr (IL) kern = (const void*)bssn_tma_il_kernel<TX, TY, TZ, MODE, EARLY, DEEP>;
   else kern = (const void*)bssn_tma_kernel<TX, TY, TZ, MODE, ORDER>;
   if (a) return cudaFuncGetAttributes(a, kern);
   // nothing is launched unless the validator accepts what this instance will issue on this layout
@@ -1080,7 +1114,7 @@ static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, 
   if (tile_map(&tmCen, st->in, 7) != CUDA_SUCCESS || tile_map(&tmU, ubase, 1) != CUDA_SUCCESS ||
       tile_map(&tmS, sbase, 1) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
-  if (IL && (tile_map(&tmU4, ubase, 4) != CUDA_SUCCESS || tile_map(&tmS4, sbase, 4) != CUDA_SUCCESS ||
+  if ((IL || FILL) && (tile_map(&tmU4, ubase, 4) != CUDA_SUCCESS || tile_map(&tmS4, sbase, 4) != CUDA_SUCCESS ||
              tile_map(&tmU3, ubase, 3) != CUDA_SUCCESS || tile_map(&tmS3, sbase, 3) != CUDA_SUCCESS))
     return cudaErrorInvalidValue;
   // per launch: function attributes are per device, and the call is cheap
@@ -1096,7 +1130,10 @@ static cudaError_t tma_go_mode(const Layout& L, const Coef& C, const Stage* st, 
   if (blocks_per_sm < 1) blocks_per_sm = 1;
   const int grid = ntiles < sms * blocks_per_sm ? ntiles : sms * blocks_per_sm;
   const int cy = L.col_rows / TY > 0 ? L.col_rows / TY : 1;   // tile rows per traversal column
-  if constexpr (IL)
+  if constexpr (FILL)
+    bssn_fill_kernel<TX, TY, TZ, MODE, IL, DEEP><<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C,
+                                                                                 *st, ntx, nty, ntz, cy);
+  else if constexpr (IL)
     bssn_tma_il_kernel<TX, TY, TZ, MODE, EARLY, DEEP><<<grid, Cfg::THREADS, Cfg::SMEM, s>>>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C,
                                                                                 *st, ntx, nty, ntz, cy);
   else
@@ -1134,6 +1171,20 @@ static cudaError_t tma_dispatch(int order, int tile, const Layout& L, const Coef
 
 cudaError_t launch_bssn_fused(const Layout& L, const Coef& C, int order, int tile, const Stage& st, cudaStream_t s) {
   return tma_dispatch(order, tile, L, C, &st, s, nullptr);
+}
+// fill-only mode of a middle Runge-Kutta stage, 4th order (id 6 moves what id 5 moves)
+cudaError_t launch_bssn_fill(const Layout& L, const Coef& C, int tile, const Stage& st, cudaStream_t s) {
+  if (st.mode != MODE_MID) return cudaErrorInvalidValue;
+  switch (tile) {
+    case 0: return tma_go_mode<16, 4, 4, MODE_MID, 4, false, false, false, true>(L, C, &st, s, nullptr);
+    case 1: return tma_go_mode<16, 8, 2, MODE_MID, 4, false, false, false, true>(L, C, &st, s, nullptr);
+    case 2: return tma_go_mode<8, 4, 8, MODE_MID, 4, false, false, false, true>(L, C, &st, s, nullptr);
+    case 3: return tma_go_mode<16, 2, 8, MODE_MID, 4, false, false, false, true>(L, C, &st, s, nullptr);
+    case 4: return tma_go_mode<16, 4, 2, MODE_MID, 4, false, false, false, true>(L, C, &st, s, nullptr);
+    case 5: case 6: return tma_go_mode<16, 4, 4, MODE_MID, 4, true, false, false, true>(L, C, &st, s, nullptr);
+    case 7: return tma_go_mode<16, 4, 4, MODE_MID, 4, true, false, true, true>(L, C, &st, s, nullptr);
+  }
+  return cudaErrorInvalidValue;
 }
 cudaError_t kernel_info_bssn_fused(int order, int tile, cudaFuncAttributes* a) {
   Layout L{}; Coef C{};

@@ -3,6 +3,7 @@
 // warp-wise slot release and refill, the two-pass mixed derivatives with their plane barriers, the Runge-Kutta
 // epilogues -- everything but the hardware.  Test infrastructure only (tests/test_fused_kernel_emulated.py).
 //
+//   (mode 12 = the fill-only kernel of a middle stage)
 //   fused_emu <order> <tile> <mode> <nx> <ny> <nz> <g> <h> <eps> <eta> <sgc> <ko_order> <a> <ca> <cb> <grid>
 //             <in.bin> <U.bin> <S.bin> <out.bin>
 // in/U/S.bin: ghosted arrays [25][nz+2g][ny+2g][nx+2g] (ghosts of `in` filled); out.bin: three such arrays in a row:
@@ -44,7 +45,8 @@ static void from_padded(const Layout& L, const double* p, std::vector<double>& g
                &p[(size_t)v * L.vstride + (size_t)k * L.plane + (size_t)j * L.pitch + (L.xo - L.g)], tx * 8);
 }
 
-template <int TX, int TY, int TZ, int MODE, int ORDER, int IL = 0>
+// IL: 0 plain layout, 1 interleaved, 2 + early emission, 3 + six-slot ring; FILL: the fill-only kernel
+template <int TX, int TY, int TZ, int MODE, int ORDER, int IL = 0, bool FILL = false>
 static chm_emu::Stats run(const Layout& L, const Coef& C, const Stage& st, int grid_req) {
   using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL != 0, IL == 3>;
   auto map = [&](const double* base, uint32_t bx, uint32_t by, uint32_t bz, uint32_t bv) {
@@ -63,7 +65,13 @@ static chm_emu::Stats run(const Layout& L, const Coef& C, const Stage& st, int g
   const int ntx = (L.nx + TX - 1) / TX, nty = (L.ny + TY - 1) / TY, ntz = (L.nz + TZ - 1) / TZ;
   const int ntiles = ntx * nty * ntz, grid = ntiles < grid_req ? ntiles : grid_req;
   const int cy = L.col_rows / TY > 0 ? L.col_rows / TY : 1;
-  if constexpr (IL != 0) {   // the interleaved layout's operand maps: 4 and 3 consecutive variables a box
+  if constexpr (FILL && ORDER == 4) {
+    const CUtensorMap tmU4 = map(ubase, TX + 2, TY, TZ, 4), tmS4 = map(sbase, TX + 2, TY, TZ, 4),
+                      tmU3 = map(ubase, TX + 2, TY, TZ, 3), tmS3 = map(sbase, TX + 2, TY, TZ, 3);
+    return chm_emu::run_grid(grid, Cfg::THREADS, 1, Cfg::SMEM, [&] {
+      bssn_fill_kernel<TX, TY, TZ, MODE, IL != 0, IL == 3>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C, st, ntx, nty, ntz, cy);
+    });
+  } else if constexpr (IL != 0) {   // the interleaved layout's operand maps: 4 and 3 consecutive variables a box
     const CUtensorMap tmU4 = map(ubase, TX + 2, TY, TZ, 4), tmS4 = map(sbase, TX + 2, TY, TZ, 4),
                       tmU3 = map(ubase, TX + 2, TY, TZ, 3), tmS3 = map(sbase, TX + 2, TY, TZ, 3);
     return chm_emu::run_grid(grid, Cfg::THREADS, 1, Cfg::SMEM, [&] {
@@ -78,6 +86,7 @@ static chm_emu::Stats run(const Layout& L, const Coef& C, const Stage& st, int g
 
 template <int TX, int TY, int TZ, int ORDER, int IL = 0>
 static chm_emu::Stats run_mode(int mode, const Layout& L, const Coef& C, const Stage& st, int grid) {
+  if (mode == 10 + MODE_MID) return run<TX, TY, TZ, MODE_MID, ORDER, IL, true>(L, C, st, grid);   // fill-only
   switch (mode) {
     case MODE_RHS: return run<TX, TY, TZ, MODE_RHS, ORDER, IL>(L, C, st, grid);
     case MODE_FIRST: return run<TX, TY, TZ, MODE_FIRST, ORDER, IL>(L, C, st, grid);
@@ -112,7 +121,7 @@ int main(int argc, char** argv) {
   C.inv_h = 1.0 / h; C.inv_h2 = 1.0 / (h * h); C.ko = eps / (64.0 * h); C.eta = eta; C.sgc = sgc;
   const double w5[5] = {15.0, -6.0, 1.0, 0.0, 0.0}, w9[5] = {210.0, -120.0, 45.0, -10.0, 1.0};
   for (int k = 0; k < 5; ++k) C.kq[k] = ko_order == 9 ? eps / (1024.0 * h) * w9[k] : C.ko * w5[k];
-  Stage st{al(in), al(U), al(S), al(out), a, mode, ca, cb};
+  Stage st{al(in), al(U), al(S), al(out), a, mode >= 10 ? mode - 10 : mode, ca, cb};
   if (mode == MODE_FIRST) st.U = al(in);   // stage 1 reads U == in
   chm_emu::Stats s;
   if (order == 8 && tile == 0) s = run_mode<16, 4, 4, 8>(mode, L, C, st, grid);

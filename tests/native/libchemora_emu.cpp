@@ -198,6 +198,36 @@ static cudaError_t launch_bssn_fused_real(const Layout& L, const Coef& C, int or
   }
   return cudaErrorInvalidValue;
 }
+// fill-only mode (launch_bssn_fill): as emu_fused with the fill kernel
+template <int TX, int TY, int TZ, bool IL, bool DEEP>
+static cudaError_t emu_fill(const Layout& L, const Coef& C, const Stage& st) {
+  using Cfg = TmaCfg<TX, TY, TZ, 4, IL, DEEP>;
+  if (!launch_allowed(bssn_plan<TX, TY, TZ, 4, IL, DEEP>(MODE_MID, L.xo), L, st.in, L.xo - Cfg::H, Cfg::H)) return cudaErrorInvalidValue;
+  const CUtensorMap tm = emu_map(L, st.in, Cfg::BX, Cfg::BY, Cfg::BZ, 1), tmCen = emu_map(L, st.in, TX + 2, TY, TZ, 7),
+                    tmU = emu_map(L, st.U, TX + 2, TY, TZ, 1), tmS = emu_map(L, st.S, TX + 2, TY, TZ, 1),
+                    tmU4 = emu_map(L, st.U, TX + 2, TY, TZ, 4), tmS4 = emu_map(L, st.S, TX + 2, TY, TZ, 4),
+                    tmU3 = emu_map(L, st.U, TX + 2, TY, TZ, 3), tmS3 = emu_map(L, st.S, TX + 2, TY, TZ, 3);
+  const int ntx = (L.nx + TX - 1) / TX, nty = (L.ny + TY - 1) / TY, ntz = (L.nz + TZ - 1) / TZ;
+  const int ntiles = ntx * nty * ntz, grid = ntiles < kEmuSMs ? ntiles : kEmuSMs;
+  const int cy = L.col_rows / TY > 0 ? L.col_rows / TY : 1;
+  chm_emu::run_grid(grid, Cfg::THREADS, 1, Cfg::SMEM, [&] {
+    bssn_fill_kernel<TX, TY, TZ, MODE_MID, IL, DEEP>(tm, tmCen, tmU, tmS, tmU4, tmS4, tmU3, tmS3, L, C, st, ntx, nty, ntz, cy);
+  });
+  return cudaSuccess;
+}
+cudaError_t launch_bssn_fill(const Layout& L, const Coef& C, int tile, const Stage& st, cudaStream_t) {
+  if (st.mode != MODE_MID) return cudaErrorInvalidValue;
+  switch (tile) {
+    case 0: return emu_fill<16, 4, 4, false, false>(L, C, st);
+    case 1: return emu_fill<16, 8, 2, false, false>(L, C, st);
+    case 2: return emu_fill<8, 4, 8, false, false>(L, C, st);
+    case 3: return emu_fill<16, 2, 8, false, false>(L, C, st);
+    case 4: return emu_fill<16, 4, 2, false, false>(L, C, st);
+    case 5: case 6: return emu_fill<16, 4, 4, true, false>(L, C, st);
+    case 7: return emu_fill<16, 4, 4, true, true>(L, C, st);
+  }
+  return cudaErrorInvalidValue;
+}
 cudaError_t kernel_info_bssn_fused(int order, int tile, cudaFuncAttributes* a) {
   *a = fake_attr();
   return (order == 8 ? tile == 0 : (tile >= 0 && tile < kNumFused)) ? cudaSuccess : cudaErrorInvalidValue;

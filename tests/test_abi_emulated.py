@@ -184,3 +184,24 @@ def test_timing_pool_wraps_without_losing_launches(chem):
     h.timing(0)
     assert h.timing_read()["rhs_launches"] == 0
     h.destroy()
+
+
+def test_box_fill_benchmark_mode_through_the_abi(chem):
+    """chemora_measure_box_fill (the tracked form of DESIGN.md 6.5's box-fill probe): runs for every fused 4th-order
+    id, leaves U, S and YA as they were, refuses what it does not cover"""
+    nx, ny, nz = 16, 8, 4
+    h = chem.Chemora(nx, ny, nz, 3, 4, chem.SYS_BSSN, 0.05)
+    u = inputs.bssn_minkowski(nx, ny, nz) + 0.05 * np.random.default_rng(3).uniform(-1, 1, size=(25, nz, ny, nx))
+    h.set_state(u)
+    before = [h.state_view(b).clone() for b in (chem.BUF_YA, chem.BUF_S)]
+    for tile in chem.variants(chem.SYS_BSSN, 4):
+        assert h.measure_box_fill(tile) > 0.0
+    assert np.array_equal(h.get_state(), u)
+    assert all((h.state_view(b) == x).all() for b, x in zip((chem.BUF_YA, chem.BUF_S), before))
+    with pytest.raises(chem.ChemoraError):
+        h.measure_box_fill(8)
+    h.destroy()
+    w = chem.Chemora(8, 8, 8, 2, 4, chem.SYS_WAVE, 0.1)
+    with pytest.raises(chem.ChemoraError):
+        w.measure_box_fill(0)
+    w.destroy()

@@ -105,6 +105,20 @@ def test_tile_traversal_order_does_not_change_the_result(oracle, emu, tmp_path, 
     assert np.array_equal(ref[0], got[0]) and ref[3]["loads"] == got[3]["loads"]
 
 
+@pytest.mark.parametrize("tile", [0, 1, 3, 5, 7])
+def test_fill_only_mode_moves_what_the_full_kernel_moves(oracle, emu, tmp_path, tile):
+    """the benchmark mode behind chemora_measure_box_fill: the same TMA requests and bytes as a middle RK4 stage of
+    the full kernel (it runs the same issue / wait / release / refill code), no wait gives up, nothing is written"""
+    nx, ny, nz, g, h, eps = 20, 9, 6, 3, 0.05, 0.1
+    st = oracle.fill_ghosts(oracle.with_ghosts(strong(nx, ny, nz), g), g)
+    U = oracle.fill_ghosts(oracle.with_ghosts(strong(nx, ny, nz, seed=7), g), g)
+    S = oracle.fill_ghosts(oracle.with_ghosts(strong(nx, ny, nz, seed=8), g), g)
+    full = launch(emu, tmp_path, 4, tile, MODE_MID, st, U, S, g, h, eps, a=0.00625)
+    fill = launch(emu, tmp_path, 4, tile, 10 + MODE_MID, st, U, S, g, h, eps, a=0.00625)
+    assert fill[3] == full[3]                                        # TMA requests and bytes
+    assert not fill[0].any() and np.array_equal(fill[1], S) and np.array_equal(fill[2], U)
+
+
 def test_flat_space_gives_exactly_zero(oracle, emu, tmp_path):
     st = oracle.fill_ghosts(oracle.with_ghosts(inputs.bssn_minkowski(16, 8, 8), 3), 3)
     z = np.zeros_like(st)
