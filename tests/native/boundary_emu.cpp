@@ -48,8 +48,8 @@ int main(int argc, char** argv) {
   Stage st{in.data(), mode == MODE_FIRST ? in.data() : U.data(), S.data(), out.data(), a, mode, ca, cb};
   const unsigned mask = system == 1 ? (1u << 0) | (1u << 1) | (1u << 4) | (1u << 6) | (1u << 17) : 0u;   // as chemora.cu
   const RadGeom G = rad_geom(L);
-  chm_emu::run_grid((int)((G.tasks + 7) / 8), 256, 1, 0,
-                    [&] { radiative_kernel(L, st, h, mask, (int)G.rowsA, (int)G.rowsAB, G.lpr_shift); }, V);
+  chm_emu::run_grid_serial((int)((G.tasks + 7) / 8), V, 1, 256, 1,   // no barrier, no shuffle: thread after thread
+                           [&] { radiative_kernel(L, st, h, mask, (int)G.rowsA, (int)G.rowsAB, G.lpr_shift); });
   FILE* f = fopen(argv[15], "wb");
   if (!f) return 4;
   for (const std::vector<double>* b : {&out, &S, mode == MODE_FIRST ? &in : &U}) {

@@ -15,14 +15,8 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def build(tmp, name):
-    exe = str(tmp / (name + "_asan"))
-    r = subprocess.run(["g++", "-std=c++17", "-O0", "-fsanitize=address", "-fno-omit-frame-pointer", "-DCHM_EMULATE",
-                        "-pthread", "-o", exe, os.path.join(ROOT, "tests", "native", name + ".cpp")], capture_output=True,
-                       text=True)
-    if r.returncode != 0 and "asan" in (r.stderr or "").lower():
-        pytest.skip("AddressSanitizer runtime not available")
-    assert r.returncode == 0, r.stderr[-2000:]
-    return exe
+    from tests.conftest import build_emulator
+    return build_emulator(name, flags=("-O0", "-fsanitize=address"))
 
 
 def run(cmd):
@@ -68,13 +62,8 @@ def test_wave_and_boundary_kernels_under_asan(oracle, tmp_path):
 
 
 def build_tsan(tmp, name, *defines):
-    exe = str(tmp / (name + "_tsan" + str(len(defines))))
-    r = subprocess.run(["g++", "-std=c++17", "-O0", "-fsanitize=thread", "-DCHM_EMULATE", "-pthread"] + list(defines) +
-                       ["-o", exe, os.path.join(ROOT, "tests", "native", name + ".cpp")], capture_output=True, text=True)
-    if r.returncode != 0 and "tsan" in (r.stderr or "").lower():
-        pytest.skip("ThreadSanitizer runtime not available")
-    assert r.returncode == 0, r.stderr[-2000:]
-    return exe
+    from tests.conftest import build_emulator
+    return build_emulator(name, flags=("-O0", "-fsanitize=thread") + tuple(defines))
 
 
 def test_fused_kernel_under_thread_sanitizer(oracle, tmp_path):
