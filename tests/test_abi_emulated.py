@@ -64,6 +64,13 @@ def test_gpu_test_functions_against_the_emulated_library(chem, oracle):
     A.test_bssn_even_ghost_width(chem, oracle)
     A.test_enforce_constraints(chem, oracle)
     A.test_rk3_wave_systems(chem, oracle, 2, 4, 3, 5)
+    # tile-id routing of run_rhs_inner: ids 6..8 of the wave systems go to the plane-ring kernel (or fall back)
+    A.test_wave_rhs_all_tiles(chem, oracle, 4, 3, 0.1, (16, 16, 16))
+    A.test_wave_rhs_all_tiles(chem, oracle, 8, 4, 0.0, (33, 9, 12))
+    A.test_wave1_rhs_all_tiles(chem, oracle, 4, 3, 0.1, (16, 16, 16))
+    # 8th-order BSSN (5 ghost zones): the fused id-0 instance and the six split tiles; RK3 through the split variant
+    A.test_bssn_o8_rhs(chem, oracle, "strong")
+    A.test_bssn_rk3_split_variant(chem, oracle)
     Z.test_radiative_rhs_at_boundary_points(chem, oracle, 1, 4, 3, (21, 12, 10))
     Z.test_radiative_rhs_at_boundary_points(chem, oracle, 0, 8, 4, (37, 9, 12))
     Z.test_radiative_rk4_whole_block(chem, oracle, 0, 4, 2, 10, 1e-11)
