@@ -127,7 +127,7 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
                                               const Coef& C, const Stage& st, int ntx, int nty, int ntz, int cy) {
   using Cfg = TmaCfg<TX, TY, TZ, ORDER, IL, DEEP>;
   constexpr int H = Cfg::H;
-  constexpr int BX = Cfg::BX, BY = Cfg::BY, SLOT = Cfg::SLOT, SLOTX = Cfg::SLOTX, TILE = Cfg::TILE, CEN = Cfg::CEN;
+  constexpr int BX = Cfg::BX, BY = Cfg::BY, SLOT = Cfg::SLOT, SLOTX = Cfg::SLOTX, TILE = Cfg::TILE;
   constexpr unsigned NW = Cfg::NWARPS;
   constexpr int kSlots = Cfg::NS;
   constexpr bool PARK = Cfg::PARK;
