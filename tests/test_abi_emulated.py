@@ -9,6 +9,7 @@ Why: GPU access was closed for all of round 2, and that host code -- which sits 
 never executed.  This is test infrastructure: the package never loads the emulated library (no CPU fallback exists:
 tests/test_abi.py::test_no_cpu_fallback), and the -m gpu tests remain the proof on the device."""
 import ctypes
+import os
 import types
 
 import numpy as np
@@ -212,3 +213,15 @@ def test_box_fill_benchmark_mode_through_the_abi(chem):
     with pytest.raises(chem.ChemoraError):
         w.measure_box_fill(0)
     w.destroy()
+
+
+@pytest.mark.skipif(not os.environ.get("CHEMORA_EMU_LONG"), reason="several minutes under emulation: set CHEMORA_EMU_LONG=1")
+def test_north_star_tolerance_case_ten_steps(chem, oracle):
+    """BASELINE.json north_star: BSSN, <= 1e-10 after 10 steps (both norms of DESIGN.md S11 / S11b), configs[2] data at
+    24 x 20 x 18 -- the GPU test functions themselves, through the emulated ABI: the default fused variant with RK4,
+    the newest variant (id 7) with RK4 and with enforced RK3"""
+    from tests import test_gpu_a_parity as A
+    from tests import test_gpu_zz_round2 as Z
+    A.test_bssn_rk4_10_steps_small(chem, oracle, 1)
+    Z.test_interleaved_layout_10_steps_and_rk3(chem, oracle, 7)
+
