@@ -311,7 +311,7 @@ def run_sweep(args):
                               "updates_per_s": npts / (4 * m * 1e-3), "regs": info["regs"],
                               "spill_bytes": info["local_bytes"], "hbm_gbs_algorithmic": bytes_pt * npts / (m * 1e-3) / 1e9,
                               "best": (f, t) == (fused, tile)})
-                if f == 1:     # the paper's tile cost model next to the measurement
+                if f == 1 and t < 5:     # the paper's tile cost model covers the five tile shapes of the plain layout next to the measurement
                     table[-1]["sigma_model"] = binding.tile_cost(4, 3, t)[0]
         h.destroy()
         rows = [r for r in table if r["grid"] == [nx, ny, nz] and "sigma_model" in r]
