@@ -51,7 +51,8 @@ def build_emulator(name, shared=False, flags=()):
     from concurrent.futures import ThreadPoolExecutor
     key = (name, bool(shared), tuple(flags))
     if _EMU_POOL is None:
-        _EMU_POOL = ThreadPoolExecutor(max_workers=max(2, min(8, (os.cpu_count() or 2))))
+        # the longest build (libchemora_emu, ~50 s) bounds the total: four at a time is as fast as eight, at half the memory
+        _EMU_POOL = ThreadPoolExecutor(max_workers=max(2, min(4, (os.cpu_count() or 2))))
         for k in _EMU_ALL:
             _EMU[k] = _EMU_POOL.submit(_build_one, *k)
     if key not in _EMU:
