@@ -225,3 +225,26 @@ def test_north_star_tolerance_case_ten_steps(chem, oracle):
     A.test_bssn_rk4_10_steps_small(chem, oracle, 1)
     Z.test_interleaved_layout_10_steps_and_rk3(chem, oracle, 7)
 
+
+@pytest.mark.skipif(not os.environ.get("CHEMORA_EMU_LONG"), reason="about 25 minutes under emulation: set CHEMORA_EMU_LONG=1")
+def test_every_fused_variant_ten_steps_every_slot_moves(chem, oracle):
+    """10 RK4 steps on data where all 25 slots evolve by far more than 1e-10 of their size (1e-4 Gaussians; 0.02 strong
+    field), <= 1e-10 in both norms: the GPU test function for fused ids 0..4 + a split tile, then ids 5, 6, 7"""
+    from tests import test_gpu_zz_round2 as Z
+    from tests.test_gpu_a_parity import TOL_BSSN_10_STEPS, assert_bssn_close
+    nx, ny, nz, dx, dt, eps = 24, 20, 18, 0.05, 0.0125, 0.1
+    for data in ("gaussians", "strong"):
+        Z.test_bssn_rk4_10_steps_every_slot_moves(chem, oracle, data)
+        u0 = inputs.bssn_gaussians(nx, ny, nz, width_cells=4.0) if data == "gaussians" else \
+            inputs.bssn_minkowski(nx, ny, nz) + 0.02 * np.random.default_rng(23).uniform(-1, 1, size=(25, nz, ny, nx))
+        want = oracle.interior(oracle.rk4(1, oracle.with_ghosts(u0, 3), 3, 4, dx, dt, oracle.params(eps_diss=eps), 10), 3)
+        h = chem.Chemora(nx, ny, nz, 3, 4, chem.SYS_BSSN, dx)
+        h.set_param("eps_diss", eps)
+        for tile in (5, 6, 7):
+            h.set_variant(1, tile)
+            h.set_state(u0)
+            for _ in range(10):
+                h.rk4_step(dt)
+            assert_bssn_close(h.get_state(), want, TOL_BSSN_10_STEPS)
+        h.destroy()
+
