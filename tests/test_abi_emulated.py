@@ -248,3 +248,15 @@ def test_every_fused_variant_ten_steps_every_slot_moves(chem, oracle):
             assert_bssn_close(h.get_state(), want, TOL_BSSN_10_STEPS)
         h.destroy()
 
+
+@pytest.mark.skipif(not os.environ.get("CHEMORA_EMU_LONG"), reason="2 minutes under emulation: set CHEMORA_EMU_LONG=1")
+def test_papers_configuration_8th_order_five_ghost_zones(chem, oracle):
+    """the GPU test functions of the 8th-order BSSN system -- right-hand side on
+    1e-10 data, 10 RK4 steps (<= 1e-10, both norms), 5 enforced RK3 steps, the 11-point KO9 operator -- for the fused
+    8th-order kernel and the split variant"""
+    from tests import test_gpu_a_parity as A
+    A.test_bssn_o8_rhs(chem, oracle, "noise1e-10")
+    for fused in (1, 0):
+        A.test_bssn_o8_rk4_10_steps_and_rk3_enforced(chem, oracle, fused)
+        A.test_bssn_o8_ko9(chem, oracle, fused)
+
