@@ -65,7 +65,8 @@ def bench(monkeypatch):
 
 def args(**kw):
     a = dict(gpus=1, steps=2, warmup=1, impl="ours", size=8, variant="auto", e2e_steps=2, cpu_sample=16, ref_sample=16,
-             sweep=False, fill_floor=False, wave=False, wave1=False, paper_shape=False, ko_order=9)
+             sweep=False, fill_floor=False, wave=False, wave1=False, paper_shape=False, ko_order=9,
+             sweep_in_process=True, probe=False)
     a.update(kw)
     return types.SimpleNamespace(**a)
 
@@ -117,6 +118,44 @@ def test_a_failing_sweep_does_not_cost_the_run(bench, capsys, monkeypatch):
     bench.run_ours(args())
     v = last_json(capsys)["config"]["variant"]
     assert v["fused"] == 1 and v["tile_id"] == 0 and "injected" in v["sweep_error"] and v["sweep_ms"] is None
+
+
+def test_the_sweep_runs_in_a_child_by_default(bench, capsys, monkeypatch):
+    """--variant auto without --sweep-in-process: `python bench.py --probe` in a child (a sticky device fault of a
+    candidate then costs the sweep, not the headline run).  The child cannot be real here (it would load the real
+    library and find no device), so subprocess.run is replaced by one that runs bench.run_probe in this process and
+    hands back what it printed -- then by children that crash, print rubbish, or never end."""
+    import subprocess
+    seen = []
+
+    def child(cmd, **kw):
+        seen.append(cmd)
+        assert cmd[1:] == [os.path.join(ROOT, "bench.py"), "--probe", "--size", "8"] and kw["timeout"] > 0
+        bench.run_probe(args(probe=True))
+        return types.SimpleNamespace(returncode=0, stdout="torch says hello\n" + capsys.readouterr().out, stderr="")
+
+    monkeypatch.setattr(subprocess, "run", child)
+    bench.run_ours(args(sweep_in_process=False))
+    v = last_json(capsys)["config"]["variant"]
+    assert len(seen) == 1 and v["sweep_process"] == "child" and v["sweep_error"] is None
+    assert len(v["sweep_ms"]) == 18 and v["sweep_ms"][9 + v["tile_id"]] > 0 and v["fused"] == 1 and v["col_rows"] >= 1
+
+    def crashed(cmd, **kw):
+        return types.SimpleNamespace(returncode=-6, stdout="", stderr="a\nb\nCUDA error: an illegal memory access\nAborted")
+
+    def rubbish(cmd, **kw):
+        return types.SimpleNamespace(returncode=0, stdout='{"probe": {"fused": 1}}\n', stderr="")
+
+    def endless(cmd, **kw):
+        raise subprocess.TimeoutExpired(cmd, kw["timeout"])
+
+    for fake, word in ((crashed, "illegal memory access"), (rubbish, "exit 0"), (endless, "no result within")):
+        monkeypatch.setattr(subprocess, "run", fake)
+        bench.run_ours(args(sweep_in_process=False))
+        line = last_json(capsys)
+        v = line["config"]["variant"]
+        assert (v["fused"], v["tile_id"], v["sweep_ms"], v["col_rows"]) == (1, 0, None, 32) and word in v["sweep_error"]
+        assert line["value"] > 0 and line["gpu_launches"] == 16
 
 
 def test_context_modes_run(bench, capsys, monkeypatch):
