@@ -155,17 +155,25 @@ def run_probe(args):
     torch.cuda.set_device(local)
     _, u0, h = headline_handle(binding, inputs, replicas, args.size, int(os.environ.get("RANK", "0")), local)
     h.set_state(u0)
+    if args.probe_ids:
+        h.set_param("autotune_fused_ids", args.probe_ids)
     fused, tile, ms = h.autotune()
     col_rows = int(h.get_param("col_rows"))
     h.destroy()
     print(json.dumps({"probe": {"fused": fused, "tile": tile, "col_rows": col_rows, "sweep_ms": ms}}))
 
 
-def isolated_sweep(size, timeout_s=900):
+ROUND1_FUSED_IDS = 5      # fused tile ids 0..4: the kernels that ran on hardware in round 1
+
+
+def isolated_sweep(size, fused_ids=0, timeout_s=900):
     """The runtime sweep in a child process (python bench.py --probe): its candidates include kernels no GPU has run
     yet (fused ids 5..7), and a device fault is sticky for the CUDA context that saw it -- in a child it
-    costs the sweep, in this process it would cost the headline measurement.  Returns (pick or None, error or None)."""
+    costs the sweep, in this process it would cost the headline measurement.  fused_ids > 0 bounds the candidates to
+    the fused tile ids below it ("autotune_fused_ids").  Returns (pick or None, error or None)."""
     cmd = [sys.executable, os.path.abspath(__file__), "--probe", "--size", str(size)]
+    if fused_ids:
+        cmd += ["--probe-ids", str(fused_ids)]
     try:
         r = subprocess.run(cmd, capture_output=True, text=True, timeout=timeout_s)
     except subprocess.TimeoutExpired:
@@ -211,7 +219,10 @@ def run_ours(args):
     sweep_error = None
     if args.variant == "auto" and not args.sweep_in_process:
         pick, sweep_error = isolated_sweep(n)
-        fused, tile, rows, sweep_ms = pick if pick else (1, 0, None, None)   # failed sweep: the default tile, said so
+        if pick is None:                      # once more over the tiles that have run on hardware before
+            pick, again = isolated_sweep(n, ROUND1_FUSED_IDS)
+            sweep_error += "; sweep bounded to fused ids 0..%d: %s" % (ROUND1_FUSED_IDS - 1, again or "done")
+        fused, tile, rows, sweep_ms = pick if pick else (1, 0, None, None)   # failed sweeps: the default tile, said so
         h.set_variant(fused, tile)
         if rows:
             h.set_param("col_rows", rows)
@@ -488,6 +499,7 @@ def main():
     ap.add_argument("--sweep-in-process", action="store_true",
                     help="--variant auto: run the sweep in this process instead of a child (see isolated_sweep)")
     ap.add_argument("--probe", action="store_true", help=argparse.SUPPRESS)   # the child of isolated_sweep
+    ap.add_argument("--probe-ids", type=int, default=0, help=argparse.SUPPRESS)
     ap.add_argument("--e2e-steps", type=int, default=8)
     ap.add_argument("--cpu-sample", type=int, default=128)
     ap.add_argument("--ref-sample", type=int, default=64)

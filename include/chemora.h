@@ -74,7 +74,9 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
  * with the paper's 8th-order, 5-ghost-zone configuration; accepted for the 8th-order BSSN
  * system only); tuning: "col_rows" (default 32: y-extent in grid rows of the columns in which the fused BSSN
  * kernel visits its tiles, chosen so the halo planes shared by z-neighbour tiles stay in L2), "autotune_split"
- * (default 0; 1: chemora_autotune also times the derivative-split variant, which allocates its derivative scratch).
+ * (default 0; 1: chemora_autotune also times the derivative-split variant, which allocates its derivative scratch),
+ * "autotune_fused_ids" (default CHEMORA_NUM_TILES; 1..CHEMORA_NUM_TILES: chemora_autotune times only the fused tile
+ * ids below this bound, e.g. 5 = the five tile shapes of the plain section layout).
  * Unknown name or invalid value -> CHEMORA_EINVAL. */
 int chemora_set_param(chemora_t* h, const char* name, double value);
 
@@ -202,7 +204,8 @@ int chemora_variant_available(int system_id, int fd_order, int fused, int tile_i
 int chemora_tile_shape(int system_id, int fused, int tile_id, int* tx, int* ty, int* tz);
 
 /* Runtime sweep (the paper's model-based choice, replaced by measurement): times every available
- * fused tile id (and, with the parameter "autotune_split" = 1, the six split tiles) on the handle's own grid -- one
+ * fused tile id below the parameter "autotune_fused_ids" (default: all; and, with the parameter "autotune_split" = 1,
+ * the six split tiles) on the handle's own grid -- one
  * middle RK4 stage evaluated on the current U, results into the scratch buffers S and Ya; one warm-up run, then the
  * median of three timed runs -- keeps the fastest, returns it.  A variant that cannot run here (CHEMORA_ENOMEM for
  * its scratch, CHEMORA_EINVAL from its launch check) is skipped, not fatal.  Guard: every fused BSSN tile id evaluates

@@ -33,6 +33,7 @@ struct chemora {
   int fused, tile;
   int boundary;         // CHEMORA_BC_PERIODIC (ghost fill) or CHEMORA_BC_RADIATIVE (ghost layers are evolved boundary points)
   int autotune_split;   // tuning: chemora_autotune also times the derivative-split variant
+  int autotune_fused_ids;   // tuning: chemora_autotune times the fused tile ids below this bound
   chemora* nb_lo;        // z-neighbours of a linked block (chemora_link_z); nullptr: periodic in itself
   chemora* nb_hi;
   long launches;
@@ -238,6 +239,7 @@ int chemora_create(chemora_t** out, int nx, int ny, int nz, int ghost, int fd_or
   h->fused = 1; h->tile = (system_id == CHEMORA_SYS_BSSN && fd_order == 8) ? 0 : 1;
   h->launches = 0;
   h->autotune_split = 0;
+  h->autotune_fused_ids = CHEMORA_NUM_TILES;
   h->boundary = CHEMORA_BC_PERIODIC;
   h->timing = false;
   for (int c = 0; c < 2; ++c) { h->ev_used[c] = 0; h->ev_ms[c] = 0.0; h->ev_launches[c] = 0; }
@@ -294,6 +296,9 @@ int chemora_set_param(chemora_t* h, const char* name, double v) {
   } else if (!strcmp(name, "autotune_split")) {
     if (v != 0.0 && v != 1.0) return fail(h, CHEMORA_EINVAL, "autotune_split must be 0 or 1");
     h->autotune_split = (int)v;
+  } else if (!strcmp(name, "autotune_fused_ids")) {
+    if (v != (double)(int)v || v < 1.0 || v > (double)CHEMORA_NUM_TILES) return fail(h, CHEMORA_EINVAL, "autotune_fused_ids must be 1..CHEMORA_NUM_TILES");
+    h->autotune_fused_ids = (int)v;
   } else return fail(h, CHEMORA_EINVAL, std::string("unknown parameter: ") + name);
   return CHEMORA_OK;
 }
@@ -306,6 +311,7 @@ int chemora_get_param(const chemora_t* h, const char* name, double* v) {
   else if (!strcmp(name, "shift_gamma_coeff")) *v = h->sgc;
   else if (!strcmp(name, "col_rows")) *v = h->L.col_rows;
   else if (!strcmp(name, "autotune_split")) *v = h->autotune_split;
+  else if (!strcmp(name, "autotune_fused_ids")) *v = h->autotune_fused_ids;
   else return CHEMORA_EINVAL;
   return CHEMORA_OK;
 }
@@ -685,6 +691,7 @@ int chemora_autotune(chemora_t* h, int* fused_out, int* tile_out, float* ms_out)
   for (int f = 1; f >= (h->autotune_split ? 0 : 1) && !rc; --f)
     for (int t = 0; t < CHEMORA_NUM_TILES && !rc; ++t) {
       if (!chemora_variant_available(h->system, h->order, f, t)) continue;
+      if (f == 1 && t >= h->autotune_fused_ids) continue;                  // candidates bounded by the caller: ms stays -1
       h->fused = f; h->tile = t;
       // a middle RK4 stage (the common case) on scratch operands: k = f(U); S += 2k; Ya = U + a k.
       // S and Ya are scratch between steps (stage 1 overwrites them); U is only read.

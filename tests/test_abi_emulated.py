@@ -2,7 +2,7 @@
 sweep with its agreement guard and col_rows sweep, the timing event pool, ghosted state copies, the radiative step
 order, the device error word) compiled with g++ on top of the emulated kernels and a stub of the few CUDA runtime
 calls it makes (tests/native/libchemora_emu.cpp), driven through the normal Python binding by (a) the same test
-FUNCTIONS that run on the GPU (tests/test_gpu_a_parity.py, tests/test_gpu_zz_round2.py), called with the emulated
+FUNCTIONS that run on the GPU (tests/test_gpu_a_parity.py, test_gpu_zz_round2.py, test_gpu_zzz_new_fused_ids.py), called with the emulated
 library behind `chem`, and (b) small clones of the heavy ones.
 
 Why: GPU access was closed for all of round 2, and that host code -- which sits on bench.py's default path -- had
@@ -149,6 +149,17 @@ def test_runtime_sweep_guard_and_col_rows(chem, monkeypatch):
     assert all(m == -1.0 for m in ms[:nt])                             # split variant: only on request
     assert h.get_param("col_rows") in (16.0, 32.0, 64.0)
     assert np.array_equal(h.get_state(), u)
+    # candidates bounded by the caller ("autotune_fused_ids"): the later ids are not launched at all
+    assert h.get_param("autotune_fused_ids") == nt
+    h.set_param("autotune_fused_ids", 5)
+    l0 = h.launch_count()
+    fused, tile, ms = h.autotune()
+    assert tile < 5 and all(ms[nt + t] > 0 for t in range(5)) and all(m == -1.0 for m in ms[nt + 5:])
+    assert h.launch_count() - l0 <= 1 + 5 * 4 + 4 + 2 * 4               # fill, 5 ids x 4 runs, 4 guards, 2 col_rows x 4
+    for bad in (0, nt + 1, 2.5):
+        with pytest.raises(chem.ChemoraError):
+            h.set_param("autotune_fused_ids", bad)
+    h.set_param("autotune_fused_ids", nt)
     monkeypatch.setenv("CHM_EMU_BREAK_TILE", "5")
     monkeypatch.setenv("CHM_EMU_TIMEOUT_TILE", "3")
     h.set_param("autotune_split", 1)
@@ -221,9 +232,9 @@ def test_north_star_tolerance_case_ten_steps(chem, oracle):
     24 x 20 x 18 -- the GPU test functions themselves, through the emulated ABI: the default fused variant with RK4,
     the newest variant (id 7) with RK4 and with enforced RK3"""
     from tests import test_gpu_a_parity as A
-    from tests import test_gpu_zz_round2 as Z
+    from tests import test_gpu_zzz_new_fused_ids as N
     A.test_bssn_rk4_10_steps_small(chem, oracle, 1)
-    Z.test_interleaved_layout_10_steps_and_rk3(chem, oracle, 7)
+    N.test_interleaved_layout_10_steps_and_rk3(chem, oracle, 7)
 
 
 @pytest.mark.skipif(not os.environ.get("CHEMORA_EMU_LONG"), reason="about 25 minutes under emulation: set CHEMORA_EMU_LONG=1")
@@ -231,8 +242,10 @@ def test_every_fused_variant_ten_steps_every_slot_moves(chem, oracle):
     """10 RK4 steps on data where all 25 slots evolve by far more than 1e-10 of their size (1e-4 Gaussians; 0.02 strong
     field), <= 1e-10 in both norms: the GPU test function for fused ids 0..4 + a split tile, then ids 5, 6, 7"""
     from tests import test_gpu_zz_round2 as Z
+    from tests import test_gpu_zzz_new_fused_ids as N
     from tests.test_gpu_a_parity import TOL_BSSN_10_STEPS, assert_bssn_close
     nx, ny, nz, dx, dt, eps = 24, 20, 18, 0.05, 0.0125, 0.1
+    N.test_new_ids_10_steps_every_slot_moves(chem, oracle)
     for data in ("gaussians", "strong"):
         Z.test_bssn_rk4_10_steps_every_slot_moves(chem, oracle, data)
         u0 = inputs.bssn_gaussians(nx, ny, nz, width_cells=4.0) if data == "gaussians" else \
@@ -240,7 +253,7 @@ def test_every_fused_variant_ten_steps_every_slot_moves(chem, oracle):
         want = oracle.interior(oracle.rk4(1, oracle.with_ghosts(u0, 3), 3, 4, dx, dt, oracle.params(eps_diss=eps), 10), 3)
         h = chem.Chemora(nx, ny, nz, 3, 4, chem.SYS_BSSN, dx)
         h.set_param("eps_diss", eps)
-        for tile in (5, 6, 7):
+        for tile in (5, 6, 7) if data == "strong" else ():         # "gaussians": the GPU test function above
             h.set_variant(1, tile)
             h.set_state(u0)
             for _ in range(10):

@@ -66,7 +66,7 @@ def bench(monkeypatch):
 def args(**kw):
     a = dict(gpus=1, steps=2, warmup=1, impl="ours", size=8, variant="auto", e2e_steps=2, cpu_sample=16, ref_sample=16,
              sweep=False, fill_floor=False, wave=False, wave1=False, paper_shape=False, ko_order=9,
-             sweep_in_process=True, probe=False)
+             sweep_in_process=True, probe=False, probe_ids=0)
     a.update(kw)
     return types.SimpleNamespace(**a)
 
@@ -154,8 +154,23 @@ def test_the_sweep_runs_in_a_child_by_default(bench, capsys, monkeypatch):
         bench.run_ours(args(sweep_in_process=False))
         line = last_json(capsys)
         v = line["config"]["variant"]
-        assert (v["fused"], v["tile_id"], v["sweep_ms"], v["col_rows"]) == (1, 0, None, 32) and word in v["sweep_error"]
+        assert (v["fused"], v["tile_id"], v["sweep_ms"], v["col_rows"]) == (1, 0, None, 32)
+        assert v["sweep_error"].count(word) == 2 and "bounded to fused ids 0..4" in v["sweep_error"]   # both children
         assert line["value"] > 0 and line["gpu_launches"] == 16
+
+    # the unbounded child dies, the one bounded to the tiles of round 1 does not: its pick is used, and the line says so
+    def second_time_lucky(cmd, **kw):
+        if "--probe-ids" not in cmd:
+            return crashed(cmd, **kw)
+        assert cmd[-2:] == ["--probe-ids", "5"]
+        bench.run_probe(args(probe=True, probe_ids=5))
+        return types.SimpleNamespace(returncode=0, stdout=capsys.readouterr().out, stderr="")
+
+    monkeypatch.setattr(subprocess, "run", second_time_lucky)
+    bench.run_ours(args(sweep_in_process=False))
+    v = last_json(capsys)["config"]["variant"]
+    assert v["fused"] == 1 and v["tile_id"] < 5 and all(m == -1.0 for m in v["sweep_ms"][9 + 5:])
+    assert "illegal memory access" in v["sweep_error"] and v["sweep_error"].endswith("fused ids 0..4: done")
 
 
 def test_context_modes_run(bench, capsys, monkeypatch):

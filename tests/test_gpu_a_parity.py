@@ -11,7 +11,7 @@ pytestmark = pytest.mark.gpu
 TOL_WAVE_PER_STEP = 1e-12
 TOL_BSSN_10_STEPS = 1e-10
 TOL_RHS = 1e-12          # a single RHS evaluation: rounding-order differences only (difference-form stencils)
-ROUND1_FUSED_IDS = 5     # fused BSSN ids 0..4 ran green on hardware in round 1; later ids are tested in test_gpu_zz_round2.py
+ROUND1_FUSED_IDS = 5     # fused BSSN ids 0..4 ran green on hardware in round 1; later ids: test_gpu_zzz_new_fused_ids.py
 
 
 @pytest.fixture(scope="module")
@@ -309,12 +309,16 @@ def test_autotune_and_kernel_info(chem):
     h.set_param("eps_diss", 0.1)
     u = inputs.bssn_noise(n, n, n)
     h.set_state(u)
+    with pytest.raises(chem.ChemoraError):
+        h.set_param("autotune_fused_ids", 0)
+    with pytest.raises(chem.ChemoraError):
+        h.set_param("autotune_fused_ids", chem.NUM_TILES + 1)
+    h.set_param("autotune_fused_ids", ROUND1_FUSED_IDS)                 # the unbounded sweep: test_gpu_zzz_new_fused_ids.py
     fused, tile, ms = h.autotune()
     nt = chem.NUM_TILES
-    assert fused == 1 and tile in chem.variants(chem.SYS_BSSN, 4)
+    assert fused == 1 and tile < ROUND1_FUSED_IDS
     assert all(ms[nt + t] > 0 for t in range(ROUND1_FUSED_IDS))         # the five plain fused ids are timed
-    assert all(ms[nt + t] != -1.0 for t in chem.variants(chem.SYS_BSSN, 4))   # later ids: timed, or disqualified (-2, -3)
-    assert all(ms[nt + t] == -1.0 for t in range(nt) if t not in chem.variants(chem.SYS_BSSN, 4))
+    assert all(ms[nt + t] == -1.0 for t in range(ROUND1_FUSED_IDS, nt))  # no other
     assert all(m < 0 for m in ms[:nt])                                  # split variant: only on request
     h.set_param("autotune_split", 1)
     fused2, tile2, ms2 = h.autotune()

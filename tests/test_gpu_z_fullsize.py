@@ -4,7 +4,9 @@ sweep), on sampled outputs the oracle can compute one by one (`pytest -m gpu`).
 A grid point after n RK4 steps depends on the initial data within 12 n cells (4 stages x 3-cell stencils; 16 n for
 the 8th-order wave system), so the oracle evolves a small periodic block cut around each sample (the cut's own
 wrap-around is wrong, but cannot reach the block's centre) and the centre is compared with the GPU state.
-Error norm: S11 with the per-variable maximum taken over the whole GPU state."""
+Error norm: S11 with the per-variable maximum taken over the whole GPU state.
+The BSSN sweep here is bounded to the fused tile ids that ran on hardware in round 1 (0..4); the unbounded sweep, which
+may pick ids 5..7, repeats at full size in tests/test_gpu_zzz_new_fused_ids.py, the file that sorts last."""
 import numpy as np
 import pytest
 
@@ -55,6 +57,7 @@ def test_bssn_config3_256_sampled(oracle):
     h = binding.Chemora(n, n, n, g, c["order"], binding.SYS_BSSN, dx)
     h.set_param("eps_diss", c["eps_diss"])
     h.set_state(u0)
+    h.set_param("autotune_fused_ids", 5)   # the tiles that ran on hardware in round 1; the rest: test_gpu_zzz_new_fused_ids.py
     h.autotune()                       # what bench.py does
     for _ in range(steps):
         h.rk4_step(dt)
