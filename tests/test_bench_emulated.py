@@ -151,12 +151,15 @@ def test_the_sweep_runs_in_a_child_by_default(bench, capsys, monkeypatch):
 
     for fake, word in ((crashed, "illegal memory access"), (rubbish, "exit 0"), (endless, "no result within")):
         monkeypatch.setattr(subprocess, "run", fake)
-        bench.run_ours(args(sweep_in_process=False))
-        line = last_json(capsys)
-        v = line["config"]["variant"]
-        assert (v["fused"], v["tile_id"], v["sweep_ms"], v["col_rows"]) == (1, 0, None, 32)
-        assert v["sweep_error"].count(word) == 2 and "bounded to fused ids 0..4" in v["sweep_error"]   # both children
-        assert line["value"] > 0 and line["gpu_launches"] == 16
+        pick, err = bench.isolated_sweep(8)
+        assert pick is None and word in err
+    monkeypatch.setattr(subprocess, "run", crashed)                      # both children die: the default tile, said so
+    bench.run_ours(args(sweep_in_process=False))
+    line = last_json(capsys)
+    v = line["config"]["variant"]
+    assert (v["fused"], v["tile_id"], v["sweep_ms"], v["col_rows"]) == (1, 0, None, 32)
+    assert v["sweep_error"].count("illegal memory access") == 2 and "bounded to fused ids 0..4" in v["sweep_error"]
+    assert line["value"] > 0 and line["gpu_launches"] == 16
 
     # the unbounded child dies, the one bounded to the tiles of round 1 does not: its pick is used, and the line says so
     def second_time_lucky(cmd, **kw):
