@@ -14,6 +14,47 @@ from tests.test_gpu_zz_round2 import CONFIGS4_GRIDS, config3_256_full_field, con
 pytestmark = pytest.mark.gpu
 
 
+# ---- first the tests that survive a new id that is merely wrong (the sweep's guard disqualifies it), then the direct ones
+_SWEEP = {}
+
+
+def test_unbounded_sweep(chem, oracle):
+    """chemora_autotune over every fused id: the later ids are timed, or disqualified by the guard (-2: disagrees with
+    id 0, -3: a bounded wait gave up) -- never the pick if so; U untouched; two steps with the pick against the oracle"""
+    n, dx, eps = 40, 0.05, 0.1
+    h = chem.Chemora(n, n, n, 3, 4, chem.SYS_BSSN, dx)
+    h.set_param("eps_diss", eps)
+    u = inputs.bssn_noise(n, n, n)
+    h.set_state(u)
+    assert h.get_param("autotune_fused_ids") == chem.NUM_TILES
+    fused, tile, ms = h.autotune()
+    nt, ids = chem.NUM_TILES, chem.variants(chem.SYS_BSSN, 4)
+    assert fused == 1 and tile in ids and ms[nt + tile] > 0
+    assert all(ms[nt + t] > 0 for t in range(ROUND1_FUSED_IDS))
+    assert all(ms[nt + t] > 0 or ms[nt + t] in (-2.0, -3.0) for t in ids), ms[nt:]
+    assert np.array_equal(h.get_state(), u)
+    for _ in range(2):
+        h.rk4_step(0.25 * dx)
+    st = oracle.rk4(1, oracle.with_ghosts(u, 3), 3, 4, dx, 0.25 * dx, oracle.params(eps_diss=eps), 2)
+    assert_bssn_close(h.get_state(), oracle.interior(st, 3), 2e-11)
+    h.destroy()
+    _SWEEP["ms"] = ms[nt:]
+
+
+@pytest.mark.parametrize("dims", CONFIGS4_GRIDS)
+def test_configs4_grids_with_the_unbounded_sweeps_pick(oracle, dims):
+    configs4_grid_sampled(oracle, dims, NUM_TILES, ())
+
+
+def test_zzz_config3_256_full_field_with_the_unbounded_sweeps_pick(oracle):
+    """bench.py's launch configuration when its sweep picks a new id: the whole 256^3 field after 10 steps against the
+    oracle (whose result tests/test_gpu_zz_round2.py left in memory if it ran in this process).  If the pick is one of
+    ids 0..4 that test has already covered it."""
+    fused, tile, ran = config3_256_full_field(oracle, NUM_TILES, only_if_pick_at_least=ROUND1_FUSED_IDS)
+    if not ran:
+        pytest.skip("the unbounded sweep picks fused id %d at 256^3: covered by test_zz_bssn_config3_256_full_field_10_steps" % tile)
+
+
 # ------------------------------------------- fused tile id 5: the interleaved section layout (DESIGN.md section 6.6)
 @pytest.mark.parametrize("data", ["noise1e-10", "gaussians", "strong"])
 def test_interleaved_layout_rhs_and_bit_identity(chem, oracle, data):
@@ -87,38 +128,9 @@ def test_new_ids_10_steps_every_slot_moves(chem, oracle):
     h.destroy()
 
 
-def test_unbounded_sweep(chem, oracle):
-    """chemora_autotune over every fused id: the later ids are timed, or disqualified by the guard (-2: disagrees with
-    id 0, -3: a bounded wait gave up) -- never the pick if so; U untouched; two steps with the pick against the oracle"""
-    n, dx, eps = 40, 0.05, 0.1
-    h = chem.Chemora(n, n, n, 3, 4, chem.SYS_BSSN, dx)
-    h.set_param("eps_diss", eps)
-    u = inputs.bssn_noise(n, n, n)
-    h.set_state(u)
-    assert h.get_param("autotune_fused_ids") == chem.NUM_TILES
-    fused, tile, ms = h.autotune()
-    nt, ids = chem.NUM_TILES, chem.variants(chem.SYS_BSSN, 4)
-    assert fused == 1 and tile in ids and ms[nt + tile] > 0
-    assert all(ms[nt + t] > 0 for t in range(ROUND1_FUSED_IDS))
-    assert all(ms[nt + t] > 0 or ms[nt + t] in (-2.0, -3.0) for t in ids), ms[nt:]
-    assert np.array_equal(h.get_state(), u)
-    for _ in range(2):
-        h.rk4_step(0.25 * dx)
-    st = oracle.rk4(1, oracle.with_ghosts(u, 3), 3, 4, dx, 0.25 * dx, oracle.params(eps_diss=eps), 2)
-    assert_bssn_close(h.get_state(), oracle.interior(st, 3), 2e-11)
-    assert all(ms[nt + t] > 0 for t in ids), ("a new id was disqualified by the guard", ms[nt:])   # say so, last
-    h.destroy()
-
-
-@pytest.mark.parametrize("dims", CONFIGS4_GRIDS)
-def test_configs4_grids_with_the_unbounded_sweeps_pick(oracle, dims):
-    configs4_grid_sampled(oracle, dims, NUM_TILES, ())
-
-
-def test_zzz_config3_256_full_field_with_the_unbounded_sweeps_pick(oracle):
-    """bench.py's launch configuration when its sweep picks a new id: the whole 256^3 field after 10 steps against the
-    oracle (whose result tests/test_gpu_zz_round2.py left in memory if it ran in this process).  If the pick is one of
-    ids 0..4 that test has already covered it."""
-    fused, tile, ran = config3_256_full_field(oracle, NUM_TILES, only_if_pick_at_least=ROUND1_FUSED_IDS)
-    if not ran:
-        pytest.skip("the unbounded sweep picks fused id %d at 256^3: covered by test_zz_bssn_config3_256_full_field_10_steps" % tile)
+def test_zzzz_no_new_id_was_disqualified_by_the_guard():
+    """last of all: the sweep protects the results from a new id that disagrees with id 0 or whose waits give up, and
+    the tests above pass without it -- but it is a defect of that kernel on hardware, and this is where it is reported"""
+    if "ms" not in _SWEEP:
+        pytest.skip("test_unbounded_sweep did not run")
+    assert all(m > 0 or m == -1.0 for m in _SWEEP["ms"]), ("disqualified: -2 disagrees with id 0, -3 a wait gave up", _SWEEP["ms"])
