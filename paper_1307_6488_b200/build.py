@@ -91,7 +91,57 @@ def report():
         print("| `%s` | %s |" % (r[0], " | ".join(str(x) for x in r[1:])))
 
 
+def _sass_groups(path):
+    """{demangled kernel name: Counter of SASS mnemonics (up to the first '.')} of an object file or library"""
+    import collections
+    import re
+    cuda_bin = os.path.dirname(os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc"))
+    sass = subprocess.run([os.path.join(cuda_bin, "cuobjdump"), "-sass", path], capture_output=True, text=True,
+                          check=True).stdout
+    cur, cnt = None, collections.OrderedDict()
+    for line in sass.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            cur = m.group(1)
+            cnt[cur] = collections.Counter()
+            continue
+        m = re.match(r"\s+/\*[0-9a-f]{4,6}\*/\s+(@!?U?P[0-9T]+ )?([A-Z0-9_]+)", line)
+        if m and cur:
+            cnt[cur][m.group(2)] += 1
+    dem = subprocess.run(["c++filt"], input="\n".join(cnt), capture_output=True, text=True).stdout.split("\n")
+    return {re.sub(r"\(.*", "", d).replace("void chm::", "").replace("chm::", ""): c for d, c in zip(dem, cnt.values())}
+
+
+def compare(old, new):
+    """Static SASS comparison of two builds of the same kernels, e.g. the object of an earlier commit against this
+    tree's (how profiles/r02_sass_vs_round1.md was made): per kernel present in both, the count of each instruction
+    group, `a -> b` where it changed.  Says what a refactoring did to kernels that have run on hardware: which kinds
+    of instruction were added or dropped -- not more than that (no two builds schedule alike)."""
+    a, b = _sass_groups(old), _sass_groups(new)
+    groups = [("DADD", ("DADD",)), ("DMUL", ("DMUL",)), ("DFMA", ("DFMA",)), ("LDS", ("LDS",)), ("STS", ("STS",)),
+              ("LDG", ("LDG",)), ("STG", ("STG",)), ("UTMALDG", ("UTMALDG",)), ("SYNCS", ("SYNCS",)),
+              ("BAR", ("BAR",)), ("ATOMG", ("ATOMG",)), ("CS2R", ("CS2R",))]
+    print("| kernel | " + " | ".join(g for g, _ in groups) + " | all |")
+    print("|---|" + "---|" * (len(groups) + 1))
+    for k in sorted(a):
+        if k not in b:
+            continue
+        cells = []
+        for _, ops in groups + [("all", None)]:
+            x = sum(a[k].values()) if ops is None else sum(a[k][o] for o in ops)
+            y = sum(b[k].values()) if ops is None else sum(b[k][o] for o in ops)
+            cells.append(str(x) if x == y else "%d -> %d" % (x, y))
+        print("| `%s` | %s |" % (k, " | ".join(cells)))
+    print()
+    print("only in %s: %s" % (old, ", ".join("`%s`" % k for k in sorted(a) if k not in b) or "-"))
+    print("only in %s: %s" % (new, ", ".join("`%s`" % k for k in sorted(b) if k not in a) or "-"))
+
+
 if __name__ == "__main__":
+    if "--compare" in sys.argv:        # python -m paper_1307_6488_b200.build --compare OLD.o NEW.o
+        i = sys.argv.index("--compare")
+        compare(sys.argv[i + 1], sys.argv[i + 2])
+        sys.exit(0)
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
     if "--report" in sys.argv:
         report()

@@ -143,3 +143,25 @@ def test_flop_counts_of_the_fused_kernels(binding):
     executed = {4: counts[4] + 5 * 76, 8: counts[8] + 5 * 160}
     assert 3000 < executed[4] < executed[8]
     assert 7900 / 2 < executed[8] < 7900 * 2
+
+
+def test_static_sass_comparison_tool(binding, capsys):
+    """`python -m paper_1307_6488_b200.build --compare OLD.o NEW.o` (how profiles/r02_sass_vs_round1.md was made): an
+    object compared with itself shows no change, its counts are those of real instructions (the check it replaces
+    filtered every instruction line away and compared nothing), and a differing pair shows as `a -> b`"""
+    import shutil
+    from paper_1307_6488_b200 import build
+    if not (shutil.which("cuobjdump") or os.path.exists("/usr/local/cuda/bin/cuobjdump")):
+        pytest.skip("cuobjdump not available")
+    obj = os.path.join(os.path.dirname(binding.LIB_PATH), "build", "kernels_boundary.o")
+    basic = os.path.join(os.path.dirname(binding.LIB_PATH), "build", "kernels_basic.o")
+    if not (os.path.exists(obj) and os.path.exists(basic)):
+        pytest.skip("object files of the in-tree build not present")
+    g = build._sass_groups(obj)
+    assert {"radiative_kernel", "maxdiff_kernel"} <= set(g)
+    assert g["radiative_kernel"]["STG"] > 0 and g["radiative_kernel"]["LDG"] > 0 and sum(g["radiative_kernel"].values()) > 100
+    build.compare(obj, obj)
+    out = capsys.readouterr().out
+    assert "`radiative_kernel`" in out and "->" not in out
+    a = build._sass_groups(basic)
+    assert a["fill_ghosts_kernel"]["UTMALDG"] == 0 and a["enforce_kernel"]["DMUL"] > 0
