@@ -142,87 +142,6 @@ __device__ __forceinline__ void named_barrier(int id) {
 }
 #endif   // CHM_EMULATE
 
-#ifdef CHM_EMULATE   // tensor memory is not emulated: no instantiated tile parks values (TmaCfg::HEAVY is false for all)
-template <int N> inline void tmem_park(uint32_t, int, const double*) { abort(); }
-template <int N> inline void tmem_unpark(uint32_t, int, double*) { abort(); }
-#else
-// ---- tensor memory as a per-thread parking area (tcgen05.st / tcgen05.ld, shape 32x32b: lane i of warp w owns TMEM
-// lane 32*(w%4)+i; a double takes two 32-bit columns).  All 32 lanes of the warp must execute these together.
-// The wait after a load names the loaded registers as in/out operands, so no use of them can be scheduled above it.
-#define CHM_LO(x) "r"(__double2loint(x))
-#define CHM_HI(x) "r"(__double2hiint(x))
-__device__ __forceinline__ void tmem_st8(uint32_t t, const double* x) {   // 8 doubles -> 16 columns
-  asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
-               ::"r"(t), CHM_LO(x[0]), CHM_HI(x[0]), CHM_LO(x[1]), CHM_HI(x[1]), CHM_LO(x[2]), CHM_HI(x[2]), CHM_LO(x[3]),
-                 CHM_HI(x[3]), CHM_LO(x[4]), CHM_HI(x[4]), CHM_LO(x[5]), CHM_HI(x[5]), CHM_LO(x[6]), CHM_HI(x[6]),
-                 CHM_LO(x[7]), CHM_HI(x[7]) : "memory");
-}
-__device__ __forceinline__ void tmem_st4(uint32_t t, const double* x) {   // 4 doubles -> 8 columns
-  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
-               ::"r"(t), CHM_LO(x[0]), CHM_HI(x[0]), CHM_LO(x[1]), CHM_HI(x[1]), CHM_LO(x[2]), CHM_HI(x[2]), CHM_LO(x[3]),
-                 CHM_HI(x[3]) : "memory");
-}
-__device__ __forceinline__ void tmem_st2(uint32_t t, const double* x) {   // 2 doubles -> 4 columns
-  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};"
-               ::"r"(t), CHM_LO(x[0]), CHM_HI(x[0]), CHM_LO(x[1]), CHM_HI(x[1]) : "memory");
-}
-#undef CHM_LO
-#undef CHM_HI
-__device__ __forceinline__ void tmem_ld8(uint32_t t, double* x) {
-  int r[16];
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-                 "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-               : "r"(t) : "memory");
-  asm volatile("tcgen05.wait::ld.sync.aligned;"
-               : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
-                 "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15])
-               :: "memory");
-#pragma unroll
-  for (int i = 0; i < 8; ++i) x[i] = __hiloint2double(r[2 * i + 1], r[2 * i]);
-}
-__device__ __forceinline__ void tmem_ld4(uint32_t t, double* x) {
-  int r[8];
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-               : "r"(t) : "memory");
-  asm volatile("tcgen05.wait::ld.sync.aligned;"
-               : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]) :: "memory");
-#pragma unroll
-  for (int i = 0; i < 4; ++i) x[i] = __hiloint2double(r[2 * i + 1], r[2 * i]);
-}
-__device__ __forceinline__ void tmem_ld2(uint32_t t, double* x) {
-  int r[4];
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(t) : "memory");
-  asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]) :: "memory");
-  x[0] = __hiloint2double(r[1], r[0]);
-  x[1] = __hiloint2double(r[3], r[2]);
-}
-__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-// N doubles (N even) at double offset `first` of the thread's parking area, in chunks of 8 / 4 / 2
-template <int N>
-__device__ __forceinline__ void tmem_park(uint32_t base, int first, const double* x) {
-  static_assert(N % 2 == 0, "park an even number of doubles");
-  int i = 0;
-#pragma unroll
-  for (; i + 8 <= N; i += 8) tmem_st8(base + 2 * (first + i), x + i);
-  if (N - i >= 4) { tmem_st4(base + 2 * (first + i), x + i); i += 4; }
-  if (N - i >= 2) tmem_st2(base + 2 * (first + i), x + i);
-  tmem_wait_st();
-}
-template <int N>
-__device__ __forceinline__ void tmem_unpark(uint32_t base, int first, double* x) {
-  static_assert(N % 2 == 0, "park an even number of doubles");
-  int i = 0;
-#pragma unroll
-  for (; i + 8 <= N; i += 8) tmem_ld8(base + 2 * (first + i), x + i);
-  if (N - i >= 4) { tmem_ld4(base + 2 * (first + i), x + i); i += 4; }
-  if (N - i >= 2) tmem_ld2(base + 2 * (first + i), x + i);
-}
-
-#endif   // CHM_EMULATE
-
 // ---- stencil reads from the staged box -------------------------------------------------------------------------
 // `c` points at this thread's own grid point inside the current slot; BX, BY are the box row / plane extents.
 template <int BX, int BY>

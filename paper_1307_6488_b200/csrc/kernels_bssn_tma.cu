@@ -19,8 +19,8 @@
 
 namespace chm {
 
-// box ring: 5 slots for the 256-point tiles (25 variables % 5 == 0: the slot of a variable is the same in every
-// tile), 4 for the 384-point tiles (shared memory), where slot and parity follow from the load number 25 t + o
+// box ring: 5 slots for the 4th-order tiles (25 variables % 5 == 0: the slot of a variable is the same in every
+// tile), 3 for the 8th-order one (shared memory), where slot and parity follow from the load number 25 t + o
 // point ("centre") values staged per tile: variables 0..13 (chi, gt, K, At) and 17..23 (alpha, beta, B)
 constexpr int kCenVars = 21;
 __device__ __forceinline__ constexpr int cen_index(int v) { return v < 14 ? v : v - 3; }
@@ -85,11 +85,10 @@ struct TmaCfg {
   static constexpr int SLOT = (BX * BY * BZ + 15) / 16 * 16;          // doubles, 128-byte multiple
   static constexpr uint32_t BOX_BYTES = (uint32_t)BX * BY * BZ * 8u;
   static constexpr int THREADS = TX * TY * TZ;
-  static constexpr bool HEAVY = THREADS > 256;    // 12 warps at 168 registers: live values parked in tensor memory
+  static_assert(THREADS <= 256, "one point per thread at 252-255 registers: at most eight warps");
   // ring slots (a 6-slot ring fits the 16x4x4 tile but its run-time slot index costs more than the depth gains:
   // 8.2 ms vs 6.3 ms)
-  static constexpr int NS = DEEP ? 6 : ORDER == 8 ? 3 : HEAVY ? 4 : 5;   // 8th order: 41 KB boxes, three fit
-  static constexpr bool PARK = HEAVY;
+  static constexpr int NS = DEEP ? 6 : ORDER == 8 ? 3 : 5;   // 8th order: 41 KB boxes, three fit
   static constexpr int TILE = (TX + 2) * TY * TZ;                      // doubles in one (TX+2,TY,TZ) tile box
   static constexpr uint32_t TILE_BYTES = (uint32_t)TILE * 8u;
   static constexpr int SLOTX = SLOT + (DEEP ? 2 : 4) * TILE;   // box + RK4 operands (U,S) of up to two emitted variables
@@ -99,7 +98,7 @@ struct TmaCfg {
   static constexpr int DYX = TX + ORDER;             // x-halo = reach of the centred first derivative (order/2) on each side
   static constexpr int DY_N = DYX * TY * TZ, DZ_N = DYX * (TY + ORDER) * TZ;
   // (planes of 128 threads: measured no gain over the one-pass form)
-  static constexpr bool TWOPASS = !HEAVY && (TX * TY == 64 || TX * TY == 32);
+  static constexpr bool TWOPASS = TX * TY == 64 || TX * TY == 32;
   static constexpr int DB = TWOPASS ? (DY_N + DZ_N + 15) / 16 * 16 : 0;
   // IL: per-thread table of parked values: the advection + dissipation results of At_ij (6) and B^i (3), and B^i (3)
   static constexpr int TAB = IL ? 12 * THREADS : 0;
@@ -130,12 +129,8 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
   constexpr int BX = Cfg::BX, BY = Cfg::BY, SLOT = Cfg::SLOT, SLOTX = Cfg::SLOTX, TILE = Cfg::TILE;
   constexpr unsigned NW = Cfg::NWARPS;
   constexpr int kSlots = Cfg::NS;
-  constexpr bool PARK = Cfg::PARK;
-  constexpr bool TMEM = PARK;
   using Sec = std::conditional_t<IL, SecIL, SecPlain>;
   constexpr int NSEC = Sec::N;   // sections per tile: the ring position of section o of tile t is NSEC t + o
-  // parking map (offsets in doubles inside the thread's 84-double area)
-  constexpr int P_CU = 0, P_DG = 18, P_DB = 42, P_LG = 52, P_AT = 58, P_ADG = 64, P_GN = 68, P_DCA = 72, P_AU = 78;
   CHM_DYNAMIC_SMEM(smem_raw);
   double* sm = reinterpret_cast<double*>(smem_raw);   // dynamic smem base: 128-byte aligned (no static smem)
   double* cbuf = sm + Cfg::cen_off(0);                                 // [kCenVars][TILE]
@@ -161,21 +156,9 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
     for (int s = 0; s < kSlots + 1; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NW); }
     fence_mbar_init();
   }
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(empty + kSlots + 1);
-  int* org = reinterpret_cast<int*>((reinterpret_cast<uintptr_t>(tmem_slot + 1) + 15) & ~uintptr_t(15));   // [4][4]
-  uint32_t park = 0;   // this thread's parking area in tensor memory: its lane, 168 columns (84 doubles)
-  if constexpr (TMEM) {
-    if (tid < 32) {   // warp 0 allocates all 512 columns (one CTA per SM)
-      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
-      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    park = *tmem_slot + ((uint32_t)(32 * ((tid >> 5) & 3)) << 16) + (uint32_t)((tid >> 7) * 168);
-  } else {
-    __syncthreads();
-  }
+  uint32_t* after_bars = reinterpret_cast<uint32_t*>(empty + kSlots + 1);   // one word kept free, then the origins
+  int* org = reinterpret_cast<int*>((reinterpret_cast<uintptr_t>(after_bars + 1) + 15) & ~uintptr_t(15));   // [4][4]
+  __syncthreads();
 
   // tile order (see the file header): idx -> (bx, by, bz)
   auto decode = [&](int idx, int& bx, int& by, int& bz) {
@@ -267,20 +250,14 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
 
   int t = 0;
   for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++t) {
-    // 256-point tiles have the registers to keep this tile's and the next tile's origin (measured faster);
-    // 384-point tiles read them from the shared-memory ring where a refill is issued
+    // this tile's and the next tile's origin are kept in registers (measured faster than re-reading the ring)
     int4 own, nxt = make_int4(0, 0, 0, 0);
-    if constexpr (Cfg::HEAVY) {
-      own = *reinterpret_cast<const int4*>(org + 4 * (t & 3));
-      put_origin(t + 1, tile + gridDim.x);
-    } else {
-      int b0, b1, b2;
-      decode(tile, b0, b1, b2);
-      own = make_int4(b0 * TX + goffx, b1 * TY + goff, b2 * TZ + goff, 1);
-      if (tile + (int)gridDim.x < ntiles) {
-        decode(tile + gridDim.x, b0, b1, b2);
-        nxt = make_int4(b0 * TX + goffx, b1 * TY + goff, b2 * TZ + goff, 1);
-      }
+    int b0, b1, b2;
+    decode(tile, b0, b1, b2);
+    own = make_int4(b0 * TX + goffx, b1 * TY + goff, b2 * TZ + goff, 1);
+    if (tile + (int)gridDim.x < ntiles) {
+      decode(tile + gridDim.x, b0, b1, b2);
+      nxt = make_int4(b0 * TX + goffx, b1 * TY + goff, b2 * TZ + goff, 1);
     }
     const int i = own.x - goffx + lx, j = own.y - goff + ly, k = own.z - goff + lz;
     const bool valid = i < L.nx && j < L.ny && k < L.nz;
@@ -317,8 +294,7 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
     };
     auto done = [&](int o) {
       if (leave(slot_of(o))) {   // the refill is load number 25 t + o + kSlots: same slot
-        const int4 a = !Cfg::HEAVY ? (o + kSlots < NSEC ? own : nxt)
-                                   : *reinterpret_cast<const int4*>(org + 4 * ((o + kSlots < NSEC ? t : t + 1) & 3));
+        const int4 a = o + kSlots < NSEC ? own : nxt;
         if (o + kSlots < NSEC) issue(o + kSlots, slot_of(o), a.x, a.y, a.z);
         else if (a.w) issue(o + kSlots - NSEC, slot_of(o), a.x, a.y, a.z);
       }
@@ -326,7 +302,7 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
     // the point values are last read just before section 3 (At)
     auto done_cen = [&]() {
       if (leave(kSlots)) {
-        const int4 a = !Cfg::HEAVY ? nxt : *reinterpret_cast<const int4*>(org + 4 * ((t + 1) & 3));
+        const int4 a = nxt;
         if (a.w) issue_cen(a.x, a.y, a.z);
       }
     };
@@ -524,10 +500,6 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
       if constexpr (IL) park_ad(SecIL::at(i2), i2, w);   // At11, At12, At13
     }
     double divb = (db[0][0] + db[1][1]) + db[2][2];
-    if constexpr (PARK) {   // needed again only by the Gt^i right-hand side (sections 21..23)
-      const double lg[6] = {lapb[0], lapb[1], lapb[2], gdiv[0], gdiv[1], gdiv[2]};
-      tmem_park<6>(park, P_LG, lg);
-    }
 
     // ---- o = 3..8: gt_ij : d_k gt_ij kept for the Christoffels, gtu^{lm} d_l d_m gt_ij folded into R~_ij ---
     double At[6], Rt[6], dg[3][6];
@@ -553,12 +525,7 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
         };
         if constexpr (EARLY) full_var(p, w, Sec::gt(s), 3 + s, d1, d2, ad, em);
         else full_var(p, w, Sec::gt(s), 3 + s, d1, d2, ad, nothing);
-        if constexpr (PARK) {
-          const double d4[4] = {d1[0], d1[1], d1[2], 0.0};
-          tmem_park<4>(park, P_DG + 4 * s, d4);
-        } else {
-          dg[0][s] = d1[0]; dg[1][s] = d1[1]; dg[2][s] = d1[2];
-        }
+        dg[0][s] = d1[0]; dg[1][s] = d1[1]; dg[2][s] = d1[2];
         Rt[s] = -0.5 * sdot(gu, d2);
         if constexpr (!EARLY) em();
         if constexpr (IL) {
@@ -576,17 +543,6 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
     // ---- Christoffels: Cl[k][s(i,j)] = Gamma~_kij, Cu[k][s] = Gamma~^k_ij, Gn[k] = gtu^{ij} Gamma~^k_ij ----
     double Cu[3][6], Gn[3];
     {
-      if constexpr (PARK) {   // make room: d_j beta^i and At_ij rest in tensor memory until the At_ij sections
-        const double t10[10] = {db[0][0], db[0][1], db[0][2], db[1][0], db[1][1], db[1][2], db[2][0], db[2][1], db[2][2], divb};
-        tmem_park<10>(park, P_DB, t10);
-        tmem_park<6>(park, P_AT, At);
-#pragma unroll
-        for (int s = 0; s < 6; ++s) {
-          double d4[4];
-          tmem_unpark<4>(park, P_DG + 4 * s, d4);
-          dg[0][s] = d4[0]; dg[1][s] = d4[1]; dg[2][s] = d4[2];
-        }
-      }
       double Cl[3][6];
 #pragma unroll
       for (int k2 = 0; k2 < 3; ++k2)
@@ -623,11 +579,8 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
             else acc += t1 + (W[j2][0] * Cl[i2][sym(k2, 0)] + W[j2][1] * Cl[i2][sym(k2, 1)] + W[j2][2] * Cl[i2][sym(k2, 2)]);
             Rt[sym(i2, j2)] += acc;
           }
-        if constexpr (PARK) tmem_park<6>(park, P_CU + 6 * k2, Ck);
-        else {
 #pragma unroll
-          for (int s = 0; s < 6; ++s) Cu[k2][s] = Ck[s];
-        }
+        for (int s = 0; s < 6; ++s) Cu[k2][s] = Ck[s];
       }
 #pragma unroll
       for (int i2 = 0; i2 < 3; ++i2)
@@ -640,10 +593,6 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
         }
     }
 
-    if constexpr (PARK) {
-      const double g4[4] = {Gn[0], Gn[1], Gn[2], 0.0};
-      tmem_park<4>(park, P_GN, g4);
-    }
     // A (inert slot, dissipation only): the last section of the plain layout, between Gt1 and Gt2 in the interleaved one
     auto section_A = [&]() {
       auto p = box(Sec::a);
@@ -671,10 +620,6 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
         for (int j2 = i2; j2 < 3; ++j2)
           Rt[sym(i2, j2)] += 0.5 * (g[sym(k2, i2)] * d1[j2] + g[sym(k2, j2)] * d1[i2]);
     }
-    if constexpr (PARK) {
-      const double a4[4] = {adG[0], adG[1], adG[2], 0.0};
-      tmem_park<4>(park, P_ADG, a4);
-    }
 
     // ---- o = 12: chi : R_ij = R~_ij + R^chi_ij --------------------------------------------------------------
     const double ichi = 1.0 / chi;
@@ -687,23 +632,12 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
       if constexpr (EARLY) full_var(p, w, Sec::chi, 9, dchi, d2, ad, em);
       else { full_var(p, w, Sec::chi, 9, dchi, d2, ad, nothing); em(); }
       double cd[6], cc[6];   // D~_i D~_j chi ; d_i chi d_j chi
-      if constexpr (PARK) {   // Gamma~^k_ij one k at a time from tensor memory
-#pragma unroll
-        for (int s = 0; s < 6; ++s) cd[s] = d2[s];
-#pragma unroll
-        for (int k2 = 0; k2 < 3; ++k2) {
-          double Ck[6];
-          tmem_unpark<6>(park, P_CU + 6 * k2, Ck);
-#pragma unroll
-          for (int s = 0; s < 6; ++s) cd[s] -= Ck[s] * dchi[k2];
-        }
-      }
 #pragma unroll
       for (int a = 0; a < 3; ++a)
 #pragma unroll
         for (int b = a; b < 3; ++b) {
           const int s = sym(a, b);
-          if constexpr (!PARK) cd[s] = d2[s] - (Cu[0][s] * dchi[0] + Cu[1][s] * dchi[1] + Cu[2][s] * dchi[2]);
+          cd[s] = d2[s] - (Cu[0][s] * dchi[0] + Cu[1][s] * dchi[1] + Cu[2][s] * dchi[2]);
           cc[s] = dchi[a] * dchi[b];
         }
       const double trcd = sdot(gu, cd), trcc = sdot(gu, cc);
@@ -722,23 +656,12 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
       if constexpr (EARLY) full_var(p, w, Sec::alpha, 10, dal, d2, ad, em);
       else { full_var(p, w, Sec::alpha, 10, dal, d2, ad, nothing); em(); }
       double cd[6], ca[6];   // d_i d_j alpha - Gamma~^k_ij d_k alpha ; d_i chi d_j alpha + d_j chi d_i alpha
-      if constexpr (PARK) {
-#pragma unroll
-        for (int s = 0; s < 6; ++s) cd[s] = d2[s];
-#pragma unroll
-        for (int k2 = 0; k2 < 3; ++k2) {
-          double Ck[6];
-          tmem_unpark<6>(park, P_CU + 6 * k2, Ck);
-#pragma unroll
-          for (int s = 0; s < 6; ++s) cd[s] -= Ck[s] * dal[k2];
-        }
-      }
 #pragma unroll
       for (int a = 0; a < 3; ++a)
 #pragma unroll
         for (int b = a; b < 3; ++b) {
           const int s = sym(a, b);
-          if constexpr (!PARK) cd[s] = d2[s] - (Cu[0][s] * dal[0] + Cu[1][s] * dal[1] + Cu[2][s] * dal[2]);
+          cd[s] = d2[s] - (Cu[0][s] * dal[0] + Cu[1][s] * dal[1] + Cu[2][s] * dal[2]);
           ca[s] = dchi[a] * dal[b] + dchi[b] * dal[a];
         }
       const double trcd = sdot(gu, cd), trca = 0.5 * sdot(gu, ca);   // trca = gtu^{kl} d_k chi d_l alpha
@@ -747,14 +670,9 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
 #pragma unroll
       for (int s = 0; s < 6; ++s) Rt[s] = alpha * Rt[s] - (cd[s] + h2 * (ca[s] - g[s] * trca));   // Rt now holds X_ij
     }
-    if constexpr (PARK) {   // d_i chi, d_i alpha: next used by the Gt^i right-hand side
-      const double dc[6] = {dchi[0], dchi[1], dchi[2], dal[0], dal[1], dal[2]};
-      tmem_park<6>(park, P_DCA, dc);
-    }
 
     // ---- extrinsic curvature with raised indices -------------------------------------------------------------
     double Am[3][3], Au[6];   // At^i_j ; At^{ij}
-    if constexpr (PARK) tmem_unpark<6>(park, P_AT, At);
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2)
 #pragma unroll
@@ -776,18 +694,8 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
       done(Sec::k);
       emit(V_K, (alpha * (sdot(Au, At) + third * trK * trK) - lap_alpha) + ad, pr);
     }
-    if constexpr (PARK) tmem_park<6>(park, P_AU, Au);
 
     // ---- o = 15..20: At_ij -------------------------------------------------------------------------------------
-    if constexpr (PARK) {
-      double t10[10];
-      tmem_unpark<10>(park, P_DB, t10);
-#pragma unroll
-      for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = 0; b < 3; ++b) db[a][b] = t10[3 * a + b];
-      divb = t10[9];
-    }
     if constexpr (IL) {
       // Interleaved layout: the stencil results of At_ij and B^i were parked early; what is left is pointwise.  All
       // twelve right-hand sides are formed here, then leave through the three emit sections (operand tiles only).
@@ -906,19 +814,6 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
     }
 
     // ---- o = 21..23: B^i, together with Gt^i ---------------------------------------------------------------------
-    if constexpr (PARK) {
-      double lg[6], a4[4];
-      tmem_unpark<6>(park, P_LG, lg);
-      tmem_unpark<4>(park, P_ADG, a4);
-#pragma unroll
-      for (int a = 0; a < 3; ++a) { lapb[a] = lg[a]; gdiv[a] = lg[3 + a]; adG[a] = a4[a]; }
-      double g4[4], dc[6];
-      tmem_unpark<4>(park, P_GN, g4);
-      tmem_unpark<6>(park, P_DCA, dc);
-      tmem_unpark<6>(park, P_AU, Au);
-#pragma unroll
-      for (int a = 0; a < 3; ++a) { Gn[a] = g4[a]; dchi[a] = dc[a]; dal[a] = dc[3 + a]; }
-    }
 #pragma unroll
     for (int i2 = 0; i2 < 3; ++i2) {
       auto p = box(SecPlain::b(i2));
@@ -927,7 +822,6 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
       const double adB = ORDER == 4 ? var_ad(p, w) : var_ad8(p, C, w);
       done(SecPlain::b(i2));
       double r = lapb[i2];
-      if constexpr (PARK) tmem_unpark<6>(park, P_CU + 6 * i2, &Cu[i2][0]);
       double t2 = sdot(Cu[i2], Au);   // Gamma~^i_jk At^{jk}
 #pragma unroll
       for (int j2 = 0; j2 < 3; ++j2) {
@@ -942,11 +836,6 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
 
     // ---- o = 24: A (inert slot, dissipation only) -----------------------------------------------------------------
     section_A();
-  }
-  if constexpr (TMEM) {
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(*tmem_slot) : "memory");
   }
 }
 
@@ -992,7 +881,6 @@ static TmaPlan bssn_plan(int mode, int xo) {
   p.kernel = name;
   p.smem_bytes = Cfg::SMEM;
   p.threads = Cfg::THREADS;
-  p.tmem_cols = Cfg::PARK ? 512 : 0;
   p.barrier_off = (size_t)Cfg::bar_off() * 8;
   p.n_barriers = 2 * (Cfg::NS + 1);
   const int nops = mode == MODE_RHS ? 0 : (mode == MODE_FIRST ? 1 : 2);

@@ -29,7 +29,6 @@ struct TmaPlan {
   int n_barriers = 0;
   size_t smem_bytes = 0;          // dynamic shared memory of the launch
   int threads = 0;
-  int tmem_cols = 0;              // tensor-memory columns the CTA allocates (0: none)
 };
 
 constexpr size_t kSmemOptIn = 232448;   // 227 KB: the per-block opt-in limit of sm_100
@@ -41,8 +40,6 @@ inline std::string check_tma_plan(const TmaPlan& p, size_t smem_limit = kSmemOpt
   if (p.smem_bytes > smem_limit)
     return k + to_string(p.smem_bytes) + " bytes of dynamic shared memory > limit " + to_string(smem_limit);
   if (p.threads < 32 || p.threads > 1024 || p.threads % 32) return k + "bad thread count " + to_string(p.threads);
-  if (p.tmem_cols != 0 && (p.tmem_cols < 32 || p.tmem_cols > 512 || (p.tmem_cols & (p.tmem_cols - 1))))
-    return k + "tensor-memory allocation of " + to_string(p.tmem_cols) + " columns (power of two in 32..512)";
   if (p.barrier_off % 8) return k + "mbarrier offset " + to_string(p.barrier_off) + " not 8-byte aligned";
   if (p.barrier_off + 8 * (size_t)p.n_barriers > p.smem_bytes)
     return k + "mbarriers end beyond the " + to_string(p.smem_bytes) + " bytes of shared memory";

@@ -15,8 +15,7 @@
 //                                               produce; a protocol that is wrong for EVERY timing (slot, parity,
 //                                               byte count, missing refill) shows up as wrong data or a timed-out wait
 //   atomicCAS, clock64, __dadd_rn & co, __stcs  plain host equivalents
-// Not emulated: tensor memory (tcgen05; no instantiated tile uses it), timing, memory-model subtleties below the
-// granularity of these barriers.
+// Not emulated: timing, memory-model subtleties below the granularity of these barriers.
 #pragma once
 #include <algorithm>
 #include <atomic>

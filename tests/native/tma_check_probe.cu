@@ -32,7 +32,6 @@ int main() {
   p = good(); p.loads[1].smem_off = 32 * 1024 - 128; show("box_overruns_barriers", p);
   p = good(); p.barrier_off += 4; show("misaligned_barrier", p);
   p = good(); p.threads = 250; show("bad_thread_count", p);
-  p = good(); p.tmem_cols = 168; show("bad_tmem_columns", p);
   p = good(); p.loads[1].barrier = 7; show("barrier_index", p);
   Layout L{};
   L.pitch = 272; L.tot_y = 262; L.tot_z = 262; L.nvars = 25; L.vstride = 272L * 262 * 262;

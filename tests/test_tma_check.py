@@ -19,4 +19,4 @@ def test_every_rule_rejects_its_violation(tmp_path):
     out = subprocess.run([exe], check=True, capture_output=True, text=True).stdout.split()
     got = dict(zip(out[0::2], map(int, out[1::2])))
     assert got.pop("good") == 0 and got.pop("layout_good") == 0
-    assert len(got) == 14 and all(v == 1 for v in got.values()), got
+    assert len(got) == 13 and all(v == 1 for v in got.values()), got
