@@ -336,11 +336,11 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
       Dy[(lz * TY + ly) * DYX + lx + HM] = d1[1];
       Dz[(lz * (TY + 2 * HM) + ly + HM) * DYX + lx + HM] = d1[2];
       const double* sb = p.c - coff;   // slot base
-      if constexpr (TX * TY == 64 || TX * TY == 128) {
-        // One z-plane of the tile = PLANE threads = two or four warps, and every first derivative a thread reads
+      if constexpr (TX * TY == 64) {
+        // One z-plane of the tile = PLANE threads = two warps, and every first derivative a thread reads
         // below comes from its own plane: the plane's warps fill the plane's halo entries and meet at a
         // PLANE-thread named barrier instead of a block barrier.
-        constexpr int PLANE = TX * TY, WPP = PLANE / 32;
+        constexpr int PLANE = TX * TY;
         const int u0 = tid % PLANE;
         for (int u = u0; u < TX * 2 * HM; u += PLANE) {                       // D_z f on the y-halo rows -2,-1,TY,TY+1
           const int hx = u % TX, hyi = u / TX;
@@ -350,7 +350,7 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
         }
         // D_y f, D_z f on the 4 x-halo columns: 8 * TY evaluations per plane, started at a warp of the plane
         // chosen so that every scheduler (warp w runs on scheduler w % 4) gets the same share
-        const int start = WPP == 2 ? (((lz + 1) >> 1) & 1) : (2 * lz) % WPP;
+        const int start = ((lz + 1) >> 1) & 1;
         for (int l = (u0 - 32 * start + PLANE) % PLANE; l < 4 * HM * TY; l += PLANE) {
           const int kind = l / (2 * HM * TY), hh = l % (2 * HM * TY);
           const int hxi = hh % (2 * HM), hy = hh / (2 * HM);
@@ -387,27 +387,7 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
         early();
         __syncwarp();
       } else {
-      for (int h = tid; h < TX * 2 * HM * TZ; h += Cfg::THREADS) {          // D_z f on the y-halo rows -2,-1,TY,TY+1
-        const int hx = h % TX, hyi = (h / TX) % (2 * HM), hz = h / (TX * 2 * HM);
-        const int yy = hyi < HM ? hyi - HM : TY + hyi - HM;
-        const double* c = sb + ((hz + H) * BY + (yy + H)) * BX + hx + H;
-        Dz[(hz * (TY + 2 * HM) + yy + HM) * DYX + hx + HM] = D1(c, ZS);
-      }
-      // D_y f and D_z f on the 4 x-halo columns: 2 * 4 * TY * TZ single evaluations, spread over the first
-      // warps so that every scheduler (warp w runs on scheduler w % 4) gets the same share
-      for (int h = tid; h < 4 * HM * TY * TZ; h += Cfg::THREADS) {
-        const int kind = h / (2 * HM * TY * TZ), hh = h - kind * (2 * HM * TY * TZ);
-        const int hxi = hh % (2 * HM), hy = (hh / (2 * HM)) % TY, hz = hh / (2 * HM * TY);
-        const int xx = hxi < HM ? hxi - HM : TX + hxi - HM;
-        const double* c = sb + ((hz + H) * BY + (hy + H)) * BX + xx + H;
-        const int st1 = kind == 0 ? BX : ZS;
-        const double v = D1(c, st1);
-        if (kind == 0) Dy[(hz * TY + hy) * DYX + xx + HM] = v;
-        else Dz[(hz * (TY + 2 * HM) + hy + HM) * DYX + xx + HM] = v;
-      }
-      done(o);
-      early();
-      __syncthreads();
+        static_assert(TX * TY == 64 || TX * TY == 32, "two-pass mixed derivatives: a z-plane of one or two warps");
       }
       const double* y = Dy + (lz * TY + ly) * DYX + lx + HM;
       const double* z = Dz + (lz * (TY + 2 * HM) + ly + HM) * DYX + lx + HM;
