@@ -37,7 +37,6 @@ inline void tma_load_4d(void* dst, const CUtensorMap* tm, uint64_t* bar, int x, 
   chm_emu::tma_load_4d(dst, tm, bar, x, y, z, v);
 }
 inline uint64_t l2_policy_evict_first() { return 0; }
-inline uint64_t l2_policy_normal() { return 0; }
 inline void tma_load_4d_hint(void* dst, const CUtensorMap* tm, uint64_t* bar, int x, int y, int z, int v, uint64_t) {
   chm_emu::tma_load_4d(dst, tm, bar, x, y, z, v);
 }
@@ -95,11 +94,6 @@ __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, ui
 __device__ __forceinline__ uint64_t l2_policy_evict_first() {
   uint64_t p;
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-  return p;
-}
-__device__ __forceinline__ uint64_t l2_policy_normal() {
-  uint64_t p;
-  asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
   return p;
 }
 __device__ __forceinline__ void tma_load_4d_hint(void* dst, const CUtensorMap* tm, uint64_t* bar, int x, int y, int z,

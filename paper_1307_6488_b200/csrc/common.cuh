@@ -4,9 +4,6 @@
 #ifndef CHM_EMULATE   // tests/native/cta_emu.hpp stands in for the CUDA headers when the kernel source is compiled for the host
 #include <cuda_runtime.h>
 #endif
-#ifndef CHM_STCS
-#define CHM_STCS 1
-#endif
 #include <stdint.h>
 
 // inline helper usable from device code and from host-side probes of the same arithmetic (tests/native/)
@@ -14,11 +11,7 @@
 
 namespace chm {
 
-#if CHM_STCS
 #define CHM_ST(p, v) __stcs(p, v)   // streaming store: written once, re-read only by a later launch
-#else
-#define CHM_ST(p, v) (*(p) = (v))
-#endif
 // Device-side view of the padded SoA layout (include/chemora.h "Conventions").
 struct Layout {
   int nx, ny, nz, g;     // interior dims, ghost width

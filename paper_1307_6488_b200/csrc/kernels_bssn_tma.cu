@@ -13,10 +13,6 @@
 #include "bssn_tma.cuh"
 #include "tma_check.cuh"
 
-#ifndef CHM_L2HINT
-#define CHM_L2HINT 1
-#endif
-
 namespace chm {
 
 // box ring: 5 slots for the 4th-order tiles (25 variables % 5 == 0: the slot of a variable is the same in every
@@ -149,7 +145,7 @@ __device__ __forceinline__ void bssn_tma_body(const CUtensorMap& tm, const CUten
   // on a 16-byte boundary: the layout makes L.xo - 3 even, and the (TX,TY,TZ) tile boxes (point values, RK4
   // operands) are loaded two columns wider, from x0 + 2, and read at column + 1.
   const int goffx = L.xo - H, goff = L.g - H;
-  const uint64_t pol_stream = CHM_L2HINT ? l2_policy_evict_first() : l2_policy_normal();   // U, S: read once per launch
+  const uint64_t pol_stream = l2_policy_evict_first();   // U, S: read once per launch
 
   if (tid == 0) {
 #pragma unroll

@@ -274,16 +274,14 @@ static cudaError_t wv_tile(int which, const Layout& L, const Coef& C, const Stag
 // Sample-1 system (five variables): which: 0 = 16x8 threads, 1 = 16x16 (at 8th order with one plane of prefetch),
 // 2 = 32x8 (fits at 4th order only); 64-plane chunks
 // 64-plane chunks: measured 0.886 ms per launch at 256^3, 8th order (32: 0.914, 128: 1.006)
-#ifndef CHM_W1ZC
-#define CHM_W1ZC 64
-#endif
+constexpr int kW1ZC = 64;
 template <int ORDER, bool KO>
 static cudaError_t wv1_tile(int which, const Layout& L, const Coef& C, const Stage* st, cudaStream_t s,
                             cudaFuncAttributes* a) {
   switch (which) {
-    case 0: return wv_go<ORDER, KO, 16, 8, CHM_W1ZC, 5>(L, C, st, s, a);
-    case 1: return wv_go<ORDER, KO, 16, 16, CHM_W1ZC, 5>(L, C, st, s, a);
-    case 2: return wv_go<ORDER, KO, 32, 8, CHM_W1ZC, 5>(L, C, st, s, a);
+    case 0: return wv_go<ORDER, KO, 16, 8, kW1ZC, 5>(L, C, st, s, a);
+    case 1: return wv_go<ORDER, KO, 16, 16, kW1ZC, 5>(L, C, st, s, a);
+    case 2: return wv_go<ORDER, KO, 32, 8, kW1ZC, 5>(L, C, st, s, a);
   }
   return cudaErrorInvalidValue;
 }
