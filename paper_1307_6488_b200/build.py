@@ -92,22 +92,28 @@ def report():
 
 
 def _sass_groups(path):
-    """{demangled kernel name: Counter of SASS mnemonics (up to the first '.')} of an object file or library"""
+    """{demangled kernel name: Counter of SASS mnemonics (up to the first '.')} of an object file or library; the
+    key "" of a Counter holds a hash of the kernel's whole instruction text (operands included; instruction addresses
+    and encodings left out)"""
     import collections
+    import hashlib
     import re
     cuda_bin = os.path.dirname(os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc"))
     sass = subprocess.run([os.path.join(cuda_bin, "cuobjdump"), "-sass", path], capture_output=True, text=True,
                           check=True).stdout
-    cur, cnt = None, collections.OrderedDict()
+    cur, cnt, text = None, collections.OrderedDict(), {}
     for line in sass.splitlines():
         m = re.search(r"Function : (\S+)", line)
         if m:
             cur = m.group(1)
-            cnt[cur] = collections.Counter()
+            cnt[cur], text[cur] = collections.Counter(), hashlib.md5()
             continue
-        m = re.match(r"\s+/\*[0-9a-f]{4,6}\*/\s+(@!?U?P[0-9T]+ )?([A-Z0-9_]+)", line)
+        m = re.match(r"\s+/\*[0-9a-f]{4,6}\*/\s+((@!?U?P[0-9T]+ )?([A-Z0-9_]+).*?)\s*/\* 0x[0-9a-f]+ \*/", line)
         if m and cur:
-            cnt[cur][m.group(2)] += 1
+            cnt[cur][m.group(3)] += 1
+            text[cur].update(m.group(1).encode() + b"\n")
+    for k in cnt:
+        cnt[k][""] = int(text[k].hexdigest(), 16)
     dem = subprocess.run(["c++filt"], input="\n".join(cnt), capture_output=True, text=True).stdout.split("\n")
     return {re.sub(r"\(.*", "", d).replace("void chm::", "").replace("chm::", ""): c for d, c in zip(dem, cnt.values())}
 
@@ -121,16 +127,17 @@ def compare(old, new):
     groups = [("DADD", ("DADD",)), ("DMUL", ("DMUL",)), ("DFMA", ("DFMA",)), ("LDS", ("LDS",)), ("STS", ("STS",)),
               ("LDG", ("LDG",)), ("STG", ("STG",)), ("UTMALDG", ("UTMALDG",)), ("SYNCS", ("SYNCS",)),
               ("BAR", ("BAR",)), ("ATOMG", ("ATOMG",)), ("CS2R", ("CS2R",))]
-    print("| kernel | " + " | ".join(g for g, _ in groups) + " | all |")
-    print("|---|" + "---|" * (len(groups) + 1))
+    print("| kernel | " + " | ".join(g for g, _ in groups) + " | all | instruction text |")
+    print("|---|" + "---|" * (len(groups) + 2))
     for k in sorted(a):
         if k not in b:
             continue
         cells = []
         for _, ops in groups + [("all", None)]:
-            x = sum(a[k].values()) if ops is None else sum(a[k][o] for o in ops)
-            y = sum(b[k].values()) if ops is None else sum(b[k][o] for o in ops)
+            x = sum(v for o, v in a[k].items() if o) if ops is None else sum(a[k][o] for o in ops)
+            y = sum(v for o, v in b[k].items() if o) if ops is None else sum(b[k][o] for o in ops)
             cells.append(str(x) if x == y else "%d -> %d" % (x, y))
+        cells.append("same" if a[k][""] == b[k][""] else "differs")
         print("| `%s` | %s |" % (k, " | ".join(cells)))
     print()
     print("only in %s: %s" % (old, ", ".join("`%s`" % k for k in sorted(a) if k not in b) or "-"))
