@@ -211,17 +211,19 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     n = args.size
+    sweep_error, pick = None, None
+    isolated = args.variant == "auto" and not args.sweep_in_process
+    if isolated:      # before this process touches the device: the child has the GPU (and its memory) to itself
+        pick, sweep_error = isolated_sweep(n)
+        if pick is None:                      # once more over the tiles that have run on hardware before
+            pick, again = isolated_sweep(n, ROUND1_FUSED_IDS)
+            sweep_error += "; sweep bounded to fused ids 0..%d: %s" % (ROUND1_FUSED_IDS - 1, again or "done")
     c, u0, h = headline_handle(binding, inputs, replicas, n, rank, local)
     g, dx = c["ghost"], c["dx"]
     dt = 0.25 * dx
     host = torch.from_numpy(u0).pin_memory()
     h.set_state(host.numpy())
-    sweep_error = None
-    if args.variant == "auto" and not args.sweep_in_process:
-        pick, sweep_error = isolated_sweep(n)
-        if pick is None:                      # once more over the tiles that have run on hardware before
-            pick, again = isolated_sweep(n, ROUND1_FUSED_IDS)
-            sweep_error += "; sweep bounded to fused ids 0..%d: %s" % (ROUND1_FUSED_IDS - 1, again or "done")
+    if isolated:
         fused, tile, rows, sweep_ms = pick if pick else (1, 0, None, None)   # failed sweeps: the default tile, said so
         h.set_variant(fused, tile)
         if rows:
